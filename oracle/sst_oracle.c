@@ -159,8 +159,8 @@ int32_t sst_oracle_gain_correct(uint8_t adc, float gain)
 {
     volatile float t = (float)adc / gain;   /* volatile: no excess precision, no contraction */
     volatile float u = t + 0.5f;
-    int32_t q = (int32_t)floorf(u);
-    return q < 254 ? q : 254;
+    float fl = floorf(u);
+    return fl >= 254.0f ? 254 : (int32_t)fl;   /* min taken before the int conversion */
 }
 
 /* ---------------------------------------------------------------------------------------

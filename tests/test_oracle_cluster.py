@@ -353,3 +353,12 @@ def test_capacity_overflow_semantics(oracle):
     k = int(np.searchsorted(np.cumsum(full.cl_width), 50, side="right"))
     assert r.n_clusters == k and r.status[0] & oracle.FLAG_ADC_CAP
     assert as_list(r) == as_list(full)[:k]
+
+
+def test_module_never_crosses_a_fed(oracle):
+    """Reading s10: nothing is adjacent across a FED boundary, even if a (malformed) module map
+    repeats the module id on both sides."""
+    cs = cases.build_case({"95:255": 40, "96:0": 40}, n_feds=2, module_sizes=(2,))
+    cs.chan_module[96:98] = cs.chan_module[95]
+    r = run_case(oracle, cs)
+    assert [(f, w) for _, f, w, _, _ in as_list(r)] == [(511, 1), (0, 1)]
