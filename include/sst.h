@@ -1,0 +1,169 @@
+/*
+ * sst.h -- C ABI of libsst: B200-native unpacking + "three thresholds" clustering of
+ * zero-suppressed silicon-strip FED data (arXiv 2101.11489).
+ *
+ * Problem statement: PAPER.md:25 (section 2: FED = 96 optical channels x 256 strips, CSR-like
+ * zero-suppressed payload, per-strip calibration "e.g. gain and noise"), PAPER.md:31 (channel
+ * location map, unpack to a structure of arrays), PAPER.md:33 (active strips, seed strips,
+ * seed-index array, left/right boundaries, cluster charge vs cluster threshold; outputs: left
+ * and right boundary, centroid, ADC values), PAPER.md:41 (several events in flight on CUDA
+ * streams, pooled device memory).  Byte format, >= comparisons, gain formula, leftmost-seed
+ * ownership and output order: BASELINE.json north_star / config 0 (DESIGN.md section 3 lists
+ * every reading).
+ *
+ * Conventions
+ *   - Plain C, no CUDA or torch types.  `stream` arguments are a cudaStream_t passed as void*.
+ *   - "HOST" / "DEVICE" on every pointer says where the memory lives.  The caller owns every
+ *     buffer it passes and keeps it alive until the work enqueued on `stream` has completed.
+ *   - Global strip id g = (fed*96 + channel)*256 + strip.  N = n_feds*96*256.
+ *   - Every call returns an sst_status.  Host-detectable errors enqueue nothing.  Problems only
+ *     the device can see (malformed raw data, output capacity) are reported in
+ *     sst_output.dev_status once the stream has completed.
+ *   - After sst_upload_calib returns the context is read-only: sst_unpack_cluster may be called
+ *     concurrently from several host threads on different streams.
+ */
+#ifndef SST_H
+#define SST_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SST_CHANNELS_PER_FED 96u
+#define SST_STRIPS_PER_CHANNEL 256u
+#define SST_STRIPS_PER_FED (96u * 256u)
+
+typedef struct sst_ctx sst_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    SST_OK = 0,
+    SST_ERR_INVALID_ARG = 1, /* NULL pointer, n_feds == 0, threshold not finite or <= 0, ... */
+    SST_ERR_CUDA = 2,        /* a CUDA call failed; sst_last_cuda_error() returns its code   */
+    SST_ERR_NO_CALIB = 3,    /* sst_unpack_cluster before sst_upload_calib                   */
+    SST_ERR_BAD_CALIB = 4    /* gain/noise not finite or <= 0 at a non-bad strip; module map
+                                decreasing, or a module crossing a FED boundary             */
+} sst_status;
+
+typedef struct {
+    uint32_t n_feds;               /* FEDs per event (fixed for the context)                    */
+    int32_t device;                /* CUDA device ordinal                                       */
+    uint32_t max_raw_bytes;        /* every `raw` buffer holds at least this many readable bytes;
+                                      a FED whose end offset exceeds it is flagged and empty    */
+    uint32_t max_events_in_flight; /* hint for the pool (0 = default 8)                         */
+} sst_config;
+
+/* S/N thresholds of the "three thresholds" algorithm: a strip is active at
+ * adc/noise >= channel, a seed at adc/noise >= seed (both decided in exact arithmetic), a
+ * cluster is accepted at charge/sqrt(sum noise^2) >= cluster. */
+typedef struct { float channel, seed, cluster; } sst_thresholds;
+
+/* dev_status words */
+enum {
+    SST_ST_FLAGS = 0,        /* SST_FLAG_* bits                                           */
+    SST_ST_N_MALFORMED = 1,  /* channels whose run list is malformed (they contribute no strips) */
+    SST_ST_N_CLUSTERS = 2,   /* clusters found (may exceed cap_clusters)                  */
+    SST_ST_N_ADC = 3,        /* cluster ADC bytes found (may exceed cap_adc)              */
+    SST_ST_N_OVERRUN = 4,    /* FEDs with bad offsets or a channel-length chain passing the FED end */
+    SST_ST_N_SEEDS = 5,      /* seed strips found                                         */
+    SST_ST_WORDS = 8
+};
+#define SST_FLAG_CLUSTER_CAP 1u /* more clusters than cap_clusters */
+#define SST_FLAG_ADC_CAP 2u     /* more cluster ADC bytes than cap_adc */
+#define SST_FLAG_MALFORMED 4u   /* >= 1 malformed channel */
+#define SST_FLAG_OVERRUN 8u     /* >= 1 flagged FED */
+
+/*
+ * Output of one event.  All pointers are DEVICE pointers owned by the caller (HOST pointers
+ * for sst_unpack_cluster_host).  Optional members may be NULL.
+ *
+ * Clusters are written in ascending global strip order of their first strip, i.e. ordered by
+ * (module, first strip); cluster k has its gain-corrected ADCs at cl_adc[cl_adc_off[k] ..
+ * + cl_width[k]) and cl_adc_off is the exclusive prefix sum of cl_width.
+ * Capacity: cluster k is written iff k < cap_clusters and cl_adc_off[k]+cl_width[k] <= cap_adc;
+ * the clusters written are always a prefix, *n_clusters is their number and nothing is written
+ * beyond either capacity.  cap_clusters >= raw_bytes/3 and cap_adc >= raw_bytes never overflow.
+ */
+typedef struct {
+    uint8_t *strip_adc;   /* [N] dense unpacked ADC, absent strip = 0; NULL = do not materialise;
+                             should be 16-byte aligned (else a slower store path is used)      */
+    uint32_t *chan_off;   /* [n_feds*96] optional: byte offset in raw of the channel's first run */
+    uint16_t *chan_len;   /* [n_feds*96] optional: payload length L of the channel               */
+    uint32_t *seed_idx;   /* [cap_seeds] optional: ascending global ids of the seed strips       */
+    uint32_t cap_seeds;
+    uint32_t cap_clusters, cap_adc;
+    uint32_t *n_clusters; /* [1] clusters written                                                */
+    uint32_t *cl_module;  /* [cap_clusters] module id (as given in chan_module)                  */
+    uint16_t *cl_first;   /* [cap_clusters] first strip, module-local (left boundary)           */
+    uint16_t *cl_width;   /* [cap_clusters] strips in the cluster (right boundary = first+width-1) */
+    int32_t *cl_charge;   /* [cap_clusters] sum of the gain-corrected ADCs                       */
+    float *cl_bary;       /* [cap_clusters] barycenter, module-local strip units                 */
+    uint32_t *cl_adc_off; /* [cap_clusters] offset of the cluster's ADCs in cl_adc               */
+    float *cl_snr;        /* [cap_clusters] optional: charge / sqrt(sum noise^2)                 */
+    uint8_t *cl_adc;      /* [cap_adc] gain-corrected ADCs min(254, floor(adc/gain + 0.5))       */
+    uint32_t *dev_status; /* [SST_ST_WORDS], see above; fully written by every call              */
+} sst_output;
+
+/* Creates a context on cfg->device: stream-ordered memory pool, calibration storage.
+ * *out_ctx is NULL on failure. */
+sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx);
+
+/* Calibration upload, once.  HOST arrays: gain[N], noise[N] float32, bad[N]
+ * (non-zero = bad strip, never active), chan_module[n_feds*96] = module id of every channel,
+ * non-decreasing, equal ids = same module, a module never crosses a FED.  The arrays are
+ * validated, copied to the device in an internal layout and may be freed on return (the call
+ * synchronises).  Must not run concurrently with sst_unpack_cluster on the same context. */
+sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise, const uint8_t *bad,
+                            const uint32_t *chan_module);
+
+/* One event: channel-location map, unpack, active/seed flags, seed expansion with
+ * leftmost-seed ownership, gain correction, cluster threshold, ordered output
+ * (PAPER.md:31,33).  raw: DEVICE, 16-byte aligned, >= cfg.max_raw_bytes readable bytes;
+ * fed_offsets: DEVICE [n_feds+1] byte offsets of the FEDs in raw (16-byte multiples for the
+ * fast path).  thr and out are HOST structs read before the call returns.  The work is
+ * enqueued on `stream`; the call does not synchronise.  Scratch comes from the context's
+ * stream-ordered pool. */
+sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
+                              const sst_thresholds *thr, const sst_output *out, void *stream);
+
+/* The same event with HOST buffers: raw[raw_bytes] and fed_offsets[n_feds+1] are copied to
+ * pooled device buffers on `stream`, the event is processed, and dev_status, n_clusters and the
+ * cluster arrays (exactly n_clusters / n_adc elements; strip_adc, chan_off, chan_len, seed_idx
+ * too when non-NULL) are copied back into the HOST arrays of `out`.  The call returns after
+ * the stream has completed.  Pinned host memory makes the copies asynchronous to other streams. */
+sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes,
+                                   const uint32_t *fed_offsets, const sst_thresholds *thr,
+                                   const sst_output *out, void *stream);
+
+/* Stream-ordered allocation of per-event buffers from the context's pool (cudaMallocAsync;
+ * replaces the caching allocator of PAPER.md:41).  The pointer is usable by work enqueued on
+ * `stream` after the call; free it with sst_event_free on a stream that has seen all its uses. */
+sst_status sst_event_alloc(sst_ctx *ctx, uint64_t bytes, void *stream, void **out_ptr);
+sst_status sst_event_free(sst_ctx *ctx, void *ptr, void *stream);
+
+/* Stages one event: allocates pooled DEVICE buffers of cfg.max_raw_bytes and (n_feds+1)*4 bytes
+ * on `stream` and enqueues the host-to-device copies of raw[raw_bytes] and fed_offsets[n_feds+1]
+ * (HOST; pinned memory lets the copy overlap kernels of other streams).  Returns
+ * the device pointers for sst_unpack_cluster on the same stream; release both with
+ * sst_event_free.  Does not synchronise: the host arrays must stay valid until the copies ran. */
+sst_status sst_event_upload(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes,
+                            const uint32_t *fed_offsets, void *stream, uint8_t **d_raw,
+                            uint32_t **d_fed_offsets);
+
+/* Synchronises the device and frees everything the context owns. */
+sst_status sst_destroy(sst_ctx *ctx);
+
+/* The cudaError_t of the last failed CUDA call on this context (0 if none). */
+int32_t sst_last_cuda_error(const sst_ctx *ctx);
+const char *sst_status_string(sst_status s);
+
+/* Static facts about the compiled kernels, for benchmarks: bytes of dynamic shared memory per
+ * CTA, threads per CTA, resident CTAs per SM as reported by the occupancy API, SM count. */
+typedef struct { uint32_t smem_bytes, threads, ctas_per_sm, sm_count, kernels_per_event; } sst_info;
+sst_status sst_get_info(const sst_ctx *ctx, sst_info *info);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SST_H */

@@ -1,0 +1,178 @@
+"""Thin Python binding of libsst (include/sst.h): same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/sst.cu.  There is NO CPU fallback: if
+csrc/libsst.so is missing or cannot be loaded, ``load()`` raises.  torch is used for device
+memory and streams only (``tensor.data_ptr()``, ``torch.cuda.Stream.cuda_stream``).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "csrc", "libsst.so")
+
+N_CHAN, N_STRIP, FED_STRIPS = 96, 256, 96 * 256
+ST_WORDS = 8
+ST_FLAGS, ST_N_MALFORMED, ST_N_CLUSTERS, ST_N_ADC, ST_N_OVERRUN, ST_N_SEEDS = range(6)
+FLAG_CLUSTER_CAP, FLAG_ADC_CAP, FLAG_MALFORMED, FLAG_OVERRUN = 1, 2, 4, 8
+SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB = range(5)
+
+EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_cluster_host",
+           "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_destroy", "sst_last_cuda_error",
+           "sst_status_string", "sst_get_info"]
+
+
+class sst_config(C.Structure):
+    _fields_ = [("n_feds", C.c_uint32), ("device", C.c_int32), ("max_raw_bytes", C.c_uint32),
+                ("max_events_in_flight", C.c_uint32)]
+
+
+class sst_thresholds(C.Structure):
+    _fields_ = [("channel", C.c_float), ("seed", C.c_float), ("cluster", C.c_float)]
+
+
+class sst_output(C.Structure):
+    _fields_ = [("strip_adc", C.c_void_p), ("chan_off", C.c_void_p), ("chan_len", C.c_void_p),
+                ("seed_idx", C.c_void_p), ("cap_seeds", C.c_uint32), ("cap_clusters", C.c_uint32),
+                ("cap_adc", C.c_uint32), ("n_clusters", C.c_void_p), ("cl_module", C.c_void_p),
+                ("cl_first", C.c_void_p), ("cl_width", C.c_void_p), ("cl_charge", C.c_void_p),
+                ("cl_bary", C.c_void_p), ("cl_adc_off", C.c_void_p), ("cl_snr", C.c_void_p),
+                ("cl_adc", C.c_void_p), ("dev_status", C.c_void_p)]
+
+
+class sst_info(C.Structure):
+    _fields_ = [("smem_bytes", C.c_uint32), ("threads", C.c_uint32), ("ctas_per_sm", C.c_uint32),
+                ("sm_count", C.c_uint32), ("kernels_per_event", C.c_uint32)]
+
+
+class SSTError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load():
+    """dlopen csrc/libsst.so and declare the C ABI.  Raises if the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise SSTError(f"{LIB_PATH} is not built; run `python -m paper_2101_11489_b200.build` "
+                       "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp = C.c_void_p
+    L.sst_create.argtypes = [C.POINTER(sst_config), C.POINTER(vp)]
+    L.sst_upload_calib.argtypes = [vp, vp, vp, vp, vp]
+    L.sst_unpack_cluster.argtypes = [vp, vp, vp, C.POINTER(sst_thresholds), C.POINTER(sst_output), vp]
+    L.sst_unpack_cluster_host.argtypes = [vp, vp, C.c_uint32, vp, C.POINTER(sst_thresholds),
+                                          C.POINTER(sst_output), vp]
+    L.sst_event_alloc.argtypes = [vp, C.c_uint64, vp, C.POINTER(vp)]
+    L.sst_event_free.argtypes = [vp, vp, vp]
+    L.sst_event_upload.argtypes = [vp, vp, C.c_uint32, vp, vp, C.POINTER(vp), C.POINTER(vp)]
+    L.sst_destroy.argtypes = [vp]
+    L.sst_last_cuda_error.argtypes = [vp]
+    L.sst_last_cuda_error.restype = C.c_int32
+    L.sst_status_string.argtypes = [C.c_int]
+    L.sst_status_string.restype = C.c_char_p
+    L.sst_get_info.argtypes = [vp, C.POINTER(sst_info)]
+    for name in EXPORTS:
+        if name not in ("sst_last_cuda_error", "sst_status_string"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(ctx, rc: int, what: str):
+    if rc != SST_OK:
+        L = load()
+        msg = L.sst_status_string(rc).decode()
+        cu = L.sst_last_cuda_error(ctx) if ctx else 0
+        raise SSTError(f"{what}: {msg}" + (f" (cudaError {cu})" if rc == SST_ERR_CUDA else ""))
+
+
+def _ptr(t) -> Optional[int]:
+    """Device (or pinned host) pointer of a torch tensor / numpy array / int / None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def sst_create(n_feds: int, device: int = 0, max_raw_bytes: int = 1 << 22, max_events_in_flight: int = 8):
+    L = load()
+    cfg = sst_config(n_feds, device, max_raw_bytes, max_events_in_flight)
+    ctx = C.c_void_p()
+    _check(None, L.sst_create(C.byref(cfg), C.byref(ctx)), "sst_create")
+    return ctx
+
+
+def sst_upload_calib(ctx, gain, noise, bad, chan_module):
+    """HOST numpy arrays: gain/noise float32 [N], bad uint8 [N], chan_module uint32 [n_feds*96]."""
+    import numpy as np
+    g = np.ascontiguousarray(gain, np.float32)
+    n = np.ascontiguousarray(noise, np.float32)
+    b = np.ascontiguousarray(bad, np.uint8)
+    m = np.ascontiguousarray(chan_module, np.uint32)
+    _check(ctx, load().sst_upload_calib(ctx, _ptr(g), _ptr(n), _ptr(b), _ptr(m)), "sst_upload_calib")
+
+
+def make_output(*, n_clusters, cl_module, cl_first, cl_width, cl_charge, cl_bary, cl_adc_off, cl_adc,
+                dev_status, cap_clusters: int, cap_adc: int, strip_adc=None, chan_off=None,
+                chan_len=None, seed_idx=None, cap_seeds: int = 0, cl_snr=None) -> sst_output:
+    return sst_output(_ptr(strip_adc), _ptr(chan_off), _ptr(chan_len), _ptr(seed_idx), cap_seeds,
+                      cap_clusters, cap_adc, _ptr(n_clusters), _ptr(cl_module), _ptr(cl_first),
+                      _ptr(cl_width), _ptr(cl_charge), _ptr(cl_bary), _ptr(cl_adc_off), _ptr(cl_snr),
+                      _ptr(cl_adc), _ptr(dev_status))
+
+
+def sst_unpack_cluster(ctx, raw, fed_offsets, thresholds, out: sst_output, stream: int = 0):
+    """raw / fed_offsets: DEVICE tensors; stream: cudaStream_t as int.  Does not synchronise."""
+    thr = thresholds if isinstance(thresholds, sst_thresholds) else sst_thresholds(*map(float, thresholds))
+    rc = load().sst_unpack_cluster(ctx, _ptr(raw), _ptr(fed_offsets), C.byref(thr), C.byref(out),
+                                   C.c_void_p(stream))
+    _check(ctx, rc, "sst_unpack_cluster")
+
+
+def sst_unpack_cluster_host(ctx, raw, raw_bytes: int, fed_offsets, thresholds, out: sst_output,
+                            stream: int = 0):
+    """HOST buffers in and out (see sst.h); returns after the stream has completed."""
+    thr = thresholds if isinstance(thresholds, sst_thresholds) else sst_thresholds(*map(float, thresholds))
+    rc = load().sst_unpack_cluster_host(ctx, _ptr(raw), raw_bytes, _ptr(fed_offsets), C.byref(thr),
+                                        C.byref(out), C.c_void_p(stream))
+    _check(ctx, rc, "sst_unpack_cluster_host")
+
+
+def sst_event_alloc(ctx, nbytes: int, stream: int = 0) -> int:
+    p = C.c_void_p()
+    _check(ctx, load().sst_event_alloc(ctx, nbytes, C.c_void_p(stream), C.byref(p)), "sst_event_alloc")
+    return p.value
+
+
+def sst_event_free(ctx, ptr: int, stream: int = 0):
+    _check(ctx, load().sst_event_free(ctx, C.c_void_p(ptr), C.c_void_p(stream)), "sst_event_free")
+
+
+def sst_event_upload(ctx, raw, raw_bytes: int, fed_offsets, stream: int = 0):
+    """HOST (pinned) raw / fed_offsets -> pooled device buffers on `stream`; returns the two
+    device pointers (ints).  Free both with sst_event_free."""
+    d_raw, d_fo = C.c_void_p(), C.c_void_p()
+    rc = load().sst_event_upload(ctx, _ptr(raw), raw_bytes, _ptr(fed_offsets), C.c_void_p(stream),
+                                 C.byref(d_raw), C.byref(d_fo))
+    _check(ctx, rc, "sst_event_upload")
+    return d_raw.value, d_fo.value
+
+
+def sst_destroy(ctx):
+    _check(None, load().sst_destroy(ctx), "sst_destroy")
+
+
+def sst_get_info(ctx) -> dict:
+    info = sst_info()
+    _check(ctx, load().sst_get_info(ctx, C.byref(info)), "sst_get_info")
+    return {k: getattr(info, k) for k, _ in sst_info._fields_}

@@ -1,0 +1,923 @@
+// sst.cu -- libsst: unpack + three-threshold clustering of strip-tracker FED data on B200.
+//
+// One fused kernel per event, one CTA per FED (a FED is 96 channels x 256 strips;
+// modules never cross a FED, reading s10), so every step of the path
+// runs on data resident in shared memory:
+//
+//   a1 channel-location map : TMA bulk copy of the whole FED payload to smem, 96-step length
+//                             chain walked in smem (PAPER.md:31 builds this map on the CPU)
+//   a2 unpack               : one thread per channel walks its runs and scatters ADC bytes into
+//                             a dense 96x256 smem tile; the tile leaves with one TMA bulk store
+//   a3 flags                : compact list of present strips -> one gather of {noise, gain}
+//                             per present strip -> active / seed bit masks (exact >= tests)
+//   a4 seed-index array     : the seed mask + block scan; materialised on request
+//   a5 expansion/ownership  : per seed, bit scans left/right over the active mask inside the
+//                             module; only the leftmost seed of a run goes on
+//   a6 gain corr + accept   : q = min(254, floor(adc/gain + .5)) in float32, Q^2 >= t^2 * sum n^2
+//   a7 ordered output       : block scan + decoupled look-back over per-FED aggregates, records
+//                             written in (module, first strip) order
+//
+// No tensor cores: nothing here is a contraction.  See DESIGN.md for layout and rooflines.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "sst.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kChan = 96;
+constexpr int kStrip = 256;
+constexpr int kFedStrips = kChan * kStrip;  // 24576
+constexpr int kWords = kFedStrips / 32;     // 768 mask words per FED
+constexpr int kRawCap = 11264;              // FED payloads up to this size are staged in smem
+constexpr int kListCap = 4096;              // present-strip list; larger FEDs use the dense path
+constexpr int kWide = 32;                   // clusters wider than this are summed by a warp
+constexpr int kWideQ = 64;
+
+// per-FED aggregate published for the look-back (one 64-bit word)
+constexpr int kShAdc = 14, kShSeed = 29, kShMalf = 44, kShOvr = 51;
+constexpr unsigned long long kReady = 1ull << 63;
+
+struct __align__(128) Smem {
+    uint8_t tile[kFedStrips];  // dense ADC of the FED; gain-corrected in place at active strips
+    uint8_t raw[kRawCap];      // FED payload (TMA destination)
+    uint32_t act[kWords], seed[kWords], acc[kWords];
+    uint16_t list[kListCap];
+    uint32_t mod_id[kChan];
+    uint32_t chan_off[kChan];  // FED-local byte offset of the first run byte
+    uint16_t chan_len[kChan];
+    uint8_t mod_lo[kChan], mod_hi[kChan];  // first channel / end channel of the channel's module
+    uint32_t wscan[2][kWarps];
+    uint32_t red[5][kWarps];
+    uint32_t wide_q[kWideQ];
+    unsigned long long mbar;
+    uint32_t list_count, wide_count;
+    uint32_t fed_start, fed_size, in_smem, overrun;
+};
+
+struct KParams {
+    const uint8_t *raw;
+    const uint32_t *fed_offsets;
+    const float2 *calib;  // {noise (+inf at bad strips), gain} per strip
+    const uint32_t *chan_module;
+    unsigned long long *fed_state;
+    double tcl2;
+    float t_ch, t_seed;
+    uint32_t max_raw_bytes, n_feds;
+    sst_output out;
+};
+
+// ------------------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ uint32_t smem_addr(const void *p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_addr(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+// TMA bulk copy global -> shared (non-tensor form), completion on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes,
+                                         unsigned long long *bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(smem_addr(dst)),
+        "l"(src), "r"(bytes), "r"(smem_addr(bar))
+        : "memory");
+}
+// TMA bulk copy shared -> global
+__device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst),
+                 "r"(smem_addr(src)), "r"(bytes)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ unsigned long long ld_state(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_state(unsigned long long *p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// ------------------------------------------------------------------------------ arithmetic
+// adc >= t * noise decided in exact arithmetic with float32 only: t*n = p + e exactly (FMA).
+// noise = +inf (bad strip) gives p = inf, e = NaN -> false.
+__device__ __forceinline__ bool ge_exact(float a, float t, float n) {
+    const float p = __fmul_rn(t, n);
+    const float e = __fmaf_rn(t, n, -p);
+    return (a > p) || (a == p && e <= 0.0f);
+}
+// min(254, floor(fl32(fl32(adc / gain) + 0.5)))  (IEEE RN division and add, no contraction)
+__device__ __forceinline__ uint32_t gain_correct(uint32_t adc, float gain) {
+    const float u = __fadd_rn(__fdiv_rn(static_cast<float>(adc), gain), 0.5f);
+    const float fl = floorf(u);
+    return fl >= 254.0f ? 254u : static_cast<uint32_t>(fl);
+}
+
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// last strip of the maximal active run that starts at (or contains) strip s, bounded by the
+// module end `me` (exclusive, a multiple of 256)
+__device__ __forceinline__ int right_end(const uint32_t *act, int s, int me) {
+    int w = s >> 5;
+    const int b = s & 31;
+    uint32_t inact = ~act[w] & (b == 31 ? 0u : (0xffffffffu << (b + 1)));
+    while (true) {
+        if (inact) return (w << 5) + __ffs(inact) - 2;
+        if (((w + 1) << 5) >= me) return me - 1;
+        ++w;
+        inact = ~act[w];
+    }
+}
+
+// Cluster acceptance for a narrow candidate, one thread: Q^2 >= t_cl^2 * n2 with n2 the double
+// sum of noise^2 taken strictly left to right (reading s15).
+__device__ __forceinline__ bool accept_serial(const uint8_t *tile, const float *noise2f, int l, int w,
+                                              double tcl2) {
+    int Q = 0;
+    double n2 = 0.0;
+    for (int i0 = 0; i0 < w; i0 += 4) {
+        float nv[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) nv[j] = (i0 + j < w) ? __ldg(noise2f + 2 * (l + i0 + j)) : 0.0f;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (i0 + j < w) Q += tile[l + i0 + j];
+            const double d = static_cast<double>(nv[j]);
+            n2 = __dadd_rn(n2, __dmul_rn(d, d));  // + 0.0 for padding lanes is exact
+        }
+    }
+    const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
+    return lhs >= __dmul_rn(tcl2, n2);
+}
+
+// The same decision for a wide candidate by one warp.  A pairwise double sum differs from the
+// sequential one by at most ~w*2^-52 relative; the decision is taken from it only when the two
+// sides are further apart than that, otherwise lane 0 redoes the sum sequentially.
+__device__ __noinline__ bool accept_warp(const uint8_t *tile, const float *noise2f, int l, int w,
+                                         double tcl2, int lane) {
+    uint32_t Q = 0;
+    double n2p = 0.0;
+    for (int i = lane; i < w; i += 32) {
+        Q += tile[l + i];
+        const double d = static_cast<double>(__ldg(noise2f + 2 * (l + i)));
+        n2p += d * d;
+    }
+    Q = warp_sum(Q);
+    n2p = warp_sum_d(n2p);
+    const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
+    const double rhs = tcl2 * n2p;
+    int ok = lhs >= rhs;
+    if (!(fabs(lhs - rhs) > rhs * static_cast<double>(w) * 0x1p-50)) {
+        if (lane == 0) {
+            double n2 = 0.0;
+            for (int i = 0; i < w; ++i) {
+                const double d = static_cast<double>(__ldg(noise2f + 2 * (l + i)));
+                n2 = __dadd_rn(n2, __dmul_rn(d, d));
+            }
+            ok = lhs >= __dmul_rn(tcl2, n2);
+        }
+        ok = __shfl_sync(0xffffffffu, ok, 0);
+    }
+    return ok != 0;
+}
+
+// ------------------------------------------------------------------------------ the kernel
+__global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_constant__ KParams p) {
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    Smem &s = *reinterpret_cast<Smem *>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t f = blockIdx.x;
+    const sst_output &o = p.out;
+
+    // ---------------------------------------------------------------- a1: stage the FED payload
+    if (tid == 0) {
+        mbar_init(&s.mbar, 1);
+        fence_proxy_async();
+        const uint32_t fo0 = p.fed_offsets[f], fo1 = p.fed_offsets[f + 1];
+        const bool valid = fo0 <= fo1 && fo1 <= p.max_raw_bytes;
+        const uint32_t size = valid ? fo1 - fo0 : 0u;
+        const bool in_smem = size <= static_cast<uint32_t>(kRawCap) && ((fo0 | size) & 15u) == 0 &&
+                             (reinterpret_cast<uintptr_t>(p.raw) & 15u) == 0;
+        s.fed_start = fo0;
+        s.fed_size = size;
+        s.in_smem = in_smem;
+        s.overrun = valid ? 0u : 1u;
+        s.list_count = 0;
+        s.wide_count = 0;
+        if (in_smem && size) {
+            mbar_expect_tx(&s.mbar, size);
+            bulk_g2s(s.raw, p.raw + fo0, size, &s.mbar);
+        }
+    }
+    // meanwhile: clear the tile and the masks, fetch the module ids of the 96 channels
+    {
+        uint4 *t4 = reinterpret_cast<uint4 *>(s.tile);
+        const uint4 z = make_uint4(0, 0, 0, 0);
+        for (int i = tid; i < kFedStrips / 16; i += kThreads) t4[i] = z;
+        uint4 *m4 = reinterpret_cast<uint4 *>(s.act);
+        for (int i = tid; i < 3 * kWords / 4; i += kThreads) m4[i] = z;
+        if (tid < kChan) s.mod_id[tid] = p.chan_module[f * kChan + tid];
+    }
+    __syncthreads();
+    if (tid < kChan) {  // module extent of every channel (modules are runs of equal ids)
+        const uint32_t m = s.mod_id[tid];
+        int lo = tid, hi = tid + 1;
+        while (lo > 0 && s.mod_id[lo - 1] == m) --lo;
+        while (hi < kChan && s.mod_id[hi] == m) ++hi;
+        s.mod_lo[tid] = static_cast<uint8_t>(lo);
+        s.mod_hi[tid] = static_cast<uint8_t>(hi);
+    }
+    const bool in_smem = s.in_smem != 0;
+    const uint32_t fed_size = s.fed_size;
+    const uint8_t *rp = in_smem ? s.raw : p.raw + s.fed_start;
+
+    // ---------------------------------------------------------------- a1: walk the length chain
+    if (tid == 0) {
+        if (in_smem && fed_size) mbar_wait(&s.mbar, 0);
+        uint32_t pos = 0;
+        bool over = s.overrun != 0;
+        for (int c = 0; c < kChan; ++c) {
+            uint32_t off = fed_size, L = 0;
+            if (!over) {
+                if (pos + 2 > fed_size) {
+                    over = true;
+                } else {
+                    const uint32_t l16 = rp[pos] | (static_cast<uint32_t>(rp[pos + 1]) << 8);
+                    if (pos + 2 + l16 > fed_size) {
+                        over = true;
+                    } else {
+                        off = pos + 2;
+                        L = l16;
+                        pos = off + L;
+                    }
+                }
+            }
+            s.chan_off[c] = off;
+            s.chan_len[c] = static_cast<uint16_t>(L);
+        }
+        s.overrun = over ? 1u : 0u;
+    }
+    __syncthreads();
+
+    // ---------------------------------------------------------------- a2: unpack, thread per channel
+    int malformed = 0;
+    if (tid < kChan) {
+        if (in_smem && fed_size) mbar_wait(&s.mbar, 0);  // async-proxy writes visible to this thread
+        const uint32_t off = s.chan_off[tid], L = s.chan_len[tid];
+        if (o.chan_off) o.chan_off[f * kChan + tid] = s.fed_start + off;
+        if (o.chan_len) o.chan_len[f * kChan + tid] = static_cast<uint16_t>(L);
+        uint8_t *row = s.tile + tid * kStrip;
+        uint32_t q = off, next_free = 0;
+        const uint32_t qend = off + L;
+        bool ok = true;
+        while (q < qend) {
+            if (q + 2 > qend) { ok = false; break; }
+            const uint32_t first = rp[q];
+            uint32_t len = rp[q + 1];
+            if (len == 0) len = 256;
+            if (first < next_free || first + len > kStrip || q + 2 + len > qend) { ok = false; break; }
+            const uint32_t lpos = atomicAdd(&s.list_count, len);
+            for (uint32_t i = 0; i < len; ++i) {
+                row[first + i] = rp[q + 2 + i];
+                if (lpos + i < kListCap) s.list[lpos + i] = static_cast<uint16_t>(tid * kStrip + first + i);
+            }
+            next_free = first + len;
+            q += 2 + len;
+        }
+        if (!ok) {  // a malformed channel contributes no strips (stale list entries see adc = 0)
+            uint32_t *r32 = reinterpret_cast<uint32_t *>(row);
+            for (int i = 0; i < kStrip / 4; ++i) r32[i] = 0;
+            malformed = 1;
+        }
+    }
+    fence_proxy_async();  // tile writes -> visible to the TMA store below
+    const uint32_t n_malformed = __syncthreads_count(malformed);
+
+    // ---------------------------------------------------------------- a2: dense tile leaves
+    bool store_pending = false;
+    if (o.strip_adc) {
+        uint8_t *dst = o.strip_adc + static_cast<size_t>(f) * kFedStrips;
+        if ((reinterpret_cast<uintptr_t>(o.strip_adc) & 15u) == 0) {
+            if (tid == 0) bulk_s2g(dst, s.tile, kFedStrips);
+            store_pending = true;
+        } else {
+            for (int i = tid; i < kFedStrips; i += kThreads) dst[i] = s.tile[i];
+            __syncthreads();
+        }
+    }
+
+    // ---------------------------------------------------------------- a3: active / seed flags
+    const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
+    const float *noise2f = reinterpret_cast<const float *>(cal);
+    const uint32_t n_list = s.list_count;
+    bool first_batch = true;
+    if (n_list <= static_cast<uint32_t>(kListCap)) {
+        for (uint32_t base = 0; base < n_list || first_batch; base += kThreads * 4) {
+            uint32_t sidx[4], a[4];
+            float2 cv[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t i = base + j * kThreads + tid;
+                sidx[j] = i < n_list ? s.list[i] : 0u;
+                a[j] = i < n_list ? s.tile[sidx[j]] : 0u;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (a[j]) cv[j] = __ldg(cal + sidx[j]);
+            if (first_batch) {  // the TMA store must have read the tile before it is modified
+                if (store_pending && tid == 0) bulk_wait_read();
+                __syncthreads();
+                first_batch = false;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (a[j]) {
+                    const float af = static_cast<float>(a[j]);
+                    if (ge_exact(af, p.t_ch, cv[j].x)) {
+                        const uint32_t bit = 1u << (sidx[j] & 31);
+                        atomicOr(&s.act[sidx[j] >> 5], bit);
+                        if (ge_exact(af, p.t_seed, cv[j].x)) atomicOr(&s.seed[sidx[j] >> 5], bit);
+                        s.tile[sidx[j]] = static_cast<uint8_t>(gain_correct(a[j], cv[j].y));
+                    }
+                }
+            }
+        }
+    } else {  // dense path: every strip slot is visited, 8 predicated gathers in flight per thread
+        uint32_t *t32 = reinterpret_cast<uint32_t *>(s.tile);
+        for (int k = 0; k < kFedStrips / 4 / kThreads; k += 2) {
+            uint32_t wv[2];
+            float2 cv[8];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) wv[h] = t32[tid + (k + h) * kThreads];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if ((wv[h] >> (8 * j)) & 0xffu) cv[h * 4 + j] = __ldg(cal + 4 * (tid + (k + h) * kThreads) + j);
+            if (first_batch) {
+                if (store_pending && tid == 0) bulk_wait_read();
+                __syncthreads();
+                first_batch = false;
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int wi = tid + (k + h) * kThreads;  // tile word = strips 4*wi .. 4*wi+3
+                uint32_t am = 0, sm = 0, nw = wv[h];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t a = (wv[h] >> (8 * j)) & 0xffu;
+                    if (a) {
+                        const float af = static_cast<float>(a);
+                        const float2 c = cv[h * 4 + j];
+                        if (ge_exact(af, p.t_ch, c.x)) {
+                            am |= 1u << j;
+                            if (ge_exact(af, p.t_seed, c.x)) sm |= 1u << j;
+                            nw = (nw & ~(0xffu << (8 * j))) | (gain_correct(a, c.y) << (8 * j));
+                        }
+                    }
+                }
+                if (am) {
+                    t32[wi] = nw;
+                    atomicOr(&s.act[wi >> 3], am << ((wi & 7) * 4));
+                    if (sm) atomicOr(&s.seed[wi >> 3], sm << ((wi & 7) * 4));
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---------------------------------------------------------------- a5 + a6: per seed
+    for (int k = 0; k < kWords / kThreads; ++k) {
+        const int w = tid + k * kThreads;
+        uint32_t sbits = s.seed[w];
+        while (sbits) {
+            const int b = __ffs(sbits) - 1;
+            sbits &= sbits - 1;
+            const int sstrip = (w << 5) + b;
+            const int ch = sstrip >> 8;
+            const int ms = s.mod_lo[ch] * kStrip, me = s.mod_hi[ch] * kStrip;
+            // left: nearest inactive strip or nearest seed, whichever comes first
+            int ww = w, l;
+            uint32_t below = (1u << b) - 1u;
+            bool owner = true;
+            while (true) {
+                const uint32_t inact = ~s.act[ww] & below;
+                const uint32_t sd = s.seed[ww] & below;
+                if (inact) {
+                    const int hi = 31 - __clz(inact);
+                    if (sd >> hi > 1u) owner = false;  // a seed between the gap and this seed
+                    l = (ww << 5) + hi + 1;
+                    break;
+                }
+                if (sd) { owner = false; break; }
+                if ((ww << 5) <= ms) { l = ms; break; }
+                --ww;
+                below = 0xffffffffu;
+            }
+            if (!owner) continue;  // leftmost-seed ownership: another seed emits this cluster
+            const int r = right_end(s.act, sstrip, me);
+            const int wd = r - l + 1;
+            if (wd > kWide) {
+                const uint32_t slot = atomicAdd(&s.wide_count, 1u);
+                if (slot < kWideQ) {
+                    s.wide_q[slot] = static_cast<uint32_t>(l) | (static_cast<uint32_t>(wd) << 16);
+                    continue;
+                }
+            }
+            if (accept_serial(s.tile, noise2f, l, wd, p.tcl2)) atomicOr(&s.acc[l >> 5], 1u << (l & 31));
+        }
+    }
+    __syncthreads();
+    {
+        const uint32_t nq = min(s.wide_count, static_cast<uint32_t>(kWideQ));
+        for (uint32_t e = warp; e < nq; e += kWarps) {
+            const int l = s.wide_q[e] & 0xffffu, wd = s.wide_q[e] >> 16;
+            if (accept_warp(s.tile, noise2f, l, wd, p.tcl2, lane) && lane == 0)
+                atomicOr(&s.acc[l >> 5], 1u << (l & 31));
+        }
+    }
+    __syncthreads();
+
+    // ---------------------------------------------------------------- a7: local scan
+    // thread t owns mask words 3t .. 3t+2 (96 consecutive strips)
+    uint32_t my_cl = 0, my_adc = 0, my_seed = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int w = 3 * tid + k;
+        uint32_t m = s.acc[w];
+        my_cl += __popc(m);
+        my_seed += __popc(s.seed[w]);
+        while (m) {
+            const int l = (w << 5) + __ffs(m) - 1;
+            m &= m - 1;
+            my_adc += right_end(s.act, l, s.mod_hi[l >> 8] * kStrip) - l + 1;
+        }
+    }
+    uint32_t inc_a = my_cl | (my_adc << 16), inc_s = my_seed;  // my_cl <= 48, my_adc <= 96 per thread
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t ua = __shfl_up_sync(0xffffffffu, inc_a, d);
+        const uint32_t us = __shfl_up_sync(0xffffffffu, inc_s, d);
+        if (lane >= d) { inc_a += ua; inc_s += us; }
+    }
+    if (lane == 31) { s.wscan[0][warp] = inc_a; s.wscan[1][warp] = inc_s; }
+    __syncthreads();
+    uint32_t pre_a = 0, pre_s = 0, tot_a = 0, tot_s = 0;
+#pragma unroll
+    for (int i = 0; i < kWarps; ++i) {
+        if (i < warp) { pre_a += s.wscan[0][i]; pre_s += s.wscan[1][i]; }
+        tot_a += s.wscan[0][i];
+        tot_s += s.wscan[1][i];
+    }
+    // CTA totals: clusters <= 12288 and ADC bytes <= 24576 keep the packed halves apart
+    const uint32_t fed_cl = tot_a & 0xffffu, fed_adc = tot_a >> 16, fed_seed = tot_s;
+    uint32_t ex_cl = (pre_a + inc_a - (my_cl | (my_adc << 16))) & 0xffffu;
+    uint32_t ex_adc = (pre_a + inc_a - (my_cl | (my_adc << 16))) >> 16;
+    uint32_t ex_seed = pre_s + inc_s - my_seed;
+    const uint32_t fed_over = s.overrun;
+
+    // ---------------------------------------------------------------- a7: decoupled look-back
+    if (tid == 0) {
+        const unsigned long long agg = kReady | fed_cl | (static_cast<unsigned long long>(fed_adc) << kShAdc) |
+                                       (static_cast<unsigned long long>(fed_seed) << kShSeed) |
+                                       (static_cast<unsigned long long>(n_malformed) << kShMalf) |
+                                       (static_cast<unsigned long long>(fed_over) << kShOvr);
+        st_state(p.fed_state + f, agg);
+    }
+    uint32_t b_cl = 0, b_adc = 0, b_seed = 0, b_malf = 0, b_over = 0;
+    for (uint32_t j = tid; j < f; j += kThreads) {
+        unsigned long long v = ld_state(p.fed_state + j);
+        while (!(v & kReady)) {
+            __nanosleep(40);
+            v = ld_state(p.fed_state + j);
+        }
+        b_cl += static_cast<uint32_t>(v) & 0x3fffu;
+        b_adc += static_cast<uint32_t>(v >> kShAdc) & 0x7fffu;
+        b_seed += static_cast<uint32_t>(v >> kShSeed) & 0x7fffu;
+        b_malf += static_cast<uint32_t>(v >> kShMalf) & 0x7fu;
+        b_over += static_cast<uint32_t>(v >> kShOvr) & 1u;
+    }
+    b_cl = warp_sum(b_cl); b_adc = warp_sum(b_adc); b_seed = warp_sum(b_seed);
+    b_malf = warp_sum(b_malf); b_over = warp_sum(b_over);
+    if (lane == 0) {
+        s.red[0][warp] = b_cl; s.red[1][warp] = b_adc; s.red[2][warp] = b_seed;
+        s.red[3][warp] = b_malf; s.red[4][warp] = b_over;
+    }
+    __syncthreads();
+    b_cl = b_adc = b_seed = b_malf = b_over = 0;
+#pragma unroll
+    for (int i = 0; i < kWarps; ++i) {
+        b_cl += s.red[0][i]; b_adc += s.red[1][i]; b_seed += s.red[2][i];
+        b_malf += s.red[3][i]; b_over += s.red[4][i];
+    }
+
+    // ---------------------------------------------------------------- a7: emit, (module, first strip) order
+    uint32_t k_cl = b_cl + ex_cl, k_adc = b_adc + ex_adc, k_seed = b_seed + ex_seed;
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) {
+        const int w = 3 * tid + k;
+        if (o.seed_idx) {
+            uint32_t sb = s.seed[w];
+            while (sb) {
+                const int b = __ffs(sb) - 1;
+                sb &= sb - 1;
+                if (k_seed < o.cap_seeds) o.seed_idx[k_seed] = f * kFedStrips + (w << 5) + b;
+                ++k_seed;
+            }
+        }
+        uint32_t m = s.acc[w];
+        while (m) {
+            const int l = (w << 5) + __ffs(m) - 1;
+            m &= m - 1;
+            const int ch = l >> 8;
+            const int wd = right_end(s.act, l, s.mod_hi[ch] * kStrip) - l + 1;
+            const bool fits = k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc;
+            if (fits) {
+                int Q = 0;
+                long long M = 0;
+                for (int i = 0; i < wd; ++i) {
+                    const int q = s.tile[l + i];
+                    Q += q;
+                    M += static_cast<long long>(i) * q;
+                    o.cl_adc[k_adc + i] = static_cast<uint8_t>(q);
+                }
+                const int first = l - s.mod_lo[ch] * kStrip;
+                o.cl_module[k_cl] = s.mod_id[ch];
+                o.cl_first[k_cl] = static_cast<uint16_t>(first);
+                o.cl_width[k_cl] = static_cast<uint16_t>(wd);
+                o.cl_charge[k_cl] = Q;
+                o.cl_bary[k_cl] = static_cast<float>(static_cast<double>(first) +
+                                                      static_cast<double>(M) / static_cast<double>(Q));
+                o.cl_adc_off[k_cl] = k_adc;
+                if (o.cl_snr) {
+                    double n2 = 0.0;
+                    for (int i = 0; i < wd; ++i) {
+                        const double d = static_cast<double>(__ldg(noise2f + 2 * (l + i)));
+                        n2 = __dadd_rn(n2, __dmul_rn(d, d));
+                    }
+                    o.cl_snr[k_cl] = static_cast<float>(static_cast<double>(Q) / sqrt(n2));
+                }
+            } else {
+                // the first cluster that does not fit reports how many were written
+                const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
+                if (prev_fits) *o.n_clusters = k_cl;
+            }
+            ++k_cl;
+            k_adc += wd;
+        }
+    }
+    if (f == p.n_feds - 1 && tid == 0) {  // event totals = prefix of the last FED + its own
+        const uint32_t n_cl = b_cl + fed_cl, n_adc = b_adc + fed_adc, n_mal = b_malf + n_malformed,
+                       n_over = b_over + fed_over;
+        uint32_t flags = 0;
+        if (n_cl > o.cap_clusters) flags |= SST_FLAG_CLUSTER_CAP;
+        if (n_adc > o.cap_adc) flags |= SST_FLAG_ADC_CAP;
+        if (n_mal) flags |= SST_FLAG_MALFORMED;
+        if (n_over) flags |= SST_FLAG_OVERRUN;
+        if (!(flags & (SST_FLAG_CLUSTER_CAP | SST_FLAG_ADC_CAP))) *o.n_clusters = n_cl;
+        o.dev_status[SST_ST_FLAGS] = flags;
+        o.dev_status[SST_ST_N_MALFORMED] = n_mal;
+        o.dev_status[SST_ST_N_CLUSTERS] = n_cl;
+        o.dev_status[SST_ST_N_ADC] = n_adc;
+        o.dev_status[SST_ST_N_OVERRUN] = n_over;
+        o.dev_status[SST_ST_N_SEEDS] = b_seed + fed_seed;
+        o.dev_status[6] = 0;
+        o.dev_status[7] = 0;
+    }
+    // smem must stay valid until the bulk store has read it (covered above whenever it was issued)
+}
+
+}  // namespace
+
+// ====================================================================================== host
+struct sst_ctx {
+    sst_config cfg{};
+    cudaMemPool_t pool = nullptr;
+    float2 *calib = nullptr;
+    uint32_t *chan_module = nullptr;
+    bool has_calib = false;
+    std::atomic<int32_t> last_err{0};
+    int sm_count = 0;
+    int ctas_per_sm = 0;
+};
+
+namespace {
+
+inline bool cu_ok(sst_ctx *ctx, cudaError_t e) {
+    if (e == cudaSuccess) return true;
+    if (ctx) ctx->last_err.store(static_cast<int32_t>(e));
+    return false;
+}
+#define SST_CU(call) \
+    do { if (!cu_ok(ctx, (call))) return SST_ERR_CUDA; } while (0)
+
+bool thresholds_ok(const sst_thresholds *t) {
+    const float v[3] = {t->channel, t->seed, t->cluster};
+    for (float x : v)
+        if (!std::isfinite(x) || !(x > 0.0f)) return false;
+    return true;
+}
+
+bool output_ok(const sst_output *o) {
+    return o && o->n_clusters && o->dev_status && o->cl_module && o->cl_first && o->cl_width &&
+           o->cl_charge && o->cl_bary && o->cl_adc_off && o->cl_adc;
+}
+
+sst_status launch_event(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
+                        const sst_thresholds *thr, const sst_output *out, cudaStream_t st) {
+    const uint32_t nf = ctx->cfg.n_feds;
+    unsigned long long *state = nullptr;
+    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&state), sizeof(unsigned long long) * nf,
+                                   ctx->pool, st));
+    SST_CU(cudaMemsetAsync(state, 0, sizeof(unsigned long long) * nf, st));
+    KParams kp{};
+    kp.raw = raw;
+    kp.fed_offsets = fed_offsets;
+    kp.calib = ctx->calib;
+    kp.chan_module = ctx->chan_module;
+    kp.fed_state = state;
+    kp.tcl2 = static_cast<double>(thr->cluster) * static_cast<double>(thr->cluster);  // exact
+    kp.t_ch = thr->channel;
+    kp.t_seed = thr->seed;
+    kp.max_raw_bytes = ctx->cfg.max_raw_bytes;
+    kp.n_feds = nf;
+    kp.out = *out;
+    sst_fed_kernel<<<nf, kThreads, sizeof(Smem), st>>>(kp);
+    SST_CU(cudaGetLastError());
+    SST_CU(cudaFreeAsync(state, st));
+    return SST_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
+    if (out_ctx) *out_ctx = nullptr;
+    if (!cfg || !out_ctx || cfg->n_feds == 0 || cfg->n_feds > 65535u || cfg->max_raw_bytes == 0)
+        return SST_ERR_INVALID_ARG;
+    sst_ctx *ctx = new (std::nothrow) sst_ctx();
+    if (!ctx) return SST_ERR_INVALID_ARG;
+    ctx->cfg = *cfg;
+    if (ctx->cfg.max_events_in_flight == 0) ctx->cfg.max_events_in_flight = 8;
+    auto fail = [&](sst_status s) {
+        if (ctx->calib) cudaFree(ctx->calib);
+        if (ctx->chan_module) cudaFree(ctx->chan_module);
+        if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
+        delete ctx;
+        return s;
+    };
+    if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(SST_ERR_CUDA);
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = cfg->device;
+    if (cudaMemPoolCreate(&ctx->pool, &props) != cudaSuccess) return fail(SST_ERR_CUDA);
+    unsigned long long keep = ~0ull;  // never give memory back between events
+    if (cudaMemPoolSetAttribute(ctx->pool, cudaMemPoolAttrReleaseThreshold, &keep) != cudaSuccess)
+        return fail(SST_ERR_CUDA);
+    const size_t n = static_cast<size_t>(cfg->n_feds) * kFedStrips;
+    if (cudaMalloc(&ctx->calib, n * sizeof(float2)) != cudaSuccess) return fail(SST_ERR_CUDA);
+    if (cudaMalloc(&ctx->chan_module, static_cast<size_t>(cfg->n_feds) * kChan * sizeof(uint32_t)) !=
+        cudaSuccess)
+        return fail(SST_ERR_CUDA);
+    if (cudaFuncSetAttribute(sst_fed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(sizeof(Smem))) != cudaSuccess)
+        return fail(SST_ERR_CUDA);
+    cudaFuncSetAttribute(sst_fed_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->ctas_per_sm, sst_fed_kernel, kThreads,
+                                                  sizeof(Smem));
+    *out_ctx = ctx;
+    return SST_OK;
+}
+
+sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise, const uint8_t *bad,
+                            const uint32_t *chan_module) {
+    if (!ctx || !gain || !noise || !bad || !chan_module) return SST_ERR_INVALID_ARG;
+    const uint32_t nf = ctx->cfg.n_feds;
+    const size_t n = static_cast<size_t>(nf) * kFedStrips, nch = static_cast<size_t>(nf) * kChan;
+    for (size_t c = 1; c < nch; ++c) {
+        if (chan_module[c] < chan_module[c - 1]) return SST_ERR_BAD_CALIB;
+        if (c % kChan == 0 && chan_module[c] == chan_module[c - 1]) return SST_ERR_BAD_CALIB;
+    }
+    std::vector<float2> packed;
+    try {
+        packed.resize(n);
+    } catch (...) {
+        return SST_ERR_INVALID_ARG;
+    }
+    for (size_t g = 0; g < n; ++g) {
+        if (bad[g]) {
+            // a bad strip is never active: noise = +inf fails every >= test; gain is never used
+            packed[g] = make_float2(INFINITY, 1.0f);
+        } else {
+            if (!std::isfinite(gain[g]) || !(gain[g] > 0.0f) || !std::isfinite(noise[g]) || !(noise[g] > 0.0f))
+                return SST_ERR_BAD_CALIB;
+            packed[g] = make_float2(noise[g], gain[g]);
+        }
+    }
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    SST_CU(cudaMemcpy(ctx->calib, packed.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
+    SST_CU(cudaMemcpy(ctx->chan_module, chan_module, nch * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    SST_CU(cudaDeviceSynchronize());
+    ctx->has_calib = true;
+    return SST_OK;
+}
+
+sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
+                              const sst_thresholds *thr, const sst_output *out, void *stream) {
+    if (!ctx || !raw || !fed_offsets || !thr || !output_ok(out) || !thresholds_ok(thr))
+        return SST_ERR_INVALID_ARG;
+    if (out->seed_idx == nullptr && out->cap_seeds != 0) return SST_ERR_INVALID_ARG;
+    if (!ctx->has_calib) return SST_ERR_NO_CALIB;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    return launch_event(ctx, raw, fed_offsets, thr, out, static_cast<cudaStream_t>(stream));
+}
+
+sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes,
+                                   const uint32_t *fed_offsets, const sst_thresholds *thr,
+                                   const sst_output *out, void *stream) {
+    if (!ctx || !raw || !fed_offsets || !thr || !output_ok(out) || !thresholds_ok(thr))
+        return SST_ERR_INVALID_ARG;
+    if (raw_bytes > ctx->cfg.max_raw_bytes) return SST_ERR_INVALID_ARG;
+    if (!ctx->has_calib) return SST_ERR_NO_CALIB;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const uint32_t nf = ctx->cfg.n_feds;
+    const size_t n = static_cast<size_t>(nf) * kFedStrips, nch = static_cast<size_t>(nf) * kChan;
+    auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
+    // one pooled block, carved up
+    const size_t o_raw = 0, o_fo = o_raw + up(ctx->cfg.max_raw_bytes), o_st = o_fo + up((nf + 1) * 4),
+                 o_ncl = o_st + up(SST_ST_WORDS * 4), o_mod = o_ncl + 256,
+                 o_first = o_mod + up(4ull * out->cap_clusters), o_width = o_first + up(2ull * out->cap_clusters),
+                 o_charge = o_width + up(2ull * out->cap_clusters), o_bary = o_charge + up(4ull * out->cap_clusters),
+                 o_aoff = o_bary + up(4ull * out->cap_clusters), o_snr = o_aoff + up(4ull * out->cap_clusters),
+                 o_adc = o_snr + (out->cl_snr ? up(4ull * out->cap_clusters) : 0), o_dense = o_adc + up(out->cap_adc),
+                 o_coff = o_dense + (out->strip_adc ? up(n) : 0), o_clen = o_coff + (out->chan_off ? up(4 * nch) : 0),
+                 o_seed = o_clen + (out->chan_len ? up(2 * nch) : 0),
+                 total = o_seed + (out->seed_idx ? up(4ull * out->cap_seeds) : 0);
+    uint8_t *blk = nullptr;
+    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), total, ctx->pool, st));
+    sst_status rc = SST_OK;
+    auto CU = [&](cudaError_t e) { if (rc == SST_OK && !cu_ok(ctx, e)) rc = SST_ERR_CUDA; };
+    CU(cudaMemcpyAsync(blk + o_raw, raw, raw_bytes, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(blk + o_fo, fed_offsets, (nf + 1) * 4, cudaMemcpyHostToDevice, st));
+    sst_output d = *out;
+    d.dev_status = reinterpret_cast<uint32_t *>(blk + o_st);
+    d.n_clusters = reinterpret_cast<uint32_t *>(blk + o_ncl);
+    d.cl_module = reinterpret_cast<uint32_t *>(blk + o_mod);
+    d.cl_first = reinterpret_cast<uint16_t *>(blk + o_first);
+    d.cl_width = reinterpret_cast<uint16_t *>(blk + o_width);
+    d.cl_charge = reinterpret_cast<int32_t *>(blk + o_charge);
+    d.cl_bary = reinterpret_cast<float *>(blk + o_bary);
+    d.cl_adc_off = reinterpret_cast<uint32_t *>(blk + o_aoff);
+    d.cl_snr = out->cl_snr ? reinterpret_cast<float *>(blk + o_snr) : nullptr;
+    d.cl_adc = blk + o_adc;
+    d.strip_adc = out->strip_adc ? blk + o_dense : nullptr;
+    d.chan_off = out->chan_off ? reinterpret_cast<uint32_t *>(blk + o_coff) : nullptr;
+    d.chan_len = out->chan_len ? reinterpret_cast<uint16_t *>(blk + o_clen) : nullptr;
+    d.seed_idx = out->seed_idx ? reinterpret_cast<uint32_t *>(blk + o_seed) : nullptr;
+    if (rc == SST_OK) rc = launch_event(ctx, blk + o_raw, reinterpret_cast<uint32_t *>(blk + o_fo), thr, &d, st);
+    // counts first, then exactly-sized copies of the cluster arrays
+    CU(cudaMemcpyAsync(out->dev_status, d.dev_status, SST_ST_WORDS * 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(out->n_clusters, d.n_clusters, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (rc == SST_OK) {
+        const size_t k = *out->n_clusters;
+        const size_t na = out->dev_status[SST_ST_FLAGS] & (SST_FLAG_CLUSTER_CAP | SST_FLAG_ADC_CAP)
+                              ? out->cap_adc
+                              : out->dev_status[SST_ST_N_ADC];
+        if (k) {
+            CU(cudaMemcpyAsync(out->cl_module, d.cl_module, 4 * k, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(out->cl_first, d.cl_first, 2 * k, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(out->cl_width, d.cl_width, 2 * k, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(out->cl_charge, d.cl_charge, 4 * k, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(out->cl_bary, d.cl_bary, 4 * k, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(out->cl_adc_off, d.cl_adc_off, 4 * k, cudaMemcpyDeviceToHost, st));
+            if (out->cl_snr) CU(cudaMemcpyAsync(out->cl_snr, d.cl_snr, 4 * k, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(out->cl_adc, d.cl_adc, na, cudaMemcpyDeviceToHost, st));
+        }
+        if (out->strip_adc) CU(cudaMemcpyAsync(out->strip_adc, d.strip_adc, n, cudaMemcpyDeviceToHost, st));
+        if (out->chan_off) CU(cudaMemcpyAsync(out->chan_off, d.chan_off, 4 * nch, cudaMemcpyDeviceToHost, st));
+        if (out->chan_len) CU(cudaMemcpyAsync(out->chan_len, d.chan_len, 2 * nch, cudaMemcpyDeviceToHost, st));
+        if (out->seed_idx) {
+            const size_t ns = std::min<size_t>(out->dev_status[SST_ST_N_SEEDS], out->cap_seeds);
+            if (ns) CU(cudaMemcpyAsync(out->seed_idx, d.seed_idx, 4 * ns, cudaMemcpyDeviceToHost, st));
+        }
+    }
+    CU(cudaFreeAsync(blk, st));
+    CU(cudaStreamSynchronize(st));
+    return rc;
+}
+
+sst_status sst_event_alloc(sst_ctx *ctx, uint64_t bytes, void *stream, void **out_ptr) {
+    if (!ctx || !out_ptr || bytes == 0) return SST_ERR_INVALID_ARG;
+    *out_ptr = nullptr;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    SST_CU(cudaMallocFromPoolAsync(out_ptr, bytes, ctx->pool, static_cast<cudaStream_t>(stream)));
+    return SST_OK;
+}
+
+sst_status sst_event_free(sst_ctx *ctx, void *ptr, void *stream) {
+    if (!ctx || !ptr) return SST_ERR_INVALID_ARG;
+    SST_CU(cudaFreeAsync(ptr, static_cast<cudaStream_t>(stream)));
+    return SST_OK;
+}
+
+sst_status sst_event_upload(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes,
+                            const uint32_t *fed_offsets, void *stream, uint8_t **d_raw,
+                            uint32_t **d_fed_offsets) {
+    if (!ctx || !raw || !fed_offsets || !d_raw || !d_fed_offsets || raw_bytes > ctx->cfg.max_raw_bytes)
+        return SST_ERR_INVALID_ARG;
+    *d_raw = nullptr;
+    *d_fed_offsets = nullptr;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t fo_bytes = (static_cast<size_t>(ctx->cfg.n_feds) + 1) * sizeof(uint32_t);
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(d_raw), ctx->cfg.max_raw_bytes, ctx->pool, st));
+    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(d_fed_offsets), fo_bytes, ctx->pool, st));
+    if (raw_bytes) SST_CU(cudaMemcpyAsync(*d_raw, raw, raw_bytes, cudaMemcpyHostToDevice, st));
+    SST_CU(cudaMemcpyAsync(*d_fed_offsets, fed_offsets, fo_bytes, cudaMemcpyHostToDevice, st));
+    return SST_OK;
+}
+
+sst_status sst_destroy(sst_ctx *ctx) {
+    if (!ctx) return SST_ERR_INVALID_ARG;
+    cudaSetDevice(ctx->cfg.device);
+    cudaDeviceSynchronize();
+    if (ctx->calib) cudaFree(ctx->calib);
+    if (ctx->chan_module) cudaFree(ctx->chan_module);
+    if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
+    delete ctx;
+    return SST_OK;
+}
+
+int32_t sst_last_cuda_error(const sst_ctx *ctx) { return ctx ? ctx->last_err.load() : 0; }
+
+const char *sst_status_string(sst_status s) {
+    switch (s) {
+        case SST_OK: return "SST_OK";
+        case SST_ERR_INVALID_ARG: return "SST_ERR_INVALID_ARG";
+        case SST_ERR_CUDA: return "SST_ERR_CUDA";
+        case SST_ERR_NO_CALIB: return "SST_ERR_NO_CALIB";
+        case SST_ERR_BAD_CALIB: return "SST_ERR_BAD_CALIB";
+    }
+    return "SST_ERR_UNKNOWN";
+}
+
+sst_status sst_get_info(const sst_ctx *ctx, sst_info *info) {
+    if (!ctx || !info) return SST_ERR_INVALID_ARG;
+    info->smem_bytes = static_cast<uint32_t>(sizeof(Smem));
+    info->threads = kThreads;
+    info->ctas_per_sm = static_cast<uint32_t>(ctx->ctas_per_sm);
+    info->sm_count = static_cast<uint32_t>(ctx->sm_count);
+    info->kernels_per_event = 1;
+    return SST_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,119 @@
+"""Device-memory plumbing around the binding: torch tensors for the buffers of one event.
+
+Nothing here computes anything about the method; it allocates, copies and calls libsst.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Dict, Optional, Sequence
+
+import numpy as np
+
+from . import binding as B
+
+
+@dataclass
+class EventOutputs:
+    tensors: Dict[str, "object"]
+    out: B.sst_output
+    cap_clusters: int
+    cap_adc: int
+
+    def numpy(self) -> Dict[str, np.ndarray]:
+        """Synchronising read-back, trimmed to the counts the device reported."""
+        t = {k: v.cpu().numpy() for k, v in self.tensors.items()}
+        st = t["dev_status"]
+        k = int(t["n_clusters"][0])
+        overflow = bool(st[B.ST_FLAGS] & (B.FLAG_CLUSTER_CAP | B.FLAG_ADC_CAP))
+        res = {"n_clusters": k, "status": st}
+        for name in ("cl_module", "cl_first", "cl_width", "cl_charge", "cl_bary", "cl_adc_off", "cl_snr"):
+            if name in t:
+                res[name] = t[name][:k]
+        na = int(res["cl_adc_off"][-1]) + int(res["cl_width"][-1]) if k else 0
+        if not overflow:
+            assert na == int(st[B.ST_N_ADC])
+        res["cl_adc"] = t["cl_adc"][:na]
+        for name in ("strip_adc", "chan_off", "chan_len"):
+            if name in t:
+                res[name] = t[name]
+        if "seed_idx" in t:
+            res["seed_idx"] = t["seed_idx"][:min(int(st[B.ST_N_SEEDS]), t["seed_idx"].size)]
+        return res
+
+
+class Detector:
+    """A libsst context bound to one calibration (calibration is per strip, uploaded
+    once and shared by all events)."""
+
+    def __init__(self, n_feds: int, gain, noise, bad, chan_module, device: int = 0,
+                 max_raw_bytes: int = 1 << 22, max_events_in_flight: int = 8):
+        import torch
+        if not torch.cuda.is_available():
+            raise B.SSTError("no CUDA device: libsst has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        self.n_feds = n_feds
+        self.n_strips = n_feds * B.FED_STRIPS
+        self.max_raw_bytes = int(max_raw_bytes)
+        self.ctx = B.sst_create(n_feds, device, self.max_raw_bytes, max_events_in_flight)
+        B.sst_upload_calib(self.ctx, gain, noise, bad, chan_module)
+
+    def close(self):
+        if self.ctx is not None:
+            B.sst_destroy(self.ctx)
+            self.ctx = None
+
+    def info(self) -> dict:
+        return B.sst_get_info(self.ctx)
+
+    def upload_raw(self, raw: np.ndarray, fed_offsets: np.ndarray):
+        """Device copies of one event's raw bytes (padded to max_raw_bytes) and FED offsets."""
+        torch = self.torch
+        assert raw.size <= self.max_raw_bytes
+        d_raw = torch.zeros(self.max_raw_bytes, dtype=torch.uint8, device=self.device)
+        d_raw[:raw.size] = torch.from_numpy(np.ascontiguousarray(raw, np.uint8)).to(self.device)
+        d_fo = torch.from_numpy(np.ascontiguousarray(fed_offsets, np.uint32).view(np.int32)).to(self.device)
+        return d_raw, d_fo
+
+    def alloc_outputs(self, cap_clusters: int, cap_adc: int, dense: bool = True, chan_map: bool = False,
+                      seeds: bool = False, snr: bool = False, cap_seeds: Optional[int] = None) -> EventOutputs:
+        torch = self.torch
+        dev = self.device
+        cc, ca = max(int(cap_clusters), 1), max(int(cap_adc), 1)
+        t = {
+            "n_clusters": torch.zeros(1, dtype=torch.int32, device=dev),
+            "dev_status": torch.zeros(B.ST_WORDS, dtype=torch.int32, device=dev),
+            "cl_module": torch.empty(cc, dtype=torch.int32, device=dev),
+            "cl_first": torch.empty(cc, dtype=torch.int16, device=dev),
+            "cl_width": torch.empty(cc, dtype=torch.int16, device=dev),
+            "cl_charge": torch.empty(cc, dtype=torch.int32, device=dev),
+            "cl_bary": torch.empty(cc, dtype=torch.float32, device=dev),
+            "cl_adc_off": torch.empty(cc, dtype=torch.int32, device=dev),
+            "cl_adc": torch.empty(ca, dtype=torch.uint8, device=dev),
+        }
+        if dense:
+            t["strip_adc"] = torch.empty(self.n_strips, dtype=torch.uint8, device=dev)
+        if chan_map:
+            t["chan_off"] = torch.empty(self.n_feds * B.N_CHAN, dtype=torch.int32, device=dev)
+            t["chan_len"] = torch.empty(self.n_feds * B.N_CHAN, dtype=torch.int16, device=dev)
+        ncs = 0
+        if seeds:
+            ncs = self.n_strips if cap_seeds is None else int(cap_seeds)
+            t["seed_idx"] = torch.empty(max(ncs, 1), dtype=torch.int32, device=dev)
+        if snr:
+            t["cl_snr"] = torch.empty(cc, dtype=torch.float32, device=dev)
+        out = B.make_output(cap_clusters=int(cap_clusters), cap_adc=int(cap_adc), cap_seeds=ncs,
+                            **{k: v for k, v in t.items()})
+        return EventOutputs(t, out, int(cap_clusters), int(cap_adc))
+
+    def run(self, d_raw, d_fo, thresholds: Sequence[float], outputs: EventOutputs, stream=None):
+        """Enqueue one event on `stream` (a torch.cuda.Stream; default: the current stream)."""
+        st = self.torch.cuda.current_stream(self.device) if stream is None else stream
+        B.sst_unpack_cluster(self.ctx, d_raw, d_fo, thresholds, outputs.out, st.cuda_stream)
+
+
+def unsigned_view(res: Dict[str, np.ndarray]) -> Dict[str, np.ndarray]:
+    """torch has no uint16/uint32 tensors everywhere; reinterpret the signed storage."""
+    conv = {"cl_module": np.uint32, "cl_first": np.uint16, "cl_width": np.uint16, "cl_adc_off": np.uint32,
+            "chan_off": np.uint32, "chan_len": np.uint16, "seed_idx": np.uint32, "status": np.uint32}
+    return {k: (v.view(conv[k]) if k in conv and isinstance(v, np.ndarray) else v) for k, v in res.items()}

@@ -1,0 +1,377 @@
+"""GPU parity: libsst (through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): bit-exact on the unpacked SoA, the channel map, the seed-index
+array, cluster boundaries, corrected integer ADCs, charge, count and order; barycenter and float
+S/N within 1e-6 relative.
+"""
+import numpy as np
+import pytest
+
+from paper_2101_11489_b200 import synth
+from tests import cases
+
+pytestmark = pytest.mark.gpu
+
+REL = 1e-6   # north_star: "Barycenters and float S/N must agree within 1e-6 relative"
+
+
+@pytest.fixture(scope="module")
+def H():
+    from paper_2101_11489_b200 import harness
+    return harness
+
+
+def gpu_run(H, n_feds, raw, fed_offsets, gain, noise, bad, chan_module, thresholds, cap_clusters=None,
+            cap_adc=None, max_raw_bytes=None, dense=True, det=None):
+    own = det is None
+    if own:
+        mrb = max_raw_bytes if max_raw_bytes is not None else max(int(raw.size), 16)
+        det = H.Detector(n_feds, gain, noise, bad, chan_module, max_raw_bytes=mrb)
+    try:
+        d_raw, d_fo = det.upload_raw(raw, fed_offsets)
+        cc = int(raw.size // 3 + 1) if cap_clusters is None else cap_clusters
+        ca = int(raw.size + 1) if cap_adc is None else cap_adc
+        outs = det.alloc_outputs(cc, ca, dense=dense, chan_map=True, seeds=True, snr=True)
+        det.run(d_raw, d_fo, thresholds, outs)
+        det.torch.cuda.synchronize()
+        return H.unsigned_view(outs.numpy())
+    finally:
+        if own:
+            det.close()
+
+
+def compare(g, r, check_status=True):
+    """g: GPU result dict, r: OracleResult."""
+    assert np.array_equal(g["strip_adc"], r.adc), "dense SoA differs"
+    assert np.array_equal(g["chan_off"], r.chan_off)
+    assert np.array_equal(g["chan_len"], r.chan_len)
+    assert np.array_equal(g["seed_idx"], r.seed_idx), "seed-index array differs"
+    assert g["n_clusters"] == r.n_clusters
+    for name in ("cl_module", "cl_first", "cl_width", "cl_charge", "cl_adc_off", "cl_adc"):
+        assert np.array_equal(g[name], getattr(r, name)), name
+    np.testing.assert_allclose(g["cl_bary"], r.cl_bary, rtol=REL, atol=0)
+    np.testing.assert_allclose(g["cl_snr"], r.cl_snr, rtol=REL, atol=0)
+    if check_status:
+        assert np.array_equal(g["status"][:6], r.status[:6]), (g["status"], r.status)
+
+
+def both(H, oracle, cs_or_ev, cal=None, thresholds=None, **kw):
+    if cal is None:
+        cs = cs_or_ev
+        args = (cs.n_feds, cs.raw, cs.fed_offsets, cs.gain, cs.noise, cs.bad, cs.chan_module)
+        thr = thresholds or cs.thresholds
+    else:
+        ev = cs_or_ev
+        args = (cal.n_feds, ev.raw, ev.fed_offsets, cal.gain, cal.noise, cal.bad, cal.chan_module)
+        thr = thresholds
+    g = gpu_run(H, *args, thr, **kw)
+    r = oracle.run(args[1], args[2], args[0], *args[3:], thr,
+                   cap_clusters=kw.get("cap_clusters"), cap_adc=kw.get("cap_adc"))
+    return g, r
+
+
+# ------------------------------------------------------------------ worked examples
+DOC = cases.load_worked_examples()
+
+
+@pytest.mark.parametrize("case", DOC["cases"], ids=[c["id"] for c in DOC["cases"]])
+def test_worked_examples(H, oracle, case):
+    cs = cases.worked_case(DOC, case)
+    g, r = both(H, oracle, cs)
+    compare(g, r)
+    assert g["n_clusters"] == len(case["clusters"])
+    for k, e in enumerate(case["clusters"]):     # and directly against the hand values
+        assert (int(g["cl_module"][k]), int(g["cl_first"][k]), int(g["cl_width"][k]),
+                int(g["cl_charge"][k])) == (e["module"], e["first"], e["width"], e["charge"])
+        assert g["cl_bary"][k] == pytest.approx(e["bary"], rel=REL)
+        assert g["cl_snr"][k] == pytest.approx(e["snr"], rel=REL)
+
+
+def test_gain_and_strip_test_tables_on_gpu(H, oracle):
+    """Every (adc, gain) of the golden gain table and the float32 boundary cases of the strip
+    tests, as single-strip clusters."""
+    rows = DOC["gain_table"]["rows"]
+    strips, gains = {}, {}
+    for i, (adc, g, want) in enumerate(rows):
+        key = f"{2 * i}:10"
+        strips[key], gains[key] = adc, g
+    cs = cases.build_case(strips, gain_over=gains, noise=0.25, module_sizes=(2,), thresholds=(1.0, 1.0, 1e-3))
+    g, r = both(H, oracle, cs)
+    compare(g, r)
+    got = [int(x) for x in g["cl_adc"]]
+    want = [w for _, _, w in rows if w > 0]
+    assert got == want
+    for adc, n, t, want in DOC["strip_test_table"]["rows"]:
+        cs = cases.build_case({"0:5": adc}, noise_over={"0:5": n}, thresholds=(t, t, 1e-3))
+        g, r = both(H, oracle, cs)
+        compare(g, r)
+        assert g["n_clusters"] == int(want)
+
+
+def test_gain_correction_exhaustive_on_gpu(H, oracle):
+    """All 256 ADC values x 96 gains in one FED (noise tiny so that every strip is a seed);
+    strips separated by gaps so each is its own cluster."""
+    rng = np.random.Generator(np.random.PCG64(5))
+    gains = np.concatenate([np.float32([0.8, 1.0, 1.2, 1.25, 2.0, 0.5]),
+                            np.clip(rng.normal(1.0, 0.05, 90), 0.8, 1.2).astype(np.float32)])
+    n_feds = 2
+    n = n_feds * synth.FED_STRIPS
+    z = np.zeros(n, np.uint8)
+    gain = np.ones(n, np.float32)
+    for c in range(96):
+        for half in range(2):
+            ch = half * 96 + c
+            vals = np.arange(128) + 128 * half
+            z[ch * 256 + 2 * np.arange(128)] = vals
+            gain[ch * 256:(ch + 1) * 256] = gains[c]
+    raw, fo = synth.encode_dense(z, n_feds)
+    noise = np.full(n, 0.125, np.float32)
+    bad = np.zeros(n, np.uint8)
+    cm = cases.module_map_from_sizes(n_feds, (2,))
+    thr = (1.0, 1.0, 1e-3)
+    g = gpu_run(H, n_feds, raw, fo, gain, noise, bad, cm, thr)
+    r = oracle.run(raw, fo, n_feds, gain, noise, bad, cm, thr)
+    compare(g, r)
+    assert g["n_clusters"] > 96 * 250
+
+
+# ------------------------------------------------------------------ hand-built raw + malformed
+def test_hand_built_and_malformed_raw(H, oracle):
+    E = synth.EMPTY_CHANNEL
+    good = synth.channel_bytes([(7, [33, 34])])
+    bodies = [bytes([250, 10]) + bytes([1] * 10), bytes([20, 1, 5, 10, 1, 6]), bytes([20, 2, 5, 6, 21, 1, 7]),
+              bytes([20, 3, 5, 6]), bytes([20, 1, 5, 9]), bytes([1, 0]) + bytes([3] * 255)]
+    chans = {0: good, 2: bytes.fromhex("0400") + bytes([254, 2, 70, 90]), 3: bytes.fromhex("0300") + bytes([255, 1, 110]),
+             4: bytes.fromhex("0700") + bytes([10, 1, 50, 11, 2, 60, 70]),
+             5: (258).to_bytes(2, "little") + bytes([0, 0]) + bytes([60] * 256),
+             6: (260).to_bytes(2, "little") + bytes([0, 255]) + bytes([90] * 255) + bytes([255, 1, 80])}
+    for i, b in enumerate(bodies):
+        chans[10 + 2 * i] = len(b).to_bytes(2, "little") + b
+        chans[11 + 2 * i] = good
+    fed0 = [chans.get(c, E) for c in range(96)]
+    over = (4000).to_bytes(2, "little") + bytes([1, 1, 9])
+    fed1 = [good, good, over] + [good] * 93
+    fed2 = [E] * 96
+    raw, fo = synth.assemble_feds([fed0, fed1, fed2, fed0])
+    n_feds = 4
+    n = n_feds * synth.FED_STRIPS
+    gain, noise, bad = np.ones(n, np.float32), np.full(n, 4.0, np.float32), np.zeros(n, np.uint8)
+    cm = cases.module_map_from_sizes(n_feds, (2, 3))
+    g = gpu_run(H, n_feds, raw, fo, gain, noise, bad, cm, (2.0, 3.0, 5.0))
+    r = oracle.run(raw, fo, n_feds, gain, noise, bad, cm, (2.0, 3.0, 5.0))
+    compare(g, r)
+    assert r.status[1] == 12 and r.status[4] == 1
+
+
+def test_bad_fed_offsets(H, oracle):
+    cfg, cal, evs = synth.make_config(0, n_feds=3)
+    ev = evs[0]
+    for mutate in ("end_lt_start", "beyond_buffer", "truncated"):
+        fo = ev.fed_offsets.copy()
+        if mutate == "end_lt_start":
+            fo[1], fo[2] = fo[2], fo[1]
+        elif mutate == "beyond_buffer":
+            fo[3] = ev.raw.size + 4096
+        else:
+            fo[2] = fo[1] + 160
+        g = gpu_run(H, 3, ev.raw, fo, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5),
+                    max_raw_bytes=int(ev.raw.size))
+        r = oracle.run(ev.raw, fo, 3, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+        compare(g, r)
+        assert r.status[4] >= 1
+
+
+def test_unaligned_fed_offsets_use_the_slow_path(H, oracle):
+    """FEDs not padded to 16 bytes: same results through the non-TMA path."""
+    cfg, cal, evs = synth.make_config(0, n_feds=2)
+    ev = evs[0]
+    _, ln, _, _ = oracle.unpack(ev.raw, ev.fed_offsets, 2)
+    used = (ln.reshape(2, 96).astype(np.int64) + 2).sum(axis=1)
+    a = ev.raw[ev.fed_offsets[0]:ev.fed_offsets[0] + used[0]]
+    b = ev.raw[ev.fed_offsets[1]:ev.fed_offsets[1] + used[1]]
+    raw = np.concatenate([a, b, np.zeros(32, np.uint8)])
+    fo = np.array([0, used[0], used[0] + used[1]], np.uint32)
+    g = gpu_run(H, 2, raw, fo, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+    r = oracle.run(raw, fo, 2, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+    compare(g, r)
+    assert np.array_equal(g["strip_adc"], ev.z)
+
+
+# ------------------------------------------------------------------ generated events
+@pytest.mark.parametrize("cid,nf", [(0, 24), (1, 37), (2, 29), (4, 41)])
+def test_generated_configs_small(H, oracle, cid, nf):
+    """Sizes the oracle finishes in well under a second: several CTAs and a ragged FED count."""
+    cfg, cal, evs = synth.make_config(cid, n_feds=nf)
+    ev = evs[0]
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
+    try:
+        for thr in cfg.thresholds:
+            g = gpu_run(H, nf, ev.raw, ev.fed_offsets, None, None, None, None, thr, det=det)
+            r = oracle.run(ev.raw, ev.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, thr)
+            compare(g, r)
+            assert np.array_equal(g["strip_adc"], ev.z)
+            assert g["n_clusters"] > 0
+    finally:
+        det.close()
+
+
+@pytest.mark.parametrize("cid", [1, 2, 4])
+def test_full_detector_configs(H, oracle, cid):
+    """BASELINE.json configs 1, 2, 4 at full size (440 FEDs), every output compared."""
+    cfg, cal, evs = synth.make_config(cid)
+    ev = evs[0]
+    det = H.Detector(cal.n_feds, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
+    try:
+        for thr in cfg.thresholds:
+            g = gpu_run(H, cal.n_feds, ev.raw, ev.fed_offsets, None, None, None, None, thr, det=det)
+            r = oracle.run(ev.raw, ev.fed_offsets, cal.n_feds, cal.gain, cal.noise, cal.bad, cal.chan_module, thr)
+            compare(g, r)
+    finally:
+        det.close()
+
+
+def test_dense_fed_takes_the_dense_flag_path(H, oracle):
+    """A FED with > 4096 present strips and a worst-case alternating pattern (max clusters)."""
+    n_feds = 2
+    n = n_feds * synth.FED_STRIPS
+    rng = np.random.Generator(np.random.PCG64(3))
+    z = np.zeros(n, np.uint8)
+    z[0:synth.FED_STRIPS:2] = 40                                    # 12288 single-strip clusters
+    z[synth.FED_STRIPS:] = rng.integers(0, 60, synth.FED_STRIPS)    # nearly full FED, long runs
+    raw, fo = synth.encode_dense(z, n_feds)
+    assert fo[1] - fo[0] > 11264                                    # also larger than the smem stage
+    gain = np.clip(rng.normal(1.0, 0.05, n), 0.8, 1.2).astype(np.float32)
+    noise = (3 + 3 * rng.random(n)).astype(np.float32)
+    bad = (rng.random(n) < 0.02).astype(np.uint8)
+    cm = cases.module_map_from_sizes(n_feds, (2, 3, 1, 5))
+    for thr in ((2, 3, 5), (1.5, 2.5, 4)):
+        g = gpu_run(H, n_feds, raw, fo, gain, noise, bad, cm, thr)
+        r = oracle.run(raw, fo, n_feds, gain, noise, bad, cm, thr)
+        compare(g, r)
+
+
+def test_wide_clusters_and_exact_equality(H, oracle):
+    strips = {f"0:{50 + i}": 12 for i in range(64)}
+    cs = cases.build_case(strips, noise=4.0)
+    for t in (24.0, float(np.nextafter(np.float32(24), np.float32(25)))):
+        g, r = both(H, oracle, cs, thresholds=(2.0, 3.0, t))
+        compare(g, r)
+    # a 3-channel module fully occupied: one 768-strip cluster; plus > 64 wide clusters in a FED
+    z = np.zeros(synth.FED_STRIPS, np.uint8)
+    z[2 * 256:5 * 256] = 60
+    for c in range(10, 90):
+        z[c * 256 + 3:c * 256 + 3 + 40 + c] = 30
+    raw, fo = synth.encode_dense(z, 1)
+    n = synth.FED_STRIPS
+    rng = np.random.Generator(np.random.PCG64(9))
+    noise = (3 + 3 * rng.random(n)).astype(np.float32)
+    gain = np.clip(rng.normal(1.0, 0.05, n), 0.8, 1.2).astype(np.float32)
+    cm = cases.module_map_from_sizes(1, (2, 3))
+    g = gpu_run(H, 1, raw, fo, gain, noise, np.zeros(n, np.uint8), cm, (2, 3, 5))
+    r = oracle.run(raw, fo, 1, gain, noise, np.zeros(n, np.uint8), cm, (2, 3, 5))
+    compare(g, r)
+    assert 768 in set(int(w) for w in g["cl_width"])
+
+
+def test_capacity_overflow(H, oracle):
+    cfg, cal, evs = synth.make_config(0)
+    ev = evs[0]
+    for cc, ca in ((100, 10 ** 6), (10 ** 6, 50), (0, 10), (2921, 6047), (2920, 6047), (2921, 6046)):
+        g = gpu_run(H, 24, ev.raw, ev.fed_offsets, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5),
+                    cap_clusters=cc, cap_adc=ca)
+        r = oracle.run(ev.raw, ev.fed_offsets, 24, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5),
+                       cap_clusters=cc, cap_adc=ca)
+        compare(g, r)
+
+
+def test_no_dense_output_and_host_entry_point(H, oracle):
+    import ctypes
+    from paper_2101_11489_b200 import binding as B
+    cfg, cal, evs = synth.make_config(0)
+    ev = evs[0]
+    r = oracle.run(ev.raw, ev.fed_offsets, 24, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+    g = gpu_run(H, 24, ev.raw, ev.fed_offsets, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5), dense=False)
+    assert "strip_adc" not in g and g["n_clusters"] == r.n_clusters
+    assert np.array_equal(g["cl_adc"], r.cl_adc)
+    # host buffers through sst_unpack_cluster_host
+    det = H.Detector(24, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
+    try:
+        cc, ca = ev.raw.size // 3 + 1, ev.raw.size
+        h = dict(n_clusters=np.zeros(1, np.uint32), dev_status=np.zeros(8, np.uint32),
+                 cl_module=np.zeros(cc, np.uint32), cl_first=np.zeros(cc, np.uint16), cl_width=np.zeros(cc, np.uint16),
+                 cl_charge=np.zeros(cc, np.int32), cl_bary=np.zeros(cc, np.float32), cl_adc_off=np.zeros(cc, np.uint32),
+                 cl_adc=np.zeros(ca, np.uint8), strip_adc=np.zeros(cal.n_strips, np.uint8),
+                 cl_snr=np.zeros(cc, np.float32), seed_idx=np.zeros(cal.n_strips, np.uint32),
+                 chan_off=np.zeros(24 * 96, np.uint32), chan_len=np.zeros(24 * 96, np.uint16))
+        out = B.make_output(cap_clusters=cc, cap_adc=ca, cap_seeds=cal.n_strips, **h)
+        B.sst_unpack_cluster_host(det.ctx, ev.raw, int(ev.raw.size), ev.fed_offsets, (2, 3, 5), out)
+        k = int(h["n_clusters"][0])
+        res = {"n_clusters": k, "status": h["dev_status"], "strip_adc": h["strip_adc"], "chan_off": h["chan_off"],
+               "chan_len": h["chan_len"], "seed_idx": h["seed_idx"][:h["dev_status"][5]],
+               "cl_adc": h["cl_adc"][:h["dev_status"][3]]}
+        for name in ("cl_module", "cl_first", "cl_width", "cl_charge", "cl_bary", "cl_adc_off", "cl_snr"):
+            res[name] = h[name][:k]
+        compare(res, r)
+    finally:
+        det.close()
+
+
+def test_error_codes(H):
+    from paper_2101_11489_b200 import binding as B
+    cfg, cal, evs = synth.make_config(0, n_feds=1)
+    ev = evs[0]
+    with pytest.raises(B.SSTError, match="BAD_CALIB"):
+        bad_gain = cal.gain.copy()
+        bad_gain[5] = 0.0
+        H.Detector(1, bad_gain, cal.noise, np.zeros_like(cal.bad), cal.chan_module)
+    with pytest.raises(B.SSTError, match="BAD_CALIB"):
+        cm = cal.chan_module.copy()
+        cm[10] = 0
+        H.Detector(1, cal.gain, cal.noise, cal.bad, cm)
+    ctx = B.sst_create(1, 0, 4096)
+    import torch
+    d = torch.zeros(4096, dtype=torch.uint8, device="cuda")
+    det = H.Detector(1, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
+    outs = det.alloc_outputs(100, 100)
+    with pytest.raises(B.SSTError, match="NO_CALIB"):
+        B.sst_unpack_cluster(ctx, d, d, (2, 3, 5), outs.out)
+    with pytest.raises(B.SSTError, match="INVALID_ARG"):
+        B.sst_unpack_cluster(det.ctx, d, d, (2, -3, 5), outs.out)
+    with pytest.raises(B.SSTError, match="INVALID_ARG"):
+        B.sst_unpack_cluster(det.ctx, d, d, (2, 3, float("nan")), outs.out)
+    B.sst_destroy(ctx)
+    det.close()
+
+
+# ------------------------------------------------------------------ multi-event / streams
+def test_multi_event_streams_match_single_event(H, oracle):
+    """Config 3 in miniature: 12 events over 1, 3 and 8 streams with pooled per-event buffers;
+    every event's output equals its single-event oracle output."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf = 24
+    cfg, cal, evs = synth.make_config(3, n_feds=nf, event_seeds=range(1, 13))
+    want = [oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            for e in evs]
+    mrb = max(int(e.raw.size) for e in evs)
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        for n_streams in (1, 3, 8):
+            streams = [torch.cuda.Stream() for _ in range(n_streams)]
+            held = []
+            for i, e in enumerate(evs):
+                st = streams[i % n_streams]
+                pin_raw = torch.from_numpy(e.raw).pin_memory()
+                pin_fo = torch.from_numpy(e.fed_offsets.view(np.int32)).pin_memory()
+                # per-event raw buffers from the library's stream-ordered pool, pinned H2D
+                p_raw, p_fo = B.sst_event_upload(det.ctx, pin_raw, e.raw.size, pin_fo, st.cuda_stream)
+                outs = det.alloc_outputs(mrb // 3 + 1, mrb, chan_map=True, seeds=True, snr=True)
+                B.sst_unpack_cluster(det.ctx, p_raw, p_fo, (2, 3, 5), outs.out, st.cuda_stream)
+                B.sst_event_free(det.ctx, p_raw, st.cuda_stream)
+                B.sst_event_free(det.ctx, p_fo, st.cuda_stream)
+                held.append((outs, pin_raw, pin_fo))
+            torch.cuda.synchronize()
+            for (outs, _, _), r in zip(held, want):
+                compare(H.unsigned_view(outs.numpy()), r)
+    finally:
+        det.close()
