@@ -1,25 +1,29 @@
 // sst.cu -- libsst: unpack + three-threshold clustering of strip-tracker FED data on B200.
 //
 // One fused kernel per event, one CTA per FED (a FED is 96 channels x 256 strips;
-// modules never cross a FED, reading s10), so every step of the path
-// runs on data resident in shared memory:
+// modules never cross a FED, reading s10).  After the unpack everything runs in the
+// COMPACT index space of the FED's present strips (the structure of arrays of PAPER.md:31 has
+// one entry per recorded strip), kept in shared memory:
 //
-//   a1 channel-location map : TMA bulk copy of the whole FED payload to smem, 96-step length
-//                             chain walked in smem (PAPER.md:31 builds this map on the CPU)
-//   a2 unpack               : one thread per channel walks its runs and scatters ADC bytes into
-//                             a dense 96x256 smem tile; the tile leaves with one TMA bulk store
-//   a3 flags                : compact list of present strips -> one gather of {noise, gain}
-//                             per present strip -> active / seed bit masks (exact >= tests)
-//   a4 seed-index array     : the seed mask + block scan; materialised on request
-//   a5 expansion/ownership  : per seed, bit scans left/right over the active mask inside the
-//                             module; only the leftmost seed of a run goes on
+//   a1 channel-location map : TMA bulk copy of the FED payload to smem, 96-step length chain
+//                             walked in smem (PAPER.md:31 builds this map on the CPU)
+//   a2 unpack               : thread per channel; pass 1 walks the run headers (validate, count),
+//                             a 96-wide scan gives every channel its slot range, pass 2 streams
+//                             the payload bytes into {strip, adc} lists in ascending strip order
+//                             and scatters the ADCs into the zero-filled dense output
+//   a3 flags                : lane per present strip: one 8-byte gather of {noise, gain},
+//                             exact >= tests, masks built with __ballot_sync (no atomics)
+//   a4 seed-index array     : seed mask + block scan; materialised on request
+//   a5 expansion/ownership  : lane per seed: bit scans over a "linked to the previous entry"
+//                             mask; only the leftmost seed of a run goes on
 //   a6 gain corr + accept   : q = min(254, floor(adc/gain + .5)) in float32, Q^2 >= t^2 * sum n^2
-//   a7 ordered output       : block scan + decoupled look-back over per-FED aggregates, records
-//                             written in (module, first strip) order
+//   a7 ordered output       : block scan + look-back over per-FED aggregates, lane per cluster
 //
-// No tensor cores: nothing here is a contraction.  See DESIGN.md for layout and rooflines.
+// FEDs whose payload or strip count exceed the smem budgets use the same code on slices of a
+// pooled global scratch buffer.  No tensor cores: nothing here is a contraction.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdint>
@@ -37,30 +41,34 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kChan = 96;
 constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
-constexpr int kWords = kFedStrips / 32;     // 768 mask words per FED
-constexpr int kRawCap = 11264;              // FED payloads up to this size are staged in smem
-constexpr int kListCap = 4096;              // present-strip list; larger FEDs use the dense path
+constexpr int kListCap = 4096;              // present strips per FED kept in smem
+constexpr int kRawCap = 4 * kListCap;       // FED payload staged in smem (region reused for noise)
+constexpr int kMaskWords = kListCap / 32 + 1;
 constexpr int kWide = 32;                   // clusters wider than this are summed by a warp
-constexpr int kWideQ = 64;
+constexpr int kWideQ = 32;
 
 // per-FED aggregate published for the look-back (one 64-bit word)
 constexpr int kShAdc = 14, kShSeed = 29, kShMalf = 44, kShOvr = 51;
 constexpr unsigned long long kReady = 1ull << 63;
 
 struct __align__(128) Smem {
-    uint8_t tile[kFedStrips];  // dense ADC of the FED; gain-corrected in place at active strips
-    uint8_t raw[kRawCap];      // FED payload (TMA destination)
-    uint32_t act[kWords], seed[kWords], acc[kWords];
-    uint16_t list[kListCap];
+    union {                       // payload is dead once the lists are built
+        uint8_t raw[kRawCap];     // FED payload (TMA destination)
+        float noise[kListCap];    // noise of entry i          (flags .. accept)
+        uint32_t cl[kListCap];    // accepted clusters: entry | adc offset << 16   (emit)
+    } u;
+    uint16_t strip[kListCap];     // FED-local strip id of entry i, ascending
+    uint8_t adc[kListCap];        // raw ADC, replaced by the corrected ADC at active entries
+    uint32_t act[kMaskWords], seed[kMaskWords], brk[kMaskWords], link[kMaskWords], acc[kMaskWords];
     uint32_t mod_id[kChan];
-    uint32_t chan_off[kChan];  // FED-local byte offset of the first run byte
+    uint32_t chan_off[kChan];     // FED-local byte offset of the first run byte
     uint16_t chan_len[kChan];
     uint8_t mod_lo[kChan], mod_hi[kChan];  // first channel / end channel of the channel's module
     uint32_t wscan[2][kWarps];
     uint32_t red[5][kWarps];
     uint32_t wide_q[kWideQ];
     unsigned long long mbar;
-    uint32_t list_count, wide_count;
+    uint32_t wide_count, n_present;
     uint32_t fed_start, fed_size, in_smem, overrun;
 };
 
@@ -70,10 +78,17 @@ struct KParams {
     const float2 *calib;  // {noise (+inf at bad strips), gain} per strip
     const uint32_t *chan_module;
     unsigned long long *fed_state;
+    // global scratch for FEDs that do not fit the smem lists (sliced by FED offset)
+    uint16_t *g_strip;
+    uint8_t *g_adc;
+    float *g_noise;
+    uint32_t *g_mask;      // 5 arrays of g_mask_words
+    uint32_t g_mask_words;
     double tcl2;
     float t_ch, t_seed;
     uint32_t max_raw_bytes, n_feds;
     sst_output out;
+    unsigned long long *phase_clk;  // debug builds only (SST_PHASE_TIMING)
 };
 
 // ------------------------------------------------------------------------------ PTX helpers
@@ -113,16 +128,6 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         "l"(src), "r"(bytes), "r"(smem_addr(bar))
         : "memory");
 }
-// TMA bulk copy shared -> global
-__device__ __forceinline__ void bulk_s2g(void *dst, const void *src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst),
-                 "r"(smem_addr(src)), "r"(bytes)
-                 : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_wait_read() {
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-}
 __device__ __forceinline__ unsigned long long ld_state(const unsigned long long *p) {
     unsigned long long v;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
@@ -158,36 +163,26 @@ __device__ __forceinline__ double warp_sum_d(double v) {
     return v;
 }
 
-// last strip of the maximal active run that starts at (or contains) strip s, bounded by the
-// module end `me` (exclusive, a multiple of 256)
-__device__ __forceinline__ int right_end(const uint32_t *act, int s, int me) {
-    int w = s >> 5;
-    const int b = s & 31;
-    uint32_t inact = ~act[w] & (b == 31 ? 0u : (0xffffffffu << (b + 1)));
-    while (true) {
-        if (inact) return (w << 5) + __ffs(inact) - 2;
-        if (((w + 1) << 5) >= me) return me - 1;
-        ++w;
-        inact = ~act[w];
-    }
+// Entry i is "linked" when it continues the cluster candidate of entry i-1 (both active, strips
+// adjacent inside one module).  The last entry of the run that contains entry i: one before the
+// next unlinked entry.  link[] has a zero sentinel word after the last used word.
+__device__ __forceinline__ int run_end(const uint32_t *link, int i) {
+    int w = i >> 5;
+    const int b = i & 31;
+    uint32_t nl = ~link[w] & (b == 31 ? 0u : (0xffffffffu << (b + 1)));
+    while (nl == 0) nl = ~link[++w];
+    return (w << 5) + __ffs(nl) - 2;
 }
 
 // Cluster acceptance for a narrow candidate, one thread: Q^2 >= t_cl^2 * n2 with n2 the double
 // sum of noise^2 taken strictly left to right (reading s15).
-__device__ __forceinline__ bool accept_serial(const uint8_t *tile, const float *noise2f, int l, int w,
-                                              double tcl2) {
+__device__ __forceinline__ bool accept_serial(const uint8_t *q, const float *noise, int l, int w, double tcl2) {
     int Q = 0;
     double n2 = 0.0;
-    for (int i0 = 0; i0 < w; i0 += 4) {
-        float nv[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) nv[j] = (i0 + j < w) ? __ldg(noise2f + 2 * (l + i0 + j)) : 0.0f;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            if (i0 + j < w) Q += tile[l + i0 + j];
-            const double d = static_cast<double>(nv[j]);
-            n2 = __dadd_rn(n2, __dmul_rn(d, d));  // + 0.0 for padding lanes is exact
-        }
+    for (int i = 0; i < w; ++i) {
+        Q += q[l + i];
+        const double d = static_cast<double>(noise[l + i]);
+        n2 = __dadd_rn(n2, __dmul_rn(d, d));
     }
     const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
     return lhs >= __dmul_rn(tcl2, n2);
@@ -196,13 +191,13 @@ __device__ __forceinline__ bool accept_serial(const uint8_t *tile, const float *
 // The same decision for a wide candidate by one warp.  A pairwise double sum differs from the
 // sequential one by at most ~w*2^-52 relative; the decision is taken from it only when the two
 // sides are further apart than that, otherwise lane 0 redoes the sum sequentially.
-__device__ __noinline__ bool accept_warp(const uint8_t *tile, const float *noise2f, int l, int w,
-                                         double tcl2, int lane) {
+__device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, int l, int w, double tcl2,
+                                         int lane) {
     uint32_t Q = 0;
     double n2p = 0.0;
     for (int i = lane; i < w; i += 32) {
-        Q += tile[l + i];
-        const double d = static_cast<double>(__ldg(noise2f + 2 * (l + i)));
+        Q += q[l + i];
+        const double d = static_cast<double>(noise[l + i]);
         n2p += d * d;
     }
     Q = warp_sum(Q);
@@ -214,7 +209,7 @@ __device__ __noinline__ bool accept_warp(const uint8_t *tile, const float *noise
         if (lane == 0) {
             double n2 = 0.0;
             for (int i = 0; i < w; ++i) {
-                const double d = static_cast<double>(__ldg(noise2f + 2 * (l + i)));
+                const double d = static_cast<double>(noise[l + i]);
                 n2 = __dadd_rn(n2, __dmul_rn(d, d));
             }
             ok = lhs >= __dmul_rn(tcl2, n2);
@@ -224,14 +219,90 @@ __device__ __noinline__ bool accept_warp(const uint8_t *tile, const float *noise
     return ok != 0;
 }
 
+
+// ------------------------------------------------------------------------------ raw payload
+// The three loops that read the raw bytes.  They are instantiated twice: on the smem stage (the
+// compiler then emits LDS) and on the generic global pointer (oversized or unaligned FEDs).
+
+// a1: the channel-length chain of one FED.  Returns true if the chain overran the FED.
+__device__ __forceinline__ bool walk_chain(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
+                                           uint16_t *chan_len) {
+    uint32_t pos = 0;
+    int c = 0;
+    if (!over) {
+        for (; c < kChan; ++c) {
+            if (pos + 2 > fed_size) break;
+            const uint32_t l16 = rp[pos] | (static_cast<uint32_t>(rp[pos + 1]) << 8);
+            if (pos + 2 + l16 > fed_size) break;
+            chan_off[c] = pos + 2;
+            chan_len[c] = static_cast<uint16_t>(l16);
+            pos += 2 + l16;
+        }
+    }
+    over = c < kChan;
+    for (; c < kChan; ++c) {  // channels behind an overrun are empty, recorded at the FED end
+        chan_off[c] = fed_size;
+        chan_len[c] = 0;
+    }
+    return over;
+}
+
+// a2 pass 1: validate one channel's run list (reading s2b) and count its runs.
+__device__ __forceinline__ bool scan_runs(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t &n_runs) {
+    uint32_t q = off, next_free = 0;
+    const uint32_t qend = off + len_bytes;
+    n_runs = 0;
+    while (q < qend) {
+        if (q + 2 > qend) return false;
+        const uint32_t first = rp[q];
+        uint32_t len = rp[q + 1];
+        if (len == 0) len = 256;  // reading s2
+        if (first < next_free || first + len > kStrip || q + 2 + len > qend) return false;
+        next_free = first + len;
+        q += 2 + len;
+        ++n_runs;
+    }
+    return true;
+}
+
+// a2 pass 2: stream one (validated) channel: every ADC byte becomes a list entry {strip, adc}
+// and is scattered into the zero-filled dense output.
+__device__ __forceinline__ void stream_channel(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t k,
+                                               int chan, uint16_t *strip_l, uint8_t *adc_l, uint8_t *dense) {
+    uint32_t rem = 0, tgt = 0, hdr = 0;
+    const uint32_t qend = off + len_bytes;
+    for (uint32_t q = off; q < qend; ++q) {
+        const uint32_t b = rp[q];
+        if (rem) {
+            strip_l[k] = static_cast<uint16_t>(chan * kStrip + tgt);
+            adc_l[k] = static_cast<uint8_t>(b);
+            if (dense) dense[tgt] = static_cast<uint8_t>(b);
+            ++k; ++tgt; --rem;
+        } else if (!hdr) {
+            tgt = b;
+            hdr = 1;
+        } else {
+            rem = b ? b : 256u;
+            hdr = 0;
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------ the kernel
-__global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_constant__ KParams p) {
+#ifdef SST_PHASE_TIMING
+#define SST_MARK(k) do { if (tid == 0 && p.phase_clk) p.phase_clk[f * 16 + (k)] = clock64(); } while (0)
+#else
+#define SST_MARK(k) do { } while (0)
+#endif
+
+__global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_constant__ KParams p) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     Smem &s = *reinterpret_cast<Smem *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t f = blockIdx.x;
     const sst_output &o = p.out;
 
+    SST_MARK(0);
     // ---------------------------------------------------------------- a1: stage the FED payload
     if (tid == 0) {
         mbar_init(&s.mbar, 1);
@@ -245,22 +316,25 @@ __global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_const
         s.fed_size = size;
         s.in_smem = in_smem;
         s.overrun = valid ? 0u : 1u;
-        s.list_count = 0;
         s.wide_count = 0;
         if (in_smem && size) {
             mbar_expect_tx(&s.mbar, size);
-            bulk_g2s(s.raw, p.raw + fo0, size, &s.mbar);
+            bulk_g2s(s.u.raw, p.raw + fo0, size, &s.mbar);
         }
     }
-    // meanwhile: clear the tile and the masks, fetch the module ids of the 96 channels
-    {
-        uint4 *t4 = reinterpret_cast<uint4 *>(s.tile);
-        const uint4 z = make_uint4(0, 0, 0, 0);
-        for (int i = tid; i < kFedStrips / 16; i += kThreads) t4[i] = z;
-        uint4 *m4 = reinterpret_cast<uint4 *>(s.act);
-        for (int i = tid; i < 3 * kWords / 4; i += kThreads) m4[i] = z;
-        if (tid < kChan) s.mod_id[tid] = p.chan_module[f * kChan + tid];
+    // meanwhile: zero-fill this FED's slice of the dense output, fetch the module ids
+    if (o.strip_adc) {
+        uint8_t *dst = o.strip_adc + static_cast<size_t>(f) * kFedStrips;
+        if ((reinterpret_cast<uintptr_t>(o.strip_adc) & 15u) == 0) {
+            uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+            const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+            for (int i = 0; i < kFedStrips / 16 / kThreads; ++i) d4[tid + i * kThreads] = z;
+        } else {
+            for (int i = tid; i < kFedStrips; i += kThreads) dst[i] = 0;
+        }
     }
+    if (tid < kChan) s.mod_id[tid] = p.chan_module[f * kChan + tid];
     __syncthreads();
     if (tid < kChan) {  // module extent of every channel (modules are runs of equal ids)
         const uint32_t m = s.mod_id[tid];
@@ -272,231 +346,194 @@ __global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_const
     }
     const bool in_smem = s.in_smem != 0;
     const uint32_t fed_size = s.fed_size;
-    const uint8_t *rp = in_smem ? s.raw : p.raw + s.fed_start;
+    const uint8_t *rp = in_smem ? s.u.raw : p.raw + s.fed_start;
 
+    SST_MARK(1);
     // ---------------------------------------------------------------- a1: walk the length chain
     if (tid == 0) {
         if (in_smem && fed_size) mbar_wait(&s.mbar, 0);
-        uint32_t pos = 0;
-        bool over = s.overrun != 0;
-        for (int c = 0; c < kChan; ++c) {
-            uint32_t off = fed_size, L = 0;
-            if (!over) {
-                if (pos + 2 > fed_size) {
-                    over = true;
-                } else {
-                    const uint32_t l16 = rp[pos] | (static_cast<uint32_t>(rp[pos + 1]) << 8);
-                    if (pos + 2 + l16 > fed_size) {
-                        over = true;
-                    } else {
-                        off = pos + 2;
-                        L = l16;
-                        pos = off + L;
-                    }
-                }
-            }
-            s.chan_off[c] = off;
-            s.chan_len[c] = static_cast<uint16_t>(L);
-        }
+        SST_MARK(2);
+        const bool over = in_smem ? walk_chain(s.u.raw, fed_size, s.overrun != 0, s.chan_off, s.chan_len)
+                                  : walk_chain(rp, fed_size, s.overrun != 0, s.chan_off, s.chan_len);
         s.overrun = over ? 1u : 0u;
     }
     __syncthreads();
 
-    // ---------------------------------------------------------------- a2: unpack, thread per channel
+    SST_MARK(3);
+    // ---------------------------------------------------------------- a2 pass 1: run headers
+    // thread per channel: validate the run list, count the recorded strips
     int malformed = 0;
+    uint32_t my_cnt = 0, my_off = 0, my_len = 0;
     if (tid < kChan) {
         if (in_smem && fed_size) mbar_wait(&s.mbar, 0);  // async-proxy writes visible to this thread
-        const uint32_t off = s.chan_off[tid], L = s.chan_len[tid];
-        if (o.chan_off) o.chan_off[f * kChan + tid] = s.fed_start + off;
-        if (o.chan_len) o.chan_len[f * kChan + tid] = static_cast<uint16_t>(L);
-        uint8_t *row = s.tile + tid * kStrip;
-        uint32_t q = off, next_free = 0;
-        const uint32_t qend = off + L;
-        bool ok = true;
-        while (q < qend) {
-            if (q + 2 > qend) { ok = false; break; }
-            const uint32_t first = rp[q];
-            uint32_t len = rp[q + 1];
-            if (len == 0) len = 256;
-            if (first < next_free || first + len > kStrip || q + 2 + len > qend) { ok = false; break; }
-            const uint32_t lpos = atomicAdd(&s.list_count, len);
-            for (uint32_t i = 0; i < len; ++i) {
-                row[first + i] = rp[q + 2 + i];
-                if (lpos + i < kListCap) s.list[lpos + i] = static_cast<uint16_t>(tid * kStrip + first + i);
-            }
-            next_free = first + len;
-            q += 2 + len;
-        }
-        if (!ok) {  // a malformed channel contributes no strips (stale list entries see adc = 0)
-            uint32_t *r32 = reinterpret_cast<uint32_t *>(row);
-            for (int i = 0; i < kStrip / 4; ++i) r32[i] = 0;
-            malformed = 1;
-        }
-    }
-    fence_proxy_async();  // tile writes -> visible to the TMA store below
-    const uint32_t n_malformed = __syncthreads_count(malformed);
-
-    // ---------------------------------------------------------------- a2: dense tile leaves
-    bool store_pending = false;
-    if (o.strip_adc) {
-        uint8_t *dst = o.strip_adc + static_cast<size_t>(f) * kFedStrips;
-        if ((reinterpret_cast<uintptr_t>(o.strip_adc) & 15u) == 0) {
-            if (tid == 0) bulk_s2g(dst, s.tile, kFedStrips);
-            store_pending = true;
+        my_off = s.chan_off[tid];
+        my_len = s.chan_len[tid];
+        if (o.chan_off) o.chan_off[f * kChan + tid] = s.fed_start + my_off;
+        if (o.chan_len) o.chan_len[f * kChan + tid] = static_cast<uint16_t>(my_len);
+        uint32_t n_runs = 0;
+        const bool ok = in_smem ? scan_runs(s.u.raw, my_off, my_len, n_runs) : scan_runs(rp, my_off, my_len, n_runs);
+        if (ok) {
+            my_cnt = my_len - 2 * n_runs;
         } else {
-            for (int i = tid; i < kFedStrips; i += kThreads) dst[i] = s.tile[i];
-            __syncthreads();
+            malformed = 1;  // a malformed channel contributes no strips
+            my_len = 0;
         }
     }
+    // exclusive scan of the 96 counts (warps 0..2)
+    uint32_t inc = my_cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += u;
+    }
+    if (lane == 31 && warp < 3) s.wscan[0][warp] = inc;
+    const uint32_t n_malformed = __syncthreads_count(malformed);
+    uint32_t my_base = inc - my_cnt;
+    if (warp >= 1) my_base += s.wscan[0][0];
+    if (warp >= 2) my_base += s.wscan[0][1];
+    const uint32_t P = s.wscan[0][0] + s.wscan[0][1] + s.wscan[0][2];  // present strips of the FED
+    const uint32_t nw = (P + 31) >> 5;                                  // mask words in use
 
+    // list storage: smem if it fits, else this FED's slice of the pooled global scratch
+    const bool lists_smem = P <= static_cast<uint32_t>(kListCap);
+    const uint32_t slice = ((s.fed_start + 15u) & ~15u) + 16u * f;
+    uint16_t *strip_l = lists_smem ? s.strip : p.g_strip + slice;
+    uint8_t *adc_l = lists_smem ? s.adc : p.g_adc + slice;
+    float *noise_l = lists_smem ? s.u.noise : p.g_noise + slice;
+    uint32_t *cl_l = lists_smem ? s.u.cl : reinterpret_cast<uint32_t *>(p.g_noise + slice);
+    uint32_t *m_act, *m_seed, *m_brk, *m_link, *m_acc;
+    if (lists_smem) {
+        m_act = s.act; m_seed = s.seed; m_brk = s.brk; m_link = s.link; m_acc = s.acc;
+    } else {
+        uint32_t *mb = p.g_mask + (slice >> 5) + 2u * f;
+        m_act = mb; m_seed = mb + p.g_mask_words; m_brk = mb + 2 * p.g_mask_words;
+        m_link = mb + 3 * p.g_mask_words; m_acc = mb + 4 * p.g_mask_words;
+    }
+
+    SST_MARK(4);
+    // ---------------------------------------------------------------- a2 pass 2: stream the bytes
+    if (tid < kChan && my_len) {
+        uint8_t *dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips + tid * kStrip : nullptr;
+        if (in_smem) stream_channel(s.u.raw, my_off, my_len, my_base, tid, strip_l, adc_l, dense);
+        else stream_channel(rp, my_off, my_len, my_base, tid, strip_l, adc_l, dense);
+    }
+    __syncthreads();  // lists complete; the payload (smem union) is dead from here on
+
+    SST_MARK(5);
     // ---------------------------------------------------------------- a3: active / seed flags
+    // lane per entry; a warp covers one mask word per step, so the masks come from ballots
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
-    const float *noise2f = reinterpret_cast<const float *>(cal);
-    const uint32_t n_list = s.list_count;
-    bool first_batch = true;
-    if (n_list <= static_cast<uint32_t>(kListCap)) {
-        for (uint32_t base = 0; base < n_list || first_batch; base += kThreads * 4) {
-            uint32_t sidx[4], a[4];
-            float2 cv[4];
+    for (uint32_t base = 0; base < nw * 32; base += kThreads * 2) {
+        uint32_t idx[2], sv[2], av[2], sp[2];
+        float2 cv[2];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t i = base + j * kThreads + tid;
-                sidx[j] = i < n_list ? s.list[i] : 0u;
-                a[j] = i < n_list ? s.tile[sidx[j]] : 0u;
-            }
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (a[j]) cv[j] = __ldg(cal + sidx[j]);
-            if (first_batch) {  // the TMA store must have read the tile before it is modified
-                if (store_pending && tid == 0) bulk_wait_read();
-                __syncthreads();
-                first_batch = false;
-            }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if (a[j]) {
-                    const float af = static_cast<float>(a[j]);
-                    if (ge_exact(af, p.t_ch, cv[j].x)) {
-                        const uint32_t bit = 1u << (sidx[j] & 31);
-                        atomicOr(&s.act[sidx[j] >> 5], bit);
-                        if (ge_exact(af, p.t_seed, cv[j].x)) atomicOr(&s.seed[sidx[j] >> 5], bit);
-                        s.tile[sidx[j]] = static_cast<uint8_t>(gain_correct(a[j], cv[j].y));
-                    }
-                }
-            }
+        for (int j = 0; j < 2; ++j) {
+            idx[j] = base + j * kThreads + tid;
+            const bool valid = idx[j] < P;
+            sv[j] = valid ? strip_l[idx[j]] : 0u;
+            av[j] = valid ? adc_l[idx[j]] : 0u;
+            sp[j] = (valid && idx[j] > 0) ? strip_l[idx[j] - 1] : 0xffffu;
         }
-    } else {  // dense path: every strip slot is visited, 8 predicated gathers in flight per thread
-        uint32_t *t32 = reinterpret_cast<uint32_t *>(s.tile);
-        for (int k = 0; k < kFedStrips / 4 / kThreads; k += 2) {
-            uint32_t wv[2];
-            float2 cv[8];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) wv[h] = t32[tid + (k + h) * kThreads];
+        for (int j = 0; j < 2; ++j) cv[j] = av[j] ? __ldg(cal + sv[j]) : make_float2(INFINITY, 1.0f);
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if ((wv[h] >> (8 * j)) & 0xffu) cv[h * 4 + j] = __ldg(cal + 4 * (tid + (k + h) * kThreads) + j);
-            if (first_batch) {
-                if (store_pending && tid == 0) bulk_wait_read();
-                __syncthreads();
-                first_batch = false;
+        for (int j = 0; j < 2; ++j) {
+            if ((base + j * kThreads + warp * 32) >= nw * 32) continue;  // warp-uniform
+            const float af = static_cast<float>(av[j]);
+            const bool is_act = av[j] != 0 && ge_exact(af, p.t_ch, cv[j].x);
+            const bool is_seed = is_act && ge_exact(af, p.t_seed, cv[j].x);
+            const uint32_t ch = sv[j] >> 8;
+            // a new candidate must start here if the previous entry is not the strip to the left
+            // or this strip opens a module
+            const bool is_brk = sv[j] != sp[j] + 1u || ((sv[j] & 255u) == 0 && s.mod_lo[ch] == ch);
+            if (idx[j] < P) {
+                noise_l[idx[j]] = cv[j].x;
+                if (is_act) adc_l[idx[j]] = static_cast<uint8_t>(gain_correct(av[j], cv[j].y));
             }
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int wi = tid + (k + h) * kThreads;  // tile word = strips 4*wi .. 4*wi+3
-                uint32_t am = 0, sm = 0, nw = wv[h];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const uint32_t a = (wv[h] >> (8 * j)) & 0xffu;
-                    if (a) {
-                        const float af = static_cast<float>(a);
-                        const float2 c = cv[h * 4 + j];
-                        if (ge_exact(af, p.t_ch, c.x)) {
-                            am |= 1u << j;
-                            if (ge_exact(af, p.t_seed, c.x)) sm |= 1u << j;
-                            nw = (nw & ~(0xffu << (8 * j))) | (gain_correct(a, c.y) << (8 * j));
-                        }
-                    }
-                }
-                if (am) {
-                    t32[wi] = nw;
-                    atomicOr(&s.act[wi >> 3], am << ((wi & 7) * 4));
-                    if (sm) atomicOr(&s.seed[wi >> 3], sm << ((wi & 7) * 4));
-                }
+            const uint32_t wa = __ballot_sync(0xffffffffu, is_act);
+            const uint32_t ws = __ballot_sync(0xffffffffu, is_seed);
+            const uint32_t wb = __ballot_sync(0xffffffffu, is_brk);
+            if (lane == 0) {
+                const uint32_t w = idx[j] >> 5;
+                m_act[w] = wa; m_seed[w] = ws; m_brk[w] = wb;
             }
         }
     }
     __syncthreads();
-
-    // ---------------------------------------------------------------- a5 + a6: per seed
-    for (int k = 0; k < kWords / kThreads; ++k) {
-        const int w = tid + k * kThreads;
-        uint32_t sbits = s.seed[w];
-        while (sbits) {
-            const int b = __ffs(sbits) - 1;
-            sbits &= sbits - 1;
-            const int sstrip = (w << 5) + b;
-            const int ch = sstrip >> 8;
-            const int ms = s.mod_lo[ch] * kStrip, me = s.mod_hi[ch] * kStrip;
-            // left: nearest inactive strip or nearest seed, whichever comes first
-            int ww = w, l;
-            uint32_t below = (1u << b) - 1u;
-            bool owner = true;
-            while (true) {
-                const uint32_t inact = ~s.act[ww] & below;
-                const uint32_t sd = s.seed[ww] & below;
-                if (inact) {
-                    const int hi = 31 - __clz(inact);
-                    if (sd >> hi > 1u) owner = false;  // a seed between the gap and this seed
-                    l = (ww << 5) + hi + 1;
-                    break;
-                }
-                if (sd) { owner = false; break; }
-                if ((ww << 5) <= ms) { l = ms; break; }
-                --ww;
-                below = 0xffffffffu;
-            }
-            if (!owner) continue;  // leftmost-seed ownership: another seed emits this cluster
-            const int r = right_end(s.act, sstrip, me);
-            const int wd = r - l + 1;
-            if (wd > kWide) {
-                const uint32_t slot = atomicAdd(&s.wide_count, 1u);
-                if (slot < kWideQ) {
-                    s.wide_q[slot] = static_cast<uint32_t>(l) | (static_cast<uint32_t>(wd) << 16);
-                    continue;
-                }
-            }
-            if (accept_serial(s.tile, noise2f, l, wd, p.tcl2)) atomicOr(&s.acc[l >> 5], 1u << (l & 31));
+    for (uint32_t w = tid; w <= nw; w += kThreads) {  // link mask (+ zero sentinel word), clear acc
+        uint32_t lk = 0;
+        if (w < nw) {
+            const uint32_t a = m_act[w];
+            const uint32_t carry = w ? (m_act[w - 1] >> 31) : 0u;
+            lk = a & ((a << 1) | carry) & ~m_brk[w];
+        } else {
+            m_seed[w] = 0;
         }
+        m_link[w] = lk;
+        m_acc[w] = 0;
+    }
+    __syncthreads();
+
+    SST_MARK(6);
+    // ---------------------------------------------------------------- a5 + a6: lane per seed
+    for (uint32_t i = tid; i < nw * 32; i += kThreads) {
+        const int w = i >> 5, b = i & 31;
+        const uint32_t sw = m_seed[w];
+        if (!((sw >> b) & 1u)) continue;
+        // left: the run starts at the nearest unlinked entry at or below i; a seed in between owns it
+        int ww = w;
+        uint32_t nl = ~m_link[w] & (0xffffffffu >> (31 - b));
+        uint32_t sd = sw & ((1u << b) - 1u);
+        bool owner = true;
+        while (nl == 0) {  // entry 0 is never linked, so this ends
+            if (sd) { owner = false; break; }
+            --ww;
+            nl = ~m_link[ww];
+            sd = m_seed[ww];
+        }
+        if (!owner) continue;
+        const int hb = 31 - __clz(nl);
+        if (sd >> hb) continue;  // leftmost-seed ownership: another seed emits this cluster
+        const int l = (ww << 5) + hb;
+        const int wd = run_end(m_link, i) - l + 1;
+        if (wd > kWide) {
+            const uint32_t slot = atomicAdd(&s.wide_count, 1u);
+            if (slot < kWideQ) {
+                s.wide_q[slot] = static_cast<uint32_t>(l) | (static_cast<uint32_t>(wd) << 16);
+                continue;
+            }
+        }
+        if (accept_serial(adc_l, noise_l, l, wd, p.tcl2)) atomicOr(&m_acc[l >> 5], 1u << (l & 31));
     }
     __syncthreads();
     {
         const uint32_t nq = min(s.wide_count, static_cast<uint32_t>(kWideQ));
         for (uint32_t e = warp; e < nq; e += kWarps) {
             const int l = s.wide_q[e] & 0xffffu, wd = s.wide_q[e] >> 16;
-            if (accept_warp(s.tile, noise2f, l, wd, p.tcl2, lane) && lane == 0)
-                atomicOr(&s.acc[l >> 5], 1u << (l & 31));
+            if (accept_warp(adc_l, noise_l, l, wd, p.tcl2, lane) && lane == 0)
+                atomicOr(&m_acc[l >> 5], 1u << (l & 31));
         }
     }
     __syncthreads();
 
+    SST_MARK(7);
     // ---------------------------------------------------------------- a7: local scan
-    // thread t owns mask words 3t .. 3t+2 (96 consecutive strips)
+    // thread t owns mask words 3t .. 3t+2; noise is dead, its space takes the cluster list
     uint32_t my_cl = 0, my_adc = 0, my_seed = 0;
-#pragma unroll
+#pragma unroll 1
     for (int k = 0; k < 3; ++k) {
-        const int w = 3 * tid + k;
-        uint32_t m = s.acc[w];
+        const uint32_t w = 3 * tid + k;
+        if (w >= nw) break;
+        uint32_t m = m_acc[w];
         my_cl += __popc(m);
-        my_seed += __popc(s.seed[w]);
+        my_seed += __popc(m_seed[w]);
         while (m) {
             const int l = (w << 5) + __ffs(m) - 1;
             m &= m - 1;
-            my_adc += right_end(s.act, l, s.mod_hi[l >> 8] * kStrip) - l + 1;
+            my_adc += run_end(m_link, l) - l + 1;
         }
     }
-    uint32_t inc_a = my_cl | (my_adc << 16), inc_s = my_seed;  // my_cl <= 48, my_adc <= 96 per thread
+    uint32_t inc_a = my_cl | (my_adc << 16), inc_s = my_seed;  // FED totals <= 12288 / 24576
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
         const uint32_t ua = __shfl_up_sync(0xffffffffu, inc_a, d);
@@ -512,14 +549,12 @@ __global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_const
         tot_a += s.wscan[0][i];
         tot_s += s.wscan[1][i];
     }
-    // CTA totals: clusters <= 12288 and ADC bytes <= 24576 keep the packed halves apart
     const uint32_t fed_cl = tot_a & 0xffffu, fed_adc = tot_a >> 16, fed_seed = tot_s;
-    uint32_t ex_cl = (pre_a + inc_a - (my_cl | (my_adc << 16))) & 0xffffu;
-    uint32_t ex_adc = (pre_a + inc_a - (my_cl | (my_adc << 16))) >> 16;
-    uint32_t ex_seed = pre_s + inc_s - my_seed;
+    const uint32_t ex_a = pre_a + inc_a - (my_cl | (my_adc << 16));
+    uint32_t ex_cl = ex_a & 0xffffu, ex_adc = ex_a >> 16, ex_seed = pre_s + inc_s - my_seed;
     const uint32_t fed_over = s.overrun;
 
-    // ---------------------------------------------------------------- a7: decoupled look-back
+    // publish the aggregate as early as possible
     if (tid == 0) {
         const unsigned long long agg = kReady | fed_cl | (static_cast<unsigned long long>(fed_adc) << kShAdc) |
                                        (static_cast<unsigned long long>(fed_seed) << kShSeed) |
@@ -527,11 +562,30 @@ __global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_const
                                        (static_cast<unsigned long long>(fed_over) << kShOvr);
         st_state(p.fed_state + f, agg);
     }
+    // ordered list of the accepted clusters (entry | FED-local adc offset << 16); the per-word
+    // seed prefix goes where brk was
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) {
+        const uint32_t w = 3 * tid + k;
+        if (w >= nw) break;
+        m_brk[w] = ex_seed;
+        ex_seed += __popc(m_seed[w]);
+        uint32_t m = m_acc[w];
+        while (m) {
+            const int l = (w << 5) + __ffs(m) - 1;
+            m &= m - 1;
+            cl_l[ex_cl++] = static_cast<uint32_t>(l) | (ex_adc << 16);
+            ex_adc += run_end(m_link, l) - l + 1;
+        }
+    }
+
+    SST_MARK(8);
+    // ---------------------------------------------------------------- a7: look-back
     uint32_t b_cl = 0, b_adc = 0, b_seed = 0, b_malf = 0, b_over = 0;
     for (uint32_t j = tid; j < f; j += kThreads) {
         unsigned long long v = ld_state(p.fed_state + j);
         while (!(v & kReady)) {
-            __nanosleep(40);
+            __nanosleep(100);
             v = ld_state(p.fed_state + j);
         }
         b_cl += static_cast<uint32_t>(v) & 0x3fffu;
@@ -546,7 +600,7 @@ __global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_const
         s.red[0][warp] = b_cl; s.red[1][warp] = b_adc; s.red[2][warp] = b_seed;
         s.red[3][warp] = b_malf; s.red[4][warp] = b_over;
     }
-    __syncthreads();
+    __syncthreads();  // also orders the cluster list and the seed prefixes
     b_cl = b_adc = b_seed = b_malf = b_over = 0;
 #pragma unroll
     for (int i = 0; i < kWarps; ++i) {
@@ -554,59 +608,52 @@ __global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_const
         b_malf += s.red[3][i]; b_over += s.red[4][i];
     }
 
+    SST_MARK(9);
     // ---------------------------------------------------------------- a7: emit, (module, first strip) order
-    uint32_t k_cl = b_cl + ex_cl, k_adc = b_adc + ex_adc, k_seed = b_seed + ex_seed;
-#pragma unroll 1
-    for (int k = 0; k < 3; ++k) {
-        const int w = 3 * tid + k;
-        if (o.seed_idx) {
-            uint32_t sb = s.seed[w];
-            while (sb) {
-                const int b = __ffs(sb) - 1;
-                sb &= sb - 1;
-                if (k_seed < o.cap_seeds) o.seed_idx[k_seed] = f * kFedStrips + (w << 5) + b;
-                ++k_seed;
+    if (o.seed_idx) {
+        for (uint32_t i = tid; i < nw * 32; i += kThreads) {
+            const uint32_t w = i >> 5, b = i & 31, sw = m_seed[w];
+            if ((sw >> b) & 1u) {
+                const uint32_t k = b_seed + m_brk[w] + __popc(sw & ((1u << b) - 1u));
+                if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + strip_l[i];
             }
         }
-        uint32_t m = s.acc[w];
-        while (m) {
-            const int l = (w << 5) + __ffs(m) - 1;
-            m &= m - 1;
-            const int ch = l >> 8;
-            const int wd = right_end(s.act, l, s.mod_hi[ch] * kStrip) - l + 1;
-            const bool fits = k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc;
-            if (fits) {
-                int Q = 0;
-                long long M = 0;
-                for (int i = 0; i < wd; ++i) {
-                    const int q = s.tile[l + i];
-                    Q += q;
-                    M += static_cast<long long>(i) * q;
-                    o.cl_adc[k_adc + i] = static_cast<uint8_t>(q);
-                }
-                const int first = l - s.mod_lo[ch] * kStrip;
-                o.cl_module[k_cl] = s.mod_id[ch];
-                o.cl_first[k_cl] = static_cast<uint16_t>(first);
-                o.cl_width[k_cl] = static_cast<uint16_t>(wd);
-                o.cl_charge[k_cl] = Q;
-                o.cl_bary[k_cl] = static_cast<float>(static_cast<double>(first) +
-                                                      static_cast<double>(M) / static_cast<double>(Q));
-                o.cl_adc_off[k_cl] = k_adc;
-                if (o.cl_snr) {
-                    double n2 = 0.0;
-                    for (int i = 0; i < wd; ++i) {
-                        const double d = static_cast<double>(__ldg(noise2f + 2 * (l + i)));
-                        n2 = __dadd_rn(n2, __dmul_rn(d, d));
-                    }
-                    o.cl_snr[k_cl] = static_cast<float>(static_cast<double>(Q) / sqrt(n2));
-                }
-            } else {
-                // the first cluster that does not fit reports how many were written
-                const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
-                if (prev_fits) *o.n_clusters = k_cl;
+    }
+    for (uint32_t c = tid; c < fed_cl; c += kThreads) {  // lane per accepted cluster
+        const uint32_t e = cl_l[c];
+        const int l = e & 0xffffu;
+        const uint32_t k_cl = b_cl + c, k_adc = b_adc + (e >> 16);
+        const int wd = run_end(m_link, l) - l + 1;
+        if (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc) {
+            int Q = 0;
+            long long M = 0;
+            for (int i = 0; i < wd; ++i) {
+                const int q = adc_l[l + i];
+                Q += q;
+                M += static_cast<long long>(i) * q;
+                o.cl_adc[k_adc + i] = static_cast<uint8_t>(q);
             }
-            ++k_cl;
-            k_adc += wd;
+            const uint32_t st0 = strip_l[l], ch = st0 >> 8;
+            const int first = static_cast<int>(st0) - s.mod_lo[ch] * kStrip;
+            o.cl_module[k_cl] = s.mod_id[ch];
+            o.cl_first[k_cl] = static_cast<uint16_t>(first);
+            o.cl_width[k_cl] = static_cast<uint16_t>(wd);
+            o.cl_charge[k_cl] = Q;
+            o.cl_bary[k_cl] =
+                static_cast<float>(static_cast<double>(first) + static_cast<double>(M) / static_cast<double>(Q));
+            o.cl_adc_off[k_cl] = k_adc;
+            if (o.cl_snr) {  // noise list is gone by now: re-gather (optional output, tests only)
+                double n2 = 0.0;
+                for (int i = 0; i < wd; ++i) {
+                    const double d = static_cast<double>(__ldg(&cal[st0 + i].x));
+                    n2 = __dadd_rn(n2, __dmul_rn(d, d));
+                }
+                o.cl_snr[k_cl] = static_cast<float>(static_cast<double>(Q) / sqrt(n2));
+            }
+        } else {
+            // the first cluster that does not fit reports how many were written
+            const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
+            if (prev_fits) *o.n_clusters = k_cl;
         }
     }
     if (f == p.n_feds - 1 && tid == 0) {  // event totals = prefix of the last FED + its own
@@ -627,10 +674,11 @@ __global__ void __launch_bounds__(kThreads, 4) sst_fed_kernel(const __grid_const
         o.dev_status[6] = 0;
         o.dev_status[7] = 0;
     }
-    // smem must stay valid until the bulk store has read it (covered above whenever it was issued)
+    SST_MARK(10);
 }
 
 }  // namespace
+
 
 // ====================================================================================== host
 struct sst_ctx {
@@ -666,34 +714,55 @@ bool output_ok(const sst_output *o) {
            o->cl_charge && o->cl_bary && o->cl_adc_off && o->cl_adc;
 }
 
+#ifdef SST_PHASE_TIMING
+unsigned long long *g_phase_clk = nullptr;
+#endif
+
 sst_status launch_event(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
                         const sst_thresholds *thr, const sst_output *out, cudaStream_t st) {
     const uint32_t nf = ctx->cfg.n_feds;
-    unsigned long long *state = nullptr;
-    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&state), sizeof(unsigned long long) * nf,
-                                   ctx->pool, st));
-    SST_CU(cudaMemsetAsync(state, 0, sizeof(unsigned long long) * nf, st));
+    // one pooled block: look-back states (zeroed) + list/mask scratch for FEDs that overflow smem
+    const size_t ents = static_cast<size_t>(ctx->cfg.max_raw_bytes) + 16ull * nf + 64;
+    const size_t mwords = ents / 32 + 2ull * nf + 16;
+    auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
+    const size_t o_state = 0, o_noise = up(sizeof(unsigned long long) * nf), o_mask = o_noise + up(4 * ents),
+                 o_strip = o_mask + up(4 * 5 * mwords), o_adc = o_strip + up(2 * ents), total = o_adc + up(ents);
+    uint8_t *blk = nullptr;
+    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), total, ctx->pool, st));
+    SST_CU(cudaMemsetAsync(blk + o_state, 0, sizeof(unsigned long long) * nf, st));
     KParams kp{};
     kp.raw = raw;
     kp.fed_offsets = fed_offsets;
     kp.calib = ctx->calib;
     kp.chan_module = ctx->chan_module;
-    kp.fed_state = state;
+    kp.fed_state = reinterpret_cast<unsigned long long *>(blk + o_state);
+    kp.g_noise = reinterpret_cast<float *>(blk + o_noise);
+    kp.g_mask = reinterpret_cast<uint32_t *>(blk + o_mask);
+    kp.g_mask_words = static_cast<uint32_t>(mwords);
+    kp.g_strip = reinterpret_cast<uint16_t *>(blk + o_strip);
+    kp.g_adc = blk + o_adc;
     kp.tcl2 = static_cast<double>(thr->cluster) * static_cast<double>(thr->cluster);  // exact
     kp.t_ch = thr->channel;
     kp.t_seed = thr->seed;
     kp.max_raw_bytes = ctx->cfg.max_raw_bytes;
     kp.n_feds = nf;
     kp.out = *out;
+#ifdef SST_PHASE_TIMING
+    kp.phase_clk = g_phase_clk;
+#endif
     sst_fed_kernel<<<nf, kThreads, sizeof(Smem), st>>>(kp);
     SST_CU(cudaGetLastError());
-    SST_CU(cudaFreeAsync(state, st));
+    SST_CU(cudaFreeAsync(blk, st));
     return SST_OK;
 }
 
 }  // namespace
 
 extern "C" {
+
+#ifdef SST_PHASE_TIMING
+void sst_debug_set_phase_clk(unsigned long long *p) { g_phase_clk = p; }
+#endif
 
 sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (out_ctx) *out_ctx = nullptr;
