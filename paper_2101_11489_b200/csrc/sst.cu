@@ -44,45 +44,53 @@ constexpr int kFedStrips = kChan * kStrip;  // 24576
 constexpr int kListCap = 4096;              // present strips per FED kept in smem
 constexpr int kRawCap = 4 * kListCap;       // FED payload staged in smem (region reused for noise)
 constexpr int kMaskWords = kListCap / 32 + 1;
+constexpr int kRunCap = 2048;               // run-table slots (FED payloads up to ~6 KB)
+constexpr int kInline = 8;                  // runs up to this length are copied by one thread
+constexpr int kLongQ = 96;
 constexpr int kWide = 32;                   // clusters wider than this are summed by a warp
 constexpr int kWideQ = 32;
+enum { M_ACT = 0, M_SEED, M_BRK, M_LINK, M_ACC, M_WTOT, M_COUNT };
 
 // per-FED aggregate published for the look-back (one 64-bit word)
 constexpr int kShAdc = 14, kShSeed = 29, kShMalf = 44, kShOvr = 51;
 constexpr unsigned long long kReady = 1ull << 63;
 
 struct __align__(128) Smem {
-    union {                       // payload is dead once the lists are built
+    union {                       // the payload is dead once the lists are built
         uint8_t raw[kRawCap];     // FED payload (TMA destination)
-        float noise[kListCap];    // noise of entry i          (flags .. accept)
-        uint32_t cl[kListCap];    // accepted clusters: entry | adc offset << 16   (emit)
+        float noise[kListCap];    // noise of entry i
     } u;
     uint16_t strip[kListCap];     // FED-local strip id of entry i, ascending
     uint8_t adc[kListCap];        // raw ADC, replaced by the corrected ADC at active entries
-    uint32_t act[kMaskWords], seed[kMaskWords], brk[kMaskWords], link[kMaskWords], acc[kMaskWords];
+    uint32_t mask[M_COUNT][kMaskWords];
+    alignas(16) uint32_t runs[kRunCap];  // one record per run, slot = (runs of earlier channels' bound) + ordinal
     uint32_t mod_id[kChan];
     uint32_t chan_off[kChan];     // FED-local byte offset of the first run byte
     uint16_t chan_len[kChan];
+    uint16_t chan_base[kChan];    // first list entry of the channel
+    uint16_t slot_base[kChan + 1];
     uint8_t mod_lo[kChan], mod_hi[kChan];  // first channel / end channel of the channel's module
+    uint32_t okmask[3];
     uint32_t wscan[2][kWarps];
     uint32_t red[5][kWarps];
     uint32_t wide_q[kWideQ];
+    uint16_t long_q[kLongQ];
     unsigned long long mbar;
-    uint32_t wide_count, n_present;
+    uint32_t wide_count, long_count;
     uint32_t fed_start, fed_size, in_smem, overrun;
 };
 
 struct KParams {
     const uint8_t *raw;
     const uint32_t *fed_offsets;
-    const float2 *calib;  // {noise (+inf at bad strips), gain} per strip
-    const uint32_t *chan_module;
+    const float2 *calib;     // {noise (+inf at bad strips), gain} per strip
+    const uint2 *chan_info;  // {module id, first channel | end channel << 8 of the module}
     unsigned long long *fed_state;
     // global scratch for FEDs that do not fit the smem lists (sliced by FED offset)
     uint16_t *g_strip;
     uint8_t *g_adc;
     float *g_noise;
-    uint32_t *g_mask;      // 5 arrays of g_mask_words
+    uint32_t *g_mask;  // M_COUNT arrays of g_mask_words
     uint32_t g_mask_words;
     double tcl2;
     float t_ch, t_seed;
@@ -219,15 +227,14 @@ __device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, i
     return ok != 0;
 }
 
-
 // ------------------------------------------------------------------------------ raw payload
-// The three loops that read the raw bytes.  They are instantiated twice: on the smem stage (the
-// compiler then emits LDS) and on the generic global pointer (oversized or unaligned FEDs).
+// Loops that read the raw bytes are instantiated on the smem stage (LDS) and on the generic
+// global pointer (oversized or unaligned FEDs).
 
-// a1: the channel-length chain of one FED.  Returns true if the chain overran the FED.
-__device__ __forceinline__ bool walk_chain(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
-                                           uint16_t *chan_len) {
-    uint32_t pos = 0;
+// a1: the channel-length chain of one FED, checked as it goes (generic path).
+__device__ __forceinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
+                                                   uint16_t *chan_len, uint16_t *slot_base) {
+    uint32_t pos = 0, slots = 0;
     int c = 0;
     if (!over) {
         for (; c < kChan; ++c) {
@@ -236,6 +243,8 @@ __device__ __forceinline__ bool walk_chain(const uint8_t *rp, uint32_t fed_size,
             if (pos + 2 + l16 > fed_size) break;
             chan_off[c] = pos + 2;
             chan_len[c] = static_cast<uint16_t>(l16);
+            slot_base[c] = static_cast<uint16_t>(min(slots, 0xffffu));
+            slots += l16 / 3;
             pos += 2 + l16;
         }
     }
@@ -243,30 +252,56 @@ __device__ __forceinline__ bool walk_chain(const uint8_t *rp, uint32_t fed_size,
     for (; c < kChan; ++c) {  // channels behind an overrun are empty, recorded at the FED end
         chan_off[c] = fed_size;
         chan_len[c] = 0;
+        slot_base[c] = static_cast<uint16_t>(min(slots, 0xffffu));
     }
+    slot_base[kChan] = static_cast<uint16_t>(min(slots, 0xffffu));
     return over;
 }
 
-// a2 pass 1: validate one channel's run list (reading s2b) and count its runs.
-__device__ __forceinline__ bool scan_runs(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t &n_runs) {
-    uint32_t q = off, next_free = 0;
+// a1, smem stage: the same chain walked speculatively -- no bounds checks inside the serial
+// loop (addresses wrap inside the stage), the 96 results are validated in parallel afterwards.
+__device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uint32_t *chan_off, uint16_t *chan_len,
+                                                       uint16_t *slot_base) {
+    uint32_t pos = 0, slots = 0;
+#pragma unroll 4
+    for (int c = 0; c < kChan; ++c) {
+        const uint32_t a = pos & (kRawCap - 1);
+        const uint32_t l16 = stage[a] | (static_cast<uint32_t>(stage[(a + 1) & (kRawCap - 1)]) << 8);
+        chan_off[c] = pos + 2;
+        chan_len[c] = static_cast<uint16_t>(l16);
+        slot_base[c] = static_cast<uint16_t>(min(slots, 0xffffu));
+        slots += l16 / 3;
+        pos += 2 + l16;
+    }
+    slot_base[kChan] = static_cast<uint16_t>(min(slots, 0xffffu));
+}
+
+// a2 pass 1: validate one channel's run list (reading s2b), count its strips and, when
+// the run table is in use, leave one record per run: strips before | first << 8 | (len-1) << 16
+// | channel << 24 | valid << 31.  Returns false for a malformed channel.
+__device__ __forceinline__ bool scan_runs(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t chan,
+                                          uint32_t *slots, uint32_t &n_runs, uint32_t &n_strips) {
+    uint32_t q = off, next_free = 0, k = 0, within = 0;
     const uint32_t qend = off + len_bytes;
-    n_runs = 0;
+    bool ok = true;
     while (q < qend) {
-        if (q + 2 > qend) return false;
+        if (q + 2 > qend) { ok = false; break; }
         const uint32_t first = rp[q];
         uint32_t len = rp[q + 1];
         if (len == 0) len = 256;  // reading s2
-        if (first < next_free || first + len > kStrip || q + 2 + len > qend) return false;
+        if (first < next_free || first + len > kStrip || q + 2 + len > qend) { ok = false; break; }
+        if (slots) slots[k] = within | (first << 8) | ((len - 1) << 16) | (chan << 24) | 0x80000000u;
         next_free = first + len;
         q += 2 + len;
-        ++n_runs;
+        within += len;
+        ++k;
     }
-    return true;
+    n_runs = k;
+    n_strips = within;
+    return ok;
 }
 
-// a2 pass 2: stream one (validated) channel: every ADC byte becomes a list entry {strip, adc}
-// and is scattered into the zero-filled dense output.
+// a2 pass 2, fallback without the run table: stream one (validated) channel byte by byte.
 __device__ __forceinline__ void stream_channel(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t k,
                                                int chan, uint16_t *strip_l, uint8_t *adc_l, uint8_t *dense) {
     uint32_t rem = 0, tgt = 0, hdr = 0;
@@ -276,7 +311,7 @@ __device__ __forceinline__ void stream_channel(const uint8_t *rp, uint32_t off, 
         if (rem) {
             strip_l[k] = static_cast<uint16_t>(chan * kStrip + tgt);
             adc_l[k] = static_cast<uint8_t>(b);
-            if (dense) dense[tgt] = static_cast<uint8_t>(b);
+            if (dense) dense[chan * kStrip + tgt] = static_cast<uint8_t>(b);
             ++k; ++tgt; --rem;
         } else if (!hdr) {
             tgt = b;
@@ -288,134 +323,70 @@ __device__ __forceinline__ void stream_channel(const uint8_t *rp, uint32_t off, 
     }
 }
 
-// ------------------------------------------------------------------------------ the kernel
 #ifdef SST_PHASE_TIMING
-#define SST_MARK(k) do { if (tid == 0 && p.phase_clk) p.phase_clk[f * 16 + (k)] = clock64(); } while (0)
+#define SST_MARK(k) do { if (threadIdx.x == 0 && p.phase_clk) p.phase_clk[blockIdx.x * 16 + (k)] = clock64(); } while (0)
 #else
 #define SST_MARK(k) do { } while (0)
 #endif
 
-__global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_constant__ KParams p) {
-    extern __shared__ __align__(128) uint8_t smem_raw[];
-    Smem &s = *reinterpret_cast<Smem *>(smem_raw);
+// ------------------------------------------------------------------------------ lists -> clusters
+// Everything after the channel walk, on the FED's lists of present strips.  kSmem = true: lists
+// and masks in shared memory (LDS/STS); false: in this FED's slice of the global scratch.
+template <bool kSmem>
+__device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, const uint8_t *rp, const uint32_t P,
+                                                  const bool table_ok, const uint32_t n_slots,
+                                                  const uint32_t n_malformed, const uint32_t my_off,
+                                                  const uint32_t my_len, const uint32_t my_base) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t f = blockIdx.x;
     const sst_output &o = p.out;
-
-    SST_MARK(0);
-    // ---------------------------------------------------------------- a1: stage the FED payload
-    if (tid == 0) {
-        mbar_init(&s.mbar, 1);
-        fence_proxy_async();
-        const uint32_t fo0 = p.fed_offsets[f], fo1 = p.fed_offsets[f + 1];
-        const bool valid = fo0 <= fo1 && fo1 <= p.max_raw_bytes;
-        const uint32_t size = valid ? fo1 - fo0 : 0u;
-        const bool in_smem = size <= static_cast<uint32_t>(kRawCap) && ((fo0 | size) & 15u) == 0 &&
-                             (reinterpret_cast<uintptr_t>(p.raw) & 15u) == 0;
-        s.fed_start = fo0;
-        s.fed_size = size;
-        s.in_smem = in_smem;
-        s.overrun = valid ? 0u : 1u;
-        s.wide_count = 0;
-        if (in_smem && size) {
-            mbar_expect_tx(&s.mbar, size);
-            bulk_g2s(s.u.raw, p.raw + fo0, size, &s.mbar);
-        }
-    }
-    // meanwhile: zero-fill this FED's slice of the dense output, fetch the module ids
-    if (o.strip_adc) {
-        uint8_t *dst = o.strip_adc + static_cast<size_t>(f) * kFedStrips;
-        if ((reinterpret_cast<uintptr_t>(o.strip_adc) & 15u) == 0) {
-            uint4 *d4 = reinterpret_cast<uint4 *>(dst);
-            const uint4 z = make_uint4(0, 0, 0, 0);
-#pragma unroll
-            for (int i = 0; i < kFedStrips / 16 / kThreads; ++i) d4[tid + i * kThreads] = z;
-        } else {
-            for (int i = tid; i < kFedStrips; i += kThreads) dst[i] = 0;
-        }
-    }
-    if (tid < kChan) s.mod_id[tid] = p.chan_module[f * kChan + tid];
-    __syncthreads();
-    if (tid < kChan) {  // module extent of every channel (modules are runs of equal ids)
-        const uint32_t m = s.mod_id[tid];
-        int lo = tid, hi = tid + 1;
-        while (lo > 0 && s.mod_id[lo - 1] == m) --lo;
-        while (hi < kChan && s.mod_id[hi] == m) ++hi;
-        s.mod_lo[tid] = static_cast<uint8_t>(lo);
-        s.mod_hi[tid] = static_cast<uint8_t>(hi);
-    }
-    const bool in_smem = s.in_smem != 0;
-    const uint32_t fed_size = s.fed_size;
-    const uint8_t *rp = in_smem ? s.u.raw : p.raw + s.fed_start;
-
-    SST_MARK(1);
-    // ---------------------------------------------------------------- a1: walk the length chain
-    if (tid == 0) {
-        if (in_smem && fed_size) mbar_wait(&s.mbar, 0);
-        SST_MARK(2);
-        const bool over = in_smem ? walk_chain(s.u.raw, fed_size, s.overrun != 0, s.chan_off, s.chan_len)
-                                  : walk_chain(rp, fed_size, s.overrun != 0, s.chan_off, s.chan_len);
-        s.overrun = over ? 1u : 0u;
-    }
-    __syncthreads();
-
-    SST_MARK(3);
-    // ---------------------------------------------------------------- a2 pass 1: run headers
-    // thread per channel: validate the run list, count the recorded strips
-    int malformed = 0;
-    uint32_t my_cnt = 0, my_off = 0, my_len = 0;
-    if (tid < kChan) {
-        if (in_smem && fed_size) mbar_wait(&s.mbar, 0);  // async-proxy writes visible to this thread
-        my_off = s.chan_off[tid];
-        my_len = s.chan_len[tid];
-        if (o.chan_off) o.chan_off[f * kChan + tid] = s.fed_start + my_off;
-        if (o.chan_len) o.chan_len[f * kChan + tid] = static_cast<uint16_t>(my_len);
-        uint32_t n_runs = 0;
-        const bool ok = in_smem ? scan_runs(s.u.raw, my_off, my_len, n_runs) : scan_runs(rp, my_off, my_len, n_runs);
-        if (ok) {
-            my_cnt = my_len - 2 * n_runs;
-        } else {
-            malformed = 1;  // a malformed channel contributes no strips
-            my_len = 0;
-        }
-    }
-    // exclusive scan of the 96 counts (warps 0..2)
-    uint32_t inc = my_cnt;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t u = __shfl_up_sync(0xffffffffu, inc, d);
-        if (lane >= d) inc += u;
-    }
-    if (lane == 31 && warp < 3) s.wscan[0][warp] = inc;
-    const uint32_t n_malformed = __syncthreads_count(malformed);
-    uint32_t my_base = inc - my_cnt;
-    if (warp >= 1) my_base += s.wscan[0][0];
-    if (warp >= 2) my_base += s.wscan[0][1];
-    const uint32_t P = s.wscan[0][0] + s.wscan[0][1] + s.wscan[0][2];  // present strips of the FED
-    const uint32_t nw = (P + 31) >> 5;                                  // mask words in use
-
-    // list storage: smem if it fits, else this FED's slice of the pooled global scratch
-    const bool lists_smem = P <= static_cast<uint32_t>(kListCap);
+    const uint32_t nw = (P + 31) >> 5;  // mask words in use
     const uint32_t slice = ((s.fed_start + 15u) & ~15u) + 16u * f;
-    uint16_t *strip_l = lists_smem ? s.strip : p.g_strip + slice;
-    uint8_t *adc_l = lists_smem ? s.adc : p.g_adc + slice;
-    float *noise_l = lists_smem ? s.u.noise : p.g_noise + slice;
-    uint32_t *cl_l = lists_smem ? s.u.cl : reinterpret_cast<uint32_t *>(p.g_noise + slice);
-    uint32_t *m_act, *m_seed, *m_brk, *m_link, *m_acc;
-    if (lists_smem) {
-        m_act = s.act; m_seed = s.seed; m_brk = s.brk; m_link = s.link; m_acc = s.acc;
-    } else {
-        uint32_t *mb = p.g_mask + (slice >> 5) + 2u * f;
-        m_act = mb; m_seed = mb + p.g_mask_words; m_brk = mb + 2 * p.g_mask_words;
-        m_link = mb + 3 * p.g_mask_words; m_acc = mb + 4 * p.g_mask_words;
-    }
+    uint16_t *const strip_l = kSmem ? s.strip : p.g_strip + slice;
+    uint8_t *const adc_l = kSmem ? s.adc : p.g_adc + slice;
+    float *const noise_l = kSmem ? s.u.noise : p.g_noise + slice;
+    uint32_t *const mbase = kSmem ? &s.mask[0][0] : p.g_mask + (slice >> 5) + 2u * f;
+    const uint32_t mstride = kSmem ? static_cast<uint32_t>(kMaskWords) : p.g_mask_words;
+#define MASK(k) (mbase + (k) * mstride)
+    uint8_t *const dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips : nullptr;
 
-    SST_MARK(4);
-    // ---------------------------------------------------------------- a2 pass 2: stream the bytes
-    if (tid < kChan && my_len) {
-        uint8_t *dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips + tid * kStrip : nullptr;
-        if (in_smem) stream_channel(s.u.raw, my_off, my_len, my_base, tid, strip_l, adc_l, dense);
-        else stream_channel(rp, my_off, my_len, my_base, tid, strip_l, adc_l, dense);
+    // ---------------------------------------------------------------- a2 pass 2: thread per run
+    if (table_ok) {
+        for (uint32_t slot = tid; slot < n_slots; slot += kThreads) {
+            const uint32_t rec = s.runs[slot];
+            if (!(rec >> 31)) continue;
+            const uint32_t c = (rec >> 24) & 127u, within = rec & 255u, first = (rec >> 8) & 255u,
+                           len = ((rec >> 16) & 255u) + 1u;
+            if (len > kInline) {
+                const uint32_t qi = atomicAdd(&s.long_count, 1u);
+                if (qi < kLongQ) { s.long_q[qi] = static_cast<uint16_t>(slot); continue; }
+            }
+            const uint32_t src = s.chan_off[c] + within + 2u * (slot - s.slot_base[c] + 1u);
+            const uint32_t dst = s.chan_base[c] + within, g = c * kStrip + first;
+            for (uint32_t i = 0; i < len; ++i) {
+                const uint8_t b = rp[src + i];
+                strip_l[dst + i] = static_cast<uint16_t>(g + i);
+                adc_l[dst + i] = b;
+                if (dense) dense[g + i] = b;
+            }
+        }
+        __syncthreads();
+        const uint32_t nq = min(s.long_count, static_cast<uint32_t>(kLongQ));
+        for (uint32_t e = warp; e < nq; e += kWarps) {  // long runs: one warp each, lane per byte
+            const uint32_t slot = s.long_q[e], rec = s.runs[slot];
+            const uint32_t c = (rec >> 24) & 127u, within = rec & 255u, first = (rec >> 8) & 255u,
+                           len = ((rec >> 16) & 255u) + 1u;
+            const uint32_t src = s.chan_off[c] + within + 2u * (slot - s.slot_base[c] + 1u);
+            const uint32_t dst = s.chan_base[c] + within, g = c * kStrip + first;
+            for (uint32_t i = lane; i < len; i += 32) {
+                const uint8_t b = rp[src + i];
+                strip_l[dst + i] = static_cast<uint16_t>(g + i);
+                adc_l[dst + i] = b;
+                if (dense) dense[g + i] = b;
+            }
+        }
+    } else if (tid < kChan && my_len) {
+        stream_channel(rp, my_off, my_len, my_base, tid, strip_l, adc_l, dense);
     }
     __syncthreads();  // lists complete; the payload (smem union) is dead from here on
 
@@ -455,7 +426,7 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
             const uint32_t wb = __ballot_sync(0xffffffffu, is_brk);
             if (lane == 0) {
                 const uint32_t w = idx[j] >> 5;
-                m_act[w] = wa; m_seed[w] = ws; m_brk[w] = wb;
+                MASK(M_ACT)[w] = wa; MASK(M_SEED)[w] = ws; MASK(M_BRK)[w] = wb;
             }
         }
     }
@@ -463,19 +434,22 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
     for (uint32_t w = tid; w <= nw; w += kThreads) {  // link mask (+ zero sentinel word), clear acc
         uint32_t lk = 0;
         if (w < nw) {
-            const uint32_t a = m_act[w];
-            const uint32_t carry = w ? (m_act[w - 1] >> 31) : 0u;
-            lk = a & ((a << 1) | carry) & ~m_brk[w];
+            const uint32_t a = MASK(M_ACT)[w];
+            const uint32_t carry = w ? (MASK(M_ACT)[w - 1] >> 31) : 0u;
+            lk = a & ((a << 1) | carry) & ~MASK(M_BRK)[w];
         } else {
-            m_seed[w] = 0;
+            MASK(M_SEED)[w] = 0;
         }
-        m_link[w] = lk;
-        m_acc[w] = 0;
+        MASK(M_LINK)[w] = lk;
+        MASK(M_ACC)[w] = 0;
     }
     __syncthreads();
 
     SST_MARK(6);
     // ---------------------------------------------------------------- a5 + a6: lane per seed
+    const uint32_t *const m_link = MASK(M_LINK);
+    const uint32_t *const m_seed = MASK(M_SEED);
+    uint32_t *const m_acc = MASK(M_ACC);
     for (uint32_t i = tid; i < nw * 32; i += kThreads) {
         const int w = i >> 5, b = i & 31;
         const uint32_t sw = m_seed[w];
@@ -513,27 +487,32 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
             if (accept_warp(adc_l, noise_l, l, wd, p.tcl2, lane) && lane == 0)
                 atomicOr(&m_acc[l >> 5], 1u << (l & 31));
         }
+        if (nq) __syncthreads();
     }
-    __syncthreads();
 
     SST_MARK(7);
     // ---------------------------------------------------------------- a7: local scan
-    // thread t owns mask words 3t .. 3t+2; noise is dead, its space takes the cluster list
-    uint32_t my_cl = 0, my_adc = 0, my_seed = 0;
-#pragma unroll 1
+    // per mask word (warp per word): accepted clusters and their ADC bytes
+    uint32_t *const m_wtot = MASK(M_WTOT);
+    uint32_t *const m_spre = MASK(M_BRK);  // brk is dead: per-word seed prefix goes here
+    for (uint32_t w = warp; w < nw; w += kWarps) {
+        const uint32_t aw = m_acc[w];
+        uint32_t wsum = 0;
+        if (aw) {  // warp-uniform
+            const int i = (w << 5) + lane;
+            wsum = warp_sum(((aw >> lane) & 1u) ? static_cast<uint32_t>(run_end(m_link, i) - i + 1) : 0u);
+        }
+        if (lane == 0) m_wtot[w] = __popc(aw) | (wsum << 16);
+    }
+    __syncthreads();
+    // thread t owns words 3t .. 3t+2: block-wide exclusive scan of the word totals
+    uint32_t my_a = 0, my_s = 0;
+#pragma unroll
     for (int k = 0; k < 3; ++k) {
         const uint32_t w = 3 * tid + k;
-        if (w >= nw) break;
-        uint32_t m = m_acc[w];
-        my_cl += __popc(m);
-        my_seed += __popc(m_seed[w]);
-        while (m) {
-            const int l = (w << 5) + __ffs(m) - 1;
-            m &= m - 1;
-            my_adc += run_end(m_link, l) - l + 1;
-        }
+        if (w < nw) { my_a += m_wtot[w]; my_s += __popc(m_seed[w]); }
     }
-    uint32_t inc_a = my_cl | (my_adc << 16), inc_s = my_seed;  // FED totals <= 12288 / 24576
+    uint32_t inc_a = my_a, inc_s = my_s;  // FED totals <= 12288 clusters / 24576 ADC bytes: halves stay apart
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
         const uint32_t ua = __shfl_up_sync(0xffffffffu, inc_a, d);
@@ -550,32 +529,26 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
         tot_s += s.wscan[1][i];
     }
     const uint32_t fed_cl = tot_a & 0xffffu, fed_adc = tot_a >> 16, fed_seed = tot_s;
-    const uint32_t ex_a = pre_a + inc_a - (my_cl | (my_adc << 16));
-    uint32_t ex_cl = ex_a & 0xffffu, ex_adc = ex_a >> 16, ex_seed = pre_s + inc_s - my_seed;
     const uint32_t fed_over = s.overrun;
-
-    // publish the aggregate as early as possible
-    if (tid == 0) {
+    if (tid == 0) {  // publish the aggregate as early as possible
         const unsigned long long agg = kReady | fed_cl | (static_cast<unsigned long long>(fed_adc) << kShAdc) |
                                        (static_cast<unsigned long long>(fed_seed) << kShSeed) |
                                        (static_cast<unsigned long long>(n_malformed) << kShMalf) |
                                        (static_cast<unsigned long long>(fed_over) << kShOvr);
         st_state(p.fed_state + f, agg);
     }
-    // ordered list of the accepted clusters (entry | FED-local adc offset << 16); the per-word
-    // seed prefix goes where brk was
-#pragma unroll 1
-    for (int k = 0; k < 3; ++k) {
-        const uint32_t w = 3 * tid + k;
-        if (w >= nw) break;
-        m_brk[w] = ex_seed;
-        ex_seed += __popc(m_seed[w]);
-        uint32_t m = m_acc[w];
-        while (m) {
-            const int l = (w << 5) + __ffs(m) - 1;
-            m &= m - 1;
-            cl_l[ex_cl++] = static_cast<uint32_t>(l) | (ex_adc << 16);
-            ex_adc += run_end(m_link, l) - l + 1;
+    {
+        uint32_t ex_a = pre_a + inc_a - my_a, ex_s = pre_s + inc_s - my_s;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const uint32_t w = 3 * tid + k;
+            if (w < nw) {
+                const uint32_t t = m_wtot[w];
+                m_wtot[w] = ex_a;
+                m_spre[w] = ex_s;
+                ex_a += t;
+                ex_s += __popc(m_seed[w]);
+            }
         }
     }
 
@@ -600,7 +573,7 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
         s.red[0][warp] = b_cl; s.red[1][warp] = b_adc; s.red[2][warp] = b_seed;
         s.red[3][warp] = b_malf; s.red[4][warp] = b_over;
     }
-    __syncthreads();  // also orders the cluster list and the seed prefixes
+    __syncthreads();  // also orders the per-word prefixes
     b_cl = b_adc = b_seed = b_malf = b_over = 0;
 #pragma unroll
     for (int i = 0; i < kWarps; ++i) {
@@ -610,30 +583,39 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
 
     SST_MARK(9);
     // ---------------------------------------------------------------- a7: emit, (module, first strip) order
-    if (o.seed_idx) {
-        for (uint32_t i = tid; i < nw * 32; i += kThreads) {
-            const uint32_t w = i >> 5, b = i & 31, sw = m_seed[w];
-            if ((sw >> b) & 1u) {
-                const uint32_t k = b_seed + m_brk[w] + __popc(sw & ((1u << b) - 1u));
-                if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + strip_l[i];
-            }
+    // warp per mask word, lane per entry: cluster index and ADC offset come from the word
+    // prefix plus a scan inside the word
+    for (uint32_t w = warp; w < nw; w += kWarps) {
+        const uint32_t aw = m_acc[w], sw = m_seed[w];
+        const int i = (w << 5) + lane;
+        const uint32_t lt = (1u << lane) - 1u;
+        if (o.seed_idx && ((sw >> lane) & 1u)) {
+            const uint32_t k = b_seed + m_spre[w] + __popc(sw & lt);
+            if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + strip_l[i];
         }
-    }
-    for (uint32_t c = tid; c < fed_cl; c += kThreads) {  // lane per accepted cluster
-        const uint32_t e = cl_l[c];
-        const int l = e & 0xffffu;
-        const uint32_t k_cl = b_cl + c, k_adc = b_adc + (e >> 16);
-        const int wd = run_end(m_link, l) - l + 1;
+        if (!aw) continue;  // warp-uniform
+        const bool mine = (aw >> lane) & 1u;
+        const int wd = mine ? run_end(m_link, i) - i + 1 : 0;
+        uint32_t incw = wd;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, incw, d);
+            if (lane >= d) incw += u;
+        }
+        if (!mine) continue;
+        const uint32_t pre = m_wtot[w];
+        const uint32_t k_cl = b_cl + (pre & 0xffffu) + __popc(aw & lt);
+        const uint32_t k_adc = b_adc + (pre >> 16) + (incw - wd);
         if (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc) {
             int Q = 0;
             long long M = 0;
-            for (int i = 0; i < wd; ++i) {
-                const int q = adc_l[l + i];
+            for (int j = 0; j < wd; ++j) {
+                const int q = adc_l[i + j];
                 Q += q;
-                M += static_cast<long long>(i) * q;
-                o.cl_adc[k_adc + i] = static_cast<uint8_t>(q);
+                M += static_cast<long long>(j) * q;
+                o.cl_adc[k_adc + j] = static_cast<uint8_t>(q);
             }
-            const uint32_t st0 = strip_l[l], ch = st0 >> 8;
+            const uint32_t st0 = strip_l[i], ch = st0 >> 8;
             const int first = static_cast<int>(st0) - s.mod_lo[ch] * kStrip;
             o.cl_module[k_cl] = s.mod_id[ch];
             o.cl_first[k_cl] = static_cast<uint16_t>(first);
@@ -642,10 +624,10 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
             o.cl_bary[k_cl] =
                 static_cast<float>(static_cast<double>(first) + static_cast<double>(M) / static_cast<double>(Q));
             o.cl_adc_off[k_cl] = k_adc;
-            if (o.cl_snr) {  // noise list is gone by now: re-gather (optional output, tests only)
+            if (o.cl_snr) {
                 double n2 = 0.0;
-                for (int i = 0; i < wd; ++i) {
-                    const double d = static_cast<double>(__ldg(&cal[st0 + i].x));
+                for (int j = 0; j < wd; ++j) {
+                    const double d = static_cast<double>(noise_l[i + j]);
                     n2 = __dadd_rn(n2, __dmul_rn(d, d));
                 }
                 o.cl_snr[k_cl] = static_cast<float>(static_cast<double>(Q) / sqrt(n2));
@@ -675,17 +657,158 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
         o.dev_status[7] = 0;
     }
     SST_MARK(10);
+#undef MASK
+}
+
+// ------------------------------------------------------------------------------ the kernel
+__global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_constant__ KParams p) {
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    Smem &s = *reinterpret_cast<Smem *>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t f = blockIdx.x;
+    const sst_output &o = p.out;
+
+    SST_MARK(0);
+    // ---------------------------------------------------------------- a1: stage the FED payload
+    if (tid == 0) {
+        mbar_init(&s.mbar, 1);
+        fence_proxy_async();
+        const uint32_t fo0 = p.fed_offsets[f], fo1 = p.fed_offsets[f + 1];
+        const bool valid = fo0 <= fo1 && fo1 <= p.max_raw_bytes;
+        const uint32_t size = valid ? fo1 - fo0 : 0u;
+        const bool in_smem = size <= static_cast<uint32_t>(kRawCap) && ((fo0 | size) & 15u) == 0 &&
+                             (reinterpret_cast<uintptr_t>(p.raw) & 15u) == 0;
+        s.fed_start = fo0;
+        s.fed_size = size;
+        s.in_smem = in_smem;
+        s.overrun = valid ? 0u : 1u;
+        s.wide_count = 0;
+        s.long_count = 0;
+        if (in_smem && size) {
+            mbar_expect_tx(&s.mbar, size);
+            bulk_g2s(s.u.raw, p.raw + fo0, size, &s.mbar);
+        }
+    }
+    // meanwhile: zero-fill this FED's slice of the dense output, clear the run table, fetch the
+    // module map of the 96 channels
+    if (o.strip_adc) {
+        uint8_t *dst = o.strip_adc + static_cast<size_t>(f) * kFedStrips;
+        if ((reinterpret_cast<uintptr_t>(o.strip_adc) & 15u) == 0) {
+            uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+            const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+            for (int i = 0; i < kFedStrips / 16 / kThreads; ++i) d4[tid + i * kThreads] = z;
+        } else {
+            for (int i = tid; i < kFedStrips; i += kThreads) dst[i] = 0;
+        }
+    }
+    {
+        uint4 *r4 = reinterpret_cast<uint4 *>(s.runs);
+        const uint4 z = make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int i = 0; i < kRunCap / 4 / kThreads; ++i) r4[tid + i * kThreads] = z;
+    }
+    if (tid < kChan) {
+        const uint2 ci = __ldg(p.chan_info + f * kChan + tid);
+        s.mod_id[tid] = ci.x;
+        s.mod_lo[tid] = static_cast<uint8_t>(ci.y & 0xffu);
+        s.mod_hi[tid] = static_cast<uint8_t>((ci.y >> 8) & 0xffu);
+    }
+    __syncthreads();
+    const bool in_smem = s.in_smem != 0;
+    const uint32_t fed_size = s.fed_size;
+    const uint8_t *rp = in_smem ? s.u.raw : p.raw + s.fed_start;
+
+    SST_MARK(1);
+    // ---------------------------------------------------------------- a1: walk the length chain
+    if (tid == 0) {
+        if (in_smem) {
+            if (fed_size) mbar_wait(&s.mbar, 0);
+            SST_MARK(2);
+            walk_chain_speculative(s.u.raw, s.chan_off, s.chan_len, s.slot_base);
+        } else {
+            SST_MARK(2);
+            if (walk_chain_checked(rp, fed_size, s.overrun != 0, s.chan_off, s.chan_len, s.slot_base)) s.overrun = 1;
+        }
+    }
+    __syncthreads();
+    if (in_smem && fed_size) mbar_wait(&s.mbar, 0);  // async-proxy writes visible to every reader
+    uint32_t my_off = 0, my_len = 0;
+    if (tid < kChan) {
+        my_off = s.chan_off[tid];
+        my_len = s.chan_len[tid];
+    }
+    if (in_smem) {  // validate the speculative chain: channels from the first bad one on are empty
+        const bool ok = tid >= kChan || (s.overrun == 0 && my_off <= fed_size && my_off + my_len <= fed_size);
+        const uint32_t okm = __ballot_sync(0xffffffffu, ok);
+        if (lane == 0 && warp < 3) s.okmask[warp] = okm;
+        __syncthreads();
+        const uint32_t m0 = ~s.okmask[0], m1 = ~s.okmask[1], m2 = ~s.okmask[2];
+        const int first_bad = m0 ? __ffs(m0) - 1 : (m1 ? 31 + __ffs(m1) : (m2 ? 63 + __ffs(m2) : kChan));
+        if (tid < kChan && tid >= first_bad) {
+            my_off = fed_size;
+            my_len = 0;
+            s.chan_off[tid] = fed_size;
+            s.chan_len[tid] = 0;
+        }
+        if (tid == 0 && first_bad < kChan) s.overrun = 1;
+    }
+    // the run table is usable if every channel's slot range fits
+    const uint32_t n_slots = s.slot_base[kChan];
+    const bool table_ok = n_slots <= static_cast<uint32_t>(kRunCap);
+
+    SST_MARK(3);
+    // ---------------------------------------------------------------- a2 pass 1: run headers
+    // thread per channel: validate the run list, count the strips, fill the run table
+    int malformed = 0;
+    uint32_t my_cnt = 0;
+    if (tid < kChan) {
+        if (o.chan_off) o.chan_off[f * kChan + tid] = s.fed_start + my_off;
+        if (o.chan_len) o.chan_len[f * kChan + tid] = static_cast<uint16_t>(my_len);
+        uint32_t n_runs = 0, n_strips = 0;
+        uint32_t *slots = table_ok ? s.runs + s.slot_base[tid] : nullptr;
+        const bool ok = in_smem ? scan_runs(s.u.raw, my_off, my_len, tid, slots, n_runs, n_strips)
+                                : scan_runs(rp, my_off, my_len, tid, slots, n_runs, n_strips);
+        if (ok) {
+            my_cnt = n_strips;
+        } else {  // a malformed channel contributes no strips
+            malformed = 1;
+            my_len = 0;
+            if (slots)
+                for (uint32_t k = 0; k < n_runs; ++k) slots[k] = 0;
+        }
+    }
+    // exclusive scan of the 96 counts (warps 0..2)
+    uint32_t inc = my_cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += u;
+    }
+    if (lane == 31 && warp < 3) s.wscan[0][warp] = inc;
+    const uint32_t n_malformed = __syncthreads_count(malformed);
+    uint32_t my_base = inc - my_cnt;
+    if (warp >= 1) my_base += s.wscan[0][0];
+    if (warp >= 2) my_base += s.wscan[0][1];
+    if (tid < kChan) s.chan_base[tid] = static_cast<uint16_t>(my_base);
+    const uint32_t P = s.wscan[0][0] + s.wscan[0][1] + s.wscan[0][2];  // present strips of the FED
+    __syncthreads();
+
+    SST_MARK(4);
+    if (P <= static_cast<uint32_t>(kListCap))
+        lists_to_clusters<true>(p, s, rp, P, table_ok, n_slots, n_malformed, my_off, my_len, my_base);
+    else
+        lists_to_clusters<false>(p, s, rp, P, table_ok, n_slots, n_malformed, my_off, my_len, my_base);
 }
 
 }  // namespace
-
 
 // ====================================================================================== host
 struct sst_ctx {
     sst_config cfg{};
     cudaMemPool_t pool = nullptr;
     float2 *calib = nullptr;
-    uint32_t *chan_module = nullptr;
+    uint2 *chan_info = nullptr;
     bool has_calib = false;
     std::atomic<int32_t> last_err{0};
     int sm_count = 0;
@@ -726,7 +849,7 @@ sst_status launch_event(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_of
     const size_t mwords = ents / 32 + 2ull * nf + 16;
     auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
     const size_t o_state = 0, o_noise = up(sizeof(unsigned long long) * nf), o_mask = o_noise + up(4 * ents),
-                 o_strip = o_mask + up(4 * 5 * mwords), o_adc = o_strip + up(2 * ents), total = o_adc + up(ents);
+                 o_strip = o_mask + up(4 * M_COUNT * mwords), o_adc = o_strip + up(2 * ents), total = o_adc + up(ents);
     uint8_t *blk = nullptr;
     SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), total, ctx->pool, st));
     SST_CU(cudaMemsetAsync(blk + o_state, 0, sizeof(unsigned long long) * nf, st));
@@ -734,7 +857,7 @@ sst_status launch_event(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_of
     kp.raw = raw;
     kp.fed_offsets = fed_offsets;
     kp.calib = ctx->calib;
-    kp.chan_module = ctx->chan_module;
+    kp.chan_info = ctx->chan_info;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + o_state);
     kp.g_noise = reinterpret_cast<float *>(blk + o_noise);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + o_mask);
@@ -774,7 +897,7 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (ctx->cfg.max_events_in_flight == 0) ctx->cfg.max_events_in_flight = 8;
     auto fail = [&](sst_status s) {
         if (ctx->calib) cudaFree(ctx->calib);
-        if (ctx->chan_module) cudaFree(ctx->chan_module);
+        if (ctx->chan_info) cudaFree(ctx->chan_info);
         if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
         delete ctx;
         return s;
@@ -791,7 +914,7 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         return fail(SST_ERR_CUDA);
     const size_t n = static_cast<size_t>(cfg->n_feds) * kFedStrips;
     if (cudaMalloc(&ctx->calib, n * sizeof(float2)) != cudaSuccess) return fail(SST_ERR_CUDA);
-    if (cudaMalloc(&ctx->chan_module, static_cast<size_t>(cfg->n_feds) * kChan * sizeof(uint32_t)) !=
+    if (cudaMalloc(&ctx->chan_info, static_cast<size_t>(cfg->n_feds) * kChan * sizeof(uint2)) !=
         cudaSuccess)
         return fail(SST_ERR_CUDA);
     if (cudaFuncSetAttribute(sst_fed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -832,7 +955,16 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
     }
     SST_CU(cudaSetDevice(ctx->cfg.device));
     SST_CU(cudaMemcpy(ctx->calib, packed.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
-    SST_CU(cudaMemcpy(ctx->chan_module, chan_module, nch * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    // module extent of every channel (modules are runs of equal ids inside one FED)
+    std::vector<uint2> info(nch);
+    for (size_t c0 = 0; c0 < nch;) {
+        size_t c1 = c0 + 1;
+        while (c1 < nch && c1 % kChan != 0 && chan_module[c1] == chan_module[c0]) ++c1;
+        for (size_t c = c0; c < c1; ++c)
+            info[c] = make_uint2(chan_module[c0], static_cast<uint32_t>(c0 % kChan) | (static_cast<uint32_t>((c1 - 1) % kChan + 1) << 8));
+        c0 = c1;
+    }
+    SST_CU(cudaMemcpy(ctx->chan_info, info.data(), nch * sizeof(uint2), cudaMemcpyHostToDevice));
     SST_CU(cudaDeviceSynchronize());
     ctx->has_calib = true;
     return SST_OK;
@@ -960,7 +1092,7 @@ sst_status sst_destroy(sst_ctx *ctx) {
     cudaSetDevice(ctx->cfg.device);
     cudaDeviceSynchronize();
     if (ctx->calib) cudaFree(ctx->calib);
-    if (ctx->chan_module) cudaFree(ctx->chan_module);
+    if (ctx->chan_info) cudaFree(ctx->chan_info);
     if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
     delete ctx;
     return SST_OK;
