@@ -123,9 +123,18 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
  * fed_offsets: DEVICE [n_feds+1] byte offsets of the FEDs in raw (16-byte multiples for the
  * fast path).  thr and out are HOST structs read before the call returns.  The work is
  * enqueued on `stream`; the call does not synchronise.  Scratch comes from the context's
- * stream-ordered pool. */
+ * stream-ordered pool: one block per stream, allocated on the stream's first event and reused
+ * (so a stream must not be driven by two host threads at once). */
 sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
                               const sst_thresholds *thr, const sst_output *out, void *stream);
+
+/* n_events independent events in one call (several events in flight): event e is
+ * enqueued on streams[e % n_streams] exactly as sst_unpack_cluster would, with raw[e],
+ * fed_offsets[e] (DEVICE) and outs[e].  raw, fed_offsets, outs and streams are HOST arrays read
+ * before the call returns.  Does not synchronise. */
+sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
+                                    const uint32_t *const *fed_offsets, const sst_thresholds *thr,
+                                    const sst_output *outs, void *const *streams, uint32_t n_streams);
 
 /* The same event with HOST buffers: raw[raw_bytes] and fed_offsets[n_feds+1] are copied to
  * pooled device buffers on `stream`, the event is processed, and dev_status, n_clusters and the

@@ -19,7 +19,7 @@ ST_FLAGS, ST_N_MALFORMED, ST_N_CLUSTERS, ST_N_ADC, ST_N_OVERRUN, ST_N_SEEDS = ra
 FLAG_CLUSTER_CAP, FLAG_ADC_CAP, FLAG_MALFORMED, FLAG_OVERRUN = 1, 2, 4, 8
 SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB = range(5)
 
-EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_cluster_host",
+EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
            "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_destroy", "sst_last_cuda_error",
            "sst_status_string", "sst_get_info"]
 
@@ -67,6 +67,7 @@ def load():
     L.sst_create.argtypes = [C.POINTER(sst_config), C.POINTER(vp)]
     L.sst_upload_calib.argtypes = [vp, vp, vp, vp, vp]
     L.sst_unpack_cluster.argtypes = [vp, vp, vp, C.POINTER(sst_thresholds), C.POINTER(sst_output), vp]
+    L.sst_unpack_cluster_batch.argtypes = [vp, C.c_uint32, vp, vp, C.POINTER(sst_thresholds), vp, vp, C.c_uint32]
     L.sst_unpack_cluster_host.argtypes = [vp, vp, C.c_uint32, vp, C.POINTER(sst_thresholds),
                                           C.POINTER(sst_output), vp]
     L.sst_event_alloc.argtypes = [vp, C.c_uint64, vp, C.POINTER(vp)]
@@ -137,6 +138,27 @@ def sst_unpack_cluster(ctx, raw, fed_offsets, thresholds, out: sst_output, strea
     rc = load().sst_unpack_cluster(ctx, _ptr(raw), _ptr(fed_offsets), C.byref(thr), C.byref(out),
                                    C.c_void_p(stream))
     _check(ctx, rc, "sst_unpack_cluster")
+
+
+class Batch:
+    """Marshalled arguments of sst_unpack_cluster_batch, built once and reused every step."""
+
+    def __init__(self, raws, fed_offsets, thresholds, outs, streams):
+        n = len(raws)
+        self.n = n
+        self.raw = (C.c_void_p * n)(*[_ptr(r) for r in raws])
+        self.fo = (C.c_void_p * n)(*[_ptr(f) for f in fed_offsets])
+        self.outs = (sst_output * n)(*outs)
+        self.streams = (C.c_void_p * len(streams))(*streams)
+        self.n_streams = len(streams)
+        self.thr = thresholds if isinstance(thresholds, sst_thresholds) else sst_thresholds(*map(float, thresholds))
+
+
+def sst_unpack_cluster_batch(ctx, batch: Batch):
+    """Enqueue batch.n events, event e on batch.streams[e % n_streams].  Does not synchronise."""
+    rc = load().sst_unpack_cluster_batch(ctx, batch.n, batch.raw, batch.fo, C.byref(batch.thr), batch.outs,
+                                         batch.streams, batch.n_streams)
+    _check(ctx, rc, "sst_unpack_cluster_batch")
 
 
 def sst_unpack_cluster_host(ctx, raw, raw_bytes: int, fed_offsets, thresholds, out: sst_output,

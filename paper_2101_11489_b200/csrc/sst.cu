@@ -29,6 +29,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -52,8 +53,16 @@ constexpr int kWideQ = 32;
 enum { M_ACT = 0, M_SEED, M_BRK, M_LINK, M_ACC, M_WTOT, M_COUNT };
 
 // per-FED aggregate published for the look-back (one 64-bit word)
-constexpr int kShAdc = 14, kShSeed = 29, kShMalf = 44, kShOvr = 51;
+// look-back state, two 64-bit words per FED, living in a per-stream scratch that is never cleared:
+// every word carries the 8-bit epoch of the call that wrote it and counts only if that matches.
+// Word 0: status (bits 62-63: 1 = aggregate, 2 = inclusive prefix) | epoch (bits 54-61) | clusters
+// (26 bits) | ADC bytes << 26 (28 bits).  Word 1, aggregate only: ready (bit 63) | epoch (bits 55-62)
+// | seeds (20 bits) | malformed channels << 20 (7 bits) | overrun << 27.
+constexpr unsigned long long kStA = 1ull << 62, kStP = 2ull << 62, kStMask = (1ull << 54) - 1;
+constexpr int kShEp0 = 54, kShEp1 = 55, kShAdc = 26;
+constexpr int kShMalf = 20, kShOvr = 27;
 constexpr unsigned long long kReady = 1ull << 63;
+constexpr uint32_t kMaxFeds = 4096;  // keeps event totals inside the 26/28-bit prefix fields
 
 struct __align__(128) Smem {
     union {                       // the payload is dead once the lists are built
@@ -95,6 +104,7 @@ struct KParams {
     double tcl2;
     float t_ch, t_seed;
     uint32_t max_raw_bytes, n_feds;
+    uint32_t epoch;  // 1..255, changes on every use of the scratch
     sst_output out;
     unsigned long long *phase_clk;  // debug builds only (SST_PHASE_TIMING)
 };
@@ -154,7 +164,7 @@ __device__ __forceinline__ bool ge_exact(float a, float t, float n) {
     return (a > p) || (a == p && e <= 0.0f);
 }
 // min(254, floor(fl32(fl32(adc / gain) + 0.5)))  (IEEE RN division and add, no contraction)
-__device__ __forceinline__ uint32_t gain_correct(uint32_t adc, float gain) {
+__device__ __noinline__ uint32_t gain_correct(uint32_t adc, float gain) {
     const float u = __fadd_rn(__fdiv_rn(static_cast<float>(adc), gain), 0.5f);
     const float fl = floorf(u);
     return fl >= 254.0f ? 254u : static_cast<uint32_t>(fl);
@@ -187,6 +197,7 @@ __device__ __forceinline__ int run_end(const uint32_t *link, int i) {
 __device__ __forceinline__ bool accept_serial(const uint8_t *q, const float *noise, int l, int w, double tcl2) {
     int Q = 0;
     double n2 = 0.0;
+    #pragma unroll 1
     for (int i = 0; i < w; ++i) {
         Q += q[l + i];
         const double d = static_cast<double>(noise[l + i]);
@@ -203,6 +214,7 @@ __device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, i
                                          int lane) {
     uint32_t Q = 0;
     double n2p = 0.0;
+    #pragma unroll 1
     for (int i = lane; i < w; i += 32) {
         Q += q[l + i];
         const double d = static_cast<double>(noise[l + i]);
@@ -216,6 +228,7 @@ __device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, i
     if (!(fabs(lhs - rhs) > rhs * static_cast<double>(w) * 0x1p-50)) {
         if (lane == 0) {
             double n2 = 0.0;
+            #pragma unroll 1
             for (int i = 0; i < w; ++i) {
                 const double d = static_cast<double>(noise[l + i]);
                 n2 = __dadd_rn(n2, __dmul_rn(d, d));
@@ -225,6 +238,17 @@ __device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, i
         ok = __shfl_sync(0xffffffffu, ok, 0);
     }
     return ok != 0;
+}
+
+// optional output: cluster S/N = Q / sqrt(sum noise^2), sequential double sum
+__device__ __noinline__ float cluster_snr(const float *noise, int l, int w, int Q) {
+    double n2 = 0.0;
+#pragma unroll 1
+    for (int i = 0; i < w; ++i) {
+        const double d = static_cast<double>(noise[l + i]);
+        n2 = __dadd_rn(n2, __dmul_rn(d, d));
+    }
+    return static_cast<float>(static_cast<double>(Q) / sqrt(n2));
 }
 
 // ------------------------------------------------------------------------------ raw payload
@@ -237,6 +261,7 @@ __device__ __forceinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t f
     uint32_t pos = 0, slots = 0;
     int c = 0;
     if (!over) {
+        #pragma unroll 1
         for (; c < kChan; ++c) {
             if (pos + 2 > fed_size) break;
             const uint32_t l16 = rp[pos] | (static_cast<uint32_t>(rp[pos + 1]) << 8);
@@ -249,6 +274,7 @@ __device__ __forceinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t f
         }
     }
     over = c < kChan;
+    #pragma unroll 1
     for (; c < kChan; ++c) {  // channels behind an overrun are empty, recorded at the FED end
         chan_off[c] = fed_size;
         chan_len[c] = 0;
@@ -284,6 +310,7 @@ __device__ __forceinline__ bool scan_runs(const uint8_t *rp, uint32_t off, uint3
     uint32_t q = off, next_free = 0, k = 0, within = 0;
     const uint32_t qend = off + len_bytes;
     bool ok = true;
+    #pragma unroll 1
     while (q < qend) {
         if (q + 2 > qend) { ok = false; break; }
         const uint32_t first = rp[q];
@@ -306,6 +333,7 @@ __device__ __forceinline__ void stream_channel(const uint8_t *rp, uint32_t off, 
                                                int chan, uint16_t *strip_l, uint8_t *adc_l, uint8_t *dense) {
     uint32_t rem = 0, tgt = 0, hdr = 0;
     const uint32_t qend = off + len_bytes;
+    #pragma unroll 1
     for (uint32_t q = off; q < qend; ++q) {
         const uint32_t b = rp[q];
         if (rem) {
@@ -333,7 +361,7 @@ __device__ __forceinline__ void stream_channel(const uint8_t *rp, uint32_t off, 
 // Everything after the channel walk, on the FED's lists of present strips.  kSmem = true: lists
 // and masks in shared memory (LDS/STS); false: in this FED's slice of the global scratch.
 template <bool kSmem>
-__device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, const uint8_t *rp, const uint32_t P,
+__device__ __noinline__ void lists_to_clusters(const KParams &p, Smem &s, const uint8_t *rp, const uint32_t P,
                                                   const bool table_ok, const uint32_t n_slots,
                                                   const uint32_t n_malformed, const uint32_t my_off,
                                                   const uint32_t my_len, const uint32_t my_base) {
@@ -352,6 +380,7 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
 
     // ---------------------------------------------------------------- a2 pass 2: thread per run
     if (table_ok) {
+        #pragma unroll 1
         for (uint32_t slot = tid; slot < n_slots; slot += kThreads) {
             const uint32_t rec = s.runs[slot];
             if (!(rec >> 31)) continue;
@@ -363,6 +392,7 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
             }
             const uint32_t src = s.chan_off[c] + within + 2u * (slot - s.slot_base[c] + 1u);
             const uint32_t dst = s.chan_base[c] + within, g = c * kStrip + first;
+            #pragma unroll 1
             for (uint32_t i = 0; i < len; ++i) {
                 const uint8_t b = rp[src + i];
                 strip_l[dst + i] = static_cast<uint16_t>(g + i);
@@ -372,12 +402,14 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
         }
         __syncthreads();
         const uint32_t nq = min(s.long_count, static_cast<uint32_t>(kLongQ));
+        #pragma unroll 1
         for (uint32_t e = warp; e < nq; e += kWarps) {  // long runs: one warp each, lane per byte
             const uint32_t slot = s.long_q[e], rec = s.runs[slot];
             const uint32_t c = (rec >> 24) & 127u, within = rec & 255u, first = (rec >> 8) & 255u,
                            len = ((rec >> 16) & 255u) + 1u;
             const uint32_t src = s.chan_off[c] + within + 2u * (slot - s.slot_base[c] + 1u);
             const uint32_t dst = s.chan_base[c] + within, g = c * kStrip + first;
+            #pragma unroll 1
             for (uint32_t i = lane; i < len; i += 32) {
                 const uint8_t b = rp[src + i];
                 strip_l[dst + i] = static_cast<uint16_t>(g + i);
@@ -394,6 +426,7 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
     // ---------------------------------------------------------------- a3: active / seed flags
     // lane per entry; a warp covers one mask word per step, so the masks come from ballots
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
+    #pragma unroll 1
     for (uint32_t base = 0; base < nw * 32; base += kThreads * 2) {
         uint32_t idx[2], sv[2], av[2], sp[2];
         float2 cv[2];
@@ -431,6 +464,7 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
         }
     }
     __syncthreads();
+    #pragma unroll 1
     for (uint32_t w = tid; w <= nw; w += kThreads) {  // link mask (+ zero sentinel word), clear acc
         uint32_t lk = 0;
         if (w < nw) {
@@ -442,6 +476,7 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
         }
         MASK(M_LINK)[w] = lk;
         MASK(M_ACC)[w] = 0;
+        MASK(M_WTOT)[w] = 0;
     }
     __syncthreads();
 
@@ -450,6 +485,7 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
     const uint32_t *const m_link = MASK(M_LINK);
     const uint32_t *const m_seed = MASK(M_SEED);
     uint32_t *const m_acc = MASK(M_ACC);
+    #pragma unroll 1
     for (uint32_t i = tid; i < nw * 32; i += kThreads) {
         const int w = i >> 5, b = i & 31;
         const uint32_t sw = m_seed[w];
@@ -477,168 +513,206 @@ __device__ __forceinline__ void lists_to_clusters(const KParams &p, Smem &s, con
                 continue;
             }
         }
-        if (accept_serial(adc_l, noise_l, l, wd, p.tcl2)) atomicOr(&m_acc[l >> 5], 1u << (l & 31));
+        if (accept_serial(adc_l, noise_l, l, wd, p.tcl2)) {
+            atomicOr(&m_acc[l >> 5], 1u << (l & 31));
+            atomicAdd(&MASK(M_WTOT)[l >> 5], 1u | (static_cast<uint32_t>(wd) << 16));
+        }
     }
     __syncthreads();
     {
         const uint32_t nq = min(s.wide_count, static_cast<uint32_t>(kWideQ));
+        #pragma unroll 1
         for (uint32_t e = warp; e < nq; e += kWarps) {
             const int l = s.wide_q[e] & 0xffffu, wd = s.wide_q[e] >> 16;
-            if (accept_warp(adc_l, noise_l, l, wd, p.tcl2, lane) && lane == 0)
+            if (accept_warp(adc_l, noise_l, l, wd, p.tcl2, lane) && lane == 0) {
                 atomicOr(&m_acc[l >> 5], 1u << (l & 31));
-        }
-        if (nq) __syncthreads();
-    }
-
-    SST_MARK(7);
-    // ---------------------------------------------------------------- a7: local scan
-    // per mask word (warp per word): accepted clusters and their ADC bytes
-    uint32_t *const m_wtot = MASK(M_WTOT);
-    uint32_t *const m_spre = MASK(M_BRK);  // brk is dead: per-word seed prefix goes here
-    for (uint32_t w = warp; w < nw; w += kWarps) {
-        const uint32_t aw = m_acc[w];
-        uint32_t wsum = 0;
-        if (aw) {  // warp-uniform
-            const int i = (w << 5) + lane;
-            wsum = warp_sum(((aw >> lane) & 1u) ? static_cast<uint32_t>(run_end(m_link, i) - i + 1) : 0u);
-        }
-        if (lane == 0) m_wtot[w] = __popc(aw) | (wsum << 16);
-    }
-    __syncthreads();
-    // thread t owns words 3t .. 3t+2: block-wide exclusive scan of the word totals
-    uint32_t my_a = 0, my_s = 0;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        const uint32_t w = 3 * tid + k;
-        if (w < nw) { my_a += m_wtot[w]; my_s += __popc(m_seed[w]); }
-    }
-    uint32_t inc_a = my_a, inc_s = my_s;  // FED totals <= 12288 clusters / 24576 ADC bytes: halves stay apart
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t ua = __shfl_up_sync(0xffffffffu, inc_a, d);
-        const uint32_t us = __shfl_up_sync(0xffffffffu, inc_s, d);
-        if (lane >= d) { inc_a += ua; inc_s += us; }
-    }
-    if (lane == 31) { s.wscan[0][warp] = inc_a; s.wscan[1][warp] = inc_s; }
-    __syncthreads();
-    uint32_t pre_a = 0, pre_s = 0, tot_a = 0, tot_s = 0;
-#pragma unroll
-    for (int i = 0; i < kWarps; ++i) {
-        if (i < warp) { pre_a += s.wscan[0][i]; pre_s += s.wscan[1][i]; }
-        tot_a += s.wscan[0][i];
-        tot_s += s.wscan[1][i];
-    }
-    const uint32_t fed_cl = tot_a & 0xffffu, fed_adc = tot_a >> 16, fed_seed = tot_s;
-    const uint32_t fed_over = s.overrun;
-    if (tid == 0) {  // publish the aggregate as early as possible
-        const unsigned long long agg = kReady | fed_cl | (static_cast<unsigned long long>(fed_adc) << kShAdc) |
-                                       (static_cast<unsigned long long>(fed_seed) << kShSeed) |
-                                       (static_cast<unsigned long long>(n_malformed) << kShMalf) |
-                                       (static_cast<unsigned long long>(fed_over) << kShOvr);
-        st_state(p.fed_state + f, agg);
-    }
-    {
-        uint32_t ex_a = pre_a + inc_a - my_a, ex_s = pre_s + inc_s - my_s;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const uint32_t w = 3 * tid + k;
-            if (w < nw) {
-                const uint32_t t = m_wtot[w];
-                m_wtot[w] = ex_a;
-                m_spre[w] = ex_s;
-                ex_a += t;
-                ex_s += __popc(m_seed[w]);
+                atomicAdd(&MASK(M_WTOT)[l >> 5], 1u | (static_cast<uint32_t>(wd) << 16));
             }
         }
     }
+    __syncthreads();
 
-    SST_MARK(8);
-    // ---------------------------------------------------------------- a7: look-back
-    uint32_t b_cl = 0, b_adc = 0, b_seed = 0, b_malf = 0, b_over = 0;
-    for (uint32_t j = tid; j < f; j += kThreads) {
-        unsigned long long v = ld_state(p.fed_state + j);
-        while (!(v & kReady)) {
-            __nanosleep(100);
-            v = ld_state(p.fed_state + j);
+    SST_MARK(7);
+    // ---------------------------------------------------------------- a7: scan + look-back, warp 0
+    // Word totals (accepted clusters | ADC bytes << 16) were accumulated by the accepting lanes.
+    // Warp 0 turns them into exclusive prefixes, publishes the FED aggregate and resolves the
+    // FED's base offsets with a decoupled look-back over the earlier FEDs.
+    uint32_t *const m_wtot = MASK(M_WTOT);
+    uint32_t *const m_spre = MASK(M_BRK);  // brk is dead: per-word seed prefix goes here
+    const uint32_t fed_over = s.overrun;
+    if (warp == 0) {
+        const uint32_t K = (nw + 31) >> 5;  // words per lane
+        uint32_t my_a = 0, my_s = 0;
+        #pragma unroll 1
+        for (uint32_t k = 0; k < K; ++k) {
+            const uint32_t w = lane * K + k;
+            if (w < nw) { my_a += m_wtot[w]; my_s += __popc(m_seed[w]); }
         }
-        b_cl += static_cast<uint32_t>(v) & 0x3fffu;
-        b_adc += static_cast<uint32_t>(v >> kShAdc) & 0x7fffu;
-        b_seed += static_cast<uint32_t>(v >> kShSeed) & 0x7fffu;
-        b_malf += static_cast<uint32_t>(v >> kShMalf) & 0x7fu;
-        b_over += static_cast<uint32_t>(v >> kShOvr) & 1u;
-    }
-    b_cl = warp_sum(b_cl); b_adc = warp_sum(b_adc); b_seed = warp_sum(b_seed);
-    b_malf = warp_sum(b_malf); b_over = warp_sum(b_over);
-    if (lane == 0) {
-        s.red[0][warp] = b_cl; s.red[1][warp] = b_adc; s.red[2][warp] = b_seed;
-        s.red[3][warp] = b_malf; s.red[4][warp] = b_over;
-    }
-    __syncthreads();  // also orders the per-word prefixes
-    b_cl = b_adc = b_seed = b_malf = b_over = 0;
+        uint32_t inc_a = my_a, inc_s = my_s;  // FED totals <= 12288 clusters / 24576 ADC bytes: halves stay apart
 #pragma unroll
-    for (int i = 0; i < kWarps; ++i) {
-        b_cl += s.red[0][i]; b_adc += s.red[1][i]; b_seed += s.red[2][i];
-        b_malf += s.red[3][i]; b_over += s.red[4][i];
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t ua = __shfl_up_sync(0xffffffffu, inc_a, d);
+            const uint32_t us = __shfl_up_sync(0xffffffffu, inc_s, d);
+            if (lane >= d) { inc_a += ua; inc_s += us; }
+        }
+        const uint32_t tot_a = __shfl_sync(0xffffffffu, inc_a, 31), tot_s = __shfl_sync(0xffffffffu, inc_s, 31);
+        const uint32_t fed_cl = tot_a & 0xffffu, fed_adc = tot_a >> 16;
+        // publish: word 0 = status | clusters | ADC bytes << 30 (aggregate now, inclusive prefix
+        // later); word 1 = ready | seeds | malformed | overrun (aggregate only)
+        const unsigned long long agg0 = fed_cl | (static_cast<unsigned long long>(fed_adc) << kShAdc);
+        const unsigned long long ep0 = static_cast<unsigned long long>(p.epoch) << kShEp0;
+        if (lane == 0) {
+            st_state(p.fed_state + 2 * f, (f == 0 ? kStP : kStA) | ep0 | agg0);
+            st_state(p.fed_state + 2 * f + 1, kReady | (static_cast<unsigned long long>(p.epoch) << kShEp1) | tot_s |
+                                                  (static_cast<unsigned long long>(n_malformed) << kShMalf) |
+                                                  (static_cast<unsigned long long>(fed_over) << kShOvr));
+        }
+        {
+            uint32_t ex_a = inc_a - my_a, ex_s = inc_s - my_s;
+            #pragma unroll 1
+            for (uint32_t k = 0; k < K; ++k) {
+                const uint32_t w = lane * K + k;
+                if (w < nw) {
+                    const uint32_t t = m_wtot[w];
+                    m_wtot[w] = ex_a;
+                    m_spre[w] = ex_s;
+                    ex_a += t;
+                    ex_s += __popc(m_seed[w]);
+                }
+            }
+        }
+        SST_MARK(8);
+        // look-back: lane 0 reads the nearest predecessor; stop at the first inclusive prefix
+        unsigned long long excl = 0;
+        #pragma unroll 1
+        for (int base = static_cast<int>(f) - 1; base >= 0; base -= 32) {
+            const int j = base - lane;
+            unsigned long long v = kStP;  // before FED 0: prefix 0
+            if (j >= 0) {
+                v = ld_state(p.fed_state + 2 * j);
+                while (!(v >> 62) || ((v >> kShEp0) & 0xffull) != p.epoch) {  // not written by this call yet
+                    __nanosleep(64);
+                    v = ld_state(p.fed_state + 2 * j);
+                }
+            }
+            const uint32_t pm = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);
+            const int stop = pm ? __ffs(pm) - 1 : 31;  // lanes 0..stop contribute
+            unsigned long long c = lane <= stop ? (v & kStMask) : 0ull;
+#pragma unroll
+            for (int o2 = 16; o2 > 0; o2 >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o2);
+            excl += c;
+            if (pm) break;
+        }
+        if (lane == 0) {
+            if (f) st_state(p.fed_state + 2 * f, kStP | ep0 | (excl + agg0));
+            s.red[0][0] = static_cast<uint32_t>(excl & ((1ull << kShAdc) - 1));  // clusters before this FED
+            s.red[0][1] = static_cast<uint32_t>(excl >> kShAdc);                 // ADC bytes before this FED
+            s.red[0][2] = fed_cl;
+            s.red[0][3] = fed_adc;
+            s.red[0][4] = tot_s;
+        }
+    }
+    __syncthreads();
+    const uint32_t b_cl = s.red[0][0], b_adc = s.red[0][1], fed_cl = s.red[0][2], fed_adc = s.red[0][3],
+                   fed_seed = s.red[0][4];
+
+    // seed-index base (only when that output is requested) and, in the last FED, the event totals:
+    // sums over the aggregate-only word of every earlier FED
+    uint32_t b_seed = 0, b_malf = 0, b_over = 0;
+    const bool last = f == p.n_feds - 1;
+    if (o.seed_idx || last) {
+        #pragma unroll 1
+        for (uint32_t j = tid; j < f; j += kThreads) {
+            unsigned long long v = ld_state(p.fed_state + 2 * j + 1);
+            while (!(v & kReady) || ((v >> kShEp1) & 0xffull) != p.epoch) {
+                __nanosleep(100);
+                v = ld_state(p.fed_state + 2 * j + 1);
+            }
+            b_seed += static_cast<uint32_t>(v) & 0xfffffu;
+            b_malf += static_cast<uint32_t>(v >> kShMalf) & 0x7fu;
+            b_over += static_cast<uint32_t>(v >> kShOvr) & 1u;
+        }
+        b_seed = warp_sum(b_seed); b_malf = warp_sum(b_malf); b_over = warp_sum(b_over);
+        if (lane == 0) { s.red[1][warp] = b_seed; s.red[2][warp] = b_malf; s.red[3][warp] = b_over; }
+        __syncthreads();
+        b_seed = b_malf = b_over = 0;
+#pragma unroll
+        for (int i = 0; i < kWarps; ++i) { b_seed += s.red[1][i]; b_malf += s.red[2][i]; b_over += s.red[3][i]; }
     }
 
     SST_MARK(9);
     // ---------------------------------------------------------------- a7: emit, (module, first strip) order
-    // warp per mask word, lane per entry: cluster index and ADC offset come from the word
-    // prefix plus a scan inside the word
-    for (uint32_t w = warp; w < nw; w += kWarps) {
-        const uint32_t aw = m_acc[w], sw = m_seed[w];
-        const int i = (w << 5) + lane;
-        const uint32_t lt = (1u << lane) - 1u;
-        if (o.seed_idx && ((sw >> lane) & 1u)) {
-            const uint32_t k = b_seed + m_spre[w] + __popc(sw & lt);
-            if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + strip_l[i];
-        }
-        if (!aw) continue;  // warp-uniform
-        const bool mine = (aw >> lane) & 1u;
-        const int wd = mine ? run_end(m_link, i) - i + 1 : 0;
-        uint32_t incw = wd;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t u = __shfl_up_sync(0xffffffffu, incw, d);
-            if (lane >= d) incw += u;
-        }
-        if (!mine) continue;
-        const uint32_t pre = m_wtot[w];
-        const uint32_t k_cl = b_cl + (pre & 0xffffu) + __popc(aw & lt);
-        const uint32_t k_adc = b_adc + (pre >> 16) + (incw - wd);
-        if (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc) {
-            int Q = 0;
-            long long M = 0;
-            for (int j = 0; j < wd; ++j) {
-                const int q = adc_l[i + j];
-                Q += q;
-                M += static_cast<long long>(j) * q;
-                o.cl_adc[k_adc + j] = static_cast<uint8_t>(q);
+    if (o.seed_idx) {
+        #pragma unroll 1
+        for (uint32_t i = tid; i < nw * 32; i += kThreads) {
+            const uint32_t w = i >> 5, b = i & 31, sw = m_seed[w];
+            if ((sw >> b) & 1u) {
+                const uint32_t k = b_seed + m_spre[w] + __popc(sw & ((1u << b) - 1u));
+                if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + strip_l[i];
             }
-            const uint32_t st0 = strip_l[i], ch = st0 >> 8;
-            const int first = static_cast<int>(st0) - s.mod_lo[ch] * kStrip;
-            o.cl_module[k_cl] = s.mod_id[ch];
-            o.cl_first[k_cl] = static_cast<uint16_t>(first);
-            o.cl_width[k_cl] = static_cast<uint16_t>(wd);
-            o.cl_charge[k_cl] = Q;
-            o.cl_bary[k_cl] =
-                static_cast<float>(static_cast<double>(first) + static_cast<double>(M) / static_cast<double>(Q));
-            o.cl_adc_off[k_cl] = k_adc;
-            if (o.cl_snr) {
-                double n2 = 0.0;
-                for (int j = 0; j < wd; ++j) {
-                    const double d = static_cast<double>(noise_l[i + j]);
-                    n2 = __dadd_rn(n2, __dmul_rn(d, d));
-                }
-                o.cl_snr[k_cl] = static_cast<float>(static_cast<double>(Q) / sqrt(n2));
-            }
-        } else {
-            // the first cluster that does not fit reports how many were written
-            const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
-            if (prev_fits) *o.n_clusters = k_cl;
         }
     }
-    if (f == p.n_feds - 1 && tid == 0) {  // event totals = prefix of the last FED + its own
+    // ordered list of the FED's accepted clusters (entry | FED-local ADC offset << 16) in the dead
+    // run table, then lane per cluster; FEDs with more clusters than the table go in rounds
+    uint32_t *const cl_l = s.runs;
+    #pragma unroll 1
+    for (uint32_t c0 = 0; c0 < fed_cl; c0 += kRunCap) {
+        if (c0) __syncthreads();
+        #pragma unroll 1
+        for (uint32_t w = warp; w < nw; w += kWarps) {
+            const uint32_t aw = m_acc[w];
+            if (!aw) continue;  // warp-uniform
+            const int i = (w << 5) + lane;
+            const bool mine = (aw >> lane) & 1u;
+            const uint32_t wd = mine ? static_cast<uint32_t>(run_end(m_link, i) - i + 1) : 0u;
+            uint32_t incw = wd;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incw, d);
+                if (lane >= d) incw += u;
+            }
+            const uint32_t pre = m_wtot[w];
+            const uint32_t c = (pre & 0xffffu) + __popc(aw & ((1u << lane) - 1u)) - c0;
+            if (mine && c < static_cast<uint32_t>(kRunCap))
+                cl_l[c] = static_cast<uint32_t>(i) | (((pre >> 16) + incw - wd) << 16);
+        }
+        __syncthreads();
+        const uint32_t nc = min(fed_cl - c0, static_cast<uint32_t>(kRunCap));
+        #pragma unroll 1
+        for (uint32_t c = tid; c < nc; c += kThreads) {
+            const uint32_t e = cl_l[c];
+            const int i = e & 0xffffu;
+            const uint32_t k_cl = b_cl + c0 + c, k_adc = b_adc + (e >> 16);
+            const int wd = run_end(m_link, i) - i + 1;
+            if (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc) {
+                int Q = 0;
+                long long M = 0;
+                #pragma unroll 1
+                for (int j = 0; j < wd; ++j) {
+                    const int q = adc_l[i + j];
+                    Q += q;
+                    M += static_cast<long long>(j) * q;
+                    o.cl_adc[k_adc + j] = static_cast<uint8_t>(q);
+                }
+                const uint32_t st0 = strip_l[i], ch = st0 >> 8;
+                const int first = static_cast<int>(st0) - s.mod_lo[ch] * kStrip;
+                o.cl_module[k_cl] = s.mod_id[ch];
+                o.cl_first[k_cl] = static_cast<uint16_t>(first);
+                o.cl_width[k_cl] = static_cast<uint16_t>(wd);
+                o.cl_charge[k_cl] = Q;
+                // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
+                o.cl_bary[k_cl] = __fadd_rn(static_cast<float>(first),
+                                            __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
+                o.cl_adc_off[k_cl] = k_adc;
+                if (o.cl_snr) o.cl_snr[k_cl] = cluster_snr(noise_l, i, wd, Q);
+            } else {
+                // the first cluster that does not fit reports how many were written
+                const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
+                if (prev_fits) *o.n_clusters = k_cl;
+            }
+        }
+    }
+    if (last && tid == 0) {  // event totals = prefix of the last FED + its own
         const uint32_t n_cl = b_cl + fed_cl, n_adc = b_adc + fed_adc, n_mal = b_malf + n_malformed,
                        n_over = b_over + fed_over;
         uint32_t flags = 0;
@@ -699,6 +773,7 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
 #pragma unroll
             for (int i = 0; i < kFedStrips / 16 / kThreads; ++i) d4[tid + i * kThreads] = z;
         } else {
+            #pragma unroll 1
             for (int i = tid; i < kFedStrips; i += kThreads) dst[i] = 0;
         }
     }
@@ -775,6 +850,7 @@ __global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_const
             malformed = 1;
             my_len = 0;
             if (slots)
+                #pragma unroll 1
                 for (uint32_t k = 0; k < n_runs; ++k) slots[k] = 0;
         }
     }
@@ -813,6 +889,11 @@ struct sst_ctx {
     std::atomic<int32_t> last_err{0};
     int sm_count = 0;
     int ctas_per_sm = 0;
+    // per-stream scratch (look-back states + overflow lists), taken from the pool on a stream's
+    // first event and kept: stream order makes reuse safe, the epoch makes clearing unnecessary
+    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t epoch; };
+    std::mutex slot_mu;
+    std::vector<Slot> slots;
 };
 
 namespace {
@@ -841,41 +922,76 @@ bool output_ok(const sst_output *o) {
 unsigned long long *g_phase_clk = nullptr;
 #endif
 
+struct ScratchLayout {
+    size_t ents, mwords, o_state, o_noise, o_mask, o_strip, o_adc, total, state_bytes;
+};
+ScratchLayout scratch_layout(const sst_ctx *ctx) {
+    ScratchLayout L{};
+    const uint32_t nf = ctx->cfg.n_feds;
+    auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
+    L.ents = static_cast<size_t>(ctx->cfg.max_raw_bytes) + 16ull * nf + 64;
+    L.mwords = L.ents / 32 + 2ull * nf + 16;
+    L.state_bytes = 2 * sizeof(unsigned long long) * nf;
+    L.o_state = 0;
+    L.o_noise = up(L.state_bytes);
+    L.o_mask = L.o_noise + up(4 * L.ents);
+    L.o_strip = L.o_mask + up(4 * M_COUNT * L.mwords);
+    L.o_adc = L.o_strip + up(2 * L.ents);
+    L.total = L.o_adc + up(L.ents);
+    return L;
+}
+
+// The scratch of `st`: allocated (stream-ordered, from the pool) and cleared once, then reused.
+sst_status stream_scratch(sst_ctx *ctx, cudaStream_t st, uint8_t **mem, uint32_t *epoch) {
+    std::lock_guard<std::mutex> lock(ctx->slot_mu);
+    for (auto &sl : ctx->slots)
+        if (sl.stream == st) {
+            sl.epoch = sl.epoch % 255u + 1u;
+            *mem = sl.mem;
+            *epoch = sl.epoch;
+            return SST_OK;
+        }
+    const ScratchLayout L = scratch_layout(ctx);
+    uint8_t *blk = nullptr;
+    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), L.total, ctx->pool, st));
+    SST_CU(cudaMemsetAsync(blk + L.o_state, 0, L.state_bytes, st));
+    ctx->slots.push_back({st, blk, 1u});
+    *mem = blk;
+    *epoch = 1u;
+    return SST_OK;
+}
+
 sst_status launch_event(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
                         const sst_thresholds *thr, const sst_output *out, cudaStream_t st) {
     const uint32_t nf = ctx->cfg.n_feds;
-    // one pooled block: look-back states (zeroed) + list/mask scratch for FEDs that overflow smem
-    const size_t ents = static_cast<size_t>(ctx->cfg.max_raw_bytes) + 16ull * nf + 64;
-    const size_t mwords = ents / 32 + 2ull * nf + 16;
-    auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
-    const size_t o_state = 0, o_noise = up(sizeof(unsigned long long) * nf), o_mask = o_noise + up(4 * ents),
-                 o_strip = o_mask + up(4 * M_COUNT * mwords), o_adc = o_strip + up(2 * ents), total = o_adc + up(ents);
     uint8_t *blk = nullptr;
-    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), total, ctx->pool, st));
-    SST_CU(cudaMemsetAsync(blk + o_state, 0, sizeof(unsigned long long) * nf, st));
+    uint32_t epoch = 0;
+    const sst_status rc = stream_scratch(ctx, st, &blk, &epoch);
+    if (rc != SST_OK) return rc;
+    const ScratchLayout L = scratch_layout(ctx);
     KParams kp{};
     kp.raw = raw;
     kp.fed_offsets = fed_offsets;
     kp.calib = ctx->calib;
     kp.chan_info = ctx->chan_info;
-    kp.fed_state = reinterpret_cast<unsigned long long *>(blk + o_state);
-    kp.g_noise = reinterpret_cast<float *>(blk + o_noise);
-    kp.g_mask = reinterpret_cast<uint32_t *>(blk + o_mask);
-    kp.g_mask_words = static_cast<uint32_t>(mwords);
-    kp.g_strip = reinterpret_cast<uint16_t *>(blk + o_strip);
-    kp.g_adc = blk + o_adc;
+    kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
+    kp.g_noise = reinterpret_cast<float *>(blk + L.o_noise);
+    kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
+    kp.g_mask_words = static_cast<uint32_t>(L.mwords);
+    kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
+    kp.g_adc = blk + L.o_adc;
     kp.tcl2 = static_cast<double>(thr->cluster) * static_cast<double>(thr->cluster);  // exact
     kp.t_ch = thr->channel;
     kp.t_seed = thr->seed;
     kp.max_raw_bytes = ctx->cfg.max_raw_bytes;
     kp.n_feds = nf;
+    kp.epoch = epoch;
     kp.out = *out;
 #ifdef SST_PHASE_TIMING
     kp.phase_clk = g_phase_clk;
 #endif
     sst_fed_kernel<<<nf, kThreads, sizeof(Smem), st>>>(kp);
     SST_CU(cudaGetLastError());
-    SST_CU(cudaFreeAsync(blk, st));
     return SST_OK;
 }
 
@@ -889,7 +1005,7 @@ void sst_debug_set_phase_clk(unsigned long long *p) { g_phase_clk = p; }
 
 sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (out_ctx) *out_ctx = nullptr;
-    if (!cfg || !out_ctx || cfg->n_feds == 0 || cfg->n_feds > 65535u || cfg->max_raw_bytes == 0)
+    if (!cfg || !out_ctx || cfg->n_feds == 0 || cfg->n_feds > kMaxFeds || cfg->max_raw_bytes == 0)
         return SST_ERR_INVALID_ARG;
     sst_ctx *ctx = new (std::nothrow) sst_ctx();
     if (!ctx) return SST_ERR_INVALID_ARG;
@@ -978,6 +1094,24 @@ sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *
     if (!ctx->has_calib) return SST_ERR_NO_CALIB;
     SST_CU(cudaSetDevice(ctx->cfg.device));
     return launch_event(ctx, raw, fed_offsets, thr, out, static_cast<cudaStream_t>(stream));
+}
+
+sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
+                                    const uint32_t *const *fed_offsets, const sst_thresholds *thr,
+                                    const sst_output *outs, void *const *streams, uint32_t n_streams) {
+    if (!ctx || !raw || !fed_offsets || !thr || !outs || !streams || n_streams == 0 || !thresholds_ok(thr))
+        return SST_ERR_INVALID_ARG;
+    if (!ctx->has_calib) return SST_ERR_NO_CALIB;
+    for (uint32_t e = 0; e < n_events; ++e)
+        if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e]) || (!outs[e].seed_idx && outs[e].cap_seeds))
+            return SST_ERR_INVALID_ARG;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    for (uint32_t e = 0; e < n_events; ++e) {
+        const sst_status rc = launch_event(ctx, raw[e], fed_offsets[e], thr, &outs[e],
+                                           static_cast<cudaStream_t>(streams[e % n_streams]));
+        if (rc != SST_OK) return rc;
+    }
+    return SST_OK;
 }
 
 sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes,
@@ -1090,6 +1224,8 @@ sst_status sst_event_upload(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes
 sst_status sst_destroy(sst_ctx *ctx) {
     if (!ctx) return SST_ERR_INVALID_ARG;
     cudaSetDevice(ctx->cfg.device);
+    cudaDeviceSynchronize();
+    for (auto &sl : ctx->slots) cudaFreeAsync(sl.mem, nullptr);
     cudaDeviceSynchronize();
     if (ctx->calib) cudaFree(ctx->calib);
     if (ctx->chan_info) cudaFree(ctx->chan_info);
