@@ -52,6 +52,10 @@ typedef struct {
     uint32_t max_raw_bytes;        /* every `raw` buffer holds at least this many readable bytes;
                                       a FED whose end offset exceeds it is flagged and empty    */
     uint32_t max_events_in_flight; /* hint for the pool (0 = default 8)                         */
+    uint32_t fed_strips_hint;      /* expected maximum of present (zero-suppressed) strips in one
+                                      FED; sizes the per-FED shared-memory working set.  0 = derive
+                                      it from max_raw_bytes / n_feds.  A FED above the hint is still
+                                      processed correctly, through a slower global-memory path    */
 } sst_config;
 
 /* S/N thresholds of the "three thresholds" algorithm: a strip is active at
@@ -121,17 +125,19 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
  * leftmost-seed ownership, gain correction, cluster threshold, ordered output
  * (PAPER.md:31,33).  raw: DEVICE, 16-byte aligned, >= cfg.max_raw_bytes readable bytes;
  * fed_offsets: DEVICE [n_feds+1] byte offsets of the FEDs in raw (16-byte multiples for the
- * fast path).  thr and out are HOST structs read before the call returns.  The work is
- * enqueued on `stream`; the call does not synchronise.  Scratch comes from the context's
+ * fast path; a FED with start > end or end > cfg.max_raw_bytes is flagged and empty).  thr and
+ * out are HOST structs read before the call returns.  The work is enqueued on `stream` as one
+ * kernel launch; the call does not synchronise.  Scratch comes from the context's
  * stream-ordered pool: one block per stream, allocated on the stream's first event and reused
  * (so a stream must not be driven by two host threads at once). */
 sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
                               const sst_thresholds *thr, const sst_output *out, void *stream);
 
 /* n_events independent events in one call (several events in flight): event e is
- * enqueued on streams[e % n_streams] exactly as sst_unpack_cluster would, with raw[e],
- * fed_offsets[e] (DEVICE) and outs[e].  raw, fed_offsets, outs and streams are HOST arrays read
- * before the call returns.  Does not synchronise. */
+ * enqueued on streams[e % n_streams] with raw[e], fed_offsets[e] (DEVICE) and outs[e]; the
+ * events of one stream share kernel launches (up to sst_info.events_per_launch events each),
+ * and every event's result is exactly what sst_unpack_cluster gives.  raw, fed_offsets, outs and
+ * streams are HOST arrays read before the call returns.  Does not synchronise. */
 sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
                                     const uint32_t *const *fed_offsets, const sst_thresholds *thr,
                                     const sst_output *outs, void *const *streams, uint32_t n_streams);
@@ -167,9 +173,13 @@ sst_status sst_destroy(sst_ctx *ctx);
 int32_t sst_last_cuda_error(const sst_ctx *ctx);
 const char *sst_status_string(sst_status s);
 
-/* Static facts about the compiled kernels, for benchmarks: bytes of dynamic shared memory per
- * CTA, threads per CTA, resident CTAs per SM as reported by the occupancy API, SM count. */
-typedef struct { uint32_t smem_bytes, threads, ctas_per_sm, sm_count, kernels_per_event; } sst_info;
+/* Static facts about the compiled kernel and this context, for benchmarks: bytes of dynamic
+ * shared memory per CTA (one CTA = one warp = one FED at a time), threads per CTA, resident CTAs
+ * per SM as reported by the occupancy API, SM count, kernel launches per event, the part of
+ * smem_bytes that holds a FED's payload and lists, events one launch can take. */
+typedef struct {
+    uint32_t smem_bytes, threads, ctas_per_sm, sm_count, kernels_per_event, slot_bytes, events_per_launch;
+} sst_info;
 sst_status sst_get_info(const sst_ctx *ctx, sst_info *info);
 
 #ifdef __cplusplus

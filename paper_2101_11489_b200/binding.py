@@ -26,7 +26,7 @@ EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_c
 
 class sst_config(C.Structure):
     _fields_ = [("n_feds", C.c_uint32), ("device", C.c_int32), ("max_raw_bytes", C.c_uint32),
-                ("max_events_in_flight", C.c_uint32)]
+                ("max_events_in_flight", C.c_uint32), ("fed_strips_hint", C.c_uint32)]
 
 
 class sst_thresholds(C.Structure):
@@ -44,7 +44,8 @@ class sst_output(C.Structure):
 
 class sst_info(C.Structure):
     _fields_ = [("smem_bytes", C.c_uint32), ("threads", C.c_uint32), ("ctas_per_sm", C.c_uint32),
-                ("sm_count", C.c_uint32), ("kernels_per_event", C.c_uint32)]
+                ("sm_count", C.c_uint32), ("kernels_per_event", C.c_uint32), ("slot_bytes", C.c_uint32),
+                ("events_per_launch", C.c_uint32)]
 
 
 class SSTError(RuntimeError):
@@ -105,9 +106,10 @@ def _ptr(t) -> Optional[int]:
     return t.ctypes.data
 
 
-def sst_create(n_feds: int, device: int = 0, max_raw_bytes: int = 1 << 22, max_events_in_flight: int = 8):
+def sst_create(n_feds: int, device: int = 0, max_raw_bytes: int = 1 << 22, max_events_in_flight: int = 8,
+               fed_strips_hint: int = 0):
     L = load()
-    cfg = sst_config(n_feds, device, max_raw_bytes, max_events_in_flight)
+    cfg = sst_config(n_feds, device, max_raw_bytes, max_events_in_flight, fed_strips_hint)
     ctx = C.c_void_p()
     _check(None, L.sst_create(C.byref(cfg), C.byref(ctx)), "sst_create")
     return ctx

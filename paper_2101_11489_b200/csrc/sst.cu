@@ -1,26 +1,33 @@
 // sst.cu -- libsst: unpack + three-threshold clustering of strip-tracker FED data on B200.
 //
-// One fused kernel per event, one CTA per FED (a FED is 96 channels x 256 strips;
-// modules never cross a FED, reading s10).  After the unpack everything runs in the
-// COMPACT index space of the FED's present strips (the structure of arrays of PAPER.md:31 has
-// one entry per recorded strip), kept in shared memory:
+// One persistent kernel per launch, ONE WARP PER FED (a FED is 96 channels x 256
+// strips; modules never cross a FED, reading s10).  A CTA is a single warp with a
+// ~10 KB shared-memory slot, so ~20 FEDs are in flight per SM and the serial parts of the
+// method (the channel-length chain, the run headers) of one FED hide behind the parallel parts
+// of the others; there is no block-wide barrier anywhere.  Warps draw FEDs from a ticket
+// counter, in (event, FED) order, so a launch takes up to kMaxEv events.
 //
-//   a1 channel-location map : TMA bulk copy of the FED payload to smem, 96-step length chain
-//                             walked in smem (PAPER.md:31 builds this map on the CPU)
-//   a2 unpack               : thread per channel; pass 1 walks the run headers (validate, count),
-//                             a 96-wide scan gives every channel its slot range, pass 2 streams
-//                             the payload bytes into {strip, adc} lists in ascending strip order
-//                             and scatters the ADCs into the zero-filled dense output
-//   a3 flags                : lane per present strip: one 8-byte gather of {noise, gain},
-//                             exact >= tests, masks built with __ballot_sync (no atomics)
-//   a4 seed-index array     : seed mask + block scan; materialised on request
-//   a5 expansion/ownership  : lane per seed: bit scans over a "linked to the previous entry"
-//                             mask; only the leftmost seed of a run goes on
-//   a6 gain corr + accept   : q = min(254, floor(adc/gain + .5)) in float32, Q^2 >= t^2 * sum n^2
-//   a7 ordered output       : block scan + look-back over per-FED aggregates, lane per cluster
+// Per FED, everything after the unpack runs in the COMPACT index space of the FED's present
+// strips (the structure of arrays of PAPER.md:31 has one entry per recorded strip):
 //
-// FEDs whose payload or strip count exceed the smem budgets use the same code on slices of a
-// pooled global scratch buffer.  No tensor cores: nothing here is a contraction.
+//   a1 channel-location map : TMA bulk copy of the FED payload into the slot, the 96-step length
+//                             chain walked in shared memory (PAPER.md:31 builds it on the CPU)
+//   a2 unpack               : lane per channel: pass 1 validates the run headers and counts, a
+//                             warp scan gives every channel its slot range, pass 2 writes the
+//                             {strip, adc} lists in ascending strip order
+//   a3 flags                : lane per present strip: one 8-byte gather of {noise, gain} (64-byte
+//                             L2 fetch), exact >= tests, masks by __ballot_sync, dense SoA scatter
+//   a4 seed-index array     : seed mask + ordered compaction; materialised on request
+//   a5 expansion/ownership  : bit-parallel flood fill of the seed mask down the link mask, lane
+//                             per 32 entries: marks the head of every run that holds a seed, so
+//                             each candidate is evaluated once, by (the lane of) its leftmost seed
+//   a6 gain corr + accept   : q = min(254, floor(adc/gain + .5)) in float32; lane per candidate:
+//                             Q^2 >= t^2 * sum n^2 with the double sum taken left to right
+//   a7 ordered output       : FED aggregate published in one 64-bit word, every FED sums the
+//                             words of its predecessors (one round trip), lane per cluster emit
+//
+// FEDs whose payload or lists exceed the slot run the same code on a pooled global scratch.
+// No tensor cores: nothing here is a contraction.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -37,77 +44,55 @@
 
 namespace {
 
-constexpr int kThreads = 256;
-constexpr int kWarps = kThreads / 32;
 constexpr int kChan = 96;
 constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
-constexpr int kListCap = 4096;              // present strips per FED kept in smem
-constexpr int kRawCap = 4 * kListCap;       // FED payload staged in smem (region reused for noise)
-constexpr int kMaskWords = kListCap / 32 + 1;
-constexpr int kRunCap = 2048;               // run-table slots (FED payloads up to ~6 KB)
-constexpr int kInline = 8;                  // runs up to this length are copied by one thread
-constexpr int kLongQ = 96;
-constexpr int kWide = 32;                   // clusters wider than this are summed by a warp
-constexpr int kWideQ = 32;
-enum { M_ACT = 0, M_SEED, M_BRK, M_LINK, M_ACC, M_WTOT, M_COUNT };
+constexpr int kMaxEv = 8;                   // events per launch
+constexpr int kQCap = 256;                  // candidate / cluster queue (entries)
+constexpr int kWide = 48;                   // candidates wider than this are summed by the warp
+constexpr int kU = 4;                       // mask words per batch of the flag pass (loads in flight)
+constexpr uint32_t kFull = 0xffffffffu;
+constexpr uint32_t kMaxFeds = 4096;
 
-// per-FED aggregate published for the look-back (one 64-bit word)
-// look-back state, two 64-bit words per FED, living in a per-stream scratch that is never cleared:
-// every word carries the 8-bit epoch of the call that wrote it and counts only if that matches.
-// Word 0: status (bits 62-63: 1 = aggregate, 2 = inclusive prefix) | epoch (bits 54-61) | clusters
-// (26 bits) | ADC bytes << 26 (28 bits).  Word 1, aggregate only: ready (bit 63) | epoch (bits 55-62)
-// | seeds (20 bits) | malformed channels << 20 (7 bits) | overrun << 27.
-constexpr unsigned long long kStA = 1ull << 62, kStP = 2ull << 62, kStMask = (1ull << 54) - 1;
-constexpr int kShEp0 = 54, kShEp1 = 55, kShAdc = 26;
-constexpr int kShMalf = 20, kShOvr = 27;
-constexpr unsigned long long kReady = 1ull << 63;
-constexpr uint32_t kMaxFeds = 4096;  // keeps event totals inside the 26/28-bit prefix fields
+// Published FED aggregate, one 64-bit word: epoch (12 bits, never 0) << 52 | overrun << 51 |
+// malformed channels (7) << 44 | seeds (15) << 29 | cluster ADC bytes (15) << 14 | clusters (14).
+// A word counts only if its epoch is the launch's; the host clears the array when the epoch wraps.
+constexpr int kShEpoch = 52, kShOver = 51, kShMalf = 44, kShSeed = 29, kShAdc = 14;
+constexpr uint32_t kEpochMax = 4095;
 
-struct __align__(128) Smem {
-    union {                       // the payload is dead once the lists are built
-        uint8_t raw[kRawCap];     // FED payload (TMA destination)
-        float noise[kListCap];    // noise of entry i
-    } u;
-    uint16_t strip[kListCap];     // FED-local strip id of entry i, ascending
-    uint8_t adc[kListCap];        // raw ADC, replaced by the corrected ADC at active entries
-    uint32_t mask[M_COUNT][kMaskWords];
-    alignas(16) uint32_t runs[kRunCap];  // one record per run, slot = (runs of earlier channels' bound) + ordinal
-    uint32_t mod_id[kChan];
-    uint32_t chan_off[kChan];     // FED-local byte offset of the first run byte
-    uint16_t chan_len[kChan];
-    uint16_t chan_base[kChan];    // first list entry of the channel
-    uint16_t slot_base[kChan + 1];
-    uint8_t mod_lo[kChan], mod_hi[kChan];  // first channel / end channel of the channel's module
-    uint32_t okmask[3];
-    uint32_t wscan[2][kWarps];
-    uint32_t red[5][kWarps];
-    uint32_t wide_q[kWideQ];
-    uint16_t long_q[kLongQ];
-    unsigned long long mbar;
-    uint32_t wide_count, long_count;
-    uint32_t fed_start, fed_size, in_smem, overrun;
+struct EventDesc {
+    const uint8_t *raw;
+    const uint32_t *fed_offsets;
+    sst_output out;
 };
 
 struct KParams {
-    const uint8_t *raw;
-    const uint32_t *fed_offsets;
     const float2 *calib;     // {noise (+inf at bad strips), gain} per strip
     const uint2 *chan_info;  // {module id, first channel | end channel << 8 of the module}
-    unsigned long long *fed_state;
-    // global scratch for FEDs that do not fit the smem lists (sliced by FED offset)
+    unsigned long long *fed_state;  // [kMaxEv][n_feds]
+    unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+grid)
+    unsigned long long ticket_base;
+    // global scratch of the slow path, one slice set per event
+    float *g_noise;
     uint16_t *g_strip;
     uint8_t *g_adc;
-    float *g_noise;
-    uint32_t *g_mask;  // M_COUNT arrays of g_mask_words
-    uint32_t g_mask_words;
+    uint32_t *g_mask;  // 4 arrays of g_mwords per event
+    uint32_t g_ents, g_mwords;
     double tcl2;
     float t_ch, t_seed;
-    uint32_t max_raw_bytes, n_feds;
-    uint32_t epoch;  // 1..255, changes on every use of the scratch
-    sst_output out;
+    uint32_t max_raw_bytes, n_feds, n_events, epoch, slot_bytes;
     unsigned long long *phase_clk;  // debug builds only (SST_PHASE_TIMING)
+    EventDesc ev[kMaxEv];
 };
+
+// per-warp shared memory: fixed header, then the slot (payload stage, later the lists and masks)
+struct __align__(16) Hdr {
+    unsigned long long mbar;
+    uint32_t chan_off[kChan];  // FED-local byte offset of the channel's first run byte
+    uint16_t chan_len[kChan];
+    uint16_t queue[kQCap];
+};
+constexpr uint32_t kHdrBytes = (sizeof(Hdr) + 127u) & ~127u;
 
 // ------------------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_addr(const void *p) {
@@ -125,11 +110,11 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t pari
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
+        "WAIT_LOOP_%=:\n"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
+        "@p bra WAIT_DONE_%=;\n"
+        "bra WAIT_LOOP_%=;\n"
+        "WAIT_DONE_%=:\n"
         "}\n" ::"r"(smem_addr(bar)),
         "r"(parity)
         : "memory");
@@ -139,11 +124,11 @@ __device__ __forceinline__ void fence_proxy_async() {
 }
 // TMA bulk copy global -> shared (non-tensor form), completion on an mbarrier
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes,
-                                         unsigned long long *bar) {
+                                         unsigned long long *bar, unsigned long long pol) {
     asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::
             "r"(smem_addr(dst)),
-        "l"(src), "r"(bytes), "r"(smem_addr(bar))
+        "l"(src), "r"(bytes), "r"(smem_addr(bar)), "l"(pol)
         : "memory");
 }
 __device__ __forceinline__ unsigned long long ld_state(const unsigned long long *p) {
@@ -153,6 +138,50 @@ __device__ __forceinline__ unsigned long long ld_state(const unsigned long long 
 }
 __device__ __forceinline__ void st_state(unsigned long long *p, unsigned long long v) {
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// L2 residency.  The calibration (8 B per strip, 86.5 MB for 440 FEDs) is read by every event and
+// fits the L2 set-aside that sst_create reserves, while raw data and outputs stream through once:
+// calibration loads carry an evict_last policy, everything else that touches HBM evict_first.
+__device__ __forceinline__ unsigned long long policy_evict_last() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ unsigned long long policy_evict_first() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// Calibration gather.  On B200 a plain load that misses L2 pulls the whole 128-byte line from
+// DRAM; the .L2::64B qualifier halves that (measured, profiles/r01_v4.md), and nothing is reused
+// through L1.
+__device__ __forceinline__ float2 ld_calib(const float2 *p, unsigned long long pol) {
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.L2::64B.v2.f32 {%0,%1}, [%2], %3;"
+                 : "=f"(v.x), "=f"(v.y)
+                 : "l"(p), "l"(pol));
+    return v;
+}
+// streaming stores of the outputs
+__device__ __forceinline__ void st_stream(uint4 *p, uint4 v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void st_stream(uint8_t *p, uint32_t v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.u8 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_stream(uint16_t *p, uint32_t v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.u16 [%0], %1, %2;" ::"l"(p), "h"(static_cast<unsigned short>(v)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_stream(uint32_t *p, uint32_t v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.u32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_stream(int32_t *p, int32_t v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.s32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_stream(float *p, float v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v), "l"(pol) : "memory");
 }
 
 // ------------------------------------------------------------------------------ arithmetic
@@ -164,57 +193,85 @@ __device__ __forceinline__ bool ge_exact(float a, float t, float n) {
     return (a > p) || (a == p && e <= 0.0f);
 }
 // min(254, floor(fl32(fl32(adc / gain) + 0.5)))  (IEEE RN division and add, no contraction)
-__device__ __noinline__ uint32_t gain_correct(uint32_t adc, float gain) {
-    const float u = __fadd_rn(__fdiv_rn(static_cast<float>(adc), gain), 0.5f);
+__device__ __forceinline__ uint32_t gain_correct(float adc, float gain) {
+    const float u = __fadd_rn(__fdiv_rn(adc, gain), 0.5f);
     const float fl = floorf(u);
     return fl >= 254.0f ? 254u : static_cast<uint32_t>(fl);
 }
 
 __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+__device__ __forceinline__ unsigned long long warp_sum64(unsigned long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
     return v;
 }
 __device__ __forceinline__ double warp_sum_d(double v) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, int lane) {
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(kFull, v, d);
+        if (lane >= d) v += u;
+    }
     return v;
 }
 
 // Entry i is "linked" when it continues the cluster candidate of entry i-1 (both active, strips
 // adjacent inside one module).  The last entry of the run that contains entry i: one before the
-// next unlinked entry.  link[] has a zero sentinel word after the last used word.
+// next unlinked entry.  link[] has zero sentinel words after the last used word.
 __device__ __forceinline__ int run_end(const uint32_t *link, int i) {
     int w = i >> 5;
     const int b = i & 31;
-    uint32_t nl = ~link[w] & (b == 31 ? 0u : (0xffffffffu << (b + 1)));
+    uint32_t nl = ~link[w] & (b == 31 ? 0u : (kFull << (b + 1)));
     while (nl == 0) nl = ~link[++w];
     return (w << 5) + __ffs(nl) - 2;
 }
 
-// Cluster acceptance for a narrow candidate, one thread: Q^2 >= t_cl^2 * n2 with n2 the double
-// sum of noise^2 taken strictly left to right (reading s15).
+// x |= every entry from which a set entry of x is reached by walking up through linked entries
+// (bit j of l: entry j continues entry j-1).  Kogge-Stone fill, five doubling steps.
+__device__ __forceinline__ uint32_t fill_down(uint32_t x, uint32_t l) {
+    x |= (x & l) >> 1;
+    l &= l << 1;
+    x |= (x & l) >> 2;
+    l &= l << 2;
+    x |= (x & l) >> 4;
+    l &= l << 4;
+    x |= (x & l) >> 8;
+    l &= l << 8;
+    x |= (x & l) >> 16;
+    return x;
+}
+
+// Cluster acceptance for a narrow candidate, one lane: Q^2 >= t_cl^2 * n2 with n2 the double sum
+// of noise^2 taken strictly left to right (reading s15; noise^2 is exact in double, so
+// the fused multiply-add below rounds exactly like the oracle's separate multiply and add).
 __device__ __forceinline__ bool accept_serial(const uint8_t *q, const float *noise, int l, int w, double tcl2) {
     int Q = 0;
     double n2 = 0.0;
-    #pragma unroll 1
+#pragma unroll 1
     for (int i = 0; i < w; ++i) {
         Q += q[l + i];
         const double d = static_cast<double>(noise[l + i]);
-        n2 = __dadd_rn(n2, __dmul_rn(d, d));
+        n2 = __fma_rn(d, d, n2);
     }
     const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
     return lhs >= __dmul_rn(tcl2, n2);
 }
 
-// The same decision for a wide candidate by one warp.  A pairwise double sum differs from the
-// sequential one by at most ~w*2^-52 relative; the decision is taken from it only when the two
-// sides are further apart than that, otherwise lane 0 redoes the sum sequentially.
-__device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, int l, int w, double tcl2,
-                                         int lane) {
+// The same decision for a wide candidate by the whole warp.  A pairwise double sum differs from
+// the sequential one by at most ~w*2^-52 relative; the decision is taken from it only when the
+// two sides are further apart than that, otherwise lane 0 redoes the sum sequentially.
+__device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, int l, int w, double tcl2, int lane) {
     uint32_t Q = 0;
     double n2p = 0.0;
-    #pragma unroll 1
+#pragma unroll 1
     for (int i = lane; i < w; i += 32) {
         Q += q[l + i];
         const double d = static_cast<double>(noise[l + i]);
@@ -228,14 +285,14 @@ __device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, i
     if (!(fabs(lhs - rhs) > rhs * static_cast<double>(w) * 0x1p-50)) {
         if (lane == 0) {
             double n2 = 0.0;
-            #pragma unroll 1
+#pragma unroll 1
             for (int i = 0; i < w; ++i) {
                 const double d = static_cast<double>(noise[l + i]);
-                n2 = __dadd_rn(n2, __dmul_rn(d, d));
+                n2 = __fma_rn(d, d, n2);
             }
             ok = lhs >= __dmul_rn(tcl2, n2);
         }
-        ok = __shfl_sync(0xffffffffu, ok, 0);
+        ok = __shfl_sync(kFull, ok, 0);
     }
     return ok != 0;
 }
@@ -246,475 +303,460 @@ __device__ __noinline__ float cluster_snr(const float *noise, int l, int w, int 
 #pragma unroll 1
     for (int i = 0; i < w; ++i) {
         const double d = static_cast<double>(noise[l + i]);
-        n2 = __dadd_rn(n2, __dmul_rn(d, d));
+        n2 = __fma_rn(d, d, n2);
     }
     return static_cast<float>(static_cast<double>(Q) / sqrt(n2));
 }
 
 // ------------------------------------------------------------------------------ raw payload
-// Loops that read the raw bytes are instantiated on the smem stage (LDS) and on the generic
-// global pointer (oversized or unaligned FEDs).
-
-// a1: the channel-length chain of one FED, checked as it goes (generic path).
-__device__ __forceinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
-                                                   uint16_t *chan_len, uint16_t *slot_base) {
-    uint32_t pos = 0, slots = 0;
+// a1, generic path (payload not staged): the channel-length chain of one FED, checked as it goes.
+__device__ __noinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
+                                                uint16_t *chan_len) {
+    uint32_t pos = 0;
     int c = 0;
     if (!over) {
-        #pragma unroll 1
+#pragma unroll 1
         for (; c < kChan; ++c) {
             if (pos + 2 > fed_size) break;
             const uint32_t l16 = rp[pos] | (static_cast<uint32_t>(rp[pos + 1]) << 8);
             if (pos + 2 + l16 > fed_size) break;
             chan_off[c] = pos + 2;
             chan_len[c] = static_cast<uint16_t>(l16);
-            slot_base[c] = static_cast<uint16_t>(min(slots, 0xffffu));
-            slots += l16 / 3;
             pos += 2 + l16;
         }
     }
     over = c < kChan;
-    #pragma unroll 1
+#pragma unroll 1
     for (; c < kChan; ++c) {  // channels behind an overrun are empty, recorded at the FED end
         chan_off[c] = fed_size;
         chan_len[c] = 0;
-        slot_base[c] = static_cast<uint16_t>(min(slots, 0xffffu));
     }
-    slot_base[kChan] = static_cast<uint16_t>(min(slots, 0xffffu));
     return over;
 }
 
-// a1, smem stage: the same chain walked speculatively -- no bounds checks inside the serial
-// loop (addresses wrap inside the stage), the 96 results are validated in parallel afterwards.
-__device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uint32_t *chan_off, uint16_t *chan_len,
-                                                       uint16_t *slot_base) {
-    uint32_t pos = 0, slots = 0;
-#pragma unroll 4
+// a1, staged payload: the same chain walked speculatively by one lane -- no bounds checks inside
+// the serial loop (reads are clamped into the slot), the 96 results are validated in parallel.
+__device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uint32_t clamp, uint32_t *chan_off,
+                                                       uint16_t *chan_len) {
+    uint32_t pos = 0;
+#pragma unroll 8
     for (int c = 0; c < kChan; ++c) {
-        const uint32_t a = pos & (kRawCap - 1);
-        const uint32_t l16 = stage[a] | (static_cast<uint32_t>(stage[(a + 1) & (kRawCap - 1)]) << 8);
+        const uint32_t a = min(pos, clamp);
+        const uint32_t l16 = stage[a] | (static_cast<uint32_t>(stage[a + 1]) << 8);
         chan_off[c] = pos + 2;
         chan_len[c] = static_cast<uint16_t>(l16);
-        slot_base[c] = static_cast<uint16_t>(min(slots, 0xffffu));
-        slots += l16 / 3;
         pos += 2 + l16;
     }
-    slot_base[kChan] = static_cast<uint16_t>(min(slots, 0xffffu));
 }
 
-// a2 pass 1: validate one channel's run list (reading s2b), count its strips and, when
-// the run table is in use, leave one record per run: strips before | first << 8 | (len-1) << 16
-// | channel << 24 | valid << 31.  Returns false for a malformed channel.
-__device__ __forceinline__ bool scan_runs(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t chan,
-                                          uint32_t *slots, uint32_t &n_runs, uint32_t &n_strips) {
-    uint32_t q = off, next_free = 0, k = 0, within = 0;
+// a2 pass 1: validate one channel's run list (reading s2b) and count its strips.
+// Returns false for a malformed channel.
+__device__ __forceinline__ bool scan_runs(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t &n_strips) {
+    uint32_t q = off, next_free = 0, within = 0;
     const uint32_t qend = off + len_bytes;
     bool ok = true;
-    #pragma unroll 1
+#pragma unroll 1
     while (q < qend) {
         if (q + 2 > qend) { ok = false; break; }
         const uint32_t first = rp[q];
         uint32_t len = rp[q + 1];
         if (len == 0) len = 256;  // reading s2
         if (first < next_free || first + len > kStrip || q + 2 + len > qend) { ok = false; break; }
-        if (slots) slots[k] = within | (first << 8) | ((len - 1) << 16) | (chan << 24) | 0x80000000u;
         next_free = first + len;
         q += 2 + len;
         within += len;
-        ++k;
     }
-    n_runs = k;
     n_strips = within;
     return ok;
 }
 
-// a2 pass 2, fallback without the run table: stream one (validated) channel byte by byte.
-__device__ __forceinline__ void stream_channel(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t k,
-                                               int chan, uint16_t *strip_l, uint8_t *adc_l, uint8_t *dense) {
-    uint32_t rem = 0, tgt = 0, hdr = 0;
-    const uint32_t qend = off + len_bytes;
-    #pragma unroll 1
-    for (uint32_t q = off; q < qend; ++q) {
-        const uint32_t b = rp[q];
-        if (rem) {
-            strip_l[k] = static_cast<uint16_t>(chan * kStrip + tgt);
-            adc_l[k] = static_cast<uint8_t>(b);
-            if (dense) dense[chan * kStrip + tgt] = static_cast<uint8_t>(b);
-            ++k; ++tgt; --rem;
-        } else if (!hdr) {
-            tgt = b;
-            hdr = 1;
-        } else {
-            rem = b ? b : 256u;
-            hdr = 0;
-        }
-    }
-}
-
 #ifdef SST_PHASE_TIMING
-#define SST_MARK(k) do { if (threadIdx.x == 0 && p.phase_clk) p.phase_clk[blockIdx.x * 16 + (k)] = clock64(); } while (0)
+#define SST_MARK(k) do { if (lane == 0 && p.phase_clk) p.phase_clk[static_cast<size_t>(ticket) * 16 + (k)] = clock64(); } while (0)
 #else
 #define SST_MARK(k) do { } while (0)
 #endif
 
+struct FedCtx {
+    uint32_t ticket, ev, f;
+    uint32_t fo0;                 // the FED's start offset as given (reported in chan_off)
+    uint32_t fed_start, fed_size;  // what is read: [fed_start, +fed_size), empty for a bad FED
+    uint32_t overrun, n_malformed;
+    uint32_t P;
+    uint32_t off[3], len[3], base[3];  // of channels lane, lane+32, lane+64
+    uint32_t opens;                    // bit k: channel lane+32k opens a module
+};
+
 // ------------------------------------------------------------------------------ lists -> clusters
-// Everything after the channel walk, on the FED's lists of present strips.  kSmem = true: lists
-// and masks in shared memory (LDS/STS); false: in this FED's slice of the global scratch.
-template <bool kSmem>
-__device__ __noinline__ void lists_to_clusters(const KParams &p, Smem &s, const uint8_t *rp, const uint32_t P,
-                                                  const bool table_ok, const uint32_t n_slots,
-                                                  const uint32_t n_malformed, const uint32_t my_off,
-                                                  const uint32_t my_len, const uint32_t my_base) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t f = blockIdx.x;
-    const sst_output &o = p.out;
+// Everything after pass 1, on the FED's lists of present strips, by one warp.  kFast: lists and
+// masks live in the warp's shared-memory slot (LDS/STS) and the payload is staged there; else
+// lists and masks live in this FED's slice of the global scratch and rp is a generic pointer.
+template <bool kFast>
+__device__ __forceinline__ void fed_lists(const KParams &p, Hdr &h, uint8_t *slot, const uint8_t *rp,
+                                          const FedCtx &c, const int lane, uint32_t &next_ticket) {
+    const uint32_t f = c.f, P = c.P, ticket = c.ticket;
+    const EventDesc &E = p.ev[c.ev];
+    const sst_output &o = E.out;
     const uint32_t nw = (P + 31) >> 5;  // mask words in use
-    const uint32_t slice = ((s.fed_start + 15u) & ~15u) + 16u * f;
-    uint16_t *const strip_l = kSmem ? s.strip : p.g_strip + slice;
-    uint8_t *const adc_l = kSmem ? s.adc : p.g_adc + slice;
-    float *const noise_l = kSmem ? s.u.noise : p.g_noise + slice;
-    uint32_t *const mbase = kSmem ? &s.mask[0][0] : p.g_mask + (slice >> 5) + 2u * f;
-    const uint32_t mstride = kSmem ? static_cast<uint32_t>(kMaskWords) : p.g_mask_words;
-#define MASK(k) (mbase + (k) * mstride)
+    const uint32_t lt = (1u << lane) - 1u;
+    (void)ticket;
+
+    float *noise_l;
+    uint16_t *strip_l;
+    uint8_t *adc_l;
+    uint32_t *mS, *mL, *mH, *mX;
+    if (kFast) {
+        const uint32_t A = (max((c.fed_size + 15u) & ~15u, 4u * P) + 15u) & ~15u;
+        noise_l = reinterpret_cast<float *>(slot);  // overlays the payload once the lists are built
+        strip_l = reinterpret_cast<uint16_t *>(slot + A);
+        adc_l = slot + A + 2u * P;
+        mS = reinterpret_cast<uint32_t *>(slot + ((A + 3u * P + 3u) & ~3u));
+        mL = mS + (nw + 2);
+        mH = mL + (nw + 2);
+        mX = mH + (nw + 2);
+    } else {
+        const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
+        const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
+        noise_l = p.g_noise + eb + slice;
+        strip_l = p.g_strip + eb + slice;
+        adc_l = p.g_adc + eb + slice;
+        mS = p.g_mask + static_cast<size_t>(c.ev) * 4u * p.g_mwords + (slice >> 5) + 4u * f;
+        mL = mS + p.g_mwords;
+        mH = mL + p.g_mwords;
+        mX = mH + p.g_mwords;
+    }
     uint8_t *const dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips : nullptr;
 
-    // ---------------------------------------------------------------- a2 pass 2: thread per run
-    if (table_ok) {
-        #pragma unroll 1
-        for (uint32_t slot = tid; slot < n_slots; slot += kThreads) {
-            const uint32_t rec = s.runs[slot];
-            if (!(rec >> 31)) continue;
-            const uint32_t c = (rec >> 24) & 127u, within = rec & 255u, first = (rec >> 8) & 255u,
-                           len = ((rec >> 16) & 255u) + 1u;
-            if (len > kInline) {
-                const uint32_t qi = atomicAdd(&s.long_count, 1u);
-                if (qi < kLongQ) { s.long_q[qi] = static_cast<uint16_t>(slot); continue; }
+    // ---------------------------------------------------------------- a2 pass 2: lane per channel
+    // writes {strip, adc} in ascending strip order; bit 15 of a strip id marks strip 0 of a channel
+    // that opens a module (nothing links across it)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        uint32_t q = c.off[k], e = c.base[k];
+        const uint32_t qend = q + c.len[k];
+        const uint32_t g0 = static_cast<uint32_t>(lane + 32 * k) * kStrip;
+        const uint32_t open_bit = ((c.opens >> k) & 1u) << 15;
+#pragma unroll 1
+        while (q < qend) {
+            const uint32_t first = rp[q];
+            uint32_t len = rp[q + 1];
+            if (len == 0) len = 256;
+            // most runs hold one or two strips; on the fast path the second byte is read
+            // unconditionally (it is inside the slot or its 16-byte tail pad)
+            const uint32_t b0 = rp[q + 2], b1 = (kFast || len > 1) ? rp[q + 3] : 0u;
+            const uint32_t sid = g0 + first;
+            strip_l[e] = static_cast<uint16_t>(first == 0 ? sid | open_bit : sid);
+            adc_l[e] = static_cast<uint8_t>(b0);
+            if (len > 1) {
+                strip_l[e + 1] = static_cast<uint16_t>(sid + 1u);
+                adc_l[e + 1] = static_cast<uint8_t>(b1);
             }
-            const uint32_t src = s.chan_off[c] + within + 2u * (slot - s.slot_base[c] + 1u);
-            const uint32_t dst = s.chan_base[c] + within, g = c * kStrip + first;
-            #pragma unroll 1
-            for (uint32_t i = 0; i < len; ++i) {
-                const uint8_t b = rp[src + i];
-                strip_l[dst + i] = static_cast<uint16_t>(g + i);
-                adc_l[dst + i] = b;
-                if (dense) dense[g + i] = b;
+#pragma unroll 1
+            for (uint32_t i = 2; i < len; ++i) {
+                strip_l[e + i] = static_cast<uint16_t>(sid + i);
+                adc_l[e + i] = rp[q + 2 + i];
             }
+            e += len;
+            q += 2 + len;
         }
-        __syncthreads();
-        const uint32_t nq = min(s.long_count, static_cast<uint32_t>(kLongQ));
-        #pragma unroll 1
-        for (uint32_t e = warp; e < nq; e += kWarps) {  // long runs: one warp each, lane per byte
-            const uint32_t slot = s.long_q[e], rec = s.runs[slot];
-            const uint32_t c = (rec >> 24) & 127u, within = rec & 255u, first = (rec >> 8) & 255u,
-                           len = ((rec >> 16) & 255u) + 1u;
-            const uint32_t src = s.chan_off[c] + within + 2u * (slot - s.slot_base[c] + 1u);
-            const uint32_t dst = s.chan_base[c] + within, g = c * kStrip + first;
-            #pragma unroll 1
-            for (uint32_t i = lane; i < len; i += 32) {
-                const uint8_t b = rp[src + i];
-                strip_l[dst + i] = static_cast<uint16_t>(g + i);
-                adc_l[dst + i] = b;
-                if (dense) dense[g + i] = b;
-            }
-        }
-    } else if (tid < kChan && my_len) {
-        stream_channel(rp, my_off, my_len, my_base, tid, strip_l, adc_l, dense);
+        __syncwarp();
     }
-    __syncthreads();  // lists complete; the payload (smem union) is dead from here on
+    __syncwarp();  // lists complete; the payload is dead from here on
+
+    SST_MARK(4);
+    // ---------------------------------------------------------------- a3: active / seed flags
+    // lane per entry, a warp covers one mask word per step, so the masks come from ballots; kU
+    // words per batch keep kU calibration gathers in flight per lane
+    const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
+    const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
+    {
+        uint32_t carry_sv = 0xffffu, carry_act = 0;
+        uint32_t filled = 0;  // the dense output is zero up to here (multiple of 16)
+        const bool dense16 = (reinterpret_cast<uintptr_t>(dense) & 15u) == 0;
+        auto fill_to = [&](uint32_t upto) {
+            if (dense16) {
+#pragma unroll 1
+                for (uint32_t b = filled + 16u * lane; b < upto; b += 512u)
+                    st_stream(reinterpret_cast<uint4 *>(dense + b), make_uint4(0, 0, 0, 0), pol_first);
+            } else {
+#pragma unroll 1
+                for (uint32_t b = filled + lane; b < upto; b += 32u) dense[b] = 0;
+            }
+            filled = upto;
+            __syncwarp();
+        };
+#pragma unroll 1
+        for (uint32_t w0 = 0; w0 < nw; w0 += kU) {
+            uint32_t sv[kU], av[kU];
+            float2 cv[kU];
+#pragma unroll
+            for (int j = 0; j < kU; ++j) {
+                const uint32_t i = (w0 + j) * 32u + lane;
+                const bool valid = i < P;
+                sv[j] = valid ? strip_l[i] : 0xffffu;
+                av[j] = valid ? adc_l[i] : 0u;
+            }
+#pragma unroll
+            for (int j = 0; j < kU; ++j)
+                cv[j] = av[j] ? ld_calib(cal + (sv[j] & 0x7fffu), pol_last) : make_float2(INFINITY, 1.0f);
+            if (dense) {
+                // zero-fill the dense output up to the last strip of this batch (to the FED's end in
+                // the last batch), just ahead of the scatter below: both hit the same L2 lines
+                const uint32_t i_last = min(P, (w0 + kU) * 32u) - 1u;
+                fill_to((w0 + kU) * 32u >= P ? static_cast<uint32_t>(kFedStrips)
+                                             : ((strip_l[i_last] & 0x7fffu) + 16u) & ~15u);
+            }
+#pragma unroll
+            for (int j = 0; j < kU; ++j) {
+                if (w0 + j >= nw) break;  // warp-uniform
+                const uint32_t i = (w0 + j) * 32u + lane;
+                const bool valid = sv[j] != 0xffffu;
+                const uint32_t s15 = sv[j] & 0x7fffu;
+                if (dense && valid) st_stream(dense + s15, av[j], pol_first);
+                const float af = static_cast<float>(av[j]);
+                const bool is_act = av[j] != 0 && ge_exact(af, p.t_ch, cv[j].x);
+                const bool is_seed = is_act && ge_exact(af, p.t_seed, cv[j].x);
+                uint32_t p_sv = __shfl_up_sync(kFull, sv[j], 1);
+                uint32_t p_act = __shfl_up_sync(kFull, static_cast<uint32_t>(is_act), 1);
+                if (lane == 0) { p_sv = carry_sv; p_act = carry_act; }
+                // this entry continues the candidate of the previous one
+                const bool is_link = is_act && p_act && !(sv[j] & 0x8000u) && s15 == (p_sv & 0x7fffu) + 1u;
+                const uint32_t wa = __ballot_sync(kFull, is_act);
+                const uint32_t ws = __ballot_sync(kFull, is_seed);
+                const uint32_t wl = __ballot_sync(kFull, is_link);
+                if (valid) {
+                    noise_l[i] = cv[j].x;
+                    if (is_act) adc_l[i] = static_cast<uint8_t>(gain_correct(af, cv[j].y));
+                }
+                if (lane == 0) {
+                    mS[w0 + j] = ws;
+                    mL[w0 + j] = wl;
+                    mH[w0 + j] = wa & ~wl;  // heads: active entries that start a candidate
+                }
+                carry_sv = __shfl_sync(kFull, sv[j], 31);
+                carry_act = __shfl_sync(kFull, static_cast<uint32_t>(is_act), 31);
+            }
+        }
+        if (dense && filled < static_cast<uint32_t>(kFedStrips)) fill_to(kFedStrips);  // a FED without strips
+        if (lane < 2) {  // zero sentinels behind the last word
+            mS[nw + lane] = 0;
+            mL[nw + lane] = 0;
+            mH[nw + lane] = 0;
+            mX[nw + lane] = 0;
+        }
+    }
+    __syncwarp();
 
     SST_MARK(5);
-    // ---------------------------------------------------------------- a3: active / seed flags
-    // lane per entry; a warp covers one mask word per step, so the masks come from ballots
-    const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
-    #pragma unroll 1
-    for (uint32_t base = 0; base < nw * 32; base += kThreads * 2) {
-        uint32_t idx[2], sv[2], av[2], sp[2];
-        float2 cv[2];
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            idx[j] = base + j * kThreads + tid;
-            const bool valid = idx[j] < P;
-            sv[j] = valid ? strip_l[idx[j]] : 0u;
-            av[j] = valid ? adc_l[idx[j]] : 0u;
-            sp[j] = (valid && idx[j] > 0) ? strip_l[idx[j] - 1] : 0xffffu;
-        }
-#pragma unroll
-        for (int j = 0; j < 2; ++j) cv[j] = av[j] ? __ldg(cal + sv[j]) : make_float2(INFINITY, 1.0f);
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            if ((base + j * kThreads + warp * 32) >= nw * 32) continue;  // warp-uniform
-            const float af = static_cast<float>(av[j]);
-            const bool is_act = av[j] != 0 && ge_exact(af, p.t_ch, cv[j].x);
-            const bool is_seed = is_act && ge_exact(af, p.t_seed, cv[j].x);
-            const uint32_t ch = sv[j] >> 8;
-            // a new candidate must start here if the previous entry is not the strip to the left
-            // or this strip opens a module
-            const bool is_brk = sv[j] != sp[j] + 1u || ((sv[j] & 255u) == 0 && s.mod_lo[ch] == ch);
-            if (idx[j] < P) {
-                noise_l[idx[j]] = cv[j].x;
-                if (is_act) adc_l[idx[j]] = static_cast<uint8_t>(gain_correct(av[j], cv[j].y));
-            }
-            const uint32_t wa = __ballot_sync(0xffffffffu, is_act);
-            const uint32_t ws = __ballot_sync(0xffffffffu, is_seed);
-            const uint32_t wb = __ballot_sync(0xffffffffu, is_brk);
-            if (lane == 0) {
-                const uint32_t w = idx[j] >> 5;
-                MASK(M_ACT)[w] = wa; MASK(M_SEED)[w] = ws; MASK(M_BRK)[w] = wb;
+    // ---------------------------------------------------------------- a4/a5: seeds -> candidates
+    // lane per mask word: X = entries with a seed at or above them in their run (flood fill of
+    // the seed mask down the links); a head in X starts a candidate that holds a seed.  Runs that
+    // cross a word boundary hand the fill to the word below until nothing changes.
+    uint32_t n_seed = 0;
+#pragma unroll 1
+    for (uint32_t w = lane; w < nw; w += 32) {
+        const uint32_t s = mS[w];
+        n_seed += __popc(s);
+        mX[w] = fill_down(s, mL[w]);
+    }
+    __syncwarp();
+    for (;;) {
+        bool changed = false;
+#pragma unroll 1
+        for (uint32_t w = lane; w < nw; w += 32) {
+            const uint32_t cin = mX[w + 1] & mL[w + 1] & 1u;
+            const uint32_t x = mX[w];
+            if (cin && !(x >> 31)) {
+                mX[w] = fill_down(x | 0x80000000u, mL[w]);
+                changed = true;
             }
         }
+        __syncwarp();
+        if (!__any_sync(kFull, changed)) break;
     }
-    __syncthreads();
-    #pragma unroll 1
-    for (uint32_t w = tid; w <= nw; w += kThreads) {  // link mask (+ zero sentinel word), clear acc
-        uint32_t lk = 0;
-        if (w < nw) {
-            const uint32_t a = MASK(M_ACT)[w];
-            const uint32_t carry = w ? (MASK(M_ACT)[w - 1] >> 31) : 0u;
-            lk = a & ((a << 1) | carry) & ~MASK(M_BRK)[w];
-        } else {
-            MASK(M_SEED)[w] = 0;
-        }
-        MASK(M_LINK)[w] = lk;
-        MASK(M_ACC)[w] = 0;
-        MASK(M_WTOT)[w] = 0;
-    }
-    __syncthreads();
+#pragma unroll 1
+    for (uint32_t w = lane; w < nw; w += 32) mH[w] &= mX[w];
+    __syncwarp();
 
     SST_MARK(6);
-    // ---------------------------------------------------------------- a5 + a6: lane per seed
-    const uint32_t *const m_link = MASK(M_LINK);
-    const uint32_t *const m_seed = MASK(M_SEED);
-    uint32_t *const m_acc = MASK(M_ACC);
-    #pragma unroll 1
-    for (uint32_t i = tid; i < nw * 32; i += kThreads) {
-        const int w = i >> 5, b = i & 31;
-        const uint32_t sw = m_seed[w];
-        if (!((sw >> b) & 1u)) continue;
-        // left: the run starts at the nearest unlinked entry at or below i; a seed in between owns it
-        int ww = w;
-        uint32_t nl = ~m_link[w] & (0xffffffffu >> (31 - b));
-        uint32_t sd = sw & ((1u << b) - 1u);
-        bool owner = true;
-        while (nl == 0) {  // entry 0 is never linked, so this ends
-            if (sd) { owner = false; break; }
-            --ww;
-            nl = ~m_link[ww];
-            sd = m_seed[ww];
-        }
-        if (!owner) continue;
-        const int hb = 31 - __clz(nl);
-        if (sd >> hb) continue;  // leftmost-seed ownership: another seed emits this cluster
-        const int l = (ww << 5) + hb;
-        const int wd = run_end(m_link, i) - l + 1;
-        if (wd > kWide) {
-            const uint32_t slot = atomicAdd(&s.wide_count, 1u);
-            if (slot < kWideQ) {
-                s.wide_q[slot] = static_cast<uint32_t>(l) | (static_cast<uint32_t>(wd) << 16);
-                continue;
-            }
-        }
-        if (accept_serial(adc_l, noise_l, l, wd, p.tcl2)) {
-            atomicOr(&m_acc[l >> 5], 1u << (l & 31));
-            atomicAdd(&MASK(M_WTOT)[l >> 5], 1u | (static_cast<uint32_t>(wd) << 16));
-        }
-    }
-    __syncthreads();
+    // ---------------------------------------------------------------- a6: lane per candidate
+    // candidates are queued in order, kQCap at a time; a rejected one clears its head bit, so mH
+    // ends as the mask of accepted clusters
+    uint32_t my_cl = 0, my_adc = 0;
     {
-        const uint32_t nq = min(s.wide_count, static_cast<uint32_t>(kWideQ));
-        #pragma unroll 1
-        for (uint32_t e = warp; e < nq; e += kWarps) {
-            const int l = s.wide_q[e] & 0xffffu, wd = s.wide_q[e] >> 16;
-            if (accept_warp(adc_l, noise_l, l, wd, p.tcl2, lane) && lane == 0) {
-                atomicOr(&m_acc[l >> 5], 1u << (l & 31));
-                atomicAdd(&MASK(M_WTOT)[l >> 5], 1u | (static_cast<uint32_t>(wd) << 16));
+        uint32_t qn = 0;
+        auto flush = [&]() {
+            __syncwarp();
+#pragma unroll 1
+            for (uint32_t c0 = 0; c0 < qn; c0 += 32) {
+                const uint32_t ci = c0 + lane;
+                const bool have = ci < qn;
+                int hd = 0, wd = 0;
+                bool ok = false;
+                if (have) {
+                    hd = h.queue[ci];
+                    wd = run_end(mL, hd) - hd + 1;
+                    if (wd <= kWide) ok = accept_serial(adc_l, noise_l, hd, wd, p.tcl2);
+                }
+                uint32_t widem = __ballot_sync(kFull, have && wd > kWide);
+                while (widem) {
+                    const int src = __ffs(widem) - 1;
+                    widem &= widem - 1;
+                    const int hh = __shfl_sync(kFull, hd, src), ww = __shfl_sync(kFull, wd, src);
+                    const bool r = accept_warp(adc_l, noise_l, hh, ww, p.tcl2, lane);
+                    if (lane == src) ok = r;
+                }
+                if (have) {
+                    if (ok) {
+                        ++my_cl;
+                        my_adc += wd;
+                    } else {
+                        atomicAnd(&mH[hd >> 5], ~(1u << (hd & 31)));
+                    }
+                }
+                __syncwarp();
             }
+            qn = 0;
+        };
+#pragma unroll 1
+        for (uint32_t w = 0; w < nw; ++w) {
+            const uint32_t hs = mH[w];
+            const uint32_t n = __popc(hs);
+            if (!n) continue;
+            if (qn + n > static_cast<uint32_t>(kQCap)) flush();
+            if ((hs >> lane) & 1u) h.queue[qn + __popc(hs & lt)] = static_cast<uint16_t>(w * 32u + lane);
+            qn += n;
         }
+        flush();
     }
-    __syncthreads();
+    const uint32_t fed_cl = warp_sum(my_cl), fed_adc = warp_sum(my_adc), fed_seed = warp_sum(n_seed);
 
     SST_MARK(7);
-    // ---------------------------------------------------------------- a7: scan + look-back, warp 0
-    // Word totals (accepted clusters | ADC bytes << 16) were accumulated by the accepting lanes.
-    // Warp 0 turns them into exclusive prefixes, publishes the FED aggregate and resolves the
-    // FED's base offsets with a decoupled look-back over the earlier FEDs.
-    uint32_t *const m_wtot = MASK(M_WTOT);
-    uint32_t *const m_spre = MASK(M_BRK);  // brk is dead: per-word seed prefix goes here
-    const uint32_t fed_over = s.overrun;
-    if (warp == 0) {
-        const uint32_t K = (nw + 31) >> 5;  // words per lane
-        uint32_t my_a = 0, my_s = 0;
-        #pragma unroll 1
-        for (uint32_t k = 0; k < K; ++k) {
-            const uint32_t w = lane * K + k;
-            if (w < nw) { my_a += m_wtot[w]; my_s += __popc(m_seed[w]); }
-        }
-        uint32_t inc_a = my_a, inc_s = my_s;  // FED totals <= 12288 clusters / 24576 ADC bytes: halves stay apart
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t ua = __shfl_up_sync(0xffffffffu, inc_a, d);
-            const uint32_t us = __shfl_up_sync(0xffffffffu, inc_s, d);
-            if (lane >= d) { inc_a += ua; inc_s += us; }
-        }
-        const uint32_t tot_a = __shfl_sync(0xffffffffu, inc_a, 31), tot_s = __shfl_sync(0xffffffffu, inc_s, 31);
-        const uint32_t fed_cl = tot_a & 0xffffu, fed_adc = tot_a >> 16;
-        // publish: word 0 = status | clusters | ADC bytes << 30 (aggregate now, inclusive prefix
-        // later); word 1 = ready | seeds | malformed | overrun (aggregate only)
-        const unsigned long long agg0 = fed_cl | (static_cast<unsigned long long>(fed_adc) << kShAdc);
-        const unsigned long long ep0 = static_cast<unsigned long long>(p.epoch) << kShEp0;
-        if (lane == 0) {
-            st_state(p.fed_state + 2 * f, (f == 0 ? kStP : kStA) | ep0 | agg0);
-            st_state(p.fed_state + 2 * f + 1, kReady | (static_cast<unsigned long long>(p.epoch) << kShEp1) | tot_s |
-                                                  (static_cast<unsigned long long>(n_malformed) << kShMalf) |
-                                                  (static_cast<unsigned long long>(fed_over) << kShOvr));
-        }
-        {
-            uint32_t ex_a = inc_a - my_a, ex_s = inc_s - my_s;
-            #pragma unroll 1
-            for (uint32_t k = 0; k < K; ++k) {
-                const uint32_t w = lane * K + k;
-                if (w < nw) {
-                    const uint32_t t = m_wtot[w];
-                    m_wtot[w] = ex_a;
-                    m_spre[w] = ex_s;
-                    ex_a += t;
-                    ex_s += __popc(m_seed[w]);
-                }
-            }
-        }
-        SST_MARK(8);
-        // look-back: lane 0 reads the nearest predecessor; stop at the first inclusive prefix
-        unsigned long long excl = 0;
-        #pragma unroll 1
-        for (int base = static_cast<int>(f) - 1; base >= 0; base -= 32) {
-            const int j = base - lane;
-            unsigned long long v = kStP;  // before FED 0: prefix 0
-            if (j >= 0) {
-                v = ld_state(p.fed_state + 2 * j);
-                while (!(v >> 62) || ((v >> kShEp0) & 0xffull) != p.epoch) {  // not written by this call yet
-                    __nanosleep(64);
-                    v = ld_state(p.fed_state + 2 * j);
-                }
-            }
-            const uint32_t pm = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);
-            const int stop = pm ? __ffs(pm) - 1 : 31;  // lanes 0..stop contribute
-            unsigned long long c = lane <= stop ? (v & kStMask) : 0ull;
-#pragma unroll
-            for (int o2 = 16; o2 > 0; o2 >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o2);
-            excl += c;
-            if (pm) break;
-        }
-        if (lane == 0) {
-            if (f) st_state(p.fed_state + 2 * f, kStP | ep0 | (excl + agg0));
-            s.red[0][0] = static_cast<uint32_t>(excl & ((1ull << kShAdc) - 1));  // clusters before this FED
-            s.red[0][1] = static_cast<uint32_t>(excl >> kShAdc);                 // ADC bytes before this FED
-            s.red[0][2] = fed_cl;
-            s.red[0][3] = fed_adc;
-            s.red[0][4] = tot_s;
-        }
+    // ---------------------------------------------------------------- a7: publish, sum predecessors
+    unsigned long long *const st = p.fed_state + static_cast<size_t>(c.ev) * p.n_feds;
+    if (lane == 0) {
+        st_state(st + f, (static_cast<unsigned long long>(p.epoch) << kShEpoch) |
+                             (static_cast<unsigned long long>(c.overrun) << kShOver) |
+                             (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
+                             (static_cast<unsigned long long>(fed_seed) << kShSeed) |
+                             (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl);
+        // next FED of this warp: the ticket arrives while the look-back and the emit run
+        next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
     }
-    __syncthreads();
-    const uint32_t b_cl = s.red[0][0], b_adc = s.red[0][1], fed_cl = s.red[0][2], fed_adc = s.red[0][3],
-                   fed_seed = s.red[0][4];
-
-    // seed-index base (only when that output is requested) and, in the last FED, the event totals:
-    // sums over the aggregate-only word of every earlier FED
-    uint32_t b_seed = 0, b_malf = 0, b_over = 0;
-    const bool last = f == p.n_feds - 1;
-    if (o.seed_idx || last) {
-        #pragma unroll 1
-        for (uint32_t j = tid; j < f; j += kThreads) {
-            unsigned long long v = ld_state(p.fed_state + 2 * j + 1);
-            while (!(v & kReady) || ((v >> kShEp1) & 0xffull) != p.epoch) {
-                __nanosleep(100);
-                v = ld_state(p.fed_state + 2 * j + 1);
-            }
-            b_seed += static_cast<uint32_t>(v) & 0xfffffu;
-            b_malf += static_cast<uint32_t>(v >> kShMalf) & 0x7fu;
-            b_over += static_cast<uint32_t>(v >> kShOvr) & 1u;
-        }
-        b_seed = warp_sum(b_seed); b_malf = warp_sum(b_malf); b_over = warp_sum(b_over);
-        if (lane == 0) { s.red[1][warp] = b_seed; s.red[2][warp] = b_malf; s.red[3][warp] = b_over; }
-        __syncthreads();
-        b_seed = b_malf = b_over = 0;
+    // clusters | ADC bytes << 32 ; seeds | malformed << 32 (20 bits) | overrun << 52 (n_feds <= 4096)
+    unsigned long long accA = 0, accB = 0;
+#pragma unroll 1
+    for (uint32_t j0 = 0; j0 < f; j0 += 128) {  // warp-uniform control flow: the lanes poll together
+        unsigned long long v[4];
+        bool need[4];
 #pragma unroll
-        for (int i = 0; i < kWarps; ++i) { b_seed += s.red[1][i]; b_malf += s.red[2][i]; b_over += s.red[3][i]; }
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t j = j0 + 32u * u + lane;
+            need[u] = j < f;
+            v[u] = need[u] ? ld_state(st + j) : 0ull;
+        }
+        for (;;) {
+            bool ok = true;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) ok = ok && (!need[u] || (v[u] >> kShEpoch) == p.epoch);
+            if (__all_sync(kFull, ok)) break;
+            __nanosleep(100);  // some predecessor has not published in this launch yet
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (need[u] && (v[u] >> kShEpoch) != p.epoch) v[u] = ld_state(st + j0 + 32u * u + lane);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (need[u]) {
+                accA += (v[u] & 0x3fffull) | (((v[u] >> kShAdc) & 0x7fffull) << 32);
+                accB += ((v[u] >> kShSeed) & 0x7fffull) | (((v[u] >> kShMalf) & 0x7full) << 32) |
+                        (((v[u] >> kShOver) & 1ull) << 52);
+            }
     }
+    accA = warp_sum64(accA);
+    accB = warp_sum64(accB);
+    const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
+    const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
+                   b_over = static_cast<uint32_t>(accB >> 52);
 
-    SST_MARK(9);
-    // ---------------------------------------------------------------- a7: emit, (module, first strip) order
+    SST_MARK(8);
+    // ---------------------------------------------------------------- a4: seed-index array (on request)
     if (o.seed_idx) {
-        #pragma unroll 1
-        for (uint32_t i = tid; i < nw * 32; i += kThreads) {
-            const uint32_t w = i >> 5, b = i & 31, sw = m_seed[w];
-            if ((sw >> b) & 1u) {
-                const uint32_t k = b_seed + m_spre[w] + __popc(sw & ((1u << b) - 1u));
-                if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + strip_l[i];
+        uint32_t k0 = b_seed;
+#pragma unroll 1
+        for (uint32_t w = 0; w < nw; ++w) {
+            const uint32_t sw = mS[w];
+            if ((sw >> lane) & 1u) {
+                const uint32_t k = k0 + __popc(sw & lt);
+                if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + (strip_l[w * 32u + lane] & 0x7fffu);
             }
+            k0 += __popc(sw);
         }
     }
-    // ordered list of the FED's accepted clusters (entry | FED-local ADC offset << 16) in the dead
-    // run table, then lane per cluster; FEDs with more clusters than the table go in rounds
-    uint32_t *const cl_l = s.runs;
-    #pragma unroll 1
-    for (uint32_t c0 = 0; c0 < fed_cl; c0 += kRunCap) {
-        if (c0) __syncthreads();
-        #pragma unroll 1
-        for (uint32_t w = warp; w < nw; w += kWarps) {
-            const uint32_t aw = m_acc[w];
-            if (!aw) continue;  // warp-uniform
-            const int i = (w << 5) + lane;
-            const bool mine = (aw >> lane) & 1u;
-            const uint32_t wd = mine ? static_cast<uint32_t>(run_end(m_link, i) - i + 1) : 0u;
-            uint32_t incw = wd;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const uint32_t u = __shfl_up_sync(0xffffffffu, incw, d);
-                if (lane >= d) incw += u;
-            }
-            const uint32_t pre = m_wtot[w];
-            const uint32_t c = (pre & 0xffffu) + __popc(aw & ((1u << lane) - 1u)) - c0;
-            if (mine && c < static_cast<uint32_t>(kRunCap))
-                cl_l[c] = static_cast<uint32_t>(i) | (((pre >> 16) + incw - wd) << 16);
-        }
-        __syncthreads();
-        const uint32_t nc = min(fed_cl - c0, static_cast<uint32_t>(kRunCap));
-        #pragma unroll 1
-        for (uint32_t c = tid; c < nc; c += kThreads) {
-            const uint32_t e = cl_l[c];
-            const int i = e & 0xffffu;
-            const uint32_t k_cl = b_cl + c0 + c, k_adc = b_adc + (e >> 16);
-            const int wd = run_end(m_link, i) - i + 1;
-            if (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc) {
-                int Q = 0;
-                long long M = 0;
-                #pragma unroll 1
-                for (int j = 0; j < wd; ++j) {
-                    const int q = adc_l[i + j];
-                    Q += q;
-                    M += static_cast<long long>(j) * q;
-                    o.cl_adc[k_adc + j] = static_cast<uint8_t>(q);
+    // ---------------------------------------------------------------- a7: emit, (module, first strip) order
+    {
+        uint32_t qn = 0, run_cl = b_cl, run_adc = b_adc;
+        const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
+        auto flush = [&]() {
+            __syncwarp();
+#pragma unroll 1
+            for (uint32_t c0 = 0; c0 < qn; c0 += 32) {
+                const uint32_t ci = c0 + lane;
+                const bool have = ci < qn;
+                int hd = 0, wd = 0;
+                if (have) {
+                    hd = h.queue[ci];
+                    wd = run_end(mL, hd) - hd + 1;
                 }
-                const uint32_t st0 = strip_l[i], ch = st0 >> 8;
-                const int first = static_cast<int>(st0) - s.mod_lo[ch] * kStrip;
-                o.cl_module[k_cl] = s.mod_id[ch];
-                o.cl_first[k_cl] = static_cast<uint16_t>(first);
-                o.cl_width[k_cl] = static_cast<uint16_t>(wd);
-                o.cl_charge[k_cl] = Q;
-                // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
-                o.cl_bary[k_cl] = __fadd_rn(static_cast<float>(first),
-                                            __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
-                o.cl_adc_off[k_cl] = k_adc;
-                if (o.cl_snr) o.cl_snr[k_cl] = cluster_snr(noise_l, i, wd, Q);
-            } else {
-                // the first cluster that does not fit reports how many were written
-                const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
-                if (prev_fits) *o.n_clusters = k_cl;
+                const uint32_t incl = warp_incl_scan(static_cast<uint32_t>(wd), lane);
+                const uint32_t k_cl = run_cl + ci, k_adc = run_adc + incl - wd;
+                run_adc += __shfl_sync(kFull, incl, 31);
+                if (have && k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc) {
+                    int Q = 0;
+                    long long M = 0;
+#pragma unroll 1
+                    for (int j = 0; j < wd; ++j) {
+                        const int q = adc_l[hd + j];
+                        Q += q;
+                        M += static_cast<long long>(j) * q;
+                        st_stream(o.cl_adc + k_adc + j, static_cast<uint32_t>(q), pol_first);
+                    }
+                    const uint32_t st0 = strip_l[hd] & 0x7fffu;
+                    const uint2 cm = __ldg(cinfo + (st0 >> 8));
+                    const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
+                    st_stream(o.cl_module + k_cl, cm.x, pol_first);
+                    st_stream(o.cl_first + k_cl, static_cast<uint32_t>(first), pol_first);
+                    st_stream(o.cl_width + k_cl, static_cast<uint32_t>(wd), pol_first);
+                    st_stream(o.cl_charge + k_cl, Q, pol_first);
+                    // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
+                    st_stream(o.cl_bary + k_cl,
+                              __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q))),
+                              pol_first);
+                    st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
+                    if (o.cl_snr) o.cl_snr[k_cl] = cluster_snr(noise_l, hd, wd, Q);
+                } else if (have) {
+                    // the first cluster that does not fit reports how many were written
+                    const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
+                    if (prev_fits) *o.n_clusters = k_cl;
+                }
+                __syncwarp();
             }
+            run_cl += qn;
+            qn = 0;
+        };
+#pragma unroll 1
+        for (uint32_t w = 0; w < nw; ++w) {
+            const uint32_t hs = mH[w];
+            const uint32_t n = __popc(hs);
+            if (!n) continue;
+            if (qn + n > static_cast<uint32_t>(kQCap)) flush();
+            if ((hs >> lane) & 1u) h.queue[qn + __popc(hs & lt)] = static_cast<uint16_t>(w * 32u + lane);
+            qn += n;
         }
+        flush();
     }
-    if (last && tid == 0) {  // event totals = prefix of the last FED + its own
-        const uint32_t n_cl = b_cl + fed_cl, n_adc = b_adc + fed_adc, n_mal = b_malf + n_malformed,
-                       n_over = b_over + fed_over;
+    if (f == p.n_feds - 1 && lane == 0) {  // event totals = prefix of the last FED + its own
+        const uint32_t n_cl = b_cl + fed_cl, n_adc = b_adc + fed_adc, n_mal = b_malf + c.n_malformed,
+                       n_over = b_over + c.overrun;
         uint32_t flags = 0;
         if (n_cl > o.cap_clusters) flags |= SST_FLAG_CLUSTER_CAP;
         if (n_adc > o.cap_adc) flags |= SST_FLAG_ADC_CAP;
@@ -730,151 +772,150 @@ __device__ __noinline__ void lists_to_clusters(const KParams &p, Smem &s, const 
         o.dev_status[6] = 0;
         o.dev_status[7] = 0;
     }
-    SST_MARK(10);
-#undef MASK
+    SST_MARK(9);
 }
 
-// ------------------------------------------------------------------------------ the kernel
-__global__ void __launch_bounds__(kThreads, 5) sst_fed_kernel(const __grid_constant__ KParams p) {
-    extern __shared__ __align__(128) uint8_t smem_raw[];
-    Smem &s = *reinterpret_cast<Smem *>(smem_raw);
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t f = blockIdx.x;
-    const sst_output &o = p.out;
+// bytes of slot a FED needs on the fast path: payload stage (later noise), lists, four masks
+__device__ __forceinline__ uint32_t slot_need(uint32_t fed_size, uint32_t P) {
+    const uint32_t A = (max((fed_size + 15u) & ~15u, 4u * P) + 15u) & ~15u;
+    return ((A + 3u * P + 3u) & ~3u) + 16u * (((P + 31u) >> 5) + 2u);
+}
+
+// ------------------------------------------------------------------------------ one FED, one warp
+__device__ __forceinline__ void process_fed(const KParams &p, Hdr &h, uint8_t *slot, const uint32_t ticket,
+                                            const int lane, uint32_t &mbar_phase, uint32_t &next_ticket) {
+    FedCtx c;
+    c.ticket = ticket;
+    c.ev = ticket / p.n_feds;
+    c.f = ticket - c.ev * p.n_feds;
+    const uint32_t f = c.f;
+    const EventDesc &E = p.ev[c.ev];
+    const sst_output &o = E.out;
 
     SST_MARK(0);
     // ---------------------------------------------------------------- a1: stage the FED payload
-    if (tid == 0) {
-        mbar_init(&s.mbar, 1);
-        fence_proxy_async();
-        const uint32_t fo0 = p.fed_offsets[f], fo1 = p.fed_offsets[f + 1];
-        const bool valid = fo0 <= fo1 && fo1 <= p.max_raw_bytes;
-        const uint32_t size = valid ? fo1 - fo0 : 0u;
-        const bool in_smem = size <= static_cast<uint32_t>(kRawCap) && ((fo0 | size) & 15u) == 0 &&
-                             (reinterpret_cast<uintptr_t>(p.raw) & 15u) == 0;
-        s.fed_start = fo0;
-        s.fed_size = size;
-        s.in_smem = in_smem;
-        s.overrun = valid ? 0u : 1u;
-        s.wide_count = 0;
-        s.long_count = 0;
-        if (in_smem && size) {
-            mbar_expect_tx(&s.mbar, size);
-            bulk_g2s(s.u.raw, p.raw + fo0, size, &s.mbar);
-        }
+    // lanes 0/1 fetch the two offsets; lane 0 starts the bulk copy
+    const uint32_t fo = lane < 2 ? E.fed_offsets[f + lane] : 0u;
+    const uint32_t fo0 = __shfl_sync(kFull, fo, 0), fo1 = __shfl_sync(kFull, fo, 1);
+    const bool valid = fo0 <= fo1 && fo1 <= p.max_raw_bytes;
+    c.fo0 = fo0;
+    c.fed_start = valid ? fo0 : 0u;
+    c.fed_size = valid ? fo1 - fo0 : 0u;
+    c.overrun = valid ? 0u : 1u;
+    const bool staged = c.fed_size <= p.slot_bytes && ((c.fed_start | c.fed_size) & 15u) == 0 &&
+                        (reinterpret_cast<uintptr_t>(E.raw) & 15u) == 0;
+    __syncwarp();  // every lane is done with the slot of the previous FED
+    if (staged && c.fed_size && lane == 0) {
+        fence_proxy_async();  // earlier generic-proxy accesses to the slot before the async write
+        mbar_expect_tx(&h.mbar, c.fed_size);
+        bulk_g2s(slot, E.raw + c.fed_start, c.fed_size, &h.mbar, policy_evict_first());
     }
-    // meanwhile: zero-fill this FED's slice of the dense output, clear the run table, fetch the
-    // module map of the 96 channels
-    if (o.strip_adc) {
-        uint8_t *dst = o.strip_adc + static_cast<size_t>(f) * kFedStrips;
-        if ((reinterpret_cast<uintptr_t>(o.strip_adc) & 15u) == 0) {
-            uint4 *d4 = reinterpret_cast<uint4 *>(dst);
-            const uint4 z = make_uint4(0, 0, 0, 0);
+    // meanwhile: fetch the module map
+    c.opens = 0;
 #pragma unroll
-            for (int i = 0; i < kFedStrips / 16 / kThreads; ++i) d4[tid + i * kThreads] = z;
-        } else {
-            #pragma unroll 1
-            for (int i = tid; i < kFedStrips; i += kThreads) dst[i] = 0;
-        }
+    for (int k = 0; k < 3; ++k) {
+        const uint32_t ch = lane + 32 * k;
+        const uint2 ci = __ldg(p.chan_info + static_cast<size_t>(f) * kChan + ch);
+        if ((ci.y & 0xffu) == ch) c.opens |= 1u << k;
     }
-    {
-        uint4 *r4 = reinterpret_cast<uint4 *>(s.runs);
-        const uint4 z = make_uint4(0, 0, 0, 0);
-#pragma unroll
-        for (int i = 0; i < kRunCap / 4 / kThreads; ++i) r4[tid + i * kThreads] = z;
+    const uint8_t *rp = staged ? slot : E.raw + c.fed_start;
+    if (staged && c.fed_size) {
+        mbar_wait(&h.mbar, mbar_phase);  // every lane waits: async-proxy writes visible to all readers
+        mbar_phase ^= 1u;
     }
-    if (tid < kChan) {
-        const uint2 ci = __ldg(p.chan_info + f * kChan + tid);
-        s.mod_id[tid] = ci.x;
-        s.mod_lo[tid] = static_cast<uint8_t>(ci.y & 0xffu);
-        s.mod_hi[tid] = static_cast<uint8_t>((ci.y >> 8) & 0xffu);
-    }
-    __syncthreads();
-    const bool in_smem = s.in_smem != 0;
-    const uint32_t fed_size = s.fed_size;
-    const uint8_t *rp = in_smem ? s.u.raw : p.raw + s.fed_start;
 
     SST_MARK(1);
     // ---------------------------------------------------------------- a1: walk the length chain
-    if (tid == 0) {
-        if (in_smem) {
-            if (fed_size) mbar_wait(&s.mbar, 0);
-            SST_MARK(2);
-            walk_chain_speculative(s.u.raw, s.chan_off, s.chan_len, s.slot_base);
-        } else {
-            SST_MARK(2);
-            if (walk_chain_checked(rp, fed_size, s.overrun != 0, s.chan_off, s.chan_len, s.slot_base)) s.overrun = 1;
+    if (staged) {
+        if (lane == 0) walk_chain_speculative(slot, p.slot_bytes - 2u, h.chan_off, h.chan_len);
+        __syncwarp();
+        // validate the speculative chain: channels from the first bad one on are empty
+        uint32_t bad = 0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            c.off[k] = h.chan_off[lane + 32 * k];
+            c.len[k] = h.chan_len[lane + 32 * k];
+            const bool ok = c.overrun == 0 && c.off[k] <= c.fed_size && c.off[k] + c.len[k] <= c.fed_size;
+            const uint32_t m = ~__ballot_sync(kFull, ok);
+            if (!bad && m) bad = 32u * k + __ffs(m);  // 1 + index of the first bad channel
+        }
+        if (bad) {
+            c.overrun = 1;
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+                if (static_cast<uint32_t>(lane + 32 * k) >= bad - 1u) {
+                    c.off[k] = c.fed_size;
+                    c.len[k] = 0;
+                }
+        }
+    } else {
+        uint32_t over = c.overrun;
+        if (lane == 0) over = walk_chain_checked(rp, c.fed_size, c.overrun != 0, h.chan_off, h.chan_len) ? 1u : 0u;
+        c.overrun = __shfl_sync(kFull, over, 0);
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            c.off[k] = h.chan_off[lane + 32 * k];
+            c.len[k] = h.chan_len[lane + 32 * k];
         }
     }
-    __syncthreads();
-    if (in_smem && fed_size) mbar_wait(&s.mbar, 0);  // async-proxy writes visible to every reader
-    uint32_t my_off = 0, my_len = 0;
-    if (tid < kChan) {
-        my_off = s.chan_off[tid];
-        my_len = s.chan_len[tid];
+
+    SST_MARK(2);
+    // ---------------------------------------------------------------- a2 pass 1: run headers
+    // lane per channel: validate the run list, count the strips
+    uint32_t cnt[3];
+    c.n_malformed = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const uint32_t ch = lane + 32 * k;
+        if (o.chan_off) o.chan_off[f * kChan + ch] = c.fo0 + c.off[k];
+        if (o.chan_len) o.chan_len[f * kChan + ch] = static_cast<uint16_t>(c.len[k]);
+        uint32_t n_strips = 0;
+        const bool ok = staged ? scan_runs(slot, c.off[k], c.len[k], n_strips) : scan_runs(rp, c.off[k], c.len[k], n_strips);
+        __syncwarp();
+        cnt[k] = ok ? n_strips : 0u;
+        if (!ok) c.len[k] = 0;  // a malformed channel contributes no strips
+        c.n_malformed += __popc(__ballot_sync(kFull, !ok));
     }
-    if (in_smem) {  // validate the speculative chain: channels from the first bad one on are empty
-        const bool ok = tid >= kChan || (s.overrun == 0 && my_off <= fed_size && my_off + my_len <= fed_size);
-        const uint32_t okm = __ballot_sync(0xffffffffu, ok);
-        if (lane == 0 && warp < 3) s.okmask[warp] = okm;
-        __syncthreads();
-        const uint32_t m0 = ~s.okmask[0], m1 = ~s.okmask[1], m2 = ~s.okmask[2];
-        const int first_bad = m0 ? __ffs(m0) - 1 : (m1 ? 31 + __ffs(m1) : (m2 ? 63 + __ffs(m2) : kChan));
-        if (tid < kChan && tid >= first_bad) {
-            my_off = fed_size;
-            my_len = 0;
-            s.chan_off[tid] = fed_size;
-            s.chan_len[tid] = 0;
-        }
-        if (tid == 0 && first_bad < kChan) s.overrun = 1;
+    // exclusive scan of the 96 counts
+    uint32_t run = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const uint32_t inc = warp_incl_scan(cnt[k], lane);
+        c.base[k] = run + inc - cnt[k];
+        run += __shfl_sync(kFull, inc, 31);
     }
-    // the run table is usable if every channel's slot range fits
-    const uint32_t n_slots = s.slot_base[kChan];
-    const bool table_ok = n_slots <= static_cast<uint32_t>(kRunCap);
+    c.P = run;  // present strips of the FED
 
     SST_MARK(3);
-    // ---------------------------------------------------------------- a2 pass 1: run headers
-    // thread per channel: validate the run list, count the strips, fill the run table
-    int malformed = 0;
-    uint32_t my_cnt = 0;
-    if (tid < kChan) {
-        if (o.chan_off) o.chan_off[f * kChan + tid] = s.fed_start + my_off;
-        if (o.chan_len) o.chan_len[f * kChan + tid] = static_cast<uint16_t>(my_len);
-        uint32_t n_runs = 0, n_strips = 0;
-        uint32_t *slots = table_ok ? s.runs + s.slot_base[tid] : nullptr;
-        const bool ok = in_smem ? scan_runs(s.u.raw, my_off, my_len, tid, slots, n_runs, n_strips)
-                                : scan_runs(rp, my_off, my_len, tid, slots, n_runs, n_strips);
-        if (ok) {
-            my_cnt = n_strips;
-        } else {  // a malformed channel contributes no strips
-            malformed = 1;
-            my_len = 0;
-            if (slots)
-                #pragma unroll 1
-                for (uint32_t k = 0; k < n_runs; ++k) slots[k] = 0;
-        }
-    }
-    // exclusive scan of the 96 counts (warps 0..2)
-    uint32_t inc = my_cnt;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t u = __shfl_up_sync(0xffffffffu, inc, d);
-        if (lane >= d) inc += u;
-    }
-    if (lane == 31 && warp < 3) s.wscan[0][warp] = inc;
-    const uint32_t n_malformed = __syncthreads_count(malformed);
-    uint32_t my_base = inc - my_cnt;
-    if (warp >= 1) my_base += s.wscan[0][0];
-    if (warp >= 2) my_base += s.wscan[0][1];
-    if (tid < kChan) s.chan_base[tid] = static_cast<uint16_t>(my_base);
-    const uint32_t P = s.wscan[0][0] + s.wscan[0][1] + s.wscan[0][2];  // present strips of the FED
-    __syncthreads();
-
-    SST_MARK(4);
-    if (P <= static_cast<uint32_t>(kListCap))
-        lists_to_clusters<true>(p, s, rp, P, table_ok, n_slots, n_malformed, my_off, my_len, my_base);
+    if (staged && slot_need(c.fed_size, c.P) <= p.slot_bytes)
+        fed_lists<true>(p, h, slot, slot, c, lane, next_ticket);
     else
-        lists_to_clusters<false>(p, s, rp, P, table_ok, n_slots, n_malformed, my_off, my_len, my_base);
+        fed_lists<false>(p, h, slot, rp, c, lane, next_ticket);
+}
+
+// ------------------------------------------------------------------------------ the kernel
+// A CTA is one warp.  Warps draw (event, FED) tickets until the launch's work is used up.
+__global__ void __launch_bounds__(32, 24) sst_event_kernel(const __grid_constant__ KParams p) {
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    Hdr &h = *reinterpret_cast<Hdr *>(smem_raw);
+    uint8_t *slot = smem_raw + kHdrBytes;
+    const int lane = threadIdx.x;
+    if (lane == 0) {
+        mbar_init(&h.mbar, 1);
+        fence_proxy_async();
+    }
+    __syncwarp();
+    const uint32_t total = p.n_events * p.n_feds;
+    uint32_t mbar_phase = 0;
+    uint32_t ticket = 0;
+    if (lane == 0) ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
+    ticket = __shfl_sync(kFull, ticket, 0);
+    while (ticket < total) {
+        uint32_t next_ticket = 0;
+        process_fed(p, h, slot, ticket, lane, mbar_phase, next_ticket);
+        ticket = __shfl_sync(kFull, next_ticket, 0);
+    }
 }
 
 }  // namespace
@@ -889,9 +930,12 @@ struct sst_ctx {
     std::atomic<int32_t> last_err{0};
     int sm_count = 0;
     int ctas_per_sm = 0;
-    // per-stream scratch (look-back states + overflow lists), taken from the pool on a stream's
-    // first event and kept: stream order makes reuse safe, the epoch makes clearing unnecessary
-    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t epoch; };
+    uint32_t slot_bytes = 0;  // shared-memory slot of one warp (one FED)
+    uint32_t smem_bytes = 0;  // header + slot
+    // per-stream scratch (ticket counter, FED states, slow-path lists), taken from the pool on a
+    // stream's first launch and kept: stream order makes reuse safe, the epoch and the running
+    // ticket base make clearing unnecessary
+    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t epoch; unsigned long long ticket_base; };
     std::mutex slot_mu;
     std::vector<Slot> slots;
 };
@@ -915,7 +959,7 @@ bool thresholds_ok(const sst_thresholds *t) {
 
 bool output_ok(const sst_output *o) {
     return o && o->n_clusters && o->dev_status && o->cl_module && o->cl_first && o->cl_width &&
-           o->cl_charge && o->cl_bary && o->cl_adc_off && o->cl_adc;
+           o->cl_charge && o->cl_bary && o->cl_adc_off && o->cl_adc && !(o->seed_idx == nullptr && o->cap_seeds != 0);
 }
 
 #ifdef SST_PHASE_TIMING
@@ -923,74 +967,86 @@ unsigned long long *g_phase_clk = nullptr;
 #endif
 
 struct ScratchLayout {
-    size_t ents, mwords, o_state, o_noise, o_mask, o_strip, o_adc, total, state_bytes;
+    size_t ents, mwords, state_bytes, o_ticket, o_state, o_noise, o_mask, o_strip, o_adc, total;
 };
 ScratchLayout scratch_layout(const sst_ctx *ctx) {
     ScratchLayout L{};
     const uint32_t nf = ctx->cfg.n_feds;
     auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
-    L.ents = static_cast<size_t>(ctx->cfg.max_raw_bytes) + 16ull * nf + 64;
-    L.mwords = L.ents / 32 + 2ull * nf + 16;
-    L.state_bytes = 2 * sizeof(unsigned long long) * nf;
-    L.o_state = 0;
-    L.o_noise = up(L.state_bytes);
-    L.o_mask = L.o_noise + up(4 * L.ents);
-    L.o_strip = L.o_mask + up(4 * M_COUNT * L.mwords);
-    L.o_adc = L.o_strip + up(2 * L.ents);
-    L.total = L.o_adc + up(L.ents);
+    L.ents = (static_cast<size_t>(ctx->cfg.max_raw_bytes) + 16ull * nf + 64 + 31) & ~static_cast<size_t>(31);
+    L.mwords = L.ents / 32 + 4ull * nf + 16;
+    L.state_bytes = sizeof(unsigned long long) * nf * kMaxEv;
+    L.o_ticket = 0;
+    L.o_state = 256;
+    L.o_noise = L.o_state + up(L.state_bytes);
+    L.o_mask = L.o_noise + up(4 * L.ents * kMaxEv);
+    L.o_strip = L.o_mask + up(4 * 4 * L.mwords * kMaxEv);
+    L.o_adc = L.o_strip + up(2 * L.ents * kMaxEv);
+    L.total = L.o_adc + up(L.ents * kMaxEv);
     return L;
 }
 
-// The scratch of `st`: allocated (stream-ordered, from the pool) and cleared once, then reused.
-sst_status stream_scratch(sst_ctx *ctx, cudaStream_t st, uint8_t **mem, uint32_t *epoch) {
-    std::lock_guard<std::mutex> lock(ctx->slot_mu);
-    for (auto &sl : ctx->slots)
-        if (sl.stream == st) {
-            sl.epoch = sl.epoch % 255u + 1u;
-            *mem = sl.mem;
-            *epoch = sl.epoch;
-            return SST_OK;
-        }
-    const ScratchLayout L = scratch_layout(ctx);
-    uint8_t *blk = nullptr;
-    SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), L.total, ctx->pool, st));
-    SST_CU(cudaMemsetAsync(blk + L.o_state, 0, L.state_bytes, st));
-    ctx->slots.push_back({st, blk, 1u});
-    *mem = blk;
-    *epoch = 1u;
-    return SST_OK;
-}
-
-sst_status launch_event(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
-                        const sst_thresholds *thr, const sst_output *out, cudaStream_t st) {
+// Launches one kernel for `n` (<= kMaxEv) events on `st`.
+sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, const uint32_t *const *fed_offsets,
+                         const sst_thresholds *thr, const sst_output *const *outs, cudaStream_t st) {
     const uint32_t nf = ctx->cfg.n_feds;
+    const ScratchLayout L = scratch_layout(ctx);
+    const uint32_t total = n * nf;
+    const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm);
+    const uint32_t grid = std::min(total, capacity);
     uint8_t *blk = nullptr;
     uint32_t epoch = 0;
-    const sst_status rc = stream_scratch(ctx, st, &blk, &epoch);
-    if (rc != SST_OK) return rc;
-    const ScratchLayout L = scratch_layout(ctx);
+    unsigned long long ticket_base = 0;
+    {
+        std::lock_guard<std::mutex> lock(ctx->slot_mu);
+        sst_ctx::Slot *sl = nullptr;
+        for (auto &s : ctx->slots)
+            if (s.stream == st) sl = &s;
+        if (!sl) {
+            SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), L.total, ctx->pool, st));
+            SST_CU(cudaMemsetAsync(blk, 0, L.o_noise, st));  // ticket counter and states
+            ctx->slots.push_back({st, blk, 0u, 0ull});
+            sl = &ctx->slots.back();
+        }
+        if (sl->epoch == kEpochMax) {  // epoch wraps: stale words of 4095 launches ago must not match
+            SST_CU(cudaMemsetAsync(sl->mem + L.o_state, 0, L.state_bytes, st));
+            sl->epoch = 0;
+        }
+        sl->epoch += 1;
+        blk = sl->mem;
+        epoch = sl->epoch;
+        ticket_base = sl->ticket_base;
+        sl->ticket_base += static_cast<unsigned long long>(total) + grid;  // every warp draws one ticket too many
+    }
     KParams kp{};
-    kp.raw = raw;
-    kp.fed_offsets = fed_offsets;
     kp.calib = ctx->calib;
     kp.chan_info = ctx->chan_info;
+    kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
+    kp.ticket_base = ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
     kp.g_noise = reinterpret_cast<float *>(blk + L.o_noise);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
-    kp.g_mask_words = static_cast<uint32_t>(L.mwords);
     kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
     kp.g_adc = blk + L.o_adc;
+    kp.g_ents = static_cast<uint32_t>(L.ents);
+    kp.g_mwords = static_cast<uint32_t>(L.mwords);
     kp.tcl2 = static_cast<double>(thr->cluster) * static_cast<double>(thr->cluster);  // exact
     kp.t_ch = thr->channel;
     kp.t_seed = thr->seed;
     kp.max_raw_bytes = ctx->cfg.max_raw_bytes;
     kp.n_feds = nf;
+    kp.n_events = n;
     kp.epoch = epoch;
-    kp.out = *out;
+    kp.slot_bytes = ctx->slot_bytes;
 #ifdef SST_PHASE_TIMING
     kp.phase_clk = g_phase_clk;
 #endif
-    sst_fed_kernel<<<nf, kThreads, sizeof(Smem), st>>>(kp);
+    for (uint32_t e = 0; e < n; ++e) {
+        kp.ev[e].raw = raw[e];
+        kp.ev[e].fed_offsets = fed_offsets[e];
+        kp.ev[e].out = *outs[e];
+    }
+    sst_event_kernel<<<grid, 32, ctx->smem_bytes, st>>>(kp);
     SST_CU(cudaGetLastError());
     return SST_OK;
 }
@@ -1033,13 +1089,36 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (cudaMalloc(&ctx->chan_info, static_cast<size_t>(cfg->n_feds) * kChan * sizeof(uint2)) !=
         cudaSuccess)
         return fail(SST_ERR_CUDA);
-    if (cudaFuncSetAttribute(sst_fed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             static_cast<int>(sizeof(Smem))) != cudaSuccess)
+    // shared-memory slot of one warp: sized for the largest FED the configuration expects (FEDs
+    // that do not fit take the slow path through the global scratch)
+    {
+        const double m = static_cast<double>(cfg->max_raw_bytes) / cfg->n_feds;  // mean payload bound
+        const uint32_t p_hint = cfg->fed_strips_hint ? std::min(cfg->fed_strips_hint, static_cast<uint32_t>(kFedStrips))
+                                                     : static_cast<uint32_t>(0.55 * m) + 32u;
+        const uint32_t r_hint = (static_cast<uint32_t>(std::min(1.15 * m + 64.0, 65536.0)) + 15u) & ~15u;
+        const uint32_t A = (std::max(r_hint, 4u * p_hint) + 15u) & ~15u;
+        uint32_t need = ((A + 3u * p_hint + 3u) & ~3u) + 16u * (((p_hint + 31u) >> 5) + 2u);
+        need = (need + 127u) & ~127u;
+        ctx->slot_bytes = std::min(std::max(need, 2048u), 200u * 1024u);
+        ctx->smem_bytes = kHdrBytes + ctx->slot_bytes + 16u;  // tail pad, see pass 2
+    }
+    if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(ctx->smem_bytes)) != cudaSuccess)
         return fail(SST_ERR_CUDA);
-    cudaFuncSetAttribute(sst_fed_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    {
+        // L2 set-aside for the calibration (read by every event with an evict_last policy): the
+        // device maximum (79 of 126 MB on B200).  A device-wide limit; failure is not fatal.
+        int max_persist = 0;
+        if (cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, cfg->device) == cudaSuccess &&
+            max_persist > 0)
+            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, static_cast<size_t>(max_persist));
+        cudaGetLastError();
+    }
     cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->ctas_per_sm, sst_fed_kernel, kThreads,
-                                                  sizeof(Smem));
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->ctas_per_sm, sst_event_kernel, 32,
+                                                      ctx->smem_bytes) != cudaSuccess || ctx->ctas_per_sm < 1)
+        return fail(SST_ERR_CUDA);
     *out_ctx = ctx;
     return SST_OK;
 }
@@ -1090,10 +1169,9 @@ sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *
                               const sst_thresholds *thr, const sst_output *out, void *stream) {
     if (!ctx || !raw || !fed_offsets || !thr || !output_ok(out) || !thresholds_ok(thr))
         return SST_ERR_INVALID_ARG;
-    if (out->seed_idx == nullptr && out->cap_seeds != 0) return SST_ERR_INVALID_ARG;
     if (!ctx->has_calib) return SST_ERR_NO_CALIB;
     SST_CU(cudaSetDevice(ctx->cfg.device));
-    return launch_event(ctx, raw, fed_offsets, thr, out, static_cast<cudaStream_t>(stream));
+    return launch_events(ctx, 1, &raw, &fed_offsets, thr, &out, static_cast<cudaStream_t>(stream));
 }
 
 sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
@@ -1103,13 +1181,24 @@ sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8
         return SST_ERR_INVALID_ARG;
     if (!ctx->has_calib) return SST_ERR_NO_CALIB;
     for (uint32_t e = 0; e < n_events; ++e)
-        if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e]) || (!outs[e].seed_idx && outs[e].cap_seeds))
-            return SST_ERR_INVALID_ARG;
+        if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e])) return SST_ERR_INVALID_ARG;
     SST_CU(cudaSetDevice(ctx->cfg.device));
-    for (uint32_t e = 0; e < n_events; ++e) {
-        const sst_status rc = launch_event(ctx, raw[e], fed_offsets[e], thr, &outs[e],
-                                           static_cast<cudaStream_t>(streams[e % n_streams]));
-        if (rc != SST_OK) return rc;
+    // the events of one stream go into launches of up to kMaxEv events each
+    for (uint32_t s = 0; s < n_streams && s < n_events; ++s) {
+        const uint8_t *r[kMaxEv];
+        const uint32_t *fo[kMaxEv];
+        const sst_output *o[kMaxEv];
+        uint32_t n = 0;
+        for (uint32_t e = s; e < n_events; e += n_streams) {
+            r[n] = raw[e];
+            fo[n] = fed_offsets[e];
+            o[n] = &outs[e];
+            if (++n == kMaxEv || e + n_streams >= n_events) {
+                const sst_status rc = launch_events(ctx, n, r, fo, thr, o, static_cast<cudaStream_t>(streams[s]));
+                if (rc != SST_OK) return rc;
+                n = 0;
+            }
+        }
     }
     return SST_OK;
 }
@@ -1157,7 +1246,12 @@ sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t ra
     d.chan_off = out->chan_off ? reinterpret_cast<uint32_t *>(blk + o_coff) : nullptr;
     d.chan_len = out->chan_len ? reinterpret_cast<uint16_t *>(blk + o_clen) : nullptr;
     d.seed_idx = out->seed_idx ? reinterpret_cast<uint32_t *>(blk + o_seed) : nullptr;
-    if (rc == SST_OK) rc = launch_event(ctx, blk + o_raw, reinterpret_cast<uint32_t *>(blk + o_fo), thr, &d, st);
+    if (rc == SST_OK) {
+        const uint8_t *d_raw = blk + o_raw;
+        const uint32_t *d_fo = reinterpret_cast<uint32_t *>(blk + o_fo);
+        const sst_output *d_out = &d;
+        rc = launch_events(ctx, 1, &d_raw, &d_fo, thr, &d_out, st);
+    }
     // counts first, then exactly-sized copies of the cluster arrays
     CU(cudaMemcpyAsync(out->dev_status, d.dev_status, SST_ST_WORDS * 4, cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(out->n_clusters, d.n_clusters, 4, cudaMemcpyDeviceToHost, st));
@@ -1249,11 +1343,13 @@ const char *sst_status_string(sst_status s) {
 
 sst_status sst_get_info(const sst_ctx *ctx, sst_info *info) {
     if (!ctx || !info) return SST_ERR_INVALID_ARG;
-    info->smem_bytes = static_cast<uint32_t>(sizeof(Smem));
-    info->threads = kThreads;
+    info->smem_bytes = ctx->smem_bytes;
+    info->threads = 32;
     info->ctas_per_sm = static_cast<uint32_t>(ctx->ctas_per_sm);
     info->sm_count = static_cast<uint32_t>(ctx->sm_count);
     info->kernels_per_event = 1;
+    info->slot_bytes = ctx->slot_bytes;
+    info->events_per_launch = kMaxEv;
     return SST_OK;
 }
 

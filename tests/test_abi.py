@@ -29,7 +29,8 @@ def test_library_builds_loads_and_exports_everything():
 def test_binding_struct_layout_matches_header():
     # sst_output: 4 pointers, 3 uint32 (+pad), 10 pointers
     assert ctypes.sizeof(binding.sst_output) == 4 * 8 + 16 + 10 * 8
-    assert ctypes.sizeof(binding.sst_config) == 16
+    assert ctypes.sizeof(binding.sst_config) == 20
+    assert ctypes.sizeof(binding.sst_info) == 28
     assert ctypes.sizeof(binding.sst_thresholds) == 12
 
 
