@@ -9,7 +9,7 @@ once, per-event output buffers taken from the library's stream-ordered pool.
   value      whole-job events/s with the raw data already resident in HBM (CUDA-event timed)
   e2e        the same metric through sst_unpack_cluster_host: pinned HOST buffers, H2D of the raw
              data and D2H of the clusters inside the timed region
-  roofline   algorithmic HBM bytes of a launch / launch duration for sst_fed_kernel (the only
+  roofline   algorithmic HBM bytes of a launch / launch duration for sst_event_kernel (the only
              kernel of the path) against MEASURED_PEAKS.json
   cpu_baseline  the CPU oracle as it stands, timed on this box's host cores (reported, not a target)
 
@@ -326,7 +326,7 @@ def main():
                     [st.cuda_stream for st in streams])
 
     def step():
-        """One pass over the workload: n_events launches over the streams, one C call."""
+        """One pass over the workload: the events of each stream share launches, one C call."""
         B.sst_unpack_cluster_batch(det.ctx, batch)
 
     def fork_join_begin(ev):
@@ -398,12 +398,14 @@ def main():
     ms_step = ms_total / args.steps
     value = world * n_events * args.steps / (ms_total * 1e-3)
 
-    # ---- roofline of sst_fed_kernel: launches overlap on 8 streams, so a launch's share of the
+    # ---- roofline of sst_event_kernel: launches overlap on 8 streams, so a launch's share of the
     # device is the event-timed span / launches; also the kernel alone on one stream (serial)
     peak, peak_src = measured_peak()
-    launches = n_events * args.steps
+    epl = int(info.get("events_per_launch", 1))
+    launches_step = sum(-(-len(range(s, n_events, N_STREAMS)) // epl) for s in range(min(N_STREAMS, n_events)))
+    launches = launches_step * args.steps
     dur_us = 1e3 * ms_total / launches
-    achieved = (b_alg_step / n_events) / (dur_us * 1e-6) / 1e9
+    achieved = (b_alg_step / launches_step) / (dur_us * 1e-6) / 1e9
     serial = None
     if True:
         s0 = streams[0]
@@ -504,7 +506,8 @@ def main():
             "host_wall_ms_per_step": 1e3 * t_host / args.steps,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": ncu_traffic("config3_event"), "peak_source": peak_src,
-                         "kernel": "sst_fed_kernel", "algorithmic_bytes_per_launch": b_alg_step / n_events,
+                         "kernel": "sst_event_kernel", "algorithmic_bytes_per_launch": b_alg_step / launches_step,
+                         "events_per_launch": n_events / launches_step,
                          "launch_us": dur_us,
                          "how": "B_alg = raw + N dense + 32 B x noise sectors of present strips + 32 B x gain "
                                 "sectors of accepted-cluster strips + 20 B x clusters + cluster ADC bytes; launches "
