@@ -1,12 +1,13 @@
 // sst.cu -- libsst: unpack + three-threshold clustering of strip-tracker FED data on B200.
 //
-// One persistent kernel per launch, ONE WARP PER FED (a FED is 96 channels x 256
-// strips; modules never cross a FED, reading s10).  A CTA is a single warp with a
-// ~10 KB shared-memory slot, so ~20 FEDs are in flight per SM and the serial parts of the
-// method (the channel-length chain, the run headers) of one FED hide behind the parallel parts
-// of the others; there is no block-wide barrier anywhere.  Warps draw FEDs from a ticket
-// counter, in (event, FED) order, so a launch takes up to kMaxEv events.
+// Two kernels per launch, ONE WARP PER FED (a FED is 96 channels x 256 strips;
+// modules never cross a FED, reading s10).
 //
+// sst_event_kernel: a CTA is four independent warps, each with a ~7 KB shared-memory slot, so 28
+// FEDs are in flight per SM and the serial parts of the method (the channel-length chain, the run
+// headers) of one FED hide behind the parallel parts of the others; there is no block-wide
+// barrier anywhere.  Warps draw (FED, event) tickets in FED-major order, so the FED's slab of the
+// calibration is read from HBM once per launch and serves all the launch's events from L2.
 // Per FED, everything after the unpack runs in the COMPACT index space of the FED's present
 // strips (the structure of arrays of PAPER.md:31 has one entry per recorded strip):
 //
@@ -14,17 +15,20 @@
 //                             chain walked in shared memory (PAPER.md:31 builds it on the CPU)
 //   a2 unpack               : lane per channel: pass 1 validates the run headers and counts, a
 //                             warp scan gives every channel its slot range, pass 2 writes the
-//                             {strip, adc} lists in ascending strip order
-//   a3 flags                : lane per present strip: one 8-byte gather of {noise, gain} (64-byte
-//                             L2 fetch), exact >= tests, masks by __ballot_sync, dense SoA scatter
+//                             {strip, adc} lists in ascending strip order and scatters the dense SoA
+//   a3-a6 sweep             : lane per CHUNK of consecutive entries, walked serially: one 8-byte
+//                             gather of {noise, gain}, exact >= tests, link to the previous entry,
+//                             q = min(254, floor(adc/gain + .5)) in float32, and the open
+//                             candidate's (charge, sum noise^2 in double left to right, seed) in
+//                             registers; a candidate is tested where it ends (leftmost-seed
+//                             ownership is implicit: one test per maximal run).  Results are mask
+//                             bits (seeds, members and heads of accepted clusters)
 //   a4 seed-index array     : seed mask + ordered compaction; materialised on request
-//   a5 expansion/ownership  : bit-parallel flood fill of the seed mask down the link mask, lane
-//                             per 32 entries: marks the head of every run that holds a seed, so
-//                             each candidate is evaluated once, by (the lane of) its leftmost seed
-//   a6 gain corr + accept   : q = min(254, floor(adc/gain + .5)) in float32; lane per candidate:
-//                             Q^2 >= t^2 * sum n^2 with the double sum taken left to right
-//   a7 ordered output       : FED aggregate published in one 64-bit word, every FED sums the
-//                             words of its predecessors (one round trip), lane per cluster emit
+//   a7 ordered output, 1/2  : counts by popcount scan, cluster records built lane per cluster and
+//                             staged FED-locally in global scratch, FED totals in one 64-bit word
+//
+// sst_emit_kernel (a7, 2/2), behind it on the same stream: exclusive prefix of the FED totals,
+// staged clusters moved to their (module, first strip)-ordered place.  No warp waits for another.
 //
 // FEDs whose payload or lists exceed the slot run the same code on a pooled global scratch.
 // No tensor cores: nothing here is a contraction.
@@ -42,23 +46,33 @@
 
 #include "sst.h"
 
+#ifndef SST_MAXEV
+#define SST_MAXEV 32
+#endif
+#ifdef SST_X_NO_SCATTER
+#define SST_X_SCATTER false
+#else
+#define SST_X_SCATTER true
+#endif
+
 namespace {
 
 constexpr int kChan = 96;
 constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
-constexpr int kMaxEv = 8;                   // events per launch
-constexpr int kQCap = 256;                  // candidate / cluster queue (entries)
-constexpr int kWide = 48;                   // candidates wider than this are summed by the warp
+constexpr int kMaxEv = SST_MAXEV;                   // events per launch
+constexpr int kWarpsPerCta = 4;             // warps (= FEDs in flight) per CTA, each with its own slot
 constexpr int kU = 4;                       // mask words per batch of the flag pass (loads in flight)
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
+constexpr uint32_t kTabBytes = kChan * 4 + kChan * 2;  // channel map of the FED, at the slot's end
+constexpr uint32_t kWarpHdr = 16;                      // mbarrier
+constexpr uint32_t kTailPad = 16;                      // readable bytes behind the slot (pass 2)
 
-// Published FED aggregate, one 64-bit word: epoch (12 bits, never 0) << 52 | overrun << 51 |
-// malformed channels (7) << 44 | seeds (15) << 29 | cluster ADC bytes (15) << 14 | clusters (14).
-// A word counts only if its epoch is the launch's; the host clears the array when the epoch wraps.
-constexpr int kShEpoch = 52, kShOver = 51, kShMalf = 44, kShSeed = 29, kShAdc = 14;
-constexpr uint32_t kEpochMax = 4095;
+// FED aggregate, one 64-bit word per (event, FED), written by sst_event_kernel and read by
+// sst_emit_kernel: overrun << 51 | malformed channels (7) << 44 | seeds (15) << 29 | cluster ADC
+// bytes (15) << 14 | clusters (14).
+constexpr int kShOver = 51, kShMalf = 44, kShSeed = 29, kShAdc = 14;
 
 struct EventDesc {
     const uint8_t *raw;
@@ -70,29 +84,27 @@ struct KParams {
     const float2 *calib;     // {noise (+inf at bad strips), gain} per strip
     const uint2 *chan_info;  // {module id, first channel | end channel << 8 of the module}
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
-    unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+grid)
+    unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+warps)
     unsigned long long ticket_base;
     // global scratch of the slow path, one slice set per event
-    float *g_noise;
+    uint32_t *g_rec;
     uint16_t *g_strip;
     uint8_t *g_adc;
     uint32_t *g_mask;  // 4 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
+    // staging of the FED-local results, read by sst_emit_kernel
+    uint4 *s_rec;     // {module, first | width << 16, charge, barycenter}
+    uint32_t *s_off;  // offset of the cluster's ADCs inside its FED
+    float *s_snr;
+    uint8_t *s_adc;
+    uint16_t *s_seed;
+    uint32_t s_cl_stride;  // staged cluster slots per event
     double tcl2;
     float t_ch, t_seed;
-    uint32_t max_raw_bytes, n_feds, n_events, epoch, slot_bytes;
+    uint32_t max_raw_bytes, n_feds, n_events, slot_bytes;
     unsigned long long *phase_clk;  // debug builds only (SST_PHASE_TIMING)
     EventDesc ev[kMaxEv];
 };
-
-// per-warp shared memory: fixed header, then the slot (payload stage, later the lists and masks)
-struct __align__(16) Hdr {
-    unsigned long long mbar;
-    uint32_t chan_off[kChan];  // FED-local byte offset of the channel's first run byte
-    uint16_t chan_len[kChan];
-    uint16_t queue[kQCap];
-};
-constexpr uint32_t kHdrBytes = (sizeof(Hdr) + 127u) & ~127u;
 
 // ------------------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_addr(const void *p) {
@@ -131,14 +143,6 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         "l"(src), "r"(bytes), "r"(smem_addr(bar)), "l"(pol)
         : "memory");
 }
-__device__ __forceinline__ unsigned long long ld_state(const unsigned long long *p) {
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_state(unsigned long long *p, unsigned long long v) {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
 // L2 residency.  The calibration (8 B per strip, 86.5 MB for 440 FEDs) is read by every event and
 // fits the L2 set-aside that sst_create reserves, while raw data and outputs stream through once:
 // calibration loads carry an evict_last policy, everything else that touches HBM evict_first.
@@ -149,7 +153,11 @@ __device__ __forceinline__ unsigned long long policy_evict_last() {
 }
 __device__ __forceinline__ unsigned long long policy_evict_first() {
     unsigned long long pol;
+#ifdef SST_X_NORMAL_STORES
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+#else
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+#endif
     return pol;
 }
 // Calibration gather.  On B200 a plain load that misses L2 pulls the whole 128-byte line from
@@ -157,10 +165,19 @@ __device__ __forceinline__ unsigned long long policy_evict_first() {
 // through L1.
 __device__ __forceinline__ float2 ld_calib(const float2 *p, unsigned long long pol) {
     float2 v;
+#ifdef SST_X_NO_GATHER
+    return make_float2(4.0f, 1.0f);
+#endif
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.L2::64B.v2.f32 {%0,%1}, [%2], %3;"
                  : "=f"(v.x), "=f"(v.y)
                  : "l"(p), "l"(pol));
     return v;
+}
+// Fire-and-forget fetch of a strip's calibration into L2: issued from pass 2 as soon as the strip
+// id is known, so that the gather of the sweep, tens of microseconds later, is an L2 hit and DRAM
+// sees all FEDs' misses at once instead of four per lane and round trip.
+__device__ __forceinline__ void prefetch_calib(const float2 *p) {
+    asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(p));
 }
 // streaming stores of the outputs
 __device__ __forceinline__ void st_stream(uint4 *p, uint4 v, unsigned long long pol) {
@@ -199,17 +216,7 @@ __device__ __forceinline__ uint32_t gain_correct(float adc, float gain) {
     return fl >= 254.0f ? 254u : static_cast<uint32_t>(fl);
 }
 
-__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-    return v;
-}
 __device__ __forceinline__ unsigned long long warp_sum64(unsigned long long v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-    return v;
-}
-__device__ __forceinline__ double warp_sum_d(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
     return v;
@@ -222,92 +229,26 @@ __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, int lane) {
     }
     return v;
 }
-
-// Entry i is "linked" when it continues the cluster candidate of entry i-1 (both active, strips
-// adjacent inside one module).  The last entry of the run that contains entry i: one before the
-// next unlinked entry.  link[] has zero sentinel words after the last used word.
-__device__ __forceinline__ int run_end(const uint32_t *link, int i) {
-    int w = i >> 5;
-    const int b = i & 31;
-    uint32_t nl = ~link[w] & (b == 31 ? 0u : (kFull << (b + 1)));
-    while (nl == 0) nl = ~link[++w];
-    return (w << 5) + __ffs(nl) - 2;
-}
-
-// x |= every entry from which a set entry of x is reached by walking up through linked entries
-// (bit j of l: entry j continues entry j-1).  Kogge-Stone fill, five doubling steps.
-__device__ __forceinline__ uint32_t fill_down(uint32_t x, uint32_t l) {
-    x |= (x & l) >> 1;
-    l &= l << 1;
-    x |= (x & l) >> 2;
-    l &= l << 2;
-    x |= (x & l) >> 4;
-    l &= l << 4;
-    x |= (x & l) >> 8;
-    l &= l << 8;
-    x |= (x & l) >> 16;
-    return x;
-}
-
-// Cluster acceptance for a narrow candidate, one lane: Q^2 >= t_cl^2 * n2 with n2 the double sum
-// of noise^2 taken strictly left to right (reading s15; noise^2 is exact in double, so
-// the fused multiply-add below rounds exactly like the oracle's separate multiply and add).
-__device__ __forceinline__ bool accept_serial(const uint8_t *q, const float *noise, int l, int w, double tcl2) {
-    int Q = 0;
+// Cluster acceptance, the defining form (reading s15): Q^2 >= t_cl^2 * n2 with n2 the
+// double sum of noise^2 over the candidate's strips taken strictly left to right (noise^2 is
+// exact in double, so the fused multiply-add rounds exactly like a separate multiply and add).
+// The noise is gathered again from the calibration: this runs only for candidates that cross a
+// chunk boundary of the sweep and land within rounding distance of the threshold, and for the
+// optional S/N output.
+__device__ __noinline__ double n2_sequential(const float2 *cal, const uint16_t *strip_l, uint32_t head, uint32_t w) {
     double n2 = 0.0;
 #pragma unroll 1
-    for (int i = 0; i < w; ++i) {
-        Q += q[l + i];
-        const double d = static_cast<double>(noise[l + i]);
+    for (uint32_t i = 0; i < w; ++i) {
+        const double d = static_cast<double>(__ldg(&cal[strip_l[head + i] & 0x7fffu].x));
         n2 = __fma_rn(d, d, n2);
     }
+    return n2;
+}
+__device__ __forceinline__ bool accept_exact(const float2 *cal, const uint16_t *strip_l, uint32_t head, uint32_t w,
+                                             uint32_t Q, double tcl2) {
     const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
-    return lhs >= __dmul_rn(tcl2, n2);
+    return lhs >= __dmul_rn(tcl2, n2_sequential(cal, strip_l, head, w));
 }
-
-// The same decision for a wide candidate by the whole warp.  A pairwise double sum differs from
-// the sequential one by at most ~w*2^-52 relative; the decision is taken from it only when the
-// two sides are further apart than that, otherwise lane 0 redoes the sum sequentially.
-__device__ __noinline__ bool accept_warp(const uint8_t *q, const float *noise, int l, int w, double tcl2, int lane) {
-    uint32_t Q = 0;
-    double n2p = 0.0;
-#pragma unroll 1
-    for (int i = lane; i < w; i += 32) {
-        Q += q[l + i];
-        const double d = static_cast<double>(noise[l + i]);
-        n2p += d * d;
-    }
-    Q = warp_sum(Q);
-    n2p = warp_sum_d(n2p);
-    const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
-    const double rhs = tcl2 * n2p;
-    int ok = lhs >= rhs;
-    if (!(fabs(lhs - rhs) > rhs * static_cast<double>(w) * 0x1p-50)) {
-        if (lane == 0) {
-            double n2 = 0.0;
-#pragma unroll 1
-            for (int i = 0; i < w; ++i) {
-                const double d = static_cast<double>(noise[l + i]);
-                n2 = __fma_rn(d, d, n2);
-            }
-            ok = lhs >= __dmul_rn(tcl2, n2);
-        }
-        ok = __shfl_sync(kFull, ok, 0);
-    }
-    return ok != 0;
-}
-
-// optional output: cluster S/N = Q / sqrt(sum noise^2), sequential double sum
-__device__ __noinline__ float cluster_snr(const float *noise, int l, int w, int Q) {
-    double n2 = 0.0;
-#pragma unroll 1
-    for (int i = 0; i < w; ++i) {
-        const double d = static_cast<double>(noise[l + i]);
-        n2 = __fma_rn(d, d, n2);
-    }
-    return static_cast<float>(static_cast<double>(Q) / sqrt(n2));
-}
-
 // ------------------------------------------------------------------------------ raw payload
 // a1, generic path (payload not staged): the channel-length chain of one FED, checked as it goes.
 __device__ __noinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
@@ -349,29 +290,8 @@ __device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uin
     }
 }
 
-// a2 pass 1: validate one channel's run list (reading s2b) and count its strips.
-// Returns false for a malformed channel.
-__device__ __forceinline__ bool scan_runs(const uint8_t *rp, uint32_t off, uint32_t len_bytes, uint32_t &n_strips) {
-    uint32_t q = off, next_free = 0, within = 0;
-    const uint32_t qend = off + len_bytes;
-    bool ok = true;
-#pragma unroll 1
-    while (q < qend) {
-        if (q + 2 > qend) { ok = false; break; }
-        const uint32_t first = rp[q];
-        uint32_t len = rp[q + 1];
-        if (len == 0) len = 256;  // reading s2
-        if (first < next_free || first + len > kStrip || q + 2 + len > qend) { ok = false; break; }
-        next_free = first + len;
-        q += 2 + len;
-        within += len;
-    }
-    n_strips = within;
-    return ok;
-}
-
 #ifdef SST_PHASE_TIMING
-#define SST_MARK(k) do { if (lane == 0 && p.phase_clk) p.phase_clk[static_cast<size_t>(ticket) * 16 + (k)] = clock64(); } while (0)
+#define SST_MARK(k) do { if (lane == 0 && p.phase_clk) p.phase_clk[static_cast<size_t>(c.ticket) * 16 + (k)] = clock64(); } while (0)
 #else
 #define SST_MARK(k) do { } while (0)
 #endif
@@ -386,411 +306,454 @@ struct FedCtx {
     uint32_t opens;                    // bit k: channel lane+32k opens a module
 };
 
+// a2 pass 1: a lane validates the run lists of its three channels (reading s2b) and
+// counts their strips; the three cursors advance in one loop, so the three dependent chains of
+// byte loads overlap.  A malformed channel contributes no strips.
+__device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_t (&cnt)[3]) {
+    uint32_t q[3], qe[3], nf[3];
+    bool ok[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        q[k] = c.off[k];
+        qe[k] = q[k] + c.len[k];
+        nf[k] = 0;
+        cnt[k] = 0;
+        ok[k] = true;
+    }
+    bool more = (q[0] < qe[0]) | (q[1] < qe[1]) | (q[2] < qe[2]);
+#pragma unroll 1
+    while (more) {
+        more = false;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            if (q[k] < qe[k]) {
+                bool bad = q[k] + 2 > qe[k];
+                uint32_t first = 0, len = 0;
+                if (!bad) {
+                    first = rp[q[k]];
+                    len = rp[q[k] + 1];
+                    if (len == 0) len = 256;  // reading s2
+                    bad = first < nf[k] || first + len > kStrip || q[k] + 2 + len > qe[k];
+                }
+                if (bad) {
+                    ok[k] = false;
+                    q[k] = qe[k];
+                } else {
+                    nf[k] = first + len;
+                    q[k] += 2 + len;
+                    cnt[k] += len;
+                    more |= q[k] < qe[k];
+                }
+            }
+        }
+    }
+    c.n_malformed = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        if (!ok[k]) {
+            cnt[k] = 0;
+            c.len[k] = 0;
+        }
+        c.n_malformed += __popc(__ballot_sync(kFull, !ok[k]));
+    }
+}
+
 // ------------------------------------------------------------------------------ lists -> clusters
-// Everything after pass 1, on the FED's lists of present strips, by one warp.  kFast: lists and
-// masks live in the warp's shared-memory slot (LDS/STS) and the payload is staged there; else
-// lists and masks live in this FED's slice of the global scratch and rp is a generic pointer.
+// Everything after pass 1, on the FED's lists of present strips, by one warp.  kFast: lists, masks
+// and cluster records live in the warp's shared-memory slot and the payload is staged there; else
+// they live in this FED's slice of the global scratch and rp is a generic pointer.  Returns false
+// (fast path only) when the cluster records outgrow the slot: the FED is then redone on the slow
+// path (nothing has been published and every output written so far is rewritten identically).
 template <bool kFast>
-__device__ __forceinline__ void fed_lists(const KParams &p, Hdr &h, uint8_t *slot, const uint8_t *rp,
-                                          const FedCtx &c, const int lane, uint32_t &next_ticket) {
-    const uint32_t f = c.f, P = c.P, ticket = c.ticket;
+__device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, const FedCtx &c,
+                                          const int lane, uint32_t &next_ticket) {
+    const uint32_t f = c.f, P = c.P;
     const EventDesc &E = p.ev[c.ev];
     const sst_output &o = E.out;
     const uint32_t nw = (P + 31) >> 5;  // mask words in use
     const uint32_t lt = (1u << lane) - 1u;
-    (void)ticket;
 
-    float *noise_l;
     uint16_t *strip_l;
     uint8_t *adc_l;
-    uint32_t *mS, *mL, *mH, *mX;
+    uint32_t *mS, *mA, *mH, *mP, *rec;
+    uint32_t rec_cap;  // cluster records besides the end sentinel
     if (kFast) {
-        const uint32_t A = (max((c.fed_size + 15u) & ~15u, 4u * P) + 15u) & ~15u;
-        noise_l = reinterpret_cast<float *>(slot);  // overlays the payload once the lists are built
+        // [0, A): the payload, and once the lists are built the masks and the cluster records
+        const uint32_t A = (c.fed_size + 15u) & ~15u;
         strip_l = reinterpret_cast<uint16_t *>(slot + A);
         adc_l = slot + A + 2u * P;
-        mS = reinterpret_cast<uint32_t *>(slot + ((A + 3u * P + 3u) & ~3u));
-        mL = mS + (nw + 2);
-        mH = mL + (nw + 2);
-        mX = mH + (nw + 2);
+        mS = reinterpret_cast<uint32_t *>(slot);
+        mA = mS + (nw + 2);
+        mH = mA + (nw + 2);
+        mP = mH + (nw + 2);
+        rec = mP + (nw + 2);
+        rec_cap = (A - 16u * (nw + 2)) / 4u - 1u;
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
-        noise_l = p.g_noise + eb + slice;
         strip_l = p.g_strip + eb + slice;
         adc_l = p.g_adc + eb + slice;
+        rec = p.g_rec + eb + slice;
         mS = p.g_mask + static_cast<size_t>(c.ev) * 4u * p.g_mwords + (slice >> 5) + 4u * f;
-        mL = mS + p.g_mwords;
-        mH = mL + p.g_mwords;
-        mX = mH + p.g_mwords;
+        mA = mS + p.g_mwords;
+        mH = mA + p.g_mwords;
+        mP = mH + p.g_mwords;
+        rec_cap = 0xffffffffu;
     }
+    const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
+
+    // ---------------------------------------------------------------- a2: dense SoA, zero fill
+    // the whole FED row block by the warp (coalesced 16-byte stores), just before pass 2 scatters
+    // the present strips into it
     uint8_t *const dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips : nullptr;
+#ifdef SST_X_NO_FILL
+    if (false) {
+#else
+    if (dense) {
+#endif
+        if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0) {
+#pragma unroll 4
+            for (uint32_t b = 16u * lane; b < static_cast<uint32_t>(kFedStrips); b += 512u)
+                st_stream(reinterpret_cast<uint4 *>(dense + b), make_uint4(0, 0, 0, 0), pol_first);
+        } else {
+#pragma unroll 1
+            for (uint32_t b = lane; b < static_cast<uint32_t>(kFedStrips); b += 32u) dense[b] = 0;
+        }
+        __syncwarp();  // orders the zeros before the scatter of other lanes
+    }
 
     // ---------------------------------------------------------------- a2 pass 2: lane per channel
     // writes {strip, adc} in ascending strip order; bit 15 of a strip id marks strip 0 of a channel
-    // that opens a module (nothing links across it)
+    // that opens a module (nothing links across it).  Three cursors per lane as in pass 1.
+#ifdef SST_X_SMALL_CAL
+    const float2 *cal = p.calib + static_cast<size_t>(f & 7u) * kFedStrips;  // 1.5 MB of calibration: always an L2 hit
+#else
+    const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
+#endif
+    {
+        uint32_t q[3], qe[3], e[3];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        uint32_t q = c.off[k], e = c.base[k];
-        const uint32_t qend = q + c.len[k];
-        const uint32_t g0 = static_cast<uint32_t>(lane + 32 * k) * kStrip;
-        const uint32_t open_bit = ((c.opens >> k) & 1u) << 15;
-#pragma unroll 1
-        while (q < qend) {
-            const uint32_t first = rp[q];
-            uint32_t len = rp[q + 1];
-            if (len == 0) len = 256;
-            // most runs hold one or two strips; on the fast path the second byte is read
-            // unconditionally (it is inside the slot or its 16-byte tail pad)
-            const uint32_t b0 = rp[q + 2], b1 = (kFast || len > 1) ? rp[q + 3] : 0u;
-            const uint32_t sid = g0 + first;
-            strip_l[e] = static_cast<uint16_t>(first == 0 ? sid | open_bit : sid);
-            adc_l[e] = static_cast<uint8_t>(b0);
-            if (len > 1) {
-                strip_l[e + 1] = static_cast<uint16_t>(sid + 1u);
-                adc_l[e + 1] = static_cast<uint8_t>(b1);
-            }
-#pragma unroll 1
-            for (uint32_t i = 2; i < len; ++i) {
-                strip_l[e + i] = static_cast<uint16_t>(sid + i);
-                adc_l[e + i] = rp[q + 2 + i];
-            }
-            e += len;
-            q += 2 + len;
+        for (int k = 0; k < 3; ++k) {
+            q[k] = c.off[k];
+            qe[k] = q[k] + c.len[k];
+            e[k] = c.base[k];
         }
-        __syncwarp();
+        bool more = (q[0] < qe[0]) | (q[1] < qe[1]) | (q[2] < qe[2]);
+#pragma unroll 1
+        while (more) {
+            more = false;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                if (q[k] < qe[k]) {
+                    const uint32_t qq = q[k], ee = e[k];
+                    const uint32_t first = rp[qq];
+                    uint32_t len = rp[qq + 1];
+                    if (len == 0) len = 256;
+                    // most runs hold one or two strips; on the fast path the second byte is read
+                    // unconditionally (it is inside the slot or its 16-byte tail pad)
+                    const uint32_t b0 = rp[qq + 2], b1 = (kFast || len > 1) ? rp[qq + 3] : 0u;
+                    const uint32_t sid = static_cast<uint32_t>(lane + 32 * k) * kStrip + first;
+                    const uint32_t open_bit = ((c.opens >> k) & 1u) << 15;
+                    strip_l[ee] = static_cast<uint16_t>(first == 0 ? sid | open_bit : sid);
+                    adc_l[ee] = static_cast<uint8_t>(b0);
+                    prefetch_calib(cal + sid);
+                    if (SST_X_SCATTER && dense) st_stream(dense + sid, b0, pol_first);
+                    if (len > 1) {
+                        strip_l[ee + 1] = static_cast<uint16_t>(sid + 1u);
+                        adc_l[ee + 1] = static_cast<uint8_t>(b1);
+                        if (((sid + 1u) & 3u) == 0) prefetch_calib(cal + sid + 1u);
+                        if (SST_X_SCATTER && dense) st_stream(dense + sid + 1u, b1, pol_first);
+#pragma unroll 1
+                        for (uint32_t i = 2; i < len; ++i) {
+                            const uint32_t bi = rp[qq + 2 + i];
+                            strip_l[ee + i] = static_cast<uint16_t>(sid + i);
+                            adc_l[ee + i] = static_cast<uint8_t>(bi);
+                            if (((sid + i) & 3u) == 0) prefetch_calib(cal + sid + i);  // next 32-byte sector
+                            if (SST_X_SCATTER && dense) st_stream(dense + sid + i, bi, pol_first);
+                        }
+                    }
+                    e[k] = ee + len;
+                    q[k] = qq + 2 + len;
+                    more |= q[k] < qe[k];
+                }
+            }
+        }
     }
     __syncwarp();  // lists complete; the payload is dead from here on
 
     SST_MARK(4);
-    // ---------------------------------------------------------------- a3: active / seed flags
-    // lane per entry, a warp covers one mask word per step, so the masks come from ballots; kU
-    // words per batch keep kU calibration gathers in flight per lane
-    const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
-    const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
+    // ---------------------------------------------------------------- a3..a6: one sweep over the lists
+    // Lane per CHUNK of consecutive entries, walked serially: active/seed tests, link to the previous
+    // entry, and the running (charge, noise^2, seed) of the open candidate are thread-local, so a
+    // candidate inside one chunk is decided exactly as the oracle does (double sum of noise^2,
+    // left to right) with no cross-lane traffic.  Results are mask bits: mA members and mH heads of
+    // accepted clusters, mS seeds.  A candidate that crosses a chunk boundary is put together
+    // afterwards from the tail partial of one lane and the lead partials of the next lanes.
+#pragma unroll 1
+    for (uint32_t w = lane; w < nw + 2; w += 32) {
+        mS[w] = 0;
+        mA[w] = 0;
+        mH[w] = 0;
+    }
+    const uint32_t Lc = ((P + 31u) >> 5) | 1u;  // odd: the lanes' list reads fall into different banks
+    const uint32_t e0 = min(lane * Lc, P), e1 = min(e0 + Lc, P);
+    auto mark = [&](uint32_t hd, uint32_t end) {  // accepted cluster [hd, end]
+        atomicOr(&mH[hd >> 5], 1u << (hd & 31u));
+        uint32_t w = hd >> 5, m = kFull << (hd & 31u);
+        const uint32_t we = end >> 5;
+#pragma unroll 1
+        for (; w < we; ++w) {
+            atomicOr(&mA[w], m);
+            m = kFull;
+        }
+        atomicOr(&mA[we], m & (kFull >> (31u - (end & 31u))));
+    };
+    auto decide = [&](uint32_t hd, uint32_t end, uint32_t Q, double N, bool seed) {
+        if (seed) {
+            const double dq = static_cast<double>(Q);
+            if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) mark(hd, end);
+        }
+    };
     {
-        uint32_t carry_sv = 0xffffu, carry_act = 0;
-        uint32_t filled = 0;  // the dense output is zero up to here (multiple of 16)
-        const bool dense16 = (reinterpret_cast<uintptr_t>(dense) & 15u) == 0;
-        auto fill_to = [&](uint32_t upto) {
-            if (dense16) {
+        // is the entry before the chunk active?  (its raw ADC is read before any lane overwrites it)
+        bool open = false;
+        uint32_t prev_s = 0;
+        if (e0 > 0) {
+            const uint32_t s = strip_l[e0 - 1], a = adc_l[e0 - 1];
+            prev_s = s & 0x7fffu;
+            if (a) open = ge_exact(static_cast<float>(a), p.t_ch, ld_calib(cal + prev_s, pol_last).x);
+        }
+        __syncwarp();
+        bool lead = open;  // an open candidate at the chunk start began in an earlier chunk
+        uint32_t hd = 0, Q = 0, accS = 0;
+        double N = 0.0;
+        bool seed = false;
+        uint32_t lQ = 0, lEnd = 0;  // lead partial: the part of an earlier candidate inside this chunk
+        double lN = 0.0;
+        bool lSeed = false, lClosed = false;
 #pragma unroll 1
-                for (uint32_t b = filled + 16u * lane; b < upto; b += 512u)
-                    st_stream(reinterpret_cast<uint4 *>(dense + b), make_uint4(0, 0, 0, 0), pol_first);
-            } else {
-#pragma unroll 1
-                for (uint32_t b = filled + lane; b < upto; b += 32u) dense[b] = 0;
-            }
-            filled = upto;
-            __syncwarp();
-        };
-#pragma unroll 1
-        for (uint32_t w0 = 0; w0 < nw; w0 += kU) {
+        for (uint32_t eb = e0; eb < e1; eb += kU) {
             uint32_t sv[kU], av[kU];
             float2 cv[kU];
 #pragma unroll
             for (int j = 0; j < kU; ++j) {
-                const uint32_t i = (w0 + j) * 32u + lane;
-                const bool valid = i < P;
-                sv[j] = valid ? strip_l[i] : 0xffffu;
-                av[j] = valid ? adc_l[i] : 0u;
+                const uint32_t e = eb + j;
+                const bool valid = e < e1;
+                sv[j] = valid ? strip_l[e] : 0xffffu;
+                av[j] = valid ? adc_l[e] : 0u;
             }
 #pragma unroll
             for (int j = 0; j < kU; ++j)
                 cv[j] = av[j] ? ld_calib(cal + (sv[j] & 0x7fffu), pol_last) : make_float2(INFINITY, 1.0f);
-            if (dense) {
-                // zero-fill the dense output up to the last strip of this batch (to the FED's end in
-                // the last batch), just ahead of the scatter below: both hit the same L2 lines
-                const uint32_t i_last = min(P, (w0 + kU) * 32u) - 1u;
-                fill_to((w0 + kU) * 32u >= P ? static_cast<uint32_t>(kFedStrips)
-                                             : ((strip_l[i_last] & 0x7fffu) + 16u) & ~15u);
-            }
 #pragma unroll
             for (int j = 0; j < kU; ++j) {
-                if (w0 + j >= nw) break;  // warp-uniform
-                const uint32_t i = (w0 + j) * 32u + lane;
-                const bool valid = sv[j] != 0xffffu;
-                const uint32_t s15 = sv[j] & 0x7fffu;
-                if (dense && valid) st_stream(dense + s15, av[j], pol_first);
-                const float af = static_cast<float>(av[j]);
-                const bool is_act = av[j] != 0 && ge_exact(af, p.t_ch, cv[j].x);
-                const bool is_seed = is_act && ge_exact(af, p.t_seed, cv[j].x);
-                uint32_t p_sv = __shfl_up_sync(kFull, sv[j], 1);
-                uint32_t p_act = __shfl_up_sync(kFull, static_cast<uint32_t>(is_act), 1);
-                if (lane == 0) { p_sv = carry_sv; p_act = carry_act; }
-                // this entry continues the candidate of the previous one
-                const bool is_link = is_act && p_act && !(sv[j] & 0x8000u) && s15 == (p_sv & 0x7fffu) + 1u;
-                const uint32_t wa = __ballot_sync(kFull, is_act);
-                const uint32_t ws = __ballot_sync(kFull, is_seed);
-                const uint32_t wl = __ballot_sync(kFull, is_link);
-                if (valid) {
-                    noise_l[i] = cv[j].x;
-                    if (is_act) adc_l[i] = static_cast<uint8_t>(gain_correct(af, cv[j].y));
+                const uint32_t e = eb + j;
+                if (e < e1) {
+                    const uint32_t s15 = sv[j] & 0x7fffu;
+                    const float af = static_cast<float>(av[j]);
+                    const bool is_act = av[j] != 0 && ge_exact(af, p.t_ch, cv[j].x);
+                    const bool is_seed = is_act && ge_exact(af, p.t_seed, cv[j].x);
+                    // this entry continues the candidate of the previous one
+                    const bool is_link = is_act && open && !(sv[j] & 0x8000u) && s15 == prev_s + 1u;
+                    if (open && !is_link) {  // the open candidate ended with entry e - 1
+                        if (lead) {
+                            lQ = Q; lN = N; lSeed = seed; lEnd = e - 1u; lClosed = true;
+                            lead = false;
+                        } else {
+                            decide(hd, e - 1u, Q, N, seed);
+                        }
+                    }
+                    if (is_act) {
+                        if (!is_link) {
+                            hd = e; Q = 0; N = 0.0; seed = false;
+                        }
+                        const uint32_t q = gain_correct(af, cv[j].y);
+                        adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
+                        Q += q;
+                        const double d = static_cast<double>(cv[j].x);
+                        N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
+                        seed = seed || is_seed;
+                    }
+                    open = is_act;
+                    prev_s = s15;
+                    if (is_seed) accS |= 1u << (e & 31u);
+                    if ((e & 31u) == 31u || e + 1u == e1) {
+                        if (accS) atomicOr(&mS[e >> 5], accS);
+                        accS = 0;
+                    }
                 }
-                if (lane == 0) {
-                    mS[w0 + j] = ws;
-                    mL[w0 + j] = wl;
-                    mH[w0 + j] = wa & ~wl;  // heads: active entries that start a candidate
-                }
-                carry_sv = __shfl_sync(kFull, sv[j], 31);
-                carry_act = __shfl_sync(kFull, static_cast<uint32_t>(is_act), 31);
             }
         }
-        if (dense && filled < static_cast<uint32_t>(kFedStrips)) fill_to(kFedStrips);  // a FED without strips
-        if (lane < 2) {  // zero sentinels behind the last word
-            mS[nw + lane] = 0;
-            mL[nw + lane] = 0;
-            mH[nw + lane] = 0;
-            mX[nw + lane] = 0;
+        bool pend = false;  // an open candidate that began in this chunk and runs on
+        if (open) {
+            if (e1 == P) {  // the lists end here
+                if (lead) {
+                    lQ = Q; lN = N; lSeed = seed; lEnd = P - 1u; lClosed = true;
+                } else {
+                    decide(hd, P - 1u, Q, N, seed);
+                }
+            } else if (lead) {  // the whole chunk lies inside a candidate of an earlier chunk
+                lQ = Q; lN = N; lSeed = seed; lEnd = e1 - 1u; lClosed = false;
+            } else {
+                pend = true;
+            }
+        }
+        // candidates across chunk boundaries: tail + lead partials of the following lanes.  The sum
+        // of partial sums is not the oracle's left-to-right sum; they differ by < (2w + 32) * 2^-53
+        // relative, so the comparison is taken from it only outside that band.
+        for (uint32_t dd = 1; __any_sync(kFull, pend); ++dd) {
+            const uint32_t pk = __shfl_down_sync(kFull, lQ | (static_cast<uint32_t>(lSeed) << 30) |
+                                                            (static_cast<uint32_t>(lClosed) << 31), dd);
+            const uint32_t end_s = __shfl_down_sync(kFull, lEnd, dd);
+            const double n_s = __shfl_down_sync(kFull, lN, dd);
+            if (pend) {
+                if (lane + dd > 31u) {
+                    pend = false;  // cannot happen: the last lane's chunk ends the lists
+                } else {
+                    Q += pk & 0x3fffffffu;
+                    N += n_s;
+                    seed = seed || ((pk >> 30) & 1u);
+                    if (pk >> 31) {
+                        pend = false;
+                        if (seed) {
+                            const uint32_t wd = end_s - hd + 1u;
+                            const double dq = static_cast<double>(Q);
+                            const double lhs = __dmul_rn(dq, dq), rhs = __dmul_rn(p.tcl2, N);
+                            bool acc;
+                            if (fabs(lhs - rhs) > rhs * (static_cast<double>(wd + 16u) * 0x1p-51)) acc = lhs > rhs;
+                            else acc = accept_exact(cal, strip_l, hd, wd, Q, p.tcl2);
+                            if (acc) mark(hd, end_s);
+                        }
+                    }
+                }
+            }
         }
     }
     __syncwarp();
 
     SST_MARK(5);
-    // ---------------------------------------------------------------- a4/a5: seeds -> candidates
-    // lane per mask word: X = entries with a seed at or above them in their run (flood fill of
-    // the seed mask down the links); a head in X starts a candidate that holds a seed.  Runs that
-    // cross a word boundary hand the fill to the word below until nothing changes.
-    uint32_t n_seed = 0;
+    // ---------------------------------------------------------------- counts and cluster records
+    // lane per mask word: exclusive prefix of (accepted heads, accepted members) per word, then
+    // every head gets its record {head entry, offset of its ADCs}
+    uint32_t fed_cl = 0, fed_adc = 0, fed_seed = 0;
+    {
+        uint32_t run = 0;  // heads << 16 | members
 #pragma unroll 1
-    for (uint32_t w = lane; w < nw; w += 32) {
-        const uint32_t s = mS[w];
-        n_seed += __popc(s);
-        mX[w] = fill_down(s, mL[w]);
-    }
-    __syncwarp();
-    for (;;) {
-        bool changed = false;
+        for (uint32_t w0 = 0; w0 < nw; w0 += 32) {
+            const uint32_t w = w0 + lane;
+            uint32_t v = 0, ns = 0;
+            if (w < nw) {
+                v = (__popc(mH[w]) << 16) | __popc(mA[w]);
+                ns = __popc(mS[w]);
+            }
+            const uint32_t incl = warp_incl_scan(v, lane);
+            if (w < nw) mP[w] = run + incl - v;
+            run += __shfl_sync(kFull, incl, 31);
+            fed_seed += __reduce_add_sync(kFull, ns);
+        }
+        fed_cl = run >> 16;
+        fed_adc = run & 0xffffu;
+        if (kFast && fed_cl > rec_cap) return false;
+        __syncwarp();
 #pragma unroll 1
         for (uint32_t w = lane; w < nw; w += 32) {
-            const uint32_t cin = mX[w + 1] & mL[w + 1] & 1u;
-            const uint32_t x = mX[w];
-            if (cin && !(x >> 31)) {
-                mX[w] = fill_down(x | 0x80000000u, mL[w]);
-                changed = true;
+            uint32_t mh = mH[w];
+            const uint32_t ma = mA[w], pre = mP[w];
+            uint32_t k = pre >> 16;
+            while (mh) {
+                const uint32_t b = __ffs(mh) - 1u;
+                mh &= mh - 1u;
+                rec[k++] = (w * 32u + b) | (((pre & 0xffffu) + __popc(ma & ((1u << b) - 1u))) << 16);
             }
         }
-        __syncwarp();
-        if (!__any_sync(kFull, changed)) break;
+        if (P && lane == 0) rec[fed_cl] = fed_adc << 16;  // end sentinel: widths are offset differences
     }
-#pragma unroll 1
-    for (uint32_t w = lane; w < nw; w += 32) mH[w] &= mX[w];
     __syncwarp();
 
-    SST_MARK(6);
-    // ---------------------------------------------------------------- a6: lane per candidate
-    // candidates are queued in order, kQCap at a time; a rejected one clears its head bit, so mH
-    // ends as the mask of accepted clusters
-    uint32_t my_cl = 0, my_adc = 0;
-    {
-        uint32_t qn = 0;
-        auto flush = [&]() {
-            __syncwarp();
-#pragma unroll 1
-            for (uint32_t c0 = 0; c0 < qn; c0 += 32) {
-                const uint32_t ci = c0 + lane;
-                const bool have = ci < qn;
-                int hd = 0, wd = 0;
-                bool ok = false;
-                if (have) {
-                    hd = h.queue[ci];
-                    wd = run_end(mL, hd) - hd + 1;
-                    if (wd <= kWide) ok = accept_serial(adc_l, noise_l, hd, wd, p.tcl2);
-                }
-                uint32_t widem = __ballot_sync(kFull, have && wd > kWide);
-                while (widem) {
-                    const int src = __ffs(widem) - 1;
-                    widem &= widem - 1;
-                    const int hh = __shfl_sync(kFull, hd, src), ww = __shfl_sync(kFull, wd, src);
-                    const bool r = accept_warp(adc_l, noise_l, hh, ww, p.tcl2, lane);
-                    if (lane == src) ok = r;
-                }
-                if (have) {
-                    if (ok) {
-                        ++my_cl;
-                        my_adc += wd;
-                    } else {
-                        atomicAnd(&mH[hd >> 5], ~(1u << (hd & 31)));
-                    }
-                }
-                __syncwarp();
-            }
-            qn = 0;
-        };
-#pragma unroll 1
-        for (uint32_t w = 0; w < nw; ++w) {
-            const uint32_t hs = mH[w];
-            const uint32_t n = __popc(hs);
-            if (!n) continue;
-            if (qn + n > static_cast<uint32_t>(kQCap)) flush();
-            if ((hs >> lane) & 1u) h.queue[qn + __popc(hs & lt)] = static_cast<uint16_t>(w * 32u + lane);
-            qn += n;
-        }
-        flush();
-    }
-    const uint32_t fed_cl = warp_sum(my_cl), fed_adc = warp_sum(my_adc), fed_seed = warp_sum(n_seed);
-
     SST_MARK(7);
-    // ---------------------------------------------------------------- a7: publish, sum predecessors
-    unsigned long long *const st = p.fed_state + static_cast<size_t>(c.ev) * p.n_feds;
+    // ---------------------------------------------------------------- a7, first half: publish + stage
+    // The FED's counts go into its state word; its clusters, cluster ADCs and seeds are staged in
+    // FED-local order in global scratch.  sst_emit_kernel, launched behind this kernel on the same
+    // stream, turns the counts into offsets and moves everything to its (module, first strip)
+    // ordered place -- no warp ever waits for another one.
     if (lane == 0) {
-        st_state(st + f, (static_cast<unsigned long long>(p.epoch) << kShEpoch) |
-                             (static_cast<unsigned long long>(c.overrun) << kShOver) |
-                             (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
-                             (static_cast<unsigned long long>(fed_seed) << kShSeed) |
-                             (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl);
-        // next FED of this warp: the ticket arrives while the look-back and the emit run
+        p.fed_state[static_cast<size_t>(c.ev) * p.n_feds + f] =
+            (static_cast<unsigned long long>(c.overrun) << kShOver) |
+            (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
+            (static_cast<unsigned long long>(fed_seed) << kShSeed) |
+            (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl;
+        // next FED of this warp: the ticket arrives while the staging runs
         next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
     }
-    // clusters | ADC bytes << 32 ; seeds | malformed << 32 (20 bits) | overrun << 52 (n_feds <= 4096)
-    unsigned long long accA = 0, accB = 0;
-#pragma unroll 1
-    for (uint32_t j0 = 0; j0 < f; j0 += 128) {  // warp-uniform control flow: the lanes poll together
-        unsigned long long v[4];
-        bool need[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const uint32_t j = j0 + 32u * u + lane;
-            need[u] = j < f;
-            v[u] = need[u] ? ld_state(st + j) : 0ull;
-        }
-        for (;;) {
-            bool ok = true;
-#pragma unroll
-            for (int u = 0; u < 4; ++u) ok = ok && (!need[u] || (v[u] >> kShEpoch) == p.epoch);
-            if (__all_sync(kFull, ok)) break;
-            __nanosleep(100);  // some predecessor has not published in this launch yet
-#pragma unroll
-            for (int u = 0; u < 4; ++u)
-                if (need[u] && (v[u] >> kShEpoch) != p.epoch) v[u] = ld_state(st + j0 + 32u * u + lane);
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-            if (need[u]) {
-                accA += (v[u] & 0x3fffull) | (((v[u] >> kShAdc) & 0x7fffull) << 32);
-                accB += ((v[u] >> kShSeed) & 0x7fffull) | (((v[u] >> kShMalf) & 0x7full) << 32) |
-                        (((v[u] >> kShOver) & 1ull) << 52);
-            }
-    }
-    accA = warp_sum64(accA);
-    accB = warp_sum64(accB);
-    const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
-    const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
-                   b_over = static_cast<uint32_t>(accB >> 52);
-
-    SST_MARK(8);
-    // ---------------------------------------------------------------- a4: seed-index array (on request)
-    if (o.seed_idx) {
-        uint32_t k0 = b_seed;
-#pragma unroll 1
-        for (uint32_t w = 0; w < nw; ++w) {
-            const uint32_t sw = mS[w];
-            if ((sw >> lane) & 1u) {
-                const uint32_t k = k0 + __popc(sw & lt);
-                if (k < o.cap_seeds) o.seed_idx[k] = f * kFedStrips + (strip_l[w * 32u + lane] & 0x7fffu);
-            }
-            k0 += __popc(sw);
-        }
-    }
-    // ---------------------------------------------------------------- a7: emit, (module, first strip) order
     {
-        uint32_t qn = 0, run_cl = b_cl, run_adc = b_adc;
+        // cluster records: lane per cluster, consecutive lanes write consecutive records
+        const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 3u + f;
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
-        auto flush = [&]() {
-            __syncwarp();
 #pragma unroll 1
-            for (uint32_t c0 = 0; c0 < qn; c0 += 32) {
-                const uint32_t ci = c0 + lane;
-                const bool have = ci < qn;
-                int hd = 0, wd = 0;
-                if (have) {
-                    hd = h.queue[ci];
-                    wd = run_end(mL, hd) - hd + 1;
-                }
-                const uint32_t incl = warp_incl_scan(static_cast<uint32_t>(wd), lane);
-                const uint32_t k_cl = run_cl + ci, k_adc = run_adc + incl - wd;
-                run_adc += __shfl_sync(kFull, incl, 31);
-                if (have && k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc) {
-                    int Q = 0;
-                    long long M = 0;
+        for (uint32_t k0 = 0; k0 < fed_cl; k0 += 32) {
+            const uint32_t k = k0 + lane;
+            if (k < fed_cl) {
+                const uint32_t r0 = rec[k], r1 = rec[k + 1];
+                const uint32_t hd = r0 & 0xffffu, off = r0 >> 16, wd = (r1 >> 16) - off;
+                int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
 #pragma unroll 1
-                    for (int j = 0; j < wd; ++j) {
-                        const int q = adc_l[hd + j];
-                        Q += q;
-                        M += static_cast<long long>(j) * q;
-                        st_stream(o.cl_adc + k_adc + j, static_cast<uint32_t>(q), pol_first);
-                    }
-                    const uint32_t st0 = strip_l[hd] & 0x7fffu;
-                    const uint2 cm = __ldg(cinfo + (st0 >> 8));
-                    const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
-                    st_stream(o.cl_module + k_cl, cm.x, pol_first);
-                    st_stream(o.cl_first + k_cl, static_cast<uint32_t>(first), pol_first);
-                    st_stream(o.cl_width + k_cl, static_cast<uint32_t>(wd), pol_first);
-                    st_stream(o.cl_charge + k_cl, Q, pol_first);
-                    // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
-                    st_stream(o.cl_bary + k_cl,
-                              __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q))),
-                              pol_first);
-                    st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
-                    if (o.cl_snr) o.cl_snr[k_cl] = cluster_snr(noise_l, hd, wd, Q);
-                } else if (have) {
-                    // the first cluster that does not fit reports how many were written
-                    const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
-                    if (prev_fits) *o.n_clusters = k_cl;
+                for (uint32_t j = 0; j < wd; ++j) {
+                    const int q = adc_l[hd + j];
+                    Q += q;
+                    M += static_cast<int>(j) * q;
                 }
-                __syncwarp();
+                const uint32_t st0 = strip_l[hd] & 0x7fffu;
+                const uint2 cm = __ldg(cinfo + (st0 >> 8));
+                const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
+                // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
+                const float bary = __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
+                p.s_rec[sb + k] = make_uint4(cm.x, static_cast<uint32_t>(first) | (wd << 16), static_cast<uint32_t>(Q),
+                                             __float_as_uint(bary));
+                p.s_off[sb + k] = off;
+                if (o.cl_snr)
+                    p.s_snr[sb + k] = static_cast<float>(static_cast<double>(Q) / sqrt(n2_sequential(cal, strip_l, hd, wd)));
             }
-            run_cl += qn;
-            qn = 0;
-        };
-#pragma unroll 1
-        for (uint32_t w = 0; w < nw; ++w) {
-            const uint32_t hs = mH[w];
-            const uint32_t n = __popc(hs);
-            if (!n) continue;
-            if (qn + n > static_cast<uint32_t>(kQCap)) flush();
-            if ((hs >> lane) & 1u) h.queue[qn + __popc(hs & lt)] = static_cast<uint16_t>(w * 32u + lane);
-            qn += n;
         }
-        flush();
-    }
-    if (f == p.n_feds - 1 && lane == 0) {  // event totals = prefix of the last FED + its own
-        const uint32_t n_cl = b_cl + fed_cl, n_adc = b_adc + fed_adc, n_mal = b_malf + c.n_malformed,
-                       n_over = b_over + c.overrun;
-        uint32_t flags = 0;
-        if (n_cl > o.cap_clusters) flags |= SST_FLAG_CLUSTER_CAP;
-        if (n_adc > o.cap_adc) flags |= SST_FLAG_ADC_CAP;
-        if (n_mal) flags |= SST_FLAG_MALFORMED;
-        if (n_over) flags |= SST_FLAG_OVERRUN;
-        if (!(flags & (SST_FLAG_CLUSTER_CAP | SST_FLAG_ADC_CAP))) *o.n_clusters = n_cl;
-        o.dev_status[SST_ST_FLAGS] = flags;
-        o.dev_status[SST_ST_N_MALFORMED] = n_mal;
-        o.dev_status[SST_ST_N_CLUSTERS] = n_cl;
-        o.dev_status[SST_ST_N_ADC] = n_adc;
-        o.dev_status[SST_ST_N_OVERRUN] = n_over;
-        o.dev_status[SST_ST_N_SEEDS] = b_seed + fed_seed;
-        o.dev_status[6] = 0;
-        o.dev_status[7] = 0;
+        // cluster ADCs: lane per entry, the entries of accepted clusters compacted in order
+        const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
+        if (fed_adc) {
+#pragma unroll 2
+            for (uint32_t w = 0; w < nw; ++w) {
+                const uint32_t m = mA[w];
+                if ((m >> lane) & 1u) p.s_adc[ab + (mP[w] & 0xffffu) + __popc(m & lt)] = adc_l[w * 32u + lane];
+            }
+        }
+        // a4: seed-index array (on request), FED-local strip ids
+        if (o.seed_idx) {
+            uint32_t k0 = 0;
+#pragma unroll 1
+            for (uint32_t w = 0; w < nw; ++w) {
+                const uint32_t sw = mS[w];
+                if ((sw >> lane) & 1u) p.s_seed[ab + k0 + __popc(sw & lt)] = strip_l[w * 32u + lane] & 0x7fffu;
+                k0 += __popc(sw);
+            }
+        }
     }
     SST_MARK(9);
-}
-
-// bytes of slot a FED needs on the fast path: payload stage (later noise), lists, four masks
-__device__ __forceinline__ uint32_t slot_need(uint32_t fed_size, uint32_t P) {
-    const uint32_t A = (max((fed_size + 15u) & ~15u, 4u * P) + 15u) & ~15u;
-    return ((A + 3u * P + 3u) & ~3u) + 16u * (((P + 31u) >> 5) + 2u);
+    return true;
 }
 
 // ------------------------------------------------------------------------------ one FED, one warp
-__device__ __forceinline__ void process_fed(const KParams &p, Hdr &h, uint8_t *slot, const uint32_t ticket,
-                                            const int lane, uint32_t &mbar_phase, uint32_t &next_ticket) {
+// Returns false when the FED has to be redone with force_slow (see fed_lists).
+__device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot,
+                                            const uint32_t ticket, const int lane, const bool force_slow,
+                                            uint32_t &mbar_phase, uint32_t &next_ticket) {
     FedCtx c;
     c.ticket = ticket;
-    c.ev = ticket / p.n_feds;
-    c.f = ticket - c.ev * p.n_feds;
+    // FED-major order: the same FED of all the launch's events back to back, so the FED's slab of
+    // the calibration (196 KB) is reused from L2 while it is hot
+    c.f = ticket / p.n_events;
+    c.ev = ticket - c.f * p.n_events;
     const uint32_t f = c.f;
     const EventDesc &E = p.ev[c.ev];
     const sst_output &o = E.out;
+    uint32_t *const chan_off = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
+    uint16_t *const chan_len = reinterpret_cast<uint16_t *>(chan_off + kChan);
 
     SST_MARK(0);
     // ---------------------------------------------------------------- a1: stage the FED payload
@@ -802,13 +765,13 @@ __device__ __forceinline__ void process_fed(const KParams &p, Hdr &h, uint8_t *s
     c.fed_start = valid ? fo0 : 0u;
     c.fed_size = valid ? fo1 - fo0 : 0u;
     c.overrun = valid ? 0u : 1u;
-    const bool staged = c.fed_size <= p.slot_bytes && ((c.fed_start | c.fed_size) & 15u) == 0 &&
+    const bool staged = !force_slow && c.fed_size + kTabBytes <= p.slot_bytes && ((c.fed_start | c.fed_size) & 15u) == 0 &&
                         (reinterpret_cast<uintptr_t>(E.raw) & 15u) == 0;
     __syncwarp();  // every lane is done with the slot of the previous FED
     if (staged && c.fed_size && lane == 0) {
         fence_proxy_async();  // earlier generic-proxy accesses to the slot before the async write
-        mbar_expect_tx(&h.mbar, c.fed_size);
-        bulk_g2s(slot, E.raw + c.fed_start, c.fed_size, &h.mbar, policy_evict_first());
+        mbar_expect_tx(mbar, c.fed_size);
+        bulk_g2s(slot, E.raw + c.fed_start, c.fed_size, mbar, policy_evict_first());
     }
     // meanwhile: fetch the module map
     c.opens = 0;
@@ -820,21 +783,21 @@ __device__ __forceinline__ void process_fed(const KParams &p, Hdr &h, uint8_t *s
     }
     const uint8_t *rp = staged ? slot : E.raw + c.fed_start;
     if (staged && c.fed_size) {
-        mbar_wait(&h.mbar, mbar_phase);  // every lane waits: async-proxy writes visible to all readers
+        mbar_wait(mbar, mbar_phase);  // every lane waits: async-proxy writes visible to all readers
         mbar_phase ^= 1u;
     }
 
     SST_MARK(1);
     // ---------------------------------------------------------------- a1: walk the length chain
     if (staged) {
-        if (lane == 0) walk_chain_speculative(slot, p.slot_bytes - 2u, h.chan_off, h.chan_len);
+        if (lane == 0) walk_chain_speculative(slot, p.slot_bytes - kTabBytes - 2u, chan_off, chan_len);
         __syncwarp();
         // validate the speculative chain: channels from the first bad one on are empty
         uint32_t bad = 0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            c.off[k] = h.chan_off[lane + 32 * k];
-            c.len[k] = h.chan_len[lane + 32 * k];
+            c.off[k] = chan_off[lane + 32 * k];
+            c.len[k] = chan_len[lane + 32 * k];
             const bool ok = c.overrun == 0 && c.off[k] <= c.fed_size && c.off[k] + c.len[k] <= c.fed_size;
             const uint32_t m = ~__ballot_sync(kFull, ok);
             if (!bad && m) bad = 32u * k + __ffs(m);  // 1 + index of the first bad channel
@@ -850,33 +813,28 @@ __device__ __forceinline__ void process_fed(const KParams &p, Hdr &h, uint8_t *s
         }
     } else {
         uint32_t over = c.overrun;
-        if (lane == 0) over = walk_chain_checked(rp, c.fed_size, c.overrun != 0, h.chan_off, h.chan_len) ? 1u : 0u;
+        if (lane == 0) over = walk_chain_checked(rp, c.fed_size, c.overrun != 0, chan_off, chan_len) ? 1u : 0u;
         c.overrun = __shfl_sync(kFull, over, 0);
         __syncwarp();
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            c.off[k] = h.chan_off[lane + 32 * k];
-            c.len[k] = h.chan_len[lane + 32 * k];
+            c.off[k] = chan_off[lane + 32 * k];
+            c.len[k] = chan_len[lane + 32 * k];
         }
     }
+    __syncwarp();  // the channel table is in registers: its place in the slot is free
 
     SST_MARK(2);
     // ---------------------------------------------------------------- a2 pass 1: run headers
-    // lane per channel: validate the run list, count the strips
-    uint32_t cnt[3];
-    c.n_malformed = 0;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         const uint32_t ch = lane + 32 * k;
         if (o.chan_off) o.chan_off[f * kChan + ch] = c.fo0 + c.off[k];
         if (o.chan_len) o.chan_len[f * kChan + ch] = static_cast<uint16_t>(c.len[k]);
-        uint32_t n_strips = 0;
-        const bool ok = staged ? scan_runs(slot, c.off[k], c.len[k], n_strips) : scan_runs(rp, c.off[k], c.len[k], n_strips);
-        __syncwarp();
-        cnt[k] = ok ? n_strips : 0u;
-        if (!ok) c.len[k] = 0;  // a malformed channel contributes no strips
-        c.n_malformed += __popc(__ballot_sync(kFull, !ok));
     }
+    uint32_t cnt[3];
+    if (staged) scan_runs3(slot, c, cnt);
+    else scan_runs3(rp, c, cnt);
     // exclusive scan of the 96 counts
     uint32_t run = 0;
 #pragma unroll
@@ -888,21 +846,25 @@ __device__ __forceinline__ void process_fed(const KParams &p, Hdr &h, uint8_t *s
     c.P = run;  // present strips of the FED
 
     SST_MARK(3);
-    if (staged && slot_need(c.fed_size, c.P) <= p.slot_bytes)
-        fed_lists<true>(p, h, slot, slot, c, lane, next_ticket);
-    else
-        fed_lists<false>(p, h, slot, rp, c, lane, next_ticket);
+    // fast path: lists behind the payload, masks and at least a few records in its place
+    const uint32_t A = (c.fed_size + 15u) & ~15u;
+    if (staged && A + 3u * c.P <= p.slot_bytes && 16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
+        return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
+    return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
 
 // ------------------------------------------------------------------------------ the kernel
-// A CTA is one warp.  Warps draw (event, FED) tickets until the launch's work is used up.
-__global__ void __launch_bounds__(32, 24) sst_event_kernel(const __grid_constant__ KParams p) {
+// Every warp works alone: it draws (event, FED) tickets until the launch's work is used up and
+// never meets a block-wide barrier.  A CTA is just 1..kWarpsPerCta such warps sharing the SM's
+// shared memory (one driver reserve per CTA instead of one per warp).
+__global__ void __launch_bounds__(32 * kWarpsPerCta, 7) sst_event_kernel(const __grid_constant__ KParams p) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
-    Hdr &h = *reinterpret_cast<Hdr *>(smem_raw);
-    uint8_t *slot = smem_raw + kHdrBytes;
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    uint8_t *const mine = smem_raw + static_cast<size_t>(threadIdx.x >> 5) * (kWarpHdr + p.slot_bytes + kTailPad);
+    unsigned long long *const mbar = reinterpret_cast<unsigned long long *>(mine);
+    uint8_t *const slot = mine + kWarpHdr;
     if (lane == 0) {
-        mbar_init(&h.mbar, 1);
+        mbar_init(mbar, 1);
         fence_proxy_async();
     }
     __syncwarp();
@@ -913,8 +875,95 @@ __global__ void __launch_bounds__(32, 24) sst_event_kernel(const __grid_constant
     ticket = __shfl_sync(kFull, ticket, 0);
     while (ticket < total) {
         uint32_t next_ticket = 0;
-        process_fed(p, h, slot, ticket, lane, mbar_phase, next_ticket);
+        if (!process_fed(p, mbar, slot, ticket, lane, false, mbar_phase, next_ticket))
+            process_fed(p, mbar, slot, ticket, lane, true, mbar_phase, next_ticket);
         ticket = __shfl_sync(kFull, next_ticket, 0);
+    }
+}
+
+// ------------------------------------------------------------------------------ a7, second half
+// One warp per (event, FED), behind sst_event_kernel on the same stream: sums the state words of
+// the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then moves the staged
+// records, cluster ADCs and seeds of the FED to their final place.  Output capacity and the event
+// totals are handled here.
+__global__ void __launch_bounds__(128) sst_emit_kernel(const __grid_constant__ KParams p) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (t >= p.n_events * p.n_feds) return;
+    const uint32_t ev = t / p.n_feds, f = t - ev * p.n_feds;
+    const EventDesc &E = p.ev[ev];
+    const sst_output &o = E.out;
+    const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
+    const unsigned long long own = st[f];
+    const uint32_t fed_cl = static_cast<uint32_t>(own & 0x3fffull), fed_adc = static_cast<uint32_t>((own >> kShAdc) & 0x7fffull),
+                   fed_seed = static_cast<uint32_t>((own >> kShSeed) & 0x7fffull),
+                   fed_malf = static_cast<uint32_t>((own >> kShMalf) & 0x7full), fed_over = static_cast<uint32_t>((own >> kShOver) & 1ull);
+    // clusters | ADC bytes << 32 ; seeds | malformed << 32 (20 bits) | overrun << 52 (n_feds <= 4096)
+    unsigned long long accA = 0, accB = 0;
+#pragma unroll 2
+    for (uint32_t j = lane; j < f; j += 32) {
+        const unsigned long long v = st[j];
+        accA += (v & 0x3fffull) | (((v >> kShAdc) & 0x7fffull) << 32);
+        accB += ((v >> kShSeed) & 0x7fffull) | (((v >> kShMalf) & 0x7full) << 32) | (((v >> kShOver) & 1ull) << 52);
+    }
+    accA = warp_sum64(accA);
+    accB = warp_sum64(accB);
+    const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
+    const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
+                   b_over = static_cast<uint32_t>(accB >> 52);
+    // where sst_event_kernel staged this FED
+    const uint32_t fo0 = E.fed_offsets[f], fo1 = E.fed_offsets[f + 1];
+    const uint32_t fed_start = (fo0 <= fo1 && fo1 <= p.max_raw_bytes) ? fo0 : 0u;
+    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 3u + f;
+    const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
+    const unsigned long long pol_first = policy_evict_first();
+
+    const bool all_fit = b_cl + fed_cl <= o.cap_clusters && b_adc + fed_adc <= o.cap_adc;
+    uint32_t lim = 0;  // ADC bytes of this FED that belong to clusters that fit
+#pragma unroll 1
+    for (uint32_t k = lane; k < fed_cl; k += 32) {
+        const uint4 r = p.s_rec[sb + k];
+        const uint32_t off = p.s_off[sb + k], wd = r.y >> 16;
+        const uint32_t k_cl = b_cl + k, k_adc = b_adc + off;
+        if (all_fit || (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc)) {
+            st_stream(o.cl_module + k_cl, r.x, pol_first);
+            st_stream(o.cl_first + k_cl, r.y & 0xffffu, pol_first);
+            st_stream(o.cl_width + k_cl, wd, pol_first);
+            st_stream(o.cl_charge + k_cl, static_cast<int32_t>(r.z), pol_first);
+            st_stream(o.cl_bary + k_cl, __uint_as_float(r.w), pol_first);
+            st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
+            if (o.cl_snr) o.cl_snr[k_cl] = p.s_snr[sb + k];
+            lim = off + wd;
+        } else {
+            // the first cluster that does not fit reports how many were written
+            const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
+            if (prev_fits) *o.n_clusters = k_cl;
+        }
+    }
+    lim = all_fit ? fed_adc : __reduce_max_sync(kFull, lim);
+#pragma unroll 2
+    for (uint32_t i = lane; i < lim; i += 32) st_stream(o.cl_adc + b_adc + i, static_cast<uint32_t>(p.s_adc[ab + i]), pol_first);
+    if (o.seed_idx) {
+#pragma unroll 1
+        for (uint32_t i = lane; i < fed_seed; i += 32)
+            if (b_seed + i < o.cap_seeds) o.seed_idx[b_seed + i] = f * kFedStrips + p.s_seed[ab + i];
+    }
+    if (f == p.n_feds - 1 && lane == 0) {  // event totals = prefix of the last FED + its own
+        const uint32_t t_cl = b_cl + fed_cl, t_adc = b_adc + fed_adc, n_mal = b_malf + fed_malf, n_over = b_over + fed_over;
+        uint32_t flags = 0;
+        if (t_cl > o.cap_clusters) flags |= SST_FLAG_CLUSTER_CAP;
+        if (t_adc > o.cap_adc) flags |= SST_FLAG_ADC_CAP;
+        if (n_mal) flags |= SST_FLAG_MALFORMED;
+        if (n_over) flags |= SST_FLAG_OVERRUN;
+        if (!(flags & (SST_FLAG_CLUSTER_CAP | SST_FLAG_ADC_CAP))) *o.n_clusters = t_cl;
+        o.dev_status[SST_ST_FLAGS] = flags;
+        o.dev_status[SST_ST_N_MALFORMED] = n_mal;
+        o.dev_status[SST_ST_N_CLUSTERS] = t_cl;
+        o.dev_status[SST_ST_N_ADC] = t_adc;
+        o.dev_status[SST_ST_N_OVERRUN] = n_over;
+        o.dev_status[SST_ST_N_SEEDS] = b_seed + fed_seed;
+        o.dev_status[6] = 0;
+        o.dev_status[7] = 0;
     }
 }
 
@@ -929,13 +978,17 @@ struct sst_ctx {
     bool has_calib = false;
     std::atomic<int32_t> last_err{0};
     int sm_count = 0;
-    int ctas_per_sm = 0;
-    uint32_t slot_bytes = 0;  // shared-memory slot of one warp (one FED)
-    uint32_t smem_bytes = 0;  // header + slot
+    int ctas_per_sm = 0;       // resident CTAs of kWarpsPerCta warps
+    uint32_t slot_bytes = 0;   // shared-memory slot of one warp (one FED)
+    uint32_t warp_stride = 0;  // mbarrier + slot + tail pad
+    uint32_t smem_bytes = 0;   // kWarpsPerCta * warp_stride
     // per-stream scratch (ticket counter, FED states, slow-path lists), taken from the pool on a
     // stream's first launch and kept: stream order makes reuse safe, the epoch and the running
     // ticket base make clearing unnecessary
-    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t epoch; unsigned long long ticket_base; };
+    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t cap_events; unsigned long long ticket_base; };
+    // cross-stream dependencies of the batched entry point: one event per stream, made on first use
+    struct StreamEvent { cudaStream_t stream; cudaEvent_t ev; };
+    std::vector<StreamEvent> stream_events;
     std::mutex slot_mu;
     std::vector<Slot> slots;
 };
@@ -967,22 +1020,31 @@ unsigned long long *g_phase_clk = nullptr;
 #endif
 
 struct ScratchLayout {
-    size_t ents, mwords, state_bytes, o_ticket, o_state, o_noise, o_mask, o_strip, o_adc, total;
+    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr,
+        o_sadc, o_sseed, total;
 };
-ScratchLayout scratch_layout(const sst_ctx *ctx) {
+ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     ScratchLayout L{};
     const uint32_t nf = ctx->cfg.n_feds;
     auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
     L.ents = (static_cast<size_t>(ctx->cfg.max_raw_bytes) + 16ull * nf + 64 + 31) & ~static_cast<size_t>(31);
     L.mwords = L.ents / 32 + 4ull * nf + 16;
-    L.state_bytes = sizeof(unsigned long long) * nf * kMaxEv;
+    L.cl_slots = static_cast<size_t>(ctx->cfg.max_raw_bytes) / 3 + nf + 8;  // a cluster costs >= 3 raw bytes
+    L.state_bytes = sizeof(unsigned long long) * nf * cap_events;
     L.o_ticket = 0;
     L.o_state = 256;
-    L.o_noise = L.o_state + up(L.state_bytes);
-    L.o_mask = L.o_noise + up(4 * L.ents * kMaxEv);
-    L.o_strip = L.o_mask + up(4 * 4 * L.mwords * kMaxEv);
-    L.o_adc = L.o_strip + up(2 * L.ents * kMaxEv);
-    L.total = L.o_adc + up(L.ents * kMaxEv);
+    // slow-path lists
+    L.o_rec = L.o_state + up(L.state_bytes);
+    L.o_mask = L.o_rec + up(4 * L.ents * cap_events);
+    L.o_strip = L.o_mask + up(4 * 4 * L.mwords * cap_events);
+    L.o_adc = L.o_strip + up(2 * L.ents * cap_events);
+    // staging between the two kernels
+    L.o_srec = L.o_adc + up(L.ents * cap_events);
+    L.o_soff = L.o_srec + up(16 * L.cl_slots * cap_events);
+    L.o_ssnr = L.o_soff + up(4 * L.cl_slots * cap_events);
+    L.o_sadc = L.o_ssnr + up(4 * L.cl_slots * cap_events);
+    L.o_sseed = L.o_sadc + up(L.ents * cap_events);
+    L.total = L.o_sseed + up(2 * L.ents * cap_events);
     return L;
 }
 
@@ -990,44 +1052,58 @@ ScratchLayout scratch_layout(const sst_ctx *ctx) {
 sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, const uint32_t *const *fed_offsets,
                          const sst_thresholds *thr, const sst_output *const *outs, cudaStream_t st) {
     const uint32_t nf = ctx->cfg.n_feds;
-    const ScratchLayout L = scratch_layout(ctx);
     const uint32_t total = n * nf;
-    const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm);
-    const uint32_t grid = std::min(total, capacity);
+    // warps per CTA: full CTAs once the work fills the GPU, smaller ones to spread a small launch
+    const uint32_t sms = static_cast<uint32_t>(ctx->sm_count);
+    const uint32_t wpc = total >= 8u * sms ? kWarpsPerCta : total >= 4u * sms ? 2u : 1u;
+    const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (kWarpsPerCta / wpc);
+    const uint32_t grid = std::min((total + wpc - 1) / wpc, capacity);
     uint8_t *blk = nullptr;
-    uint32_t epoch = 0;
     unsigned long long ticket_base = 0;
+    uint32_t cap = 0;
     {
         std::lock_guard<std::mutex> lock(ctx->slot_mu);
         sst_ctx::Slot *sl = nullptr;
         for (auto &s : ctx->slots)
             if (s.stream == st) sl = &s;
         if (!sl) {
-            SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), L.total, ctx->pool, st));
-            SST_CU(cudaMemsetAsync(blk, 0, L.o_noise, st));  // ticket counter and states
-            ctx->slots.push_back({st, blk, 0u, 0ull});
+            ctx->slots.push_back({st, nullptr, 0u, 0ull});
             sl = &ctx->slots.back();
         }
-        if (sl->epoch == kEpochMax) {  // epoch wraps: stale words of 4095 launches ago must not match
-            SST_CU(cudaMemsetAsync(sl->mem + L.o_state, 0, L.state_bytes, st));
-            sl->epoch = 0;
+        if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8 or kMaxEv events
+            if (sl->mem) SST_CU(cudaFreeAsync(sl->mem, st));
+            sl->mem = nullptr;
+            sl->cap_events = 0;
+            const uint32_t want = n <= 1 ? 1u : n <= 8 ? 8u : static_cast<uint32_t>(kMaxEv);
+            const ScratchLayout Ln = scratch_layout(ctx, want);
+            SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), Ln.total, ctx->pool, st));
+            SST_CU(cudaMemsetAsync(blk, 0, Ln.o_rec, st));  // ticket counter and states
+            sl->mem = blk;
+            sl->cap_events = want;
+            sl->ticket_base = 0;
         }
-        sl->epoch += 1;
         blk = sl->mem;
-        epoch = sl->epoch;
+        cap = sl->cap_events;
         ticket_base = sl->ticket_base;
-        sl->ticket_base += static_cast<unsigned long long>(total) + grid;  // every warp draws one ticket too many
+        sl->ticket_base += static_cast<unsigned long long>(total) + grid * wpc;  // every warp draws one ticket too many
     }
+    const ScratchLayout L = scratch_layout(ctx, cap);
     KParams kp{};
     kp.calib = ctx->calib;
     kp.chan_info = ctx->chan_info;
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
     kp.ticket_base = ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
-    kp.g_noise = reinterpret_cast<float *>(blk + L.o_noise);
+    kp.g_rec = reinterpret_cast<uint32_t *>(blk + L.o_rec);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
     kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
     kp.g_adc = blk + L.o_adc;
+    kp.s_rec = reinterpret_cast<uint4 *>(blk + L.o_srec);
+    kp.s_off = reinterpret_cast<uint32_t *>(blk + L.o_soff);
+    kp.s_snr = reinterpret_cast<float *>(blk + L.o_ssnr);
+    kp.s_adc = blk + L.o_sadc;
+    kp.s_seed = reinterpret_cast<uint16_t *>(blk + L.o_sseed);
+    kp.s_cl_stride = static_cast<uint32_t>(L.cl_slots);
     kp.g_ents = static_cast<uint32_t>(L.ents);
     kp.g_mwords = static_cast<uint32_t>(L.mwords);
     kp.tcl2 = static_cast<double>(thr->cluster) * static_cast<double>(thr->cluster);  // exact
@@ -1036,7 +1112,6 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.max_raw_bytes = ctx->cfg.max_raw_bytes;
     kp.n_feds = nf;
     kp.n_events = n;
-    kp.epoch = epoch;
     kp.slot_bytes = ctx->slot_bytes;
 #ifdef SST_PHASE_TIMING
     kp.phase_clk = g_phase_clk;
@@ -1046,7 +1121,9 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         kp.ev[e].fed_offsets = fed_offsets[e];
         kp.ev[e].out = *outs[e];
     }
-    sst_event_kernel<<<grid, 32, ctx->smem_bytes, st>>>(kp);
+    sst_event_kernel<<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
+    SST_CU(cudaGetLastError());
+    sst_emit_kernel<<<(total + 3) / 4, 128, 0, st>>>(kp);
     SST_CU(cudaGetLastError());
     return SST_OK;
 }
@@ -1089,36 +1166,62 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (cudaMalloc(&ctx->chan_info, static_cast<size_t>(cfg->n_feds) * kChan * sizeof(uint2)) !=
         cudaSuccess)
         return fail(SST_ERR_CUDA);
-    // shared-memory slot of one warp: sized for the largest FED the configuration expects (FEDs
-    // that do not fit take the slow path through the global scratch)
+    // Shared-memory slot of one warp: payload stage + the lists {strip u16, adc u8} of the present
+    // strips (masks and cluster records reuse the payload's place), sized from the configuration's
+    // hints; FEDs that do not fit take the slow path through the global scratch.  The slot is then
+    // grown to whatever the SM's shared memory leaves at the same number of resident CTAs.
+    cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device);
     {
         const double m = static_cast<double>(cfg->max_raw_bytes) / cfg->n_feds;  // mean payload bound
         const uint32_t p_hint = cfg->fed_strips_hint ? std::min(cfg->fed_strips_hint, static_cast<uint32_t>(kFedStrips))
-                                                     : static_cast<uint32_t>(0.55 * m) + 32u;
+                                                     : static_cast<uint32_t>(0.5 * m) + 32u;
         const uint32_t r_hint = (static_cast<uint32_t>(std::min(1.15 * m + 64.0, 65536.0)) + 15u) & ~15u;
-        const uint32_t A = (std::max(r_hint, 4u * p_hint) + 15u) & ~15u;
-        uint32_t need = ((A + 3u * p_hint + 3u) & ~3u) + 16u * (((p_hint + 31u) >> 5) + 2u);
-        need = (need + 127u) & ~127u;
-        ctx->slot_bytes = std::min(std::max(need, 2048u), 200u * 1024u);
-        ctx->smem_bytes = kHdrBytes + ctx->slot_bytes + 16u;  // tail pad, see pass 2
+        uint32_t need = std::max(r_hint + kTabBytes, r_hint + 3u * p_hint);
+        need = std::min(std::max((need + 15u) & ~15u, 2048u), 50u * 1024u);
+        auto set_slot = [&](uint32_t slot) {
+            ctx->slot_bytes = slot;
+            ctx->warp_stride = kWarpHdr + slot + kTailPad;
+            ctx->smem_bytes = kWarpsPerCta * ctx->warp_stride;
+        };
+        set_slot(need);
+        if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 static_cast<int>(ctx->smem_bytes)) != cudaSuccess)
+            return fail(SST_ERR_CUDA);
+        cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->ctas_per_sm, sst_event_kernel, 32 * kWarpsPerCta,
+                                                          ctx->smem_bytes) != cudaSuccess || ctx->ctas_per_sm < 1)
+            return fail(SST_ERR_CUDA);
+        size_t avail = 0;
+        if (cudaOccupancyAvailableDynamicSMemPerBlock(&avail, sst_event_kernel, ctx->ctas_per_sm, 32 * kWarpsPerCta) ==
+                cudaSuccess && avail > ctx->smem_bytes) {
+            const uint32_t per_warp = static_cast<uint32_t>(std::min<size_t>(avail, 227u * 1024u) / kWarpsPerCta);
+            const uint32_t slot = (per_warp - kWarpHdr - kTailPad) & ~15u;
+            if (slot > ctx->slot_bytes) {
+                set_slot(slot);
+                if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(ctx->smem_bytes)) != cudaSuccess)
+                    return fail(SST_ERR_CUDA);
+                int check = 0;
+                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel, 32 * kWarpsPerCta,
+                                                                  ctx->smem_bytes) != cudaSuccess || check < ctx->ctas_per_sm) {
+                    set_slot(need);  // the grown slot lost a CTA: keep the hinted size
+                }
+            }
+        }
+        cudaGetLastError();
     }
-    if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             static_cast<int>(ctx->smem_bytes)) != cudaSuccess)
-        return fail(SST_ERR_CUDA);
-    cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     {
         // L2 set-aside for the calibration (read by every event with an evict_last policy): the
         // device maximum (79 of 126 MB on B200).  A device-wide limit; failure is not fatal.
         int max_persist = 0;
-        if (cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, cfg->device) == cudaSuccess &&
+#ifndef SST_X_PERSIST
+        max_persist = -1;
+#endif
+        if (max_persist >= 0 && cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, cfg->device) == cudaSuccess &&
             max_persist > 0)
             cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, static_cast<size_t>(max_persist));
         cudaGetLastError();
     }
-    cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->ctas_per_sm, sst_event_kernel, 32,
-                                                      ctx->smem_bytes) != cudaSuccess || ctx->ctas_per_sm < 1)
-        return fail(SST_ERR_CUDA);
     *out_ctx = ctx;
     return SST_OK;
 }
@@ -1183,20 +1286,60 @@ sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8
     for (uint32_t e = 0; e < n_events; ++e)
         if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e])) return SST_ERR_INVALID_ARG;
     SST_CU(cudaSetDevice(ctx->cfg.device));
-    // the events of one stream go into launches of up to kMaxEv events each
-    for (uint32_t s = 0; s < n_streams && s < n_events; ++s) {
+    // Launch groups.  The events of several streams share one launch so that the kernel walks them
+    // FED by FED (the FED's calibration slab is then read from HBM once per launch, not once per
+    // event): stream s belongs to group s % G, the group's launches run on its first stream, which
+    // first waits for the other streams of the group (their uploads) and is waited for by them
+    // afterwards, so every event's result is stream-ordered on its own stream as documented.
+    const uint32_t ns = std::min(n_streams, n_events);
+    const uint32_t G = std::min(ns, 2u);
+    auto event_of = [&](cudaStream_t st, cudaEvent_t *out) -> bool {
+        std::lock_guard<std::mutex> lock(ctx->slot_mu);
+        for (auto &se : ctx->stream_events)
+            if (se.stream == st) { *out = se.ev; return true; }
+        cudaEvent_t ev = nullptr;
+        if (!cu_ok(ctx, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming))) return false;
+        ctx->stream_events.push_back({st, ev});
+        *out = ev;
+        return true;
+    };
+    for (uint32_t g = 0; g < G; ++g) {
+        cudaStream_t lead = static_cast<cudaStream_t>(streams[g]);
+        for (uint32_t s = g + G; s < ns; s += G) {  // the group's other streams: inputs ready
+            cudaStream_t st = static_cast<cudaStream_t>(streams[s]);
+            if (st == lead) continue;
+            cudaEvent_t ev;
+            if (!event_of(st, &ev)) return SST_ERR_CUDA;
+            SST_CU(cudaEventRecord(ev, st));
+            SST_CU(cudaStreamWaitEvent(lead, ev, 0));
+        }
         const uint8_t *r[kMaxEv];
         const uint32_t *fo[kMaxEv];
         const sst_output *o[kMaxEv];
-        uint32_t n = 0;
-        for (uint32_t e = s; e < n_events; e += n_streams) {
+        uint32_t n = 0, left = 0;
+        for (uint32_t e = 0; e < n_events; ++e)
+            if ((e % n_streams) % G == g) ++left;
+        for (uint32_t e = 0; e < n_events; ++e) {
+            if ((e % n_streams) % G != g) continue;
             r[n] = raw[e];
             fo[n] = fed_offsets[e];
             o[n] = &outs[e];
-            if (++n == kMaxEv || e + n_streams >= n_events) {
-                const sst_status rc = launch_events(ctx, n, r, fo, thr, o, static_cast<cudaStream_t>(streams[s]));
+            --left;
+            if (++n == kMaxEv || left == 0) {
+                const sst_status rc = launch_events(ctx, n, r, fo, thr, o, lead);
                 if (rc != SST_OK) return rc;
                 n = 0;
+            }
+        }
+        bool others = false;
+        for (uint32_t s = g + G; s < ns; s += G) others = others || static_cast<cudaStream_t>(streams[s]) != lead;
+        if (others) {
+            cudaEvent_t done;
+            if (!event_of(lead, &done)) return SST_ERR_CUDA;
+            SST_CU(cudaEventRecord(done, lead));
+            for (uint32_t s = g + G; s < ns; s += G) {
+                cudaStream_t st = static_cast<cudaStream_t>(streams[s]);
+                if (st != lead) SST_CU(cudaStreamWaitEvent(st, done, 0));
             }
         }
     }
@@ -1319,7 +1462,9 @@ sst_status sst_destroy(sst_ctx *ctx) {
     if (!ctx) return SST_ERR_INVALID_ARG;
     cudaSetDevice(ctx->cfg.device);
     cudaDeviceSynchronize();
-    for (auto &sl : ctx->slots) cudaFreeAsync(sl.mem, nullptr);
+    for (auto &sl : ctx->slots)
+        if (sl.mem) cudaFreeAsync(sl.mem, nullptr);
+    for (auto &se : ctx->stream_events) cudaEventDestroy(se.ev);
     cudaDeviceSynchronize();
     if (ctx->calib) cudaFree(ctx->calib);
     if (ctx->chan_info) cudaFree(ctx->chan_info);
@@ -1344,10 +1489,10 @@ const char *sst_status_string(sst_status s) {
 sst_status sst_get_info(const sst_ctx *ctx, sst_info *info) {
     if (!ctx || !info) return SST_ERR_INVALID_ARG;
     info->smem_bytes = ctx->smem_bytes;
-    info->threads = 32;
+    info->threads = 32 * kWarpsPerCta;
     info->ctas_per_sm = static_cast<uint32_t>(ctx->ctas_per_sm);
     info->sm_count = static_cast<uint32_t>(ctx->sm_count);
-    info->kernels_per_event = 1;
+    info->kernels_per_event = 2;
     info->slot_bytes = ctx->slot_bytes;
     info->events_per_launch = kMaxEv;
     return SST_OK;

@@ -375,3 +375,38 @@ def test_multi_event_streams_match_single_event(H, oracle):
                 compare(H.unsigned_view(outs.numpy()), r)
     finally:
         det.close()
+
+
+def test_batched_entry_point_matches_single_event(H, oracle):
+    """sst_unpack_cluster_batch: events of several streams share FED-major launches; every event's
+    output still equals its single-event oracle output, for 1, 3 and 8 streams and for more events
+    than one launch takes."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf = 7
+    n_ev = 70
+    cfg, cal, evs = synth.make_config(3, n_feds=nf, event_seeds=range(1, n_ev + 1))
+    want = [oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            for e in evs]
+    mrb = max(int(e.raw.size) for e in evs)
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        d_in = [det.upload_raw(e.raw, e.fed_offsets) for e in evs]
+        for n_streams in (1, 3, 8):
+            streams = [torch.cuda.Stream() for _ in range(n_streams)]
+            outs = [det.alloc_outputs(mrb // 3 + 1, mrb, chan_map=True, seeds=True, snr=True) for _ in evs]
+            batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs],
+                            [s.cuda_stream for s in streams])
+            torch.cuda.synchronize()
+            for _ in range(2):          # twice: scratch and ticket counters are reused
+                B.sst_unpack_cluster_batch(det.ctx, batch)
+            # each event's result is ordered on its own stream
+            for i, o in enumerate(outs):
+                with torch.cuda.stream(streams[i % n_streams]):
+                    got = {k: v.clone() for k, v in o.tensors.items()}
+                o.tensors.update(got)
+            torch.cuda.synchronize()
+            for o, r in zip(outs, want):
+                compare(H.unsigned_view(o.numpy()), r)
+    finally:
+        det.close()
