@@ -46,6 +46,9 @@
 
 #include "sst.h"
 
+#ifndef SST_MIN_CTAS
+#define SST_MIN_CTAS 7
+#endif
 #ifndef SST_MAXEV
 #define SST_MAXEV 32
 #endif
@@ -172,12 +175,6 @@ __device__ __forceinline__ float2 ld_calib(const float2 *p, unsigned long long p
                  : "=f"(v.x), "=f"(v.y)
                  : "l"(p), "l"(pol));
     return v;
-}
-// Fire-and-forget fetch of a strip's calibration into L2: issued from pass 2 as soon as the strip
-// id is known, so that the gather of the sweep, tens of microseconds later, is an L2 hit and DRAM
-// sees all FEDs' misses at once instead of four per lane and round trip.
-__device__ __forceinline__ void prefetch_calib(const float2 *p) {
-    asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(p));
 }
 // streaming stores of the outputs
 __device__ __forceinline__ void st_stream(uint4 *p, uint4 v, unsigned long long pol) {
@@ -377,6 +374,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     uint8_t *adc_l;
     uint32_t *mS, *mA, *mH, *mP, *rec;
     uint32_t rec_cap;  // cluster records besides the end sentinel
+    uint8_t *window;   // 1 KB of shared memory for the dense SoA, free between pass 2 and the sweep
     if (kFast) {
         // [0, A): the payload, and once the lists are built the masks and the cluster records
         const uint32_t A = (c.fed_size + 15u) & ~15u;
@@ -388,6 +386,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         mP = mH + (nw + 2);
         rec = mP + (nw + 2);
         rec_cap = (A - 16u * (nw + 2)) / 4u - 1u;
+        window = A >= 1024u ? slot : slot + ((A + 3u * P + 15u) & ~15u);
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
@@ -399,28 +398,11 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         mH = mA + p.g_mwords;
         mP = mH + p.g_mwords;
         rec_cap = 0xffffffffu;
+        window = slot;
     }
     const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
 
-    // ---------------------------------------------------------------- a2: dense SoA, zero fill
-    // the whole FED row block by the warp (coalesced 16-byte stores), just before pass 2 scatters
-    // the present strips into it
     uint8_t *const dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips : nullptr;
-#ifdef SST_X_NO_FILL
-    if (false) {
-#else
-    if (dense) {
-#endif
-        if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0) {
-#pragma unroll 4
-            for (uint32_t b = 16u * lane; b < static_cast<uint32_t>(kFedStrips); b += 512u)
-                st_stream(reinterpret_cast<uint4 *>(dense + b), make_uint4(0, 0, 0, 0), pol_first);
-        } else {
-#pragma unroll 1
-            for (uint32_t b = lane; b < static_cast<uint32_t>(kFedStrips); b += 32u) dense[b] = 0;
-        }
-        __syncwarp();  // orders the zeros before the scatter of other lanes
-    }
 
     // ---------------------------------------------------------------- a2 pass 2: lane per channel
     // writes {strip, adc} in ascending strip order; bit 15 of a strip id marks strip 0 of a channel
@@ -456,20 +438,14 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     const uint32_t open_bit = ((c.opens >> k) & 1u) << 15;
                     strip_l[ee] = static_cast<uint16_t>(first == 0 ? sid | open_bit : sid);
                     adc_l[ee] = static_cast<uint8_t>(b0);
-                    prefetch_calib(cal + sid);
-                    if (SST_X_SCATTER && dense) st_stream(dense + sid, b0, pol_first);
                     if (len > 1) {
                         strip_l[ee + 1] = static_cast<uint16_t>(sid + 1u);
                         adc_l[ee + 1] = static_cast<uint8_t>(b1);
-                        if (((sid + 1u) & 3u) == 0) prefetch_calib(cal + sid + 1u);
-                        if (SST_X_SCATTER && dense) st_stream(dense + sid + 1u, b1, pol_first);
 #pragma unroll 1
                         for (uint32_t i = 2; i < len; ++i) {
                             const uint32_t bi = rp[qq + 2 + i];
                             strip_l[ee + i] = static_cast<uint16_t>(sid + i);
                             adc_l[ee + i] = static_cast<uint8_t>(bi);
-                            if (((sid + i) & 3u) == 0) prefetch_calib(cal + sid + i);  // next 32-byte sector
-                            if (SST_X_SCATTER && dense) st_stream(dense + sid + i, bi, pol_first);
                         }
                     }
                     e[k] = ee + len;
@@ -480,6 +456,45 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         }
     }
     __syncwarp();  // lists complete; the payload is dead from here on
+
+    // ---------------------------------------------------------------- a2: dense SoA
+    // The FED's 24576-byte block of the dense strip array is put together 1024 strips at a time
+    // in a shared-memory window (zeros, then the present strips of the window from the sorted
+    // lists) and leaves as full 16-byte stores: no zero-fill pass over HBM, no byte scatter.
+    if (dense) {
+        if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0) {
+            uint4 *const win = reinterpret_cast<uint4 *>(window);
+            uint32_t i0 = 0;  // first entry not yet placed
+#pragma unroll 1
+            for (uint32_t r = 0; r < static_cast<uint32_t>(kFedStrips) / 1024u; ++r) {
+                win[lane] = make_uint4(0, 0, 0, 0);
+                win[lane + 32] = make_uint4(0, 0, 0, 0);
+                __syncwarp();
+                const uint32_t limit = (r + 1u) * 1024u;
+                for (;;) {
+                    const uint32_t i = i0 + lane;
+                    const uint32_t sid = i < P ? strip_l[i] & 0x7fffu : 0xffffu;
+                    const bool in = sid < limit;
+                    if (in) window[sid & 1023u] = adc_l[i];
+                    const uint32_t cnt = __popc(__ballot_sync(kFull, in));
+                    i0 += cnt;
+                    if (cnt < 32u) break;
+                }
+                __syncwarp();
+                const uint4 v0 = win[lane], v1 = win[lane + 32];
+                __syncwarp();
+                st_stream(reinterpret_cast<uint4 *>(dense + r * 1024u) + lane, v0, pol_first);
+                st_stream(reinterpret_cast<uint4 *>(dense + r * 1024u) + lane + 32, v1, pol_first);
+            }
+        } else {  // unaligned output: bytes
+#pragma unroll 1
+            for (uint32_t b = lane; b < static_cast<uint32_t>(kFedStrips); b += 32u) dense[b] = 0;
+            __syncwarp();
+#pragma unroll 1
+            for (uint32_t i = lane; i < P; i += 32u) dense[strip_l[i] & 0x7fffu] = adc_l[i];
+        }
+        __syncwarp();
+    }
 
     SST_MARK(4);
     // ---------------------------------------------------------------- a3..a6: one sweep over the lists
@@ -695,6 +710,8 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             if (k < fed_cl) {
                 const uint32_t r0 = rec[k], r1 = rec[k + 1];
                 const uint32_t hd = r0 & 0xffffu, off = r0 >> 16, wd = (r1 >> 16) - off;
+                const uint32_t st0 = strip_l[hd] & 0x7fffu;
+                const uint2 cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
                 int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
 #pragma unroll 1
                 for (uint32_t j = 0; j < wd; ++j) {
@@ -702,8 +719,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     Q += q;
                     M += static_cast<int>(j) * q;
                 }
-                const uint32_t st0 = strip_l[hd] & 0x7fffu;
-                const uint2 cm = __ldg(cinfo + (st0 >> 8));
                 const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
                 // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
                 const float bary = __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
@@ -848,7 +863,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     SST_MARK(3);
     // fast path: lists behind the payload, masks and at least a few records in its place
     const uint32_t A = (c.fed_size + 15u) & ~15u;
-    if (staged && A + 3u * c.P <= p.slot_bytes && 16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
+    if (staged && A + 3u * c.P + (A >= 1024u ? 0u : 1040u) <= p.slot_bytes && 16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
         return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
     return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
@@ -857,7 +872,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
 // Every warp works alone: it draws (event, FED) tickets until the launch's work is used up and
 // never meets a block-wide barrier.  A CTA is just 1..kWarpsPerCta such warps sharing the SM's
 // shared memory (one driver reserve per CTA instead of one per warp).
-__global__ void __launch_bounds__(32 * kWarpsPerCta, 7) sst_event_kernel(const __grid_constant__ KParams p) {
+__global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_kernel(const __grid_constant__ KParams p) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int lane = threadIdx.x & 31;
     uint8_t *const mine = smem_raw + static_cast<size_t>(threadIdx.x >> 5) * (kWarpHdr + p.slot_bytes + kTailPad);
