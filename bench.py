@@ -405,7 +405,7 @@ def main():
     epl = int(info.get("events_per_launch", 1))
     # sst_unpack_cluster_batch: stream s belongs to launch group s % G, a group's events share
     # launches of up to `epl` events; every launch is sst_event_kernel followed by sst_emit_kernel
-    n_groups = min(N_STREAMS, n_events, 2)
+    n_groups = min(N_STREAMS, n_events, max(1, -(-n_events // epl)))
     launches_step = sum(-(-sum(1 for e in range(n_events) if (e % N_STREAMS) % n_groups == g) // epl)
                         for g in range(n_groups))
     launches = launches_step * args.steps

@@ -49,8 +49,11 @@
 #ifndef SST_MIN_CTAS
 #define SST_MIN_CTAS 7
 #endif
+#ifndef SST_SLAB_AHEAD
+#define SST_SLAB_AHEAD 2
+#endif
 #ifndef SST_MAXEV
-#define SST_MAXEV 32
+#define SST_MAXEV 64
 #endif
 #ifdef SST_X_NO_SCATTER
 #define SST_X_SCATTER false
@@ -70,6 +73,8 @@ constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
 constexpr uint32_t kTabBytes = kChan * 4 + kChan * 2;  // channel map of the FED, at the slot's end
 constexpr uint32_t kWarpHdr = 16;                      // mbarrier
+constexpr uint32_t kWin = 2048;                       // strips per step of the dense SoA assembly
+constexpr uint32_t kSlabAhead = SST_SLAB_AHEAD;        // FEDs between a calibration prefetch and its use
 constexpr uint32_t kTailPad = 16;                      // readable bytes behind the slot (pass 2)
 
 // FED aggregate, one 64-bit word per (event, FED), written by sst_event_kernel and read by
@@ -374,7 +379,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     uint8_t *adc_l;
     uint32_t *mS, *mA, *mH, *mP, *rec;
     uint32_t rec_cap;  // cluster records besides the end sentinel
-    uint8_t *window;   // 1 KB of shared memory for the dense SoA, free between pass 2 and the sweep
+    uint8_t *window;   // kWin bytes of shared memory for the dense SoA, free between pass 2 and the sweep
     if (kFast) {
         // [0, A): the payload, and once the lists are built the masks and the cluster records
         const uint32_t A = (c.fed_size + 15u) & ~15u;
@@ -386,7 +391,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         mP = mH + (nw + 2);
         rec = mP + (nw + 2);
         rec_cap = (A - 16u * (nw + 2)) / 4u - 1u;
-        window = A >= 1024u ? slot : slot + ((A + 3u * P + 15u) & ~15u);
+        window = A >= kWin ? slot : slot + ((A + 3u * P + 15u) & ~15u);
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
@@ -458,7 +463,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     __syncwarp();  // lists complete; the payload is dead from here on
 
     // ---------------------------------------------------------------- a2: dense SoA
-    // The FED's 24576-byte block of the dense strip array is put together 1024 strips at a time
+    // The FED's 24576-byte block of the dense strip array is put together kWin strips at a time
     // in a shared-memory window (zeros, then the present strips of the window from the sorted
     // lists) and leaves as full 16-byte stores: no zero-fill pass over HBM, no byte scatter.
     if (dense) {
@@ -466,25 +471,28 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             uint4 *const win = reinterpret_cast<uint4 *>(window);
             uint32_t i0 = 0;  // first entry not yet placed
 #pragma unroll 1
-            for (uint32_t r = 0; r < static_cast<uint32_t>(kFedStrips) / 1024u; ++r) {
-                win[lane] = make_uint4(0, 0, 0, 0);
-                win[lane + 32] = make_uint4(0, 0, 0, 0);
+            for (uint32_t r = 0; r < static_cast<uint32_t>(kFedStrips) / kWin; ++r) {
+#pragma unroll
+                for (uint32_t k = 0; k < kWin / 512u; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
                 __syncwarp();
-                const uint32_t limit = (r + 1u) * 1024u;
+                const uint32_t limit = (r + 1u) * kWin;
                 for (;;) {
                     const uint32_t i = i0 + lane;
                     const uint32_t sid = i < P ? strip_l[i] & 0x7fffu : 0xffffu;
                     const bool in = sid < limit;
-                    if (in) window[sid & 1023u] = adc_l[i];
+                    if (in) window[sid & (kWin - 1u)] = adc_l[i];
                     const uint32_t cnt = __popc(__ballot_sync(kFull, in));
                     i0 += cnt;
                     if (cnt < 32u) break;
                 }
                 __syncwarp();
-                const uint4 v0 = win[lane], v1 = win[lane + 32];
+                uint4 v[kWin / 512u];
+#pragma unroll
+                for (uint32_t k = 0; k < kWin / 512u; ++k) v[k] = win[lane + 32u * k];
                 __syncwarp();
-                st_stream(reinterpret_cast<uint4 *>(dense + r * 1024u) + lane, v0, pol_first);
-                st_stream(reinterpret_cast<uint4 *>(dense + r * 1024u) + lane + 32, v1, pol_first);
+#pragma unroll
+                for (uint32_t k = 0; k < kWin / 512u; ++k)
+                    st_stream(reinterpret_cast<uint4 *>(dense + r * kWin) + lane + 32u * k, v[k], pol_first);
             }
         } else {  // unaligned output: bytes
 #pragma unroll 1
@@ -511,17 +519,21 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         mH[w] = 0;
     }
     const uint32_t Lc = ((P + 31u) >> 5) | 1u;  // odd: the lanes' list reads fall into different banks
+    const bool want_seeds = o.seed_idx != nullptr;
+    uint32_t n_seed_lane = 0;
     const uint32_t e0 = min(lane * Lc, P), e1 = min(e0 + Lc, P);
     auto mark = [&](uint32_t hd, uint32_t end) {  // accepted cluster [hd, end]
-        atomicOr(&mH[hd >> 5], 1u << (hd & 31u));
-        uint32_t w = hd >> 5, m = kFull << (hd & 31u);
-        const uint32_t we = end >> 5;
+        const uint32_t wh = hd >> 5, we = end >> 5;
+        const uint32_t mh = kFull << (hd & 31u), me = kFull >> (31u - (end & 31u));
+        atomicOr(&mH[wh], 1u << (hd & 31u));
+        if (wh == we) {  // nearly always
+            atomicOr(&mA[wh], mh & me);
+        } else {
+            atomicOr(&mA[wh], mh);
 #pragma unroll 1
-        for (; w < we; ++w) {
-            atomicOr(&mA[w], m);
-            m = kFull;
+            for (uint32_t w = wh + 1u; w < we; ++w) atomicOr(&mA[w], kFull);
+            atomicOr(&mA[we], me);
         }
-        atomicOr(&mA[we], m & (kFull >> (31u - (end & 31u))));
     };
     auto decide = [&](uint32_t hd, uint32_t end, uint32_t Q, double N, bool seed) {
         if (seed) {
@@ -591,10 +603,13 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     }
                     open = is_act;
                     prev_s = s15;
-                    if (is_seed) accS |= 1u << (e & 31u);
-                    if ((e & 31u) == 31u || e + 1u == e1) {
-                        if (accS) atomicOr(&mS[e >> 5], accS);
-                        accS = 0;
+                    n_seed_lane += is_seed;
+                    if (want_seeds) {  // warp-uniform: the seed mask only feeds the seed-index array
+                        if (is_seed) accS |= 1u << (e & 31u);
+                        if ((e & 31u) == 31u || e + 1u == e1) {
+                            if (accS) atomicOr(&mS[e >> 5], accS);
+                            accS = 0;
+                        }
                     }
                 }
             }
@@ -656,16 +671,13 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 #pragma unroll 1
         for (uint32_t w0 = 0; w0 < nw; w0 += 32) {
             const uint32_t w = w0 + lane;
-            uint32_t v = 0, ns = 0;
-            if (w < nw) {
-                v = (__popc(mH[w]) << 16) | __popc(mA[w]);
-                ns = __popc(mS[w]);
-            }
+            uint32_t v = 0;
+            if (w < nw) v = (__popc(mH[w]) << 16) | __popc(mA[w]);
             const uint32_t incl = warp_incl_scan(v, lane);
             if (w < nw) mP[w] = run + incl - v;
             run += __shfl_sync(kFull, incl, 31);
-            fed_seed += __reduce_add_sync(kFull, ns);
         }
+        fed_seed = __reduce_add_sync(kFull, n_seed_lane);
         fed_cl = run >> 16;
         fed_adc = run & 0xffffu;
         if (kFast && fed_cl > rec_cap) return false;
@@ -767,6 +779,14 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     const uint32_t f = c.f;
     const EventDesc &E = p.ev[c.ev];
     const sst_output &o = E.out;
+    // The first event of a FED streams the calibration slab of a FED a few places ahead into L2
+    // (one bulk prefetch of 6 KB per lane): the launch's events then gather from L2, and HBM sees
+    // sequential reads instead of the first-touch misses of scattered 8-byte loads.
+    if (c.ev == 0 && p.n_events > 1 && f + kSlabAhead < p.n_feds) {
+        const uint8_t *slab = reinterpret_cast<const uint8_t *>(p.calib + static_cast<size_t>(f + kSlabAhead) * kFedStrips);
+        constexpr uint32_t kPiece = kFedStrips * sizeof(float2) / 32;
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(slab + lane * kPiece), "r"(kPiece) : "memory");
+    }
     uint32_t *const chan_off = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
     uint16_t *const chan_len = reinterpret_cast<uint16_t *>(chan_off + kChan);
 
@@ -863,7 +883,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     SST_MARK(3);
     // fast path: lists behind the payload, masks and at least a few records in its place
     const uint32_t A = (c.fed_size + 15u) & ~15u;
-    if (staged && A + 3u * c.P + (A >= 1024u ? 0u : 1040u) <= p.slot_bytes && 16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
+    if (staged && A + 3u * c.P + (A >= kWin ? 0u : kWin + 16u) <= p.slot_bytes && 16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
         return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
     return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
@@ -1085,11 +1105,11 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
             ctx->slots.push_back({st, nullptr, 0u, 0ull});
             sl = &ctx->slots.back();
         }
-        if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8 or kMaxEv events
+        if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 32 or kMaxEv events
             if (sl->mem) SST_CU(cudaFreeAsync(sl->mem, st));
             sl->mem = nullptr;
             sl->cap_events = 0;
-            const uint32_t want = n <= 1 ? 1u : n <= 8 ? 8u : static_cast<uint32_t>(kMaxEv);
+            const uint32_t want = n <= 1 ? 1u : n <= 8 ? 8u : n <= 32 ? 32u : static_cast<uint32_t>(kMaxEv);
             const ScratchLayout Ln = scratch_layout(ctx, want);
             SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), Ln.total, ctx->pool, st));
             SST_CU(cudaMemsetAsync(blk, 0, Ln.o_rec, st));  // ticket counter and states
@@ -1301,13 +1321,14 @@ sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8
     for (uint32_t e = 0; e < n_events; ++e)
         if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e])) return SST_ERR_INVALID_ARG;
     SST_CU(cudaSetDevice(ctx->cfg.device));
-    // Launch groups.  The events of several streams share one launch so that the kernel walks them
-    // FED by FED (the FED's calibration slab is then read from HBM once per launch, not once per
-    // event): stream s belongs to group s % G, the group's launches run on its first stream, which
+    // Launch groups.  The events of all streams share one launch (two or more only beyond kMaxEv
+    // events) so that the kernel walks them FED by FED (the FED's calibration slab is then read from
+    // HBM once per launch, not once per event): stream s belongs to group s % G, the group's
+    // launches run on its first stream, which
     // first waits for the other streams of the group (their uploads) and is waited for by them
     // afterwards, so every event's result is stream-ordered on its own stream as documented.
     const uint32_t ns = std::min(n_streams, n_events);
-    const uint32_t G = std::min(ns, 2u);
+    const uint32_t G = std::min(ns, std::max(1u, (n_events + kMaxEv - 1) / kMaxEv));
     auto event_of = [&](cudaStream_t st, cudaEvent_t *out) -> bool {
         std::lock_guard<std::mutex> lock(ctx->slot_mu);
         for (auto &se : ctx->stream_events)
