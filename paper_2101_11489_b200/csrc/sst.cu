@@ -52,6 +52,12 @@
 #ifndef SST_SLAB_AHEAD
 #define SST_SLAB_AHEAD 2
 #endif
+#ifndef SST_SEQ_CHANNELS
+#define SST_SEQ_CHANNELS 1
+#endif
+#ifndef SST_KU
+#define SST_KU 1
+#endif
 #ifndef SST_MAXEV
 #define SST_MAXEV 64
 #endif
@@ -68,7 +74,7 @@ constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
 constexpr int kMaxEv = SST_MAXEV;                   // events per launch
 constexpr int kWarpsPerCta = 4;             // warps (= FEDs in flight) per CTA, each with its own slot
-constexpr int kU = 4;                       // mask words per batch of the flag pass (loads in flight)
+constexpr int kU = SST_KU;                       // mask words per batch of the flag pass (loads in flight)
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
 constexpr uint32_t kTabBytes = kChan * 4 + kChan * 2;  // channel map of the FED, at the slot's end
@@ -251,6 +257,21 @@ __device__ __forceinline__ bool accept_exact(const float2 *cal, const uint16_t *
     const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
     return lhs >= __dmul_rn(tcl2, n2_sequential(cal, strip_l, head, w));
 }
+// Mask bits of an accepted cluster [hd, end]: its head in mH, its entries in mA.
+__device__ __forceinline__ void mark_cluster(uint32_t *mH, uint32_t *mA, uint32_t hd, uint32_t end) {
+    const uint32_t wh = hd >> 5, we = end >> 5;
+    const uint32_t mh = kFull << (hd & 31u), me = kFull >> (31u - (end & 31u));
+    atomicOr(&mH[wh], 1u << (hd & 31u));
+    if (wh == we) {  // nearly always
+        atomicOr(&mA[wh], mh & me);
+    } else {
+        atomicOr(&mA[wh], mh);
+#pragma unroll 1
+        for (uint32_t w = wh + 1u; w < we; ++w) atomicOr(&mA[w], kFull);
+        atomicOr(&mA[we], me);
+    }
+}
+
 // ------------------------------------------------------------------------------ raw payload
 // a1, generic path (payload not staged): the channel-length chain of one FED, checked as it goes.
 __device__ __noinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
@@ -311,6 +332,47 @@ struct FedCtx {
 // a2 pass 1: a lane validates the run lists of its three channels (reading s2b) and
 // counts their strips; the three cursors advance in one loop, so the three dependent chains of
 // byte loads overlap.  A malformed channel contributes no strips.
+#if SST_SEQ_CHANNELS
+__device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_t (&cnt)[3]) {
+    uint32_t o0 = c.off[0], o1 = c.off[1], o2 = c.off[2], l0 = c.len[0], l1 = c.len[1], l2 = c.len[2];
+    uint32_t n0 = 0, n1 = 0, n2 = 0, okbits = 0;
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) {  // one channel after the other, the register sets rotate
+        uint32_t q = o0, nf = 0, n = 0;
+        const uint32_t qe = o0 + l0;
+        bool ok = true;
+#pragma unroll 1
+        while (q < qe) {
+            bool bad = q + 2 > qe;
+            uint32_t first = 0, len = 0;
+            if (!bad) {
+                first = rp[q];
+                len = rp[q + 1];
+                if (len == 0) len = 256;  // reading s2
+                bad = first < nf || first + len > kStrip || q + 2 + len > qe;
+            }
+            if (bad) {
+                ok = false;
+                break;
+            }
+            nf = first + len;
+            q += 2 + len;
+            n += len;
+        }
+        o0 = o1; o1 = o2; l0 = l1; l1 = l2;
+        n0 = n1; n1 = n2; n2 = ok ? n : 0u;
+        okbits = (okbits >> 1) | (ok ? 4u : 0u);
+    }
+    cnt[0] = n0; cnt[1] = n1; cnt[2] = n2;
+    c.n_malformed = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const bool ok = (okbits >> k) & 1u;
+        if (!ok) c.len[k] = 0;
+        c.n_malformed += __popc(__ballot_sync(kFull, !ok));
+    }
+}
+#else
 __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_t (&cnt)[3]) {
     uint32_t q[3], qe[3], nf[3];
     bool ok[3];
@@ -359,6 +421,7 @@ __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_
         c.n_malformed += __popc(__ballot_sync(kFull, !ok[k]));
     }
 }
+#endif
 
 // ------------------------------------------------------------------------------ lists -> clusters
 // Everything after pass 1, on the FED's lists of present strips, by one warp.  kFast: lists, masks
@@ -417,6 +480,45 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 #else
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
 #endif
+#if SST_SEQ_CHANNELS
+    {
+        // one channel after the other (the three register sets rotate): a third of the code of the
+        // three-cursor form, and the instruction cache is what this kernel is short of
+        uint32_t o0 = c.off[0], o1 = c.off[1], o2 = c.off[2], l0 = c.len[0], l1 = c.len[1], l2 = c.len[2];
+        uint32_t b0_ = c.base[0], b1_ = c.base[1], b2_ = c.base[2], opens = c.opens;
+#pragma unroll 1
+        for (int k = 0; k < 3; ++k) {
+            uint32_t qq = o0, ee = b0_;
+            const uint32_t qe = o0 + l0;
+            const uint32_t g0 = static_cast<uint32_t>(lane + 32 * k) * kStrip, open_bit = (opens & 1u) << 15;
+#pragma unroll 1
+            while (qq < qe) {
+                const uint32_t first = rp[qq];
+                uint32_t len = rp[qq + 1];
+                if (len == 0) len = 256;
+                // most runs hold one or two strips; on the fast path the second byte is read
+                // unconditionally (it is inside the slot or its 16-byte tail pad)
+                const uint32_t b0 = rp[qq + 2], b1 = (kFast || len > 1) ? rp[qq + 3] : 0u;
+                const uint32_t sid = g0 + first;
+                strip_l[ee] = static_cast<uint16_t>(first == 0 ? sid | open_bit : sid);
+                adc_l[ee] = static_cast<uint8_t>(b0);
+                if (len > 1) {
+                    strip_l[ee + 1] = static_cast<uint16_t>(sid + 1u);
+                    adc_l[ee + 1] = static_cast<uint8_t>(b1);
+#pragma unroll 1
+                    for (uint32_t i = 2; i < len; ++i) {
+                        const uint32_t bi = rp[qq + 2 + i];
+                        strip_l[ee + i] = static_cast<uint16_t>(sid + i);
+                        adc_l[ee + i] = static_cast<uint8_t>(bi);
+                    }
+                }
+                ee += len;
+                qq += 2 + len;
+            }
+            o0 = o1; o1 = o2; l0 = l1; l1 = l2; b0_ = b1_; b1_ = b2_; opens >>= 1;
+        }
+    }
+#else
     {
         uint32_t q[3], qe[3], e[3];
 #pragma unroll
@@ -460,6 +562,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             }
         }
     }
+#endif
     __syncwarp();  // lists complete; the payload is dead from here on
 
     // ---------------------------------------------------------------- a2: dense SoA
@@ -522,19 +625,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     const bool want_seeds = o.seed_idx != nullptr;
     uint32_t n_seed_lane = 0;
     const uint32_t e0 = min(lane * Lc, P), e1 = min(e0 + Lc, P);
-    auto mark = [&](uint32_t hd, uint32_t end) {  // accepted cluster [hd, end]
-        const uint32_t wh = hd >> 5, we = end >> 5;
-        const uint32_t mh = kFull << (hd & 31u), me = kFull >> (31u - (end & 31u));
-        atomicOr(&mH[wh], 1u << (hd & 31u));
-        if (wh == we) {  // nearly always
-            atomicOr(&mA[wh], mh & me);
-        } else {
-            atomicOr(&mA[wh], mh);
-#pragma unroll 1
-            for (uint32_t w = wh + 1u; w < we; ++w) atomicOr(&mA[w], kFull);
-            atomicOr(&mA[we], me);
-        }
-    };
+    auto mark = [&](uint32_t hd, uint32_t end) { mark_cluster(mH, mA, hd, end); };
     auto decide = [&](uint32_t hd, uint32_t end, uint32_t Q, double N, bool seed) {
         if (seed) {
             const double dq = static_cast<double>(Q);
