@@ -55,7 +55,9 @@ def _gen_one(args):
     cfg = synth.CONFIGS[cfg_id]
     calib = _gen_one.calib
     ev = synth.make_event(cfg, calib, seed)
-    return ev.raw, ev.fed_offsets, ev.meta
+    meta = dict(ev.meta)
+    meta["max_fed_strips"] = int(np.count_nonzero(ev.z.reshape(n_feds, -1), axis=1).max())
+    return ev.raw, ev.fed_offsets, meta
 
 
 def generate_events(cfg_id: int, n_feds: int, seeds, calib, workers: int = 0):
@@ -294,8 +296,11 @@ def main():
     events = generate_events(3, n_feds, event_seeds_for_rank(rank, world, n_events), calib)
     max_raw = max(int(e[0].size) for e in events)
     max_raw = (max_raw + 4095) // 4096 * 4096
+    # sst_config.fed_strips_hint (the expected maximum of present strips in one FED) sizes the
+    # shared-memory working set: taken from the data, as a site would take it from its occupancy
+    strips_hint = int(1.05 * max(int(e[2]["max_fed_strips"]) for e in events)) + 16
     det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, device=local_rank,
-                           max_raw_bytes=max_raw, max_events_in_flight=N_STREAMS)
+                           max_raw_bytes=max_raw, max_events_in_flight=N_STREAMS, fed_strips_hint=strips_hint)
     info = det.info()
     dev = det.device
     n_strips = n_feds * B.FED_STRIPS

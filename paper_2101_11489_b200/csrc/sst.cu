@@ -47,13 +47,16 @@
 #include "sst.h"
 
 #ifndef SST_MIN_CTAS
-#define SST_MIN_CTAS 7
+#define SST_MIN_CTAS 4
 #endif
 #ifndef SST_SLAB_AHEAD
 #define SST_SLAB_AHEAD 2
 #endif
 #ifndef SST_SEQ_CHANNELS
 #define SST_SEQ_CHANNELS 1
+#endif
+#ifndef SST_WPC
+#define SST_WPC 8
 #endif
 #ifndef SST_KU
 #define SST_KU 1
@@ -73,7 +76,7 @@ constexpr int kChan = 96;
 constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
 constexpr int kMaxEv = SST_MAXEV;                   // events per launch
-constexpr int kWarpsPerCta = 4;             // warps (= FEDs in flight) per CTA, each with its own slot
+constexpr int kWarpsPerCta = SST_WPC;       // warps (= FEDs in flight) per CTA, each with its own slot
 constexpr int kU = SST_KU;                       // mask words per batch of the flag pass (loads in flight)
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
@@ -1181,7 +1184,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     const uint32_t total = n * nf;
     // warps per CTA: full CTAs once the work fills the GPU, smaller ones to spread a small launch
     const uint32_t sms = static_cast<uint32_t>(ctx->sm_count);
-    const uint32_t wpc = total >= 8u * sms ? kWarpsPerCta : total >= 4u * sms ? 2u : 1u;
+    const uint32_t wpc = total >= 16u * sms ? kWarpsPerCta : total >= 8u * sms ? std::min(4, kWarpsPerCta) : total >= 4u * sms ? 2u : 1u;
     const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (kWarpsPerCta / wpc);
     const uint32_t grid = std::min((total + wpc - 1) / wpc, capacity);
     uint8_t *blk = nullptr;
@@ -1303,7 +1306,7 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
                                                      : static_cast<uint32_t>(0.5 * m) + 32u;
         const uint32_t r_hint = (static_cast<uint32_t>(std::min(1.15 * m + 64.0, 65536.0)) + 15u) & ~15u;
         uint32_t need = std::max(r_hint + kTabBytes, r_hint + 3u * p_hint);
-        need = std::min(std::max((need + 15u) & ~15u, 2048u), 50u * 1024u);
+        need = std::min(std::max((need + 15u) & ~15u, 2048u), (227u * 1024u / kWarpsPerCta - kWarpHdr - kTailPad) & ~15u);
         auto set_slot = [&](uint32_t slot) {
             ctx->slot_bytes = slot;
             ctx->warp_stride = kWarpHdr + slot + kTailPad;
