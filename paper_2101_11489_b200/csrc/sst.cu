@@ -55,6 +55,9 @@
 #ifndef SST_SEQ_CHANNELS
 #define SST_SEQ_CHANNELS 1
 #endif
+#ifndef SST_EMIT_CTAS
+#define SST_EMIT_CTAS 8
+#endif
 #ifndef SST_WPC
 #define SST_WPC 8
 #endif
@@ -1015,7 +1018,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
 // the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then moves the staged
 // records, cluster ADCs and seeds of the FED to their final place.  Output capacity and the event
 // totals are handled here.
-__global__ void __launch_bounds__(128) sst_emit_kernel(const __grid_constant__ KParams p) {
+__global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __grid_constant__ KParams p) {
     const int lane = threadIdx.x & 31;
     const uint32_t t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (t >= p.n_events * p.n_feds) return;
@@ -1029,7 +1032,7 @@ __global__ void __launch_bounds__(128) sst_emit_kernel(const __grid_constant__ K
                    fed_malf = static_cast<uint32_t>((own >> kShMalf) & 0x7full), fed_over = static_cast<uint32_t>((own >> kShOver) & 1ull);
     // clusters | ADC bytes << 32 ; seeds | malformed << 32 (20 bits) | overrun << 52 (n_feds <= 4096)
     unsigned long long accA = 0, accB = 0;
-#pragma unroll 2
+#pragma unroll 8
     for (uint32_t j = lane; j < f; j += 32) {
         const unsigned long long v = st[j];
         accA += (v & 0x3fffull) | (((v >> kShAdc) & 0x7fffull) << 32);
@@ -1049,29 +1052,57 @@ __global__ void __launch_bounds__(128) sst_emit_kernel(const __grid_constant__ K
 
     const bool all_fit = b_cl + fed_cl <= o.cap_clusters && b_adc + fed_adc <= o.cap_adc;
     uint32_t lim = 0;  // ADC bytes of this FED that belong to clusters that fit
+    // the loop bodies first gather a few independent loads, then store: the kernel is a plain copy
+    // and lives off loads in flight
+    constexpr int kB = 4;
 #pragma unroll 1
-    for (uint32_t k = lane; k < fed_cl; k += 32) {
-        const uint4 r = p.s_rec[sb + k];
-        const uint32_t off = p.s_off[sb + k], wd = r.y >> 16;
-        const uint32_t k_cl = b_cl + k, k_adc = b_adc + off;
-        if (all_fit || (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc)) {
-            st_stream(o.cl_module + k_cl, r.x, pol_first);
-            st_stream(o.cl_first + k_cl, r.y & 0xffffu, pol_first);
-            st_stream(o.cl_width + k_cl, wd, pol_first);
-            st_stream(o.cl_charge + k_cl, static_cast<int32_t>(r.z), pol_first);
-            st_stream(o.cl_bary + k_cl, __uint_as_float(r.w), pol_first);
-            st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
-            if (o.cl_snr) o.cl_snr[k_cl] = p.s_snr[sb + k];
-            lim = off + wd;
-        } else {
-            // the first cluster that does not fit reports how many were written
-            const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
-            if (prev_fits) *o.n_clusters = k_cl;
+    for (uint32_t k0 = lane; k0 < fed_cl; k0 += 32 * kB) {
+        uint4 r[kB];
+        uint32_t off[kB];
+        float snr[kB];
+#pragma unroll
+        for (int j = 0; j < kB; ++j) {
+            const uint32_t k = k0 + 32 * j;
+            if (k < fed_cl) {
+                r[j] = p.s_rec[sb + k];
+                off[j] = p.s_off[sb + k];
+                if (o.cl_snr) snr[j] = p.s_snr[sb + k];
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < kB; ++j) {
+            const uint32_t k = k0 + 32 * j;
+            if (k < fed_cl) {
+                const uint32_t wd = r[j].y >> 16;
+                const uint32_t k_cl = b_cl + k, k_adc = b_adc + off[j];
+                if (all_fit || (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc)) {
+                    st_stream(o.cl_module + k_cl, r[j].x, pol_first);
+                    st_stream(o.cl_first + k_cl, r[j].y & 0xffffu, pol_first);
+                    st_stream(o.cl_width + k_cl, wd, pol_first);
+                    st_stream(o.cl_charge + k_cl, static_cast<int32_t>(r[j].z), pol_first);
+                    st_stream(o.cl_bary + k_cl, __uint_as_float(r[j].w), pol_first);
+                    st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
+                    if (o.cl_snr) o.cl_snr[k_cl] = snr[j];
+                    lim = max(lim, off[j] + wd);
+                } else {
+                    // the first cluster that does not fit reports how many were written
+                    const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
+                    if (prev_fits) *o.n_clusters = k_cl;
+                }
+            }
         }
     }
     lim = all_fit ? fed_adc : __reduce_max_sync(kFull, lim);
-#pragma unroll 2
-    for (uint32_t i = lane; i < lim; i += 32) st_stream(o.cl_adc + b_adc + i, static_cast<uint32_t>(p.s_adc[ab + i]), pol_first);
+#pragma unroll 1
+    for (uint32_t i0 = lane; i0 < lim; i0 += 32 * 8) {
+        uint32_t v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (i0 + 32 * j < lim) v[j] = p.s_adc[ab + i0 + 32 * j];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (i0 + 32 * j < lim) st_stream(o.cl_adc + b_adc + i0 + 32 * j, v[j], pol_first);
+    }
     if (o.seed_idx) {
 #pragma unroll 1
         for (uint32_t i = lane; i < fed_seed; i += 32)
