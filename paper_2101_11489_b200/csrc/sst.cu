@@ -306,16 +306,13 @@ __device__ __noinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_
 
 // a1, staged payload: the same chain walked speculatively by one lane -- no bounds checks inside
 // the serial loop (reads are clamped into the slot), the 96 results are validated in parallel.
-__device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uint32_t clamp, uint32_t *chan_off,
-                                                       uint16_t *chan_len) {
+__device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uint32_t clamp, uint32_t *chan_off) {
     uint32_t pos = 0;
 #pragma unroll 8
     for (int c = 0; c < kChan; ++c) {
         const uint32_t a = min(pos, clamp);
-        const uint32_t l16 = stage[a] | (static_cast<uint32_t>(stage[a + 1]) << 8);
-        chan_off[c] = pos + 2;
-        chan_len[c] = static_cast<uint16_t>(l16);
-        pos += 2 + l16;
+        pos += 2u + (stage[a] | (static_cast<uint32_t>(stage[a + 1]) << 8));
+        chan_off[c + 1] = pos + 2u;  // chan_off[0] = 2; the lengths are differences
     }
 }
 
@@ -511,11 +508,13 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 if (len > 1) {
                     strip_l[ee + 1] = static_cast<uint16_t>(sid + 1u);
                     adc_l[ee + 1] = static_cast<uint8_t>(b1);
+                    if (len > 2) {
 #pragma unroll 1
-                    for (uint32_t i = 2; i < len; ++i) {
-                        const uint32_t bi = rp[qq + 2 + i];
-                        strip_l[ee + i] = static_cast<uint16_t>(sid + i);
-                        adc_l[ee + i] = static_cast<uint8_t>(bi);
+                        for (uint32_t i = 2; i < len; ++i) {
+                            const uint32_t bi = rp[qq + 2 + i];
+                            strip_l[ee + i] = static_cast<uint16_t>(sid + i);
+                            adc_l[ee + i] = static_cast<uint8_t>(bi);
+                        }
                     }
                 }
                 ee += len;
@@ -585,14 +584,16 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 for (uint32_t k = 0; k < kWin / 512u; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
                 __syncwarp();
                 const uint32_t limit = (r + 1u) * kWin;
-                for (;;) {
-                    const uint32_t i = i0 + lane;
-                    const uint32_t sid = i < P ? strip_l[i] & 0x7fffu : 0xffffu;
-                    const bool in = sid < limit;
-                    if (in) window[sid & (kWin - 1u)] = adc_l[i];
-                    const uint32_t cnt = __popc(__ballot_sync(kFull, in));
+                for (;;) {  // two consecutive entries per lane; the list is sorted by strip
+                    const uint32_t i = i0 + 2u * lane;
+                    const uint32_t sa = i < P ? strip_l[i] & 0x7fffu : 0xffffu;
+                    const uint32_t sb = i + 1u < P ? strip_l[i + 1u] & 0x7fffu : 0xffffu;
+                    const bool ina = sa < limit, inb = sb < limit;
+                    if (ina) window[sa & (kWin - 1u)] = adc_l[i];
+                    if (inb) window[sb & (kWin - 1u)] = adc_l[i + 1u];
+                    const uint32_t cnt = __popc(__ballot_sync(kFull, ina)) + __popc(__ballot_sync(kFull, inb));
                     i0 += cnt;
-                    if (cnt < 32u) break;
+                    if (cnt < 64u) break;
                 }
                 __syncwarp();
                 uint4 v[kWin / 512u];
@@ -813,6 +814,8 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         // cluster records: lane per cluster, consecutive lanes write consecutive records
         const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 3u + f;
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
+        const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
+        uint8_t *const sa = p.s_adc + ab;  // the FED's cluster ADCs, in order
 #pragma unroll 1
         for (uint32_t k0 = 0; k0 < fed_cl; k0 += 32) {
             const uint32_t k = k0 + lane;
@@ -827,6 +830,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     const int q = adc_l[hd + j];
                     Q += q;
                     M += static_cast<int>(j) * q;
+                    sa[off + j] = static_cast<uint8_t>(q);  // neighbouring lanes write neighbouring bytes
                 }
                 const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
                 // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
@@ -836,15 +840,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 p.s_off[sb + k] = off;
                 if (o.cl_snr)
                     p.s_snr[sb + k] = static_cast<float>(static_cast<double>(Q) / sqrt(n2_sequential(cal, strip_l, hd, wd)));
-            }
-        }
-        // cluster ADCs: lane per entry, the entries of accepted clusters compacted in order
-        const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
-        if (fed_adc) {
-#pragma unroll 2
-            for (uint32_t w = 0; w < nw; ++w) {
-                const uint32_t m = mA[w];
-                if ((m >> lane) & 1u) p.s_adc[ab + (mP[w] & 0xffffu) + __popc(m & lt)] = adc_l[w * 32u + lane];
             }
         }
         // a4: seed-index array (on request), FED-local strip ids
@@ -922,14 +917,17 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     SST_MARK(1);
     // ---------------------------------------------------------------- a1: walk the length chain
     if (staged) {
-        if (lane == 0) walk_chain_speculative(slot, p.slot_bytes - kTabBytes - 2u, chan_off, chan_len);
+        if (lane == 0) {
+            chan_off[0] = 2u;
+            walk_chain_speculative(slot, p.slot_bytes - kTabBytes - 2u, chan_off);
+        }
         __syncwarp();
         // validate the speculative chain: channels from the first bad one on are empty
         uint32_t bad = 0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             c.off[k] = chan_off[lane + 32 * k];
-            c.len[k] = chan_len[lane + 32 * k];
+            c.len[k] = (chan_off[lane + 32 * k + 1] - c.off[k] - 2u) & 0xffffu;
             const bool ok = c.overrun == 0 && c.off[k] <= c.fed_size && c.off[k] + c.len[k] <= c.fed_size;
             const uint32_t m = ~__ballot_sync(kFull, ok);
             if (!bad && m) bad = 32u * k + __ffs(m);  // 1 + index of the first bad channel
