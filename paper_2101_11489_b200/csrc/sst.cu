@@ -67,12 +67,6 @@
 #ifndef SST_MAXEV
 #define SST_MAXEV 64
 #endif
-#ifdef SST_X_NO_SCATTER
-#define SST_X_SCATTER false
-#else
-#define SST_X_SCATTER true
-#endif
-
 namespace {
 
 constexpr int kChan = 96;
@@ -163,9 +157,10 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         "l"(src), "r"(bytes), "r"(smem_addr(bar)), "l"(pol)
         : "memory");
 }
-// L2 residency.  The calibration (8 B per strip, 86.5 MB for 440 FEDs) is read by every event and
-// fits the L2 set-aside that sst_create reserves, while raw data and outputs stream through once:
-// calibration loads carry an evict_last policy, everything else that touches HBM evict_first.
+// L2 residency.  The calibration (8 B per strip, 86.5 MB for 440 FEDs) is read by every event;
+// the FED-major ticket order keeps the slabs in use hot, and raw data and outputs stream through
+// once: calibration loads carry an evict_last policy, everything else that touches HBM
+// evict_first.  (The persisting-L2 set-aside was measured slower and is not used.)
 __device__ __forceinline__ unsigned long long policy_evict_last() {
     unsigned long long pol;
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
@@ -173,11 +168,7 @@ __device__ __forceinline__ unsigned long long policy_evict_last() {
 }
 __device__ __forceinline__ unsigned long long policy_evict_first() {
     unsigned long long pol;
-#ifdef SST_X_NORMAL_STORES
-    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
-#else
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-#endif
     return pol;
 }
 // Calibration gather.  On B200 a plain load that misses L2 pulls the whole 128-byte line from
@@ -185,9 +176,6 @@ __device__ __forceinline__ unsigned long long policy_evict_first() {
 // through L1.
 __device__ __forceinline__ float2 ld_calib(const float2 *p, unsigned long long pol) {
     float2 v;
-#ifdef SST_X_NO_GATHER
-    return make_float2(4.0f, 1.0f);
-#endif
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.L2::64B.v2.f32 {%0,%1}, [%2], %3;"
                  : "=f"(v.x), "=f"(v.y)
                  : "l"(p), "l"(pol));
@@ -478,11 +466,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // ---------------------------------------------------------------- a2 pass 2: lane per channel
     // writes {strip, adc} in ascending strip order; bit 15 of a strip id marks strip 0 of a channel
     // that opens a module (nothing links across it).  Three cursors per lane as in pass 1.
-#ifdef SST_X_SMALL_CAL
-    const float2 *cal = p.calib + static_cast<size_t>(f & 7u) * kFedStrips;  // 1.5 MB of calibration: always an L2 hit
-#else
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
-#endif
 #if SST_SEQ_CHANNELS
     {
         // one channel after the other (the three register sets rotate): a third of the code of the
@@ -1366,18 +1350,6 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
                 }
             }
         }
-        cudaGetLastError();
-    }
-    {
-        // L2 set-aside for the calibration (read by every event with an evict_last policy): the
-        // device maximum (79 of 126 MB on B200).  A device-wide limit; failure is not fatal.
-        int max_persist = 0;
-#ifndef SST_X_PERSIST
-        max_persist = -1;
-#endif
-        if (max_persist >= 0 && cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, cfg->device) == cudaSuccess &&
-            max_persist > 0)
-            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, static_cast<size_t>(max_persist));
         cudaGetLastError();
     }
     *out_ctx = ctx;
