@@ -58,6 +58,12 @@
 #ifndef SST_EMIT_CTAS
 #define SST_EMIT_CTAS 8
 #endif
+#ifndef SST_T_CALIB_LD
+#define SST_T_CALIB_LD 1
+#endif
+#ifndef SST_T_PF_HINT
+#define SST_T_PF_HINT 1
+#endif
 #ifndef SST_WPC
 #define SST_WPC 8
 #endif
@@ -176,9 +182,17 @@ __device__ __forceinline__ unsigned long long policy_evict_first() {
 // through L1.
 __device__ __forceinline__ float2 ld_calib(const float2 *p, unsigned long long pol) {
     float2 v;
+#if SST_T_CALIB_LD == 1
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;"
+                 : "=f"(v.x), "=f"(v.y)
+                 : "l"(p), "l"(pol));
+#elif SST_T_CALIB_LD == 2
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+#else
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.L2::64B.v2.f32 {%0,%1}, [%2], %3;"
                  : "=f"(v.x), "=f"(v.y)
                  : "l"(p), "l"(pol));
+#endif
     return v;
 }
 // streaming stores of the outputs
@@ -861,7 +875,11 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     if (c.ev == 0 && p.n_events > 1 && f + kSlabAhead < p.n_feds) {
         const uint8_t *slab = reinterpret_cast<const uint8_t *>(p.calib + static_cast<size_t>(f + kSlabAhead) * kFedStrips);
         constexpr uint32_t kPiece = kFedStrips * sizeof(float2) / 32;
+#if SST_T_PF_HINT
+        asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(slab + lane * kPiece), "r"(kPiece), "l"(policy_evict_last()) : "memory");
+#else
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(slab + lane * kPiece), "r"(kPiece) : "memory");
+#endif
     }
     uint32_t *const chan_off = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
     uint16_t *const chan_len = reinterpret_cast<uint16_t *>(chan_off + kChan);
