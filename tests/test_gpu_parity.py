@@ -410,3 +410,35 @@ def test_batched_entry_point_matches_single_event(H, oracle):
                 compare(H.unsigned_view(o.numpy()), r)
     finally:
         det.close()
+
+
+def test_full_size_batch_in_the_bench_configuration(H, oracle):
+    """BASELINE.json config 3 at full size in the launch configuration bench.py times: 440 FEDs,
+    events over 8 streams through sst_unpack_cluster_batch (one FED-major launch), the
+    shared-memory slot sized by fed_strips_hint as bench.py does; every event compared in full."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    n_ev = 10
+    cfg, cal, evs = synth.make_config(3, event_seeds=range(1, n_ev + 1))
+    nf = cal.n_feds
+    mrb = (max(int(e.raw.size) for e in evs) + 4095) // 4096 * 4096
+    hint = int(1.05 * max(int(np.count_nonzero(e.z.reshape(nf, -1), axis=1).max()) for e in evs)) + 16
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb, fed_strips_hint=hint)
+    try:
+        info = det.info()
+        assert info["ctas_per_sm"] * info["threads"] // 32 >= 24      # the fast path's occupancy
+        d_in = [det.upload_raw(e.raw, e.fed_offsets) for e in evs]
+        streams = [torch.cuda.Stream() for _ in range(8)]
+        outs = [det.alloc_outputs(mrb // 3 + 1, mrb, chan_map=True, seeds=True, snr=True) for _ in evs]
+        batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs],
+                        [s.cuda_stream for s in streams])
+        torch.cuda.synchronize()
+        B.sst_unpack_cluster_batch(det.ctx, batch)
+        torch.cuda.synchronize()
+        for e, o in zip(evs, outs):
+            r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            g = H.unsigned_view(o.numpy())
+            compare(g, r)
+            assert np.array_equal(g["strip_adc"], e.z)
+    finally:
+        det.close()
