@@ -151,6 +151,19 @@ sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t ra
                                    const uint32_t *fed_offsets, const sst_thresholds *thr,
                                    const sst_output *out, void *stream);
 
+/* n_events events with HOST buffers in one call (transfers of some events overlap the
+ * kernels of others): the events are cut into small chunks, chunk c is uploaded, processed in one
+ * launch and read back on streams[c % n_streams] (use >= 3 streams for full overlap).  raw[e]
+ * (raw_bytes[e] bytes), fed_offsets[e] and every array of outs[e] are HOST pointers.  When an
+ * event's status and cluster arrays are pinned (mapped) host memory the kernels write them
+ * directly over PCIe; otherwise they are staged in pooled device memory and copied back exactly
+ * sized.  Results are as for sst_unpack_cluster_host.  Returns after all the streams it used have
+ * completed. */
+sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
+                                         const uint32_t *raw_bytes, const uint32_t *const *fed_offsets,
+                                         const sst_thresholds *thr, const sst_output *outs, void *const *streams,
+                                         uint32_t n_streams);
+
 /* Stream-ordered allocation of per-event buffers from the context's pool (cudaMallocAsync;
  * replaces the caching allocator of PAPER.md:41).  The pointer is usable by work enqueued on
  * `stream` after the call; free it with sst_event_free on a stream that has seen all its uses. */

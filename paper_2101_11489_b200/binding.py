@@ -20,6 +20,7 @@ FLAG_CLUSTER_CAP, FLAG_ADC_CAP, FLAG_MALFORMED, FLAG_OVERRUN = 1, 2, 4, 8
 SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB = range(5)
 
 EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
+           "sst_unpack_cluster_host_batch",
            "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_destroy", "sst_last_cuda_error",
            "sst_status_string", "sst_get_info"]
 
@@ -71,6 +72,7 @@ def load():
     L.sst_unpack_cluster_batch.argtypes = [vp, C.c_uint32, vp, vp, C.POINTER(sst_thresholds), vp, vp, C.c_uint32]
     L.sst_unpack_cluster_host.argtypes = [vp, vp, C.c_uint32, vp, C.POINTER(sst_thresholds),
                                           C.POINTER(sst_output), vp]
+    L.sst_unpack_cluster_host_batch.argtypes = [vp, C.c_uint32, vp, vp, vp, C.POINTER(sst_thresholds), vp, vp, C.c_uint32]
     L.sst_event_alloc.argtypes = [vp, C.c_uint64, vp, C.POINTER(vp)]
     L.sst_event_free.argtypes = [vp, vp, vp]
     L.sst_event_upload.argtypes = [vp, vp, C.c_uint32, vp, vp, C.POINTER(vp), C.POINTER(vp)]
@@ -170,6 +172,29 @@ def sst_unpack_cluster_host(ctx, raw, raw_bytes: int, fed_offsets, thresholds, o
     rc = load().sst_unpack_cluster_host(ctx, _ptr(raw), raw_bytes, _ptr(fed_offsets), C.byref(thr),
                                         C.byref(out), C.c_void_p(stream))
     _check(ctx, rc, "sst_unpack_cluster_host")
+
+
+class HostBatch:
+    """Marshalled arguments of sst_unpack_cluster_host_batch (HOST buffers), built once."""
+
+    def __init__(self, raws, raw_bytes, fed_offsets, thresholds, outs, streams):
+        n = len(raws)
+        self.n = n
+        self.keep = (list(raws), list(fed_offsets), list(outs))
+        self.raw = (C.c_void_p * n)(*[_ptr(r) for r in raws])
+        self.raw_bytes = (C.c_uint32 * n)(*[int(x) for x in raw_bytes])
+        self.fo = (C.c_void_p * n)(*[_ptr(f) for f in fed_offsets])
+        self.outs = (sst_output * n)(*outs)
+        self.streams = (C.c_void_p * len(streams))(*streams)
+        self.n_streams = len(streams)
+        self.thr = thresholds if isinstance(thresholds, sst_thresholds) else sst_thresholds(*map(float, thresholds))
+
+
+def sst_unpack_cluster_host_batch(ctx, batch: HostBatch):
+    """batch.n events with HOST buffers, chunked over batch.streams; returns when all are done."""
+    rc = load().sst_unpack_cluster_host_batch(ctx, batch.n, batch.raw, batch.raw_bytes, batch.fo, C.byref(batch.thr),
+                                              batch.outs, batch.streams, batch.n_streams)
+    _check(ctx, rc, "sst_unpack_cluster_host_batch")
 
 
 def sst_event_alloc(ctx, nbytes: int, stream: int = 0) -> int:

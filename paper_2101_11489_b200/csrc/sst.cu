@@ -67,9 +67,6 @@
 #ifndef SST_WPC
 #define SST_WPC 8
 #endif
-#ifndef SST_KU
-#define SST_KU 1
-#endif
 #ifndef SST_MAXEV
 #define SST_MAXEV 64
 #endif
@@ -80,7 +77,6 @@ constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
 constexpr int kMaxEv = SST_MAXEV;                   // events per launch
 constexpr int kWarpsPerCta = SST_WPC;       // warps (= FEDs in flight) per CTA, each with its own slot
-constexpr int kU = SST_KU;                       // mask words per batch of the flag pass (loads in flight)
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
 constexpr uint32_t kTabBytes = kChan * 4 + kChan * 2;  // channel map of the FED, at the slot's end
@@ -654,59 +650,56 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         uint32_t lQ = 0, lEnd = 0;  // lead partial: the part of an earlier candidate inside this chunk
         double lN = 0.0;
         bool lSeed = false, lClosed = false;
-#pragma unroll 1
-        for (uint32_t eb = e0; eb < e1; eb += kU) {
-            uint32_t sv[kU], av[kU];
-            float2 cv[kU];
-#pragma unroll
-            for (int j = 0; j < kU; ++j) {
-                const uint32_t e = eb + j;
-                const bool valid = e < e1;
-                sv[j] = valid ? strip_l[e] : 0xffffu;
-                av[j] = valid ? adc_l[e] : 0u;
+        // software pipeline of depth one: the next entry's list reads and calibration gather are
+        // issued before the current entry is worked on
+        uint32_t sv_n = 0xffffu, av_n = 0;
+        float2 cv_n = make_float2(INFINITY, 1.0f);
+        auto fetch = [&](uint32_t e) {
+            if (e < e1) {
+                sv_n = strip_l[e];
+                av_n = adc_l[e];
+                cv_n = av_n ? ld_calib(cal + (sv_n & 0x7fffu), pol_last) : make_float2(INFINITY, 1.0f);
             }
-#pragma unroll
-            for (int j = 0; j < kU; ++j)
-                cv[j] = av[j] ? ld_calib(cal + (sv[j] & 0x7fffu), pol_last) : make_float2(INFINITY, 1.0f);
-#pragma unroll
-            for (int j = 0; j < kU; ++j) {
-                const uint32_t e = eb + j;
-                if (e < e1) {
-                    const uint32_t s15 = sv[j] & 0x7fffu;
-                    const float af = static_cast<float>(av[j]);
-                    const bool is_act = av[j] != 0 && ge_exact(af, p.t_ch, cv[j].x);
-                    const bool is_seed = is_act && ge_exact(af, p.t_seed, cv[j].x);
-                    // this entry continues the candidate of the previous one
-                    const bool is_link = is_act && open && !(sv[j] & 0x8000u) && s15 == prev_s + 1u;
-                    if (open && !is_link) {  // the open candidate ended with entry e - 1
-                        if (lead) {
-                            lQ = Q; lN = N; lSeed = seed; lEnd = e - 1u; lClosed = true;
-                            lead = false;
-                        } else {
-                            decide(hd, e - 1u, Q, N, seed);
-                        }
-                    }
-                    if (is_act) {
-                        if (!is_link) {
-                            hd = e; Q = 0; N = 0.0; seed = false;
-                        }
-                        const uint32_t q = gain_correct(af, cv[j].y);
-                        adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
-                        Q += q;
-                        const double d = static_cast<double>(cv[j].x);
-                        N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
-                        seed = seed || is_seed;
-                    }
-                    open = is_act;
-                    prev_s = s15;
-                    n_seed_lane += is_seed;
-                    if (want_seeds) {  // warp-uniform: the seed mask only feeds the seed-index array
-                        if (is_seed) accS |= 1u << (e & 31u);
-                        if ((e & 31u) == 31u || e + 1u == e1) {
-                            if (accS) atomicOr(&mS[e >> 5], accS);
-                            accS = 0;
-                        }
-                    }
+        };
+        fetch(e0);
+#pragma unroll 1
+        for (uint32_t e = e0; e < e1; ++e) {
+            const uint32_t sv = sv_n, av = av_n;
+            const float2 cv = cv_n;
+            fetch(e + 1u);
+            const uint32_t s15 = sv & 0x7fffu;
+            const float af = static_cast<float>(av);
+            const bool is_act = av != 0 && ge_exact(af, p.t_ch, cv.x);
+            const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
+            // this entry continues the candidate of the previous one
+            const bool is_link = is_act && open && !(sv & 0x8000u) && s15 == prev_s + 1u;
+            if (open && !is_link) {  // the open candidate ended with entry e - 1
+                if (lead) {
+                    lQ = Q; lN = N; lSeed = seed; lEnd = e - 1u; lClosed = true;
+                    lead = false;
+                } else {
+                    decide(hd, e - 1u, Q, N, seed);
+                }
+            }
+            if (is_act) {
+                if (!is_link) {
+                    hd = e; Q = 0; N = 0.0; seed = false;
+                }
+                const uint32_t q = gain_correct(af, cv.y);
+                adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
+                Q += q;
+                const double d = static_cast<double>(cv.x);
+                N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
+                seed = seed || is_seed;
+            }
+            open = is_act;
+            prev_s = s15;
+            n_seed_lane += is_seed;
+            if (want_seeds) {  // warp-uniform: the seed mask only feeds the seed-index array
+                if (is_seed) accS |= 1u << (e & 31u);
+                if ((e & 31u) == 31u || e + 1u == e1) {
+                    if (accS) atomicOr(&mS[e >> 5], accS);
+                    accS = 0;
                 }
             }
         }
@@ -1230,11 +1223,11 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
             ctx->slots.push_back({st, nullptr, 0u, 0ull});
             sl = &ctx->slots.back();
         }
-        if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 32 or kMaxEv events
+        if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 16, 32 or kMaxEv events
             if (sl->mem) SST_CU(cudaFreeAsync(sl->mem, st));
             sl->mem = nullptr;
             sl->cap_events = 0;
-            const uint32_t want = n <= 1 ? 1u : n <= 8 ? 8u : n <= 32 ? 32u : static_cast<uint32_t>(kMaxEv);
+            const uint32_t want = n <= 1 ? 1u : n <= 8 ? 8u : n <= 16 ? 16u : n <= 32 ? 32u : static_cast<uint32_t>(kMaxEv);
             const ScratchLayout Ln = scratch_layout(ctx, want);
             SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), Ln.total, ctx->pool, st));
             SST_CU(cudaMemsetAsync(blk, 0, Ln.o_rec, st));  // ticket counter and states
@@ -1573,6 +1566,178 @@ sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t ra
     }
     CU(cudaFreeAsync(blk, st));
     CU(cudaStreamSynchronize(st));
+    return rc;
+}
+
+namespace {
+// A list of copies of one chunk, issued together.
+struct CopyList {
+    std::vector<void *> dst, src;
+    std::vector<size_t> bytes;
+    void add(void *d, const void *s, size_t n) {
+        if (!n) return;
+        dst.push_back(d);
+        src.push_back(const_cast<void *>(s));
+        bytes.push_back(n);
+    }
+    cudaError_t run(cudaStream_t st) {
+        if (dst.empty()) return cudaSuccess;
+        cudaError_t e = cudaSuccess;
+        for (size_t i = 0; i < dst.size() && e == cudaSuccess; ++i)
+            e = cudaMemcpyAsync(dst[i], src[i], bytes[i], cudaMemcpyDefault, st);
+        dst.clear();
+        src.clear();
+        bytes.clear();
+        return e;
+    }
+};
+}  // namespace
+
+sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
+                                         const uint32_t *raw_bytes, const uint32_t *const *fed_offsets,
+                                         const sst_thresholds *thr, const sst_output *outs, void *const *streams,
+                                         uint32_t n_streams) {
+    if (!ctx || !raw || !raw_bytes || !fed_offsets || !thr || !outs || !streams || n_streams == 0 || !thresholds_ok(thr))
+        return SST_ERR_INVALID_ARG;
+    if (!ctx->has_calib) return SST_ERR_NO_CALIB;
+    for (uint32_t e = 0; e < n_events; ++e)
+        if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e]) || raw_bytes[e] > ctx->cfg.max_raw_bytes)
+            return SST_ERR_INVALID_ARG;
+    if (n_events == 0) return SST_OK;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    const uint32_t nf = ctx->cfg.n_feds;
+    const size_t n = static_cast<size_t>(nf) * kFedStrips, nch = static_cast<size_t>(nf) * kChan;
+    auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
+    // Chunks of up to kHostChunk events: chunk c runs on streams[c % n_streams] -- upload, one
+    // FED-major launch, counts back -- so the uploads, kernels and downloads of neighbouring chunks
+    // overlap.  The cluster arrays are then fetched chunk by chunk with exactly-sized
+    // copies while later chunks are still being processed.
+#ifndef SST_HOST_CHUNK
+#define SST_HOST_CHUNK 4
+#endif
+    constexpr uint32_t kHostChunk = SST_HOST_CHUNK;
+    auto mapped = [](const void *h, void *&d) {
+        cudaPointerAttributes a{};
+        if (!h || cudaPointerGetAttributes(&a, h) != cudaSuccess) {
+            cudaGetLastError();
+            return false;
+        }
+        d = a.devicePointer;
+        return a.type == cudaMemoryTypeHost && a.devicePointer != nullptr;
+    };
+    struct EvDev { sst_output d; uint8_t *raw; uint32_t *fo; bool direct; };
+    struct Chunk { uint32_t e0, n; cudaStream_t st; uint8_t *blk; };
+    std::vector<EvDev> dev(n_events);
+    std::vector<Chunk> chunks;
+    CopyList copies;
+    sst_status rc = SST_OK;
+    auto CU = [&](cudaError_t e) { if (rc == SST_OK && !cu_ok(ctx, e)) rc = SST_ERR_CUDA; };
+    for (uint32_t e0 = 0; e0 < n_events && rc == SST_OK; e0 += kHostChunk) {
+        Chunk ck{e0, std::min(kHostChunk, n_events - e0), static_cast<cudaStream_t>(streams[chunks.size() % n_streams]), nullptr};
+        // one pooled block per chunk, carved up
+        std::vector<size_t> off(ck.n + 1, 0);
+        for (uint32_t i = 0; i < ck.n; ++i) {
+            const sst_output &o = outs[e0 + i];
+            size_t b = up(ctx->cfg.max_raw_bytes) + up((nf + 1) * 4) + up(SST_ST_WORDS * 4) + 256 +
+                       up(4ull * o.cap_clusters) * 4 + up(2ull * o.cap_clusters) * 2 + up(o.cap_adc) +
+                       (o.cl_snr ? up(4ull * o.cap_clusters) : 0) + (o.strip_adc ? up(n) : 0) +
+                       (o.chan_off ? up(4 * nch) : 0) + (o.chan_len ? up(2 * nch) : 0) +
+                       (o.seed_idx ? up(4ull * o.cap_seeds) : 0);
+            off[i + 1] = off[i] + b;
+        }
+        CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&ck.blk), off[ck.n], ctx->pool, ck.st));
+        if (rc != SST_OK) break;
+        const uint8_t *r[kHostChunk];
+        const uint32_t *fo[kHostChunk];
+        const sst_output *po[kHostChunk];
+        for (uint32_t i = 0; i < ck.n; ++i) {
+            const sst_output &o = outs[e0 + i];
+            EvDev &v = dev[e0 + i];
+            uint8_t *q = ck.blk + off[i];
+            auto take = [&](size_t bytes) { uint8_t *r0 = q; q += up(bytes); return r0; };
+            v.raw = take(ctx->cfg.max_raw_bytes);
+            v.fo = reinterpret_cast<uint32_t *>(take((nf + 1) * 4));
+            v.d = o;
+            // Pinned (mapped) host arrays are written by the emit kernel directly over PCIe: no
+            // device copy of the cluster arrays, no count round trip, no per-array download.
+            void *m[10] = {};
+            v.direct = mapped(o.dev_status, m[0]) && mapped(o.n_clusters, m[1]) && mapped(o.cl_module, m[2]) &&
+                       mapped(o.cl_charge, m[3]) && mapped(o.cl_bary, m[4]) && mapped(o.cl_adc_off, m[5]) &&
+                       mapped(o.cl_first, m[6]) && mapped(o.cl_width, m[7]) && mapped(o.cl_adc, m[8]) &&
+                       (!o.cl_snr || mapped(o.cl_snr, m[9]));
+            if (v.direct) {
+                v.d.dev_status = static_cast<uint32_t *>(m[0]);
+                v.d.n_clusters = static_cast<uint32_t *>(m[1]);
+                v.d.cl_module = static_cast<uint32_t *>(m[2]);
+                v.d.cl_charge = static_cast<int32_t *>(m[3]);
+                v.d.cl_bary = static_cast<float *>(m[4]);
+                v.d.cl_adc_off = static_cast<uint32_t *>(m[5]);
+                v.d.cl_first = static_cast<uint16_t *>(m[6]);
+                v.d.cl_width = static_cast<uint16_t *>(m[7]);
+                v.d.cl_adc = static_cast<uint8_t *>(m[8]);
+                v.d.cl_snr = o.cl_snr ? static_cast<float *>(m[9]) : nullptr;
+            } else {
+                v.d.dev_status = reinterpret_cast<uint32_t *>(take(SST_ST_WORDS * 4));
+                v.d.n_clusters = reinterpret_cast<uint32_t *>(take(256));
+                v.d.cl_module = reinterpret_cast<uint32_t *>(take(4ull * o.cap_clusters));
+                v.d.cl_charge = reinterpret_cast<int32_t *>(take(4ull * o.cap_clusters));
+                v.d.cl_bary = reinterpret_cast<float *>(take(4ull * o.cap_clusters));
+                v.d.cl_adc_off = reinterpret_cast<uint32_t *>(take(4ull * o.cap_clusters));
+                v.d.cl_first = reinterpret_cast<uint16_t *>(take(2ull * o.cap_clusters));
+                v.d.cl_width = reinterpret_cast<uint16_t *>(take(2ull * o.cap_clusters));
+                v.d.cl_adc = take(o.cap_adc);
+                v.d.cl_snr = o.cl_snr ? reinterpret_cast<float *>(take(4ull * o.cap_clusters)) : nullptr;
+            }
+            v.d.strip_adc = o.strip_adc ? take(n) : nullptr;
+            v.d.chan_off = o.chan_off ? reinterpret_cast<uint32_t *>(take(4 * nch)) : nullptr;
+            v.d.chan_len = o.chan_len ? reinterpret_cast<uint16_t *>(take(2 * nch)) : nullptr;
+            v.d.seed_idx = o.seed_idx ? reinterpret_cast<uint32_t *>(take(4ull * o.cap_seeds)) : nullptr;
+            copies.add(v.raw, raw[e0 + i], raw_bytes[e0 + i]);
+            copies.add(v.fo, fed_offsets[e0 + i], (nf + 1) * 4);
+            r[i] = v.raw;
+            fo[i] = v.fo;
+            po[i] = &v.d;
+        }
+        CU(copies.run(ck.st));
+        if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st);
+        for (uint32_t i = 0; i < ck.n; ++i) {
+            const sst_output &o = outs[e0 + i];
+            if (dev[e0 + i].direct) continue;
+            copies.add(o.dev_status, dev[e0 + i].d.dev_status, SST_ST_WORDS * 4);
+            copies.add(o.n_clusters, dev[e0 + i].d.n_clusters, 4);
+        }
+        CU(copies.run(ck.st));
+        chunks.push_back(ck);
+    }
+    // counts are on the host once a chunk's stream has drained: exactly-sized copies of the rest
+    for (const Chunk &ck : chunks) {
+        CU(cudaStreamSynchronize(ck.st));
+        if (rc != SST_OK) break;
+        for (uint32_t i = 0; i < ck.n; ++i) {
+            const sst_output &o = outs[ck.e0 + i];
+            const sst_output &d = dev[ck.e0 + i].d;
+            const size_t k = *o.n_clusters;
+            const size_t na = o.dev_status[SST_ST_FLAGS] & (SST_FLAG_CLUSTER_CAP | SST_FLAG_ADC_CAP) ? o.cap_adc
+                                                                                                     : o.dev_status[SST_ST_N_ADC];
+            if (k && !dev[ck.e0 + i].direct) {
+                copies.add(o.cl_module, d.cl_module, 4 * k);
+                copies.add(o.cl_first, d.cl_first, 2 * k);
+                copies.add(o.cl_width, d.cl_width, 2 * k);
+                copies.add(o.cl_charge, d.cl_charge, 4 * k);
+                copies.add(o.cl_bary, d.cl_bary, 4 * k);
+                copies.add(o.cl_adc_off, d.cl_adc_off, 4 * k);
+                if (o.cl_snr) copies.add(o.cl_snr, d.cl_snr, 4 * k);
+                copies.add(o.cl_adc, d.cl_adc, na);
+            }
+            if (o.strip_adc) copies.add(o.strip_adc, d.strip_adc, n);
+            if (o.chan_off) copies.add(o.chan_off, d.chan_off, 4 * nch);
+            if (o.chan_len) copies.add(o.chan_len, d.chan_len, 2 * nch);
+            if (o.seed_idx) copies.add(o.seed_idx, d.seed_idx, 4 * std::min<size_t>(o.dev_status[SST_ST_N_SEEDS], o.cap_seeds));
+        }
+        CU(copies.run(ck.st));
+        CU(cudaFreeAsync(ck.blk, ck.st));
+    }
+    for (const Chunk &ck : chunks) cu_ok(ctx, cudaStreamSynchronize(ck.st));
     return rc;
 }
 

@@ -442,3 +442,42 @@ def test_full_size_batch_in_the_bench_configuration(H, oracle):
             assert np.array_equal(g["strip_adc"], e.z)
     finally:
         det.close()
+
+
+def test_host_batch_entry_point(H, oracle):
+    """sst_unpack_cluster_host_batch: HOST buffers in and out, chunks pipelined over streams; 21
+    events (two chunks, the second ragged) against the oracle."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf, n_ev = 9, 21
+    cfg, cal, evs = synth.make_config(3, n_feds=nf, event_seeds=range(1, n_ev + 1))
+    mrb = max(int(e.raw.size) for e in evs)
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        cc, ca = mrb // 3 + 1, mrb
+        hs = []
+        for _ in evs:
+            h = dict(n_clusters=np.zeros(1, np.uint32), dev_status=np.zeros(8, np.uint32),
+                     cl_module=np.zeros(cc, np.uint32), cl_first=np.zeros(cc, np.uint16), cl_width=np.zeros(cc, np.uint16),
+                     cl_charge=np.zeros(cc, np.int32), cl_bary=np.zeros(cc, np.float32), cl_adc_off=np.zeros(cc, np.uint32),
+                     cl_adc=np.zeros(ca, np.uint8), strip_adc=np.zeros(cal.n_strips, np.uint8),
+                     cl_snr=np.zeros(cc, np.float32), seed_idx=np.zeros(cal.n_strips, np.uint32),
+                     chan_off=np.zeros(nf * 96, np.uint32), chan_len=np.zeros(nf * 96, np.uint16))
+            hs.append(h)
+        outs = [B.make_output(cap_clusters=cc, cap_adc=ca, cap_seeds=cal.n_strips, **h) for h in hs]
+        streams = [torch.cuda.Stream() for _ in range(3)]
+        hb = B.HostBatch([e.raw for e in evs], [e.raw.size for e in evs], [e.fed_offsets for e in evs], (2, 3, 5), outs,
+                         [s.cuda_stream for s in streams])
+        for _ in range(2):
+            B.sst_unpack_cluster_host_batch(det.ctx, hb)
+        for e, h in zip(evs, hs):
+            r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            k = int(h["n_clusters"][0])
+            res = {"n_clusters": k, "status": h["dev_status"], "strip_adc": h["strip_adc"], "chan_off": h["chan_off"],
+                   "chan_len": h["chan_len"], "seed_idx": h["seed_idx"][:h["dev_status"][5]],
+                   "cl_adc": h["cl_adc"][:h["dev_status"][3]]}
+            for name in ("cl_module", "cl_first", "cl_width", "cl_charge", "cl_bary", "cl_adc_off", "cl_snr"):
+                res[name] = h[name][:k]
+            compare(res, r)
+    finally:
+        det.close()
