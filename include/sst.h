@@ -126,18 +126,23 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
  * (PAPER.md:31,33).  raw: DEVICE, 16-byte aligned, >= cfg.max_raw_bytes readable bytes;
  * fed_offsets: DEVICE [n_feds+1] byte offsets of the FEDs in raw (16-byte multiples for the
  * fast path; a FED with start > end or end > cfg.max_raw_bytes is flagged and empty).  thr and
- * out are HOST structs read before the call returns.  The work is enqueued on `stream` as one
- * kernel launch; the call does not synchronise.  Scratch comes from the context's
+ * out are HOST structs read before the call returns.  The work is enqueued on `stream` as two
+ * kernel launches (unpack + cluster per FED, then the ordered move of the clusters); the call
+ * does not synchronise.  Scratch comes from the context's
  * stream-ordered pool: one block per stream, allocated on the stream's first event and reused
  * (so a stream must not be driven by two host threads at once). */
 sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
                               const sst_thresholds *thr, const sst_output *out, void *stream);
 
-/* n_events independent events in one call (several events in flight): event e is
- * enqueued on streams[e % n_streams] with raw[e], fed_offsets[e] (DEVICE) and outs[e]; the
- * events of one stream share kernel launches (up to sst_info.events_per_launch events each),
- * and every event's result is exactly what sst_unpack_cluster gives.  raw, fed_offsets, outs and
- * streams are HOST arrays read before the call returns.  Does not synchronise. */
+/* n_events independent events in one call (several events in flight): event e
+ * belongs to streams[e % n_streams] with raw[e], fed_offsets[e] (DEVICE) and outs[e].  The events
+ * share kernel launches (up to sst_info.events_per_launch events each, walked FED by FED so that
+ * they share the calibration in L2): a launch runs on the first stream of its group after that
+ * stream has waited (by CUDA event) for whatever the group's other streams had enqueued, and
+ * those streams wait for the launch in turn -- so every event's inputs are honoured and its
+ * result is complete in stream order on its own stream.  Every event's result is exactly what
+ * sst_unpack_cluster gives.  raw, fed_offsets, outs and streams are HOST arrays read before the
+ * call returns.  Does not synchronise. */
 sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
                                     const uint32_t *const *fed_offsets, const sst_thresholds *thr,
                                     const sst_output *outs, void *const *streams, uint32_t n_streams);
@@ -187,9 +192,10 @@ int32_t sst_last_cuda_error(const sst_ctx *ctx);
 const char *sst_status_string(sst_status s);
 
 /* Static facts about the compiled kernel and this context, for benchmarks: bytes of dynamic
- * shared memory per CTA (one CTA = one warp = one FED at a time), threads per CTA, resident CTAs
- * per SM as reported by the occupancy API, SM count, kernel launches per event, the part of
- * smem_bytes that holds a FED's payload and lists, events one launch can take. */
+ * shared memory per CTA of sst_event_kernel (a CTA is threads/32 independent warps, one FED at a
+ * time each), threads per CTA, resident CTAs per SM as reported by the occupancy API, SM count,
+ * kernels per launch (sst_event_kernel + sst_emit_kernel), the part of a warp's shared memory
+ * that holds a FED's payload and lists, events one launch can take. */
 typedef struct {
     uint32_t smem_bytes, threads, ctas_per_sm, sm_count, kernels_per_event, slot_bytes, events_per_launch;
 } sst_info;

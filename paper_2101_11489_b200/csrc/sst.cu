@@ -580,11 +580,12 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 const uint32_t limit = (r + 1u) * kWin;
                 for (;;) {  // two consecutive entries per lane; the list is sorted by strip
                     const uint32_t i = i0 + 2u * lane;
-                    const uint32_t sa = i < P ? strip_l[i] & 0x7fffu : 0xffffu;
-                    const uint32_t sb = i + 1u < P ? strip_l[i + 1u] & 0x7fffu : 0xffffu;
-                    const bool ina = sa < limit, inb = sb < limit;
-                    if (ina) window[sa & (kWin - 1u)] = adc_l[i];
-                    if (inb) window[sb & (kWin - 1u)] = adc_l[i + 1u];
+                    const uint32_t ia = i < P ? i : 0u, ib = i + 1u < P ? i + 1u : 0u;  // loads stay in the lists
+                    const uint32_t sa = strip_l[ia] & 0x7fffu, sb = strip_l[ib] & 0x7fffu;
+                    const uint32_t va = adc_l[ia], vb = adc_l[ib];
+                    const bool ina = i < P && sa < limit, inb = i + 1u < P && sb < limit;
+                    if (ina) window[sa & (kWin - 1u)] = static_cast<uint8_t>(va);
+                    if (inb) window[sb & (kWin - 1u)] = static_cast<uint8_t>(vb);
                     const uint32_t cnt = __popc(__ballot_sync(kFull, ina)) + __popc(__ballot_sync(kFull, inb));
                     i0 += cnt;
                     if (cnt < 64u) break;
