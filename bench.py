@@ -7,7 +7,7 @@ strips, generator of config 1, seeds 1..64) processed over 8 CUDA streams, calib
 once, per-event output buffers taken from the library's stream-ordered pool.
 
   value      whole-job events/s with the raw data already resident in HBM (CUDA-event timed)
-  e2e        the same metric through sst_unpack_cluster_host_batch: pinned HOST buffers, H2D of the raw
+  e2e        the same metric through sst_unpack_cluster_host_packed: pinned HOST buffers, H2D of the raw
              data and D2H of the clusters inside the timed region
   roofline   algorithmic HBM bytes of a launch / launch duration for sst_event_kernel (the dominant
              kernel; sst_emit_kernel behind it moves the staged clusters into order) against
@@ -436,7 +436,7 @@ def main():
                   "note": "one stream, CUDA events around each launch, launches queued behind a sleep kernel"}
         del outs1
 
-    # ---- e2e: HOST buffers through sst_unpack_cluster_host_batch
+    # ---- e2e: HOST buffers through sst_unpack_cluster_host_packed
     e2e = None
     if not args.no_e2e:
         pin = [(torch.from_numpy(e[0]).pin_memory(), torch.from_numpy(e[1].view(np.int32)).pin_memory())
@@ -455,16 +455,18 @@ def main():
                  "cl_adc": torch.empty(cap_adc, dtype=torch.uint8).pin_memory()}
             return t, B.make_output(cap_clusters=cap_cl, cap_adc=cap_adc, **t)
 
-        # one pinned output set per event; one C call per step: sst_unpack_cluster_host_batch cuts the
-        # 64 events into chunks whose uploads, launches and downloads overlap on the 8 streams
-        houts = [host_outputs() for _ in range(n_events)]
+        # one pinned, packed result block per event; one C call per step:
+        # sst_unpack_cluster_host_packed cuts the 64 events into chunks whose uploads, launches and
+        # (single, exactly-sized) downloads overlap on the 8 streams
+        host_blocks = [torch.zeros(64 + 20 * cap_cl + cap_adc, dtype=torch.uint8).pin_memory() for _ in range(n_events)]
         e2e_steps = max(1, min(args.steps, 20))
-        hbatch = B.HostBatch([p[0] for p in pin], [int(e[0].size) for e in events], [p[1] for p in pin], THRESHOLDS,
-                             [h[1] for h in houts], [st.cuda_stream for st in streams])
+        pbatch = B.PackedBatch([p[0] for p in pin], [int(e[0].size) for e in events], [p[1] for p in pin], THRESHOLDS,
+                               cap_cl, cap_adc, host_blocks, [st.cuda_stream for st in streams])
+        counts_view = [blk.numpy()[32:36].view(np.uint32) for blk in host_blocks]
 
         def e2e_step():
-            B.sst_unpack_cluster_host_batch(det.ctx, hbatch)
-            return sum(int(h[0]["n_clusters"][0]) for h in houts)
+            B.sst_unpack_cluster_host_packed(det.ctx, pbatch)
+            return sum(int(c[0]) for c in counts_view)
 
         for _ in range(2):
             e2e_step()
@@ -483,8 +485,8 @@ def main():
         d2h = sum(36 + 20 * p["n_clusters"] + p["n_adc"] for p in per_event)
         e2e = {"value": world * n_events * e2e_steps / dt, "unit": "events/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": e2e_steps, "host_threads": 1,
-               "api": "sst_unpack_cluster_host_batch (pinned host raw in; status, cluster records and ADCs out; "
-                      "chunks of 4 events pipelined over the 8 streams, pinned outputs written by the kernel over PCIe)"}
+               "api": "sst_unpack_cluster_host_packed (pinned host raw in; status, cluster records and ADCs out as one "
+                      "packed block per event; chunks of 4 events pipelined over the 8 streams)"}
 
     # ---- CPU baseline (rank 0, N = 1 only)
     cpu = cpu_omp = None

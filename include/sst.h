@@ -169,6 +169,24 @@ sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const 
                                          const sst_thresholds *thr, const sst_output *outs, void *const *streams,
                                          uint32_t n_streams);
 
+/* The host entry point with PACKED results: one download per event instead of one per array.
+ * results[e].block is a HOST block (pinned for asynchronous copies) of at least
+ * 64 + 20*cap_clusters + cap_adc bytes; on return it holds {dev_status[8], n_clusters, pad to 64
+ * bytes} followed by the arrays cl_module, cl_charge, cl_bary, cl_adc_off (4 bytes per cluster),
+ * cl_first, cl_width (2 bytes) and cl_adc back to back, each with K = min(clusters found,
+ * cap_clusters) elements, and results[e].view is an sst_output whose HOST pointers point into the
+ * block (strip_adc, chan_off, chan_len, seed_idx, cl_snr are not produced: NULL).  Events are
+ * chunked over the streams as in sst_unpack_cluster_host_batch; returns when all are done. */
+typedef struct {
+    void *block;          /* HOST, caller-owned */
+    uint64_t block_bytes; /* its size */
+    sst_output view;      /* filled by the call */
+} sst_packed_result;
+sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
+                                          const uint32_t *raw_bytes, const uint32_t *const *fed_offsets,
+                                          const sst_thresholds *thr, uint32_t cap_clusters, uint32_t cap_adc,
+                                          sst_packed_result *results, void *const *streams, uint32_t n_streams);
+
 /* Stream-ordered allocation of per-event buffers from the context's pool (cudaMallocAsync;
  * replaces the caching allocator of PAPER.md:41).  The pointer is usable by work enqueued on
  * `stream` after the call; free it with sst_event_free on a stream that has seen all its uses. */

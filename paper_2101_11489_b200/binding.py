@@ -20,7 +20,7 @@ FLAG_CLUSTER_CAP, FLAG_ADC_CAP, FLAG_MALFORMED, FLAG_OVERRUN = 1, 2, 4, 8
 SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB = range(5)
 
 EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
-           "sst_unpack_cluster_host_batch",
+           "sst_unpack_cluster_host_batch", "sst_unpack_cluster_host_packed",
            "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_destroy", "sst_last_cuda_error",
            "sst_status_string", "sst_get_info"]
 
@@ -73,6 +73,8 @@ def load():
     L.sst_unpack_cluster_host.argtypes = [vp, vp, C.c_uint32, vp, C.POINTER(sst_thresholds),
                                           C.POINTER(sst_output), vp]
     L.sst_unpack_cluster_host_batch.argtypes = [vp, C.c_uint32, vp, vp, vp, C.POINTER(sst_thresholds), vp, vp, C.c_uint32]
+    L.sst_unpack_cluster_host_packed.argtypes = [vp, C.c_uint32, vp, vp, vp, C.POINTER(sst_thresholds), C.c_uint32,
+                                                 C.c_uint32, vp, vp, C.c_uint32]
     L.sst_event_alloc.argtypes = [vp, C.c_uint64, vp, C.POINTER(vp)]
     L.sst_event_free.argtypes = [vp, vp, vp]
     L.sst_event_upload.argtypes = [vp, vp, C.c_uint32, vp, vp, C.POINTER(vp), C.POINTER(vp)]
@@ -195,6 +197,58 @@ def sst_unpack_cluster_host_batch(ctx, batch: HostBatch):
     rc = load().sst_unpack_cluster_host_batch(ctx, batch.n, batch.raw, batch.raw_bytes, batch.fo, C.byref(batch.thr),
                                               batch.outs, batch.streams, batch.n_streams)
     _check(ctx, rc, "sst_unpack_cluster_host_batch")
+
+
+class sst_packed_result(C.Structure):
+    _fields_ = [("block", C.c_void_p), ("block_bytes", C.c_uint64), ("view", sst_output)]
+
+
+class PackedBatch:
+    """Marshalled arguments of sst_unpack_cluster_host_packed: one HOST result block per event."""
+
+    def __init__(self, raws, raw_bytes, fed_offsets, thresholds, cap_clusters, cap_adc, blocks, streams):
+        n = len(raws)
+        self.n = n
+        self.keep = (list(raws), list(fed_offsets), list(blocks))
+        self.raw = (C.c_void_p * n)(*[_ptr(r) for r in raws])
+        self.raw_bytes = (C.c_uint32 * n)(*[int(x) for x in raw_bytes])
+        self.fo = (C.c_void_p * n)(*[_ptr(f) for f in fed_offsets])
+        self.cap_clusters, self.cap_adc = int(cap_clusters), int(cap_adc)
+        self.results = (sst_packed_result * n)()
+        for i, blk in enumerate(blocks):
+            self.results[i].block = _ptr(blk)
+            self.results[i].block_bytes = int(blk.nbytes if hasattr(blk, "nbytes") else blk.numel() * blk.element_size())
+        self.streams = (C.c_void_p * len(streams))(*streams)
+        self.n_streams = len(streams)
+        self.thr = thresholds if isinstance(thresholds, sst_thresholds) else sst_thresholds(*map(float, thresholds))
+
+    def view(self, i: int):
+        """numpy views of event i's arrays inside its block (valid after the call)."""
+        import numpy as np
+        r = self.results[i]
+        blk = self.keep[2][i]
+        a = blk.numpy() if hasattr(blk, "numpy") and not isinstance(blk, np.ndarray) else blk
+        a = a.view(np.uint8).reshape(-1)
+        st = a[:32].view(np.uint32)
+        k = int(a[32:36].view(np.uint32)[0])
+        K = min(int(st[ST_N_CLUSTERS]), self.cap_clusters)
+        na = min(int(st[ST_N_ADC]), self.cap_adc)
+        o = 64
+        out = {"status": st, "n_clusters": k}
+        for name, dt, w in (("cl_module", np.uint32, 4), ("cl_charge", np.int32, 4), ("cl_bary", np.float32, 4),
+                            ("cl_adc_off", np.uint32, 4), ("cl_first", np.uint16, 2), ("cl_width", np.uint16, 2)):
+            out[name] = a[o:o + w * K].view(dt)[:k]
+            o += w * K
+        out["cl_adc"] = a[o:o + na]
+        return out
+
+
+def sst_unpack_cluster_host_packed(ctx, batch: PackedBatch):
+    """batch.n events with HOST buffers and packed HOST result blocks; returns when all are done."""
+    rc = load().sst_unpack_cluster_host_packed(ctx, batch.n, batch.raw, batch.raw_bytes, batch.fo, C.byref(batch.thr),
+                                               batch.cap_clusters, batch.cap_adc, batch.results, batch.streams,
+                                               batch.n_streams)
+    _check(ctx, rc, "sst_unpack_cluster_host_packed")
 
 
 def sst_event_alloc(ctx, nbytes: int, stream: int = 0) -> int:

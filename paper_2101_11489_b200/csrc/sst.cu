@@ -64,6 +64,9 @@
 #ifndef SST_T_PF_HINT
 #define SST_T_PF_HINT 1
 #endif
+#ifndef SST_HOST_CHUNK
+#define SST_HOST_CHUNK 4
+#endif
 #ifndef SST_WPC
 #define SST_WPC 8
 #endif
@@ -93,6 +96,7 @@ constexpr int kShOver = 51, kShMalf = 44, kShSeed = 29, kShAdc = 14;
 struct EventDesc {
     const uint8_t *raw;
     const uint32_t *fed_offsets;
+    uint8_t *packed;  // result block of the packed host entry point (else NULL): see emit kernel
     sst_output out;
 };
 
@@ -1012,28 +1016,51 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
 // the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then moves the staged
 // records, cluster ADCs and seeds of the FED to their final place.  Output capacity and the event
 // totals are handled here.
+template <bool kPacked>
 __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __grid_constant__ KParams p) {
     const int lane = threadIdx.x & 31;
     const uint32_t t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (t >= p.n_events * p.n_feds) return;
     const uint32_t ev = t / p.n_feds, f = t - ev * p.n_feds;
     const EventDesc &E = p.ev[ev];
-    const sst_output &o = E.out;
+    sst_output o = E.out;
+    constexpr bool packed = kPacked;  // every event of a launch is, or none
     const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
     const unsigned long long own = st[f];
     const uint32_t fed_cl = static_cast<uint32_t>(own & 0x3fffull), fed_adc = static_cast<uint32_t>((own >> kShAdc) & 0x7fffull),
                    fed_seed = static_cast<uint32_t>((own >> kShSeed) & 0x7fffull),
                    fed_malf = static_cast<uint32_t>((own >> kShMalf) & 0x7full), fed_over = static_cast<uint32_t>((own >> kShOver) & 1ull);
     // clusters | ADC bytes << 32 ; seeds | malformed << 32 (20 bits) | overrun << 52 (n_feds <= 4096)
-    unsigned long long accA = 0, accB = 0;
+    unsigned long long accA = 0, accB = 0, totA = 0;
+    const uint32_t jend = packed ? p.n_feds : f;  // the packed layout needs the event's totals too
 #pragma unroll 8
-    for (uint32_t j = lane; j < f; j += 32) {
+    for (uint32_t j = lane; j < jend; j += 32) {
         const unsigned long long v = st[j];
-        accA += (v & 0x3fffull) | (((v >> kShAdc) & 0x7fffull) << 32);
-        accB += ((v >> kShSeed) & 0x7fffull) | (((v >> kShMalf) & 0x7full) << 32) | (((v >> kShOver) & 1ull) << 52);
+        const unsigned long long a = (v & 0x3fffull) | (((v >> kShAdc) & 0x7fffull) << 32);
+        totA += a;
+        if (j < f) {
+            accA += a;
+            accB += ((v >> kShSeed) & 0x7fffull) | (((v >> kShMalf) & 0x7full) << 32) | (((v >> kShOver) & 1ull) << 52);
+        }
     }
     accA = warp_sum64(accA);
     accB = warp_sum64(accB);
+    if (packed) {
+        // one block per event: {dev_status[8], n_clusters, pad to 64 B}, then the arrays back to
+        // back with K = min(clusters found, cap_clusters) elements each: module, charge, bary,
+        // adc_off (4 B), first, width (2 B), and the cluster ADCs -- one download per event
+        const size_t K = min(static_cast<uint32_t>(warp_sum64(totA)), o.cap_clusters);
+        uint8_t *b = E.packed;
+        o.dev_status = reinterpret_cast<uint32_t *>(b);
+        o.n_clusters = reinterpret_cast<uint32_t *>(b + 32);
+        o.cl_module = reinterpret_cast<uint32_t *>(b + 64);
+        o.cl_charge = reinterpret_cast<int32_t *>(b + 64 + 4 * K);
+        o.cl_bary = reinterpret_cast<float *>(b + 64 + 8 * K);
+        o.cl_adc_off = reinterpret_cast<uint32_t *>(b + 64 + 12 * K);
+        o.cl_first = reinterpret_cast<uint16_t *>(b + 64 + 16 * K);
+        o.cl_width = reinterpret_cast<uint16_t *>(b + 64 + 18 * K);
+        o.cl_adc = b + 64 + 20 * K;
+    }
     const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
     const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
                    b_over = static_cast<uint32_t>(accB >> 52);
@@ -1204,7 +1231,8 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
 
 // Launches one kernel for `n` (<= kMaxEv) events on `st`.
 sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, const uint32_t *const *fed_offsets,
-                         const sst_thresholds *thr, const sst_output *const *outs, cudaStream_t st) {
+                         const sst_thresholds *thr, const sst_output *const *outs, cudaStream_t st,
+                         uint8_t *const *packed = nullptr) {
     const uint32_t nf = ctx->cfg.n_feds;
     const uint32_t total = n * nf;
     // warps per CTA: full CTAs once the work fills the GPU, smaller ones to spread a small launch
@@ -1274,10 +1302,12 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         kp.ev[e].raw = raw[e];
         kp.ev[e].fed_offsets = fed_offsets[e];
         kp.ev[e].out = *outs[e];
+        kp.ev[e].packed = packed ? packed[e] : nullptr;
     }
     sst_event_kernel<<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
     SST_CU(cudaGetLastError());
-    sst_emit_kernel<<<(total + 3) / 4, 128, 0, st>>>(kp);
+    if (packed) sst_emit_kernel<true><<<(total + 3) / 4, 128, 0, st>>>(kp);
+    else sst_emit_kernel<false><<<(total + 3) / 4, 128, 0, st>>>(kp);
     SST_CU(cudaGetLastError());
     return SST_OK;
 }
@@ -1613,9 +1643,6 @@ sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const 
     // FED-major launch, counts back -- so the uploads, kernels and downloads of neighbouring chunks
     // overlap.  The cluster arrays are then fetched chunk by chunk with exactly-sized
     // copies while later chunks are still being processed.
-#ifndef SST_HOST_CHUNK
-#define SST_HOST_CHUNK 4
-#endif
     constexpr uint32_t kHostChunk = SST_HOST_CHUNK;
     auto mapped = [](const void *h, void *&d) {
         cudaPointerAttributes a{};
@@ -1736,6 +1763,85 @@ sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const 
             if (o.seed_idx) copies.add(o.seed_idx, d.seed_idx, 4 * std::min<size_t>(o.dev_status[SST_ST_N_SEEDS], o.cap_seeds));
         }
         CU(copies.run(ck.st));
+        CU(cudaFreeAsync(ck.blk, ck.st));
+    }
+    for (const Chunk &ck : chunks) cu_ok(ctx, cudaStreamSynchronize(ck.st));
+    return rc;
+}
+
+sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
+                                          const uint32_t *raw_bytes, const uint32_t *const *fed_offsets,
+                                          const sst_thresholds *thr, uint32_t cap_clusters, uint32_t cap_adc,
+                                          sst_packed_result *results, void *const *streams, uint32_t n_streams) {
+    if (!ctx || !raw || !raw_bytes || !fed_offsets || !thr || !results || !streams || n_streams == 0 || !thresholds_ok(thr))
+        return SST_ERR_INVALID_ARG;
+    if (!ctx->has_calib) return SST_ERR_NO_CALIB;
+    const size_t block_need = 64 + 20ull * cap_clusters + cap_adc;
+    for (uint32_t e = 0; e < n_events; ++e)
+        if (!raw[e] || !fed_offsets[e] || !results[e].block || results[e].block_bytes < block_need ||
+            raw_bytes[e] > ctx->cfg.max_raw_bytes)
+            return SST_ERR_INVALID_ARG;
+    if (n_events == 0) return SST_OK;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    const uint32_t nf = ctx->cfg.n_feds;
+    auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
+    constexpr uint32_t kHostChunk = SST_HOST_CHUNK;
+    struct Chunk { uint32_t e0, n; cudaStream_t st; uint8_t *blk; };
+    std::vector<Chunk> chunks;
+    std::vector<uint8_t *> d_block(n_events);
+    const size_t per_event = up(ctx->cfg.max_raw_bytes) + up((nf + 1) * 4) + up(block_need);
+    sst_status rc = SST_OK;
+    auto CU = [&](cudaError_t e) { if (rc == SST_OK && !cu_ok(ctx, e)) rc = SST_ERR_CUDA; };
+    sst_output proto{};
+    proto.cap_clusters = cap_clusters;
+    proto.cap_adc = cap_adc;
+    for (uint32_t e0 = 0; e0 < n_events && rc == SST_OK; e0 += kHostChunk) {
+        Chunk ck{e0, std::min(kHostChunk, n_events - e0), static_cast<cudaStream_t>(streams[chunks.size() % n_streams]), nullptr};
+        CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&ck.blk), per_event * ck.n, ctx->pool, ck.st));
+        if (rc != SST_OK) break;
+        const uint8_t *r[kHostChunk];
+        const uint32_t *fo[kHostChunk];
+        const sst_output *po[kHostChunk];
+        uint8_t *pk[kHostChunk];
+        for (uint32_t i = 0; i < ck.n; ++i) {
+            uint8_t *q = ck.blk + per_event * i;
+            uint8_t *d_raw = q;
+            uint32_t *d_fo = reinterpret_cast<uint32_t *>(q + up(ctx->cfg.max_raw_bytes));
+            d_block[e0 + i] = q + up(ctx->cfg.max_raw_bytes) + up((nf + 1) * 4);
+            if (raw_bytes[e0 + i]) CU(cudaMemcpyAsync(d_raw, raw[e0 + i], raw_bytes[e0 + i], cudaMemcpyHostToDevice, ck.st));
+            CU(cudaMemcpyAsync(d_fo, fed_offsets[e0 + i], (nf + 1) * 4, cudaMemcpyHostToDevice, ck.st));
+            r[i] = d_raw;
+            fo[i] = d_fo;
+            po[i] = &proto;
+            pk[i] = d_block[e0 + i];
+        }
+        if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st, pk);
+        for (uint32_t i = 0; i < ck.n; ++i)  // status and count first: they size the one big copy
+            CU(cudaMemcpyAsync(results[e0 + i].block, d_block[e0 + i], 64, cudaMemcpyDeviceToHost, ck.st));
+        chunks.push_back(ck);
+    }
+    for (const Chunk &ck : chunks) {
+        CU(cudaStreamSynchronize(ck.st));
+        if (rc != SST_OK) break;
+        for (uint32_t i = 0; i < ck.n; ++i) {
+            sst_packed_result &R = results[ck.e0 + i];
+            uint8_t *b = static_cast<uint8_t *>(R.block);
+            const uint32_t *stw = reinterpret_cast<const uint32_t *>(b);
+            const size_t K = std::min(stw[SST_ST_N_CLUSTERS], cap_clusters);
+            const size_t na = std::min(stw[SST_ST_N_ADC], cap_adc);
+            CU(cudaMemcpyAsync(b + 64, d_block[ck.e0 + i] + 64, 20 * K + na, cudaMemcpyDeviceToHost, ck.st));
+            sst_output &v = R.view;
+            v = proto;
+            v.dev_status = reinterpret_cast<uint32_t *>(b);
+            v.n_clusters = reinterpret_cast<uint32_t *>(b + 32);
+            v.cl_module = reinterpret_cast<uint32_t *>(b + 64);
+            v.cl_charge = reinterpret_cast<int32_t *>(b + 64 + 4 * K);
+            v.cl_bary = reinterpret_cast<float *>(b + 64 + 8 * K);
+            v.cl_adc_off = reinterpret_cast<uint32_t *>(b + 64 + 12 * K);
+            v.cl_first = reinterpret_cast<uint16_t *>(b + 64 + 16 * K);
+            v.cl_width = reinterpret_cast<uint16_t *>(b + 64 + 18 * K);
+            v.cl_adc = b + 64 + 20 * K;
+        }
         CU(cudaFreeAsync(ck.blk, ck.st));
     }
     for (const Chunk &ck : chunks) cu_ok(ctx, cudaStreamSynchronize(ck.st));

@@ -481,3 +481,35 @@ def test_host_batch_entry_point(H, oracle):
             compare(res, r)
     finally:
         det.close()
+
+
+def test_host_packed_entry_point(H, oracle):
+    """sst_unpack_cluster_host_packed: one packed HOST result block per event; clusters against the
+    oracle, including a capacity overflow (the packed layout then holds cap_clusters slots)."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf, n_ev = 9, 11
+    cfg, cal, evs = synth.make_config(3, n_feds=nf, event_seeds=range(1, n_ev + 1))
+    mrb = max(int(e.raw.size) for e in evs)
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        streams = [torch.cuda.Stream() for _ in range(3)]
+        for cc, ca in ((mrb // 3 + 1, mrb), (500, mrb), (mrb // 3 + 1, 700)):
+            blocks = [torch.zeros(64 + 20 * cc + ca, dtype=torch.uint8).pin_memory() for _ in evs]
+            pb = B.PackedBatch([e.raw for e in evs], [e.raw.size for e in evs], [e.fed_offsets for e in evs], (2, 3, 5),
+                               cc, ca, blocks, [s.cuda_stream for s in streams])
+            for _ in range(2):
+                B.sst_unpack_cluster_host_packed(det.ctx, pb)
+            for i, e in enumerate(evs):
+                r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5),
+                               cap_clusters=cc, cap_adc=ca)
+                g = pb.view(i)
+                assert g["n_clusters"] == r.n_clusters
+                assert np.array_equal(g["status"][:6], r.status[:6])
+                for name in ("cl_module", "cl_first", "cl_width", "cl_charge", "cl_adc_off"):
+                    assert np.array_equal(g[name], getattr(r, name)), name
+                np.testing.assert_allclose(g["cl_bary"], r.cl_bary, rtol=REL, atol=0)
+                na = int(r.cl_adc_off[-1]) + int(r.cl_width[-1]) if r.n_clusters else 0
+                assert np.array_equal(g["cl_adc"][:na], r.cl_adc[:na])
+    finally:
+        det.close()
