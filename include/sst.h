@@ -87,7 +87,9 @@ enum {
  * + cl_width[k]) and cl_adc_off is the exclusive prefix sum of cl_width.
  * Capacity: cluster k is written iff k < cap_clusters and cl_adc_off[k]+cl_width[k] <= cap_adc;
  * the clusters written are always a prefix, *n_clusters is their number and nothing is written
- * beyond either capacity.  cap_clusters >= raw_bytes/3 and cap_adc >= raw_bytes never overflow.
+ * beyond either capacity.  cap_clusters >= raw_bytes/2 and cap_adc >= raw_bytes never overflow
+ * (a cluster costs at least two raw bytes: one ADC byte and an inactive strip or a run header
+ * behind it; in zero-suppressed data, where every cluster is its own run, raw_bytes/3 suffices).
  */
 typedef struct {
     uint8_t *strip_adc;   /* [N] dense unpacked ADC, absent strip = 0; NULL = do not materialise;

@@ -808,7 +808,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     }
     {
         // cluster records: lane per cluster, consecutive lanes write consecutive records
-        const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 3u + f;
+        const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
         const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
         uint8_t *const sa = p.s_adc + ab;  // the FED's cluster ADCs, in order
@@ -1067,7 +1067,7 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     // where sst_event_kernel staged this FED
     const uint32_t fo0 = E.fed_offsets[f], fo1 = E.fed_offsets[f + 1];
     const uint32_t fed_start = (fo0 <= fo1 && fo1 <= p.max_raw_bytes) ? fo0 : 0u;
-    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 3u + f;
+    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
     const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
     const unsigned long long pol_first = policy_evict_first();
 
@@ -1210,7 +1210,8 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
     L.ents = (static_cast<size_t>(ctx->cfg.max_raw_bytes) + 16ull * nf + 64 + 31) & ~static_cast<size_t>(31);
     L.mwords = L.ents / 32 + 4ull * nf + 16;
-    L.cl_slots = static_cast<size_t>(ctx->cfg.max_raw_bytes) / 3 + nf + 8;  // a cluster costs >= 3 raw bytes
+    // a cluster costs >= 2 raw bytes: one ADC byte and a separator (an inactive strip, or a run header)
+    L.cl_slots = static_cast<size_t>(ctx->cfg.max_raw_bytes) / 2 + nf + 8;
     L.state_bytes = sizeof(unsigned long long) * nf * cap_events;
     L.o_ticket = 0;
     L.o_state = 256;

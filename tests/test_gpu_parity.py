@@ -513,3 +513,24 @@ def test_host_packed_entry_point(H, oracle):
                 assert np.array_equal(g["cl_adc"][:na], r.cl_adc[:na])
     finally:
         det.close()
+
+
+def test_densest_possible_clusters(H, oracle):
+    """Worst case of clusters per raw byte: full 256-strip runs alternating a seed-level ADC and a
+    present-but-inactive one (12288 single-strip clusters in 24960 bytes of one FED, more than
+    raw/3): the FED-local staging must hold them, neighbours must stay intact."""
+    n_feds = 3
+    n = n_feds * synth.FED_STRIPS
+    z = np.zeros(n, np.uint8)
+    z[0::2] = 40
+    z[1::2] = 5                                    # present, 5 / 4 < 2: inactive
+    z[2 * synth.FED_STRIPS:] = 0
+    z[2 * synth.FED_STRIPS + 100:2 * synth.FED_STRIPS + 104] = (9, 40, 10, 7)
+    raw, fo = synth.encode_dense(z, n_feds)
+    gain, noise, bad = np.ones(n, np.float32), np.full(n, 4.0, np.float32), np.zeros(n, np.uint8)
+    cm = cases.module_map_from_sizes(n_feds, (2, 3))
+    cc, ca = int(raw.size), int(raw.size)
+    g = gpu_run(H, n_feds, raw, fo, gain, noise, bad, cm, (2, 3, 5), cap_clusters=cc, cap_adc=ca)
+    r = oracle.run(raw, fo, n_feds, gain, noise, bad, cm, (2, 3, 5), cap_clusters=cc, cap_adc=ca)
+    compare(g, r)
+    assert g["n_clusters"] == 2 * 12288 + 1 and g["n_clusters"] > raw.size // 3
