@@ -3,11 +3,12 @@
 // Two kernels per launch, ONE WARP PER FED (a FED is 96 channels x 256 strips;
 // modules never cross a FED, reading s10).
 //
-// sst_event_kernel: a CTA is four independent warps, each with a ~7 KB shared-memory slot, so 28
+// sst_event_kernel: a CTA is eight independent warps, each with a ~7 KB shared-memory slot, so 32
 // FEDs are in flight per SM and the serial parts of the method (the channel-length chain, the run
 // headers) of one FED hide behind the parallel parts of the others; there is no block-wide
 // barrier anywhere.  Warps draw (FED, event) tickets in FED-major order, so the FED's slab of the
-// calibration is read from HBM once per launch and serves all the launch's events from L2.
+// calibration is read from HBM once per launch (bulk-prefetched into L2 two FEDs ahead) and serves
+// all the launch's events from L2.
 // Per FED, everything after the unpack runs in the COMPACT index space of the FED's present
 // strips (the structure of arrays of PAPER.md:31 has one entry per recorded strip):
 //
@@ -15,7 +16,8 @@
 //                             chain walked in shared memory (PAPER.md:31 builds it on the CPU)
 //   a2 unpack               : lane per channel: pass 1 validates the run headers and counts, a
 //                             warp scan gives every channel its slot range, pass 2 writes the
-//                             {strip, adc} lists in ascending strip order and scatters the dense SoA
+//                             {strip, adc} lists in ascending strip order; the dense SoA is put
+//                             together in a 2 KB shared-memory window and stored as full vectors
 //   a3-a6 sweep             : lane per CHUNK of consecutive entries, walked serially: one 8-byte
 //                             gather of {noise, gain}, exact >= tests, link to the previous entry,
 //                             q = min(254, floor(adc/gain + .5)) in float32, and the open
