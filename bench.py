@@ -253,6 +253,69 @@ def workload_config(n_feds, n_events):
 
 
 # --------------------------------------------------------------------------- GPU arm
+
+def run_sweep(args):
+    """Single-event device latency of every single-event config, and config 3 throughput against
+    the events per call (Table 1 sweeps the events in flight)."""
+    import torch
+    from paper_2101_11489_b200 import binding as B, harness
+    torch.cuda.set_device(0)
+    out = {"single_event": [], "events_per_call": []}
+    for cid in (0, 1, 2, 4):
+        cfg, cal, evs = synth.make_config(cid)
+        ev = evs[0]
+        nf = cal.n_feds
+        mrb = (int(ev.raw.size) + 4095) // 4096 * 4096
+        hint = int(1.05 * int(np.count_nonzero(ev.z.reshape(nf, -1), axis=1).max())) + 16
+        det = harness.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb, fed_strips_hint=hint)
+        d_raw, d_fo = det.upload_raw(ev.raw, ev.fed_offsets)
+        outs = det.alloc_outputs(mrb // 3 + 1, mrb, dense=True)
+        st = torch.cuda.Stream()
+        for thr in cfg.thresholds:
+            n_rep = 30
+            evs_t = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_rep)]
+            for rep in range(2):
+                with torch.cuda.stream(st):
+                    torch.cuda._sleep(2_000_000)
+                for a, b in evs_t:
+                    a.record(st)
+                    det.run(d_raw, d_fo, thr, outs, stream=st)
+                    b.record(st)
+                torch.cuda.synchronize()
+            us = float(np.median([a.elapsed_time(b) for a, b in evs_t])) * 1e3
+            g = outs.numpy()
+            out["single_event"].append({"config": cid, "n_feds": nf, "thresholds": list(thr), "latency_us": us,
+                                        "present_strips": int(ev.meta["present"]), "clusters": int(g["n_clusters"]),
+                                        "raw_bytes": int(ev.raw.size), "info": det.info()})
+        del outs
+        det.close()
+    n_feds = args.n_feds
+    calib = synth.make_calibration(n_feds, synth.CONFIGS[3].bad_frac)
+    events = generate_events(3, n_feds, range(1, N_EVENTS + 1), calib)
+    mrb = (max(int(e[0].size) for e in events) + 4095) // 4096 * 4096
+    hint = int(1.05 * max(int(e[2]["max_fed_strips"]) for e in events)) + 16
+    det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, max_raw_bytes=mrb, fed_strips_hint=hint)
+    d_in = [det.upload_raw(e[0], e[1]) for e in events]
+    streams = [torch.cuda.Stream() for _ in range(N_STREAMS)]
+    outs = [det.alloc_outputs(mrb // 3 + 1, mrb, dense=True) for _ in events]
+    for n in (1, 2, 4, 8, 16, 32, 64):
+        batch = B.Batch([d[0] for d in d_in[:n]], [d[1] for d in d_in[:n]], THRESHOLDS, [o.out for o in outs[:n]],
+                        [s.cuda_stream for s in streams])
+        steps = max(20, 640 // n)
+        for _ in range(5):
+            B.sst_unpack_cluster_batch(det.ctx, batch)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            B.sst_unpack_cluster_batch(det.ctx, batch)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        out["events_per_call"].append({"events": n, "streams": min(n, N_STREAMS), "events_per_s": n * steps / dt,
+                                       "us_per_event": 1e6 * dt / (n * steps)})
+    det.close()
+    print(json.dumps({"sweep": out}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -266,9 +329,14 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--serial", action="store_true", help="also time the kernel alone on one stream")
+    ap.add_argument("--sweep", action="store_true",
+                    help="instead of the bench line: single-event latency of configs 0, 1, 2, 4 and events/s against "
+                         "the number of events per call (mirrors the N sweep of PAPER.md Table 1)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3
+    if args.sweep:
+        return run_sweep(args)
     if args.impl == "reference":
         run_reference(args)
         return

@@ -455,12 +455,21 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         const uint32_t A = (c.fed_size + 15u) & ~15u;
         strip_l = reinterpret_cast<uint16_t *>(slot + A);
         adc_l = slot + A + 2u * P;
-        mS = reinterpret_cast<uint32_t *>(slot);
+        // masks behind the lists when there is room (the records then get all of the payload's
+        // place), else in front of the records
+        const uint32_t tail = (A + 3u * P + 15u) & ~15u, mbytes = 16u * (nw + 2);
+        if (tail + mbytes <= p.slot_bytes) {
+            mS = reinterpret_cast<uint32_t *>(slot + tail);
+            rec = reinterpret_cast<uint32_t *>(slot);
+            rec_cap = A / 4u - 1u;
+        } else {
+            mS = reinterpret_cast<uint32_t *>(slot);
+            rec = mS + 4u * (nw + 2);
+            rec_cap = (A - mbytes) / 4u - 1u;
+        }
         mA = mS + (nw + 2);
         mH = mA + (nw + 2);
         mP = mH + (nw + 2);
-        rec = mP + (nw + 2);
-        rec_cap = (A - 16u * (nw + 2)) / 4u - 1u;
         window = A >= kWin ? slot : slot + ((A + 3u * P + 15u) & ~15u);
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
@@ -894,7 +903,8 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     c.fed_start = valid ? fo0 : 0u;
     c.fed_size = valid ? fo1 - fo0 : 0u;
     c.overrun = valid ? 0u : 1u;
-    const bool staged = !force_slow && c.fed_size + kTabBytes <= p.slot_bytes && ((c.fed_start | c.fed_size) & 15u) == 0 &&
+    // (force_slow only moves the lists to global memory; the payload is staged all the same)
+    const bool staged = c.fed_size + kTabBytes <= p.slot_bytes && ((c.fed_start | c.fed_size) & 15u) == 0 &&
                         (reinterpret_cast<uintptr_t>(E.raw) & 15u) == 0;
     __syncwarp();  // every lane is done with the slot of the previous FED
     if (staged && c.fed_size && lane == 0) {
@@ -980,7 +990,8 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     SST_MARK(3);
     // fast path: lists behind the payload, masks and at least a few records in its place
     const uint32_t A = (c.fed_size + 15u) & ~15u;
-    if (staged && A + 3u * c.P + (A >= kWin ? 0u : kWin + 16u) <= p.slot_bytes && 16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
+    if (!force_slow && staged && A + 3u * c.P + (A >= kWin ? 0u : kWin + 16u) <= p.slot_bytes &&
+        16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
         return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
     return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
