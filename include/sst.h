@@ -49,8 +49,9 @@ typedef enum {
 typedef struct {
     uint32_t n_feds;               /* FEDs per event (fixed for the context)                    */
     int32_t device;                /* CUDA device ordinal                                       */
-    uint32_t max_raw_bytes;        /* every `raw` buffer holds at least this many readable bytes;
-                                      a FED whose end offset exceeds it is flagged and empty    */
+    uint32_t max_raw_bytes;        /* every DEVICE `raw` buffer holds at least this many readable
+                                      bytes; a FED whose end offset exceeds it (or, in the HOST
+                                      entry points, the event's raw_bytes) is flagged and empty */
     uint32_t max_events_in_flight; /* hint for the pool (0 = default 8)                         */
     uint32_t fed_strips_hint;      /* expected maximum of present (zero-suppressed) strips in one
                                       FED; sizes the per-FED shared-memory working set.  0 = derive
@@ -127,7 +128,8 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
  * leftmost-seed ownership, gain correction, cluster threshold, ordered output
  * (PAPER.md:31,33).  raw: DEVICE, 16-byte aligned, >= cfg.max_raw_bytes readable bytes;
  * fed_offsets: DEVICE [n_feds+1] byte offsets of the FEDs in raw (16-byte multiples for the
- * fast path; a FED with start > end or end > cfg.max_raw_bytes is flagged and empty).  thr and
+ * fast path; the offsets must not step back: a FED with start > end, end > cfg.max_raw_bytes or a
+ * start below any earlier entry of fed_offsets is flagged and empty).  thr and
  * out are HOST structs read before the call returns.  The work is enqueued on `stream` as two
  * kernel launches (unpack + cluster per FED, then the ordered move of the clusters); the call
  * does not synchronise.  Scratch comes from the context's
@@ -203,6 +205,12 @@ sst_status sst_event_free(sst_ctx *ctx, void *ptr, void *stream);
 sst_status sst_event_upload(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes,
                             const uint32_t *fed_offsets, void *stream, uint8_t **d_raw,
                             uint32_t **d_fed_offsets);
+
+/* Enqueues the device-to-host copy of `bytes` bytes from a DEVICE buffer (an output of
+ * sst_unpack_cluster, e.g. one carved out of an sst_event_alloc block) into HOST memory on
+ * `stream` (transfers of one event overlap the kernels of the others when dst is
+ * pinned).  Does not synchronise: dst is valid once the stream has completed. */
+sst_status sst_event_download(sst_ctx *ctx, void *dst, const void *src, uint64_t bytes, void *stream);
 
 /* Synchronises the device and frees everything the context owns. */
 sst_status sst_destroy(sst_ctx *ctx);

@@ -54,7 +54,9 @@
  *          status[0] |= flags, status[1] = malformed channels, status[4] = overrun FEDs.
  * A FED whose offsets are not 0 <= start <= end <= raw_bytes, or whose length chain passes
  * `end`, is flagged; the channel where that happens and all later channels of the FED are
- * empty, recorded as (chan_off = end, chan_len = 0) (reading s3b).
+ * empty, recorded as (chan_off = end, chan_len = 0) (reading s3b).  The offsets of an event
+ * never step back: a FED whose start lies below an earlier entry of fed_offsets is flagged
+ * and empty in the same way (reading s3c), so the FEDs that are decoded never overlap.
  * A malformed channel (reading s2b) contributes no strips.
  * ------------------------------------------------------------------------------------- */
 void sst_oracle_unpack(const uint8_t *raw, uint64_t raw_bytes, const uint32_t *fed_offsets,
@@ -62,11 +64,14 @@ void sst_oracle_unpack(const uint8_t *raw, uint64_t raw_bytes, const uint32_t *f
                        uint32_t *status /* [8] */)
 {
     uint32_t n_malformed = 0, n_overrun = 0;
+    uint64_t fo_max = 0; /* largest of fed_offsets[0..f) */
     for (uint32_t f = 0; f < n_feds; ++f) {
         uint64_t pos = fed_offsets[f];
         uint64_t end = fed_offsets[f + 1];
         int overrun = 0;
-        if (pos > end || end > raw_bytes) {
+        int steps_back = pos < fo_max;
+        if (pos > fo_max) fo_max = pos;
+        if (steps_back || pos > end || end > raw_bytes) {
             overrun = 1;
             end = pos; /* nothing readable */
         }

@@ -21,7 +21,7 @@ SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB =
 
 EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
            "sst_unpack_cluster_host_batch", "sst_unpack_cluster_host_packed",
-           "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_destroy", "sst_last_cuda_error",
+           "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_event_download", "sst_destroy", "sst_last_cuda_error",
            "sst_status_string", "sst_get_info"]
 
 
@@ -78,6 +78,7 @@ def load():
     L.sst_event_alloc.argtypes = [vp, C.c_uint64, vp, C.POINTER(vp)]
     L.sst_event_free.argtypes = [vp, vp, vp]
     L.sst_event_upload.argtypes = [vp, vp, C.c_uint32, vp, vp, C.POINTER(vp), C.POINTER(vp)]
+    L.sst_event_download.argtypes = [vp, vp, vp, C.c_uint64, vp]
     L.sst_destroy.argtypes = [vp]
     L.sst_last_cuda_error.argtypes = [vp]
     L.sst_last_cuda_error.restype = C.c_int32
@@ -269,6 +270,13 @@ def sst_event_upload(ctx, raw, raw_bytes: int, fed_offsets, stream: int = 0):
                                  C.byref(d_raw), C.byref(d_fo))
     _check(ctx, rc, "sst_event_upload")
     return d_raw.value, d_fo.value
+
+
+def sst_event_download(ctx, dst, src: int, nbytes: int, stream: int = 0):
+    """DEVICE pointer `src` (int) -> HOST buffer `dst` (pinned tensor / numpy array) on `stream`;
+    does not synchronise."""
+    _check(ctx, load().sst_event_download(ctx, _ptr(dst), C.c_void_p(src), nbytes, C.c_void_p(stream)),
+           "sst_event_download")
 
 
 def sst_destroy(ctx):

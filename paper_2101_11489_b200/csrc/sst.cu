@@ -54,17 +54,8 @@
 #ifndef SST_SLAB_AHEAD
 #define SST_SLAB_AHEAD 2
 #endif
-#ifndef SST_SEQ_CHANNELS
-#define SST_SEQ_CHANNELS 1
-#endif
 #ifndef SST_EMIT_CTAS
 #define SST_EMIT_CTAS 8
-#endif
-#ifndef SST_T_CALIB_LD
-#define SST_T_CALIB_LD 1
-#endif
-#ifndef SST_T_PF_HINT
-#define SST_T_PF_HINT 1
 #endif
 #ifndef SST_HOST_CHUNK
 #define SST_HOST_CHUNK 4
@@ -99,6 +90,7 @@ struct EventDesc {
     const uint8_t *raw;
     const uint32_t *fed_offsets;
     uint8_t *packed;  // result block of the packed host entry point (else NULL): see emit kernel
+    uint32_t raw_limit;  // readable bytes of raw: a FED ending beyond it is flagged and empty
     sst_output out;
 };
 
@@ -124,7 +116,6 @@ struct KParams {
     double tcl2;
     float t_ch, t_seed;
     uint32_t max_raw_bytes, n_feds, n_events, slot_bytes;
-    unsigned long long *phase_clk;  // debug builds only (SST_PHASE_TIMING)
     EventDesc ev[kMaxEv];
 };
 
@@ -179,22 +170,13 @@ __device__ __forceinline__ unsigned long long policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
-// Calibration gather.  On B200 a plain load that misses L2 pulls the whole 128-byte line from
-// DRAM; the .L2::64B qualifier halves that (measured, profiles/r01_v4.md), and nothing is reused
-// through L1.
+// Calibration gather: nothing is reused through L1, and the line stays in L2 for the launch's
+// other events (evict_last).
 __device__ __forceinline__ float2 ld_calib(const float2 *p, unsigned long long pol) {
     float2 v;
-#if SST_T_CALIB_LD == 1
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;"
                  : "=f"(v.x), "=f"(v.y)
                  : "l"(p), "l"(pol));
-#elif SST_T_CALIB_LD == 2
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
-#else
-    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.L2::64B.v2.f32 {%0,%1}, [%2], %3;"
-                 : "=f"(v.x), "=f"(v.y)
-                 : "l"(p), "l"(pol));
-#endif
     return v;
 }
 // streaming stores of the outputs
@@ -320,12 +302,6 @@ __device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uin
     }
 }
 
-#ifdef SST_PHASE_TIMING
-#define SST_MARK(k) do { if (lane == 0 && p.phase_clk) p.phase_clk[static_cast<size_t>(c.ticket) * 16 + (k)] = clock64(); } while (0)
-#else
-#define SST_MARK(k) do { } while (0)
-#endif
-
 struct FedCtx {
     uint32_t ticket, ev, f;
     uint32_t fo0;                 // the FED's start offset as given (reported in chan_off)
@@ -339,7 +315,6 @@ struct FedCtx {
 // a2 pass 1: a lane validates the run lists of its three channels (reading s2b) and
 // counts their strips; the three cursors advance in one loop, so the three dependent chains of
 // byte loads overlap.  A malformed channel contributes no strips.
-#if SST_SEQ_CHANNELS
 __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_t (&cnt)[3]) {
     uint32_t o0 = c.off[0], o1 = c.off[1], o2 = c.off[2], l0 = c.len[0], l1 = c.len[1], l2 = c.len[2];
     uint32_t n0 = 0, n1 = 0, n2 = 0, okbits = 0;
@@ -379,56 +354,6 @@ __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_
         c.n_malformed += __popc(__ballot_sync(kFull, !ok));
     }
 }
-#else
-__device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_t (&cnt)[3]) {
-    uint32_t q[3], qe[3], nf[3];
-    bool ok[3];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        q[k] = c.off[k];
-        qe[k] = q[k] + c.len[k];
-        nf[k] = 0;
-        cnt[k] = 0;
-        ok[k] = true;
-    }
-    bool more = (q[0] < qe[0]) | (q[1] < qe[1]) | (q[2] < qe[2]);
-#pragma unroll 1
-    while (more) {
-        more = false;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            if (q[k] < qe[k]) {
-                bool bad = q[k] + 2 > qe[k];
-                uint32_t first = 0, len = 0;
-                if (!bad) {
-                    first = rp[q[k]];
-                    len = rp[q[k] + 1];
-                    if (len == 0) len = 256;  // reading s2
-                    bad = first < nf[k] || first + len > kStrip || q[k] + 2 + len > qe[k];
-                }
-                if (bad) {
-                    ok[k] = false;
-                    q[k] = qe[k];
-                } else {
-                    nf[k] = first + len;
-                    q[k] += 2 + len;
-                    cnt[k] += len;
-                    more |= q[k] < qe[k];
-                }
-            }
-        }
-    }
-    c.n_malformed = 0;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        if (!ok[k]) {
-            cnt[k] = 0;
-            c.len[k] = 0;
-        }
-        c.n_malformed += __popc(__ballot_sync(kFull, !ok[k]));
-    }
-}
-#endif
 
 // ------------------------------------------------------------------------------ lists -> clusters
 // Everything after pass 1, on the FED's lists of present strips, by one warp.  kFast: lists, masks
@@ -492,7 +417,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // writes {strip, adc} in ascending strip order; bit 15 of a strip id marks strip 0 of a channel
     // that opens a module (nothing links across it).  Three cursors per lane as in pass 1.
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
-#if SST_SEQ_CHANNELS
     {
         // one channel after the other (the three register sets rotate): a third of the code of the
         // three-cursor form, and the instruction cache is what this kernel is short of
@@ -532,51 +456,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             o0 = o1; o1 = o2; l0 = l1; l1 = l2; b0_ = b1_; b1_ = b2_; opens >>= 1;
         }
     }
-#else
-    {
-        uint32_t q[3], qe[3], e[3];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            q[k] = c.off[k];
-            qe[k] = q[k] + c.len[k];
-            e[k] = c.base[k];
-        }
-        bool more = (q[0] < qe[0]) | (q[1] < qe[1]) | (q[2] < qe[2]);
-#pragma unroll 1
-        while (more) {
-            more = false;
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                if (q[k] < qe[k]) {
-                    const uint32_t qq = q[k], ee = e[k];
-                    const uint32_t first = rp[qq];
-                    uint32_t len = rp[qq + 1];
-                    if (len == 0) len = 256;
-                    // most runs hold one or two strips; on the fast path the second byte is read
-                    // unconditionally (it is inside the slot or its 16-byte tail pad)
-                    const uint32_t b0 = rp[qq + 2], b1 = (kFast || len > 1) ? rp[qq + 3] : 0u;
-                    const uint32_t sid = static_cast<uint32_t>(lane + 32 * k) * kStrip + first;
-                    const uint32_t open_bit = ((c.opens >> k) & 1u) << 15;
-                    strip_l[ee] = static_cast<uint16_t>(first == 0 ? sid | open_bit : sid);
-                    adc_l[ee] = static_cast<uint8_t>(b0);
-                    if (len > 1) {
-                        strip_l[ee + 1] = static_cast<uint16_t>(sid + 1u);
-                        adc_l[ee + 1] = static_cast<uint8_t>(b1);
-#pragma unroll 1
-                        for (uint32_t i = 2; i < len; ++i) {
-                            const uint32_t bi = rp[qq + 2 + i];
-                            strip_l[ee + i] = static_cast<uint16_t>(sid + i);
-                            adc_l[ee + i] = static_cast<uint8_t>(bi);
-                        }
-                    }
-                    e[k] = ee + len;
-                    q[k] = qq + 2 + len;
-                    more |= q[k] < qe[k];
-                }
-            }
-        }
-    }
-#endif
     __syncwarp();  // lists complete; the payload is dead from here on
 
     // ---------------------------------------------------------------- a2: dense SoA
@@ -624,7 +503,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         __syncwarp();
     }
 
-    SST_MARK(4);
     // ---------------------------------------------------------------- a3..a6: one sweep over the lists
     // Lane per CHUNK of consecutive entries, walked serially: active/seed tests, link to the previous
     // entry, and the running (charge, noise^2, seed) of the open candidate are thread-local, so a
@@ -766,7 +644,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     }
     __syncwarp();
 
-    SST_MARK(5);
     // ---------------------------------------------------------------- counts and cluster records
     // lane per mask word: exclusive prefix of (accepted heads, accepted members) per word, then
     // every head gets its record {head entry, offset of its ADCs}
@@ -802,7 +679,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     }
     __syncwarp();
 
-    SST_MARK(7);
     // ---------------------------------------------------------------- a7, first half: publish + stage
     // The FED's counts go into its state word; its clusters, cluster ADCs and seeds are staged in
     // FED-local order in global scratch.  sst_emit_kernel, launched behind this kernel on the same
@@ -860,7 +736,6 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             }
         }
     }
-    SST_MARK(9);
     return true;
 }
 
@@ -884,21 +759,23 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     if (c.ev == 0 && p.n_events > 1 && f + kSlabAhead < p.n_feds) {
         const uint8_t *slab = reinterpret_cast<const uint8_t *>(p.calib + static_cast<size_t>(f + kSlabAhead) * kFedStrips);
         constexpr uint32_t kPiece = kFedStrips * sizeof(float2) / 32;
-#if SST_T_PF_HINT
         asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(slab + lane * kPiece), "r"(kPiece), "l"(policy_evict_last()) : "memory");
-#else
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(slab + lane * kPiece), "r"(kPiece) : "memory");
-#endif
     }
     uint32_t *const chan_off = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
     uint16_t *const chan_len = reinterpret_cast<uint16_t *>(chan_off + kChan);
 
-    SST_MARK(0);
     // ---------------------------------------------------------------- a1: stage the FED payload
     // lanes 0/1 fetch the two offsets; lane 0 starts the bulk copy
     const uint32_t fo = lane < 2 ? E.fed_offsets[f + lane] : 0u;
     const uint32_t fo0 = __shfl_sync(kFull, fo, 0), fo1 = __shfl_sync(kFull, fo, 1);
-    const bool valid = fo0 <= fo1 && fo1 <= p.max_raw_bytes;
+    // reading s3c: the offsets never step back -- a FED that starts below an earlier offset is
+    // flagged and empty, so the valid FEDs of an event are disjoint and ascending (the FED-local
+    // staging areas are keyed by the start offset)
+    uint32_t fo_max = 0;
+#pragma unroll 1
+    for (uint32_t j = lane; j < f; j += 32) fo_max = max(fo_max, E.fed_offsets[j]);
+    fo_max = __reduce_max_sync(kFull, fo_max);
+    const bool valid = fo_max <= fo0 && fo0 <= fo1 && fo1 <= E.raw_limit;
     c.fo0 = fo0;
     c.fed_start = valid ? fo0 : 0u;
     c.fed_size = valid ? fo1 - fo0 : 0u;
@@ -926,7 +803,6 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         mbar_phase ^= 1u;
     }
 
-    SST_MARK(1);
     // ---------------------------------------------------------------- a1: walk the length chain
     if (staged) {
         if (lane == 0) {
@@ -966,7 +842,6 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     }
     __syncwarp();  // the channel table is in registers: its place in the slot is free
 
-    SST_MARK(2);
     // ---------------------------------------------------------------- a2 pass 1: run headers
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -987,7 +862,6 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     }
     c.P = run;  // present strips of the FED
 
-    SST_MARK(3);
     // fast path: lists behind the payload, masks and at least a few records in its place
     const uint32_t A = (c.fed_size + 15u) & ~15u;
     if (!force_slow && staged && A + 3u * c.P + (A >= kWin ? 0u : kWin + 16u) <= p.slot_bytes &&
@@ -1077,9 +951,9 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
     const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
                    b_over = static_cast<uint32_t>(accB >> 52);
-    // where sst_event_kernel staged this FED
-    const uint32_t fo0 = E.fed_offsets[f], fo1 = E.fed_offsets[f + 1];
-    const uint32_t fed_start = (fo0 <= fo1 && fo1 <= p.max_raw_bytes) ? fo0 : 0u;
+    // where sst_event_kernel staged this FED (a FED with bad offsets staged nothing: its counts
+    // are zero and the addresses below are never used)
+    const uint32_t fed_start = E.fed_offsets[f];
     const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
     const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
     const unsigned long long pol_first = policy_evict_first();
@@ -1209,10 +1083,6 @@ bool output_ok(const sst_output *o) {
            o->cl_charge && o->cl_bary && o->cl_adc_off && o->cl_adc && !(o->seed_idx == nullptr && o->cap_seeds != 0);
 }
 
-#ifdef SST_PHASE_TIMING
-unsigned long long *g_phase_clk = nullptr;
-#endif
-
 struct ScratchLayout {
     size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr,
         o_sadc, o_sseed, total;
@@ -1243,10 +1113,13 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     return L;
 }
 
-// Launches one kernel for `n` (<= kMaxEv) events on `st`.
+// Launches the two kernels for `n` (<= kMaxEv) events on `st`.  raw_limit[e] (NULL: the context's
+// max_raw_bytes) is the number of readable bytes of raw[e].  The context's launch lock is held
+// until both kernels are enqueued, so the ticket range a launch is given and the order in which
+// the launches reach the stream always agree.
 sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, const uint32_t *const *fed_offsets,
                          const sst_thresholds *thr, const sst_output *const *outs, cudaStream_t st,
-                         uint8_t *const *packed = nullptr) {
+                         uint8_t *const *packed = nullptr, const uint32_t *raw_limit = nullptr) {
     const uint32_t nf = ctx->cfg.n_feds;
     const uint32_t total = n * nf;
     // warps per CTA: full CTAs once the work fills the GPU, smaller ones to spread a small launch
@@ -1254,41 +1127,37 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     const uint32_t wpc = total >= 16u * sms ? kWarpsPerCta : total >= 8u * sms ? std::min(4, kWarpsPerCta) : total >= 4u * sms ? 2u : 1u;
     const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (kWarpsPerCta / wpc);
     const uint32_t grid = std::min((total + wpc - 1) / wpc, capacity);
-    uint8_t *blk = nullptr;
-    unsigned long long ticket_base = 0;
-    uint32_t cap = 0;
-    {
-        std::lock_guard<std::mutex> lock(ctx->slot_mu);
-        sst_ctx::Slot *sl = nullptr;
-        for (auto &s : ctx->slots)
-            if (s.stream == st) sl = &s;
-        if (!sl) {
-            ctx->slots.push_back({st, nullptr, 0u, 0ull});
-            sl = &ctx->slots.back();
-        }
-        if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 16, 32 or kMaxEv events
-            if (sl->mem) SST_CU(cudaFreeAsync(sl->mem, st));
-            sl->mem = nullptr;
-            sl->cap_events = 0;
-            const uint32_t want = n <= 1 ? 1u : n <= 8 ? 8u : n <= 16 ? 16u : n <= 32 ? 32u : static_cast<uint32_t>(kMaxEv);
-            const ScratchLayout Ln = scratch_layout(ctx, want);
-            SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&blk), Ln.total, ctx->pool, st));
-            SST_CU(cudaMemsetAsync(blk, 0, Ln.o_rec, st));  // ticket counter and states
-            sl->mem = blk;
-            sl->cap_events = want;
-            sl->ticket_base = 0;
-        }
-        blk = sl->mem;
-        cap = sl->cap_events;
-        ticket_base = sl->ticket_base;
-        sl->ticket_base += static_cast<unsigned long long>(total) + grid * wpc;  // every warp draws one ticket too many
+    std::lock_guard<std::mutex> lock(ctx->slot_mu);
+    sst_ctx::Slot *sl = nullptr;
+    for (auto &s : ctx->slots)
+        if (s.stream == st) sl = &s;
+    if (!sl) {
+        ctx->slots.push_back({st, nullptr, 0u, 0ull});
+        sl = &ctx->slots.back();
     }
-    const ScratchLayout L = scratch_layout(ctx, cap);
+    if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 16, 32 or kMaxEv events
+        if (sl->mem) SST_CU(cudaFreeAsync(sl->mem, st));
+        sl->mem = nullptr;
+        sl->cap_events = 0;
+        const uint32_t want = n <= 1 ? 1u : n <= 8 ? 8u : n <= 16 ? 16u : n <= 32 ? 32u : static_cast<uint32_t>(kMaxEv);
+        const ScratchLayout Ln = scratch_layout(ctx, want);
+        uint8_t *mem = nullptr;
+        SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&mem), Ln.total, ctx->pool, st));
+        if (!cu_ok(ctx, cudaMemsetAsync(mem, 0, Ln.o_rec, st))) {  // ticket counter and states
+            cudaFreeAsync(mem, st);
+            return SST_ERR_CUDA;
+        }
+        sl->mem = mem;
+        sl->cap_events = want;
+        sl->ticket_base = 0;
+    }
+    uint8_t *const blk = sl->mem;
+    const ScratchLayout L = scratch_layout(ctx, sl->cap_events);
     KParams kp{};
     kp.calib = ctx->calib;
     kp.chan_info = ctx->chan_info;
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
-    kp.ticket_base = ticket_base;
+    kp.ticket_base = sl->ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
     kp.g_rec = reinterpret_cast<uint32_t *>(blk + L.o_rec);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
@@ -1309,30 +1178,36 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.n_feds = nf;
     kp.n_events = n;
     kp.slot_bytes = ctx->slot_bytes;
-#ifdef SST_PHASE_TIMING
-    kp.phase_clk = g_phase_clk;
-#endif
     for (uint32_t e = 0; e < n; ++e) {
         kp.ev[e].raw = raw[e];
         kp.ev[e].fed_offsets = fed_offsets[e];
         kp.ev[e].out = *outs[e];
         kp.ev[e].packed = packed ? packed[e] : nullptr;
+        kp.ev[e].raw_limit = raw_limit ? std::min(raw_limit[e], ctx->cfg.max_raw_bytes) : ctx->cfg.max_raw_bytes;
     }
     sst_event_kernel<<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
-    SST_CU(cudaGetLastError());
-    if (packed) sst_emit_kernel<true><<<(total + 3) / 4, 128, 0, st>>>(kp);
-    else sst_emit_kernel<false><<<(total + 3) / 4, 128, 0, st>>>(kp);
-    SST_CU(cudaGetLastError());
+    cudaError_t err = cudaGetLastError();
+    if (err == cudaSuccess) {
+        // every warp draws one ticket too many before it stops
+        sl->ticket_base += static_cast<unsigned long long>(total) + grid * wpc;
+        if (packed) sst_emit_kernel<true><<<(total + 3) / 4, 128, 0, st>>>(kp);
+        else sst_emit_kernel<false><<<(total + 3) / 4, 128, 0, st>>>(kp);
+        err = cudaGetLastError();
+    }
+    if (err != cudaSuccess) {
+        // a launch that did not happen must not leave the stream's ticket counter and the host's
+        // copy of it apart: start the stream's scratch over (stream-ordered, like everything else)
+        cu_ok(ctx, err);
+        cudaMemsetAsync(blk, 0, L.o_rec, st);
+        sl->ticket_base = 0;
+        return SST_ERR_CUDA;
+    }
     return SST_OK;
 }
 
 }  // namespace
 
 extern "C" {
-
-#ifdef SST_PHASE_TIMING
-void sst_debug_set_phase_clk(unsigned long long *p) { g_phase_clk = p; }
-#endif
 
 sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (out_ctx) *out_ctx = nullptr;
@@ -1382,8 +1257,13 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
             ctx->smem_bytes = kWarpsPerCta * ctx->warp_stride;
         };
         set_slot(need);
-        if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 static_cast<int>(ctx->smem_bytes)) != cudaSuccess)
+        // The dynamic shared-memory limit is per-FUNCTION state shared by every context of the
+        // process: it is set to the device maximum, never to this context's size, so contexts with
+        // different slot sizes can be used side by side.
+        int smem_optin = 0;
+        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device);
+        if (static_cast<uint32_t>(smem_optin) < ctx->smem_bytes ||
+            cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
             return fail(SST_ERR_CUDA);
         cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->ctas_per_sm, sst_event_kernel, 32 * kWarpsPerCta,
@@ -1392,13 +1272,10 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         size_t avail = 0;
         if (cudaOccupancyAvailableDynamicSMemPerBlock(&avail, sst_event_kernel, ctx->ctas_per_sm, 32 * kWarpsPerCta) ==
                 cudaSuccess && avail > ctx->smem_bytes) {
-            const uint32_t per_warp = static_cast<uint32_t>(std::min<size_t>(avail, 227u * 1024u) / kWarpsPerCta);
+            const uint32_t per_warp = static_cast<uint32_t>(std::min<size_t>(avail, static_cast<size_t>(smem_optin)) / kWarpsPerCta);
             const uint32_t slot = (per_warp - kWarpHdr - kTailPad) & ~15u;
             if (slot > ctx->slot_bytes) {
                 set_slot(slot);
-                if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         static_cast<int>(ctx->smem_bytes)) != cudaSuccess)
-                    return fail(SST_ERR_CUDA);
                 int check = 0;
                 if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel, 32 * kWarpsPerCta,
                                                                   ctx->smem_bytes) != cudaSuccess || check < ctx->ctas_per_sm) {
@@ -1580,7 +1457,7 @@ sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t ra
         const uint8_t *d_raw = blk + o_raw;
         const uint32_t *d_fo = reinterpret_cast<uint32_t *>(blk + o_fo);
         const sst_output *d_out = &d;
-        rc = launch_events(ctx, 1, &d_raw, &d_fo, thr, &d_out, st);
+        rc = launch_events(ctx, 1, &d_raw, &d_fo, thr, &d_out, st, nullptr, &raw_bytes);
     }
     // counts first, then exactly-sized copies of the cluster arrays
     CU(cudaMemcpyAsync(out->dev_status, d.dev_status, SST_ST_WORDS * 4, cudaMemcpyDeviceToHost, st));
@@ -1741,7 +1618,7 @@ sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const 
             po[i] = &v.d;
         }
         CU(copies.run(ck.st));
-        if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st);
+        if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st, nullptr, raw_bytes + e0);
         for (uint32_t i = 0; i < ck.n; ++i) {
             const sst_output &o = outs[e0 + i];
             if (dev[e0 + i].direct) continue;
@@ -1829,7 +1706,7 @@ sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const
             po[i] = &proto;
             pk[i] = d_block[e0 + i];
         }
-        if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st, pk);
+        if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st, pk, raw_bytes + e0);
         for (uint32_t i = 0; i < ck.n; ++i)  // status and count first: they size the one big copy
             CU(cudaMemcpyAsync(results[e0 + i].block, d_block[e0 + i], 64, cudaMemcpyDeviceToHost, ck.st));
         chunks.push_back(ck);
@@ -1890,6 +1767,14 @@ sst_status sst_event_upload(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes
     SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(d_fed_offsets), fo_bytes, ctx->pool, st));
     if (raw_bytes) SST_CU(cudaMemcpyAsync(*d_raw, raw, raw_bytes, cudaMemcpyHostToDevice, st));
     SST_CU(cudaMemcpyAsync(*d_fed_offsets, fed_offsets, fo_bytes, cudaMemcpyHostToDevice, st));
+    return SST_OK;
+}
+
+sst_status sst_event_download(sst_ctx *ctx, void *dst, const void *src, uint64_t bytes, void *stream) {
+    if (!ctx || !dst || !src) return SST_ERR_INVALID_ARG;
+    if (bytes == 0) return SST_OK;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    SST_CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, static_cast<cudaStream_t>(stream)));
     return SST_OK;
 }
 

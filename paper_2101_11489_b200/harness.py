@@ -112,6 +112,70 @@ class Detector:
         B.sst_unpack_cluster(self.ctx, d_raw, d_fo, thresholds, outputs.out, st.cuda_stream)
 
 
+_FIELDS = (("strip_adc", np.uint8, "N"), ("chan_off", np.uint32, "C"), ("chan_len", np.uint16, "C"),
+           ("seed_idx", np.uint32, "S"), ("cl_module", np.uint32, "K"), ("cl_first", np.uint16, "K"),
+           ("cl_width", np.uint16, "K"), ("cl_charge", np.int32, "K"), ("cl_bary", np.float32, "K"),
+           ("cl_adc_off", np.uint32, "K"), ("cl_snr", np.float32, "K"), ("cl_adc", np.uint8, "A"),
+           ("n_clusters", np.uint32, 1), ("dev_status", np.uint32, B.ST_WORDS))
+
+
+class PooledOutputs:
+    """The output arrays of one event carved out of ONE block of the library's stream-ordered pool
+    (sst_event_alloc; PAPER.md:41 uses a caching allocator for the same purpose), read back with
+    sst_event_download."""
+
+    def __init__(self, det: "Detector", cap_clusters: int, cap_adc: int, stream: int = 0, dense: bool = True,
+                 chan_map: bool = False, seeds: bool = False, snr: bool = False, cap_seeds: Optional[int] = None):
+        self.det, self.cap_clusters, self.cap_adc = det, int(cap_clusters), int(cap_adc)
+        self.cap_seeds = (det.n_strips if cap_seeds is None else int(cap_seeds)) if seeds else 0
+        dims = {"N": det.n_strips, "C": det.n_feds * B.N_CHAN, "S": max(self.cap_seeds, 1),
+                "K": max(self.cap_clusters, 1), "A": max(self.cap_adc, 1)}
+        want = {"strip_adc": dense, "chan_off": chan_map, "chan_len": chan_map, "seed_idx": seeds, "cl_snr": snr}
+        self.layout, off = {}, 0
+        for name, dt, dim in _FIELDS:
+            if not want.get(name, True):
+                continue
+            n = dims[dim] if isinstance(dim, str) else dim
+            self.layout[name] = (off, np.dtype(dt), n)
+            off += (n * np.dtype(dt).itemsize + 255) // 256 * 256
+        self.nbytes = off
+        self.base = B.sst_event_alloc(det.ctx, self.nbytes, stream)
+        self.out = B.make_output(cap_clusters=self.cap_clusters, cap_adc=self.cap_adc, cap_seeds=self.cap_seeds,
+                                 **{k: self.base + v[0] for k, v in self.layout.items()})
+
+    def numpy(self, stream: int = 0, skip: Sequence[str] = ()) -> Dict[str, np.ndarray]:
+        """Downloads the block on `stream`, synchronises, and trims the arrays to the counts the
+        device reported (same dictionary as EventOutputs.numpy() after unsigned_view)."""
+        torch = self.det.torch
+        host = torch.empty(self.nbytes, dtype=torch.uint8).pin_memory()
+        lo = 0   # the dense array is the block's first region: skipping it shortens the copy
+        if "strip_adc" in skip and "strip_adc" in self.layout:
+            lo = (self.layout["strip_adc"][2] + 255) // 256 * 256
+        B.sst_event_download(self.det.ctx, host.data_ptr() + lo, self.base + lo, self.nbytes - lo, stream)
+        torch.cuda.synchronize(self.det.device)
+        a = host.numpy()
+        t = {k: a[o:o + n * dt.itemsize].view(dt) for k, (o, dt, n) in self.layout.items()}
+        st = t["dev_status"]
+        k = int(t["n_clusters"][0])
+        res = {"n_clusters": k, "status": st}
+        for name in ("cl_module", "cl_first", "cl_width", "cl_charge", "cl_bary", "cl_adc_off", "cl_snr"):
+            if name in t:
+                res[name] = t[name][:k]
+        na = int(res["cl_adc_off"][-1]) + int(res["cl_width"][-1]) if k else 0
+        res["cl_adc"] = t["cl_adc"][:na]
+        for name in ("strip_adc", "chan_off", "chan_len"):
+            if name in t and name not in skip:
+                res[name] = t[name]
+        if "seed_idx" in t:
+            res["seed_idx"] = t["seed_idx"][:min(int(st[B.ST_N_SEEDS]), self.cap_seeds)]
+        return res
+
+    def free(self, stream: int = 0):
+        if self.base:
+            B.sst_event_free(self.det.ctx, self.base, stream)
+            self.base = 0
+
+
 def unsigned_view(res: Dict[str, np.ndarray]) -> Dict[str, np.ndarray]:
     """torch has no uint16/uint32 tensors everywhere; reinterpret the signed storage."""
     conv = {"cl_module": np.uint32, "cl_first": np.uint16, "cl_width": np.uint16, "cl_adc_off": np.uint32,

@@ -81,3 +81,18 @@ def worked_case(doc, case) -> Case:
     return build_case(case.get("strips", {}), d["n_feds"], d["module_sizes"], d["noise"], d["gain"],
                       case.get("gain"), None, case.get("bad", ()), case.get("full_channels"),
                       d["thresholds"])
+
+
+def move_fed_padding(raw: np.ndarray, fo: np.ndarray, f: int, used: int, k: int):
+    """FED f loses k of its trailing pad bytes, FED f+1 gains them behind its last channel: both
+    keep their content, FED f gets an unaligned size and FED f+1 an unaligned start (the non-TMA
+    path of the kernel).  `used` = bytes of FED f up to the end of its channel 95."""
+    fo = fo.astype(np.int64)
+    assert 0 < k <= fo[f + 1] - fo[f] - used and f + 2 < fo.size
+    a = raw[:fo[f + 1] - k]
+    b = raw[fo[f + 1]:fo[f + 2]]
+    out = np.concatenate([a, b, np.zeros(k, np.uint8), raw[fo[f + 2]:]])
+    fo2 = fo.copy()
+    fo2[f + 1] -= k
+    assert out.size == raw.size
+    return out, fo2.astype(np.uint32)

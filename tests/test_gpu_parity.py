@@ -166,12 +166,16 @@ def test_hand_built_and_malformed_raw(H, oracle):
 def test_bad_fed_offsets(H, oracle):
     cfg, cal, evs = synth.make_config(0, n_feds=3)
     ev = evs[0]
-    for mutate in ("end_lt_start", "beyond_buffer", "truncated"):
+    for mutate in ("end_lt_start", "beyond_buffer", "truncated", "steps_back", "overlap"):
         fo = ev.fed_offsets.copy()
         if mutate == "end_lt_start":
             fo[1], fo[2] = fo[2], fo[1]
         elif mutate == "beyond_buffer":
             fo[3] = ev.raw.size + 4096
+        elif mutate == "steps_back":            # reading s3c: [0, a, 0, a] -- FED 2 would re-read FED 0
+            fo[2], fo[3] = 0, fo[1]
+        elif mutate == "overlap":               # FED 2 starts inside FED 0
+            fo = np.array([0, ev.fed_offsets[1], ev.fed_offsets[1] - 32, ev.fed_offsets[3]], np.uint32)
         else:
             fo[2] = fo[1] + 160
         g = gpu_run(H, 3, ev.raw, fo, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5),
@@ -412,10 +416,11 @@ def test_batched_entry_point_matches_single_event(H, oracle):
         det.close()
 
 
-def test_full_size_batch_in_the_bench_configuration(H, oracle):
-    """BASELINE.json config 3 at full size in the launch configuration bench.py times: 440 FEDs,
-    events over 8 streams through sst_unpack_cluster_batch (one FED-major launch), the
-    shared-memory slot sized by fed_strips_hint as bench.py does; every event compared in full."""
+def test_full_size_batch_one_ticket_per_warp(H, oracle):
+    """BASELINE.json config 3 at full size with 10 events: 440 FEDs, events over 8 streams through
+    sst_unpack_cluster_batch (one FED-major launch of 4400 tickets, at most one per resident warp),
+    the shared-memory slot sized by fed_strips_hint as bench.py does; every event compared in full.
+    (The 64-event shape bench.py times is test_config3_64_events_440_feds_in_the_timed_shape.)"""
     import torch
     from paper_2101_11489_b200 import binding as B
     n_ev = 10
@@ -534,3 +539,195 @@ def test_densest_possible_clusters(H, oracle):
     r = oracle.run(raw, fo, n_feds, gain, noise, bad, cm, (2, 3, 5), cap_clusters=cc, cap_adc=ca)
     compare(g, r)
     assert g["n_clusters"] == 2 * 12288 + 1 and g["n_clusters"] > raw.size // 3
+
+
+# ------------------------------------------------------------------ the timed launch shape
+def _tickets_and_warps(info, n_events, n_feds):
+    return n_events * n_feds, info["sm_count"] * info["ctas_per_sm"] * (info["threads"] // 32)
+
+
+def test_config3_64_events_440_feds_in_the_timed_shape(H, oracle):
+    """BASELINE.json config 3 EXACTLY as bench.py times it: 64 events x 440 FEDs over 8 streams in
+    one sst_unpack_cluster_batch call, pooled output blocks, fed_strips_hint from the data.  A warp
+    takes ~6 tickets here (slot reuse, mbarrier parity flips, proxy fences between tickets).  The
+    call runs twice in a row; then EVERY output of EVERY event is compared with the oracle."""
+    import bench
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    n_ev, nf = 64, 440
+    calib = synth.make_calibration(nf, synth.CONFIGS[3].bad_frac)
+    events = bench.generate_events(3, nf, list(range(1, n_ev + 1)), calib)
+    mrb = (max(int(e[0].size) for e in events) + 4095) // 4096 * 4096
+    hint = int(1.05 * max(int(e[2]["max_fed_strips"]) for e in events)) + 16
+    det = H.Detector(nf, calib.gain, calib.noise, calib.bad, calib.chan_module, max_raw_bytes=mrb,
+                     max_events_in_flight=8, fed_strips_hint=hint)
+    try:
+        tickets, warps = _tickets_and_warps(det.info(), n_ev, nf)
+        assert tickets > 4 * warps, "the launch must give every warp several tickets"
+        streams = [torch.cuda.Stream() for _ in range(8)]
+        d_in = [det.upload_raw(e[0], e[1]) for e in events]
+        outs = [H.PooledOutputs(det, mrb // 3 + 1, mrb, streams[i % 8].cuda_stream, dense=True, chan_map=True,
+                                seeds=True, snr=True, cap_seeds=mrb) for i in range(n_ev)]
+        batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs],
+                        [s.cuda_stream for s in streams])
+        torch.cuda.synchronize()
+        B.sst_unpack_cluster_batch(det.ctx, batch)
+        B.sst_unpack_cluster_batch(det.ctx, batch)
+        torch.cuda.synchronize()
+        for i, (e, o) in enumerate(zip(events, outs)):
+            r = oracle.run(e[0], e[1], nf, calib.gain, calib.noise, calib.bad, calib.chan_module, (2, 3, 5))
+            compare(o.numpy(streams[i % 8].cuda_stream), r)
+            o.free(streams[i % 8].cuda_stream)
+    finally:
+        det.close()
+
+
+def test_several_tickets_per_warp_with_irregular_feds_in_the_stream(H, oracle):
+    """64 events x 80 FEDs = 5120 tickets on at most 4736 resident warps: warps loop over tickets.
+    In the middle of the ticket stream sit a FED whose clusters outgrow the shared-memory record
+    area (600 isolated single-strip clusters in a 2 KB payload: the redo path), two FEDs with
+    unaligned offsets (the non-TMA path) and a FED with a malformed channel."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    n_ev, nf = 64, 80
+    cfg, cal, evs = synth.make_config(3, n_feds=nf, event_seeds=range(1, n_ev + 1))
+    raws, fos = [e.raw for e in evs], [e.fed_offsets for e in evs]
+    # event 20, FED 40: isolated single strips, every one its own run and its own cluster
+    z = evs[20].z.copy()
+    z[40 * synth.FED_STRIPS:41 * synth.FED_STRIPS] = 0
+    z[40 * synth.FED_STRIPS:40 * synth.FED_STRIPS + 1200:2] = 40
+    raws[20], fos[20] = synth.encode_dense(z, nf)
+    # event 41, FEDs 30/31: unaligned size / unaligned start
+    off, ln, _, _ = oracle.unpack(raws[41], fos[41], nf)
+    f_un = next(f for f in range(30, 60)
+                if (int(off[f * 96 + 95]) + int(ln[f * 96 + 95]) - int(fos[41][f])) % 16 not in (0, 15))
+    used = int(off[f_un * 96 + 95]) + int(ln[f_un * 96 + 95]) - int(fos[41][f_un])
+    raws[41], fos[41] = cases.move_fed_padding(raws[41], fos[41], f_un, used, 1)
+    # event 7, FED 55: channel 3 gets a run that passes strip 255 (malformed: contributes nothing)
+    r7 = raws[7].copy()
+    off7, ln7, _, _ = oracle.unpack(r7, fos[7], nf)
+    c_bad = next(c for c in range(55 * 96, 56 * 96) if ln7[c] >= 3)
+    r7[off7[c_bad]] = 255
+    r7[off7[c_bad] + 1] = 2
+    raws[7] = r7
+    want = [oracle.run(raws[i], fos[i], nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5)) for i in range(n_ev)]
+    assert want[7].status[1] >= 1 and want[20].n_clusters > 600
+    mrb = (max(int(r.size) for r in raws) + 4095) // 4096 * 4096
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        tickets, warps = _tickets_and_warps(det.info(), n_ev, nf)
+        assert tickets > warps, "some warps must take more than one ticket"
+        streams = [torch.cuda.Stream() for _ in range(8)]
+        d_in = [det.upload_raw(raws[i], fos[i]) for i in range(n_ev)]
+        outs = [det.alloc_outputs(mrb // 2 + 1, mrb, chan_map=True, seeds=True, snr=True, cap_seeds=mrb) for _ in range(n_ev)]
+        batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs],
+                        [s.cuda_stream for s in streams])
+        torch.cuda.synchronize()
+        for _ in range(3):
+            B.sst_unpack_cluster_batch(det.ctx, batch)
+        torch.cuda.synchronize()
+        for o, r in zip(outs, want):
+            compare(H.unsigned_view(o.numpy()), r)
+    finally:
+        det.close()
+
+
+def test_strip_tests_exhaustive_on_gpu(H, oracle):
+    """The float32 + FMA form of `adc >= t * noise` (reading s5) against exact rational
+    arithmetic: all 255 ADC values x every threshold of BASELINE.json's three triples x the noise
+    values within 3 float32 steps of adc / t (where fl(t * noise) rounds up, down or not at all)."""
+    from fractions import Fraction
+    ts = [1.5, 2.0, 2.5, 3.0, 5.0]
+    n = synth.FED_STRIPS
+    z = np.zeros(n, np.uint8)
+    noise = np.full(n, 1000.0, np.float32)
+    pos = 0
+    placed = []
+    for t in ts:
+        for a in range(1, 256):
+            n0 = np.float32(a / t)
+            vals = [n0]
+            for _ in range(3):
+                vals.append(np.nextafter(vals[-1], np.float32(np.inf)))
+            lo = n0
+            for _ in range(3):
+                lo = np.nextafter(lo, np.float32(0))
+                vals.append(lo)
+            for v in vals:
+                if pos % 256 > 253:          # keep a gap at channel ends
+                    pos += 256 - pos % 256
+                z[pos], noise[pos] = a, v
+                placed.append((pos, a, float(v)))
+                pos += 2
+    assert pos <= n and len(placed) == 255 * 5 * 7
+    raw, fo = synth.encode_dense(z, 1)
+    gain, bad = np.ones(n, np.float32), np.zeros(n, np.uint8)
+    cm = cases.module_map_from_sizes(1, (2, 3))
+    det = H.Detector(1, gain, noise, bad, cm, max_raw_bytes=int(raw.size))
+    try:
+        for thr in [(t, t, 1e-3) for t in ts] + [(2, 3, 5), (1.5, 2.5, 4), (3, 5, 8)]:
+            g = gpu_run(H, 1, raw, fo, None, None, None, None, thr, det=det, cap_clusters=int(raw.size), cap_adc=int(raw.size))
+            r = oracle.run(raw, fo, 1, gain, noise, bad, cm, thr, cap_clusters=int(raw.size), cap_adc=int(raw.size))
+            compare(g, r)
+            t_seed = Fraction(float(np.float32(thr[1])))
+            t_ch = Fraction(float(np.float32(thr[0])))
+            exact = [p for p, a, v in placed if Fraction(a) >= t_seed * Fraction(v) and Fraction(a) >= t_ch * Fraction(v)]
+            assert np.array_equal(g["seed_idx"], np.asarray(exact, np.uint32))
+    finally:
+        det.close()
+
+
+def test_two_contexts_with_different_slot_sizes_alternate(H, oracle):
+    """The dynamic shared-memory limit is per-function state: a second context with another slot
+    size must not break launches of the first (alternating calls, both checked every time)."""
+    cfg, cal, evs = synth.make_config(0, n_feds=6)
+    ev = evs[0]
+    r = oracle.run(ev.raw, ev.fed_offsets, 6, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+    big = H.Detector(6, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=6 * 40000, fed_strips_hint=20000)
+    small = H.Detector(6, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
+    try:
+        assert big.info()["smem_bytes"] != small.info()["smem_bytes"]
+        for det in (big, small, big, small, big):
+            compare(gpu_run(H, 6, ev.raw, ev.fed_offsets, None, None, None, None, (2, 3, 5), det=det), r)
+    finally:
+        big.close()
+        small.close()
+
+
+def test_two_host_threads_on_distinct_streams(H, oracle):
+    """sst.h: concurrent sst_unpack_cluster calls from different host threads on different streams
+    are allowed after sst_upload_calib."""
+    import threading
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf = 12
+    cfg, cal, evs = synth.make_config(3, n_feds=nf, event_seeds=range(1, 9))
+    want = [oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5)) for e in evs]
+    mrb = max(int(e.raw.size) for e in evs)
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        d_in = [det.upload_raw(e.raw, e.fed_offsets) for e in evs]
+        outs = [det.alloc_outputs(mrb // 3 + 1, mrb, chan_map=True, seeds=True, snr=True) for _ in evs]
+        streams = [torch.cuda.Stream() for _ in range(2)]
+        torch.cuda.synchronize()
+        errors = []
+
+        def worker(tid):
+            try:
+                for rep in range(25):
+                    for i in range(tid, len(evs), 2):
+                        B.sst_unpack_cluster(det.ctx, d_in[i][0], d_in[i][1], (2, 3, 5), outs[i].out, streams[tid].cuda_stream)
+            except Exception as exc:     # noqa: BLE001
+                errors.append(exc)
+
+        th = [threading.Thread(target=worker, args=(t,)) for t in range(2)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        torch.cuda.synchronize()
+        assert not errors, errors
+        for o, r in zip(outs, want):
+            compare(H.unsigned_view(o.numpy()), r)
+    finally:
+        det.close()

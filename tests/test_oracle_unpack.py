@@ -134,6 +134,27 @@ def test_truncated_fed_and_bad_offsets(oracle):
     assert not adc.any() and st[4] == 1
 
 
+def test_offsets_that_step_back_are_flagged_and_empty(oracle):
+    """Reading s3c: a FED whose start lies below an earlier entry of fed_offsets is flagged and
+    empty, so decoded FEDs never overlap.  Offsets [0, n, 0, n]: FED 0 decodes, FED 1 has end <
+    start, FED 2 would re-read FED 0's bytes and is refused."""
+    good = synth.channel_bytes([(7, [33])])
+    raw, fo = synth.assemble_feds([fed_with({0: good})])
+    n = int(fo[1])
+    off, ln, adc, st = oracle.unpack(raw, np.array([0, n, 0, n], np.uint32), 3)
+    a = adc.reshape(3 * 96, 256)
+    assert a[0, 7] == 33 and not a[96:].any()
+    assert st[4] == 2 and st[0] & oracle.FLAG_OVERRUN
+    assert np.all(off[96:192] == n) and np.all(off[192:] == 0) and not ln[96:].any()   # (start as given, 0)
+    # [0, n, n/2.., 2n] with the middle FED starting inside FED 0: refused; a later FED that starts
+    # at or above every earlier offset is decoded again
+    raw2 = np.concatenate([raw, raw])
+    off, ln, adc, st = oracle.unpack(raw2, np.array([0, n, 16, n, 2 * n], np.uint32), 4)
+    a = adc.reshape(4 * 96, 256)
+    assert a[0, 7] == 33 and not a[96:3 * 96].any() and a[3 * 96, 7] == 33
+    assert st[4] == 2
+
+
 def test_worked_example_dense_holds_bad_strips(oracle):
     doc = cases.load_worked_examples()
     w5 = next(c for c in doc["cases"] if c["id"] == "W5")
