@@ -75,9 +75,8 @@ constexpr int kMaxEv = SST_MAXEV;                   // events per launch
 constexpr int kWarpsPerCta = SST_WPC;       // warps (= FEDs in flight) per CTA, each with its own slot
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
-constexpr uint32_t kTabBytes = kChan * 4 + kChan * 2;  // channel map of the FED, at the slot's end
+constexpr uint32_t kTabBytes = ((kChan + 1) * 4 + kChan * 2 + 15) & ~15;  // channel map of the FED, at the slot's end
 constexpr uint32_t kWarpHdr = 16;                      // mbarrier
-constexpr uint32_t kWin = 2048;                       // strips per step of the dense SoA assembly
 constexpr uint32_t kSlabAhead = SST_SLAB_AHEAD;        // FEDs between a calibration prefetch and its use
 constexpr uint32_t kTailPad = 16;                      // readable bytes behind the slot (pass 2)
 
@@ -98,17 +97,18 @@ struct KParams {
     const float2 *calib;     // {noise (+inf at bad strips), gain} per strip
     const uint2 *chan_info;  // {module id, first channel | end channel << 8 of the module}
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
+    uint32_t *fed_cand;             // [kMaxEv][n_feds] staged candidates (clusters before the cluster test)
     unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+warps)
     unsigned long long ticket_base;
     // global scratch of the slow path, one slice set per event
-    uint32_t *g_rec;
+    uint16_t *g_rec;
     uint16_t *g_strip;
     uint8_t *g_adc;
-    uint32_t *g_mask;  // 4 arrays of g_mwords per event
+    uint32_t *g_mask;  // 5 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
-    uint4 *s_rec;     // {module, first | width << 16, charge, barycenter}
-    uint32_t *s_off;  // offset of the cluster's ADCs inside its FED
+    uint4 *s_rec;     // per candidate {module, first | width << 16 | accepted << 31, charge, barycenter}
+    uint32_t *s_off;  // list entry of the candidate's first strip (its ADCs are s_adc[entry .. +width))
     float *s_snr;
     uint8_t *s_adc;
     uint16_t *s_seed;
@@ -229,41 +229,6 @@ __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, int lane) {
     }
     return v;
 }
-// Cluster acceptance, the defining form (reading s15): Q^2 >= t_cl^2 * n2 with n2 the
-// double sum of noise^2 over the candidate's strips taken strictly left to right (noise^2 is
-// exact in double, so the fused multiply-add rounds exactly like a separate multiply and add).
-// The noise is gathered again from the calibration: this runs only for candidates that cross a
-// chunk boundary of the sweep and land within rounding distance of the threshold, and for the
-// optional S/N output.
-__device__ __noinline__ double n2_sequential(const float2 *cal, const uint16_t *strip_l, uint32_t head, uint32_t w) {
-    double n2 = 0.0;
-#pragma unroll 1
-    for (uint32_t i = 0; i < w; ++i) {
-        const double d = static_cast<double>(__ldg(&cal[strip_l[head + i] & 0x7fffu].x));
-        n2 = __fma_rn(d, d, n2);
-    }
-    return n2;
-}
-__device__ __forceinline__ bool accept_exact(const float2 *cal, const uint16_t *strip_l, uint32_t head, uint32_t w,
-                                             uint32_t Q, double tcl2) {
-    const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
-    return lhs >= __dmul_rn(tcl2, n2_sequential(cal, strip_l, head, w));
-}
-// Mask bits of an accepted cluster [hd, end]: its head in mH, its entries in mA.
-__device__ __forceinline__ void mark_cluster(uint32_t *mH, uint32_t *mA, uint32_t hd, uint32_t end) {
-    const uint32_t wh = hd >> 5, we = end >> 5;
-    const uint32_t mh = kFull << (hd & 31u), me = kFull >> (31u - (end & 31u));
-    atomicOr(&mH[wh], 1u << (hd & 31u));
-    if (wh == we) {  // nearly always
-        atomicOr(&mA[wh], mh & me);
-    } else {
-        atomicOr(&mA[wh], mh);
-#pragma unroll 1
-        for (uint32_t w = wh + 1u; w < we; ++w) atomicOr(&mA[w], kFull);
-        atomicOr(&mA[we], me);
-    }
-}
-
 // ------------------------------------------------------------------------------ raw payload
 // a1, generic path (payload not staged): the channel-length chain of one FED, checked as it goes.
 __device__ __noinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_size, bool over, uint32_t *chan_off,
@@ -292,60 +257,65 @@ __device__ __noinline__ bool walk_chain_checked(const uint8_t *rp, uint32_t fed_
 
 // a1, staged payload: the same chain walked speculatively by one lane -- no bounds checks inside
 // the serial loop (reads are clamped into the slot), the 96 results are validated in parallel.
-__device__ __forceinline__ void walk_chain_speculative(const uint8_t *stage, uint32_t clamp, uint32_t *chan_off) {
-    uint32_t pos = 0;
+// It works on 32-bit shared-memory addresses: per channel one min, two byte loads, a multiply-add,
+// an add and a store.  tab[c] = stage_addr + offset of the first run byte of channel c, c = 0..96
+// (the lengths are differences).
+__device__ __forceinline__ void walk_chain_speculative(uint32_t stage_addr, uint32_t clamp_addr, uint32_t tab_addr) {
+    uint32_t pos = stage_addr + 2u;
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(tab_addr), "r"(pos) : "memory");
 #pragma unroll 8
     for (int c = 0; c < kChan; ++c) {
-        const uint32_t a = min(pos, clamp);
-        pos += 2u + (stage[a] | (static_cast<uint32_t>(stage[a + 1]) << 8));
-        chan_off[c + 1] = pos + 2u;  // chan_off[0] = 2; the lengths are differences
+        const uint32_t a = min(pos, clamp_addr);
+        uint32_t lo, hi;
+        asm volatile("ld.shared.u8 %0, [%1+-2];" : "=r"(lo) : "r"(a) : "memory");
+        asm volatile("ld.shared.u8 %0, [%1+-1];" : "=r"(hi) : "r"(a) : "memory");
+        pos = pos + 2u + (hi * 256u + lo);
+        asm volatile("st.shared.u32 [%0], %1;" ::"r"(tab_addr + 4u * static_cast<uint32_t>(c + 1)), "r"(pos) : "memory");
     }
 }
 
 struct FedCtx {
     uint32_t ticket, ev, f;
-    uint32_t fo0;                 // the FED's start offset as given (reported in chan_off)
+    uint32_t fo0;                  // the FED's start offset as given (reported in chan_off)
     uint32_t fed_start, fed_size;  // what is read: [fed_start, +fed_size), empty for a bad FED
     uint32_t overrun, n_malformed;
-    uint32_t P;
-    uint32_t off[3], len[3], base[3];  // of channels lane, lane+32, lane+64
-    uint32_t opens;                    // bit k: channel lane+32k opens a module
+    uint32_t P, R;                 // present strips (list entries) and runs of the FED
+    uint32_t off[3], len[3];       // of channels lane, lane+32, lane+64
+    uint32_t ebase[3];             // first list entry of those channels
+    uint32_t opens;                // bit k: channel lane+32k opens a module
 };
 
 // a2 pass 1: a lane validates the run lists of its three channels (reading s2b) and
-// counts their strips; the three cursors advance in one loop, so the three dependent chains of
-// byte loads overlap.  A malformed channel contributes no strips.
-__device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_t (&cnt)[3]) {
+// counts their strips and runs, one channel after the other.  The loop body has no exit: a
+// malformed channel is walked to its end like any other (every step advances by >= 3 bytes) and
+// recognised afterwards.  A malformed channel contributes no strips (its length is zeroed).
+__device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_t (&cnt)[3], uint32_t (&runs)[3]) {
     uint32_t o0 = c.off[0], o1 = c.off[1], o2 = c.off[2], l0 = c.len[0], l1 = c.len[1], l2 = c.len[2];
-    uint32_t n0 = 0, n1 = 0, n2 = 0, okbits = 0;
+    uint32_t n0 = 0, n1 = 0, n2 = 0, r0 = 0, r1 = 0, r2 = 0, okbits = 0;
 #pragma unroll 1
-    for (int k = 0; k < 3; ++k) {  // one channel after the other, the register sets rotate
-        uint32_t q = o0, nf = 0, n = 0;
+    for (int k = 0; k < 3; ++k) {  // the register sets rotate
+        uint32_t q = o0, nf = 0, r = 0, n = 0;
         const uint32_t qe = o0 + l0;
-        bool ok = true;
+        bool bad = false;
 #pragma unroll 1
-        while (q < qe) {
-            bool bad = q + 2 > qe;
-            uint32_t first = 0, len = 0;
-            if (!bad) {
-                first = rp[q];
-                len = rp[q + 1];
-                if (len == 0) len = 256;  // reading s2
-                bad = first < nf || first + len > kStrip || q + 2 + len > qe;
-            }
-            if (bad) {
-                ok = false;
-                break;
-            }
+        while (q + 2u <= qe) {
+            const uint32_t first = rp[q];
+            uint32_t len = rp[q + 1];
+            if (len == 0) len = 256;  // reading s2
+            bad = bad || first < nf || first + len > static_cast<uint32_t>(kStrip);
             nf = first + len;
-            q += 2 + len;
+            q += 2u + len;
             n += len;
+            ++r;
         }
+        const bool ok = !bad && q == qe;  // truncated header, or run bytes passing the payload end: q != qe
         o0 = o1; o1 = o2; l0 = l1; l1 = l2;
         n0 = n1; n1 = n2; n2 = ok ? n : 0u;
+        r0 = r1; r1 = r2; r2 = ok ? r : 0u;
         okbits = (okbits >> 1) | (ok ? 4u : 0u);
     }
     cnt[0] = n0; cnt[1] = n1; cnt[2] = n2;
+    runs[0] = r0; runs[1] = r1; runs[2] = r2;
     c.n_malformed = 0;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -355,145 +325,184 @@ __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_
     }
 }
 
+// Seeds smeared towards lower entries along the links, inside one 32-entry word: bit e of the
+// result is set iff some seed bit s >= e is set with link bits e+1 .. s all set (link bit i:
+// entry i continues the candidate of entry i-1).  Five doubling steps.
+__device__ __forceinline__ uint32_t smear_down(uint32_t x, uint32_t g) {
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+        x |= (x & g) >> s;
+        g &= g << s;
+    }
+    return x;
+}
+
 // ------------------------------------------------------------------------------ lists -> clusters
-// Everything after pass 1, on the FED's lists of present strips, by one warp.  kFast: lists, masks
-// and cluster records live in the warp's shared-memory slot and the payload is staged there; else
-// they live in this FED's slice of the global scratch and rp is a generic pointer.  Returns false
-// (fast path only) when the cluster records outgrow the slot: the FED is then redone on the slow
-// path (nothing has been published and every output written so far is rewritten identically).
+// Everything after pass 1, by one warp, data-parallel over the FED's list of present strips (the
+// structure of arrays of PAPER.md:31: one entry per recorded strip).  kFast: lists, masks and the
+// candidate list live in the warp's shared-memory slot and the payload is staged there (the ADC
+// list is the payload squeezed in place); else they live in this FED's slice of the global
+// scratch and rp is whatever holds the payload.  Returns false (fast path only) when the
+// candidate list outgrows the slot: the FED is then redone on the slow path (nothing has been
+// published and every output written so far is rewritten identically).
 template <bool kFast>
 __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, const FedCtx &c,
                                           const int lane, uint32_t &next_ticket) {
     const uint32_t f = c.f, P = c.P;
     const EventDesc &E = p.ev[c.ev];
     const sst_output &o = E.out;
-    const uint32_t nw = (P + 31) >> 5;  // mask words in use
-    const uint32_t lt = (1u << lane) - 1u;
+    const uint32_t nw = (P + 31) >> 5;  // mask words in use; every mask has one more (zero) word
+    const uint32_t lt = (1u << lane) - 1u, le = lt | (1u << lane);
 
-    uint16_t *strip_l;
+    // per-channel constant of the payload address of an entry: src(e) = e + 2 * run(e) + ktab[channel]
+    uint32_t *const ktab = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
+    uint16_t *strip_l, *rec;
     uint8_t *adc_l;
-    uint32_t *mS, *mA, *mH, *mP, *rec;
-    uint32_t rec_cap;  // cluster records besides the end sentinel
-    uint8_t *window;   // kWin bytes of shared memory for the dense SoA, free between pass 2 and the sweep
+    uint32_t *mR, *mA, *mL, *mS, *mX;
+    uint32_t rec_cap;      // seeded candidates the list can hold
+    uint8_t *window = nullptr;  // shared memory for the dense SoA assembly, free once the lists are complete
+    uint32_t kw = 0;            // its size in units of 512 strips
     if (kFast) {
-        // [0, A): the payload, and once the lists are built the masks and the cluster records
-        const uint32_t A = (c.fed_size + 15u) & ~15u;
+        // [0, A): the payload; the ADC list takes its place ([0, P)), the rest holds the window and
+        // then the candidate list.  [A, A + 2P): strip ids.  Behind: five masks.
+        const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (P + 15u) & ~15u;
+        adc_l = slot;
         strip_l = reinterpret_cast<uint16_t *>(slot + A);
-        adc_l = slot + A + 2u * P;
-        // masks behind the lists when there is room (the records then get all of the payload's
-        // place), else in front of the records
-        const uint32_t tail = (A + 3u * P + 15u) & ~15u, mbytes = 16u * (nw + 2);
-        if (tail + mbytes <= p.slot_bytes) {
-            mS = reinterpret_cast<uint32_t *>(slot + tail);
-            rec = reinterpret_cast<uint32_t *>(slot);
-            rec_cap = A / 4u - 1u;
-        } else {
-            mS = reinterpret_cast<uint32_t *>(slot);
-            rec = mS + 4u * (nw + 2);
-            rec_cap = (A - mbytes) / 4u - 1u;
+        const uint32_t tail = (A + 2u * P + 15u) & ~15u;
+        mR = reinterpret_cast<uint32_t *>(slot + tail);
+        mA = mR + (nw + 1);
+        mL = mA + (nw + 1);
+        mS = mL + (nw + 1);
+        mX = mS + (nw + 1);
+        const uint32_t tail2 = (tail + 20u * (nw + 1) + 15u) & ~15u;
+        rec = reinterpret_cast<uint16_t *>(slot + P16);
+        rec_cap = (A - P16) / 2u;
+        kw = min(4u, (A - P16) / 512u);
+        if (kw) {
+            window = slot + P16;
+        } else {  // a nearly empty FED: the caller made sure there is room behind the masks
+            kw = 4;
+            window = slot + tail2;
         }
-        mA = mS + (nw + 2);
-        mH = mA + (nw + 2);
-        mP = mH + (nw + 2);
-        window = A >= kWin ? slot : slot + ((A + 3u * P + 15u) & ~15u);
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
         strip_l = p.g_strip + eb + slice;
         adc_l = p.g_adc + eb + slice;
         rec = p.g_rec + eb + slice;
-        mS = p.g_mask + static_cast<size_t>(c.ev) * 4u * p.g_mwords + (slice >> 5) + 4u * f;
-        mA = mS + p.g_mwords;
-        mH = mA + p.g_mwords;
-        mP = mH + p.g_mwords;
+        mR = p.g_mask + static_cast<size_t>(c.ev) * 5u * p.g_mwords + (slice >> 5) + 4u * f;
+        mA = mR + p.g_mwords;
+        mL = mA + p.g_mwords;
+        mS = mL + p.g_mwords;
+        mX = mS + p.g_mwords;
         rec_cap = 0xffffffffu;
-        window = slot;
+        // the slot is free up to the channel table unless the payload is staged in it
+        if (rp != slot) {
+            window = slot;
+            kw = 4;
+        } else if (((c.fed_size + 15u) & ~15u) + 2048u + kTabBytes <= p.slot_bytes) {
+            window = slot + ((c.fed_size + 15u) & ~15u);
+            kw = 4;
+        }
     }
     const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
-
     uint8_t *const dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips : nullptr;
-
-    // ---------------------------------------------------------------- a2 pass 2: lane per channel
-    // writes {strip, adc} in ascending strip order; bit 15 of a strip id marks strip 0 of a channel
-    // that opens a module (nothing links across it).  Three cursors per lane as in pass 1.
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
+
+    // ---------------------------------------------------------------- a2 pass 2: the run starts
+    // Lane per channel again, headers only: the first strip of every run gets its list entry
+    // (strip id; bit 15 marks strip 0 of a channel that opens a module: nothing links across it)
+    // and a bit in the run-start mask.  Everything per strip is left to the expansion below.
+#pragma unroll 1
+    for (uint32_t w = lane; w < nw + 1; w += 32) mR[w] = 0;
+    __syncwarp();
     {
-        // one channel after the other (the three register sets rotate): a third of the code of the
-        // three-cursor form, and the instruction cache is what this kernel is short of
         uint32_t o0 = c.off[0], o1 = c.off[1], o2 = c.off[2], l0 = c.len[0], l1 = c.len[1], l2 = c.len[2];
-        uint32_t b0_ = c.base[0], b1_ = c.base[1], b2_ = c.base[2], opens = c.opens;
+        uint32_t b0 = c.ebase[0], b1 = c.ebase[1], b2 = c.ebase[2], opens = c.opens;
 #pragma unroll 1
         for (int k = 0; k < 3; ++k) {
-            uint32_t qq = o0, ee = b0_;
+            uint32_t q = o0, e = b0;
             const uint32_t qe = o0 + l0;
             const uint32_t g0 = static_cast<uint32_t>(lane + 32 * k) * kStrip, open_bit = (opens & 1u) << 15;
 #pragma unroll 1
-            while (qq < qe) {
-                const uint32_t first = rp[qq];
-                uint32_t len = rp[qq + 1];
+            while (q < qe) {
+                const uint32_t first = rp[q];
+                uint32_t len = rp[q + 1];
                 if (len == 0) len = 256;
-                // most runs hold one or two strips; on the fast path the second byte is read
-                // unconditionally (it is inside the slot or its 16-byte tail pad)
-                const uint32_t b0 = rp[qq + 2], b1 = (kFast || len > 1) ? rp[qq + 3] : 0u;
-                const uint32_t sid = g0 + first;
-                strip_l[ee] = static_cast<uint16_t>(first == 0 ? sid | open_bit : sid);
-                adc_l[ee] = static_cast<uint8_t>(b0);
-                if (len > 1) {
-                    strip_l[ee + 1] = static_cast<uint16_t>(sid + 1u);
-                    adc_l[ee + 1] = static_cast<uint8_t>(b1);
-                    if (len > 2) {
-#pragma unroll 1
-                        for (uint32_t i = 2; i < len; ++i) {
-                            const uint32_t bi = rp[qq + 2 + i];
-                            strip_l[ee + i] = static_cast<uint16_t>(sid + i);
-                            adc_l[ee + i] = static_cast<uint8_t>(bi);
-                        }
-                    }
-                }
-                ee += len;
-                qq += 2 + len;
+                strip_l[e] = static_cast<uint16_t>(first == 0 ? (g0 | open_bit) : g0 + first);
+                atomicOr(&mR[e >> 5], 1u << (e & 31u));
+                e += len;
+                q += 2u + len;
             }
-            o0 = o1; o1 = o2; l0 = l1; l1 = l2; b0_ = b1_; b1_ = b2_; opens >>= 1;
+            o0 = o1; o1 = o2; l0 = l1; l1 = l2; b0 = b1; b1 = b2; opens >>= 1;
+        }
+    }
+    __syncwarp();
+
+    // ---------------------------------------------------------------- a2: expansion, lane per entry
+    // Entry e belongs to the last run that starts at or before it (run-start mask): its strip id is
+    // that run's first strip + the distance, and its ADC byte sits at e + 2 * (runs up to it) + a
+    // per-channel constant in the payload (each earlier run costs two header bytes).  On the fast
+    // path the ADC list is written over the payload itself: an iteration reads at addresses >= e + 4
+    // and writes 32 bytes at e, after all its reads.
+    {
+        uint32_t run_before = 0, start_before = 0;  // runs / last run start below this word
+#pragma unroll 1
+        for (uint32_t w = 0; w < nw; ++w) {
+            const uint32_t e = w * 32u + lane;
+            const uint32_t m = mR[w];
+            const uint32_t below = m & le;
+            const uint32_t e_r = below ? w * 32u + 31u - __clz(below) : start_before;
+            const uint32_t r1 = run_before + __popc(below);  // 1 + index of the entry's run
+            const uint32_t s0 = strip_l[e_r];
+            const uint32_t sid = (s0 & 0x7fffu) + (e - e_r);
+            uint32_t a = 0;
+            if (e < P) a = rp[e + 2u * r1 + ktab[sid >> 8]];
+            __syncwarp();
+            if (e < P) {
+                adc_l[e] = static_cast<uint8_t>(a);
+                if (e != e_r) strip_l[e] = static_cast<uint16_t>(sid);
+            }
+            run_before += __popc(m);
+            if (m) start_before = w * 32u + 31u - __clz(m);
         }
     }
     __syncwarp();  // lists complete; the payload is dead from here on
 
     // ---------------------------------------------------------------- a2: dense SoA
-    // The FED's 24576-byte block of the dense strip array is put together kWin strips at a time
+    // The FED's 24576-byte block of the dense strip array is put together 512*kw strips at a time
     // in a shared-memory window (zeros, then the present strips of the window from the sorted
     // lists) and leaves as full 16-byte stores: no zero-fill pass over HBM, no byte scatter.
     if (dense) {
-        if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0) {
+        if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0 && kw) {
             uint4 *const win = reinterpret_cast<uint4 *>(window);
+            const uint32_t wb = 512u * kw;
             uint32_t i0 = 0;  // first entry not yet placed
 #pragma unroll 1
-            for (uint32_t r = 0; r < static_cast<uint32_t>(kFedStrips) / kWin; ++r) {
-#pragma unroll
-                for (uint32_t k = 0; k < kWin / 512u; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
+            for (uint32_t base = 0; base < static_cast<uint32_t>(kFedStrips); base += wb) {
+#pragma unroll 1
+                for (uint32_t k = 0; k < kw; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
                 __syncwarp();
-                const uint32_t limit = (r + 1u) * kWin;
+                const uint32_t limit = base + wb;
                 for (;;) {  // two consecutive entries per lane; the list is sorted by strip
                     const uint32_t i = i0 + 2u * lane;
                     const uint32_t ia = i < P ? i : 0u, ib = i + 1u < P ? i + 1u : 0u;  // loads stay in the lists
                     const uint32_t sa = strip_l[ia] & 0x7fffu, sb = strip_l[ib] & 0x7fffu;
                     const uint32_t va = adc_l[ia], vb = adc_l[ib];
                     const bool ina = i < P && sa < limit, inb = i + 1u < P && sb < limit;
-                    if (ina) window[sa & (kWin - 1u)] = static_cast<uint8_t>(va);
-                    if (inb) window[sb & (kWin - 1u)] = static_cast<uint8_t>(vb);
+                    if (ina) window[sa - base] = static_cast<uint8_t>(va);
+                    if (inb) window[sb - base] = static_cast<uint8_t>(vb);
                     const uint32_t cnt = __popc(__ballot_sync(kFull, ina)) + __popc(__ballot_sync(kFull, inb));
                     i0 += cnt;
                     if (cnt < 64u) break;
                 }
                 __syncwarp();
-                uint4 v[kWin / 512u];
-#pragma unroll
-                for (uint32_t k = 0; k < kWin / 512u; ++k) v[k] = win[lane + 32u * k];
+#pragma unroll 1
+                for (uint32_t k = 0; k < kw; ++k)
+                    st_stream(reinterpret_cast<uint4 *>(dense + base) + lane + 32u * k, win[lane + 32u * k], pol_first);
                 __syncwarp();
-#pragma unroll
-                for (uint32_t k = 0; k < kWin / 512u; ++k)
-                    st_stream(reinterpret_cast<uint4 *>(dense + r * kWin) + lane + 32u * k, v[k], pol_first);
             }
-        } else {  // unaligned output: bytes
+        } else {  // unaligned output or no room for a window: bytes
 #pragma unroll 1
             for (uint32_t b = lane; b < static_cast<uint32_t>(kFedStrips); b += 32u) dense[b] = 0;
             __syncwarp();
@@ -503,237 +512,191 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         __syncwarp();
     }
 
-    // ---------------------------------------------------------------- a3..a6: one sweep over the lists
-    // Lane per CHUNK of consecutive entries, walked serially: active/seed tests, link to the previous
-    // entry, and the running (charge, noise^2, seed) of the open candidate are thread-local, so a
-    // candidate inside one chunk is decided exactly as the oracle does (double sum of noise^2,
-    // left to right) with no cross-lane traffic.  Results are mask bits: mA members and mH heads of
-    // accepted clusters, mS seeds.  A candidate that crosses a chunk boundary is put together
-    // afterwards from the tail partial of one lane and the lead partials of the next lanes.
-#pragma unroll 1
-    for (uint32_t w = lane; w < nw + 2; w += 32) {
-        mS[w] = 0;
-        mA[w] = 0;
-        mH[w] = 0;
-    }
-    const uint32_t Lc = ((P + 31u) >> 5) | 1u;  // odd: the lanes' list reads fall into different banks
-    const bool want_seeds = o.seed_idx != nullptr;
-    uint32_t n_seed_lane = 0;
-    const uint32_t e0 = min(lane * Lc, P), e1 = min(e0 + Lc, P);
-    auto mark = [&](uint32_t hd, uint32_t end) { mark_cluster(mH, mA, hd, end); };
-    auto decide = [&](uint32_t hd, uint32_t end, uint32_t Q, double N, bool seed) {
-        if (seed) {
-            const double dq = static_cast<double>(Q);
-            if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) mark(hd, end);
-        }
-    };
+    // ---------------------------------------------------------------- a3: flags, lane per entry
+    // One 8-byte gather of {noise, gain} per entry; exact >= tests (a3); the link to the previous
+    // entry (same module, adjacent strip, both active); the gain-corrected ADC replaces the raw one
+    // in the list.  Three bit masks come out: active, linked, seed (a4: the seed mask is what the
+    // seed-index array is compacted from).
+    uint32_t fed_seed = 0;
     {
-        // is the entry before the chunk active?  (its raw ADC is read before any lane overwrites it)
-        bool open = false;
-        uint32_t prev_s = 0;
-        if (e0 > 0) {
-            const uint32_t s = strip_l[e0 - 1], a = adc_l[e0 - 1];
-            prev_s = s & 0x7fffu;
-            if (a) open = ge_exact(static_cast<float>(a), p.t_ch, ld_calib(cal + prev_s, pol_last).x);
-        }
-        __syncwarp();
-        bool lead = open;  // an open candidate at the chunk start began in an earlier chunk
-        uint32_t hd = 0, Q = 0, accS = 0;
-        double N = 0.0;
-        bool seed = false;
-        uint32_t lQ = 0, lEnd = 0;  // lead partial: the part of an earlier candidate inside this chunk
-        double lN = 0.0;
-        bool lSeed = false, lClosed = false;
-        // software pipeline of depth one: the next entry's list reads and calibration gather are
-        // issued before the current entry is worked on
-        uint32_t sv_n = 0xffffu, av_n = 0;
-        float2 cv_n = make_float2(INFINITY, 1.0f);
-        auto fetch = [&](uint32_t e) {
-            if (e < e1) {
-                sv_n = strip_l[e];
-                av_n = adc_l[e];
-                cv_n = av_n ? ld_calib(cal + (sv_n & 0x7fffu), pol_last) : make_float2(INFINITY, 1.0f);
-            }
-        };
-        fetch(e0);
+        uint32_t carry = 0;  // strip id | active << 15 of the entry before this word
 #pragma unroll 1
-        for (uint32_t e = e0; e < e1; ++e) {
-            const uint32_t sv = sv_n, av = av_n;
-            const float2 cv = cv_n;
-            fetch(e + 1u);
+        for (uint32_t w = 0; w < nw; ++w) {
+            const uint32_t e = w * 32u + lane;
+            const bool valid = e < P;
+            const uint32_t sv = valid ? strip_l[e] : 0u, av = valid ? adc_l[e] : 0u;
             const uint32_t s15 = sv & 0x7fffu;
+            const float2 cv = ld_calib(cal + s15, pol_last);
             const float af = static_cast<float>(av);
             const bool is_act = av != 0 && ge_exact(af, p.t_ch, cv.x);
             const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
-            // this entry continues the candidate of the previous one
-            const bool is_link = is_act && open && !(sv & 0x8000u) && s15 == prev_s + 1u;
-            if (open && !is_link) {  // the open candidate ended with entry e - 1
-                if (lead) {
-                    lQ = Q; lN = N; lSeed = seed; lEnd = e - 1u; lClosed = true;
-                    lead = false;
-                } else {
-                    decide(hd, e - 1u, Q, N, seed);
-                }
+            if (is_act) adc_l[e] = static_cast<uint8_t>(gain_correct(af, cv.y));
+            const uint32_t pk = s15 | (static_cast<uint32_t>(is_act) << 15);
+            uint32_t pv = __shfl_up_sync(kFull, pk, 1);
+            if (lane == 0) pv = carry;
+            // (pv: active bit set and strip id one below, in one comparison)
+            const bool is_link = is_act && !(sv & 0x8000u) && pv == ((s15 - 1u) | 0x8000u);
+            const uint32_t bA = __ballot_sync(kFull, is_act), bL = __ballot_sync(kFull, is_link),
+                           bS = __ballot_sync(kFull, is_seed);
+            if (lane == 0) {
+                mA[w] = bA;
+                mL[w] = bL;
+                mS[w] = bS;
             }
-            if (is_act) {
-                if (!is_link) {
-                    hd = e; Q = 0; N = 0.0; seed = false;
-                }
-                const uint32_t q = gain_correct(af, cv.y);
-                adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
-                Q += q;
-                const double d = static_cast<double>(cv.x);
-                N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
-                seed = seed || is_seed;
-            }
-            open = is_act;
-            prev_s = s15;
-            n_seed_lane += is_seed;
-            if (want_seeds) {  // warp-uniform: the seed mask only feeds the seed-index array
-                if (is_seed) accS |= 1u << (e & 31u);
-                if ((e & 31u) == 31u || e + 1u == e1) {
-                    if (accS) atomicOr(&mS[e >> 5], accS);
-                    accS = 0;
-                }
-            }
+            carry = __shfl_sync(kFull, pk, 31);
+            fed_seed += __popc(bS);
         }
-        bool pend = false;  // an open candidate that began in this chunk and runs on
-        if (open) {
-            if (e1 == P) {  // the lists end here
-                if (lead) {
-                    lQ = Q; lN = N; lSeed = seed; lEnd = P - 1u; lClosed = true;
-                } else {
-                    decide(hd, P - 1u, Q, N, seed);
-                }
-            } else if (lead) {  // the whole chunk lies inside a candidate of an earlier chunk
-                lQ = Q; lN = N; lSeed = seed; lEnd = e1 - 1u; lClosed = false;
-            } else {
-                pend = true;
-            }
-        }
-        // candidates across chunk boundaries: tail + lead partials of the following lanes.  The sum
-        // of partial sums is not the oracle's left-to-right sum; they differ by < (2w + 32) * 2^-53
-        // relative, so the comparison is taken from it only outside that band.
-        for (uint32_t dd = 1; __any_sync(kFull, pend); ++dd) {
-            const uint32_t pk = __shfl_down_sync(kFull, lQ | (static_cast<uint32_t>(lSeed) << 30) |
-                                                            (static_cast<uint32_t>(lClosed) << 31), dd);
-            const uint32_t end_s = __shfl_down_sync(kFull, lEnd, dd);
-            const double n_s = __shfl_down_sync(kFull, lN, dd);
-            if (pend) {
-                if (lane + dd > 31u) {
-                    pend = false;  // cannot happen: the last lane's chunk ends the lists
-                } else {
-                    Q += pk & 0x3fffffffu;
-                    N += n_s;
-                    seed = seed || ((pk >> 30) & 1u);
-                    if (pk >> 31) {
-                        pend = false;
-                        if (seed) {
-                            const uint32_t wd = end_s - hd + 1u;
-                            const double dq = static_cast<double>(Q);
-                            const double lhs = __dmul_rn(dq, dq), rhs = __dmul_rn(p.tcl2, N);
-                            bool acc;
-                            if (fabs(lhs - rhs) > rhs * (static_cast<double>(wd + 16u) * 0x1p-51)) acc = lhs > rhs;
-                            else acc = accept_exact(cal, strip_l, hd, wd, Q, p.tcl2);
-                            if (acc) mark(hd, end_s);
-                        }
-                    }
-                }
-            }
+        if (lane == 0) {
+            mA[nw] = 0;
+            mL[nw] = 0;
+            mS[nw] = 0;
         }
     }
     __syncwarp();
 
-    // ---------------------------------------------------------------- counts and cluster records
-    // lane per mask word: exclusive prefix of (accepted heads, accepted members) per word, then
-    // every head gets its record {head entry, offset of its ADCs}
-    uint32_t fed_cl = 0, fed_adc = 0, fed_seed = 0;
+    // ---------------------------------------------------------------- a5: candidates that hold a seed
+    // A candidate is a maximal run of linked active entries: it starts at an active entry that is
+    // not linked.  Lane per mask word: the seed bits are smeared down along the links, across word
+    // boundaries until nothing changes (a second round only happens for candidates wider than a
+    // word), so the head of every candidate that holds a seed ends up marked (leftmost-seed
+    // ownership is implicit: one head per maximal run).  The marked heads are compacted into the
+    // candidate list.
+    uint32_t n_cand = 0;
     {
-        uint32_t run = 0;  // heads << 16 | members
+        // groups of 32 words, from the top: a group's lowest word carries into the group below
+        uint32_t carry_up = 0;  // (x & link & 1) of the word just above the group
+#pragma unroll 1
+        for (uint32_t g = (nw + 31u) >> 5; g-- > 0;) {
+            const uint32_t w = g * 32u + lane;
+            const bool in = w < nw;
+            const uint32_t lw = in ? mL[w] : 0u;
+            uint32_t x = smear_down(in ? mS[w] : 0u, lw);
+            for (;;) {
+                uint32_t up = __shfl_down_sync(kFull, x & lw & 1u, 1);
+                if (lane == 31) up = carry_up;
+                const bool grow = up && !(x >> 31);
+                if (grow) x = smear_down(x | 0x80000000u, lw);
+                if (!__any_sync(kFull, grow)) break;
+            }
+            if (in) mX[w] = x;
+            carry_up = __shfl_sync(kFull, x & lw & 1u, 0);
+        }
+        __syncwarp();
+        // compaction, lane per word, ascending
+        uint32_t run = 0;
 #pragma unroll 1
         for (uint32_t w0 = 0; w0 < nw; w0 += 32) {
             const uint32_t w = w0 + lane;
-            uint32_t v = 0;
-            if (w < nw) v = (__popc(mH[w]) << 16) | __popc(mA[w]);
-            const uint32_t incl = warp_incl_scan(v, lane);
-            if (w < nw) mP[w] = run + incl - v;
-            run += __shfl_sync(kFull, incl, 31);
-        }
-        fed_seed = __reduce_add_sync(kFull, n_seed_lane);
-        fed_cl = run >> 16;
-        fed_adc = run & 0xffffu;
-        if (kFast && fed_cl > rec_cap) return false;
-        __syncwarp();
-#pragma unroll 1
-        for (uint32_t w = lane; w < nw; w += 32) {
-            uint32_t mh = mH[w];
-            const uint32_t ma = mA[w], pre = mP[w];
-            uint32_t k = pre >> 16;
-            while (mh) {
-                const uint32_t b = __ffs(mh) - 1u;
-                mh &= mh - 1u;
-                rec[k++] = (w * 32u + b) | (((pre & 0xffffu) + __popc(ma & ((1u << b) - 1u))) << 16);
+            uint32_t hs = 0;
+            if (w < nw) hs = mA[w] & ~mL[w] & mX[w];
+            const uint32_t cnt = __popc(hs);
+            const uint32_t incl = warp_incl_scan(cnt, lane);
+            const uint32_t tot = __shfl_sync(kFull, incl, 31);
+            if (kFast && run + tot > rec_cap) return false;
+            uint32_t k = run + incl - cnt;
+            while (hs) {
+                const uint32_t b = __ffs(hs) - 1u;
+                hs &= hs - 1u;
+                rec[k++] = static_cast<uint16_t>(w * 32u + b);
             }
+            run += tot;
         }
-        if (P && lane == 0) rec[fed_cl] = fed_adc << 16;  // end sentinel: widths are offset differences
+        n_cand = run;
     }
     __syncwarp();
 
-    // ---------------------------------------------------------------- a7, first half: publish + stage
-    // The FED's counts go into its state word; its clusters, cluster ADCs and seeds are staged in
-    // FED-local order in global scratch.  sst_emit_kernel, launched behind this kernel on the same
-    // stream, turns the counts into offsets and moves everything to its (module, first strip)
-    // ordered place -- no warp ever waits for another one.
+    // ---------------------------------------------------------------- a5/a6/a7: lane per candidate
+    // The lane walks its candidate left to right: charge, first moment and the double sum of
+    // noise^2 in exactly the oracle's order (reading s15), then the cluster test, and stages the
+    // record {module, first | width << 16 | accepted << 31, charge, barycenter} + the list entry of
+    // its first strip in FED-local order.  sst_emit_kernel drops the rejected ones, turns counts
+    // into offsets and moves everything to its (module, first strip)-ordered place.
+    const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
+    const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
+    uint32_t fed_cl = 0, fed_adc = 0;
+    {
+        const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
+#pragma unroll 1
+        for (uint32_t k0 = 0; k0 < n_cand; k0 += 32) {
+            const uint32_t k = k0 + lane;
+            uint32_t acc_w = 0;  // width if accepted
+            if (k < n_cand) {
+                const uint32_t hd = rec[k];
+                const uint32_t st0 = strip_l[hd] & 0x7fffu;
+                const uint2 cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
+                // width: the link bits behind the head, 32 at a time
+                uint32_t wd = 1;
+                {
+                    const uint32_t wi = hd >> 5, b = hd & 31u;
+                    const uint32_t v = __funnelshift_rc(mL[wi], mL[wi + 1], b + 1u);
+                    uint32_t n1 = __ffs(~v) - 1u;  // trailing ones; ~v == 0 gives 0xffffffff
+                    if (v == kFull) {
+                        n1 = 32;
+                        while ((mL[(hd + n1 + 1u) >> 5] >> ((hd + n1 + 1u) & 31u)) & 1u) ++n1;  // (the pad word ends it)
+                    }
+                    wd += n1;
+                }
+                int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
+                double N = 0.0;
+                float nz = ld_calib(cal + st0, pol_last).x;
+#pragma unroll 1
+                for (uint32_t j = 0; j < wd; ++j) {
+                    const float nj = nz;
+                    if (j + 1u < wd) nz = ld_calib(cal + st0 + j + 1u, pol_last).x;
+                    const int q = adc_l[hd + j];
+                    Q += q;
+                    M += static_cast<int>(j) * q;
+                    const double d = static_cast<double>(nj);
+                    N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
+                }
+                const double dq = static_cast<double>(Q);
+                const bool acc = __dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N);
+                const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
+                // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
+                const float bary = __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
+                p.s_rec[sb + k] = make_uint4(cm.x, static_cast<uint32_t>(first) | (wd << 16) | (static_cast<uint32_t>(acc) << 31),
+                                             static_cast<uint32_t>(Q), __float_as_uint(bary));
+                p.s_off[sb + k] = hd;
+                if (o.cl_snr) p.s_snr[sb + k] = static_cast<float>(dq / sqrt(N));
+                if (acc) acc_w = wd;
+            }
+            fed_cl += __popc(__ballot_sync(kFull, acc_w != 0));
+            fed_adc += __reduce_add_sync(kFull, acc_w);
+        }
+    }
+
+    // ---------------------------------------------------------------- a7, first half: publish
+    // The FED's counts go into its state word and the next ticket is drawn; the list of corrected
+    // ADCs and (on request) the seeds are staged in FED-local order.
     if (lane == 0) {
         p.fed_state[static_cast<size_t>(c.ev) * p.n_feds + f] =
             (static_cast<unsigned long long>(c.overrun) << kShOver) |
             (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
             (static_cast<unsigned long long>(fed_seed) << kShSeed) |
             (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl;
+        p.fed_cand[static_cast<size_t>(c.ev) * p.n_feds + f] = n_cand;
         // next FED of this warp: the ticket arrives while the staging runs
         next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
     }
-    {
-        // cluster records: lane per cluster, consecutive lanes write consecutive records
-        const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
-        const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
-        const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
-        uint8_t *const sa = p.s_adc + ab;  // the FED's cluster ADCs, in order
+    if (n_cand) {
+        uint8_t *const sa = p.s_adc + ab;
+        if (kFast && (ab & 15u) == 0) {  // 16 bytes per lane; the list may be read up to 15 bytes past its end
+            const uint4 *src = reinterpret_cast<const uint4 *>(adc_l);
 #pragma unroll 1
-        for (uint32_t k0 = 0; k0 < fed_cl; k0 += 32) {
-            const uint32_t k = k0 + lane;
-            if (k < fed_cl) {
-                const uint32_t r0 = rec[k], r1 = rec[k + 1];
-                const uint32_t hd = r0 & 0xffffu, off = r0 >> 16, wd = (r1 >> 16) - off;
-                const uint32_t st0 = strip_l[hd] & 0x7fffu;
-                const uint2 cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
-                int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
+            for (uint32_t i = lane; i * 16u < P; i += 32u) st_stream(reinterpret_cast<uint4 *>(sa) + i, src[i], pol_first);
+        } else {
 #pragma unroll 1
-                for (uint32_t j = 0; j < wd; ++j) {
-                    const int q = adc_l[hd + j];
-                    Q += q;
-                    M += static_cast<int>(j) * q;
-                    sa[off + j] = static_cast<uint8_t>(q);  // neighbouring lanes write neighbouring bytes
-                }
-                const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
-                // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
-                const float bary = __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
-                p.s_rec[sb + k] = make_uint4(cm.x, static_cast<uint32_t>(first) | (wd << 16), static_cast<uint32_t>(Q),
-                                             __float_as_uint(bary));
-                p.s_off[sb + k] = off;
-                if (o.cl_snr)
-                    p.s_snr[sb + k] = static_cast<float>(static_cast<double>(Q) / sqrt(n2_sequential(cal, strip_l, hd, wd)));
-            }
+            for (uint32_t i = lane; i < P; i += 32u) sa[i] = adc_l[i];
         }
-        // a4: seed-index array (on request), FED-local strip ids
-        if (o.seed_idx) {
-            uint32_t k0 = 0;
+    }
+    // a4: seed-index array (on request), FED-local strip ids
+    if (o.seed_idx) {
+        uint32_t k0 = 0;
 #pragma unroll 1
-            for (uint32_t w = 0; w < nw; ++w) {
-                const uint32_t sw = mS[w];
-                if ((sw >> lane) & 1u) p.s_seed[ab + k0 + __popc(sw & lt)] = strip_l[w * 32u + lane] & 0x7fffu;
-                k0 += __popc(sw);
-            }
+        for (uint32_t w = 0; w < nw; ++w) {
+            const uint32_t sw = mS[w];
+            if ((sw >> lane) & 1u) p.s_seed[ab + k0 + __popc(sw & lt)] = strip_l[w * 32u + lane] & 0x7fffu;
+            k0 += __popc(sw);
         }
     }
     return true;
@@ -762,7 +725,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(slab + lane * kPiece), "r"(kPiece), "l"(policy_evict_last()) : "memory");
     }
     uint32_t *const chan_off = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
-    uint16_t *const chan_len = reinterpret_cast<uint16_t *>(chan_off + kChan);
+    uint16_t *const chan_len = reinterpret_cast<uint16_t *>(chan_off + kChan + 1);
 
     // ---------------------------------------------------------------- a1: stage the FED payload
     // lanes 0/1 fetch the two offsets; lane 0 starts the bulk copy
@@ -805,17 +768,15 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
 
     // ---------------------------------------------------------------- a1: walk the length chain
     if (staged) {
-        if (lane == 0) {
-            chan_off[0] = 2u;
-            walk_chain_speculative(slot, p.slot_bytes - kTabBytes - 2u, chan_off);
-        }
+        const uint32_t sa = smem_addr(slot);
+        if (lane == 0) walk_chain_speculative(sa, sa + p.slot_bytes - kTabBytes, smem_addr(chan_off));
         __syncwarp();
         // validate the speculative chain: channels from the first bad one on are empty
         uint32_t bad = 0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            c.off[k] = chan_off[lane + 32 * k];
-            c.len[k] = (chan_off[lane + 32 * k + 1] - c.off[k] - 2u) & 0xffffu;
+            c.off[k] = chan_off[lane + 32 * k] - sa;
+            c.len[k] = (chan_off[lane + 32 * k + 1] - sa - c.off[k] - 2u) & 0xffffu;
             const bool ok = c.overrun == 0 && c.off[k] <= c.fed_size && c.off[k] + c.len[k] <= c.fed_size;
             const uint32_t m = ~__ballot_sync(kFull, ok);
             if (!bad && m) bad = 32u * k + __ffs(m);  // 1 + index of the first bad channel
@@ -849,23 +810,32 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         if (o.chan_off) o.chan_off[f * kChan + ch] = c.fo0 + c.off[k];
         if (o.chan_len) o.chan_len[f * kChan + ch] = static_cast<uint16_t>(c.len[k]);
     }
-    uint32_t cnt[3];
-    if (staged) scan_runs3(slot, c, cnt);
-    else scan_runs3(rp, c, cnt);
-    // exclusive scan of the 96 counts
-    uint32_t run = 0;
+    uint32_t cnt[3], runs[3];
+    if (staged) scan_runs3(slot, c, cnt, runs);
+    else scan_runs3(rp, c, cnt, runs);
+    // exclusive scans of the 96 strip and run counts (one scan: runs in the upper half word)
+    uint32_t tot = 0;
+    uint32_t *const ktab = chan_off;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        const uint32_t inc = warp_incl_scan(cnt[k], lane);
-        c.base[k] = run + inc - cnt[k];
-        run += __shfl_sync(kFull, inc, 31);
+        const uint32_t v = cnt[k] | (runs[k] << 16);
+        const uint32_t inc = warp_incl_scan(v, lane);
+        const uint32_t ex = tot + inc - v;
+        c.ebase[k] = ex & 0xffffu;
+        // payload address of entry e of this channel: off + (e - ebase) + 2 * (run(e) - rbase + 1),
+        // i.e. e + 2 * (runs up to and including its own) + this constant
+        ktab[lane + 32 * k] = c.off[k] - (ex & 0xffffu) - 2u * (ex >> 16);
+        tot += __shfl_sync(kFull, inc, 31);
     }
-    c.P = run;  // present strips of the FED
+    c.P = tot & 0xffffu;  // present strips of the FED (<= 24576), runs <= 12288
+    c.R = tot >> 16;
+    __syncwarp();
 
-    // fast path: lists behind the payload, masks and at least a few records in its place
-    const uint32_t A = (c.fed_size + 15u) & ~15u;
-    if (!force_slow && staged && A + 3u * c.P + (A >= kWin ? 0u : kWin + 16u) <= p.slot_bytes &&
-        16u * (((c.P + 31u) >> 5) + 2u) + 64u <= A)
+    // fast path: lists and masks behind the payload, the dense window and then the candidate list
+    // in its place
+    const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (c.P + 15u) & ~15u;
+    const uint32_t tail2 = ((((A + 2u * c.P + 15u) & ~15u) + 20u * (((c.P + 31u) >> 5) + 1u)) + 15u) & ~15u;
+    if (!force_slow && staged && tail2 + (A - P16 >= 512u ? 0u : 2048u) + kTabBytes <= p.slot_bytes)
         return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
     return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
@@ -900,9 +870,11 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
 
 // ------------------------------------------------------------------------------ a7, second half
 // One warp per (event, FED), behind sst_event_kernel on the same stream: sums the state words of
-// the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then moves the staged
-// records, cluster ADCs and seeds of the FED to their final place.  Output capacity and the event
-// totals are handled here.
+// the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then goes through the
+// FED's staged candidates in order: the accepted ones get their cluster index (ballot) and ADC
+// offset (warp scan of the widths) and are written to their final place together with their
+// corrected ADCs (copied out of the staged list).  Output capacity and the event totals are
+// handled here.
 template <bool kPacked>
 __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __grid_constant__ KParams p) {
     const int lane = threadIdx.x & 31;
@@ -914,6 +886,8 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     constexpr bool packed = kPacked;  // every event of a launch is, or none
     const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
     const unsigned long long own = st[f];
+    const uint32_t n_cand = p.fed_cand[static_cast<size_t>(ev) * p.n_feds + f];
+    const uint32_t fed_start = E.fed_offsets[f];
     const uint32_t fed_cl = static_cast<uint32_t>(own & 0x3fffull), fed_adc = static_cast<uint32_t>((own >> kShAdc) & 0x7fffull),
                    fed_seed = static_cast<uint32_t>((own >> kShSeed) & 0x7fffull),
                    fed_malf = static_cast<uint32_t>((own >> kShMalf) & 0x7full), fed_over = static_cast<uint32_t>((own >> kShOver) & 1ull);
@@ -953,36 +927,43 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
                    b_over = static_cast<uint32_t>(accB >> 52);
     // where sst_event_kernel staged this FED (a FED with bad offsets staged nothing: its counts
     // are zero and the addresses below are never used)
-    const uint32_t fed_start = E.fed_offsets[f];
     const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
     const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
     const unsigned long long pol_first = policy_evict_first();
+    const uint32_t lt = (1u << lane) - 1u;
 
     const bool all_fit = b_cl + fed_cl <= o.cap_clusters && b_adc + fed_adc <= o.cap_adc;
-    uint32_t lim = 0;  // ADC bytes of this FED that belong to clusters that fit
-    // the loop bodies first gather a few independent loads, then store: the kernel is a plain copy
-    // and lives off loads in flight
-    constexpr int kB = 4;
+    uint32_t run_cl = b_cl, run_adc = b_adc;
+    // two groups of 32 candidates per step: the loads of both are issued before either is used
+    // (the kernel is a plain copy and lives off loads in flight)
+    constexpr int kB = 2;
 #pragma unroll 1
-    for (uint32_t k0 = lane; k0 < fed_cl; k0 += 32 * kB) {
+    for (uint32_t k0 = 0; k0 < n_cand; k0 += 32 * kB) {
         uint4 r[kB];
-        uint32_t off[kB];
+        uint32_t hd[kB];
         float snr[kB];
 #pragma unroll
         for (int j = 0; j < kB; ++j) {
-            const uint32_t k = k0 + 32 * j;
-            if (k < fed_cl) {
-                r[j] = p.s_rec[sb + k];
-                off[j] = p.s_off[sb + k];
-                if (o.cl_snr) snr[j] = p.s_snr[sb + k];
+            const uint32_t k = k0 + 32 * j + lane;
+            r[j] = make_uint4(0, 0, 0, 0);
+            hd[j] = 0;
+            snr[j] = 0.0f;
+            if (k < n_cand) {
+                r[j] = __ldcs(p.s_rec + sb + k);
+                hd[j] = __ldcs(p.s_off + sb + k);
+                if (o.cl_snr) snr[j] = __ldcs(p.s_snr + sb + k);
             }
         }
 #pragma unroll
         for (int j = 0; j < kB; ++j) {
-            const uint32_t k = k0 + 32 * j;
-            if (k < fed_cl) {
-                const uint32_t wd = r[j].y >> 16;
-                const uint32_t k_cl = b_cl + k, k_adc = b_adc + off[j];
+            const bool acc = r[j].y >> 31;
+            const uint32_t wd = acc ? (r[j].y >> 16) & 0x7fffu : 0u;
+            const uint32_t bal = __ballot_sync(kFull, acc);
+            const uint32_t incl = warp_incl_scan(wd, lane);
+            const uint32_t k_cl = run_cl + __popc(bal & lt), k_adc = run_adc + incl - wd;
+            run_cl += __popc(bal);
+            run_adc += __shfl_sync(kFull, incl, 31);
+            if (acc) {
                 if (all_fit || (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc)) {
                     st_stream(o.cl_module + k_cl, r[j].x, pol_first);
                     st_stream(o.cl_first + k_cl, r[j].y & 0xffffu, pol_first);
@@ -991,7 +972,9 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
                     st_stream(o.cl_bary + k_cl, __uint_as_float(r[j].w), pol_first);
                     st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
                     if (o.cl_snr) o.cl_snr[k_cl] = snr[j];
-                    lim = max(lim, off[j] + wd);
+                    const uint8_t *src = p.s_adc + ab + hd[j];
+#pragma unroll 1
+                    for (uint32_t i = 0; i < wd; ++i) st_stream(o.cl_adc + k_adc + i, src[i], pol_first);
                 } else {
                     // the first cluster that does not fit reports how many were written
                     const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
@@ -999,17 +982,6 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
                 }
             }
         }
-    }
-    lim = all_fit ? fed_adc : __reduce_max_sync(kFull, lim);
-#pragma unroll 1
-    for (uint32_t i0 = lane; i0 < lim; i0 += 32 * 8) {
-        uint32_t v[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j)
-            if (i0 + 32 * j < lim) v[j] = p.s_adc[ab + i0 + 32 * j];
-#pragma unroll
-        for (int j = 0; j < 8; ++j)
-            if (i0 + 32 * j < lim) st_stream(o.cl_adc + b_adc + i0 + 32 * j, v[j], pol_first);
     }
     if (o.seed_idx) {
 #pragma unroll 1
@@ -1084,7 +1056,7 @@ bool output_ok(const sst_output *o) {
 }
 
 struct ScratchLayout {
-    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr,
+    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_cand, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr,
         o_sadc, o_sseed, total;
 };
 ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
@@ -1099,9 +1071,10 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     L.o_ticket = 0;
     L.o_state = 256;
     // slow-path lists
-    L.o_rec = L.o_state + up(L.state_bytes);
-    L.o_mask = L.o_rec + up(4 * L.ents * cap_events);
-    L.o_strip = L.o_mask + up(4 * 4 * L.mwords * cap_events);
+    L.o_cand = L.o_state + up(L.state_bytes);
+    L.o_rec = L.o_cand + up(L.state_bytes / 2);
+    L.o_mask = L.o_rec + up(2 * L.ents * cap_events);
+    L.o_strip = L.o_mask + up(5 * 4 * L.mwords * cap_events);
     L.o_adc = L.o_strip + up(2 * L.ents * cap_events);
     // staging between the two kernels
     L.o_srec = L.o_adc + up(L.ents * cap_events);
@@ -1159,7 +1132,8 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
     kp.ticket_base = sl->ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
-    kp.g_rec = reinterpret_cast<uint32_t *>(blk + L.o_rec);
+    kp.fed_cand = reinterpret_cast<uint32_t *>(blk + L.o_cand);
+    kp.g_rec = reinterpret_cast<uint16_t *>(blk + L.o_rec);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
     kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
     kp.g_adc = blk + L.o_adc;
@@ -1250,7 +1224,7 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
                                                      : static_cast<uint32_t>(0.5 * m) + 32u;
         const uint32_t r_hint = (static_cast<uint32_t>(std::min(1.15 * m + 64.0, 65536.0)) + 15u) & ~15u;
         uint32_t need = std::max(r_hint + kTabBytes, r_hint + 3u * p_hint);
-        need = std::min(std::max((need + 15u) & ~15u, 2048u), (227u * 1024u / kWarpsPerCta - kWarpHdr - kTailPad) & ~15u);
+        need = std::min(std::max((need + 15u) & ~15u, 4096u), (227u * 1024u / kWarpsPerCta - kWarpHdr - kTailPad) & ~15u);
         auto set_slot = [&](uint32_t slot) {
             ctx->slot_bytes = slot;
             ctx->warp_stride = kWarpHdr + slot + kTailPad;
