@@ -104,7 +104,7 @@ struct KParams {
     uint16_t *g_rec;
     uint16_t *g_strip;
     uint8_t *g_adc;
-    uint32_t *g_mask;  // 5 arrays of g_mwords per event
+    uint32_t *g_mask;  // 4 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
     uint4 *s_rec;     // per candidate {module, first | width << 16 | accepted << 31, charge, barycenter}
@@ -337,6 +337,13 @@ __device__ __forceinline__ uint32_t smear_down(uint32_t x, uint32_t g) {
     return x;
 }
 
+// Fast-path layout of a warp's slot: offset of the strip-id list.  The payload (A bytes, the ADC
+// list is squeezed into its first P16 bytes) is followed by a gap when the dense SoA is wanted, so
+// that the 2048-byte window fits between the ADC list and the strip ids.
+__device__ __forceinline__ uint32_t fast_strip_base(uint32_t A, uint32_t P16, bool want_dense) {
+    return want_dense ? max(A, P16 + 2048u) : A;
+}
+
 // ------------------------------------------------------------------------------ lists -> clusters
 // Everything after pass 1, by one warp, data-parallel over the FED's list of present strips (the
 // structure of arrays of PAPER.md:31: one entry per recorded strip).  kFast: lists, masks and the
@@ -358,63 +365,56 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     uint32_t *const ktab = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
     uint16_t *strip_l, *rec;
     uint8_t *adc_l;
-    uint32_t *mR, *mA, *mL, *mS, *mX;
-    uint32_t rec_cap;      // seeded candidates the list can hold
-    uint8_t *window = nullptr;  // shared memory for the dense SoA assembly, free once the lists are complete
-    uint32_t kw = 0;            // its size in units of 512 strips
+    uint32_t *mA, *mL, *mS, *mX;
+    uint32_t rec_cap;           // seeded candidates the list can hold
+    uint8_t *window = nullptr;  // 2048 bytes for the dense SoA assembly, free once the lists are complete
     if (kFast) {
-        // [0, A): the payload; the ADC list takes its place ([0, P)), the rest holds the window and
-        // then the candidate list.  [A, A + 2P): strip ids.  Behind: five masks.
+        // [0, A): the payload; the ADC list takes its place ([0, P)), the rest (grown by a gap to
+        // 2048 bytes when the dense SoA is wanted) holds the window and then the candidate list.
+        // Behind it the strip ids (2P bytes) and four masks.
         const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (P + 15u) & ~15u;
+        const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
         adc_l = slot;
-        strip_l = reinterpret_cast<uint16_t *>(slot + A);
-        const uint32_t tail = (A + 2u * P + 15u) & ~15u;
-        mR = reinterpret_cast<uint32_t *>(slot + tail);
-        mA = mR + (nw + 1);
+        strip_l = reinterpret_cast<uint16_t *>(slot + S0);
+        mA = reinterpret_cast<uint32_t *>(slot + ((S0 + 2u * P + 15u) & ~15u));
         mL = mA + (nw + 1);
         mS = mL + (nw + 1);
         mX = mS + (nw + 1);
-        const uint32_t tail2 = (tail + 20u * (nw + 1) + 15u) & ~15u;
         rec = reinterpret_cast<uint16_t *>(slot + P16);
-        rec_cap = (A - P16) / 2u;
-        kw = min(4u, (A - P16) / 512u);
-        if (kw) {
-            window = slot + P16;
-        } else {  // a nearly empty FED: the caller made sure there is room behind the masks
-            kw = 4;
-            window = slot + tail2;
-        }
+        rec_cap = (S0 - P16) / 2u;
+        window = slot + P16;
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
         strip_l = p.g_strip + eb + slice;
         adc_l = p.g_adc + eb + slice;
         rec = p.g_rec + eb + slice;
-        mR = p.g_mask + static_cast<size_t>(c.ev) * 5u * p.g_mwords + (slice >> 5) + 4u * f;
-        mA = mR + p.g_mwords;
+        mA = p.g_mask + static_cast<size_t>(c.ev) * 4u * p.g_mwords + (slice >> 5) + 4u * f;
         mL = mA + p.g_mwords;
         mS = mL + p.g_mwords;
         mX = mS + p.g_mwords;
         rec_cap = 0xffffffffu;
         // the slot is free up to the channel table unless the payload is staged in it
-        if (rp != slot) {
-            window = slot;
-            kw = 4;
-        } else if (((c.fed_size + 15u) & ~15u) + 2048u + kTabBytes <= p.slot_bytes) {
-            window = slot + ((c.fed_size + 15u) & ~15u);
-            kw = 4;
-        }
+        const uint32_t A = (c.fed_size + 15u) & ~15u;
+        if (rp != slot) window = slot;
+        else if (A + 2048u + kTabBytes <= p.slot_bytes) window = slot + A;
     }
     const unsigned long long pol_last = policy_evict_last(), pol_first = policy_evict_first();
     uint8_t *const dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips : nullptr;
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
 
     // ---------------------------------------------------------------- a2 pass 2: the run starts
-    // Lane per channel again, headers only: the first strip of every run gets its list entry
-    // (strip id; bit 15 marks strip 0 of a channel that opens a module: nothing links across it)
-    // and a bit in the run-start mask.  Everything per strip is left to the expansion below.
+    // Lane per channel again, headers only: the list entry of the first strip of every run gets
+    // 1 + its strip id (bit 15 marks strip 0 of a channel that opens a module: nothing links across
+    // it); all other entries stay zero.  Everything per strip is left to the expansion below.
+    if (kFast) {
+        uint4 *z = reinterpret_cast<uint4 *>(strip_l);  // 16-byte aligned; the masks behind it are not in use yet
 #pragma unroll 1
-    for (uint32_t w = lane; w < nw + 1; w += 32) mR[w] = 0;
+        for (uint32_t i = lane; i * 8u < P; i += 32u) z[i] = make_uint4(0, 0, 0, 0);
+    } else {
+#pragma unroll 1
+        for (uint32_t i = lane; i < P; i += 32u) strip_l[i] = 0;
+    }
     __syncwarp();
     {
         uint32_t o0 = c.off[0], o1 = c.off[1], o2 = c.off[2], l0 = c.len[0], l1 = c.len[1], l2 = c.len[2];
@@ -423,67 +423,74 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         for (int k = 0; k < 3; ++k) {
             uint32_t q = o0, e = b0;
             const uint32_t qe = o0 + l0;
-            const uint32_t g0 = static_cast<uint32_t>(lane + 32 * k) * kStrip, open_bit = (opens & 1u) << 15;
+            const uint32_t g1 = static_cast<uint32_t>(lane + 32 * k) * kStrip + 1u, open_bit = (opens & 1u) << 15;
 #pragma unroll 1
             while (q < qe) {
                 const uint32_t first = rp[q];
                 uint32_t len = rp[q + 1];
                 if (len == 0) len = 256;
-                strip_l[e] = static_cast<uint16_t>(first == 0 ? (g0 | open_bit) : g0 + first);
-                atomicOr(&mR[e >> 5], 1u << (e & 31u));
+                strip_l[e] = static_cast<uint16_t>(first == 0 ? (g1 | open_bit) : g1 + first);
                 e += len;
                 q += 2u + len;
             }
+            __syncwarp();  // the lanes leave the walk at different times
             o0 = o1; o1 = o2; l0 = l1; l1 = l2; b0 = b1; b1 = b2; opens >>= 1;
         }
     }
     __syncwarp();
 
     // ---------------------------------------------------------------- a2: expansion, lane per entry
-    // Entry e belongs to the last run that starts at or before it (run-start mask): its strip id is
-    // that run's first strip + the distance, and its ADC byte sits at e + 2 * (runs up to it) + a
-    // per-channel constant in the payload (each earlier run costs two header bytes).  On the fast
-    // path the ADC list is written over the payload itself: an iteration reads at addresses >= e + 4
-    // and writes 32 bytes at e, after all its reads.
+    // Entry e belongs to the last run that starts at or before it (the non-zero entries, by ballot):
+    // its strip id is that run's first strip + the distance, and its ADC byte sits at e + 2 * (runs
+    // up to it) + a per-channel constant in the payload (each earlier run costs two header bytes).
+    // On the fast path the ADC list is written over the payload itself: an iteration reads at
+    // addresses >= e + 4 and writes 32 bytes at e, after all its reads.
     {
-        uint32_t run_before = 0, start_before = 0;  // runs / last run start below this word
+        uint32_t run_before = 0, start_before = 0, v_before = 0;  // runs / last run start / its entry below this word
 #pragma unroll 1
         for (uint32_t w = 0; w < nw; ++w) {
             const uint32_t e = w * 32u + lane;
-            const uint32_t m = mR[w];
+            const uint32_t v = e < P ? strip_l[e] : 0u;
+            const uint32_t m = __ballot_sync(kFull, v != 0);
             const uint32_t below = m & le;
-            const uint32_t e_r = below ? w * 32u + 31u - __clz(below) : start_before;
+            const uint32_t top = 31u - __clz(below);  // (32 when below == 0: the shuffle then reads lane 0, unused)
+            const uint32_t vs = __shfl_sync(kFull, v, top);
+            const uint32_t e_r = below ? w * 32u + top : start_before;
+            const uint32_t s0 = below ? vs : v_before;
+            const uint32_t sid = (s0 & 0x7fffu) - 1u + (e - e_r);
             const uint32_t r1 = run_before + __popc(below);  // 1 + index of the entry's run
-            const uint32_t s0 = strip_l[e_r];
-            const uint32_t sid = (s0 & 0x7fffu) + (e - e_r);
             uint32_t a = 0;
             if (e < P) a = rp[e + 2u * r1 + ktab[sid >> 8]];
             __syncwarp();
             if (e < P) {
                 adc_l[e] = static_cast<uint8_t>(a);
-                if (e != e_r) strip_l[e] = static_cast<uint16_t>(sid);
+                strip_l[e] = static_cast<uint16_t>(e == e_r ? sid | (s0 & 0x8000u) : sid);
+            }
+            if (m) {
+                const uint32_t mt = 31u - __clz(m);
+                v_before = __shfl_sync(kFull, v, mt);
+                start_before = w * 32u + mt;
             }
             run_before += __popc(m);
-            if (m) start_before = w * 32u + 31u - __clz(m);
         }
     }
     __syncwarp();  // lists complete; the payload is dead from here on
 
     // ---------------------------------------------------------------- a2: dense SoA
-    // The FED's 24576-byte block of the dense strip array is put together 512*kw strips at a time
+    // The FED's 24576-byte block of the dense strip array is put together 2048 strips at a time
     // in a shared-memory window (zeros, then the present strips of the window from the sorted
     // lists) and leaves as full 16-byte stores: no zero-fill pass over HBM, no byte scatter.
     if (dense) {
-        if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0 && kw) {
+        if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0 && window) {
+            constexpr uint32_t kWin = 2048;
             uint4 *const win = reinterpret_cast<uint4 *>(window);
-            const uint32_t wb = 512u * kw;
             uint32_t i0 = 0;  // first entry not yet placed
+#pragma unroll
+            for (uint32_t k = 0; k < kWin / 512u; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
 #pragma unroll 1
-            for (uint32_t base = 0; base < static_cast<uint32_t>(kFedStrips); base += wb) {
-#pragma unroll 1
-                for (uint32_t k = 0; k < kw; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
+            for (uint32_t base = 0; base < static_cast<uint32_t>(kFedStrips); base += kWin) {
                 __syncwarp();
-                const uint32_t limit = base + wb;
+                const uint32_t limit = base + kWin;
                 for (;;) {  // two consecutive entries per lane; the list is sorted by strip
                     const uint32_t i = i0 + 2u * lane;
                     const uint32_t ia = i < P ? i : 0u, ib = i + 1u < P ? i + 1u : 0u;  // loads stay in the lists
@@ -497,10 +504,13 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     if (cnt < 64u) break;
                 }
                 __syncwarp();
-#pragma unroll 1
-                for (uint32_t k = 0; k < kw; ++k)
-                    st_stream(reinterpret_cast<uint4 *>(dense + base) + lane + 32u * k, win[lane + 32u * k], pol_first);
-                __syncwarp();
+                // out, and zero again for the next window in the same sweep
+#pragma unroll
+                for (uint32_t k = 0; k < kWin / 512u; ++k) {
+                    const uint4 v = win[lane + 32u * k];
+                    win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
+                    st_stream(reinterpret_cast<uint4 *>(dense + base) + lane + 32u * k, v, pol_first);
+                }
             }
         } else {  // unaligned output or no room for a window: bytes
 #pragma unroll 1
@@ -731,27 +741,35 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     // lanes 0/1 fetch the two offsets; lane 0 starts the bulk copy
     const uint32_t fo = lane < 2 ? E.fed_offsets[f + lane] : 0u;
     const uint32_t fo0 = __shfl_sync(kFull, fo, 0), fo1 = __shfl_sync(kFull, fo, 1);
-    // reading s3c: the offsets never step back -- a FED that starts below an earlier offset is
-    // flagged and empty, so the valid FEDs of an event are disjoint and ascending (the FED-local
-    // staging areas are keyed by the start offset)
-    uint32_t fo_max = 0;
-#pragma unroll 1
-    for (uint32_t j = lane; j < f; j += 32) fo_max = max(fo_max, E.fed_offsets[j]);
-    fo_max = __reduce_max_sync(kFull, fo_max);
-    const bool valid = fo_max <= fo0 && fo0 <= fo1 && fo1 <= E.raw_limit;
+    // (the bulk copy is started on the FED's own two offsets; reading s3c -- the offsets never step
+    // back: a FED that starts below an earlier offset is flagged and empty -- is checked while it
+    // is in flight, and a refused FED simply ignores what was copied)
+    const bool valid0 = fo0 <= fo1 && fo1 <= E.raw_limit;
     c.fo0 = fo0;
-    c.fed_start = valid ? fo0 : 0u;
-    c.fed_size = valid ? fo1 - fo0 : 0u;
-    c.overrun = valid ? 0u : 1u;
+    c.fed_start = valid0 ? fo0 : 0u;
+    c.fed_size = valid0 ? fo1 - fo0 : 0u;
     // (force_slow only moves the lists to global memory; the payload is staged all the same)
     const bool staged = c.fed_size + kTabBytes <= p.slot_bytes && ((c.fed_start | c.fed_size) & 15u) == 0 &&
                         (reinterpret_cast<uintptr_t>(E.raw) & 15u) == 0;
     __syncwarp();  // every lane is done with the slot of the previous FED
-    if (staged && c.fed_size && lane == 0) {
+    const bool copying = staged && c.fed_size;
+    if (copying && lane == 0) {
         fence_proxy_async();  // earlier generic-proxy accesses to the slot before the async write
         mbar_expect_tx(mbar, c.fed_size);
         bulk_g2s(slot, E.raw + c.fed_start, c.fed_size, mbar, policy_evict_first());
     }
+    // the valid FEDs of an event are disjoint and ascending (the FED-local staging areas are keyed
+    // by the start offset)
+    uint32_t fo_max = 0;
+#pragma unroll 1
+    for (uint32_t j = lane; j < f; j += 32) fo_max = max(fo_max, E.fed_offsets[j]);
+    fo_max = __reduce_max_sync(kFull, fo_max);
+    const bool valid = valid0 && fo_max <= fo0;
+    if (!valid) {
+        c.fed_start = 0;
+        c.fed_size = 0;
+    }
+    c.overrun = valid ? 0u : 1u;
     // meanwhile: fetch the module map
     c.opens = 0;
 #pragma unroll
@@ -761,7 +779,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         if ((ci.y & 0xffu) == ch) c.opens |= 1u << k;
     }
     const uint8_t *rp = staged ? slot : E.raw + c.fed_start;
-    if (staged && c.fed_size) {
+    if (copying) {
         mbar_wait(mbar, mbar_phase);  // every lane waits: async-proxy writes visible to all readers
         mbar_phase ^= 1u;
     }
@@ -831,11 +849,10 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     c.R = tot >> 16;
     __syncwarp();
 
-    // fast path: lists and masks behind the payload, the dense window and then the candidate list
-    // in its place
+    // fast path: window / candidate list, strip ids and masks fit behind the ADC list
     const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (c.P + 15u) & ~15u;
-    const uint32_t tail2 = ((((A + 2u * c.P + 15u) & ~15u) + 20u * (((c.P + 31u) >> 5) + 1u)) + 15u) & ~15u;
-    if (!force_slow && staged && tail2 + (A - P16 >= 512u ? 0u : 2048u) + kTabBytes <= p.slot_bytes)
+    const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
+    if (!force_slow && staged && ((S0 + 2u * c.P + 15u) & ~15u) + 16u * (((c.P + 31u) >> 5) + 1u) + kTabBytes <= p.slot_bytes)
         return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
     return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
@@ -1074,7 +1091,7 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     L.o_cand = L.o_state + up(L.state_bytes);
     L.o_rec = L.o_cand + up(L.state_bytes / 2);
     L.o_mask = L.o_rec + up(2 * L.ents * cap_events);
-    L.o_strip = L.o_mask + up(5 * 4 * L.mwords * cap_events);
+    L.o_strip = L.o_mask + up(4 * 4 * L.mwords * cap_events);
     L.o_adc = L.o_strip + up(2 * L.ents * cap_events);
     // staging between the two kernels
     L.o_srec = L.o_adc + up(L.ents * cap_events);
