@@ -55,7 +55,7 @@
 #define SST_SLAB_AHEAD 2
 #endif
 #ifndef SST_EMIT_CTAS
-#define SST_EMIT_CTAS 8
+#define SST_EMIT_CTAS 6
 #endif
 #ifndef SST_HOST_CHUNK
 #define SST_HOST_CHUNK 4
@@ -97,7 +97,6 @@ struct KParams {
     const float2 *calib;     // {noise (+inf at bad strips), gain} per strip
     const uint2 *chan_info;  // {module id, first channel | end channel << 8 of the module}
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
-    uint32_t *fed_cand;             // [kMaxEv][n_feds] staged candidates (clusters before the cluster test)
     unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+warps)
     unsigned long long ticket_base;
     // global scratch of the slow path, one slice set per event
@@ -107,8 +106,7 @@ struct KParams {
     uint32_t *g_mask;  // 4 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
-    uint4 *s_rec;     // per candidate {module, first | width << 16 | accepted << 31, charge, barycenter}
-    uint32_t *s_off;  // list entry of the candidate's first strip (its ADCs are s_adc[entry .. +width))
+    uint4 *s_rec;     // per accepted cluster {module, first | width << 16, charge, barycenter}
     float *s_snr;
     uint8_t *s_adc;
     uint16_t *s_seed;
@@ -617,37 +615,40 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 
     // ---------------------------------------------------------------- a5/a6/a7: lane per candidate
     // The lane walks its candidate left to right: charge, first moment and the double sum of
-    // noise^2 in exactly the oracle's order (reading s15), then the cluster test, and stages the
-    // record {module, first | width << 16 | accepted << 31, charge, barycenter} + the list entry of
-    // its first strip in FED-local order.  sst_emit_kernel drops the rejected ones, turns counts
+    // noise^2 in exactly the oracle's order (reading s15), then the cluster test.  The accepted ones
+    // get their FED-local cluster index (ballot) and ADC offset (warp scan of the widths) on the
+    // spot -- the candidates are taken in strip order -- and are staged: record {module, first |
+    // width << 16, charge, barycenter} and corrected ADCs.  sst_emit_kernel turns the FED totals
     // into offsets and moves everything to its (module, first strip)-ordered place.
     const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
     const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
     uint32_t fed_cl = 0, fed_adc = 0;
     {
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
+        uint8_t *const sa = p.s_adc + ab;
 #pragma unroll 1
         for (uint32_t k0 = 0; k0 < n_cand; k0 += 32) {
             const uint32_t k = k0 + lane;
-            uint32_t acc_w = 0;  // width if accepted
+            uint32_t hd = 0, wd = 0, st0 = 0;
+            int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
+            double N = 0.0;
+            uint2 cm = make_uint2(0, 0);
+            bool acc = false;
             if (k < n_cand) {
-                const uint32_t hd = rec[k];
-                const uint32_t st0 = strip_l[hd] & 0x7fffu;
-                const uint2 cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
+                hd = rec[k];
+                st0 = strip_l[hd] & 0x7fffu;
+                cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
                 // width: the link bits behind the head, 32 at a time
-                uint32_t wd = 1;
                 {
                     const uint32_t wi = hd >> 5, b = hd & 31u;
                     const uint32_t v = __funnelshift_rc(mL[wi], mL[wi + 1], b + 1u);
-                    uint32_t n1 = __ffs(~v) - 1u;  // trailing ones; ~v == 0 gives 0xffffffff
+                    uint32_t n1 = __ffs(~v) - 1u;  // trailing ones
                     if (v == kFull) {
                         n1 = 32;
                         while ((mL[(hd + n1 + 1u) >> 5] >> ((hd + n1 + 1u) & 31u)) & 1u) ++n1;  // (the pad word ends it)
                     }
-                    wd += n1;
+                    wd = 1u + n1;
                 }
-                int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
-                double N = 0.0;
                 float nz = ld_calib(cal + st0, pol_last).x;
 #pragma unroll 1
                 for (uint32_t j = 0; j < wd; ++j) {
@@ -660,44 +661,36 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
                 }
                 const double dq = static_cast<double>(Q);
-                const bool acc = __dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N);
+                acc = __dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N);
+            }
+            const uint32_t bal = __ballot_sync(kFull, acc);
+            const uint32_t aw = acc ? wd : 0u;
+            const uint32_t incl = warp_incl_scan(aw, lane);
+            if (acc) {
+                const uint32_t kc = fed_cl + __popc(bal & lt), off = fed_adc + incl - wd;
                 const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
                 // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
                 const float bary = __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
-                p.s_rec[sb + k] = make_uint4(cm.x, static_cast<uint32_t>(first) | (wd << 16) | (static_cast<uint32_t>(acc) << 31),
-                                             static_cast<uint32_t>(Q), __float_as_uint(bary));
-                p.s_off[sb + k] = hd;
-                if (o.cl_snr) p.s_snr[sb + k] = static_cast<float>(dq / sqrt(N));
-                if (acc) acc_w = wd;
+                p.s_rec[sb + kc] = make_uint4(cm.x, static_cast<uint32_t>(first) | (wd << 16), static_cast<uint32_t>(Q),
+                                              __float_as_uint(bary));
+                if (o.cl_snr) p.s_snr[sb + kc] = static_cast<float>(static_cast<double>(Q) / sqrt(N));
+#pragma unroll 1
+                for (uint32_t j = 0; j < wd; ++j) sa[off + j] = adc_l[hd + j];  // neighbouring lanes write neighbouring bytes
             }
-            fed_cl += __popc(__ballot_sync(kFull, acc_w != 0));
-            fed_adc += __reduce_add_sync(kFull, acc_w);
+            fed_cl += __popc(bal);
+            fed_adc += __shfl_sync(kFull, incl, 31);
         }
     }
 
     // ---------------------------------------------------------------- a7, first half: publish
-    // The FED's counts go into its state word and the next ticket is drawn; the list of corrected
-    // ADCs and (on request) the seeds are staged in FED-local order.
+    // The FED's counts go into its state word and the next ticket is drawn.
     if (lane == 0) {
         p.fed_state[static_cast<size_t>(c.ev) * p.n_feds + f] =
             (static_cast<unsigned long long>(c.overrun) << kShOver) |
             (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
             (static_cast<unsigned long long>(fed_seed) << kShSeed) |
             (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl;
-        p.fed_cand[static_cast<size_t>(c.ev) * p.n_feds + f] = n_cand;
-        // next FED of this warp: the ticket arrives while the staging runs
         next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
-    }
-    if (n_cand) {
-        uint8_t *const sa = p.s_adc + ab;
-        if (kFast && (ab & 15u) == 0) {  // 16 bytes per lane; the list may be read up to 15 bytes past its end
-            const uint4 *src = reinterpret_cast<const uint4 *>(adc_l);
-#pragma unroll 1
-            for (uint32_t i = lane; i * 16u < P; i += 32u) st_stream(reinterpret_cast<uint4 *>(sa) + i, src[i], pol_first);
-        } else {
-#pragma unroll 1
-            for (uint32_t i = lane; i < P; i += 32u) sa[i] = adc_l[i];
-        }
     }
     // a4: seed-index array (on request), FED-local strip ids
     if (o.seed_idx) {
@@ -887,11 +880,9 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
 
 // ------------------------------------------------------------------------------ a7, second half
 // One warp per (event, FED), behind sst_event_kernel on the same stream: sums the state words of
-// the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then goes through the
-// FED's staged candidates in order: the accepted ones get their cluster index (ballot) and ADC
-// offset (warp scan of the widths) and are written to their final place together with their
-// corrected ADCs (copied out of the staged list).  Output capacity and the event totals are
-// handled here.
+// the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then moves the staged
+// records, cluster ADCs and seeds of the FED to their final place (a cluster's ADC offset is the
+// running sum of the widths).  Output capacity and the event totals are handled here.
 template <bool kPacked>
 __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __grid_constant__ KParams p) {
     const int lane = threadIdx.x & 31;
@@ -903,11 +894,20 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     constexpr bool packed = kPacked;  // every event of a launch is, or none
     const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
     const unsigned long long own = st[f];
-    const uint32_t n_cand = p.fed_cand[static_cast<size_t>(ev) * p.n_feds + f];
     const uint32_t fed_start = E.fed_offsets[f];
     const uint32_t fed_cl = static_cast<uint32_t>(own & 0x3fffull), fed_adc = static_cast<uint32_t>((own >> kShAdc) & 0x7fffull),
                    fed_seed = static_cast<uint32_t>((own >> kShSeed) & 0x7fffull),
                    fed_malf = static_cast<uint32_t>((own >> kShMalf) & 0x7full), fed_over = static_cast<uint32_t>((own >> kShOver) & 1ull);
+    // where sst_event_kernel staged this FED (a FED with bad offsets staged nothing: its counts
+    // are zero and the addresses below are never used)
+    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
+    const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
+    // the first records are requested before the prefix is known
+    constexpr int kB = 4;
+    uint4 r[kB];
+#pragma unroll
+    for (int j = 0; j < kB; ++j)
+        if (lane + 32 * j < fed_cl) r[j] = __ldcs(p.s_rec + sb + lane + 32 * j);
     // clusters | ADC bytes << 32 ; seeds | malformed << 32 (20 bits) | overrun << 52 (n_feds <= 4096)
     unsigned long long accA = 0, accB = 0, totA = 0;
     const uint32_t jend = packed ? p.n_feds : f;  // the packed layout needs the event's totals too
@@ -942,45 +942,35 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
     const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
                    b_over = static_cast<uint32_t>(accB >> 52);
-    // where sst_event_kernel staged this FED (a FED with bad offsets staged nothing: its counts
-    // are zero and the addresses below are never used)
-    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
-    const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
     const unsigned long long pol_first = policy_evict_first();
-    const uint32_t lt = (1u << lane) - 1u;
 
     const bool all_fit = b_cl + fed_cl <= o.cap_clusters && b_adc + fed_adc <= o.cap_adc;
-    uint32_t run_cl = b_cl, run_adc = b_adc;
-    // two groups of 32 candidates per step: the loads of both are issued before either is used
-    // (the kernel is a plain copy and lives off loads in flight)
-    constexpr int kB = 2;
+    uint32_t lim = 0;       // ADC bytes of this FED that belong to clusters that fit
+    uint32_t run_adc = 0;   // ADC bytes of the FED's clusters before this group
+    // the loop bodies first gather a few independent loads, then store: the kernel is a plain copy
+    // and lives off loads in flight
 #pragma unroll 1
-    for (uint32_t k0 = 0; k0 < n_cand; k0 += 32 * kB) {
-        uint4 r[kB];
-        uint32_t hd[kB];
+    for (uint32_t kb = 0; kb < fed_cl; kb += 32 * kB) {  // (warp-uniform: the scans inside need every lane)
+        const uint32_t k0 = kb + lane;
         float snr[kB];
 #pragma unroll
         for (int j = 0; j < kB; ++j) {
-            const uint32_t k = k0 + 32 * j + lane;
-            r[j] = make_uint4(0, 0, 0, 0);
-            hd[j] = 0;
-            snr[j] = 0.0f;
-            if (k < n_cand) {
-                r[j] = __ldcs(p.s_rec + sb + k);
-                hd[j] = __ldcs(p.s_off + sb + k);
+            const uint32_t k = k0 + 32 * j;
+            if (k < fed_cl) {
+                if (kb) r[j] = __ldcs(p.s_rec + sb + k);
                 if (o.cl_snr) snr[j] = __ldcs(p.s_snr + sb + k);
             }
         }
 #pragma unroll
         for (int j = 0; j < kB; ++j) {
-            const bool acc = r[j].y >> 31;
-            const uint32_t wd = acc ? (r[j].y >> 16) & 0x7fffu : 0u;
-            const uint32_t bal = __ballot_sync(kFull, acc);
+            const uint32_t k = k0 + 32 * j;
+            const bool have = k < fed_cl;
+            const uint32_t wd = have ? r[j].y >> 16 : 0u;
             const uint32_t incl = warp_incl_scan(wd, lane);
-            const uint32_t k_cl = run_cl + __popc(bal & lt), k_adc = run_adc + incl - wd;
-            run_cl += __popc(bal);
+            const uint32_t off = run_adc + incl - wd;
             run_adc += __shfl_sync(kFull, incl, 31);
-            if (acc) {
+            if (have) {
+                const uint32_t k_cl = b_cl + k, k_adc = b_adc + off;
                 if (all_fit || (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc)) {
                     st_stream(o.cl_module + k_cl, r[j].x, pol_first);
                     st_stream(o.cl_first + k_cl, r[j].y & 0xffffu, pol_first);
@@ -989,9 +979,7 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
                     st_stream(o.cl_bary + k_cl, __uint_as_float(r[j].w), pol_first);
                     st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
                     if (o.cl_snr) o.cl_snr[k_cl] = snr[j];
-                    const uint8_t *src = p.s_adc + ab + hd[j];
-#pragma unroll 1
-                    for (uint32_t i = 0; i < wd; ++i) st_stream(o.cl_adc + k_adc + i, src[i], pol_first);
+                    lim = max(lim, off + wd);
                 } else {
                     // the first cluster that does not fit reports how many were written
                     const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
@@ -999,6 +987,17 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
                 }
             }
         }
+    }
+    lim = all_fit ? fed_adc : __reduce_max_sync(kFull, lim);
+#pragma unroll 1
+    for (uint32_t i0 = lane; i0 < lim; i0 += 32 * 8) {
+        uint32_t v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (i0 + 32 * j < lim) v[j] = p.s_adc[ab + i0 + 32 * j];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (i0 + 32 * j < lim) st_stream(o.cl_adc + b_adc + i0 + 32 * j, v[j], pol_first);
     }
     if (o.seed_idx) {
 #pragma unroll 1
@@ -1073,7 +1072,7 @@ bool output_ok(const sst_output *o) {
 }
 
 struct ScratchLayout {
-    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_cand, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr,
+    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_ssnr,
         o_sadc, o_sseed, total;
 };
 ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
@@ -1088,15 +1087,13 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     L.o_ticket = 0;
     L.o_state = 256;
     // slow-path lists
-    L.o_cand = L.o_state + up(L.state_bytes);
-    L.o_rec = L.o_cand + up(L.state_bytes / 2);
+    L.o_rec = L.o_state + up(L.state_bytes);
     L.o_mask = L.o_rec + up(2 * L.ents * cap_events);
     L.o_strip = L.o_mask + up(4 * 4 * L.mwords * cap_events);
     L.o_adc = L.o_strip + up(2 * L.ents * cap_events);
     // staging between the two kernels
     L.o_srec = L.o_adc + up(L.ents * cap_events);
-    L.o_soff = L.o_srec + up(16 * L.cl_slots * cap_events);
-    L.o_ssnr = L.o_soff + up(4 * L.cl_slots * cap_events);
+    L.o_ssnr = L.o_srec + up(16 * L.cl_slots * cap_events);
     L.o_sadc = L.o_ssnr + up(4 * L.cl_slots * cap_events);
     L.o_sseed = L.o_sadc + up(L.ents * cap_events);
     L.total = L.o_sseed + up(2 * L.ents * cap_events);
@@ -1149,13 +1146,11 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
     kp.ticket_base = sl->ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
-    kp.fed_cand = reinterpret_cast<uint32_t *>(blk + L.o_cand);
     kp.g_rec = reinterpret_cast<uint16_t *>(blk + L.o_rec);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
     kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
     kp.g_adc = blk + L.o_adc;
     kp.s_rec = reinterpret_cast<uint4 *>(blk + L.o_srec);
-    kp.s_off = reinterpret_cast<uint32_t *>(blk + L.o_soff);
     kp.s_snr = reinterpret_cast<float *>(blk + L.o_ssnr);
     kp.s_adc = blk + L.o_sadc;
     kp.s_seed = reinterpret_cast<uint16_t *>(blk + L.o_sseed);
