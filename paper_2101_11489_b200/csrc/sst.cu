@@ -106,7 +106,7 @@ struct KParams {
     uint32_t *g_mask;  // 4 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
-    uint4 *s_rec;     // per accepted cluster {module, first | width << 16, charge, barycenter}
+    uint4 *s_rec;     // per accepted cluster {module, first | width << 16, charge, first moment}
     float *s_snr;
     uint8_t *s_adc;
     uint16_t *s_seed;
@@ -292,7 +292,7 @@ __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_
     uint32_t n0 = 0, n1 = 0, n2 = 0, r0 = 0, r1 = 0, r2 = 0, okbits = 0;
 #pragma unroll 1
     for (int k = 0; k < 3; ++k) {  // the register sets rotate
-        uint32_t q = o0, nf = 0, r = 0, n = 0;
+        uint32_t q = o0, nf = 0, r = 0;
         const uint32_t qe = o0 + l0;
         bool bad = false;
 #pragma unroll 1
@@ -300,13 +300,17 @@ __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_
             const uint32_t first = rp[q];
             uint32_t len = rp[q + 1];
             if (len == 0) len = 256;  // reading s2
-            bad = bad || first < nf || first + len > static_cast<uint32_t>(kStrip);
+            // a run that passes strip 255 leaves nf > 256: the next run (first <= 255) trips over
+            // it here, the last one is caught below
+            bad = bad || first < nf;
             nf = first + len;
             q += 2u + len;
-            n += len;
             ++r;
         }
-        const bool ok = !bad && q == qe;  // truncated header, or run bytes passing the payload end: q != qe
+        __syncwarp();  // the lanes leave the walk at different times
+        // truncated header, or run bytes passing the payload end: q != qe
+        const bool ok = !bad && q == qe && nf <= static_cast<uint32_t>(kStrip);
+        const uint32_t n = l0 - 2u * r;  // a well-formed channel of L bytes and r runs holds L - 2r strips
         o0 = o1; o1 = o2; l0 = l1; l1 = l2;
         n0 = n1; n1 = n2; n2 = ok ? n : 0u;
         r0 = r1; r1 = r2; r2 = ok ? r : 0u;
@@ -444,25 +448,34 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // On the fast path the ADC list is written over the payload itself: an iteration reads at
     // addresses >= e + 4 and writes 32 bytes at e, after all its reads.
     {
+        // In a FED without malformed channels or an overrun the per-channel constant is 2 * channel + 2
+        // (two length bytes per channel up to and including the entry's own); else it is looked up.
+        const bool regular = c.overrun == 0 && c.n_malformed == 0;
         uint32_t run_before = 0, start_before = 0, v_before = 0;  // runs / last run start / its entry below this word
+        const uint32_t last = P - 1u;                             // (P > 0 inside the loop)
+        uint32_t v_next = strip_l[min(static_cast<uint32_t>(lane), last)];
 #pragma unroll 1
         for (uint32_t w = 0; w < nw; ++w) {
             const uint32_t e = w * 32u + lane;
-            const uint32_t v = e < P ? strip_l[e] : 0u;
+            const bool in = e < P;
+            const uint32_t v = in ? v_next : 0u;
+            v_next = strip_l[min(e + 32u, last)];  // the next word's entries, ahead of their use
             const uint32_t m = __ballot_sync(kFull, v != 0);
             const uint32_t below = m & le;
-            const uint32_t top = 31u - __clz(below);  // (32 when below == 0: the shuffle then reads lane 0, unused)
+            const uint32_t top = 31u - __clz(below);  // (-1 when below == 0: the shuffle result is then unused)
             const uint32_t vs = __shfl_sync(kFull, v, top);
-            const uint32_t e_r = below ? w * 32u + top : start_before;
+            const uint32_t d = below ? lane - top : e - start_before;  // distance to the run's first strip
             const uint32_t s0 = below ? vs : v_before;
-            const uint32_t sid = (s0 & 0x7fffu) - 1u + (e - e_r);
+            const uint32_t sid = (s0 & 0x7fffu) - 1u + d;
             const uint32_t r1 = run_before + __popc(below);  // 1 + index of the entry's run
-            uint32_t a = 0;
-            if (e < P) a = rp[e + 2u * r1 + ktab[sid >> 8]];
+            const uint32_t ch = min(sid >> 8, static_cast<uint32_t>(kChan - 1));
+            uint32_t kc = 2u * ch + 2u;
+            if (!regular) kc = ktab[ch];
+            const uint32_t a = rp[min(min(e, last) + 2u * r1 + kc, c.fed_size - 1u)];  // (clamped: lanes past the end)
             __syncwarp();
-            if (e < P) {
+            if (in) {
                 adc_l[e] = static_cast<uint8_t>(a);
-                strip_l[e] = static_cast<uint16_t>(e == e_r ? sid | (s0 & 0x8000u) : sid);
+                strip_l[e] = static_cast<uint16_t>(d == 0 ? sid | (s0 & 0x8000u) : sid);
             }
             if (m) {
                 const uint32_t mt = 31u - __clz(m);
@@ -526,15 +539,26 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // in the list.  Three bit masks come out: active, linked, seed (a4: the seed mask is what the
     // seed-index array is compacted from).
     uint32_t fed_seed = 0;
-    {
+    if (nw) {
         uint32_t carry = 0;  // strip id | active << 15 of the entry before this word
+        // depth-one software pipeline: the next word's list entries and calibration gather are
+        // issued before the current word is worked on
+        const uint32_t last = P - 1u;
+        uint32_t sv_n = strip_l[min(static_cast<uint32_t>(lane), last)], av_n = adc_l[min(static_cast<uint32_t>(lane), last)];
+        float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
 #pragma unroll 1
         for (uint32_t w = 0; w < nw; ++w) {
             const uint32_t e = w * 32u + lane;
-            const bool valid = e < P;
-            const uint32_t sv = valid ? strip_l[e] : 0u, av = valid ? adc_l[e] : 0u;
+            const uint32_t sv = sv_n;
+            const uint32_t av = e < P ? av_n : 0u;  // (the entries past the end repeat the last one)
+            const float2 cv = cv_n;
+            {
+                const uint32_t en = min(e + 32u, last);
+                sv_n = strip_l[en];
+                av_n = adc_l[en];
+                cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
+            }
             const uint32_t s15 = sv & 0x7fffu;
-            const float2 cv = ld_calib(cal + s15, pol_last);
             const float af = static_cast<float>(av);
             const bool is_act = av != 0 && ge_exact(af, p.t_ch, cv.x);
             const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
@@ -554,11 +578,11 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             carry = __shfl_sync(kFull, pk, 31);
             fed_seed += __popc(bS);
         }
-        if (lane == 0) {
-            mA[nw] = 0;
-            mL[nw] = 0;
-            mS[nw] = 0;
-        }
+    }
+    if (lane == 0) {
+        mA[nw] = 0;
+        mL[nw] = 0;
+        mS[nw] = 0;
     }
     __syncwarp();
 
@@ -632,6 +656,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             uint32_t hd = 0, wd = 0, st0 = 0;
             int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
             double N = 0.0;
+            uint32_t q4 = 0;   // the first four corrected ADCs
             uint2 cm = make_uint2(0, 0);
             bool acc = false;
             if (k < n_cand) {
@@ -649,16 +674,28 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     }
                     wd = 1u + n1;
                 }
-                float nz = ld_calib(cal + st0, pol_last).x;
+                // four strips per step: their list bytes and noise gathers are issued together (strips
+                // past the end repeat the last one and count as zero, which leaves every sum unchanged)
 #pragma unroll 1
-                for (uint32_t j = 0; j < wd; ++j) {
-                    const float nj = nz;
-                    if (j + 1u < wd) nz = ld_calib(cal + st0 + j + 1u, pol_last).x;
-                    const int q = adc_l[hd + j];
-                    Q += q;
-                    M += static_cast<int>(j) * q;
-                    const double d = static_cast<double>(nj);
-                    N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
+                for (uint32_t j0 = 0; j0 < wd; j0 += 4u) {
+                    uint32_t qv[4];
+                    float nv[4];
+#pragma unroll
+                    for (uint32_t u = 0; u < 4u; ++u) {
+                        const uint32_t j = min(j0 + u, wd - 1u);
+                        qv[u] = adc_l[hd + j];
+                        nv[u] = ld_calib(cal + st0 + j, pol_last).x;
+                    }
+#pragma unroll
+                    for (uint32_t u = 0; u < 4u; ++u) {
+                        const bool in = j0 + u < wd;
+                        const int q = in ? static_cast<int>(qv[u]) : 0;
+                        const double d = in ? static_cast<double>(nv[u]) : 0.0;
+                        Q += q;
+                        M += static_cast<int>(j0 + u) * q;
+                        N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
+                        if (j0 == 0) q4 |= static_cast<uint32_t>(q) << (8u * u);
+                    }
                 }
                 const double dq = static_cast<double>(Q);
                 acc = __dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N);
@@ -668,14 +705,16 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             const uint32_t incl = warp_incl_scan(aw, lane);
             if (acc) {
                 const uint32_t kc = fed_cl + __popc(bal & lt), off = fed_adc + incl - wd;
-                const int first = static_cast<int>(st0) - static_cast<int>(cm.y & 0xffu) * kStrip;
-                // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
-                const float bary = __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
-                p.s_rec[sb + kc] = make_uint4(cm.x, static_cast<uint32_t>(first) | (wd << 16), static_cast<uint32_t>(Q),
-                                              __float_as_uint(bary));
+                const uint32_t first = st0 - (cm.y & 0xffu) * kStrip;
+                // (the barycenter first + M / Q is formed by sst_emit_kernel)
+                p.s_rec[sb + kc] = make_uint4(cm.x, first | (wd << 16), static_cast<uint32_t>(Q), static_cast<uint32_t>(M));
                 if (o.cl_snr) p.s_snr[sb + kc] = static_cast<float>(static_cast<double>(Q) / sqrt(N));
+                // neighbouring lanes write neighbouring bytes
+#pragma unroll
+                for (uint32_t u = 0; u < 4u; ++u)
+                    if (u < wd) sa[off + u] = static_cast<uint8_t>(q4 >> (8u * u));
 #pragma unroll 1
-                for (uint32_t j = 0; j < wd; ++j) sa[off + j] = adc_l[hd + j];  // neighbouring lanes write neighbouring bytes
+                for (uint32_t j = 4; j < wd; ++j) sa[off + j] = adc_l[hd + j];
             }
             fed_cl += __popc(bal);
             fed_adc += __shfl_sync(kFull, incl, 31);
@@ -976,7 +1015,11 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
                     st_stream(o.cl_first + k_cl, r[j].y & 0xffffu, pol_first);
                     st_stream(o.cl_width + k_cl, wd, pol_first);
                     st_stream(o.cl_charge + k_cl, static_cast<int32_t>(r[j].z), pol_first);
-                    st_stream(o.cl_bary + k_cl, __uint_as_float(r[j].w), pol_first);
+                    // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
+                    st_stream(o.cl_bary + k_cl,
+                              __fadd_rn(static_cast<float>(r[j].y & 0xffffu),
+                                        __fdiv_rn(static_cast<float>(static_cast<int>(r[j].w)), static_cast<float>(static_cast<int>(r[j].z)))),
+                              pol_first);
                     st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
                     if (o.cl_snr) o.cl_snr[k_cl] = snr[j];
                     lim = max(lim, off + wd);
