@@ -100,10 +100,9 @@ struct KParams {
     unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+warps)
     unsigned long long ticket_base;
     // global scratch of the slow path, one slice set per event
-    uint16_t *g_rec;
     uint16_t *g_strip;
     uint8_t *g_adc;
-    uint32_t *g_mask;  // 4 arrays of g_mwords per event
+    uint32_t *g_mask;  // g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
     uint4 *s_rec;     // per accepted cluster {module, first | width << 16, charge, first moment}
@@ -327,18 +326,6 @@ __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_
     }
 }
 
-// Seeds smeared towards lower entries along the links, inside one 32-entry word: bit e of the
-// result is set iff some seed bit s >= e is set with link bits e+1 .. s all set (link bit i:
-// entry i continues the candidate of entry i-1).  Five doubling steps.
-__device__ __forceinline__ uint32_t smear_down(uint32_t x, uint32_t g) {
-#pragma unroll
-    for (int s = 1; s < 32; s <<= 1) {
-        x |= (x & g) >> s;
-        g &= g << s;
-    }
-    return x;
-}
-
 // Fast-path layout of a warp's slot: offset of the strip-id list.  The payload (A bytes, the ADC
 // list is squeezed into its first P16 bytes) is followed by a gap when the dense SoA is wanted, so
 // that the 2048-byte window fits between the ADC list and the strip ids.
@@ -351,11 +338,9 @@ __device__ __forceinline__ uint32_t fast_strip_base(uint32_t A, uint32_t P16, bo
 // structure of arrays of PAPER.md:31: one entry per recorded strip).  kFast: lists, masks and the
 // candidate list live in the warp's shared-memory slot and the payload is staged there (the ADC
 // list is the payload squeezed in place); else they live in this FED's slice of the global
-// scratch and rp is whatever holds the payload.  Returns false (fast path only) when the
-// candidate list outgrows the slot: the FED is then redone on the slow path (nothing has been
-// published and every output written so far is rewritten identically).
+// scratch and rp is whatever holds the payload.
 template <bool kFast>
-__device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, const FedCtx &c,
+__device__ __forceinline__ void fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, const FedCtx &c,
                                           const int lane, uint32_t &next_ticket) {
     const uint32_t f = c.f, P = c.P;
     const EventDesc &E = p.ev[c.ev];
@@ -365,37 +350,26 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 
     // per-channel constant of the payload address of an entry: src(e) = e + 2 * run(e) + ktab[channel]
     uint32_t *const ktab = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
-    uint16_t *strip_l, *rec;
+    uint16_t *strip_l;
     uint8_t *adc_l;
-    uint32_t *mA, *mL, *mS, *mX;
-    uint32_t rec_cap;           // seeded candidates the list can hold
+    uint32_t *mS;               // seed mask, one bit per list entry (kept when the seed-index array is wanted)
     uint8_t *window = nullptr;  // 2048 bytes for the dense SoA assembly, free once the lists are complete
     if (kFast) {
         // [0, A): the payload; the ADC list takes its place ([0, P)), the rest (grown by a gap to
-        // 2048 bytes when the dense SoA is wanted) holds the window and then the candidate list.
-        // Behind it the strip ids (2P bytes) and four masks.
+        // 2048 bytes when the dense SoA is wanted) holds the window.  Behind it the strip ids
+        // (2P bytes) and the seed mask.
         const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (P + 15u) & ~15u;
         const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
         adc_l = slot;
         strip_l = reinterpret_cast<uint16_t *>(slot + S0);
-        mA = reinterpret_cast<uint32_t *>(slot + ((S0 + 2u * P + 15u) & ~15u));
-        mL = mA + (nw + 1);
-        mS = mL + (nw + 1);
-        mX = mS + (nw + 1);
-        rec = reinterpret_cast<uint16_t *>(slot + P16);
-        rec_cap = (S0 - P16) / 2u;
+        mS = reinterpret_cast<uint32_t *>(slot + ((S0 + 2u * P + 15u) & ~15u));
         window = slot + P16;
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
         strip_l = p.g_strip + eb + slice;
         adc_l = p.g_adc + eb + slice;
-        rec = p.g_rec + eb + slice;
-        mA = p.g_mask + static_cast<size_t>(c.ev) * 4u * p.g_mwords + (slice >> 5) + 4u * f;
-        mL = mA + p.g_mwords;
-        mS = mL + p.g_mwords;
-        mX = mS + p.g_mwords;
-        rec_cap = 0xffffffffu;
+        mS = p.g_mask + static_cast<size_t>(c.ev) * p.g_mwords + (slice >> 5) + 4u * f;
         // the slot is free up to the channel table unless the payload is staged in it
         const uint32_t A = (c.fed_size + 15u) & ~15u;
         if (rp != slot) window = slot;
@@ -533,191 +507,161 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         __syncwarp();
     }
 
-    // ---------------------------------------------------------------- a3: flags, lane per entry
-    // One 8-byte gather of {noise, gain} per entry; exact >= tests (a3); the link to the previous
-    // entry (same module, adjacent strip, both active); the gain-corrected ADC replaces the raw one
-    // in the list.  Three bit masks come out: active, linked, seed (a4: the seed mask is what the
-    // seed-index array is compacted from).
-    uint32_t fed_seed = 0;
-    if (nw) {
-        uint32_t carry = 0;  // strip id | active << 15 of the entry before this word
-        // depth-one software pipeline: the next word's list entries and calibration gather are
-        // issued before the current word is worked on
-        const uint32_t last = P - 1u;
-        uint32_t sv_n = strip_l[min(static_cast<uint32_t>(lane), last)], av_n = adc_l[min(static_cast<uint32_t>(lane), last)];
-        float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
-#pragma unroll 1
-        for (uint32_t w = 0; w < nw; ++w) {
-            const uint32_t e = w * 32u + lane;
-            const uint32_t sv = sv_n;
-            const uint32_t av = e < P ? av_n : 0u;  // (the entries past the end repeat the last one)
-            const float2 cv = cv_n;
-            {
-                const uint32_t en = min(e + 32u, last);
-                sv_n = strip_l[en];
-                av_n = adc_l[en];
-                cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
-            }
-            const uint32_t s15 = sv & 0x7fffu;
-            const float af = static_cast<float>(av);
-            const bool is_act = av != 0 && ge_exact(af, p.t_ch, cv.x);
-            const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
-            if (is_act) adc_l[e] = static_cast<uint8_t>(gain_correct(af, cv.y));
-            const uint32_t pk = s15 | (static_cast<uint32_t>(is_act) << 15);
-            uint32_t pv = __shfl_up_sync(kFull, pk, 1);
-            if (lane == 0) pv = carry;
-            // (pv: active bit set and strip id one below, in one comparison)
-            const bool is_link = is_act && !(sv & 0x8000u) && pv == ((s15 - 1u) | 0x8000u);
-            const uint32_t bA = __ballot_sync(kFull, is_act), bL = __ballot_sync(kFull, is_link),
-                           bS = __ballot_sync(kFull, is_seed);
-            if (lane == 0) {
-                mA[w] = bA;
-                mL[w] = bL;
-                mS[w] = bS;
-            }
-            carry = __shfl_sync(kFull, pk, 31);
-            fed_seed += __popc(bS);
-        }
-    }
-    if (lane == 0) {
-        mA[nw] = 0;
-        mL[nw] = 0;
-        mS[nw] = 0;
-    }
-    __syncwarp();
-
-    // ---------------------------------------------------------------- a5: candidates that hold a seed
-    // A candidate is a maximal run of linked active entries: it starts at an active entry that is
-    // not linked.  Lane per mask word: the seed bits are smeared down along the links, across word
-    // boundaries until nothing changes (a second round only happens for candidates wider than a
-    // word), so the head of every candidate that holds a seed ends up marked (leftmost-seed
-    // ownership is implicit: one head per maximal run).  The marked heads are compacted into the
-    // candidate list.
-    uint32_t n_cand = 0;
-    {
-        // groups of 32 words, from the top: a group's lowest word carries into the group below
-        uint32_t carry_up = 0;  // (x & link & 1) of the word just above the group
-#pragma unroll 1
-        for (uint32_t g = (nw + 31u) >> 5; g-- > 0;) {
-            const uint32_t w = g * 32u + lane;
-            const bool in = w < nw;
-            const uint32_t lw = in ? mL[w] : 0u;
-            uint32_t x = smear_down(in ? mS[w] : 0u, lw);
-            for (;;) {
-                uint32_t up = __shfl_down_sync(kFull, x & lw & 1u, 1);
-                if (lane == 31) up = carry_up;
-                const bool grow = up && !(x >> 31);
-                if (grow) x = smear_down(x | 0x80000000u, lw);
-                if (!__any_sync(kFull, grow)) break;
-            }
-            if (in) mX[w] = x;
-            carry_up = __shfl_sync(kFull, x & lw & 1u, 0);
-        }
-        __syncwarp();
-        // compaction, lane per word, ascending
-        uint32_t run = 0;
-#pragma unroll 1
-        for (uint32_t w0 = 0; w0 < nw; w0 += 32) {
-            const uint32_t w = w0 + lane;
-            uint32_t hs = 0;
-            if (w < nw) hs = mA[w] & ~mL[w] & mX[w];
-            const uint32_t cnt = __popc(hs);
-            const uint32_t incl = warp_incl_scan(cnt, lane);
-            const uint32_t tot = __shfl_sync(kFull, incl, 31);
-            if (kFast && run + tot > rec_cap) return false;
-            uint32_t k = run + incl - cnt;
-            while (hs) {
-                const uint32_t b = __ffs(hs) - 1u;
-                hs &= hs - 1u;
-                rec[k++] = static_cast<uint16_t>(w * 32u + b);
-            }
-            run += tot;
-        }
-        n_cand = run;
-    }
-    __syncwarp();
-
-    // ---------------------------------------------------------------- a5/a6/a7: lane per candidate
-    // The lane walks its candidate left to right: charge, first moment and the double sum of
-    // noise^2 in exactly the oracle's order (reading s15), then the cluster test.  The accepted ones
-    // get their FED-local cluster index (ballot) and ADC offset (warp scan of the widths) on the
-    // spot -- the candidates are taken in strip order -- and are staged: record {module, first |
-    // width << 16, charge, barycenter} and corrected ADCs.  sst_emit_kernel turns the FED totals
-    // into offsets and moves everything to its (module, first strip)-ordered place.
+    // ---------------------------------------------------------------- a3..a7: one loop over the list
+    // Lane per entry, a word of 32 entries per step, in two stages that are one word apart:
+    //
+    // stage A (word w+1): one 8-byte gather of {noise, gain}; exact >= tests (a3: active, seed);
+    //   the link to the previous entry (same module, adjacent strip, both active); the
+    //   gain-corrected ADC, which replaces the raw one in the list; ballots give the word's
+    //   active / linked / seed masks (a4: the seed mask is what the seed-index array is made from).
+    // stage B (word w): a candidate is a maximal run of linked active entries.  Its first lane
+    //   collects the run's charge, first moment and noise^2 from the lanes behind it by shuffles,
+    //   one strip per step, left to right -- the double sum of noise^2 is the oracle's (reading
+    //   s15).  A candidate that runs past the word's end is carried to lane 0 of the next word
+    //   (stage A of that word has already said whether it continues).  Where a candidate ends it is
+    //   tested once (a5: leftmost-seed ownership is implicit; a6: the cluster test) and, if
+    //   accepted, staged in FED-local order: record {module, first | width << 16, charge, first
+    //   moment} at its cluster index (ballot) and its corrected ADCs at the running byte offset.
+    // sst_emit_kernel turns the FED totals into offsets and moves everything to its
+    // (module, first strip)-ordered place.
     const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
     const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
-    uint32_t fed_cl = 0, fed_adc = 0;
-    {
+    uint32_t fed_seed = 0, fed_cl = 0, fed_adc = 0;
+    if (nw) {
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
         uint8_t *const sa = p.s_adc + ab;
+        const bool want_seeds = o.seed_idx != nullptr;
+        const uint32_t last = P - 1u;
+        // list entries and calibration of the word stage A takes next (issued a step ahead)
+        uint32_t sv_n = strip_l[min(static_cast<uint32_t>(lane), last)], av_n = adc_l[min(static_cast<uint32_t>(lane), last)];
+        float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
+        uint32_t link_carry = 0;  // strip id | active << 15 of the entry before stage A's word
+        // stage A's results for the word stage B takes next
+        uint32_t a_sv = 0, a_q = 0, a_bA = 0, a_bL = 0, a_bS = 0;
+        float a_nz = 0.0f;
+        // the candidate that is open at the start of stage B's word (valid when its link bit 0 is set)
+        uint32_t cQ = 0, cM = 0, cLen = 0, cSid = 0, cHd = 0, cSeed = 0;
+        double cN = 0.0;
 #pragma unroll 1
-        for (uint32_t k0 = 0; k0 < n_cand; k0 += 32) {
-            const uint32_t k = k0 + lane;
-            uint32_t hd = 0, wd = 0, st0 = 0;
-            int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
-            double N = 0.0;
-            uint32_t q4 = 0;   // the first four corrected ADCs
-            uint2 cm = make_uint2(0, 0);
-            bool acc = false;
-            if (k < n_cand) {
-                hd = rec[k];
-                st0 = strip_l[hd] & 0x7fffu;
-                cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
-                // width: the link bits behind the head, 32 at a time
+        for (uint32_t w = 0; w <= nw; ++w) {
+            // ---- stage B inputs: the word stage A produced in the previous step
+            const uint32_t sv = a_sv, q = a_q, bA = a_bA, bL = a_bL, bS = a_bS;
+            const float nz = a_nz;
+            // ---- stage A on word w
+            if (w < nw) {
+                const uint32_t e = w * 32u + lane;
+                const uint32_t svw = sv_n;
+                const uint32_t av = e < P ? av_n : 0u;  // (the entries past the end repeat the last one)
+                const float2 cv = cv_n;
                 {
-                    const uint32_t wi = hd >> 5, b = hd & 31u;
-                    const uint32_t v = __funnelshift_rc(mL[wi], mL[wi + 1], b + 1u);
-                    uint32_t n1 = __ffs(~v) - 1u;  // trailing ones
-                    if (v == kFull) {
-                        n1 = 32;
-                        while ((mL[(hd + n1 + 1u) >> 5] >> ((hd + n1 + 1u) & 31u)) & 1u) ++n1;  // (the pad word ends it)
-                    }
-                    wd = 1u + n1;
+                    const uint32_t en = min(e + 32u, last);
+                    sv_n = strip_l[en];
+                    av_n = adc_l[en];
+                    cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
                 }
-                // four strips per step: their list bytes and noise gathers are issued together (strips
-                // past the end repeat the last one and count as zero, which leaves every sum unchanged)
+                const uint32_t s15 = svw & 0x7fffu;
+                const float af = static_cast<float>(av);
+                const bool is_act = av != 0 && ge_exact(af, p.t_ch, cv.x);
+                const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
+                const uint32_t qc = is_act ? gain_correct(af, cv.y) : 0u;
+                if (is_act) adc_l[e] = static_cast<uint8_t>(qc);
+                const uint32_t pk = s15 | (static_cast<uint32_t>(is_act) << 15);
+                uint32_t pv = __shfl_up_sync(kFull, pk, 1);
+                if (lane == 0) pv = link_carry;
+                // (pv: active bit set and strip id one below, in one comparison)
+                const bool is_link = is_act && !(svw & 0x8000u) && pv == ((s15 - 1u) | 0x8000u);
+                a_bA = __ballot_sync(kFull, is_act);
+                a_bL = __ballot_sync(kFull, is_link);
+                a_bS = __ballot_sync(kFull, is_seed);
+                link_carry = __shfl_sync(kFull, pk, 31);
+                a_sv = s15;
+                a_q = qc;
+                a_nz = cv.x;
+                fed_seed += __popc(a_bS);
+                if (want_seeds && lane == 0) mS[w] = a_bS;
+            } else {
+                a_bA = a_bL = a_bS = 0;
+            }
+            if (w == 0) continue;
+            // ---- stage B on word w - 1
+            const uint32_t wb = w - 1u;
+            const bool cont_next = a_bL & 1u;     // the entry behind this word continues its last candidate
+            const bool virt = (bL & 1u) && lane == 0;  // lane 0 continues the carried candidate
+            const bool is_head = (((bA & ~bL) >> lane) & 1u) || virt;
+            // consecutive link bits behind this lane: the rest of its candidate inside the word
+            const uint32_t behind = lane == 31 ? 0u : bL >> (lane + 1);
+            const uint32_t n1 = __ffs(~behind) - 1u;
+            int Q = static_cast<int>(q), M = 0;
+            double N = 0.0;
+            uint32_t j0 = 0;  // position of this lane's strip inside its candidate
+            if (virt) {
+                j0 = cLen;
+                Q += static_cast<int>(cQ);
+                M = static_cast<int>(cM) + static_cast<int>(cLen * q);
+                N = cN;
+            }
+            {
+                const double d = static_cast<double>(nz);
+                N = __fma_rn(d, d, N);  // exact square, one rounding
+            }
+            const uint32_t trips = __reduce_max_sync(kFull, is_head ? n1 : 0u);
 #pragma unroll 1
-                for (uint32_t j0 = 0; j0 < wd; j0 += 4u) {
-                    uint32_t qv[4];
-                    float nv[4];
-#pragma unroll
-                    for (uint32_t u = 0; u < 4u; ++u) {
-                        const uint32_t j = min(j0 + u, wd - 1u);
-                        qv[u] = adc_l[hd + j];
-                        nv[u] = ld_calib(cal + st0 + j, pol_last).x;
-                    }
-#pragma unroll
-                    for (uint32_t u = 0; u < 4u; ++u) {
-                        const bool in = j0 + u < wd;
-                        const int q = in ? static_cast<int>(qv[u]) : 0;
-                        const double d = in ? static_cast<double>(nv[u]) : 0.0;
-                        Q += q;
-                        M += static_cast<int>(j0 + u) * q;
-                        N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
-                        if (j0 == 0) q4 |= static_cast<uint32_t>(q) << (8u * u);
-                    }
+            for (uint32_t j = 1; j <= trips; ++j) {
+                const uint32_t qj = __shfl_down_sync(kFull, q, j);
+                const float nj = __shfl_down_sync(kFull, nz, j);
+                if (j <= n1) {
+                    Q += static_cast<int>(qj);
+                    M += static_cast<int>((j0 + j) * qj);
+                    const double d = static_cast<double>(nj);
+                    N = __fma_rn(d, d, N);
                 }
+            }
+            const bool to_end = lane + n1 == 31u;
+            const bool open = is_head && to_end && cont_next;
+            const uint32_t segmask = ((2u << n1) - 1u) << lane;  // (n1 <= 31 - lane)
+            const bool seeded = (bS & segmask) != 0 || (virt && cSeed);
+            const uint32_t wd = j0 + 1u + n1;
+            bool acc = false;
+            if (is_head && !open && seeded) {
                 const double dq = static_cast<double>(Q);
                 acc = __dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N);
             }
             const uint32_t bal = __ballot_sync(kFull, acc);
-            const uint32_t aw = acc ? wd : 0u;
-            const uint32_t incl = warp_incl_scan(aw, lane);
-            if (acc) {
-                const uint32_t kc = fed_cl + __popc(bal & lt), off = fed_adc + incl - wd;
-                const uint32_t first = st0 - (cm.y & 0xffu) * kStrip;
-                // (the barycenter first + M / Q is formed by sst_emit_kernel)
-                p.s_rec[sb + kc] = make_uint4(cm.x, first | (wd << 16), static_cast<uint32_t>(Q), static_cast<uint32_t>(M));
-                if (o.cl_snr) p.s_snr[sb + kc] = static_cast<float>(static_cast<double>(Q) / sqrt(N));
-                // neighbouring lanes write neighbouring bytes
-#pragma unroll
-                for (uint32_t u = 0; u < 4u; ++u)
-                    if (u < wd) sa[off + u] = static_cast<uint8_t>(q4 >> (8u * u));
+            if (bal) {
+                const uint32_t macc = __reduce_or_sync(kFull, acc ? segmask : 0u);  // this word's entries in accepted clusters
+                const uint32_t extra = (bal & 1u) && (bL & 1u) ? cLen : 0u;         // + the carried part of lane 0's
+                if (extra) {  // its ADCs of the earlier words come out of the list
+                    __syncwarp();
 #pragma unroll 1
-                for (uint32_t j = 4; j < wd; ++j) sa[off + j] = adc_l[hd + j];
+                    for (uint32_t j = lane; j < extra; j += 32u) sa[fed_adc + j] = adc_l[cHd + j];
+                }
+                if ((macc >> lane) & 1u) sa[fed_adc + extra + __popc(macc & lt)] = static_cast<uint8_t>(q);
+                if (acc) {
+                    const uint32_t st0 = virt ? cSid : sv;
+                    const uint2 cm = __ldg(cinfo + (st0 >> 8));
+                    const uint32_t first = st0 - (cm.y & 0xffu) * kStrip;
+                    const uint32_t kc = fed_cl + __popc(bal & lt);
+                    // (the barycenter first + M / Q is formed by sst_emit_kernel)
+                    p.s_rec[sb + kc] = make_uint4(cm.x, first | (wd << 16), static_cast<uint32_t>(Q), static_cast<uint32_t>(M));
+                    if (o.cl_snr) p.s_snr[sb + kc] = static_cast<float>(static_cast<double>(Q) / sqrt(N));
+                }
+                fed_cl += __popc(bal);
+                fed_adc += extra + __popc(macc);
             }
-            fed_cl += __popc(bal);
-            fed_adc += __shfl_sync(kFull, incl, 31);
+            // the candidate that stays open moves to lane 0 of the next word
+            const uint32_t bo = __ballot_sync(kFull, open);
+            if (bo) {
+                const int src = __ffs(bo) - 1;
+                cQ = __shfl_sync(kFull, static_cast<uint32_t>(Q), src);
+                cM = __shfl_sync(kFull, static_cast<uint32_t>(M), src);
+                cN = __shfl_sync(kFull, N, src);
+                cLen = __shfl_sync(kFull, wd, src);
+                cSeed = __shfl_sync(kFull, static_cast<uint32_t>(seeded), src);
+                const uint32_t sid_h = __shfl_sync(kFull, virt ? cSid : sv, src);
+                const uint32_t hd_h = __shfl_sync(kFull, virt ? cHd : wb * 32u + lane, src);
+                cSid = sid_h;
+                cHd = hd_h;
+            }
         }
     }
 
@@ -741,14 +685,12 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             k0 += __popc(sw);
         }
     }
-    return true;
 }
 
 // ------------------------------------------------------------------------------ one FED, one warp
-// Returns false when the FED has to be redone with force_slow (see fed_lists).
-__device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot,
-                                            const uint32_t ticket, const int lane, const bool force_slow,
-                                            uint32_t &mbar_phase, uint32_t &next_ticket) {
+__device__ __forceinline__ void process_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot,
+                                            const uint32_t ticket, const int lane, uint32_t &mbar_phase,
+                                            uint32_t &next_ticket) {
     FedCtx c;
     c.ticket = ticket;
     // FED-major order: the same FED of all the launch's events back to back, so the FED's slab of
@@ -780,7 +722,6 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     c.fo0 = fo0;
     c.fed_start = valid0 ? fo0 : 0u;
     c.fed_size = valid0 ? fo1 - fo0 : 0u;
-    // (force_slow only moves the lists to global memory; the payload is staged all the same)
     const bool staged = c.fed_size + kTabBytes <= p.slot_bytes && ((c.fed_start | c.fed_size) & 15u) == 0 &&
                         (reinterpret_cast<uintptr_t>(E.raw) & 15u) == 0;
     __syncwarp();  // every lane is done with the slot of the previous FED
@@ -881,12 +822,13 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     c.R = tot >> 16;
     __syncwarp();
 
-    // fast path: window / candidate list, strip ids and masks fit behind the ADC list
+    // fast path: window, strip ids and seed mask fit behind the ADC list
     const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (c.P + 15u) & ~15u;
     const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
-    if (!force_slow && staged && ((S0 + 2u * c.P + 15u) & ~15u) + 16u * (((c.P + 31u) >> 5) + 1u) + kTabBytes <= p.slot_bytes)
-        return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
-    return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
+    if (staged && ((S0 + 2u * c.P + 15u) & ~15u) + 4u * (((c.P + 31u) >> 5) + 1u) + kTabBytes <= p.slot_bytes)
+        fed_lists<true>(p, slot, slot, c, lane, next_ticket);
+    else
+        fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
 
 // ------------------------------------------------------------------------------ the kernel
@@ -911,8 +853,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
     ticket = __shfl_sync(kFull, ticket, 0);
     while (ticket < total) {
         uint32_t next_ticket = 0;
-        if (!process_fed(p, mbar, slot, ticket, lane, false, mbar_phase, next_ticket))
-            process_fed(p, mbar, slot, ticket, lane, true, mbar_phase, next_ticket);
+        process_fed(p, mbar, slot, ticket, lane, mbar_phase, next_ticket);
         ticket = __shfl_sync(kFull, next_ticket, 0);
     }
 }
@@ -1115,7 +1056,7 @@ bool output_ok(const sst_output *o) {
 }
 
 struct ScratchLayout {
-    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_ssnr,
+    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_mask, o_strip, o_adc, o_srec, o_ssnr,
         o_sadc, o_sseed, total;
 };
 ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
@@ -1130,9 +1071,8 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     L.o_ticket = 0;
     L.o_state = 256;
     // slow-path lists
-    L.o_rec = L.o_state + up(L.state_bytes);
-    L.o_mask = L.o_rec + up(2 * L.ents * cap_events);
-    L.o_strip = L.o_mask + up(4 * 4 * L.mwords * cap_events);
+    L.o_mask = L.o_state + up(L.state_bytes);
+    L.o_strip = L.o_mask + up(4 * L.mwords * cap_events);
     L.o_adc = L.o_strip + up(2 * L.ents * cap_events);
     // staging between the two kernels
     L.o_srec = L.o_adc + up(L.ents * cap_events);
@@ -1173,7 +1113,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         const ScratchLayout Ln = scratch_layout(ctx, want);
         uint8_t *mem = nullptr;
         SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&mem), Ln.total, ctx->pool, st));
-        if (!cu_ok(ctx, cudaMemsetAsync(mem, 0, Ln.o_rec, st))) {  // ticket counter and states
+        if (!cu_ok(ctx, cudaMemsetAsync(mem, 0, Ln.o_mask, st))) {  // ticket counter and states
             cudaFreeAsync(mem, st);
             return SST_ERR_CUDA;
         }
@@ -1189,7 +1129,6 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
     kp.ticket_base = sl->ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
-    kp.g_rec = reinterpret_cast<uint16_t *>(blk + L.o_rec);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
     kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
     kp.g_adc = blk + L.o_adc;
@@ -1227,7 +1166,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         // a launch that did not happen must not leave the stream's ticket counter and the host's
         // copy of it apart: start the stream's scratch over (stream-ordered, like everything else)
         cu_ok(ctx, err);
-        cudaMemsetAsync(blk, 0, L.o_rec, st);
+        cudaMemsetAsync(blk, 0, L.o_mask, st);
         sl->ticket_base = 0;
         return SST_ERR_CUDA;
     }
