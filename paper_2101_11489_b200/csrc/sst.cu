@@ -102,7 +102,8 @@ struct KParams {
     // global scratch of the slow path, one slice set per event
     uint16_t *g_strip;
     uint8_t *g_adc;
-    uint32_t *g_mask;  // g_mwords per event
+    uint32_t *g_rec;   // slow-path cluster records
+    uint32_t *g_mask;  // 4 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
     uint4 *s_rec;     // per accepted cluster {module, first | width << 16, charge, first moment}
@@ -326,6 +327,42 @@ __device__ __forceinline__ void scan_runs3(const uint8_t *rp, FedCtx &c, uint32_
     }
 }
 
+// Bits smeared towards lower entries along the links, inside one 32-entry word: bit e of the
+// result is set iff some bit s >= e of x is set with link bits e+1 .. s all set (link bit i:
+// entry i continues the candidate of entry i-1).  Five doubling steps.
+__device__ __forceinline__ uint32_t smear_down(uint32_t x, uint32_t g) {
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+        x |= (x & g) >> s;
+        g &= g << s;
+    }
+    return x;
+}
+
+// Cluster acceptance, the defining form (reading s15): Q^2 >= t_cl^2 * n2 with n2 the
+// double sum of noise^2 over the candidate's strips taken strictly left to right (noise^2 is
+// exact in double, so the fused multiply-add rounds exactly like a separate multiply and add).
+// The noise is gathered again from the calibration: this runs only for candidates that cross a
+// chunk boundary of the sweep and land within rounding distance of the threshold, and for the
+// optional S/N output.
+__device__ __noinline__ double n2_sequential(const float2 *cal, const uint16_t *strip_l, uint32_t head, uint32_t w) {
+    double n2 = 0.0;
+#pragma unroll 1
+    for (uint32_t i = 0; i < w; ++i) {
+        const double d = static_cast<double>(__ldg(&cal[strip_l[head + i] & 0x7fffu].x));
+        n2 = __fma_rn(d, d, n2);
+    }
+    return n2;
+}
+__device__ __noinline__ bool accept_exact(const float2 *cal, const uint16_t *strip_l, uint32_t head, uint32_t w,
+                                          uint32_t Q, double tcl2) {
+    const double lhs = static_cast<double>(Q) * static_cast<double>(Q);
+    return lhs >= __dmul_rn(tcl2, n2_sequential(cal, strip_l, head, w));
+}
+__device__ __noinline__ float snr_exact(const float2 *cal, const uint16_t *strip_l, uint32_t head, uint32_t w, int Q) {
+    return static_cast<float>(static_cast<double>(Q) / sqrt(n2_sequential(cal, strip_l, head, w)));
+}
+
 // Fast-path layout of a warp's slot: offset of the strip-id list.  The payload (A bytes, the ADC
 // list is squeezed into its first P16 bytes) is followed by a gap when the dense SoA is wanted, so
 // that the 2048-byte window fits between the ADC list and the strip ids.
@@ -338,9 +375,11 @@ __device__ __forceinline__ uint32_t fast_strip_base(uint32_t A, uint32_t P16, bo
 // structure of arrays of PAPER.md:31: one entry per recorded strip).  kFast: lists, masks and the
 // candidate list live in the warp's shared-memory slot and the payload is staged there (the ADC
 // list is the payload squeezed in place); else they live in this FED's slice of the global
-// scratch and rp is whatever holds the payload.
+// scratch and rp is whatever holds the payload.  Returns false (fast path only) when the cluster
+// records outgrow the slot: the FED is then redone on the slow path (nothing has been published
+// and every output written so far is rewritten identically).
 template <bool kFast>
-__device__ __forceinline__ void fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, const FedCtx &c,
+__device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, const FedCtx &c,
                                           const int lane, uint32_t &next_ticket) {
     const uint32_t f = c.f, P = c.P;
     const EventDesc &E = p.ev[c.ev];
@@ -352,24 +391,37 @@ __device__ __forceinline__ void fed_lists(const KParams &p, uint8_t *slot, const
     uint32_t *const ktab = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
     uint16_t *strip_l;
     uint8_t *adc_l;
-    uint32_t *mS;               // seed mask, one bit per list entry (kept when the seed-index array is wanted)
+    // bit masks over the list entries: seeds; links, later heads of accepted clusters; ends, later
+    // members of accepted clusters; per-word prefix counts
+    uint32_t *mS, *mH, *mA, *mP, *rec;
+    uint32_t rec_cap;           // cluster records besides the end sentinel
     uint8_t *window = nullptr;  // 2048 bytes for the dense SoA assembly, free once the lists are complete
     if (kFast) {
         // [0, A): the payload; the ADC list takes its place ([0, P)), the rest (grown by a gap to
-        // 2048 bytes when the dense SoA is wanted) holds the window.  Behind it the strip ids
-        // (2P bytes) and the seed mask.
+        // 2048 bytes when the dense SoA is wanted) holds the window and then the cluster records.
+        // Behind it the strip ids (2P bytes) and the masks.
         const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (P + 15u) & ~15u;
         const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
         adc_l = slot;
         strip_l = reinterpret_cast<uint16_t *>(slot + S0);
         mS = reinterpret_cast<uint32_t *>(slot + ((S0 + 2u * P + 15u) & ~15u));
+        mH = mS + (nw + 2);
+        mA = mH + (nw + 2);
+        mP = mA + (nw + 2);
+        rec = reinterpret_cast<uint32_t *>(slot + P16);
+        rec_cap = (S0 - P16) / 4u - 1u;
         window = slot + P16;
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
         strip_l = p.g_strip + eb + slice;
         adc_l = p.g_adc + eb + slice;
-        mS = p.g_mask + static_cast<size_t>(c.ev) * p.g_mwords + (slice >> 5) + 4u * f;
+        rec = p.g_rec + eb + slice;
+        mS = p.g_mask + static_cast<size_t>(c.ev) * 4u * p.g_mwords + (slice >> 5) + 4u * f;
+        mH = mS + p.g_mwords;
+        mA = mH + p.g_mwords;
+        mP = mA + p.g_mwords;
+        rec_cap = 0xffffffffu;
         // the slot is free up to the channel table unless the payload is staged in it
         const uint32_t A = (c.fed_size + 15u) & ~15u;
         if (rp != slot) window = slot;
@@ -507,173 +559,257 @@ __device__ __forceinline__ void fed_lists(const KParams &p, uint8_t *slot, const
         __syncwarp();
     }
 
-    // ---------------------------------------------------------------- a3..a7: one loop over the list
-    // Lane per entry, a word of 32 entries per step, in two stages that are one word apart:
-    //
-    // stage A (word w+1): one 8-byte gather of {noise, gain}; exact >= tests (a3: active, seed);
-    //   the link to the previous entry (same module, adjacent strip, both active); the
-    //   gain-corrected ADC, which replaces the raw one in the list; ballots give the word's
-    //   active / linked / seed masks (a4: the seed mask is what the seed-index array is made from).
-    // stage B (word w): a candidate is a maximal run of linked active entries.  Its first lane
-    //   collects the run's charge, first moment and noise^2 from the lanes behind it by shuffles,
-    //   one strip per step, left to right -- the double sum of noise^2 is the oracle's (reading
-    //   s15).  A candidate that runs past the word's end is carried to lane 0 of the next word
-    //   (stage A of that word has already said whether it continues).  Where a candidate ends it is
-    //   tested once (a5: leftmost-seed ownership is implicit; a6: the cluster test) and, if
-    //   accepted, staged in FED-local order: record {module, first | width << 16, charge, first
-    //   moment} at its cluster index (ballot) and its corrected ADCs at the running byte offset.
-    // sst_emit_kernel turns the FED totals into offsets and moves everything to its
-    // (module, first strip)-ordered place.
-    const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
-    const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
-    uint32_t fed_seed = 0, fed_cl = 0, fed_adc = 0;
-    if (nw) {
-        const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
-        uint8_t *const sa = p.s_adc + ab;
-        const bool want_seeds = o.seed_idx != nullptr;
-        const uint32_t last = P - 1u;
-        // list entries and calibration of the word stage A takes next (issued a step ahead)
-        uint32_t sv_n = strip_l[min(static_cast<uint32_t>(lane), last)], av_n = adc_l[min(static_cast<uint32_t>(lane), last)];
-        float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
-        uint32_t link_carry = 0;  // strip id | active << 15 of the entry before stage A's word
-        // stage A's results for the word stage B takes next
-        uint32_t a_sv = 0, a_q = 0, a_bA = 0, a_bL = 0, a_bS = 0;
-        float a_nz = 0.0f;
-        // the candidate that is open at the start of stage B's word (valid when its link bit 0 is set)
-        uint32_t cQ = 0, cM = 0, cLen = 0, cSid = 0, cHd = 0, cSeed = 0;
-        double cN = 0.0;
+    // ---------------------------------------------------------------- a3..a6: one sweep over the lists
+    // Lane per CHUNK of consecutive entries, walked serially: active/seed tests, link to the previous
+    // entry, and the running (charge, noise^2, seed) of the open candidate are thread-local, so a
+    // candidate inside one chunk is decided exactly as the oracle does (double sum of noise^2,
+    // left to right) with no cross-lane traffic.  What comes out are bits, collected in registers
+    // for the 32-entry word the lane is in and flushed when it leaves the word: links, seeds, and
+    // the last entries of accepted clusters.  A candidate that crosses a chunk boundary is put
+    // together afterwards from the tail partial of one lane and the lead partials of the next lanes.
+    uint32_t *const mL = mH, *const mE = mA;  // links become heads and ends become members further down
 #pragma unroll 1
-        for (uint32_t w = 0; w <= nw; ++w) {
-            // ---- stage B inputs: the word stage A produced in the previous step
-            const uint32_t sv = a_sv, q = a_q, bA = a_bA, bL = a_bL, bS = a_bS;
-            const float nz = a_nz;
-            // ---- stage A on word w
-            if (w < nw) {
-                const uint32_t e = w * 32u + lane;
-                const uint32_t svw = sv_n;
-                const uint32_t av = e < P ? av_n : 0u;  // (the entries past the end repeat the last one)
+    for (uint32_t w = lane; w < nw + 2; w += 32) {
+        mS[w] = 0;
+        mL[w] = 0;
+        mE[w] = 0;
+    }
+    const uint32_t Lc = ((P + 31u) >> 5) | 1u;  // odd: the lanes' list reads fall into different banks
+    const bool want_seeds = o.seed_idx != nullptr;
+    uint32_t n_seed_lane = 0;
+    const uint32_t e0 = min(lane * Lc, P), e1 = min(e0 + Lc, P);
+    {
+        // is the entry before the chunk active?  (its raw ADC is read before any lane overwrites it)
+        bool open = false;
+        uint32_t prev_s = 0;
+        if (e0 > 0) {
+            const uint32_t sp = strip_l[e0 - 1], ap = adc_l[e0 - 1];
+            prev_s = sp & 0x7fffu;
+            if (ap) open = ge_exact(static_cast<float>(ap), p.t_ch, ld_calib(cal + prev_s, pol_last).x);
+        }
+        __syncwarp();
+        bool lead = open;  // an open candidate at the chunk start began in an earlier chunk
+        uint32_t hd = 0, Q = 0;
+        double N = 0.0;
+        bool seed = false;
+        uint32_t lQ = 0, lEnd = 0;  // lead partial: the part of an earlier candidate inside this chunk
+        double lN = 0.0;
+        bool lSeed = false, lClosed = false;
+        uint32_t aL = 0, aE = 0, aS = 0;  // bits of the word the lane is in
+        auto flush = [&](uint32_t wi) {
+            if (aL) atomicOr(&mL[wi], aL);
+            if (aE) atomicOr(&mE[wi], aE);
+            if (aS) {
+                n_seed_lane += __popc(aS);
+                if (want_seeds) atomicOr(&mS[wi], aS);
+            }
+            aL = aE = aS = 0;
+        };
+        if (e0 < e1) {
+            // software pipeline of depth one: the next entry's list reads and calibration gather
+            // are issued before the current entry is worked on
+            const uint32_t elast = e1 - 1u;
+            uint32_t sv_n = strip_l[e0], av_n = adc_l[e0];
+            float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
+#pragma unroll 1
+            for (uint32_t e = e0; e < e1; ++e) {
+                const uint32_t sv = sv_n, av = av_n;
                 const float2 cv = cv_n;
                 {
-                    const uint32_t en = min(e + 32u, last);
+                    const uint32_t en = min(e + 1u, elast);
                     sv_n = strip_l[en];
                     av_n = adc_l[en];
                     cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
                 }
-                const uint32_t s15 = svw & 0x7fffu;
+                const uint32_t s15 = sv & 0x7fffu;
                 const float af = static_cast<float>(av);
                 const bool is_act = av != 0 && ge_exact(af, p.t_ch, cv.x);
                 const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
-                const uint32_t qc = is_act ? gain_correct(af, cv.y) : 0u;
-                if (is_act) adc_l[e] = static_cast<uint8_t>(qc);
-                const uint32_t pk = s15 | (static_cast<uint32_t>(is_act) << 15);
-                uint32_t pv = __shfl_up_sync(kFull, pk, 1);
-                if (lane == 0) pv = link_carry;
-                // (pv: active bit set and strip id one below, in one comparison)
-                const bool is_link = is_act && !(svw & 0x8000u) && pv == ((s15 - 1u) | 0x8000u);
-                a_bA = __ballot_sync(kFull, is_act);
-                a_bL = __ballot_sync(kFull, is_link);
-                a_bS = __ballot_sync(kFull, is_seed);
-                link_carry = __shfl_sync(kFull, pk, 31);
-                a_sv = s15;
-                a_q = qc;
-                a_nz = cv.x;
-                fed_seed += __popc(a_bS);
-                if (want_seeds && lane == 0) mS[w] = a_bS;
+                // this entry continues the candidate of the previous one
+                const bool is_link = is_act && open && !(sv & 0x8000u) && s15 == prev_s + 1u;
+                if (open && !is_link) {  // the open candidate ended with entry e - 1
+                    if (lead) {
+                        lQ = Q; lN = N; lSeed = seed; lEnd = e - 1u; lClosed = true;
+                        lead = false;
+                    } else if (seed) {
+                        const double dq = static_cast<double>(Q);
+                        if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) aE |= 1u << ((e - 1u) & 31u);
+                    }
+                }
+                if ((e & 31u) == 0 && e > e0) flush((e - 1u) >> 5);  // entry e - 1 closed its word
+                if (is_act) {
+                    if (!is_link) {
+                        hd = e; Q = 0; N = 0.0; seed = false;
+                    }
+                    const uint32_t q = gain_correct(af, cv.y);
+                    adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
+                    Q += q;
+                    const double d = static_cast<double>(cv.x);
+                    N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
+                    seed = seed || is_seed;
+                }
+                aL |= static_cast<uint32_t>(is_link) << (e & 31u);
+                aS |= static_cast<uint32_t>(is_seed) << (e & 31u);
+                open = is_act;
+                prev_s = s15;
+            }
+        }
+        bool pend = false;  // an open candidate that began in this chunk and runs on
+        if (open) {
+            if (e1 == P) {  // the lists end here
+                if (lead) {
+                    lQ = Q; lN = N; lSeed = seed; lEnd = P - 1u; lClosed = true;
+                } else if (seed) {
+                    const double dq = static_cast<double>(Q);
+                    if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) aE |= 1u << ((P - 1u) & 31u);
+                }
+            } else if (lead) {  // the whole chunk lies inside a candidate of an earlier chunk
+                lQ = Q; lN = N; lSeed = seed; lEnd = e1 - 1u; lClosed = false;
             } else {
-                a_bA = a_bL = a_bS = 0;
+                pend = true;
             }
-            if (w == 0) continue;
-            // ---- stage B on word w - 1
-            const uint32_t wb = w - 1u;
-            const bool cont_next = a_bL & 1u;     // the entry behind this word continues its last candidate
-            const bool virt = (bL & 1u) && lane == 0;  // lane 0 continues the carried candidate
-            const bool is_head = (((bA & ~bL) >> lane) & 1u) || virt;
-            // consecutive link bits behind this lane: the rest of its candidate inside the word
-            const uint32_t behind = lane == 31 ? 0u : bL >> (lane + 1);
-            const uint32_t n1 = __ffs(~behind) - 1u;
-            int Q = static_cast<int>(q), M = 0;
-            double N = 0.0;
-            uint32_t j0 = 0;  // position of this lane's strip inside its candidate
-            if (virt) {
-                j0 = cLen;
-                Q += static_cast<int>(cQ);
-                M = static_cast<int>(cM) + static_cast<int>(cLen * q);
-                N = cN;
-            }
-            {
-                const double d = static_cast<double>(nz);
-                N = __fma_rn(d, d, N);  // exact square, one rounding
-            }
-            const uint32_t trips = __reduce_max_sync(kFull, is_head ? n1 : 0u);
-#pragma unroll 1
-            for (uint32_t j = 1; j <= trips; ++j) {
-                const uint32_t qj = __shfl_down_sync(kFull, q, j);
-                const float nj = __shfl_down_sync(kFull, nz, j);
-                if (j <= n1) {
-                    Q += static_cast<int>(qj);
-                    M += static_cast<int>((j0 + j) * qj);
-                    const double d = static_cast<double>(nj);
-                    N = __fma_rn(d, d, N);
+        }
+        if (e0 < e1) flush((e1 - 1u) >> 5);
+        // candidates across chunk boundaries: tail + lead partials of the following lanes.  The sum
+        // of partial sums is not the oracle's left-to-right sum; they differ by < (2w + 32) * 2^-53
+        // relative, so the comparison is taken from it only outside that band.
+        for (uint32_t dd = 1; __any_sync(kFull, pend); ++dd) {
+            const uint32_t pk = __shfl_down_sync(kFull, lQ | (static_cast<uint32_t>(lSeed) << 30) |
+                                                            (static_cast<uint32_t>(lClosed) << 31), dd);
+            const uint32_t end_s = __shfl_down_sync(kFull, lEnd, dd);
+            const double n_s = __shfl_down_sync(kFull, lN, dd);
+            if (pend) {
+                if (lane + dd > 31u) {
+                    pend = false;  // cannot happen: the last lane's chunk ends the lists
+                } else {
+                    Q += pk & 0x3fffffffu;
+                    N += n_s;
+                    seed = seed || ((pk >> 30) & 1u);
+                    if (pk >> 31) {
+                        pend = false;
+                        if (seed) {
+                            const uint32_t wd = end_s - hd + 1u;
+                            const double dq = static_cast<double>(Q);
+                            const double lhs = __dmul_rn(dq, dq), rhs = __dmul_rn(p.tcl2, N);
+                            bool acc;
+                            if (fabs(lhs - rhs) > rhs * (static_cast<double>(wd + 16u) * 0x1p-51)) acc = lhs > rhs;
+                            else acc = accept_exact(cal, strip_l, hd, wd, Q, p.tcl2);
+                            if (acc) atomicOr(&mE[end_s >> 5], 1u << (end_s & 31u));
+                        }
+                    }
                 }
-            }
-            const bool to_end = lane + n1 == 31u;
-            const bool open = is_head && to_end && cont_next;
-            const uint32_t segmask = ((2u << n1) - 1u) << lane;  // (n1 <= 31 - lane)
-            const bool seeded = (bS & segmask) != 0 || (virt && cSeed);
-            const uint32_t wd = j0 + 1u + n1;
-            bool acc = false;
-            if (is_head && !open && seeded) {
-                const double dq = static_cast<double>(Q);
-                acc = __dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N);
-            }
-            const uint32_t bal = __ballot_sync(kFull, acc);
-            if (bal) {
-                const uint32_t macc = __reduce_or_sync(kFull, acc ? segmask : 0u);  // this word's entries in accepted clusters
-                const uint32_t extra = (bal & 1u) && (bL & 1u) ? cLen : 0u;         // + the carried part of lane 0's
-                if (extra) {  // its ADCs of the earlier words come out of the list
-                    __syncwarp();
-#pragma unroll 1
-                    for (uint32_t j = lane; j < extra; j += 32u) sa[fed_adc + j] = adc_l[cHd + j];
-                }
-                if ((macc >> lane) & 1u) sa[fed_adc + extra + __popc(macc & lt)] = static_cast<uint8_t>(q);
-                if (acc) {
-                    const uint32_t st0 = virt ? cSid : sv;
-                    const uint2 cm = __ldg(cinfo + (st0 >> 8));
-                    const uint32_t first = st0 - (cm.y & 0xffu) * kStrip;
-                    const uint32_t kc = fed_cl + __popc(bal & lt);
-                    // (the barycenter first + M / Q is formed by sst_emit_kernel)
-                    p.s_rec[sb + kc] = make_uint4(cm.x, first | (wd << 16), static_cast<uint32_t>(Q), static_cast<uint32_t>(M));
-                    if (o.cl_snr) p.s_snr[sb + kc] = static_cast<float>(static_cast<double>(Q) / sqrt(N));
-                }
-                fed_cl += __popc(bal);
-                fed_adc += extra + __popc(macc);
-            }
-            // the candidate that stays open moves to lane 0 of the next word
-            const uint32_t bo = __ballot_sync(kFull, open);
-            if (bo) {
-                const int src = __ffs(bo) - 1;
-                cQ = __shfl_sync(kFull, static_cast<uint32_t>(Q), src);
-                cM = __shfl_sync(kFull, static_cast<uint32_t>(M), src);
-                cN = __shfl_sync(kFull, N, src);
-                cLen = __shfl_sync(kFull, wd, src);
-                cSeed = __shfl_sync(kFull, static_cast<uint32_t>(seeded), src);
-                const uint32_t sid_h = __shfl_sync(kFull, virt ? cSid : sv, src);
-                const uint32_t hd_h = __shfl_sync(kFull, virt ? cHd : wb * 32u + lane, src);
-                cSid = sid_h;
-                cHd = hd_h;
             }
         }
     }
+    __syncwarp();
 
-    // ---------------------------------------------------------------- a7, first half: publish
-    // The FED's counts go into its state word and the next ticket is drawn.
+    // ---------------------------------------------------------------- a5: members and heads
+    // Lane per mask word: the end bits of the accepted clusters are smeared down along the links
+    // (across word boundaries until nothing changes: a second round only happens for clusters
+    // wider than a word), which gives the member mask; a member that is not linked is a head
+    // (leftmost-seed ownership is implicit: one head per maximal run).
+    {
+        uint32_t carry_up = 0;  // (x & link & 1) of the word just above the group
+#pragma unroll 1
+        for (uint32_t g = (nw + 31u) >> 5; g-- > 0;) {  // groups of 32 words, from the top
+            const uint32_t w = g * 32u + lane;
+            const bool in = w < nw;
+            const uint32_t lw = in ? mL[w] : 0u;
+            uint32_t x = smear_down(in ? mE[w] : 0u, lw);
+            for (;;) {
+                uint32_t up = __shfl_down_sync(kFull, x & lw & 1u, 1);
+                if (lane == 31) up = carry_up;
+                const bool grow = up && !(x >> 31);
+                if (grow) x = smear_down(x | 0x80000000u, lw);
+                if (!__any_sync(kFull, grow)) break;
+            }
+            __syncwarp();
+            if (in) {
+                mA[w] = x;
+                mH[w] = x & ~lw;
+            }
+            carry_up = __shfl_sync(kFull, x & lw & 1u, 0);
+        }
+    }
+    __syncwarp();
+
+    // ---------------------------------------------------------------- counts and cluster records
+    // lane per mask word: exclusive prefix of (accepted heads, accepted members) per word, then
+    // every head gets its record {head entry, offset of its ADCs}
+    uint32_t fed_cl = 0, fed_adc = 0, fed_seed = 0;
+    {
+        uint32_t run = 0;  // heads << 16 | members
+#pragma unroll 1
+        for (uint32_t w0 = 0; w0 < nw; w0 += 32) {
+            const uint32_t w = w0 + lane;
+            uint32_t v = 0;
+            if (w < nw) v = (__popc(mH[w]) << 16) | __popc(mA[w]);
+            const uint32_t incl = warp_incl_scan(v, lane);
+            if (w < nw) mP[w] = run + incl - v;
+            run += __shfl_sync(kFull, incl, 31);
+        }
+        fed_seed = __reduce_add_sync(kFull, n_seed_lane);
+        fed_cl = run >> 16;
+        fed_adc = run & 0xffffu;
+        if (kFast && fed_cl > rec_cap) return false;
+        __syncwarp();
+#pragma unroll 1
+        for (uint32_t w = lane; w < nw; w += 32) {
+            uint32_t mh = mH[w];
+            const uint32_t ma = mA[w], pre = mP[w];
+            uint32_t k = pre >> 16;
+            while (mh) {
+                const uint32_t b = __ffs(mh) - 1u;
+                mh &= mh - 1u;
+                rec[k++] = (w * 32u + b) | (((pre & 0xffffu) + __popc(ma & ((1u << b) - 1u))) << 16);
+            }
+        }
+        if (P && lane == 0) rec[fed_cl] = fed_adc << 16;  // end sentinel: widths are offset differences
+    }
+    __syncwarp();
+
+    // ---------------------------------------------------------------- a7, first half: publish + stage
+    // The FED's counts go into its state word; its clusters, cluster ADCs and seeds are staged in
+    // FED-local order in global scratch.  sst_emit_kernel, launched behind this kernel on the same
+    // stream, turns the counts into offsets and moves everything to its (module, first strip)
+    // ordered place -- no warp ever waits for another one.
+    const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
+    const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
     if (lane == 0) {
         p.fed_state[static_cast<size_t>(c.ev) * p.n_feds + f] =
             (static_cast<unsigned long long>(c.overrun) << kShOver) |
             (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
             (static_cast<unsigned long long>(fed_seed) << kShSeed) |
             (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl;
+        // next FED of this warp: the ticket arrives while the staging runs
         next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
+    }
+    {
+        // cluster records: lane per cluster, consecutive lanes write consecutive records
+        const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
+        uint8_t *const sa = p.s_adc + ab;  // the FED's cluster ADCs, in order
+#pragma unroll 1
+        for (uint32_t k0 = 0; k0 < fed_cl; k0 += 32) {
+            const uint32_t k = k0 + lane;
+            if (k < fed_cl) {
+                const uint32_t r0 = rec[k], r1 = rec[k + 1];
+                const uint32_t hd = r0 & 0xffffu, off = r0 >> 16, wd = (r1 >> 16) - off;
+                const uint32_t st0 = strip_l[hd] & 0x7fffu;
+                const uint2 cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
+                int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
+#pragma unroll 1
+                for (uint32_t j = 0; j < wd; ++j) {
+                    const int q = adc_l[hd + j];
+                    Q += q;
+                    M += static_cast<int>(j) * q;
+                    sa[off + j] = static_cast<uint8_t>(q);  // neighbouring lanes write neighbouring bytes
+                }
+                const uint32_t first = st0 - (cm.y & 0xffu) * kStrip;
+                // (the barycenter first + M / Q is formed by sst_emit_kernel)
+                p.s_rec[sb + k] = make_uint4(cm.x, first | (wd << 16), static_cast<uint32_t>(Q), static_cast<uint32_t>(M));
+                if (o.cl_snr) p.s_snr[sb + k] = snr_exact(cal, strip_l, hd, wd, Q);
+            }
+        }
     }
     // a4: seed-index array (on request), FED-local strip ids
     if (o.seed_idx) {
@@ -685,12 +821,14 @@ __device__ __forceinline__ void fed_lists(const KParams &p, uint8_t *slot, const
             k0 += __popc(sw);
         }
     }
+    return true;
 }
 
 // ------------------------------------------------------------------------------ one FED, one warp
-__device__ __forceinline__ void process_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot,
-                                            const uint32_t ticket, const int lane, uint32_t &mbar_phase,
-                                            uint32_t &next_ticket) {
+// Returns false when the FED has to be redone with force_slow (see fed_lists).
+__device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot,
+                                            const uint32_t ticket, const int lane, const bool force_slow,
+                                            uint32_t &mbar_phase, uint32_t &next_ticket) {
     FedCtx c;
     c.ticket = ticket;
     // FED-major order: the same FED of all the launch's events back to back, so the FED's slab of
@@ -822,13 +960,12 @@ __device__ __forceinline__ void process_fed(const KParams &p, unsigned long long
     c.R = tot >> 16;
     __syncwarp();
 
-    // fast path: window, strip ids and seed mask fit behind the ADC list
+    // fast path: window / cluster records, strip ids and masks fit behind the ADC list
     const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (c.P + 15u) & ~15u;
     const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
-    if (staged && ((S0 + 2u * c.P + 15u) & ~15u) + 4u * (((c.P + 31u) >> 5) + 1u) + kTabBytes <= p.slot_bytes)
-        fed_lists<true>(p, slot, slot, c, lane, next_ticket);
-    else
-        fed_lists<false>(p, slot, rp, c, lane, next_ticket);
+    if (!force_slow && staged && ((S0 + 2u * c.P + 15u) & ~15u) + 16u * (((c.P + 31u) >> 5) + 2u) + kTabBytes <= p.slot_bytes)
+        return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
+    return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
 
 // ------------------------------------------------------------------------------ the kernel
@@ -853,7 +990,8 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
     ticket = __shfl_sync(kFull, ticket, 0);
     while (ticket < total) {
         uint32_t next_ticket = 0;
-        process_fed(p, mbar, slot, ticket, lane, mbar_phase, next_ticket);
+        if (!process_fed(p, mbar, slot, ticket, lane, false, mbar_phase, next_ticket))
+            process_fed(p, mbar, slot, ticket, lane, true, mbar_phase, next_ticket);
         ticket = __shfl_sync(kFull, next_ticket, 0);
     }
 }
@@ -1056,7 +1194,7 @@ bool output_ok(const sst_output *o) {
 }
 
 struct ScratchLayout {
-    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_mask, o_strip, o_adc, o_srec, o_ssnr,
+    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_ssnr,
         o_sadc, o_sseed, total;
 };
 ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
@@ -1071,8 +1209,9 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     L.o_ticket = 0;
     L.o_state = 256;
     // slow-path lists
-    L.o_mask = L.o_state + up(L.state_bytes);
-    L.o_strip = L.o_mask + up(4 * L.mwords * cap_events);
+    L.o_rec = L.o_state + up(L.state_bytes);
+    L.o_mask = L.o_rec + up(4 * L.ents * cap_events);
+    L.o_strip = L.o_mask + up(4 * 4 * L.mwords * cap_events);
     L.o_adc = L.o_strip + up(2 * L.ents * cap_events);
     // staging between the two kernels
     L.o_srec = L.o_adc + up(L.ents * cap_events);
@@ -1113,7 +1252,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         const ScratchLayout Ln = scratch_layout(ctx, want);
         uint8_t *mem = nullptr;
         SST_CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&mem), Ln.total, ctx->pool, st));
-        if (!cu_ok(ctx, cudaMemsetAsync(mem, 0, Ln.o_mask, st))) {  // ticket counter and states
+        if (!cu_ok(ctx, cudaMemsetAsync(mem, 0, Ln.o_rec, st))) {  // ticket counter and states
             cudaFreeAsync(mem, st);
             return SST_ERR_CUDA;
         }
@@ -1129,6 +1268,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
     kp.ticket_base = sl->ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
+    kp.g_rec = reinterpret_cast<uint32_t *>(blk + L.o_rec);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
     kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
     kp.g_adc = blk + L.o_adc;
@@ -1166,7 +1306,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         // a launch that did not happen must not leave the stream's ticket counter and the host's
         // copy of it apart: start the stream's scratch over (stream-ordered, like everything else)
         cu_ok(ctx, err);
-        cudaMemsetAsync(blk, 0, L.o_mask, st);
+        cudaMemsetAsync(blk, 0, L.o_rec, st);
         sl->ticket_base = 0;
         return SST_ERR_CUDA;
     }
