@@ -55,7 +55,7 @@
 #define SST_SLAB_AHEAD 2
 #endif
 #ifndef SST_EMIT_CTAS
-#define SST_EMIT_CTAS 6
+#define SST_EMIT_CTAS 8
 #endif
 #ifndef SST_HOST_CHUNK
 #define SST_HOST_CHUNK 4
@@ -595,25 +595,37 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         uint32_t lQ = 0, lEnd = 0;  // lead partial: the part of an earlier candidate inside this chunk
         double lN = 0.0;
         bool lSeed = false, lClosed = false;
-        uint32_t aL = 0, aE = 0, aS = 0;  // bits of the word the lane is in
-        auto flush = [&](uint32_t wi) {
-            if (aL) atomicOr(&mL[wi], aL);
-            if (aE) atomicOr(&mE[wi], aE);
-            if (aS) {
-                n_seed_lane += __popc(aS);
-                if (want_seeds) atomicOr(&mS[wi], aS);
-            }
-            aL = aE = aS = 0;
+        // Bits are collected per lane in CHUNK-local positions (bit i = entry e0 + i), 64 entries at a
+        // time, and shifted into the masks by all lanes together (the step counter is uniform):
+        // links, seeds, and the last entries of accepted clusters.
+        uint32_t aL = 0, aE = 0, aS = 0;     // the 32 positions being filled
+        uint32_t aL0 = 0, aE0 = 0, aS0 = 0;  // the 32 before them
+        auto flush64 = [&](uint32_t ebase) {  // local bit 0 = entry ebase; lower half in a?0, upper in a?
+            const uint32_t wi = ebase >> 5, sh = ebase & 31u;
+            auto put = [&](uint32_t *m, uint32_t lo, uint32_t hi) {
+                const uint32_t w0 = lo << sh, w1 = __funnelshift_l(lo, hi, sh), w2 = sh ? hi >> (32u - sh) : 0u;
+                if (w0) atomicOr(&m[wi], w0);
+                if (w1) atomicOr(&m[wi + 1], w1);
+                if (w2) atomicOr(&m[wi + 2], w2);
+            };
+            put(mL, aL0, aL);
+            put(mE, aE0, aE);
+            n_seed_lane += __popc(aS0) + __popc(aS);
+            if (want_seeds) put(mS, aS0, aS);
+            aL = aE = aS = aL0 = aE0 = aS0 = 0;
         };
-        if (e0 < e1) {
+        if (P) {  // (uniform)
             // software pipeline of depth one: the next entry's list reads and calibration gather
             // are issued before the current entry is worked on
-            const uint32_t elast = e1 - 1u;
-            uint32_t sv_n = strip_l[e0], av_n = adc_l[e0];
+            const uint32_t elast = min(max(e1, e0 + 1u), P) - 1u;
+            uint32_t sv_n = strip_l[min(e0, P - 1u)], av_n = adc_l[min(e0, P - 1u)];
             float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
+            uint32_t bit = 1u;  // 1 << (step & 31)
 #pragma unroll 1
-            for (uint32_t e = e0; e < e1; ++e) {
-                const uint32_t sv = sv_n, av = av_n;
+            for (uint32_t i = 0; i < Lc; ++i) {  // (uniform: every lane takes Lc steps, the last lanes idle in some)
+                const uint32_t e = e0 + i;
+                const bool in = e < e1;
+                const uint32_t sv = sv_n, av = in ? av_n : 0u;
                 const float2 cv = cv_n;
                 {
                     const uint32_t en = min(e + 1u, elast);
@@ -627,16 +639,19 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
                 // this entry continues the candidate of the previous one
                 const bool is_link = is_act && open && !(sv & 0x8000u) && s15 == prev_s + 1u;
-                if (open && !is_link) {  // the open candidate ended with entry e - 1
+                if (in && open && !is_link) {  // the open candidate ended with entry e - 1
                     if (lead) {
                         lQ = Q; lN = N; lSeed = seed; lEnd = e - 1u; lClosed = true;
                         lead = false;
                     } else if (seed) {
                         const double dq = static_cast<double>(Q);
-                        if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) aE |= 1u << ((e - 1u) & 31u);
+                        if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) {  // bit of entry e - 1
+                            if (bit != 1u) aE |= bit >> 1;
+                            else if (i & 32u) aE0 |= 0x80000000u;
+                            else atomicOr(&mE[(e - 1u) >> 5], 1u << ((e - 1u) & 31u));  // its 64 positions are flushed already
+                        }
                     }
                 }
-                if ((e & 31u) == 0 && e > e0) flush((e - 1u) >> 5);  // entry e - 1 closed its word
                 if (is_act) {
                     if (!is_link) {
                         hd = e; Q = 0; N = 0.0; seed = false;
@@ -648,10 +663,22 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
                     seed = seed || is_seed;
                 }
-                aL |= static_cast<uint32_t>(is_link) << (e & 31u);
-                aS |= static_cast<uint32_t>(is_seed) << (e & 31u);
-                open = is_act;
-                prev_s = s15;
+                if (is_link) aL |= bit;
+                if (is_seed) aS |= bit;
+                if (in) {
+                    open = is_act;
+                    prev_s = s15;
+                }
+                bit <<= 1;
+                if (bit == 0) {  // 32 steps done
+                    bit = 1u;
+                    if (i & 32u) {
+                        flush64(e0 + i - 63u);
+                    } else {
+                        aL0 = aL; aE0 = aE; aS0 = aS;
+                        aL = aE = aS = 0;
+                    }
+                }
             }
         }
         bool pend = false;  // an open candidate that began in this chunk and runs on
@@ -661,7 +688,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     lQ = Q; lN = N; lSeed = seed; lEnd = P - 1u; lClosed = true;
                 } else if (seed) {
                     const double dq = static_cast<double>(Q);
-                    if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) aE |= 1u << ((P - 1u) & 31u);
+                    if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) atomicOr(&mE[(P - 1u) >> 5], 1u << ((P - 1u) & 31u));
                 }
             } else if (lead) {  // the whole chunk lies inside a candidate of an earlier chunk
                 lQ = Q; lN = N; lSeed = seed; lEnd = e1 - 1u; lClosed = false;
@@ -669,7 +696,16 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 pend = true;
             }
         }
-        if (e0 < e1) flush((e1 - 1u) >> 5);
+        {   // what is left in the registers: Lc = 64 k + r steps, r < 64
+            const uint32_t r = Lc & 63u;
+            if (r) {
+                if (r < 32u) {  // only the lower half is in use, and it is still in the "being filled" set
+                    aL0 = aL; aE0 = aE; aS0 = aS;
+                    aL = aE = aS = 0;
+                }
+                flush64(e0 + (Lc - r));
+            }
+        }
         // candidates across chunk boundaries: tail + lead partials of the following lanes.  The sum
         // of partial sums is not the oracle's left-to-right sum; they differ by < (2w + 32) * 2^-53
         // relative, so the comparison is taken from it only outside that band.
@@ -1021,7 +1057,7 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
     const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
     // the first records are requested before the prefix is known
-    constexpr int kB = 4;
+    constexpr int kB = 2;
     uint4 r[kB];
 #pragma unroll
     for (int j = 0; j < kB; ++j)
