@@ -106,7 +106,8 @@ struct KParams {
     uint32_t *g_mask;  // 4 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
-    uint4 *s_rec;     // per accepted cluster {module, first | width << 16, charge, first moment}
+    uint4 *s_rec;     // per accepted cluster {module, first | width << 16, charge, barycenter}
+    uint32_t *s_off;  // offset of the cluster's ADCs inside its FED
     float *s_snr;
     uint8_t *s_adc;
     uint16_t *s_seed;
@@ -841,8 +842,10 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     sa[off + j] = static_cast<uint8_t>(q);  // neighbouring lanes write neighbouring bytes
                 }
                 const uint32_t first = st0 - (cm.y & 0xffu) * kStrip;
-                // (the barycenter first + M / Q is formed by sst_emit_kernel)
-                p.s_rec[sb + k] = make_uint4(cm.x, first | (wd << 16), static_cast<uint32_t>(Q), static_cast<uint32_t>(M));
+                // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
+                const float bary = __fadd_rn(static_cast<float>(first), __fdiv_rn(static_cast<float>(M), static_cast<float>(Q)));
+                p.s_rec[sb + k] = make_uint4(cm.x, first | (wd << 16), static_cast<uint32_t>(Q), __float_as_uint(bary));
+                p.s_off[sb + k] = off;
                 if (o.cl_snr) p.s_snr[sb + k] = snr_exact(cal, strip_l, hd, wd, Q);
             }
         }
@@ -1035,8 +1038,8 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
 // ------------------------------------------------------------------------------ a7, second half
 // One warp per (event, FED), behind sst_event_kernel on the same stream: sums the state words of
 // the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then moves the staged
-// records, cluster ADCs and seeds of the FED to their final place (a cluster's ADC offset is the
-// running sum of the widths).  Output capacity and the event totals are handled here.
+// records, cluster ADCs and seeds of the FED to their final place.  Output capacity and the event
+// totals are handled here.
 template <bool kPacked>
 __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __grid_constant__ KParams p) {
     const int lane = threadIdx.x & 31;
@@ -1048,20 +1051,9 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     constexpr bool packed = kPacked;  // every event of a launch is, or none
     const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
     const unsigned long long own = st[f];
-    const uint32_t fed_start = E.fed_offsets[f];
     const uint32_t fed_cl = static_cast<uint32_t>(own & 0x3fffull), fed_adc = static_cast<uint32_t>((own >> kShAdc) & 0x7fffull),
                    fed_seed = static_cast<uint32_t>((own >> kShSeed) & 0x7fffull),
                    fed_malf = static_cast<uint32_t>((own >> kShMalf) & 0x7full), fed_over = static_cast<uint32_t>((own >> kShOver) & 1ull);
-    // where sst_event_kernel staged this FED (a FED with bad offsets staged nothing: its counts
-    // are zero and the addresses below are never used)
-    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
-    const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
-    // the first records are requested before the prefix is known
-    constexpr int kB = 2;
-    uint4 r[kB];
-#pragma unroll
-    for (int j = 0; j < kB; ++j)
-        if (lane + 32 * j < fed_cl) r[j] = __ldcs(p.s_rec + sb + lane + 32 * j);
     // clusters | ADC bytes << 32 ; seeds | malformed << 32 (20 bits) | overrun << 52 (n_feds <= 4096)
     unsigned long long accA = 0, accB = 0, totA = 0;
     const uint32_t jend = packed ? p.n_feds : f;  // the packed layout needs the event's totals too
@@ -1096,48 +1088,47 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
     const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
     const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
                    b_over = static_cast<uint32_t>(accB >> 52);
+    // where sst_event_kernel staged this FED (a FED with bad offsets staged nothing: its counts
+    // are zero and the addresses below are never used)
+    const uint32_t fed_start = E.fed_offsets[f];
+    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
+    const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
     const unsigned long long pol_first = policy_evict_first();
 
     const bool all_fit = b_cl + fed_cl <= o.cap_clusters && b_adc + fed_adc <= o.cap_adc;
-    uint32_t lim = 0;       // ADC bytes of this FED that belong to clusters that fit
-    uint32_t run_adc = 0;   // ADC bytes of the FED's clusters before this group
+    uint32_t lim = 0;  // ADC bytes of this FED that belong to clusters that fit
     // the loop bodies first gather a few independent loads, then store: the kernel is a plain copy
     // and lives off loads in flight
+    constexpr int kB = 4;
 #pragma unroll 1
-    for (uint32_t kb = 0; kb < fed_cl; kb += 32 * kB) {  // (warp-uniform: the scans inside need every lane)
-        const uint32_t k0 = kb + lane;
+    for (uint32_t k0 = lane; k0 < fed_cl; k0 += 32 * kB) {
+        uint4 r[kB];
+        uint32_t off[kB];
         float snr[kB];
 #pragma unroll
         for (int j = 0; j < kB; ++j) {
             const uint32_t k = k0 + 32 * j;
             if (k < fed_cl) {
-                if (kb) r[j] = __ldcs(p.s_rec + sb + k);
-                if (o.cl_snr) snr[j] = __ldcs(p.s_snr + sb + k);
+                r[j] = p.s_rec[sb + k];
+                off[j] = p.s_off[sb + k];
+                if (o.cl_snr) snr[j] = p.s_snr[sb + k];
             }
         }
 #pragma unroll
         for (int j = 0; j < kB; ++j) {
             const uint32_t k = k0 + 32 * j;
-            const bool have = k < fed_cl;
-            const uint32_t wd = have ? r[j].y >> 16 : 0u;
-            const uint32_t incl = warp_incl_scan(wd, lane);
-            const uint32_t off = run_adc + incl - wd;
-            run_adc += __shfl_sync(kFull, incl, 31);
-            if (have) {
-                const uint32_t k_cl = b_cl + k, k_adc = b_adc + off;
+            if (k < fed_cl) {
+                const uint32_t wd = r[j].y >> 16;
+                const uint32_t k_cl = b_cl + k, k_adc = b_adc + off[j];
                 if (all_fit || (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc)) {
                     st_stream(o.cl_module + k_cl, r[j].x, pol_first);
                     st_stream(o.cl_first + k_cl, r[j].y & 0xffffu, pol_first);
                     st_stream(o.cl_width + k_cl, wd, pol_first);
                     st_stream(o.cl_charge + k_cl, static_cast<int32_t>(r[j].z), pol_first);
-                    // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
-                    st_stream(o.cl_bary + k_cl,
-                              __fadd_rn(static_cast<float>(r[j].y & 0xffffu),
-                                        __fdiv_rn(static_cast<float>(static_cast<int>(r[j].w)), static_cast<float>(static_cast<int>(r[j].z)))),
-                              pol_first);
+                    st_stream(o.cl_bary + k_cl, __uint_as_float(r[j].w), pol_first);
                     st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
                     if (o.cl_snr) o.cl_snr[k_cl] = snr[j];
-                    lim = max(lim, off + wd);
+                    lim = max(lim, off[j] + wd);
                 } else {
                     // the first cluster that does not fit reports how many were written
                     const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
@@ -1230,7 +1221,7 @@ bool output_ok(const sst_output *o) {
 }
 
 struct ScratchLayout {
-    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_ssnr,
+    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr,
         o_sadc, o_sseed, total;
 };
 ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
@@ -1251,7 +1242,8 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     L.o_adc = L.o_strip + up(2 * L.ents * cap_events);
     // staging between the two kernels
     L.o_srec = L.o_adc + up(L.ents * cap_events);
-    L.o_ssnr = L.o_srec + up(16 * L.cl_slots * cap_events);
+    L.o_soff = L.o_srec + up(16 * L.cl_slots * cap_events);
+    L.o_ssnr = L.o_soff + up(4 * L.cl_slots * cap_events);
     L.o_sadc = L.o_ssnr + up(4 * L.cl_slots * cap_events);
     L.o_sseed = L.o_sadc + up(L.ents * cap_events);
     L.total = L.o_sseed + up(2 * L.ents * cap_events);
@@ -1309,6 +1301,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
     kp.g_adc = blk + L.o_adc;
     kp.s_rec = reinterpret_cast<uint4 *>(blk + L.o_srec);
+    kp.s_off = reinterpret_cast<uint32_t *>(blk + L.o_soff);
     kp.s_snr = reinterpret_cast<float *>(blk + L.o_ssnr);
     kp.s_adc = blk + L.o_sadc;
     kp.s_seed = reinterpret_cast<uint16_t *>(blk + L.o_sseed);
