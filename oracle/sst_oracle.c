@@ -252,3 +252,62 @@ void sst_oracle_cluster(const uint8_t *adc, const float *gain, const float *nois
     if (n_cl > cap_clusters) status[0] |= SST_O_FLAG_CL_CAP;
     if (n_adc > cap_adc) status[0] |= SST_O_FLAG_ADC_CAP;
 }
+
+/* ---------------------------------------------------------------------------------------
+ * Compact structure of arrays: what the paper's unpacker
+ * builds -- "unpack the data to SoA format" with "detector conditions (e.g. gain and noise)"
+ * per strip, one entry per recorded strip (~800,000 per event).
+ * Plain definition: for every global strip id g in ascending order whose dense ADC is non-zero
+ * (reading s9: a recorded ADC of 0 carries nothing), the entry (g, adc[g], noise[g], gain[g],
+ * bad[g]) with the calibration exactly as it was uploaded.
+ * Entries beyond cap are not written; the return value is the number of recorded strips.
+ * ------------------------------------------------------------------------------------- */
+uint64_t sst_oracle_compact(const uint8_t *adc, const float *gain, const float *noise,
+                            const uint8_t *bad, uint64_t n, uint64_t cap, uint32_t *c_strip,
+                            uint8_t *c_adc, float *c_noise, float *c_gain, uint8_t *c_bad)
+{
+    uint64_t k = 0;
+    for (uint64_t g = 0; g < n; ++g) {
+        if (adc[g] == 0) continue;
+        if (k < cap) {
+            c_strip[k] = (uint32_t)g;
+            c_adc[k] = adc[g];
+            c_noise[k] = noise[g];
+            c_gain[k] = gain[g];
+            c_bad[k] = bad[g] ? 1 : 0;
+        }
+        ++k;
+    }
+    return k;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Clusters -> global hit coordinates ("convert
+ * clusters to global hit coordinates in order to provide the necessary input for MKFIT").
+ * The paper gives no geometry; reading s23 fixes a synthetic one: module m is a flat
+ * sensor whose strips measure the coordinate u along the direction (-sin phi, cos phi, 0) in
+ * the transverse plane, its centre sits at radius r and azimuth phi, at height z:
+ *     geom[6 m ..] = { pitch, u0, r, cos phi, sin phi, z }      (float32, as uploaded)
+ *     u = u0 + pitch * barycenter            (barycenter in module-local strip units, s16)
+ *     x = r cos phi - u sin phi,  y = r sin phi + u cos phi,  z = z
+ * evaluated here in double from the float32 inputs and rounded once to float32.
+ * A module id >= n_modules gives NaN coordinates.
+ * ------------------------------------------------------------------------------------- */
+void sst_oracle_hits(const uint32_t *cl_module, const float *cl_bary, uint64_t n_clusters,
+                     const float *geom, uint32_t n_modules, float *hit_x, float *hit_y, float *hit_z)
+{
+    for (uint64_t k = 0; k < n_clusters; ++k) {
+        const uint32_t m = cl_module[k];
+        if (m >= n_modules) {
+            hit_x[k] = hit_y[k] = hit_z[k] = NAN;
+            continue;
+        }
+        const float *gm = geom + 6ull * m;
+        const double pitch = gm[0], u0 = gm[1], r = gm[2], c = gm[3], s = gm[4], z = gm[5];
+        const double u = u0 + pitch * (double)cl_bary[k];
+        hit_x[k] = (float)(r * c - u * s);
+        hit_y[k] = (float)(r * s + u * c);
+        hit_z[k] = (float)z;
+    }
+}
+

@@ -61,6 +61,10 @@ def lib():
         L.sst_oracle_cluster.restype = None
         L.sst_oracle_cluster.argtypes = [C.c_void_p] * 6 + [C.c_uint32, C.c_float, C.c_uint32,
                                                             C.c_uint32] + [C.c_void_p] * 10
+        L.sst_oracle_compact.restype = C.c_uint64
+        L.sst_oracle_compact.argtypes = [C.c_void_p] * 4 + [C.c_uint64, C.c_uint64] + [C.c_void_p] * 5
+        L.sst_oracle_hits.restype = None
+        L.sst_oracle_hits.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint32] + [C.c_void_p] * 3
         _lib = L
     return _lib
 
@@ -168,6 +172,34 @@ def run(raw, fed_offsets, n_feds, gain, noise, bad, chan_module, thresholds,
     return OracleResult(chan_off, chan_len, adc, active, seed, seed_idx, c["n_clusters"],
                         c["cl_module"], c["cl_first"], c["cl_width"], c["cl_charge"], c["cl_bary"],
                         c["cl_adc_off"], c["cl_adc"], c["cl_snr"], status)
+
+
+def compact(adc, gain, noise, bad, cap: Optional[int] = None):
+    """Compact SoA (sst_oracle_compact): one entry per recorded strip, ascending strip id.
+    Returns (n_present, dict of arrays trimmed to min(n_present, cap))."""
+    adc = np.ascontiguousarray(adc, np.uint8)
+    gain = np.ascontiguousarray(gain, np.float32)
+    noise = np.ascontiguousarray(noise, np.float32)
+    bad = np.ascontiguousarray(bad, np.uint8)
+    capn = int(np.count_nonzero(adc)) if cap is None else int(cap)
+    m = max(capn, 1)
+    out = dict(strip=np.zeros(m, np.uint32), adc=np.zeros(m, np.uint8), noise=np.zeros(m, np.float32),
+               gain=np.zeros(m, np.float32), bad=np.zeros(m, np.uint8))
+    k = int(lib().sst_oracle_compact(_p(adc), _p(gain), _p(noise), _p(bad), adc.size, capn, _p(out["strip"]),
+                                     _p(out["adc"]), _p(out["noise"]), _p(out["gain"]), _p(out["bad"])))
+    w = min(k, capn)
+    return k, {key: v[:w] for key, v in out.items()}
+
+
+def hits(cl_module, cl_bary, geom):
+    """Global hit coordinates of clusters (sst_oracle_hits); geom float32 [n_modules, 6]."""
+    cm = np.ascontiguousarray(cl_module, np.uint32)
+    cb = np.ascontiguousarray(cl_bary, np.float32)
+    g = np.ascontiguousarray(geom, np.float32).reshape(-1, 6)
+    n = cm.size
+    x, y, z = (np.zeros(max(n, 1), np.float32) for _ in range(3))
+    lib().sst_oracle_hits(_p(cm), _p(cb), n, _p(g), g.shape[0], _p(x), _p(y), _p(z))
+    return x[:n], y[:n], z[:n]
 
 
 def events_omp(raws, fed_offsets_list, n_feds, gain, noise, bad, chan_module, thresholds,

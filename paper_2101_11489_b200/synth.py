@@ -110,6 +110,27 @@ def make_calibration(n_feds: int, bad_frac: float, seed: int = 1) -> Calibration
     return Calibration(n_feds, gain, noise, bad, make_module_map(n_feds, seed))
 
 
+TAG_GEOM = 4
+
+
+def make_geometry(chan_module: np.ndarray, seed: int = 1) -> np.ndarray:
+    """Synthetic module geometry, float32 [n_modules, 6] = {pitch, u0, r, cos phi, sin phi, z}
+    (reading s23; the paper names the hit conversion as its next step, and
+    gives no geometry).  Module ids must be 0..n_modules-1 (as make_module_map gives them).  Pitch
+    80-200 um, the sensor centred on u = 0, radii of a barrel-like tracker (20-110 cm), any azimuth,
+    |z| < 110 cm; lengths in cm."""
+    cm = np.asarray(chan_module, np.int64)
+    n_mod = int(cm.max()) + 1
+    n_strips = np.bincount(cm, minlength=n_mod).astype(np.float64) * N_STRIP
+    rng = _rng(TAG_GEOM, seed)
+    pitch = rng.uniform(0.008, 0.020, n_mod)
+    phi = rng.uniform(-np.pi, np.pi, n_mod)
+    r = rng.choice(np.array([25.5, 33.9, 41.9, 49.8, 60.8, 69.2, 78.0, 86.8, 96.5, 108.0]), n_mod)
+    z = rng.uniform(-110.0, 110.0, n_mod)
+    u0 = -pitch * (n_strips - 1.0) / 2.0
+    return np.stack([pitch, u0, r, np.cos(phi), np.sin(phi), z], axis=1).astype(np.float32)
+
+
 # --------------------------------------------------------------------------------------
 # raw encoder
 # --------------------------------------------------------------------------------------
