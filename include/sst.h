@@ -72,12 +72,15 @@ enum {
     SST_ST_N_ADC = 3,        /* cluster ADC bytes found (may exceed cap_adc)              */
     SST_ST_N_OVERRUN = 4,    /* FEDs with bad offsets or a channel-length chain passing the FED end */
     SST_ST_N_SEEDS = 5,      /* seed strips found                                         */
+    SST_ST_N_PRESENT = 6,    /* recorded strips with a non-zero ADC (when the compact SoA is
+                                requested, else 0; may exceed cap_compact)                 */
     SST_ST_WORDS = 8
 };
 #define SST_FLAG_CLUSTER_CAP 1u /* more clusters than cap_clusters */
 #define SST_FLAG_ADC_CAP 2u     /* more cluster ADC bytes than cap_adc */
 #define SST_FLAG_MALFORMED 4u   /* >= 1 malformed channel */
 #define SST_FLAG_OVERRUN 8u     /* >= 1 flagged FED */
+#define SST_FLAG_COMPACT_CAP 16u /* more recorded strips than cap_compact */
 
 /*
  * Output of one event.  All pointers are DEVICE pointers owned by the caller (HOST pointers
@@ -110,6 +113,26 @@ typedef struct {
     float *cl_snr;        /* [cap_clusters] optional: charge / sqrt(sum noise^2)                 */
     uint8_t *cl_adc;      /* [cap_adc] gain-corrected ADCs min(254, floor(adc/gain + 0.5))       */
     uint32_t *dev_status; /* [SST_ST_WORDS], see above; fully written by every call              */
+    /* Optional: the compact structure of arrays the paper's unpacker builds ("unpack
+     * the data to SoA format", one entry per recorded strip) with the calibration
+     * gathered per event: entry k is the k-th strip, in ascending global strip id,
+     * whose dense ADC is non-zero.  All five arrays or none (compact_strip == NULL = not wanted);
+     * entries beyond cap_compact are not written, dev_status[SST_ST_N_PRESENT] is the number
+     * found.  DEVICE entry points only (sst_unpack_cluster, sst_unpack_cluster_batch): the HOST entry
+     * points reject an sst_output that asks for them. */
+    uint32_t *compact_strip; /* [cap_compact] global strip id                                    */
+    uint8_t *compact_adc;    /* [cap_compact] raw ADC                                            */
+    float *compact_noise;    /* [cap_compact] noise as uploaded                                  */
+    float *compact_gain;     /* [cap_compact] gain as uploaded                                   */
+    uint8_t *compact_bad;    /* [cap_compact] 1 = bad strip                                      */
+    uint32_t cap_compact;
+    /* Optional: global hit coordinates of the clusters ("convert clusters to global
+     * hit coordinates in order to provide the necessary input for MKFIT"), from the geometry of
+     * sst_upload_geometry: u = u0 + pitch * cl_bary; x = r cos(phi) - u sin(phi),
+     * y = r sin(phi) + u cos(phi), z = z of the cluster's module, in float32 (absolute error
+     * <= 1e-6 * max(|r|, |u|, |z|) against a double evaluation).  All three or none; NaN for a
+     * module id >= n_modules or when no geometry was uploaded.  DEVICE entry points only. */
+    float *hit_x, *hit_y, *hit_z; /* [cap_clusters] each */
 } sst_output;
 
 /* Creates a context on cfg->device: stream-ordered memory pool, calibration storage.
@@ -123,6 +146,12 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx);
  * synchronises).  Must not run concurrently with sst_unpack_cluster on the same context. */
 sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise, const uint8_t *bad,
                             const uint32_t *chan_module);
+
+/* Module geometry for the hit conversion, once: HOST geom[n_modules*6] float32 =
+ * {pitch, u0, r, cos phi, sin phi, z} of module id 0..n_modules-1 (module ids as given in
+ * chan_module; reading s23: the paper gives no geometry, this flat-sensor model is the
+ * build's own).  Copied before return; must not run concurrently with sst_unpack_cluster. */
+sst_status sst_upload_geometry(sst_ctx *ctx, const float *geom, uint32_t n_modules);
 
 /* One event: channel-location map, unpack, active/seed flags, seed expansion with
  * leftmost-seed ownership, gain correction, cluster threshold, ordered output

@@ -15,11 +15,11 @@ LIB_PATH = os.path.join(HERE, "csrc", "libsst.so")
 
 N_CHAN, N_STRIP, FED_STRIPS = 96, 256, 96 * 256
 ST_WORDS = 8
-ST_FLAGS, ST_N_MALFORMED, ST_N_CLUSTERS, ST_N_ADC, ST_N_OVERRUN, ST_N_SEEDS = range(6)
-FLAG_CLUSTER_CAP, FLAG_ADC_CAP, FLAG_MALFORMED, FLAG_OVERRUN = 1, 2, 4, 8
+ST_FLAGS, ST_N_MALFORMED, ST_N_CLUSTERS, ST_N_ADC, ST_N_OVERRUN, ST_N_SEEDS, ST_N_PRESENT = range(7)
+FLAG_CLUSTER_CAP, FLAG_ADC_CAP, FLAG_MALFORMED, FLAG_OVERRUN, FLAG_COMPACT_CAP = 1, 2, 4, 8, 16
 SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB = range(5)
 
-EXPORTS = ["sst_create", "sst_upload_calib", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
+EXPORTS = ["sst_create", "sst_upload_calib", "sst_upload_geometry", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
            "sst_unpack_cluster_host_batch", "sst_unpack_cluster_host_packed",
            "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_event_download", "sst_destroy", "sst_last_cuda_error",
            "sst_status_string", "sst_get_info"]
@@ -40,7 +40,10 @@ class sst_output(C.Structure):
                 ("cap_adc", C.c_uint32), ("n_clusters", C.c_void_p), ("cl_module", C.c_void_p),
                 ("cl_first", C.c_void_p), ("cl_width", C.c_void_p), ("cl_charge", C.c_void_p),
                 ("cl_bary", C.c_void_p), ("cl_adc_off", C.c_void_p), ("cl_snr", C.c_void_p),
-                ("cl_adc", C.c_void_p), ("dev_status", C.c_void_p)]
+                ("cl_adc", C.c_void_p), ("dev_status", C.c_void_p),
+                ("compact_strip", C.c_void_p), ("compact_adc", C.c_void_p), ("compact_noise", C.c_void_p),
+                ("compact_gain", C.c_void_p), ("compact_bad", C.c_void_p), ("cap_compact", C.c_uint32),
+                ("hit_x", C.c_void_p), ("hit_y", C.c_void_p), ("hit_z", C.c_void_p)]
 
 
 class sst_info(C.Structure):
@@ -68,6 +71,7 @@ def load():
     vp = C.c_void_p
     L.sst_create.argtypes = [C.POINTER(sst_config), C.POINTER(vp)]
     L.sst_upload_calib.argtypes = [vp, vp, vp, vp, vp]
+    L.sst_upload_geometry.argtypes = [vp, vp, C.c_uint32]
     L.sst_unpack_cluster.argtypes = [vp, vp, vp, C.POINTER(sst_thresholds), C.POINTER(sst_output), vp]
     L.sst_unpack_cluster_batch.argtypes = [vp, C.c_uint32, vp, vp, C.POINTER(sst_thresholds), vp, vp, C.c_uint32]
     L.sst_unpack_cluster_host.argtypes = [vp, vp, C.c_uint32, vp, C.POINTER(sst_thresholds),
@@ -130,13 +134,24 @@ def sst_upload_calib(ctx, gain, noise, bad, chan_module):
     _check(ctx, load().sst_upload_calib(ctx, _ptr(g), _ptr(n), _ptr(b), _ptr(m)), "sst_upload_calib")
 
 
+def sst_upload_geometry(ctx, geom):
+    """HOST float32 array [n_modules, 6] = {pitch, u0, r, cos phi, sin phi, z} per module id."""
+    import numpy as np
+    g = np.ascontiguousarray(geom, np.float32).reshape(-1, 6)
+    _check(ctx, load().sst_upload_geometry(ctx, _ptr(g), g.shape[0]), "sst_upload_geometry")
+
+
 def make_output(*, n_clusters, cl_module, cl_first, cl_width, cl_charge, cl_bary, cl_adc_off, cl_adc,
                 dev_status, cap_clusters: int, cap_adc: int, strip_adc=None, chan_off=None,
-                chan_len=None, seed_idx=None, cap_seeds: int = 0, cl_snr=None) -> sst_output:
+                chan_len=None, seed_idx=None, cap_seeds: int = 0, cl_snr=None, compact_strip=None,
+                compact_adc=None, compact_noise=None, compact_gain=None, compact_bad=None,
+                cap_compact: int = 0, hit_x=None, hit_y=None, hit_z=None) -> sst_output:
     return sst_output(_ptr(strip_adc), _ptr(chan_off), _ptr(chan_len), _ptr(seed_idx), cap_seeds,
                       cap_clusters, cap_adc, _ptr(n_clusters), _ptr(cl_module), _ptr(cl_first),
                       _ptr(cl_width), _ptr(cl_charge), _ptr(cl_bary), _ptr(cl_adc_off), _ptr(cl_snr),
-                      _ptr(cl_adc), _ptr(dev_status))
+                      _ptr(cl_adc), _ptr(dev_status), _ptr(compact_strip), _ptr(compact_adc),
+                      _ptr(compact_noise), _ptr(compact_gain), _ptr(compact_bad), cap_compact,
+                      _ptr(hit_x), _ptr(hit_y), _ptr(hit_z))
 
 
 def sst_unpack_cluster(ctx, raw, fed_offsets, thresholds, out: sst_output, stream: int = 0):

@@ -96,6 +96,13 @@ struct EventDesc {
 struct KParams {
     const float2 *calib;     // {noise (+inf at bad strips), gain} per strip
     const uint2 *chan_info;  // {module id, first channel | end channel << 8 of the module}
+    const float2 *calib_orig;  // {noise, gain} as uploaded (the compact SoA reports these)
+    const uint8_t *bad;        // bad flags as uploaded
+    const float *geom;         // [n_geom][6] {pitch, u0, r, cos phi, sin phi, z}, or NULL
+    uint32_t n_geom;
+    uint32_t *fed_present;     // [kMaxEv][n_feds] list entries << 16 | entries with a non-zero ADC (compact SoA)
+    uint16_t *s_csid;          // staged list of a FED: strip ids and raw ADCs, for the compact SoA
+    uint8_t *s_cadc;
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
     unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+warps)
     unsigned long long ticket_base;
@@ -513,6 +520,26 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         }
     }
     __syncwarp();  // lists complete; the payload is dead from here on
+
+    // ---------------------------------------------------------------- compact SoA, first half (on request)
+    // the unpacker's product is a structure of arrays with one entry per recorded strip.
+    // The FED's lists are exactly that; they are staged as they are (strip id, raw ADC) and
+    // sst_emit_kernel moves them to their place in the event's arrays, adding the calibration.
+    if (o.compact_strip) {
+        const size_t cb = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
+        uint32_t nz = 0;
+#pragma unroll 1
+        for (uint32_t i = lane; i < ((P + 31u) & ~31u); i += 32u) {
+            uint32_t a = 0;
+            if (i < P) {
+                a = adc_l[i];
+                p.s_csid[cb + i] = strip_l[i] & 0x7fffu;
+                p.s_cadc[cb + i] = static_cast<uint8_t>(a);
+            }
+            nz += __popc(__ballot_sync(kFull, a != 0));
+        }
+        if (lane == 0) p.fed_present[static_cast<size_t>(c.ev) * p.n_feds + f] = (P << 16) | nz;
+    }
 
     // ---------------------------------------------------------------- a2: dense SoA
     // The FED's 24576-byte block of the dense strip array is put together 2048 strips at a time
@@ -1128,6 +1155,20 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
                     st_stream(o.cl_bary + k_cl, __uint_as_float(r[j].w), pol_first);
                     st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
                     if (o.cl_snr) o.cl_snr[k_cl] = snr[j];
+                    if (o.hit_x) {  // clusters -> global hit coordinates (reading s23)
+                        float hx = __int_as_float(0x7fc00000), hy = hx, hz = hx;
+                        if (p.geom && r[j].x < p.n_geom) {
+                            const float2 *gm = reinterpret_cast<const float2 *>(p.geom) + 3u * static_cast<size_t>(r[j].x);
+                            const float2 g0 = __ldg(gm), g1 = __ldg(gm + 1), g2 = __ldg(gm + 2);  // {pitch, u0} {r, cos} {sin, z}
+                            const float u = __fmaf_rn(g0.x, __uint_as_float(r[j].w), g0.y);
+                            hx = __fmaf_rn(g1.x, g1.y, -__fmul_rn(u, g2.x));
+                            hy = __fmaf_rn(g1.x, g2.x, __fmul_rn(u, g1.y));
+                            hz = g2.y;
+                        }
+                        o.hit_x[k_cl] = hx;
+                        o.hit_y[k_cl] = hy;
+                        o.hit_z[k_cl] = hz;
+                    }
                     lim = max(lim, off[j] + wd);
                 } else {
                     // the first cluster that does not fit reports how many were written
@@ -1153,6 +1194,41 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
         for (uint32_t i = lane; i < fed_seed; i += 32)
             if (b_seed + i < o.cap_seeds) o.seed_idx[b_seed + i] = f * kFedStrips + p.s_seed[ab + i];
     }
+    // compact SoA, second half (on request): the FED's staged list goes to its place among the
+    // event's recorded strips (exclusive prefix of the FEDs' non-zero entries), with the
+    // calibration as it was uploaded gathered per entry
+    uint32_t n_present = 0;
+    if (!packed && o.compact_strip) {
+        const uint32_t *pr = p.fed_present + static_cast<size_t>(ev) * p.n_feds;
+        uint32_t base = 0;
+#pragma unroll 4
+        for (uint32_t j = lane; j < f; j += 32) base += pr[j] & 0xffffu;
+        base = __reduce_add_sync(kFull, base);
+        const uint32_t own_p = pr[f], P = own_p >> 16;
+        const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll 1
+        for (uint32_t i0 = 0; i0 < P; i0 += 32) {
+            const uint32_t i = i0 + lane;
+            uint32_t a = 0, sid = 0;
+            if (i < P) {
+                a = p.s_cadc[ab + i];
+                sid = p.s_csid[ab + i];
+            }
+            const uint32_t keep = __ballot_sync(kFull, a != 0);
+            const uint32_t k = base + __popc(keep & lt);
+            if (a != 0 && k < o.cap_compact) {
+                const size_t g = static_cast<size_t>(f) * kFedStrips + sid;
+                const float2 cv = __ldg(p.calib_orig + g);
+                o.compact_strip[k] = static_cast<uint32_t>(g);
+                o.compact_adc[k] = static_cast<uint8_t>(a);
+                o.compact_noise[k] = cv.x;
+                o.compact_gain[k] = cv.y;
+                o.compact_bad[k] = __ldg(p.bad + g);
+            }
+            base += __popc(keep);
+        }
+        n_present = base;  // (of the last FED: the event's total)
+    }
     if (f == p.n_feds - 1 && lane == 0) {  // event totals = prefix of the last FED + its own
         const uint32_t t_cl = b_cl + fed_cl, t_adc = b_adc + fed_adc, n_mal = b_malf + fed_malf, n_over = b_over + fed_over;
         uint32_t flags = 0;
@@ -1160,6 +1236,7 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
         if (t_adc > o.cap_adc) flags |= SST_FLAG_ADC_CAP;
         if (n_mal) flags |= SST_FLAG_MALFORMED;
         if (n_over) flags |= SST_FLAG_OVERRUN;
+        if (n_present > o.cap_compact) flags |= SST_FLAG_COMPACT_CAP;
         if (!(flags & (SST_FLAG_CLUSTER_CAP | SST_FLAG_ADC_CAP))) *o.n_clusters = t_cl;
         o.dev_status[SST_ST_FLAGS] = flags;
         o.dev_status[SST_ST_N_MALFORMED] = n_mal;
@@ -1167,7 +1244,7 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
         o.dev_status[SST_ST_N_ADC] = t_adc;
         o.dev_status[SST_ST_N_OVERRUN] = n_over;
         o.dev_status[SST_ST_N_SEEDS] = b_seed + fed_seed;
-        o.dev_status[6] = 0;
+        o.dev_status[SST_ST_N_PRESENT] = n_present;
         o.dev_status[7] = 0;
     }
 }
@@ -1178,8 +1255,12 @@ __global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __gr
 struct sst_ctx {
     sst_config cfg{};
     cudaMemPool_t pool = nullptr;
-    float2 *calib = nullptr;
+    float2 *calib = nullptr;       // {noise (+inf at bad strips), gain}: what the kernels gather
+    float2 *calib_orig = nullptr;  // {noise, gain} as uploaded
+    uint8_t *bad = nullptr;        // bad flags as uploaded
     uint2 *chan_info = nullptr;
+    float *geom = nullptr;         // module geometry for the hit conversion (sst_upload_geometry)
+    uint32_t n_geom = 0;
     bool has_calib = false;
     std::atomic<int32_t> last_err{0};
     int sm_count = 0;
@@ -1208,6 +1289,9 @@ inline bool cu_ok(sst_ctx *ctx, cudaError_t e) {
 #define SST_CU(call) \
     do { if (!cu_ok(ctx, (call))) return SST_ERR_CUDA; } while (0)
 
+// the HOST entry points produce the cluster arrays, the dense SoA, the channel map and the seeds
+bool no_device_only_outputs(const sst_output *o) { return !o->compact_strip && !o->hit_x && o->cap_compact == 0; }
+
 bool thresholds_ok(const sst_thresholds *t) {
     const float v[3] = {t->channel, t->seed, t->cluster};
     for (float x : v)
@@ -1216,12 +1300,17 @@ bool thresholds_ok(const sst_thresholds *t) {
 }
 
 bool output_ok(const sst_output *o) {
-    return o && o->n_clusters && o->dev_status && o->cl_module && o->cl_first && o->cl_width &&
-           o->cl_charge && o->cl_bary && o->cl_adc_off && o->cl_adc && !(o->seed_idx == nullptr && o->cap_seeds != 0);
+    if (!(o && o->n_clusters && o->dev_status && o->cl_module && o->cl_first && o->cl_width && o->cl_charge &&
+          o->cl_bary && o->cl_adc_off && o->cl_adc && !(o->seed_idx == nullptr && o->cap_seeds != 0)))
+        return false;
+    // the optional groups come complete or not at all
+    const int nc = !!o->compact_strip + !!o->compact_adc + !!o->compact_noise + !!o->compact_gain + !!o->compact_bad;
+    const int nh = !!o->hit_x + !!o->hit_y + !!o->hit_z;
+    return (nc == 0 || nc == 5) && (nh == 0 || nh == 3) && !(nc == 0 && o->cap_compact != 0);
 }
 
 struct ScratchLayout {
-    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr,
+    size_t ents, mwords, cl_slots, state_bytes, o_ticket, o_state, o_rec, o_mask, o_strip, o_adc, o_srec, o_soff, o_ssnr, o_present, o_csid, o_cadc,
         o_sadc, o_sseed, total;
 };
 ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
@@ -1246,7 +1335,10 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     L.o_ssnr = L.o_soff + up(4 * L.cl_slots * cap_events);
     L.o_sadc = L.o_ssnr + up(4 * L.cl_slots * cap_events);
     L.o_sseed = L.o_sadc + up(L.ents * cap_events);
-    L.total = L.o_sseed + up(2 * L.ents * cap_events);
+    L.o_present = L.o_sseed + up(2 * L.ents * cap_events);
+    L.o_csid = L.o_present + up(L.state_bytes / 2);
+    L.o_cadc = L.o_csid + up(2 * L.ents * cap_events);
+    L.total = L.o_cadc + up(L.ents * cap_events);
     return L;
 }
 
@@ -1293,6 +1385,13 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     KParams kp{};
     kp.calib = ctx->calib;
     kp.chan_info = ctx->chan_info;
+    kp.calib_orig = ctx->calib_orig;
+    kp.bad = ctx->bad;
+    kp.geom = ctx->geom;
+    kp.n_geom = ctx->n_geom;
+    kp.fed_present = reinterpret_cast<uint32_t *>(blk + L.o_present);
+    kp.s_csid = reinterpret_cast<uint16_t *>(blk + L.o_csid);
+    kp.s_cadc = blk + L.o_cadc;
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
     kp.ticket_base = sl->ticket_base;
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
@@ -1356,6 +1455,8 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (ctx->cfg.max_events_in_flight == 0) ctx->cfg.max_events_in_flight = 8;
     auto fail = [&](sst_status s) {
         if (ctx->calib) cudaFree(ctx->calib);
+        if (ctx->calib_orig) cudaFree(ctx->calib_orig);
+        if (ctx->bad) cudaFree(ctx->bad);
         if (ctx->chan_info) cudaFree(ctx->chan_info);
         if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
         delete ctx;
@@ -1373,6 +1474,8 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         return fail(SST_ERR_CUDA);
     const size_t n = static_cast<size_t>(cfg->n_feds) * kFedStrips;
     if (cudaMalloc(&ctx->calib, n * sizeof(float2)) != cudaSuccess) return fail(SST_ERR_CUDA);
+    if (cudaMalloc(&ctx->calib_orig, n * sizeof(float2)) != cudaSuccess) return fail(SST_ERR_CUDA);
+    if (cudaMalloc(&ctx->bad, n) != cudaSuccess) return fail(SST_ERR_CUDA);
     if (cudaMalloc(&ctx->chan_info, static_cast<size_t>(cfg->n_feds) * kChan * sizeof(uint2)) !=
         cudaSuccess)
         return fail(SST_ERR_CUDA);
@@ -1453,6 +1556,10 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
     }
     SST_CU(cudaSetDevice(ctx->cfg.device));
     SST_CU(cudaMemcpy(ctx->calib, packed.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
+    // the values as given, for the compact SoA (PAPER.md:31 gathers the calibration into it)
+    for (size_t g = 0; g < n; ++g) packed[g] = make_float2(noise[g], gain[g]);
+    SST_CU(cudaMemcpy(ctx->calib_orig, packed.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
+    SST_CU(cudaMemcpy(ctx->bad, bad, n, cudaMemcpyHostToDevice));
     // module extent of every channel (modules are runs of equal ids inside one FED)
     std::vector<uint2> info(nch);
     for (size_t c0 = 0; c0 < nch;) {
@@ -1465,6 +1572,21 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
     SST_CU(cudaMemcpy(ctx->chan_info, info.data(), nch * sizeof(uint2), cudaMemcpyHostToDevice));
     SST_CU(cudaDeviceSynchronize());
     ctx->has_calib = true;
+    return SST_OK;
+}
+
+sst_status sst_upload_geometry(sst_ctx *ctx, const float *geom, uint32_t n_modules) {
+    if (!ctx || !geom || n_modules == 0) return SST_ERR_INVALID_ARG;
+    for (size_t i = 0; i < static_cast<size_t>(n_modules) * 6; ++i)
+        if (!std::isfinite(geom[i])) return SST_ERR_INVALID_ARG;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    SST_CU(cudaDeviceSynchronize());
+    if (ctx->geom) cudaFree(ctx->geom);
+    ctx->geom = nullptr;
+    ctx->n_geom = 0;
+    SST_CU(cudaMalloc(&ctx->geom, static_cast<size_t>(n_modules) * 6 * sizeof(float)));
+    SST_CU(cudaMemcpy(ctx->geom, geom, static_cast<size_t>(n_modules) * 6 * sizeof(float), cudaMemcpyHostToDevice));
+    ctx->n_geom = n_modules;
     return SST_OK;
 }
 
@@ -1550,7 +1672,7 @@ sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8
 sst_status sst_unpack_cluster_host(sst_ctx *ctx, const uint8_t *raw, uint32_t raw_bytes,
                                    const uint32_t *fed_offsets, const sst_thresholds *thr,
                                    const sst_output *out, void *stream) {
-    if (!ctx || !raw || !fed_offsets || !thr || !output_ok(out) || !thresholds_ok(thr))
+    if (!ctx || !raw || !fed_offsets || !thr || !output_ok(out) || !thresholds_ok(thr) || !no_device_only_outputs(out))
         return SST_ERR_INVALID_ARG;
     if (raw_bytes > ctx->cfg.max_raw_bytes) return SST_ERR_INVALID_ARG;
     if (!ctx->has_calib) return SST_ERR_NO_CALIB;
@@ -1660,7 +1782,8 @@ sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const 
         return SST_ERR_INVALID_ARG;
     if (!ctx->has_calib) return SST_ERR_NO_CALIB;
     for (uint32_t e = 0; e < n_events; ++e)
-        if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e]) || raw_bytes[e] > ctx->cfg.max_raw_bytes)
+        if (!raw[e] || !fed_offsets[e] || !output_ok(&outs[e]) || !no_device_only_outputs(&outs[e]) ||
+            raw_bytes[e] > ctx->cfg.max_raw_bytes)
             return SST_ERR_INVALID_ARG;
     if (n_events == 0) return SST_OK;
     SST_CU(cudaSetDevice(ctx->cfg.device));
@@ -1924,6 +2047,9 @@ sst_status sst_destroy(sst_ctx *ctx) {
     for (auto &se : ctx->stream_events) cudaEventDestroy(se.ev);
     cudaDeviceSynchronize();
     if (ctx->calib) cudaFree(ctx->calib);
+    if (ctx->calib_orig) cudaFree(ctx->calib_orig);
+    if (ctx->bad) cudaFree(ctx->bad);
+    if (ctx->geom) cudaFree(ctx->geom);
     if (ctx->chan_info) cudaFree(ctx->chan_info);
     if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
     delete ctx;

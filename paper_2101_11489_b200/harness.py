@@ -38,6 +38,13 @@ class EventOutputs:
                 res[name] = t[name]
         if "seed_idx" in t:
             res["seed_idx"] = t["seed_idx"][:min(int(st[B.ST_N_SEEDS]), t["seed_idx"].size)]
+        if "compact_strip" in t:
+            npres = min(int(st[B.ST_N_PRESENT]), t["compact_strip"].size)
+            for name in ("compact_strip", "compact_adc", "compact_noise", "compact_gain", "compact_bad"):
+                res[name] = t[name][:npres]
+        for name in ("hit_x", "hit_y", "hit_z"):
+            if name in t:
+                res[name] = t[name][:k]
         return res
 
 
@@ -58,6 +65,9 @@ class Detector:
         self.ctx = B.sst_create(n_feds, device, self.max_raw_bytes, max_events_in_flight, fed_strips_hint)
         B.sst_upload_calib(self.ctx, gain, noise, bad, chan_module)
 
+    def upload_geometry(self, geom):
+        B.sst_upload_geometry(self.ctx, geom)
+
     def close(self):
         if self.ctx is not None:
             B.sst_destroy(self.ctx)
@@ -76,7 +86,8 @@ class Detector:
         return d_raw, d_fo
 
     def alloc_outputs(self, cap_clusters: int, cap_adc: int, dense: bool = True, chan_map: bool = False,
-                      seeds: bool = False, snr: bool = False, cap_seeds: Optional[int] = None) -> EventOutputs:
+                      seeds: bool = False, snr: bool = False, cap_seeds: Optional[int] = None,
+                      compact: bool = False, cap_compact: Optional[int] = None, hits: bool = False) -> EventOutputs:
         torch = self.torch
         dev = self.device
         cc, ca = max(int(cap_clusters), 1), max(int(cap_adc), 1)
@@ -102,7 +113,19 @@ class Detector:
             t["seed_idx"] = torch.empty(max(ncs, 1), dtype=torch.int32, device=dev)
         if snr:
             t["cl_snr"] = torch.empty(cc, dtype=torch.float32, device=dev)
-        out = B.make_output(cap_clusters=int(cap_clusters), cap_adc=int(cap_adc), cap_seeds=ncs,
+        ncc = 0
+        if compact:
+            ncc = self.max_raw_bytes if cap_compact is None else int(cap_compact)
+            m = max(ncc, 1)
+            t["compact_strip"] = torch.empty(m, dtype=torch.int32, device=dev)
+            t["compact_adc"] = torch.empty(m, dtype=torch.uint8, device=dev)
+            t["compact_noise"] = torch.empty(m, dtype=torch.float32, device=dev)
+            t["compact_gain"] = torch.empty(m, dtype=torch.float32, device=dev)
+            t["compact_bad"] = torch.empty(m, dtype=torch.uint8, device=dev)
+        if hits:
+            for name in ("hit_x", "hit_y", "hit_z"):
+                t[name] = torch.empty(cc, dtype=torch.float32, device=dev)
+        out = B.make_output(cap_clusters=int(cap_clusters), cap_adc=int(cap_adc), cap_seeds=ncs, cap_compact=ncc,
                             **{k: v for k, v in t.items()})
         return EventOutputs(t, out, int(cap_clusters), int(cap_adc))
 
@@ -179,5 +202,6 @@ class PooledOutputs:
 def unsigned_view(res: Dict[str, np.ndarray]) -> Dict[str, np.ndarray]:
     """torch has no uint16/uint32 tensors everywhere; reinterpret the signed storage."""
     conv = {"cl_module": np.uint32, "cl_first": np.uint16, "cl_width": np.uint16, "cl_adc_off": np.uint32,
-            "chan_off": np.uint32, "chan_len": np.uint16, "seed_idx": np.uint32, "status": np.uint32}
+            "chan_off": np.uint32, "chan_len": np.uint16, "seed_idx": np.uint32, "status": np.uint32,
+            "compact_strip": np.uint32}
     return {k: (v.view(conv[k]) if k in conv and isinstance(v, np.ndarray) else v) for k, v in res.items()}

@@ -731,3 +731,75 @@ def test_two_host_threads_on_distinct_streams(H, oracle):
             compare(H.unsigned_view(o.numpy()), r)
     finally:
         det.close()
+
+
+# ------------------------------------------------------------------ compact SoA and hit conversion
+def compare_next(g, r, oracle, cal, geom):
+    """Compact SoA: bit-exact (integers and the float32 calibration copied as uploaded).  Hits:
+    float32 against the oracle's double evaluation, absolute error <= 1e-6 * max(|r|, |u|, |z|)."""
+    k, c = oracle.compact(r.adc, cal.gain, cal.noise, cal.bad)
+    assert int(g["status"][6]) == k
+    for name in ("strip", "adc", "noise", "gain", "bad"):
+        assert np.array_equal(g["compact_" + name], c[name]), name
+    x, y, z = oracle.hits(r.cl_module, r.cl_bary, geom)
+    gm = geom[r.cl_module.astype(np.int64)].astype(np.float64)
+    u = gm[:, 1] + gm[:, 0] * r.cl_bary.astype(np.float64)
+    tol = 1e-6 * np.maximum(np.maximum(np.abs(gm[:, 2]), np.abs(u)), np.abs(gm[:, 5]))
+    assert np.all(np.abs(g["hit_x"].astype(np.float64) - x) <= tol)
+    assert np.all(np.abs(g["hit_y"].astype(np.float64) - y) <= tol)
+    assert np.array_equal(g["hit_z"], z)
+
+
+@pytest.mark.parametrize("cid,nf", [(0, 24), (2, 9), (4, 11), (1, 440)])
+def test_compact_soa_and_hits(H, oracle, cid, nf):
+    """the compact structure of arrays and
+    the clusters' global hit coordinates, next to the usual outputs."""
+    cfg, cal, evs = synth.make_config(cid, n_feds=nf)
+    ev = evs[0]
+    geom = synth.make_geometry(cal.chan_module)
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
+    try:
+        det.upload_geometry(geom)
+        d_raw, d_fo = det.upload_raw(ev.raw, ev.fed_offsets)
+        outs = det.alloc_outputs(ev.raw.size // 3 + 1, ev.raw.size, chan_map=True, seeds=True, snr=True, compact=True, hits=True)
+        for thr in cfg.thresholds:
+            det.run(d_raw, d_fo, thr, outs)
+            det.torch.cuda.synchronize()
+            g = H.unsigned_view(outs.numpy())
+            r = oracle.run(ev.raw, ev.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, thr)
+            compare(g, r)
+            compare_next(g, r, oracle, cal, geom)
+        # capacity of the compact arrays: a prefix is written, the count needed is reported
+        small = det.alloc_outputs(ev.raw.size // 3 + 1, ev.raw.size, compact=True, cap_compact=1000)
+        det.run(d_raw, d_fo, cfg.thresholds[0], small)
+        det.torch.cuda.synchronize()
+        gs = H.unsigned_view(small.numpy())
+        k, c = oracle.compact(ev.z, cal.gain, cal.noise, cal.bad)
+        assert int(gs["status"][6]) == k and gs["status"][0] & 16
+        assert np.array_equal(gs["compact_strip"], c["strip"][:1000])
+    finally:
+        det.close()
+
+
+def test_hits_without_geometry_are_nan_and_host_entry_points_refuse(H, oracle):
+    from paper_2101_11489_b200 import binding as B
+    cfg, cal, evs = synth.make_config(0, n_feds=2)
+    ev = evs[0]
+    det = H.Detector(2, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
+    try:
+        d_raw, d_fo = det.upload_raw(ev.raw, ev.fed_offsets)
+        outs = det.alloc_outputs(ev.raw.size, ev.raw.size, hits=True)
+        det.run(d_raw, d_fo, (2, 3, 5), outs)
+        det.torch.cuda.synchronize()
+        g = outs.numpy()
+        assert g["n_clusters"] > 0 and np.isnan(g["hit_x"]).all() and np.isnan(g["hit_z"]).all()
+        cc = int(ev.raw.size)
+        h = dict(n_clusters=np.zeros(1, np.uint32), dev_status=np.zeros(8, np.uint32), cl_module=np.zeros(cc, np.uint32),
+                 cl_first=np.zeros(cc, np.uint16), cl_width=np.zeros(cc, np.uint16), cl_charge=np.zeros(cc, np.int32),
+                 cl_bary=np.zeros(cc, np.float32), cl_adc_off=np.zeros(cc, np.uint32), cl_adc=np.zeros(cc, np.uint8),
+                 hit_x=np.zeros(cc, np.float32), hit_y=np.zeros(cc, np.float32), hit_z=np.zeros(cc, np.float32))
+        with pytest.raises(B.SSTError, match="INVALID_ARG"):
+            B.sst_unpack_cluster_host(det.ctx, ev.raw, int(ev.raw.size), ev.fed_offsets, (2, 3, 5),
+                                      B.make_output(cap_clusters=cc, cap_adc=cc, **h))
+    finally:
+        det.close()
