@@ -14,7 +14,12 @@ once, per-event output buffers taken from the library's stream-ordered pool.
              MEASURED_PEAKS.json
   cpu_baseline  the CPU oracle as it stands, timed on this box's host cores (reported, not a target)
 
-`--impl reference` times the oracle alone on the same config (see the task's contract).
+After the timed loop the output blocks of the TIMED launches are read back and every output of
+every event is compared with the oracle (bit-exact; barycenter 1e-6 relative); a difference fails
+the run.  `--config 1|2|4` times 64 events of that BASELINE.json config instead of config 3.
+`--sweep` prints the single-event latencies, events/s against events per call and against the
+number of streams, and the OpenMP oracle's N x M table.  `--impl reference` times the oracle alone
+on the same config (see the task's contract).
 """
 from __future__ import annotations
 
@@ -80,21 +85,6 @@ def measured_peak():
         except Exception:
             pass
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md, MEASURED_PEAKS.json absent)"
-
-
-def ncu_traffic(workload: str):
-    """dram bytes per launch from the committed ncu capture (profiles/traffic.csv), or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.csv")
-    if not os.path.exists(p):
-        return None
-    for line in open(p):
-        f = [x.strip() for x in line.split(",")]
-        if len(f) >= 3 and f[0] == workload:
-            try:
-                return float(f[1]) + float(f[2])
-            except ValueError:
-                return None
-    return None
 
 
 def max_over_ranks(x: float, device=None) -> float:
@@ -164,49 +154,78 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------- CPU oracle legs
-def time_oracle(events, calib, budget_s: float, min_events: int = 4):
-    """Sequential oracle (oracle/sst_oracle.c) over the workload's events until budget_s."""
+def time_oracle(events, calib, thresholds, budget_s: float, check=None, min_events: int = 4):
+    """Sequential oracle (oracle/sst_oracle.c) over the workload's events until budget_s; only the
+    oracle calls are timed.  check(i, result) is called (untimed) for every event of the first pass."""
     from oracle import sst_oracle as O
     O.build()
-    t0 = time.perf_counter()
-    n = 0
-    ncl = []
+    spent, n = 0.0, 0
     while True:
         raw, fo, _ = events[n % len(events)]
-        r = O.run(raw, fo, calib.n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, THRESHOLDS)
-        if n < len(events):
-            ncl.append(r.n_clusters)
+        t0 = time.perf_counter()
+        r = O.run(raw, fo, calib.n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, thresholds)
+        spent += time.perf_counter() - t0
+        if n < len(events) and check is not None:
+            check(n, r)
         n += 1
-        dt = time.perf_counter() - t0
-        if (dt >= budget_s and n >= min_events) or n >= 4 * len(events):
+        if (spent >= budget_s and n >= max(min_events, len(events) if check else 0)) or n >= 4 * len(events):
             break
-    return n / dt, n, dt, ncl
+    return n / spent, n, spent
 
 
-def time_oracle_omp(events, calib, budget_s: float):
-    """OpenMP build of the oracle in the paper's N x M shapes (Table 1)."""
+def compare_with_oracle(g, r, what, dense=True):
+    """Every output of one event against the oracle: integers bit-exact, barycenter 1e-6 relative."""
+    def same(name, a, b):
+        if not np.array_equal(a, b):
+            raise SystemExit(f"VERIFICATION FAILED ({what}): {name} differs from the oracle")
+    if dense:
+        same("strip_adc", g["strip_adc"], r.adc)
+    if int(g["n_clusters"]) != int(r.n_clusters):
+        raise SystemExit(f"VERIFICATION FAILED ({what}): {g['n_clusters']} clusters, oracle {r.n_clusters}")
+    for name in ("cl_module", "cl_first", "cl_width", "cl_charge", "cl_adc_off", "cl_adc"):
+        same(name, np.asarray(g[name]).view(getattr(r, name).dtype), getattr(r, name))
+    if not np.allclose(g["cl_bary"], r.cl_bary, rtol=1e-6, atol=0):
+        raise SystemExit(f"VERIFICATION FAILED ({what}): barycenters differ from the oracle by more than 1e-6 relative")
+    same("dev_status", np.asarray(g["status"]).view(np.uint32)[:5], r.status[:5])
+
+
+def time_oracle_omp(events, calib, thresholds, budget_s: float):
+    """OpenMP build of the oracle in the paper's N x M shapes (Table 1): N events in
+    flight x M threads per event, over the divisors of the core count.  Returns (table, cores)."""
     from oracle import sst_oracle as O
     O.build()
     cores = os.cpu_count() or 1
-    shapes = sorted({(cores, 1), (max(cores // 2, 1), 2), (max(cores // 4, 1), 4), (1, cores)})
+    shapes = sorted({(cores // m, m) for m in (1, 2, 4, 8, 16, 32) if m <= cores and cores % m == 0})
     raws = [e[0] for e in events]
     fos = [e[1] for e in events]
-    best = None
+    table = []
     per = max(budget_s / len(shapes), 1.0)
     for n_outer, n_inner in shapes:
         t0 = time.perf_counter()
         done = 0
         while True:
             O.events_omp(raws, fos, calib.n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module,
-                         THRESHOLDS, n_outer, n_inner)
+                         thresholds, n_outer, n_inner)
             done += len(raws)
             dt = time.perf_counter() - t0
             if dt >= per:
                 break
-        rate = done / dt
-        if best is None or rate > best[0]:
-            best = (rate, n_outer, n_inner)
-    return best, cores
+        table.append({"N": n_outer, "M": n_inner, "events_per_s": done / dt})
+    return table, cores
+
+
+CONFIG_NOTES = {1: "generator of config 1 (2% occupancy, seeds 1..N)", 2: "generator of config 2 (6% occupancy, "
+                   "wide clusters, seeds 1..N)", 3: "generator of config 1 (2% occupancy)",
+                4: "generator of config 4 (15% occupancy, saturation, empty and full channels, seeds 1..N)"}
+
+
+def workload_config(cfg_id, n_feds, n_events, thresholds):
+    return {"workload": f"BASELINE.json config {cfg_id}: {n_events} events x {n_feds} FEDs x 96 ch x 256 strips, "
+                        f"{CONFIG_NOTES[cfg_id]}, thresholds {tuple(thresholds)}, {N_STREAMS} CUDA streams, "
+                        "one sst_unpack_cluster_batch call per step",
+            "config_id": cfg_id, "n_events": n_events, "n_feds": n_feds, "streams": N_STREAMS,
+            "l2": "working set per step (raw buffers + 86.5 MB calibration + one distinct ~20 MB output block per "
+                  "event, > 1.3 GB) exceeds the 126 MB L2; no explicit flush"}
 
 
 def run_reference(args):
@@ -216,14 +235,16 @@ def run_reference(args):
         return
     n_feds = args.n_feds
     per_step = args.ref_events
-    calib = synth.make_calibration(n_feds, synth.CONFIGS[3].bad_frac)
-    events = generate_events(3, n_feds, list(range(1, per_step + 1)), calib)
+    cfg = synth.CONFIGS[args.config]
+    thr = cfg.thresholds[0]
+    calib = synth.make_calibration(n_feds, cfg.bad_frac)
+    events = generate_events(args.config, n_feds, list(range(1, per_step + 1)), calib)
     from oracle import sst_oracle as O
     O.build()
 
     def step():
         for raw, fo, _ in events:
-            O.run(raw, fo, n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, THRESHOLDS)
+            O.run(raw, fo, n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, thr)
 
     for _ in range(args.warmup):
         step()
@@ -237,30 +258,50 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/f32/f64", "data": "synthetic",
-        "config": workload_config(n_feds, per_step),
+        "config": workload_config(args.config, n_feds, per_step, thr),
         "cpu_baseline": {"value": value, "unit": "events/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
 
 
-def workload_config(n_feds, n_events):
-    return {"workload": f"BASELINE.json config 3: {n_events} events x {n_feds} FEDs x 96 ch x 256 strips, "
-                        f"generator of config 1 (2% occupancy), thresholds (2,3,5), {N_STREAMS} CUDA streams",
-            "n_events": n_events, "n_feds": n_feds, "streams": N_STREAMS,
-            "l2": "working set per step (64 raw buffers + 86.5 MB calibration + 64 distinct output blocks "
-                  "~1.3 GB) exceeds the 126 MB L2; no explicit flush"}
-
-
 # --------------------------------------------------------------------------- GPU arm
+def ncu_traffic(cfg_id: int):
+    """Measured DRAM bytes per step (read + write of both kernels) from the committed ncu launch
+    list summary profiles/traffic.csv (rows: workload, kernel, read bytes, write bytes), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    tot, found = 0.0, False
+    for line in open(p):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 4 and f[0] == f"config{cfg_id}":
+            try:
+                tot += float(f[2]) + float(f[3])
+                found = True
+            except ValueError:
+                pass
+    return tot if found else None
+
+
+def make_detector(harness, n_feds, calib, events, device=0, hint=True):
+    max_raw = (max(int(e[0].size) for e in events) + 4095) // 4096 * 4096
+    # sst_config.fed_strips_hint (the expected maximum of present strips in one FED) sizes the
+    # shared-memory working set: taken from the data, as a site would take it from its occupancy
+    strips_hint = int(1.05 * max(int(e[2]["max_fed_strips"]) for e in events)) + 16 if hint else 0
+    det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, device=device,
+                           max_raw_bytes=max_raw, max_events_in_flight=N_STREAMS, fed_strips_hint=strips_hint)
+    return det, max_raw
+
 
 def run_sweep(args):
-    """Single-event device latency of every single-event config, and config 3 throughput against
-    the events per call (Table 1 sweeps the events in flight)."""
+    """Single-event device latency of every single-event config; config 3 throughput against the
+    events per call and against the number of streams (Table 1 sweeps the events in
+    flight); the OpenMP oracle's N x M table (Table 1)."""
     import torch
     from paper_2101_11489_b200 import binding as B, harness
     torch.cuda.set_device(0)
-    out = {"single_event": [], "events_per_call": []}
+    out = {"single_event": [], "events_per_call": [], "streams": [], "omp_oracle": None}
     for cid in (0, 1, 2, 4):
         cfg, cal, evs = synth.make_config(cid)
         ev = evs[0]
@@ -290,16 +331,16 @@ def run_sweep(args):
         del outs
         det.close()
     n_feds = args.n_feds
+    thr = THRESHOLDS
     calib = synth.make_calibration(n_feds, synth.CONFIGS[3].bad_frac)
     events = generate_events(3, n_feds, range(1, N_EVENTS + 1), calib)
-    mrb = (max(int(e[0].size) for e in events) + 4095) // 4096 * 4096
-    hint = int(1.05 * max(int(e[2]["max_fed_strips"]) for e in events)) + 16
-    det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, max_raw_bytes=mrb, fed_strips_hint=hint)
+    det, mrb = make_detector(harness, n_feds, calib, events)
     d_in = [det.upload_raw(e[0], e[1]) for e in events]
-    streams = [torch.cuda.Stream() for _ in range(N_STREAMS)]
     outs = [det.alloc_outputs(mrb // 3 + 1, mrb, dense=True) for _ in events]
-    for n in (1, 2, 4, 8, 16, 32, 64):
-        batch = B.Batch([d[0] for d in d_in[:n]], [d[1] for d in d_in[:n]], THRESHOLDS, [o.out for o in outs[:n]],
+
+    def rate(n, n_streams):
+        streams = [torch.cuda.Stream() for _ in range(n_streams)]
+        batch = B.Batch([d[0] for d in d_in[:n]], [d[1] for d in d_in[:n]], thr, [o.out for o in outs[:n]],
                         [s.cuda_stream for s in streams])
         steps = max(20, 640 // n)
         for _ in range(5):
@@ -309,11 +350,29 @@ def run_sweep(args):
         for _ in range(steps):
             B.sst_unpack_cluster_batch(det.ctx, batch)
         torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        out["events_per_call"].append({"events": n, "streams": min(n, N_STREAMS), "events_per_s": n * steps / dt,
-                                       "us_per_event": 1e6 * dt / (n * steps)})
+        return n * steps / (time.perf_counter() - t0)
+
+    for n in (1, 2, 4, 8, 16, 32, 64):
+        r = rate(n, min(n, N_STREAMS))
+        out["events_per_call"].append({"events": n, "streams": min(n, N_STREAMS), "events_per_s": r, "us_per_event": 1e6 / r})
+    for ns in (1, 2, 4, 8, 16):
+        r = rate(N_EVENTS, ns)
+        out["streams"].append({"events": N_EVENTS, "streams": ns, "events_per_s": r})
     det.close()
+    table, cores = time_oracle_omp(events[:16], calib, thr, 24.0)
+    out["omp_oracle"] = {"cores": cores, "events_per_pass": 16, "table": table}
     print(json.dumps({"sweep": out}))
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` with N > 1 and no launcher: start N ranks (one per GPU)."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    os.execv(sys.executable, cmd)
 
 
 def main():
@@ -322,21 +381,28 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4],
+                    help="BASELINE.json config the 64 events are generated from (3 = the headline workload)")
     ap.add_argument("--n-feds", type=int, default=440)
     ap.add_argument("--events", type=int, default=N_EVENTS)
     ap.add_argument("--ref-events", type=int, default=8, help="events per step of --impl reference")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle timing (rank 0, N=1)")
-    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (and with it the verification)")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--serial", action="store_true", help="also time the kernel alone on one stream")
     ap.add_argument("--sweep", action="store_true",
-                    help="instead of the bench line: single-event latency of configs 0, 1, 2, 4 and events/s against "
-                         "the number of events per call (mirrors the N sweep of PAPER.md Table 1)")
+                    help="instead of the bench line: single-event latency of configs 0, 1, 2, 4, events/s against the "
+                         "events per call and the number of streams, and the OpenMP oracle's N x M table")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3
     if args.sweep:
         return run_sweep(args)
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1:
+        return respawn_under_torchrun(args)
+    if world_env is not None and int(world_env) != args.gpus:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world_env}", file=sys.stderr)
+        sys.exit(2)
     if args.impl == "reference":
         run_reference(args)
         return
@@ -359,45 +425,22 @@ def main():
         dist.barrier()
 
     n_feds, n_events = args.n_feds, args.events
-    cfg = synth.CONFIGS[3]
+    cfg = synth.CONFIGS[args.config]
+    thr = cfg.thresholds[0]
     calib = synth.make_calibration(n_feds, cfg.bad_frac)
-    events = generate_events(3, n_feds, event_seeds_for_rank(rank, world, n_events), calib)
-    max_raw = max(int(e[0].size) for e in events)
-    max_raw = (max_raw + 4095) // 4096 * 4096
-    # sst_config.fed_strips_hint (the expected maximum of present strips in one FED) sizes the
-    # shared-memory working set: taken from the data, as a site would take it from its occupancy
-    strips_hint = int(1.05 * max(int(e[2]["max_fed_strips"]) for e in events)) + 16
-    det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, device=local_rank,
-                           max_raw_bytes=max_raw, max_events_in_flight=N_STREAMS, fed_strips_hint=strips_hint)
+    events = generate_events(args.config, n_feds, event_seeds_for_rank(rank, world, n_events), calib)
+    det, max_raw = make_detector(harness, n_feds, calib, events, device=local_rank)
     info = det.info()
     dev = det.device
     n_strips = n_feds * B.FED_STRIPS
 
-    # resident inputs
+    # resident inputs; one pooled output block per event (64 distinct blocks, ~1.3 GB)
     d_in = [det.upload_raw(e[0], e[1]) for e in events]
     cap_cl, cap_adc = max_raw // 3 + 1, max_raw
-
-    def up(x):
-        return (x + 255) // 256 * 256
-
-    # one pooled block per event, carved into the sst_output arrays
-    lay, off = {}, 0
-    for name, nbytes in (("strip_adc", n_strips), ("cl_module", 4 * cap_cl), ("cl_first", 2 * cap_cl),
-                         ("cl_width", 2 * cap_cl), ("cl_charge", 4 * cap_cl), ("cl_bary", 4 * cap_cl),
-                         ("cl_adc_off", 4 * cap_cl), ("cl_adc", cap_adc), ("n_clusters", 4), ("dev_status", 32)):
-        lay[name] = off
-        off += up(nbytes)
-    block_bytes = off
     streams = [torch.cuda.Stream(device=dev) for _ in range(N_STREAMS)]
     main_stream = torch.cuda.current_stream(dev)
-
-    def out_struct(base):
-        return B.make_output(cap_clusters=cap_cl, cap_adc=cap_adc, **{k: base + v for k, v in lay.items()})
-
-    # per-event output blocks from the library's stream-ordered pool (64 distinct blocks, ~1.3 GB)
-    blocks = [B.sst_event_alloc(det.ctx, block_bytes, streams[i % N_STREAMS].cuda_stream) for i in range(n_events)]
-    batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], THRESHOLDS, [out_struct(b) for b in blocks],
-                    [st.cuda_stream for st in streams])
+    outs = [harness.PooledOutputs(det, cap_cl, cap_adc, streams[i % N_STREAMS].cuda_stream, dense=True) for i in range(n_events)]
+    batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], thr, [o.out for o in outs], [st.cuda_stream for st in streams])
 
     def step():
         """One pass over the workload: the events of each stream share launches, one C call."""
@@ -415,17 +458,42 @@ def main():
             main_stream.wait_event(e)
         ev.record(main_stream)
 
-    # ---- verification pass (untimed): every event once, counts read back, algorithmic bytes derived
-    per_event = []
+    def timed(n_steps, warm):
+        for _ in range(warm):
+            step()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        fork_join_begin(e0)
+        for _ in range(n_steps):
+            step()
+        fork_join_end(e1)
+        torch.cuda.synchronize()
+        t_host = time.perf_counter() - t0
+        if world > 1:
+            dist.barrier()
+        return max_over_ranks(e0.elapsed_time(e1), dev), t_host
+
+    # ---- timed: device-resident inputs
+    sampler = ClockSampler(local_rank)
+    sampler.mark_start()
+    ms_total, t_host = timed(args.steps, args.warmup)
+    sampler.mark_stop()
+    clocks = sampler.finish()
+    ms_step = ms_total / args.steps
+    value = world * n_events * args.steps / (ms_total * 1e-3)
+
+    # ---- the outputs of the timed launches: counts and algorithmic bytes per event
     mod_first = np.zeros(int(calib.chan_module.max()) + 1, np.int64)
     cm = calib.chan_module.astype(np.int64)
     firsts = np.flatnonzero(np.concatenate([[True], cm[1:] != cm[:-1]]))
     mod_first[cm[firsts]] = firsts * 256
-    ver = det.alloc_outputs(cap_cl, cap_adc, dense=True)
+    results, per_event = [], []
     for i in range(n_events):
-        det.run(d_in[i][0], d_in[i][1], THRESHOLDS, ver)
-        torch.cuda.synchronize()
-        g = harness.unsigned_view(ver.numpy())
+        g = outs[i].numpy(streams[i % N_STREAMS].cuda_stream)
         st = g["status"]
         assert st[B.ST_FLAGS] == 0, f"event {i}: dev_status flags {st[B.ST_FLAGS]}"
         present = g["strip_adc"] != 0
@@ -440,44 +508,14 @@ def main():
         b_alg = int(events[i][0].size) + n_strips + 32 * s_noise + 32 * s_gain + 20 * n_cl + n_adc
         per_event.append({"n_clusters": n_cl, "n_adc": n_adc, "n_seeds": int(st[B.ST_N_SEEDS]),
                           "present": int(present.sum()), "b_alg": b_alg})
-    del ver
-    torch.cuda.synchronize()
+        results.append(g if not args.no_cpu and rank == 0 and world == 1 else None)
     b_alg_step = sum(p["b_alg"] for p in per_event)
     clusters_step = sum(p["n_clusters"] for p in per_event)
     present_step = sum(p["present"] for p in per_event)
 
-    # ---- timed: device-resident inputs
-    sampler = ClockSampler(local_rank)
-    for _ in range(args.warmup):
-        step()
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler.mark_start()
-    t_host0 = time.perf_counter()
-    fork_join_begin(e0)
-    for _ in range(args.steps):
-        step()
-    fork_join_end(e1)
-    torch.cuda.synchronize()
-    t_host = time.perf_counter() - t_host0
-    sampler.mark_stop()
-    if world > 1:
-        dist.barrier()
-    ms_total = e0.elapsed_time(e1)
-    ms_total = max_over_ranks(ms_total, dev)
-    clocks = sampler.finish()
-    ms_step = ms_total / args.steps
-    value = world * n_events * args.steps / (ms_total * 1e-3)
-
-    # ---- roofline of sst_event_kernel: launches overlap on 8 streams, so a launch's share of the
-    # device is the event-timed span / launches; also the kernel alone on one stream (serial)
+    # ---- roofline of sst_event_kernel: one launch of each kernel per step (up to 64 events per launch)
     peak, peak_src = measured_peak()
     epl = int(info.get("events_per_launch", 1))
-    # sst_unpack_cluster_batch: stream s belongs to launch group s % G, a group's events share
-    # launches of up to `epl` events; every launch is sst_event_kernel followed by sst_emit_kernel
     n_groups = min(N_STREAMS, n_events, max(1, -(-n_events // epl)))
     launches_step = sum(-(-sum(1 for e in range(n_events) if (e % N_STREAMS) % n_groups == g) // epl)
                         for g in range(n_groups))
@@ -485,50 +523,45 @@ def main():
     kernels_per_launch = int(info.get("kernels_per_event", 1))
     dur_us = 1e3 * ms_total / launches
     achieved = (b_alg_step / launches_step) / (dur_us * 1e-6) / 1e9
+    traffic = ncu_traffic(args.config)
+
+    # ---- the same with the default shared-memory sizing (fed_strips_hint = 0)
+    default_hint = None
+    if world == 1:
+        det0, _ = make_detector(harness, n_feds, calib, events, device=local_rank, hint=False)
+        main_ctx, det.ctx = det.ctx, det0.ctx
+        ms0, _ = timed(max(10, args.steps // 10), 3)
+        det.ctx = main_ctx
+        default_hint = {"value": n_events * max(10, args.steps // 10) / (ms0 * 1e-3), "unit": "events/s",
+                        "info": det0.info(), "note": "fed_strips_hint = 0: slot sized from max_raw_bytes / n_feds"}
+        det0.close()
+
+    # ---- single-event latency on one stream (launches queued behind a sleep kernel)
     serial = None
-    if True:
+    if world == 1:
         s0 = streams[0]
-        outs1 = det.alloc_outputs(cap_cl, cap_adc, dense=True)
         evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_events)]
         for rep in range(2):
             with torch.cuda.stream(s0):
                 torch.cuda._sleep(4_000_000)        # keep the stream busy while the host enqueues
             for i in range(n_events):
                 evs[i][0].record(s0)
-                det.run(d_in[i][0], d_in[i][1], THRESHOLDS, outs1, stream=s0)
+                B.sst_unpack_cluster(det.ctx, d_in[i][0], d_in[i][1], thr, outs[i].out, s0.cuda_stream)
                 evs[i][1].record(s0)
             torch.cuda.synchronize()
         d = np.array([a.elapsed_time(b) for a, b in evs]) * 1e3
         serial = {"launch_us_median": float(np.median(d)), "launch_us_min": float(d.min()),
-                  "achieved_gbs": float(np.mean([p["b_alg"] for p in per_event]) / (np.median(d) * 1e-6) / 1e9),
-                  "note": "one stream, CUDA events around each launch, launches queued behind a sleep kernel"}
-        del outs1
+                  "note": "one event per call on one stream, CUDA events around each call"}
 
     # ---- e2e: HOST buffers through sst_unpack_cluster_host_packed
-    e2e = None
+    e2e, e2e_views = None, None
     if not args.no_e2e:
-        pin = [(torch.from_numpy(e[0]).pin_memory(), torch.from_numpy(e[1].view(np.int32)).pin_memory())
-               for e in events]
-        T = N_STREAMS
-
-        def host_outputs():
-            t = {"n_clusters": torch.zeros(1, dtype=torch.int32).pin_memory(),
-                 "dev_status": torch.zeros(8, dtype=torch.int32).pin_memory(),
-                 "cl_module": torch.empty(cap_cl, dtype=torch.int32).pin_memory(),
-                 "cl_first": torch.empty(cap_cl, dtype=torch.int16).pin_memory(),
-                 "cl_width": torch.empty(cap_cl, dtype=torch.int16).pin_memory(),
-                 "cl_charge": torch.empty(cap_cl, dtype=torch.int32).pin_memory(),
-                 "cl_bary": torch.empty(cap_cl, dtype=torch.float32).pin_memory(),
-                 "cl_adc_off": torch.empty(cap_cl, dtype=torch.int32).pin_memory(),
-                 "cl_adc": torch.empty(cap_adc, dtype=torch.uint8).pin_memory()}
-            return t, B.make_output(cap_clusters=cap_cl, cap_adc=cap_adc, **t)
-
-        # one pinned, packed result block per event; one C call per step:
-        # sst_unpack_cluster_host_packed cuts the 64 events into chunks whose uploads, launches and
-        # (single, exactly-sized) downloads overlap on the 8 streams
+        pin = [(torch.from_numpy(e[0]).pin_memory(), torch.from_numpy(e[1].view(np.int32)).pin_memory()) for e in events]
+        # one pinned, packed result block per event; one C call per step: the 64 events are cut into
+        # chunks whose uploads, launches and (single, size-guessed) downloads overlap on the 8 streams
         host_blocks = [torch.zeros(64 + 20 * cap_cl + cap_adc, dtype=torch.uint8).pin_memory() for _ in range(n_events)]
         e2e_steps = max(1, min(args.steps, 20))
-        pbatch = B.PackedBatch([p[0] for p in pin], [int(e[0].size) for e in events], [p[1] for p in pin], THRESHOLDS,
+        pbatch = B.PackedBatch([p[0] for p in pin], [int(e[0].size) for e in events], [p[1] for p in pin], thr,
                                cap_cl, cap_adc, host_blocks, [st.cuda_stream for st in streams])
         counts_view = [blk.numpy()[32:36].view(np.uint32) for blk in host_blocks]
 
@@ -536,7 +569,7 @@ def main():
             B.sst_unpack_cluster_host_packed(det.ctx, pbatch)
             return sum(int(c[0]) for c in counts_view)
 
-        for _ in range(2):
+        for _ in range(3):
             e2e_step()
         torch.cuda.synchronize()
         if world > 1:
@@ -546,49 +579,69 @@ def main():
         for _ in range(e2e_steps):
             n_cl_seen += e2e_step()
         torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(dt, dev)
+        dt = max_over_ranks(time.perf_counter() - t0, dev)
         assert n_cl_seen == clusters_step * e2e_steps, "e2e cluster counts differ from the device-resident pass"
         h2d = sum(int(e[0].size) + 4 * (n_feds + 1) for e in events)
-        d2h = sum(36 + 20 * p["n_clusters"] + p["n_adc"] for p in per_event)
+        d2h = sum(64 + 20 * p["n_clusters"] + p["n_adc"] for p in per_event)
         e2e = {"value": world * n_events * e2e_steps / dt, "unit": "events/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": e2e_steps, "host_threads": 1,
                "api": "sst_unpack_cluster_host_packed (pinned host raw in; status, cluster records and ADCs out as one "
                       "packed block per event; chunks of 4 events pipelined over the 8 streams)"}
+        e2e_views = [pbatch.view(i) for i in range(n_events)]
 
-    # ---- CPU baseline (rank 0, N = 1 only)
-    cpu = cpu_omp = None
+    # ---- CPU baseline (rank 0, N = 1 only) and the verification of the timed outputs against it
+    cpu = cpu_omp = verified = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        rate, n_done, dt, ncl = time_oracle(events, calib, args.cpu_budget)
-        for i, k in enumerate(ncl):
-            assert k == per_event[i]["n_clusters"], f"event {i}: GPU {per_event[i]['n_clusters']} vs oracle {k} clusters"
+        def check(i, r):
+            compare_with_oracle(results[i], r, f"timed batch launch, event {i}")
+            results[i] = None
+            if e2e_views is not None:
+                compare_with_oracle(e2e_views[i], r, f"e2e, event {i}", dense=False)
+
+        rate, n_done, dt = time_oracle(events, calib, thr, args.cpu_budget, check=check)
+        verified = f"{n_events}/{n_events} events of the timed launches, all outputs (dense SoA, clusters, ADCs, status)" + \
+                   ("; e2e blocks: clusters, ADCs, status" if e2e_views is not None else "")
         cpu = {"value": rate, "unit": "events/s", "cores": 1, "kind": "oracle",
-               "sample": f"{n_done} events of the workload (seeds 1..{min(n_done, n_events)}), {dt:.1f} s, "
-                         "oracle/sst_oracle.c -O2 sequential; cluster counts equal the GPU's"}
-        (orate, no, ni), cores = time_oracle_omp(events[:16], calib, max(args.cpu_budget / 2, 4.0))
-        cpu_omp = {"value": orate, "unit": "events/s", "cores": cores, "kind": "oracle (OpenMP build)",
-                   "shape_NxM": f"{no}x{ni}", "sample": "16 events of the workload per pass, best of the N x M shapes"}
+               "sample": f"{n_done} events of the workload (seeds 1..{min(n_done, n_events)}), {dt:.1f} s of oracle time, "
+                         "oracle/sst_oracle.c -O2 sequential"}
+        table, cores = time_oracle_omp(events[:16], calib, thr, max(args.cpu_budget / 2, 4.0))
+        best = max(table, key=lambda t: t["events_per_s"])
+        cpu_omp = {"value": best["events_per_s"], "unit": "events/s", "cores": cores, "kind": "oracle (OpenMP build)",
+                   "shape_NxM": f"{best['N']}x{best['M']}", "table": table,
+                   "sample": "16 events of the workload per pass, N events in flight x M threads per event"}
 
     if rank == 0:
+        dram = None
+        if traffic is not None:
+            dram_gbs = traffic / (ms_step * 1e-3) / 1e9
+            dram = {"bytes_per_step": traffic, "achieved": dram_gbs, "frac": dram_gbs / peak,
+                    "source": "profiles/traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum of both kernels, "
+                              "one step) over this run's step time"}
         line = {
             "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u8/f32/f64", "data": "synthetic",
-            "config": workload_config(n_feds, n_events),
+            "config": workload_config(args.config, n_feds, n_events, thr),
+            "verified": verified,
             "strips_per_s": value * n_strips, "present_strips_per_s": value * present_step / n_events,
             "clusters_per_s": value * clusters_step / n_events,
             "host_wall_ms_per_step": 1e3 * t_host / args.steps,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": ncu_traffic("config3_event"), "peak_source": peak_src,
+                         "traffic": traffic, "peak_source": peak_src,
                          "kernel": "sst_event_kernel", "algorithmic_bytes_per_launch": b_alg_step / launches_step,
                          "events_per_launch": n_events / launches_step,
                          "launch_us": dur_us,
-                         "how": "B_alg = raw + N dense + 32 B x noise sectors of present strips + 32 B x gain "
-                                "sectors of accepted-cluster strips + 20 B x clusters + cluster ADC bytes; the launch "
-                                "groups overlap and sst_emit_kernel (the ordered move of the staged clusters) runs "
-                                "behind every sst_event_kernel, so launch duration = CUDA-event span of the timed "
-                                "region / sst_event_kernel launches (the emit kernel's time is charged to it)",
+                         "dram": dram,
+                         "limiter": "not HBM: sst_event_kernel is bound by instruction issue and the L1/LSU path "
+                                    "(profiles/r02_*.md); the calibration term of the algorithmic bytes is served by L2",
+                         "how": "achieved = algorithmic bytes per launch / launch duration, B_alg = raw + N dense + 32 B x "
+                                "noise sectors of present strips + 32 B x gain sectors of accepted-cluster strips + 20 B x "
+                                "clusters + cluster ADC bytes; sst_emit_kernel (the ordered move of the staged clusters) "
+                                "runs behind every sst_event_kernel, so launch duration = CUDA-event span of the timed "
+                                "region / sst_event_kernel launches (the emit kernel's time is charged to it); `dram` is "
+                                "the same span against the DRAM bytes ncu measured",
                          "serial": serial},
+            "default_hint": default_hint,
             "e2e": e2e, "gpu_launches": launches * kernels_per_launch, "clocks": clocks,
             "cpu_baseline": cpu, "cpu_baseline_omp": cpu_omp,
             "kernel_info": info,
@@ -596,8 +649,8 @@ def main():
                              "(TTBar PU70, ~800k strips/event; other hardware and data, context only)",
         }
         print(json.dumps(line))
-    for i, b in enumerate(blocks):
-        B.sst_event_free(det.ctx, b, streams[i % N_STREAMS].cuda_stream)
+    for i, o in enumerate(outs):
+        o.free(streams[i % N_STREAMS].cuda_stream)
     torch.cuda.synchronize()
     det.close()
     if world > 1:

@@ -1263,6 +1263,7 @@ struct sst_ctx {
     uint32_t n_geom = 0;
     bool has_calib = false;
     std::atomic<int32_t> last_err{0};
+    std::atomic<float> packed_ratio{0.0f};  // packed result bytes per raw byte seen by the last packed host call
     int sm_count = 0;
     int ctas_per_sm = 0;       // resident CTAs of kWarpsPerCta warps
     uint32_t slot_bytes = 0;   // shared-memory slot of one warp (one FED)
@@ -1946,6 +1947,12 @@ sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const
     sst_output proto{};
     proto.cap_clusters = cap_clusters;
     proto.cap_adc = cap_adc;
+    // One download per event, enqueued right behind the launch without waiting for the counts: its
+    // size is a guess from the context's running ratio of packed bytes to raw bytes; whatever a
+    // guess missed is fetched in a second copy once the counts are on the host.
+    float ratio = ctx->packed_ratio.load();
+    if (!(ratio > 0.0f)) ratio = 2.2f;
+    std::vector<size_t> guess(n_events);
     for (uint32_t e0 = 0; e0 < n_events && rc == SST_OK; e0 += kHostChunk) {
         Chunk ck{e0, std::min(kHostChunk, n_events - e0), static_cast<cudaStream_t>(streams[chunks.size() % n_streams]), nullptr};
         CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&ck.blk), per_event * ck.n, ctx->pool, ck.st));
@@ -1967,10 +1974,14 @@ sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const
             pk[i] = d_block[e0 + i];
         }
         if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st, pk, raw_bytes + e0);
-        for (uint32_t i = 0; i < ck.n; ++i)  // status and count first: they size the one big copy
-            CU(cudaMemcpyAsync(results[e0 + i].block, d_block[e0 + i], 64, cudaMemcpyDeviceToHost, ck.st));
+        for (uint32_t i = 0; i < ck.n; ++i) {
+            const size_t g = std::min(block_need, 64 + static_cast<size_t>(1.08f * ratio * raw_bytes[e0 + i]) + 4096);
+            guess[e0 + i] = g;
+            CU(cudaMemcpyAsync(results[e0 + i].block, d_block[e0 + i], g, cudaMemcpyDeviceToHost, ck.st));
+        }
         chunks.push_back(ck);
     }
+    double sum_need = 0.0, sum_raw = 0.0;
     for (const Chunk &ck : chunks) {
         CU(cudaStreamSynchronize(ck.st));
         if (rc != SST_OK) break;
@@ -1980,7 +1991,10 @@ sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const
             const uint32_t *stw = reinterpret_cast<const uint32_t *>(b);
             const size_t K = std::min(stw[SST_ST_N_CLUSTERS], cap_clusters);
             const size_t na = std::min(stw[SST_ST_N_ADC], cap_adc);
-            CU(cudaMemcpyAsync(b + 64, d_block[ck.e0 + i] + 64, 20 * K + na, cudaMemcpyDeviceToHost, ck.st));
+            const size_t need = 64 + 20 * K + na, g = guess[ck.e0 + i];
+            if (need > g) CU(cudaMemcpyAsync(b + g, d_block[ck.e0 + i] + g, need - g, cudaMemcpyDeviceToHost, ck.st));
+            sum_need += static_cast<double>(need);
+            sum_raw += static_cast<double>(raw_bytes[ck.e0 + i]);
             sst_output &v = R.view;
             v = proto;
             v.dev_status = reinterpret_cast<uint32_t *>(b);
@@ -1996,6 +2010,7 @@ sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const
         CU(cudaFreeAsync(ck.blk, ck.st));
     }
     for (const Chunk &ck : chunks) cu_ok(ctx, cudaStreamSynchronize(ck.st));
+    if (rc == SST_OK && sum_raw > 0.0) ctx->packed_ratio.store(static_cast<float>(sum_need / sum_raw));
     return rc;
 }
 
