@@ -61,7 +61,9 @@ def _gen_one(args):
     calib = _gen_one.calib
     ev = synth.make_event(cfg, calib, seed)
     meta = dict(ev.meta)
-    meta["max_fed_strips"] = int(np.count_nonzero(ev.z.reshape(n_feds, -1), axis=1).max())
+    per_fed = np.count_nonzero(ev.z.reshape(n_feds, -1), axis=1)
+    meta["max_fed_strips"] = int(per_fed.max())
+    meta["p99_fed_strips"] = int(np.percentile(per_fed, 99))
     return ev.raw, ev.fed_offsets, meta
 
 
@@ -286,9 +288,10 @@ def ncu_traffic(cfg_id: int):
 
 def make_detector(harness, n_feds, calib, events, device=0, hint=True):
     max_raw = (max(int(e[0].size) for e in events) + 4095) // 4096 * 4096
-    # sst_config.fed_strips_hint (the expected maximum of present strips in one FED) sizes the
-    # shared-memory working set: taken from the data, as a site would take it from its occupancy
-    strips_hint = int(1.05 * max(int(e[2]["max_fed_strips"]) for e in events)) + 16 if hint else 0
+    # sst_config.fed_strips_hint (present strips of a large FED) sizes the shared-memory working
+    # set: the 99th percentile of the events' FEDs, as a site would take it from its occupancy (the
+    # few larger FEDs are processed through global scratch)
+    strips_hint = int(1.02 * np.percentile([int(e[2]["p99_fed_strips"]) for e in events], 90)) + 16 if hint else 0
     det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, device=device,
                            max_raw_bytes=max_raw, max_events_in_flight=N_STREAMS, fed_strips_hint=strips_hint)
     return det, max_raw
@@ -588,6 +591,23 @@ def main():
                "api": "sst_unpack_cluster_host_packed (pinned host raw in; status, cluster records and ADCs out as one "
                       "packed block per event; chunks of 4 events pipelined over the 8 streams)"}
         e2e_views = [pbatch.view(i) for i in range(n_events)]
+        # what the link alone allows: plain copies of the same byte counts in both directions at once
+        d_up = [torch.empty(int(e[0].size), dtype=torch.uint8, device=dev) for e in events]
+        nb = [64 + 20 * p["n_clusters"] + p["n_adc"] for p in per_event]
+        d_dn = [torch.empty(n, dtype=torch.uint8, device=dev) for n in nb]
+        h_dn = [torch.empty(max(nb), dtype=torch.uint8).pin_memory() for _ in range(N_STREAMS)]
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(5):
+            for i in range(n_events):
+                with torch.cuda.stream(streams[i % N_STREAMS]):
+                    d_up[i].copy_(pin[i][0], non_blocking=True)
+                    h_dn[i % N_STREAMS][:nb[i]].copy_(d_dn[i], non_blocking=True)
+        torch.cuda.synchronize()
+        e2e["copy_floor"] = {"value": n_events * 5 / (time.perf_counter() - t0), "unit": "events/s",
+                             "note": "the step's H2D and D2H bytes as plain pinned cudaMemcpyAsync copies over the 8 "
+                                     "streams, no kernels: the PCIe ceiling of this box for this result volume"}
+        del d_up, d_dn, h_dn
 
     # ---- CPU baseline (rank 0, N = 1 only) and the verification of the timed outputs against it
     cpu = cpu_omp = verified = None

@@ -53,10 +53,11 @@ typedef struct {
                                       bytes; a FED whose end offset exceeds it (or, in the HOST
                                       entry points, the event's raw_bytes) is flagged and empty */
     uint32_t max_events_in_flight; /* hint for the pool (0 = default 8)                         */
-    uint32_t fed_strips_hint;      /* expected maximum of present (zero-suppressed) strips in one
-                                      FED; sizes the per-FED shared-memory working set.  0 = derive
-                                      it from max_raw_bytes / n_feds.  A FED above the hint is still
-                                      processed correctly, through a slower global-memory path    */
+    uint32_t fed_strips_hint;      /* present (zero-suppressed) strips of a LARGE FED, e.g. the 99th
+                                      percentile: sizes the per-FED shared-memory working set and
+                                      with it the number of FEDs in flight per SM.  0 = derive it from
+                                      max_raw_bytes / n_feds.  A FED above the hint is still processed
+                                      correctly, through a slower global-memory path               */
 } sst_config;
 
 /* S/N thresholds of the "three thresholds" algorithm: a strip is active at

@@ -1265,7 +1265,8 @@ struct sst_ctx {
     std::atomic<int32_t> last_err{0};
     std::atomic<float> packed_ratio{0.0f};  // packed result bytes per raw byte seen by the last packed host call
     int sm_count = 0;
-    int ctas_per_sm = 0;       // resident CTAs of kWarpsPerCta warps
+    int wpc = kWarpsPerCta;    // warps per CTA of a full launch
+    int ctas_per_sm = 0;       // resident CTAs of wpc warps
     uint32_t slot_bytes = 0;   // shared-memory slot of one warp (one FED)
     uint32_t warp_stride = 0;  // mbarrier + slot + tail pad
     uint32_t smem_bytes = 0;   // kWarpsPerCta * warp_stride
@@ -1354,8 +1355,9 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     const uint32_t total = n * nf;
     // warps per CTA: full CTAs once the work fills the GPU, smaller ones to spread a small launch
     const uint32_t sms = static_cast<uint32_t>(ctx->sm_count);
-    const uint32_t wpc = total >= 16u * sms ? kWarpsPerCta : total >= 8u * sms ? std::min(4, kWarpsPerCta) : total >= 4u * sms ? 2u : 1u;
-    const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (kWarpsPerCta / wpc);
+    const uint32_t wfull = static_cast<uint32_t>(ctx->wpc);
+    const uint32_t wpc = std::min(wfull, total >= 16u * sms ? 8u : total >= 8u * sms ? 4u : total >= 4u * sms ? 2u : 1u);
+    const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (wfull / wpc);
     const uint32_t grid = std::min((total + wpc - 1) / wpc, capacity);
     std::lock_guard<std::mutex> lock(ctx->slot_mu);
     sst_ctx::Slot *sl = nullptr;
@@ -1480,49 +1482,70 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (cudaMalloc(&ctx->chan_info, static_cast<size_t>(cfg->n_feds) * kChan * sizeof(uint2)) !=
         cudaSuccess)
         return fail(SST_ERR_CUDA);
-    // Shared-memory slot of one warp: payload stage + the lists {strip u16, adc u8} of the present
-    // strips (masks and cluster records reuse the payload's place), sized from the configuration's
-    // hints; FEDs that do not fit take the slow path through the global scratch.  The slot is then
-    // grown to whatever the SM's shared memory leaves at the same number of resident CTAs.
+    // Shared-memory slot of one warp, sized from the configuration's hints for the fast-path layout
+    // of fed_lists (payload with the ADC list squeezed into it, the dense window's gap, strip ids,
+    // masks, channel table); FEDs that do not fit take the slow path through the global scratch.
+    // Warps per CTA and resident CTAs are then chosen for the most resident warps, and the slot is
+    // grown to whatever the SM's shared memory leaves at that occupancy.
     cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device);
     {
         const double m = static_cast<double>(cfg->max_raw_bytes) / cfg->n_feds;  // mean payload bound
         const uint32_t p_hint = cfg->fed_strips_hint ? std::min(cfg->fed_strips_hint, static_cast<uint32_t>(kFedStrips))
                                                      : static_cast<uint32_t>(0.5 * m) + 32u;
         const uint32_t r_hint = (static_cast<uint32_t>(std::min(1.15 * m + 64.0, 65536.0)) + 15u) & ~15u;
-        uint32_t need = std::max(r_hint + kTabBytes, r_hint + 3u * p_hint);
-        need = std::min(std::max((need + 15u) & ~15u, 4096u), (227u * 1024u / kWarpsPerCta - kWarpHdr - kTailPad) & ~15u);
-        auto set_slot = [&](uint32_t slot) {
-            ctx->slot_bytes = slot;
-            ctx->warp_stride = kWarpHdr + slot + kTailPad;
-            ctx->smem_bytes = kWarpsPerCta * ctx->warp_stride;
-        };
-        set_slot(need);
+        const uint32_t p16 = (p_hint + 15u) & ~15u;
+        const uint32_t gap = r_hint >= p16 + 2048u ? 0u : p16 + 2048u - r_hint;
+        uint32_t need = r_hint + gap + 2u * p_hint + 16u * (p_hint / 32u + 3u) + kTabBytes + 32u;
+        int smem_optin = 0;
+        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device);
+        need = std::min(std::max((need + 15u) & ~15u, 4096u), (static_cast<uint32_t>(smem_optin) - kWarpHdr - kTailPad) & ~15u);
         // The dynamic shared-memory limit is per-FUNCTION state shared by every context of the
         // process: it is set to the device maximum, never to this context's size, so contexts with
         // different slot sizes can be used side by side.
-        int smem_optin = 0;
-        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device);
-        if (static_cast<uint32_t>(smem_optin) < ctx->smem_bytes ||
-            cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
+        if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
             return fail(SST_ERR_CUDA);
         cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->ctas_per_sm, sst_event_kernel, 32 * kWarpsPerCta,
-                                                          ctx->smem_bytes) != cudaSuccess || ctx->ctas_per_sm < 1)
-            return fail(SST_ERR_CUDA);
-        size_t avail = 0;
-        if (cudaOccupancyAvailableDynamicSMemPerBlock(&avail, sst_event_kernel, ctx->ctas_per_sm, 32 * kWarpsPerCta) ==
-                cudaSuccess && avail > ctx->smem_bytes) {
-            const uint32_t per_warp = static_cast<uint32_t>(std::min<size_t>(avail, static_cast<size_t>(smem_optin)) / kWarpsPerCta);
-            const uint32_t slot = (per_warp - kWarpHdr - kTailPad) & ~15u;
-            if (slot > ctx->slot_bytes) {
-                set_slot(slot);
-                int check = 0;
-                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel, 32 * kWarpsPerCta,
-                                                                  ctx->smem_bytes) != cudaSuccess || check < ctx->ctas_per_sm) {
-                    set_slot(need);  // the grown slot lost a CTA: keep the hinted size
-                }
+        const uint32_t stride = kWarpHdr + need + kTailPad;
+        int best_warps = 0;
+        for (int wpc = kWarpsPerCta; wpc >= 1; wpc >>= 1) {
+            int ctas = 0;
+            if (static_cast<size_t>(wpc) * stride > static_cast<size_t>(smem_optin)) continue;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel, 32 * wpc, static_cast<size_t>(wpc) * stride) !=
+                cudaSuccess)
+                continue;
+            if (ctas * wpc > best_warps) {
+                best_warps = ctas * wpc;
+                ctx->wpc = wpc;
+                ctx->ctas_per_sm = ctas;
             }
+        }
+        cudaGetLastError();
+        if (best_warps < 1) return fail(SST_ERR_CUDA);
+        auto set_slot = [&](uint32_t slot) {
+            ctx->slot_bytes = slot;
+            ctx->warp_stride = kWarpHdr + slot + kTailPad;
+            ctx->smem_bytes = static_cast<uint32_t>(ctx->wpc) * ctx->warp_stride;
+        };
+        set_slot(need);
+        // grow: first what the SM's shared memory divides into, then what the occupancy API offers
+        int smem_sm = 0, smem_reserved = 0;
+        cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, cfg->device);
+        cudaDeviceGetAttribute(&smem_reserved, cudaDevAttrReservedSharedMemoryPerBlock, cfg->device);
+        size_t api_avail = 0;
+        cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel, ctx->ctas_per_sm, 32 * ctx->wpc);
+        const size_t tries[2] = {smem_sm > 0 ? static_cast<size_t>(smem_sm) / ctx->ctas_per_sm - smem_reserved : 0, api_avail};
+        for (size_t avail : tries) {
+            avail = std::min<size_t>(avail, static_cast<size_t>(smem_optin));
+            if (avail <= ctx->smem_bytes) continue;
+            const uint32_t slot = (static_cast<uint32_t>(avail / ctx->wpc) - kWarpHdr - kTailPad) & ~15u;
+            if (slot <= ctx->slot_bytes) continue;
+            const uint32_t keep = ctx->slot_bytes;
+            set_slot(slot);
+            int check = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel, 32 * ctx->wpc, ctx->smem_bytes) == cudaSuccess &&
+                check >= ctx->ctas_per_sm)
+                break;
+            set_slot(keep);  // the grown slot lost a CTA
         }
         cudaGetLastError();
     }
@@ -1975,7 +1998,7 @@ sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const
         }
         if (rc == SST_OK) rc = launch_events(ctx, ck.n, r, fo, thr, po, ck.st, pk, raw_bytes + e0);
         for (uint32_t i = 0; i < ck.n; ++i) {
-            const size_t g = std::min(block_need, 64 + static_cast<size_t>(1.08f * ratio * raw_bytes[e0 + i]) + 4096);
+            const size_t g = std::min(block_need, 64 + static_cast<size_t>(1.03f * ratio * raw_bytes[e0 + i]) + 4096);
             guess[e0 + i] = g;
             CU(cudaMemcpyAsync(results[e0 + i].block, d_block[e0 + i], g, cudaMemcpyDeviceToHost, ck.st));
         }
@@ -2087,7 +2110,7 @@ const char *sst_status_string(sst_status s) {
 sst_status sst_get_info(const sst_ctx *ctx, sst_info *info) {
     if (!ctx || !info) return SST_ERR_INVALID_ARG;
     info->smem_bytes = ctx->smem_bytes;
-    info->threads = 32 * kWarpsPerCta;
+    info->threads = 32 * static_cast<uint32_t>(ctx->wpc);
     info->ctas_per_sm = static_cast<uint32_t>(ctx->ctas_per_sm);
     info->sm_count = static_cast<uint32_t>(ctx->sm_count);
     info->kernels_per_event = 2;
