@@ -30,8 +30,7 @@ def is_stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or is_stale():
-        # SST_NVCC_DEFS: extra -D switches for tuning builds (e.g. "-DSST_INLINE_EMIT=1"); empty in normal use
-        cmd = ["nvcc", *NVCC_FLAGS, *os.environ.get("SST_NVCC_DEFS", "").split(), "-I", INCLUDE, "-o", LIB, SRC]
+        cmd = ["nvcc", *NVCC_FLAGS, "-I", INCLUDE, "-o", LIB, SRC]
         if verbose:
             cmd.insert(1, "-Xptxas")
             cmd.insert(2, "-v")

@@ -3,34 +3,40 @@
 // Two kernels per launch, ONE WARP PER FED (a FED is 96 channels x 256 strips;
 // modules never cross a FED, reading s10).
 //
-// sst_event_kernel: a CTA is eight independent warps, each with a ~7 KB shared-memory slot, so 32
-// FEDs are in flight per SM and the serial parts of the method (the channel-length chain, the run
-// headers) of one FED hide behind the parallel parts of the others; there is no block-wide
-// barrier anywhere.  Warps draw (FED, event) tickets in FED-major order, so the FED's slab of the
-// calibration is read from HBM once per launch (bulk-prefetched into L2 two FEDs ahead) and serves
-// all the launch's events from L2.
+// sst_event_kernel: a CTA is up to eight independent warps, each with a ~7 KB shared-memory slot,
+// so 32 FEDs are in flight per SM and the serial parts of the method (the channel-length chain,
+// the run headers) of one FED hide behind the parallel parts of the others; there is no
+// block-wide barrier anywhere.  Warps draw (FED, event) tickets in FED-major order, so the FED's
+// slab of the calibration is read from HBM once per launch (bulk-prefetched into L2 two FEDs ahead)
+// and serves all the launch's events from L2.
 // Per FED, everything after the unpack runs in the COMPACT index space of the FED's present
 // strips (the structure of arrays of PAPER.md:31 has one entry per recorded strip):
 //
 //   a1 channel-location map : TMA bulk copy of the FED payload into the slot, the 96-step length
 //                             chain walked in shared memory (PAPER.md:31 builds it on the CPU)
-//   a2 unpack               : lane per channel: pass 1 validates the run headers and counts, a
-//                             warp scan gives every channel its slot range, pass 2 writes the
-//                             {strip, adc} lists in ascending strip order; the dense SoA is put
+//   a2 unpack               : lane per channel, run HEADERS only: pass 1 validates and counts, a
+//                             warp scan gives every channel its place in the lists, pass 2 writes the
+//                             list entry of every run's first strip; then lane per ENTRY: a ballot
+//                             finds each entry's run, its strip id and payload address follow, and
+//                             the ADC list is the payload squeezed in place.  The dense SoA is put
 //                             together in a 2 KB shared-memory window and stored as full vectors
 //   a3-a6 sweep             : lane per CHUNK of consecutive entries, walked serially: one 8-byte
 //                             gather of {noise, gain}, exact >= tests, link to the previous entry,
 //                             q = min(254, floor(adc/gain + .5)) in float32, and the open
 //                             candidate's (charge, sum noise^2 in double left to right, seed) in
 //                             registers; a candidate is tested where it ends (leftmost-seed
-//                             ownership is implicit: one test per maximal run).  Results are mask
-//                             bits (seeds, members and heads of accepted clusters)
+//                             ownership is implicit: one test per maximal run).  Results are bits
+//                             (links, seeds, ends of accepted clusters) kept in registers and
+//                             flushed by all lanes together; a bit smear turns ends into members
 //   a4 seed-index array     : seed mask + ordered compaction; materialised on request
 //   a7 ordered output, 1/2  : counts by popcount scan, cluster records built lane per cluster and
 //                             staged FED-locally in global scratch, FED totals in one 64-bit word
+//   compact SoA (request)   : the FED's lists staged as they are
 //
 // sst_emit_kernel (a7, 2/2), behind it on the same stream: exclusive prefix of the FED totals,
-// staged clusters moved to their (module, first strip)-ordered place.  No warp waits for another.
+// staged clusters moved to their (module, first strip)-ordered place; on request the clusters'
+// global hit coordinates and the compact SoA with the calibration gathered per entry
+// (PAPER.md:25, :31).  No warp waits for another.
 //
 // FEDs whose payload or lists exceed the slot run the same code on a pooled global scratch.
 // No tensor cores: nothing here is a contraction.
@@ -48,36 +54,21 @@
 
 #include "sst.h"
 
-#ifndef SST_MIN_CTAS
-#define SST_MIN_CTAS 4
-#endif
-#ifndef SST_SLAB_AHEAD
-#define SST_SLAB_AHEAD 2
-#endif
-#ifndef SST_EMIT_CTAS
-#define SST_EMIT_CTAS 8
-#endif
-#ifndef SST_HOST_CHUNK
-#define SST_HOST_CHUNK 4
-#endif
-#ifndef SST_WPC
-#define SST_WPC 8
-#endif
-#ifndef SST_MAXEV
-#define SST_MAXEV 64
-#endif
 namespace {
 
 constexpr int kChan = 96;
 constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
-constexpr int kMaxEv = SST_MAXEV;                   // events per launch
-constexpr int kWarpsPerCta = SST_WPC;       // warps (= FEDs in flight) per CTA, each with its own slot
+constexpr int kMaxEv = 64;                          // events per launch
+constexpr int kWarpsPerCta = 8;             // most warps (= FEDs in flight) per CTA, each with its own slot
+constexpr int kMinCtas = 4;                 // resident CTAs the register budget is set for (64 registers)
+constexpr int kEmitCtas = 8;                // the same for sst_emit_kernel (CTAs of 4 warps)
+constexpr uint32_t kHostChunk = 4;          // events per launch of the HOST entry points
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
 constexpr uint32_t kTabBytes = ((kChan + 1) * 4 + kChan * 2 + 15) & ~15;  // channel map of the FED, at the slot's end
 constexpr uint32_t kWarpHdr = 16;                      // mbarrier
-constexpr uint32_t kSlabAhead = SST_SLAB_AHEAD;        // FEDs between a calibration prefetch and its use
+constexpr uint32_t kSlabAhead = 2;                     // FEDs between a calibration prefetch and its use
 constexpr uint32_t kTailPad = 16;                      // readable bytes behind the slot (pass 2)
 
 // FED aggregate, one 64-bit word per (event, FED), written by sst_event_kernel and read by
@@ -1038,7 +1029,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
 // Every warp works alone: it draws (event, FED) tickets until the launch's work is used up and
 // never meets a block-wide barrier.  A CTA is just 1..kWarpsPerCta such warps sharing the SM's
 // shared memory (one driver reserve per CTA instead of one per warp).
-__global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_kernel(const __grid_constant__ KParams p) {
+__global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(const __grid_constant__ KParams p) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int lane = threadIdx.x & 31;
     uint8_t *const mine = smem_raw + static_cast<size_t>(threadIdx.x >> 5) * (kWarpHdr + p.slot_bytes + kTailPad);
@@ -1068,7 +1059,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, SST_MIN_CTAS) sst_event_ker
 // records, cluster ADCs and seeds of the FED to their final place.  Output capacity and the event
 // totals are handled here.
 template <bool kPacked>
-__global__ void __launch_bounds__(128, SST_EMIT_CTAS) sst_emit_kernel(const __grid_constant__ KParams p) {
+__global__ void __launch_bounds__(128, kEmitCtas) sst_emit_kernel(const __grid_constant__ KParams p) {
     const int lane = threadIdx.x & 31;
     const uint32_t t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (t >= p.n_events * p.n_feds) return;
@@ -1818,7 +1809,6 @@ sst_status sst_unpack_cluster_host_batch(sst_ctx *ctx, uint32_t n_events, const 
     // FED-major launch, counts back -- so the uploads, kernels and downloads of neighbouring chunks
     // overlap.  The cluster arrays are then fetched chunk by chunk with exactly-sized
     // copies while later chunks are still being processed.
-    constexpr uint32_t kHostChunk = SST_HOST_CHUNK;
     auto mapped = [](const void *h, void *&d) {
         cudaPointerAttributes a{};
         if (!h || cudaPointerGetAttributes(&a, h) != cudaSuccess) {
@@ -1960,7 +1950,6 @@ sst_status sst_unpack_cluster_host_packed(sst_ctx *ctx, uint32_t n_events, const
     SST_CU(cudaSetDevice(ctx->cfg.device));
     const uint32_t nf = ctx->cfg.n_feds;
     auto up = [](size_t b) { return (b + 255) & ~static_cast<size_t>(255); };
-    constexpr uint32_t kHostChunk = SST_HOST_CHUNK;
     struct Chunk { uint32_t e0, n; cudaStream_t st; uint8_t *blk; };
     std::vector<Chunk> chunks;
     std::vector<uint8_t *> d_block(n_events);
