@@ -68,7 +68,8 @@ constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
 constexpr uint32_t kTabBytes = ((kChan + 1) * 4 + kChan * 2 + 15) & ~15;  // channel map of the FED, at the slot's end
 constexpr uint32_t kWarpHdr = 16;                      // mbarrier
-constexpr uint32_t kSlabAhead = 2;                     // FEDs between a calibration prefetch and its use
+constexpr uint32_t kSlabAhead = 2;             
+constexpr uint32_t kSlabMinEvents = 16;  // launches with fewer events prefetch the calibration per list entry instead        // FEDs between a calibration prefetch and its use
 constexpr uint32_t kTailPad = 16;                      // readable bytes behind the slot (pass 2)
 
 // FED aggregate, one 64-bit word per (event, FED), written by sst_event_kernel and read by
@@ -392,8 +393,9 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     uint8_t *adc_l;
     // bit masks over the list entries: seeds; links, later heads of accepted clusters; ends, later
     // members of accepted clusters; per-word prefix counts
-    uint32_t *mS, *mH, *mA, *mP, *rec;
-    uint32_t rec_cap;           // cluster records besides the end sentinel
+    uint32_t *mS, *mH, *mA, *mP;
+    uint16_t *rec;              // list entries of the accepted clusters' first strips
+    uint32_t rec_cap;
     uint8_t *window = nullptr;  // 2048 bytes for the dense SoA assembly, free once the lists are complete
     if (kFast) {
         // [0, A): the payload; the ADC list takes its place ([0, P)), the rest (grown by a gap to
@@ -407,15 +409,15 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         mH = mS + (nw + 2);
         mA = mH + (nw + 2);
         mP = mA + (nw + 2);
-        rec = reinterpret_cast<uint32_t *>(slot + P16);
-        rec_cap = (S0 - P16) / 4u - 1u;
+        rec = reinterpret_cast<uint16_t *>(slot + P16);
+        rec_cap = (S0 - P16) / 2u;
         window = slot + P16;
     } else {
         const size_t eb = static_cast<size_t>(c.ev) * p.g_ents;
         const uint32_t slice = ((c.fed_start + 15u) & ~15u) + 16u * f;
         strip_l = p.g_strip + eb + slice;
         adc_l = p.g_adc + eb + slice;
-        rec = p.g_rec + eb + slice;
+        rec = reinterpret_cast<uint16_t *>(p.g_rec + eb + slice);
         mS = p.g_mask + static_cast<size_t>(c.ev) * 4u * p.g_mwords + (slice >> 5) + 4u * f;
         mH = mS + p.g_mwords;
         mA = mH + p.g_mwords;
@@ -476,6 +478,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         // In a FED without malformed channels or an overrun the per-channel constant is 2 * channel + 2
         // (two length bytes per channel up to and including the entry's own); else it is looked up.
         const bool regular = c.overrun == 0 && c.n_malformed == 0;
+        const bool entry_prefetch = p.n_events < kSlabMinEvents;
         uint32_t run_before = 0, start_before = 0, v_before = 0;  // runs / last run start / its entry below this word
         const uint32_t last = P - 1u;                             // (P > 0 inside the loop)
         uint32_t v_next = strip_l[min(static_cast<uint32_t>(lane), last)];
@@ -497,6 +500,9 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             uint32_t kc = 2u * ch + 2u;
             if (!regular) kc = ktab[ch];
             const uint32_t a = rp[min(min(e, last) + 2u * r1 + kc, c.fed_size - 1u)];  // (clamped: lanes past the end)
+            // a launch of few events cannot amortise a slab prefetch: the entry's calibration line is
+            // requested now and arrives while the dense SoA is assembled
+            if (entry_prefetch && in) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(cal + sid));
             __syncwarp();
             if (in) {
                 adc_l[e] = static_cast<uint8_t>(a);
@@ -790,7 +796,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 
     // ---------------------------------------------------------------- counts and cluster records
     // lane per mask word: exclusive prefix of (accepted heads, accepted members) per word, then
-    // every head gets its record {head entry, offset of its ADCs}
+    // every head's list entry goes into the FED's cluster list, in order
     uint32_t fed_cl = 0, fed_adc = 0, fed_seed = 0;
     {
         uint32_t run = 0;  // heads << 16 | members
@@ -810,16 +816,13 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         __syncwarp();
 #pragma unroll 1
         for (uint32_t w = lane; w < nw; w += 32) {
-            uint32_t mh = mH[w];
-            const uint32_t ma = mA[w], pre = mP[w];
-            uint32_t k = pre >> 16;
+            uint32_t mh = mH[w], k = mP[w] >> 16;
             while (mh) {
                 const uint32_t b = __ffs(mh) - 1u;
                 mh &= mh - 1u;
-                rec[k++] = (w * 32u + b) | (((pre & 0xffffu) + __popc(ma & ((1u << b) - 1u))) << 16);
+                rec[k++] = static_cast<uint16_t>(w * 32u + b);
             }
         }
-        if (P && lane == 0) rec[fed_cl] = fed_adc << 16;  // end sentinel: widths are offset differences
     }
     __syncwarp();
 
@@ -846,9 +849,28 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 #pragma unroll 1
         for (uint32_t k0 = 0; k0 < fed_cl; k0 += 32) {
             const uint32_t k = k0 + lane;
-            if (k < fed_cl) {
-                const uint32_t r0 = rec[k], r1 = rec[k + 1];
-                const uint32_t hd = r0 & 0xffffu, off = r0 >> 16, wd = (r1 >> 16) - off;
+            const bool have = k < fed_cl;
+            uint32_t hd = 0, wd = 0, off = 0;
+            if (have) {
+                hd = rec[k];
+                const uint32_t wi = hd >> 5, b = hd & 31u;
+                const uint32_t ma = mA[wi], mh = mH[wi];
+                // its ADCs start behind those of the members before it
+                off = (mP[wi] & 0xffffu) + __popc(ma & ((1u << b) - 1u));
+                // width: the members behind the head that are not heads themselves, 32 at a time
+                const uint32_t v = __funnelshift_rc(ma & ~mh, mA[wi + 1] & ~mH[wi + 1], b + 1u);
+                uint32_t n1 = __ffs(~v) - 1u;  // trailing ones
+                if (v == kFull) {
+                    n1 = 32;
+                    for (;;) {  // (the zero words behind the masks end it)
+                        const uint32_t e = hd + n1 + 1u;
+                        if (!(((mA[e >> 5] & ~mH[e >> 5]) >> (e & 31u)) & 1u)) break;
+                        ++n1;
+                    }
+                }
+                wd = 1u + n1;
+            }
+            if (have) {
                 const uint32_t st0 = strip_l[hd] & 0x7fffu;
                 const uint2 cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
                 int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
@@ -898,7 +920,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     // The first event of a FED streams the calibration slab of a FED a few places ahead into L2
     // (one bulk prefetch of 6 KB per lane): the launch's events then gather from L2, and HBM sees
     // sequential reads instead of the first-touch misses of scattered 8-byte loads.
-    if (c.ev == 0 && p.n_events > 1 && f + kSlabAhead < p.n_feds) {
+    if (c.ev == 0 && p.n_events >= kSlabMinEvents && f + kSlabAhead < p.n_feds) {
         const uint8_t *slab = reinterpret_cast<const uint8_t *>(p.calib + static_cast<size_t>(f + kSlabAhead) * kFedStrips);
         constexpr uint32_t kPiece = kFedStrips * sizeof(float2) / 32;
         asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(slab + lane * kPiece), "r"(kPiece), "l"(policy_evict_last()) : "memory");
