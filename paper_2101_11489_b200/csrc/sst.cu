@@ -205,7 +205,7 @@ __device__ __forceinline__ void st_stream(float *p, float v, unsigned long long 
 __device__ __forceinline__ bool ge_exact(float a, float t, float n) {
     const float p = __fmul_rn(t, n);
     const float e = __fmaf_rn(t, n, -p);
-    return (a > p) || (a == p && e <= 0.0f);
+    return (a > p) | ((a == p) & (e <= 0.0f));
 }
 // min(254, floor(fl32(fl32(adc / gain) + 0.5)))  (IEEE RN division and add, no contraction)
 __device__ __forceinline__ uint32_t gain_correct(float adc, float gain) {
@@ -620,23 +620,25 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         uint32_t lQ = 0, lEnd = 0;  // lead partial: the part of an earlier candidate inside this chunk
         double lN = 0.0;
         bool lSeed = false, lClosed = false;
-        // Bits are collected per lane in CHUNK-local positions (bit i = entry e0 + i), 64 entries at a
-        // time, and shifted into the masks by all lanes together (the step counter is uniform):
-        // links, seeds, and the last entries of accepted clusters.
-        uint32_t aL = 0, aE = 0, aS = 0;     // the 32 positions being filled
+        // Bits are collected per lane in CHUNK-local positions, 64 steps at a time, and shifted into
+        // the masks by all lanes together (the step counter is uniform): links and seeds of the
+        // step's entry, and "the candidate that ended with the PREVIOUS entry was accepted" -- the
+        // end bits therefore sit one position high and are flushed one entry lower.
+        uint32_t aL = 0, aE = 0, aS = 0;     // the 32 steps being filled
         uint32_t aL0 = 0, aE0 = 0, aS0 = 0;  // the 32 before them
-        auto flush64 = [&](uint32_t ebase) {  // local bit 0 = entry ebase; lower half in a?0, upper in a?
+        auto put = [&](uint32_t *m, uint32_t ebase, uint32_t lo, uint32_t hi) {  // local bit 0 = entry ebase
             const uint32_t wi = ebase >> 5, sh = ebase & 31u;
-            auto put = [&](uint32_t *m, uint32_t lo, uint32_t hi) {
-                const uint32_t w0 = lo << sh, w1 = __funnelshift_l(lo, hi, sh), w2 = sh ? hi >> (32u - sh) : 0u;
-                if (w0) atomicOr(&m[wi], w0);
-                if (w1) atomicOr(&m[wi + 1], w1);
-                if (w2) atomicOr(&m[wi + 2], w2);
-            };
-            put(mL, aL0, aL);
-            put(mE, aE0, aE);
+            const uint32_t w0 = lo << sh, w1 = __funnelshift_l(lo, hi, sh), w2 = sh ? hi >> (32u - sh) : 0u;
+            if (w0) atomicOr(&m[wi], w0);
+            if (w1) atomicOr(&m[wi + 1], w1);
+            if (w2) atomicOr(&m[wi + 2], w2);
+        };
+        auto flush64 = [&](uint32_t ebase) {  // lower half in a?0, upper in a?
+            put(mL, ebase, aL0, aL);
+            if (ebase) put(mE, ebase - 1u, aE0, aE);
+            else put(mE, 0u, __funnelshift_r(aE0, aE, 1), aE >> 1);  // (bit 0 is never set: nothing ends before entry 0)
             n_seed_lane += __popc(aS0) + __popc(aS);
-            if (want_seeds) put(mS, aS0, aS);
+            if (want_seeds) put(mS, ebase, aS0, aS);
             aL = aE = aS = aL0 = aE0 = aS0 = 0;
         };
         if (P) {  // (uniform)
@@ -645,60 +647,57 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             const uint32_t elast = min(max(e1, e0 + 1u), P) - 1u;
             uint32_t sv_n = strip_l[min(e0, P - 1u)], av_n = adc_l[min(e0, P - 1u)];
             float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
-            uint32_t bit = 1u;  // 1 << (step & 31)
 #pragma unroll 1
-            for (uint32_t i = 0; i < Lc; ++i) {  // (uniform: every lane takes Lc steps, the last lanes idle in some)
-                const uint32_t e = e0 + i;
-                const bool in = e < e1;
-                const uint32_t sv = sv_n, av = in ? av_n : 0u;
-                const float2 cv = cv_n;
-                {
-                    const uint32_t en = min(e + 1u, elast);
-                    sv_n = strip_l[en];
-                    av_n = adc_l[en];
-                    cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
-                }
-                const uint32_t s15 = sv & 0x7fffu;
-                const float af = static_cast<float>(av);
-                const bool is_act = av != 0 && ge_exact(af, p.t_ch, cv.x);
-                const bool is_seed = is_act && ge_exact(af, p.t_seed, cv.x);
-                // this entry continues the candidate of the previous one
-                const bool is_link = is_act && open && !(sv & 0x8000u) && s15 == prev_s + 1u;
-                if (in && open && !is_link) {  // the open candidate ended with entry e - 1
-                    if (lead) {
+            for (uint32_t i0 = 0; i0 < Lc; i0 += 32u) {  // (uniform: every lane takes Lc steps, the last lanes idle in some)
+                const uint32_t nsteps = min(32u, Lc - i0);
+                uint32_t bit = 1u;
+#pragma unroll 1
+                for (uint32_t j = 0; j < nsteps; ++j, bit <<= 1) {
+                    const uint32_t e = e0 + i0 + j;
+                    const bool in = e < e1;
+                    const uint32_t sv = sv_n, av = in ? av_n : 0u;
+                    const float2 cv = cv_n;
+                    {
+                        const uint32_t en = min(e + 1u, elast);
+                        sv_n = strip_l[en];
+                        av_n = adc_l[en];
+                        cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
+                    }
+                    const uint32_t s15 = sv & 0x7fffu;
+                    const float af = static_cast<float>(av);
+                    const bool is_act = (av != 0) & ge_exact(af, p.t_ch, cv.x);
+                    const bool is_seed = is_act & ge_exact(af, p.t_seed, cv.x);
+                    // this entry continues the candidate of the previous one
+                    const bool is_link = is_act & open & ((sv & 0x8000u) == 0) & (s15 == prev_s + 1u);
+                    const bool ended = in & open & !is_link;  // the open candidate ended with entry e - 1
+                    if (ended & lead) {  // (once per chunk at most)
                         lQ = Q; lN = N; lSeed = seed; lEnd = e - 1u; lClosed = true;
-                        lead = false;
-                    } else if (seed) {
+                    }
+                    {
                         const double dq = static_cast<double>(Q);
-                        if (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N)) {  // bit of entry e - 1
-                            if (bit != 1u) aE |= bit >> 1;
-                            else if (i & 32u) aE0 |= 0x80000000u;
-                            else atomicOr(&mE[(e - 1u) >> 5], 1u << ((e - 1u) & 31u));  // its 64 positions are flushed already
+                        const bool acc = ended & !lead & seed & (__dmul_rn(dq, dq) >= __dmul_rn(p.tcl2, N));
+                        aE |= acc ? bit : 0u;
+                    }
+                    lead = lead & !ended;
+                    if (is_act) {
+                        if (!is_link) {
+                            hd = e; Q = 0; N = 0.0; seed = false;
                         }
+                        const uint32_t q = gain_correct(af, cv.y);
+                        adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
+                        Q += q;
+                        const double d = static_cast<double>(cv.x);
+                        N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
+                        seed = seed | is_seed;
                     }
+                    aL |= is_link ? bit : 0u;
+                    aS |= is_seed ? bit : 0u;
+                    open = in ? is_act : open;
+                    prev_s = in ? s15 : prev_s;
                 }
-                if (is_act) {
-                    if (!is_link) {
-                        hd = e; Q = 0; N = 0.0; seed = false;
-                    }
-                    const uint32_t q = gain_correct(af, cv.y);
-                    adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
-                    Q += q;
-                    const double d = static_cast<double>(cv.x);
-                    N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
-                    seed = seed || is_seed;
-                }
-                if (is_link) aL |= bit;
-                if (is_seed) aS |= bit;
-                if (in) {
-                    open = is_act;
-                    prev_s = s15;
-                }
-                bit <<= 1;
-                if (bit == 0) {  // 32 steps done
-                    bit = 1u;
-                    if (i & 32u) {
-                        flush64(e0 + i - 63u);
+                if (nsteps == 32u) {  // a full block of 32 steps: the first of a pair is set aside, the second flushed
+                    if (i0 & 32u) {
+                        flush64(e0 + i0 - 32u);
                     } else {
                         aL0 = aL; aE0 = aE; aS0 = aS;
                         aL = aE = aS = 0;
