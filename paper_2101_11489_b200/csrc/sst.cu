@@ -1079,7 +1079,9 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
 // the FED's predecessors (exclusive prefix of clusters, ADC bytes, seeds), then moves the staged
 // records, cluster ADCs and seeds of the FED to their final place.  Output capacity and the event
 // totals are handled here.
-template <bool kPacked>
+// kExtras: some event of the launch wants hit coordinates or the compact SoA (an instantiation of
+// its own, so that the plain move keeps its registers for loads in flight).
+template <bool kPacked, bool kExtras>
 __global__ void __launch_bounds__(128, kEmitCtas) sst_emit_kernel(const __grid_constant__ KParams p) {
     const int lane = threadIdx.x & 31;
     const uint32_t t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -1167,7 +1169,7 @@ __global__ void __launch_bounds__(128, kEmitCtas) sst_emit_kernel(const __grid_c
                     st_stream(o.cl_bary + k_cl, __uint_as_float(r[j].w), pol_first);
                     st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
                     if (o.cl_snr) o.cl_snr[k_cl] = snr[j];
-                    if (o.hit_x) {  // clusters -> global hit coordinates (reading s23)
+                    if (kExtras && o.hit_x) {  // clusters -> global hit coordinates (reading s23)
                         float hx = __int_as_float(0x7fc00000), hy = hx, hz = hx;
                         if (p.geom && r[j].x < p.n_geom) {
                             const float2 *gm = reinterpret_cast<const float2 *>(p.geom) + 3u * static_cast<size_t>(r[j].x);
@@ -1210,7 +1212,7 @@ __global__ void __launch_bounds__(128, kEmitCtas) sst_emit_kernel(const __grid_c
     // event's recorded strips (exclusive prefix of the FEDs' non-zero entries), with the
     // calibration as it was uploaded gathered per entry
     uint32_t n_present = 0;
-    if (!packed && o.compact_strip) {
+    if (kExtras && !packed && o.compact_strip) {
         const uint32_t *pr = p.fed_present + static_cast<size_t>(ev) * p.n_feds;
         uint32_t base = 0;
 #pragma unroll 4
@@ -1441,8 +1443,11 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     if (err == cudaSuccess) {
         // every warp draws one ticket too many before it stops
         sl->ticket_base += static_cast<unsigned long long>(total) + grid * wpc;
-        if (packed) sst_emit_kernel<true><<<(total + 3) / 4, 128, 0, st>>>(kp);
-        else sst_emit_kernel<false><<<(total + 3) / 4, 128, 0, st>>>(kp);
+        bool extras = false;
+        for (uint32_t e = 0; e < n; ++e) extras = extras || outs[e]->hit_x || outs[e]->compact_strip;
+        if (packed) sst_emit_kernel<true, false><<<(total + 3) / 4, 128, 0, st>>>(kp);
+        else if (extras) sst_emit_kernel<false, true><<<(total + 3) / 4, 128, 0, st>>>(kp);
+        else sst_emit_kernel<false, false><<<(total + 3) / 4, 128, 0, st>>>(kp);
         err = cudaGetLastError();
     }
     if (err != cudaSuccess) {
