@@ -502,7 +502,9 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             const uint32_t a = rp[min(min(e, last) + 2u * r1 + kc, c.fed_size - 1u)];  // (clamped: lanes past the end)
             // a launch of few events cannot amortise a slab prefetch: the entry's calibration line is
             // requested now and arrives while the dense SoA is assembled
-            if (entry_prefetch && in) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(cal + sid));
+            if (entry_prefetch) {  // (uniform)
+                if (in) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(cal + sid));
+            }
             __syncwarp();
             if (in) {
                 adc_l[e] = static_cast<uint8_t>(a);
@@ -872,13 +874,29 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             if (have) {
                 const uint32_t st0 = strip_l[hd] & 0x7fffu;
                 const uint2 cm = __ldg(cinfo + (st0 >> 8));  // in flight during the sums
-                int Q = 0, M = 0;  // M <= 254 * 768^2 / 2
+                // The first four corrected ADCs in one word (two aligned loads of the list, which may be
+                // read a few bytes past its end): charge and first moment as byte dot products, the
+                // staged bytes from the same register.  Wider clusters (few) go on in a loop.
+                uint32_t q4;
+                {
+                    const uint32_t *w = reinterpret_cast<const uint32_t *>(adc_l + (hd & ~3u));
+                    q4 = __funnelshift_r(w[0], w[1], 8u * (hd & 3u));
+                    if (wd < 4u) q4 &= (1u << (8u * wd)) - 1u;
+                }
+                int Q = __dp4a(q4, 0x01010101u, 0u), M = __dp4a(q4, 0x03020100u, 0u);  // M <= 254 * 768^2 / 2
+                {
+                    uint8_t *d = sa + off;  // neighbouring lanes write neighbouring bytes
+                    d[0] = static_cast<uint8_t>(q4);
+                    if (wd > 1u) d[1] = static_cast<uint8_t>(q4 >> 8);
+                    if (wd > 2u) d[2] = static_cast<uint8_t>(q4 >> 16);
+                    if (wd > 3u) d[3] = static_cast<uint8_t>(q4 >> 24);
+                }
 #pragma unroll 1
-                for (uint32_t j = 0; j < wd; ++j) {
+                for (uint32_t j = 4; j < wd; ++j) {
                     const int q = adc_l[hd + j];
                     Q += q;
                     M += static_cast<int>(j) * q;
-                    sa[off + j] = static_cast<uint8_t>(q);  // neighbouring lanes write neighbouring bytes
+                    sa[off + j] = static_cast<uint8_t>(q);
                 }
                 const uint32_t first = st0 - (cm.y & 0xffu) * kStrip;
                 // barycenter in float32: first + M/Q is good to ~2e-7 relative (tolerance 1e-6)
