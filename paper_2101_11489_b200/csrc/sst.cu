@@ -178,11 +178,6 @@ __device__ __forceinline__ float2 ld_calib(const float2 *p, unsigned long long p
     return v;
 }
 // streaming stores of the outputs
-__device__ __forceinline__ void st_stream(uint4 *p, uint4 v, unsigned long long pol) {
-    asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
-                 "r"(v.w), "l"(pol)
-                 : "memory");
-}
 __device__ __forceinline__ void st_stream(uint8_t *p, uint32_t v, unsigned long long pol) {
     asm volatile("st.global.L2::cache_hint.u8 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(pol) : "memory");
 }
@@ -543,7 +538,8 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // ---------------------------------------------------------------- a2: dense SoA
     // The FED's 24576-byte block of the dense strip array is put together 2048 strips at a time
     // in a shared-memory window (zeros, then the present strips of the window from the sorted
-    // lists) and leaves as full 16-byte stores: no zero-fill pass over HBM, no byte scatter.
+    // lists) and leaves as one TMA bulk store per window: no zero-fill pass over HBM, no byte
+    // scatter, and the way out costs the LSU pipe nothing.
     if (dense) {
         if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0 && window) {
             constexpr uint32_t kWin = 2048;
@@ -567,14 +563,20 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     i0 += cnt;
                     if (cnt < 64u) break;
                 }
+                // out: one TMA bulk store of the window by lane 0 (the generic-proxy writes of all lanes
+                // are fenced first), then zeros again once the copy engine has read it
+                fence_proxy_async();
                 __syncwarp();
-                // out, and zero again for the next window in the same sweep
-#pragma unroll
-                for (uint32_t k = 0; k < kWin / 512u; ++k) {
-                    const uint4 v = win[lane + 32u * k];
-                    win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
-                    st_stream(reinterpret_cast<uint4 *>(dense + base) + lane + 32u * k, v, pol_first);
+                if (lane == 0) {
+                    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dense + base),
+                                 "r"(smem_addr(window)), "r"(kWin), "l"(pol_first)
+                                 : "memory");
+                    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
                 }
+                __syncwarp();
+#pragma unroll
+                for (uint32_t k = 0; k < kWin / 512u; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
             }
         } else {  // unaligned output or no room for a window: bytes
 #pragma unroll 1
