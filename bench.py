@@ -528,6 +528,39 @@ def main():
     achieved = (b_alg_step / launches_step) / (dur_us * 1e-6) / 1e9
     traffic = ncu_traffic(args.config)
 
+    # ---- two batches in flight: consecutive steps alternate between two halves of the stream set (and
+    # two sets of output blocks), so the ordered move of one step overlaps the event kernel of the next
+    pipelined, results_b = None, None
+    if world == 1:
+        half = N_STREAMS // 2
+        sets = []
+        for h in range(2):
+            ss = streams[h * half:(h + 1) * half]
+            oo = outs if h == 0 else [harness.PooledOutputs(det, cap_cl, cap_adc, ss[i % half].cuda_stream, dense=True)
+                                      for i in range(n_events)]
+            sets.append((ss, oo, B.Batch([d[0] for d in d_in], [d[1] for d in d_in], thr, [o.out for o in oo],
+                                         [st.cuda_stream for st in ss])))
+        torch.cuda.synchronize()
+        for i in range(6):
+            B.sst_unpack_cluster_batch(det.ctx, sets[i % 2][2])
+        torch.cuda.synchronize()
+        n_p = max(2, args.steps // 2 * 2)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        fork_join_begin(e0)
+        for i in range(n_p):
+            B.sst_unpack_cluster_batch(det.ctx, sets[i % 2][2])
+        fork_join_end(e1)
+        torch.cuda.synchronize()
+        pipelined = {"value": n_events * n_p / (e0.elapsed_time(e1) * 1e-3), "unit": "events/s", "steps": n_p,
+                     "note": "the same step issued alternately on streams 0-3 and 4-7 with two sets of output blocks: "
+                             "two batches in flight, the move of one overlapping the event kernel of the next (a caller's "
+                             "choice; `value` is one batch at a time)"}
+        if not args.no_cpu and rank == 0:
+            results_b = [sets[1][1][i].numpy(sets[1][0][i % half].cuda_stream) for i in range(n_events)]
+        for i, o in enumerate(sets[1][1]):
+            o.free(sets[1][0][i % half].cuda_stream)
+        torch.cuda.synchronize()
+
     # ---- the same with the default shared-memory sizing (fed_strips_hint = 0)
     default_hint = None
     if world == 1:
@@ -648,11 +681,15 @@ def main():
         def check(i, r):
             compare_with_oracle(results[i], r, f"timed batch launch, event {i}")
             results[i] = None
+            if results_b is not None:
+                compare_with_oracle(results_b[i], r, f"pipelined batches, event {i}")
+                results_b[i] = None
             if e2e_views is not None:
                 compare_with_oracle(e2e_views[i], r, f"e2e, event {i}", dense=False)
 
         rate, n_done, dt = time_oracle(events, calib, thr, args.cpu_budget, check=check)
         verified = f"{n_events}/{n_events} events of the timed launches, all outputs (dense SoA, clusters, ADCs, status)" + \
+                   ("; the second output set of the pipelined leg likewise" if results_b is not None else "") + \
                    ("; e2e blocks: clusters, ADCs, status" if e2e_views is not None else "")
         cpu = {"value": rate, "unit": "events/s", "cores": 1, "kind": "oracle",
                "sample": f"{n_done} events of the workload (seeds 1..{min(n_done, n_events)}), {dt:.1f} s of oracle time, "
@@ -694,6 +731,7 @@ def main():
                                 "region / sst_event_kernel launches (the emit kernel's time is charged to it); `dram` is "
                                 "the same span against the DRAM bytes ncu measured",
                          "serial": serial},
+            "pipelined": pipelined,
             "default_hint": default_hint,
             "e2e": e2e, "h2d_overlap": h2d_overlap, "gpu_launches": launches * kernels_per_launch, "clocks": clocks,
             "cpu_baseline": cpu, "cpu_baseline_omp": cpu_omp,
