@@ -1110,6 +1110,9 @@ __global__ void __launch_bounds__(128, kEmitCtas) sst_emit_kernel(const __grid_c
     const EventDesc &E = p.ev[ev];
     sst_output o = E.out;
     constexpr bool packed = kPacked;  // every event of a launch is, or none
+    // programmatic dependent launch: this grid may become resident while sst_event_kernel drains;
+    // nothing of that kernel is read before it has completed
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
     const unsigned long long own = st[f];
     const uint32_t fed_cl = static_cast<uint32_t>(own & 0x3fffull), fed_adc = static_cast<uint32_t>((own >> kShAdc) & 0x7fffull),
@@ -1465,10 +1468,22 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         sl->ticket_base += static_cast<unsigned long long>(total) + grid * wpc;
         bool extras = false;
         for (uint32_t e = 0; e < n; ++e) extras = extras || outs[e]->hit_x || outs[e]->compact_strip;
-        if (packed) sst_emit_kernel<true, false><<<(total + 3) / 4, 128, 0, st>>>(kp);
-        else if (extras) sst_emit_kernel<false, true><<<(total + 3) / 4, 128, 0, st>>>(kp);
-        else sst_emit_kernel<false, false><<<(total + 3) / 4, 128, 0, st>>>(kp);
-        err = cudaGetLastError();
+        // the move is launched as a programmatic dependent of the event kernel: its CTAs are set up
+        // while that kernel's last warps finish (the kernel itself waits for its completion)
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3((total + 3) / 4);
+        lc.blockDim = dim3(128);
+        lc.dynamicSmemBytes = 0;
+        lc.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        lc.attrs = at;
+        lc.numAttrs = 1;
+        if (packed) err = cudaLaunchKernelEx(&lc, sst_emit_kernel<true, false>, kp);
+        else if (extras) err = cudaLaunchKernelEx(&lc, sst_emit_kernel<false, true>, kp);
+        else err = cudaLaunchKernelEx(&lc, sst_emit_kernel<false, false>, kp);
+        if (err == cudaSuccess) err = cudaGetLastError();
     }
     if (err != cudaSuccess) {
         // a launch that did not happen must not leave the stream's ticket counter and the host's
