@@ -803,3 +803,84 @@ def test_hits_without_geometry_are_nan_and_host_entry_points_refuse(H, oracle):
                                       B.make_output(cap_clusters=cc, cap_adc=cc, **h))
     finally:
         det.close()
+
+
+# ------------------------------------------------------------------ randomised structure
+def _random_event(rng, n_feds):
+    """Raw bytes with structure the generator never makes: any occupancy, recorded zeros, runs split
+    into abutting pieces, full channels in both encodings, modules of 1-5 channels, a few malformed
+    channels; returns (raw, fed_offsets, calibration arrays, module map)."""
+    n = n_feds * synth.FED_STRIPS
+    occ = float(rng.choice([0.0, 0.003, 0.04, 0.15, 0.5, 0.95]))
+    keep = rng.random(n) < occ
+    # correlated neighbours so that runs and multi-strip clusters exist
+    keep |= np.roll(keep, 1) & (rng.random(n) < 0.5)
+    z = np.where(keep, rng.integers(0, 256, n), 0).astype(np.uint8)        # recorded zeros included
+    z = np.where(keep & (rng.random(n) < 0.05), rng.choice([254, 255], n), z).astype(np.uint8)
+    full = rng.random(n_feds * 96) < 0.02
+    feds = []
+    for f in range(n_feds):
+        chans = []
+        for c in range(96):
+            ch = f * 96 + c
+            row_keep = keep[ch * 256:(ch + 1) * 256].copy()
+            row = z[ch * 256:(ch + 1) * 256]
+            if full[ch]:
+                row_keep[:] = True
+            runs, s = [], 0
+            while s < 256:
+                if not row_keep[s]:
+                    s += 1
+                    continue
+                e = s
+                while e < 256 and row_keep[e]:
+                    e += 1
+                # split some runs into abutting pieces (255 + 1 and the like are legal, reading s2)
+                cuts = [s] + sorted(set(int(x) for x in rng.integers(s + 1, e, rng.integers(0, 3)) if s < x < e)) + [e] \
+                    if e - s > 1 and rng.random() < 0.3 else [s, e]
+                for a, b in zip(cuts[:-1], cuts[1:]):
+                    runs.append((a, [int(v) for v in row[a:b]]))
+                s = e
+            body = synth.channel_bytes(runs)
+            r = rng.random()
+            if r < 0.01 and len(body) > 4:          # malformed: a run that passes strip 255
+                body = body[:2] + bytes([250, 20]) + body[4:]
+            elif r < 0.02 and len(body) > 2:        # malformed: payload one byte short
+                body = (len(body) - 3).to_bytes(2, "little") + body[2:-1]
+            chans.append(body)
+        feds.append(chans)
+    raw, fo = synth.assemble_feds(feds)
+    noise = (0.5 + 8.0 * rng.random(n)).astype(np.float32)
+    gain = (0.3 + 2.5 * rng.random(n)).astype(np.float32)
+    bad = (rng.random(n) < float(rng.choice([0.0, 0.02, 0.3]))).astype(np.uint8)
+    sizes = [int(x) for x in rng.integers(1, 6, 40)]
+    cm = cases.module_map_from_sizes(n_feds, sizes)
+    return raw, fo, gain, noise, bad, cm
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_structure(H, oracle, seed):
+    rng = np.random.Generator(np.random.PCG64(1000 + seed))
+    n_feds = int(rng.integers(1, 4))
+    raw, fo, gain, noise, bad, cm = _random_event(rng, n_feds)
+    thr = (float(rng.choice([0.5, 1.5, 2.0, 3.0])), float(rng.choice([1.0, 2.5, 3.0, 6.0])), float(rng.choice([0.5, 4.0, 5.0, 12.0])))
+    mrb = max(int(raw.size), 16)
+    geom = synth.make_geometry(cm, seed=seed + 1)
+    class Cal:
+        pass
+    cal = Cal()
+    cal.gain, cal.noise, cal.bad = gain, noise, bad
+    det = H.Detector(n_feds, gain, noise, bad, cm, max_raw_bytes=mrb, fed_strips_hint=int(rng.choice([0, 200, 30000])))
+    try:
+        det.upload_geometry(geom)
+        d_raw, d_fo = det.upload_raw(raw, fo)
+        outs = det.alloc_outputs(mrb, mrb + 1, chan_map=True, seeds=True, snr=True, compact=True, hits=True, cap_compact=mrb + 1)
+        for _ in range(2):
+            det.run(d_raw, d_fo, thr, outs)
+        det.torch.cuda.synchronize()
+        g = H.unsigned_view(outs.numpy())
+        r = oracle.run(raw, fo, n_feds, gain, noise, bad, cm, thr, cap_clusters=mrb, cap_adc=mrb + 1)
+        compare(g, r)
+        compare_next(g, r, oracle, cal, geom)
+    finally:
+        det.close()
