@@ -19,7 +19,7 @@
 //                             list entry of every run's first strip; then lane per ENTRY: a ballot
 //                             finds each entry's run, its strip id and payload address follow, and
 //                             the ADC list is the payload squeezed in place.  The dense SoA is put
-//                             together in a 2 KB shared-memory window and stored as full vectors
+//                             together in a 2 KB shared-memory window that leaves by TMA bulk store
 //   a3-a6 sweep             : lane per CHUNK of consecutive entries, walked serially: one 8-byte
 //                             gather of {noise, gain}, exact >= tests, link to the previous entry,
 //                             q = min(254, floor(adc/gain + .5)) in float32, and the open
@@ -59,18 +59,18 @@ namespace {
 constexpr int kChan = 96;
 constexpr int kStrip = 256;
 constexpr int kFedStrips = kChan * kStrip;  // 24576
-constexpr int kMaxEv = 64;                          // events per launch
-constexpr int kWarpsPerCta = 8;             // most warps (= FEDs in flight) per CTA, each with its own slot
-constexpr int kMinCtas = 4;                 // resident CTAs the register budget is set for (64 registers)
-constexpr int kEmitCtas = 8;                // the same for sst_emit_kernel (CTAs of 4 warps)
-constexpr uint32_t kHostChunk = 4;          // events per launch of the HOST entry points
+constexpr int kMaxEv = 64;        // events per launch
+constexpr int kWarpsPerCta = 8;   // most warps (= FEDs in flight) per CTA, each with its own slot
+constexpr int kMinCtas = 4;       // resident CTAs the register budget is set for (64 registers)
+constexpr int kEmitCtas = 8;      // the same for sst_emit_kernel (CTAs of 4 warps)
+constexpr uint32_t kHostChunk = 4;       // events per launch of the HOST entry points
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
-constexpr uint32_t kTabBytes = ((kChan + 1) * 4 + kChan * 2 + 15) & ~15;  // channel map of the FED, at the slot's end
-constexpr uint32_t kWarpHdr = 16;                      // mbarrier
-constexpr uint32_t kSlabAhead = 2;             
-constexpr uint32_t kSlabMinEvents = 16;  // launches with fewer events prefetch the calibration per list entry instead        // FEDs between a calibration prefetch and its use
-constexpr uint32_t kTailPad = 16;                      // readable bytes behind the slot (pass 2)
+constexpr uint32_t kTabBytes = ((kChan + 1) * 4 + kChan * 2 + 15) & ~15;  // channel table of the FED, at the slot's end
+constexpr uint32_t kWarpHdr = 16;        // mbarrier in front of a warp's slot
+constexpr uint32_t kTailPad = 16;        // readable bytes behind the slot
+constexpr uint32_t kSlabAhead = 2;       // FEDs between a calibration slab prefetch and its use
+constexpr uint32_t kSlabMinEvents = 16;  // launches with fewer events prefetch the calibration per list entry instead
 
 // FED aggregate, one 64-bit word per (event, FED), written by sst_event_kernel and read by
 // sst_emit_kernel: overrun << 51 | malformed channels (7) << 44 | seeds (15) << 29 | cluster ADC
@@ -96,12 +96,12 @@ struct KParams {
     uint16_t *s_csid;          // staged list of a FED: strip ids and raw ADCs, for the compact SoA
     uint8_t *s_cadc;
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
-    unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, +total+warps)
+    unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, + tickets + warps)
     unsigned long long ticket_base;
     // global scratch of the slow path, one slice set per event
     uint16_t *g_strip;
     uint8_t *g_adc;
-    uint32_t *g_rec;   // slow-path cluster records
+    uint32_t *g_rec;   // slow-path cluster lists (16-bit entries)
     uint32_t *g_mask;  // 4 arrays of g_mwords per event
     uint32_t g_ents, g_mwords;
     // staging of the FED-local results, read by sst_emit_kernel
@@ -268,11 +268,11 @@ __device__ __forceinline__ void walk_chain_speculative(uint32_t stage_addr, uint
 }
 
 struct FedCtx {
-    uint32_t ticket, ev, f;
+    uint32_t ev, f;
     uint32_t fo0;                  // the FED's start offset as given (reported in chan_off)
     uint32_t fed_start, fed_size;  // what is read: [fed_start, +fed_size), empty for a bad FED
     uint32_t overrun, n_malformed;
-    uint32_t P, R;                 // present strips (list entries) and runs of the FED
+    uint32_t P;                    // present strips (list entries) of the FED
     uint32_t off[3], len[3];       // of channels lane, lane+32, lane+64
     uint32_t ebase[3];             // first list entry of those channels
     uint32_t opens;                // bit k: channel lane+32k opens a module
@@ -394,7 +394,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     uint8_t *window = nullptr;  // 2048 bytes for the dense SoA assembly, free once the lists are complete
     if (kFast) {
         // [0, A): the payload; the ADC list takes its place ([0, P)), the rest (grown by a gap to
-        // 2048 bytes when the dense SoA is wanted) holds the window and then the cluster records.
+        // 2048 bytes when the dense SoA is wanted) holds the window and then the cluster list.
         // Behind it the strip ids (2P bytes) and the masks.
         const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (P + 15u) & ~15u;
         const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
@@ -928,7 +928,6 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
                                             const uint32_t ticket, const int lane, const bool force_slow,
                                             uint32_t &mbar_phase, uint32_t &next_ticket) {
     FedCtx c;
-    c.ticket = ticket;
     // FED-major order: the same FED of all the launch's events back to back, so the FED's slab of
     // the calibration (196 KB) is reused from L2 while it is hot
     c.f = ticket / p.n_events;
@@ -1054,11 +1053,10 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         ktab[lane + 32 * k] = c.off[k] - (ex & 0xffffu) - 2u * (ex >> 16);
         tot += __shfl_sync(kFull, inc, 31);
     }
-    c.P = tot & 0xffffu;  // present strips of the FED (<= 24576), runs <= 12288
-    c.R = tot >> 16;
+    c.P = tot & 0xffffu;  // present strips of the FED (<= 24576; the runs, <= 12288, sit in the upper half)
     __syncwarp();
 
-    // fast path: window / cluster records, strip ids and masks fit behind the ADC list
+    // fast path: window / cluster list, strip ids and masks fit behind the ADC list
     const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (c.P + 15u) & ~15u;
     const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
     if (!force_slow && staged && ((S0 + 2u * c.P + 15u) & ~15u) + 16u * (((c.P + 31u) >> 5) + 2u) + kTabBytes <= p.slot_bytes)
