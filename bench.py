@@ -286,14 +286,18 @@ def ncu_traffic(cfg_id: int):
     return tot if found else None
 
 
-def make_detector(harness, n_feds, calib, events, device=0, hint=True):
+MOVE_MODE = 0  # sst_config.move_mode of the detectors the bench makes (--move-mode)
+
+
+def make_detector(harness, n_feds, calib, events, device=0, hint=True, move_mode=None):
     max_raw = (max(int(e[0].size) for e in events) + 4095) // 4096 * 4096
     # sst_config.fed_strips_hint (present strips of a large FED) sizes the shared-memory working
     # set: the 99th percentile of the events' FEDs, as a site would take it from its occupancy (the
     # few larger FEDs are processed through global scratch)
     strips_hint = int(1.02 * np.percentile([int(e[2]["p99_fed_strips"]) for e in events], 90)) + 16 if hint else 0
     det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, device=device,
-                           max_raw_bytes=max_raw, max_events_in_flight=N_STREAMS, fed_strips_hint=strips_hint)
+                           max_raw_bytes=max_raw, max_events_in_flight=N_STREAMS, fed_strips_hint=strips_hint,
+                           move_mode=MOVE_MODE if move_mode is None else move_mode)
     return det, max_raw
 
 
@@ -392,10 +396,14 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle timing (rank 0, N=1)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (and with it the verification)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--move-mode", type=int, default=0, choices=[0, 1],
+                    help="sst_config.move_mode: 0 = the ordered move inside sst_event_kernel, 1 = sst_emit_kernel behind it")
     ap.add_argument("--sweep", action="store_true",
                     help="instead of the bench line: single-event latency of configs 0, 1, 2, 4, events/s against the "
                          "events per call and the number of streams, and the OpenMP oracle's N x M table")
     args = ap.parse_args()
+    global MOVE_MODE
+    MOVE_MODE = args.move_mode
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3
     if args.sweep:
@@ -572,6 +580,18 @@ def main():
                         "info": det0.info(), "note": "fed_strips_hint = 0: slot sized from max_raw_bytes / n_feds"}
         det0.close()
 
+    # ---- the same with the other way of moving the staged clusters (sst_config.move_mode)
+    other_move = None
+    if world == 1:
+        det1, _ = make_detector(harness, n_feds, calib, events, device=local_rank, move_mode=1 - MOVE_MODE)
+        main_ctx, det.ctx = det.ctx, det1.ctx
+        ms1, _ = timed(max(10, args.steps // 4), 3)
+        det.ctx = main_ctx
+        other_move = {"value": n_events * max(10, args.steps // 4) / (ms1 * 1e-3), "unit": "events/s", "move_mode": 1 - MOVE_MODE,
+                      "note": "move_mode 0 = staged clusters moved inside sst_event_kernel (one launch per batch), "
+                              "1 = by sst_emit_kernel behind it (two launches)"}
+        det1.close()
+
     # ---- single-event latency on one stream (launches queued behind a sleep kernel)
     serial = None
     if world == 1:
@@ -733,7 +753,7 @@ def main():
                          "serial": serial},
             "pipelined": pipelined,
             "default_hint": default_hint,
-            "e2e": e2e, "h2d_overlap": h2d_overlap, "gpu_launches": launches * kernels_per_launch, "clocks": clocks,
+            "other_move": other_move, "e2e": e2e, "h2d_overlap": h2d_overlap, "gpu_launches": launches * kernels_per_launch, "clocks": clocks,
             "cpu_baseline": cpu, "cpu_baseline_omp": cpu_omp,
             "kernel_info": info,
             "paper_context": "PAPER.md Table 1: best 649 events/s on one P100, 560 events/s on 28 Broadwell cores "

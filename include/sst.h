@@ -58,6 +58,11 @@ typedef struct {
                                       with it the number of FEDs in flight per SM.  0 = derive it from
                                       max_raw_bytes / n_feds.  A FED above the hint is still processed
                                       correctly, through a slower global-memory path               */
+    uint32_t move_mode;            /* how the staged clusters reach their ordered place (same results):
+                                      0 = inside sst_event_kernel, by the warps that find the FED work
+                                      used up (one launch; launches that want the packed host block, hit
+                                      coordinates or the compact SoA always take the second kernel);
+                                      1 = always by sst_emit_kernel, launched behind it              */
 } sst_config;
 
 /* S/N thresholds of the "three thresholds" algorithm: a strip is active at

@@ -27,7 +27,7 @@ EXPORTS = ["sst_create", "sst_upload_calib", "sst_upload_geometry", "sst_unpack_
 
 class sst_config(C.Structure):
     _fields_ = [("n_feds", C.c_uint32), ("device", C.c_int32), ("max_raw_bytes", C.c_uint32),
-                ("max_events_in_flight", C.c_uint32), ("fed_strips_hint", C.c_uint32)]
+                ("max_events_in_flight", C.c_uint32), ("fed_strips_hint", C.c_uint32), ("move_mode", C.c_uint32)]
 
 
 class sst_thresholds(C.Structure):
@@ -116,9 +116,9 @@ def _ptr(t) -> Optional[int]:
 
 
 def sst_create(n_feds: int, device: int = 0, max_raw_bytes: int = 1 << 22, max_events_in_flight: int = 8,
-               fed_strips_hint: int = 0):
+               fed_strips_hint: int = 0, move_mode: int = 0):
     L = load()
-    cfg = sst_config(n_feds, device, max_raw_bytes, max_events_in_flight, fed_strips_hint)
+    cfg = sst_config(n_feds, device, max_raw_bytes, max_events_in_flight, fed_strips_hint, move_mode)
     ctx = C.c_void_p()
     _check(None, L.sst_create(C.byref(cfg), C.byref(ctx)), "sst_create")
     return ctx

@@ -75,7 +75,10 @@ constexpr uint32_t kSlabMinEvents = 16;  // launches with fewer events prefetch 
 // FED aggregate, one 64-bit word per (event, FED), written by sst_event_kernel and read by
 // sst_emit_kernel: overrun << 51 | malformed channels (7) << 44 | seeds (15) << 29 | cluster ADC
 // bytes (15) << 14 | clusters (14).
-constexpr int kShOver = 51, kShMalf = 44, kShSeed = 29, kShAdc = 14;
+// Bits 52..63 carry the launch's epoch (1..4095): a word counts as published by THIS launch only
+// with the right tag, which is what the in-kernel move (below) waits for.
+constexpr int kShOver = 51, kShMalf = 44, kShSeed = 29, kShAdc = 14, kShEpoch = 52;
+constexpr uint32_t kEpochs = 4095;
 
 struct EventDesc {
     const uint8_t *raw;
@@ -98,6 +101,9 @@ struct KParams {
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
     unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, + tickets + warps)
     unsigned long long ticket_base;
+    uint32_t epoch;       // tag of this launch's FED aggregates
+    uint32_t move_chunk;  // clusters per bulk copy of the in-kernel move (from the slot size)
+    uint32_t fused_move;  // 1: sst_event_kernel moves the staged clusters itself once its FED tickets are used up
     // global scratch of the slow path, one slice set per event
     uint16_t *g_strip;
     uint8_t *g_adc;
@@ -836,15 +842,8 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // ordered place -- no warp ever waits for another one.
     const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
     const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
-    if (lane == 0) {
-        p.fed_state[static_cast<size_t>(c.ev) * p.n_feds + f] =
-            (static_cast<unsigned long long>(c.overrun) << kShOver) |
-            (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
-            (static_cast<unsigned long long>(fed_seed) << kShSeed) |
-            (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl;
-        // next FED of this warp: the ticket arrives while the staging runs
-        next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
-    }
+    // next FED of this warp: the ticket arrives while the staging runs
+    if (lane == 0) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
     {
         // cluster records: lane per cluster, consecutive lanes write consecutive records
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
@@ -918,6 +917,17 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             if ((sw >> lane) & 1u) p.s_seed[ab + k0 + __popc(sw & lt)] = strip_l[w * 32u + lane] & 0x7fffu;
             k0 += __popc(sw);
         }
+    }
+    // publish: the FED's counts, tagged with the launch's epoch, behind everything staged above
+    // (release: the in-kernel move of another warp may read the staging as soon as it sees the word)
+    __syncwarp();
+    if (lane == 0) {
+        const unsigned long long v = (static_cast<unsigned long long>(p.epoch) << kShEpoch) |
+                                     (static_cast<unsigned long long>(c.overrun) << kShOver) |
+                                     (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
+                                     (static_cast<unsigned long long>(fed_seed) << kShSeed) |
+                                     (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl;
+        asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p.fed_state + static_cast<size_t>(c.ev) * p.n_feds + f), "l"(v) : "memory");
     }
     return true;
 }
@@ -1064,6 +1074,199 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
 }
 
+// ------------------------------------------------------------------------------ a7, second half, in the same launch
+// The ordered move of one (event, FED) by a warp of sst_event_kernel that found the FED tickets
+// used up (launches with plain outputs: cluster arrays, seeds, S/N).  Two round trips to memory per
+// FED instead of one per array and loop: (1) the FED's own state word (acquire: what its warp staged
+// is read afterwards), the words of its predecessors (their sum is the FED's place in the event's
+// arrays) and its start offset, all in flight together; (2) ONE set of TMA bulk copies that brings
+// the FED's staged records, ADC offsets and cluster ADCs into the warp's shared-memory slot, which
+// is free by now.  The lanes then read shared memory and stream the arrays out.
+__device__ __forceinline__ unsigned long long ld_state(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_state_acquire(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+constexpr uint32_t kMoveAdc = 1024;  // cluster ADC bytes per bulk copy (+ 32 for the alignment of both ends)
+
+__device__ __forceinline__ void move_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot, uint32_t &mbar_phase,
+                                         const uint32_t ev, const uint32_t f, const int lane) {
+    const EventDesc &E = p.ev[ev];
+    const sst_output &o = E.out;
+    const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
+    const uint32_t fed_start = __ldg(E.fed_offsets + f);
+    // ---- round trip 1: state words.  clusters | ADC bytes << 32 ; seeds | malformed << 32 | overrun << 52
+    unsigned long long own, accA, accB;
+    for (uint32_t tries = 0;; ++tries) {
+        own = ld_state_acquire(st + f);
+        // (after a miss: wait for the FED's own word alone -- in FED-major order it is the last to appear)
+        while (tries && static_cast<uint32_t>(own >> kShEpoch) != p.epoch) {
+            __nanosleep(400);
+            own = ld_state_acquire(st + f);
+        }
+        bool ok = static_cast<uint32_t>(own >> kShEpoch) == p.epoch;
+        accA = accB = 0;
+        constexpr int kW = 14;  // words per lane in flight (448 FEDs per pass)
+#pragma unroll 1
+        for (uint32_t j0 = lane; j0 < f; j0 += 32 * kW) {
+            unsigned long long v[kW];
+#pragma unroll
+            for (int k = 0; k < kW; ++k) {
+                const uint32_t j = j0 + 32 * k;
+                v[k] = static_cast<unsigned long long>(p.epoch) << kShEpoch;
+                if (j < f) v[k] = ld_state(st + j);
+            }
+#pragma unroll
+            for (int k = 0; k < kW; ++k) {
+                ok = ok && static_cast<uint32_t>(v[k] >> kShEpoch) == p.epoch;
+                accA += (v[k] & 0x3fffull) | (((v[k] >> kShAdc) & 0x7fffull) << 32);
+                accB += ((v[k] >> kShSeed) & 0x7fffull) | (((v[k] >> kShMalf) & 0x7full) << 32) | (((v[k] >> kShOver) & 1ull) << 52);
+            }
+        }
+        if (__all_sync(kFull, ok)) break;
+        __nanosleep(400);  // some earlier FED of the event is still being worked on
+    }
+    accA = warp_sum64(accA);
+    accB = warp_sum64(accB);
+    const uint32_t fed_cl = static_cast<uint32_t>(own & 0x3fffull), fed_adc = static_cast<uint32_t>((own >> kShAdc) & 0x7fffull),
+                   fed_seed = static_cast<uint32_t>((own >> kShSeed) & 0x7fffull),
+                   fed_malf = static_cast<uint32_t>((own >> kShMalf) & 0x7full), fed_over = static_cast<uint32_t>((own >> kShOver) & 1ull);
+    const uint32_t b_cl = static_cast<uint32_t>(accA), b_adc = static_cast<uint32_t>(accA >> 32);
+    const uint32_t b_seed = static_cast<uint32_t>(accB), b_malf = static_cast<uint32_t>(accB >> 32) & 0xfffffu,
+                   b_over = static_cast<uint32_t>(accB >> 52);
+    // where the FED's warp staged it (a FED with bad offsets staged nothing: its counts are zero)
+    const size_t sb = static_cast<size_t>(ev) * p.s_cl_stride + fed_start / 2u + f;
+    const size_t ab = static_cast<size_t>(ev) * p.g_ents + fed_start;
+    const unsigned long long pol_first = policy_evict_first();
+    const bool all_fit = b_cl + fed_cl <= o.cap_clusters && b_adc + fed_adc <= o.cap_adc;
+
+    // ---- round trip 2: the staged FED into the slot: [records C x 16 | ADC offsets (C + 8) x 4 | cluster ADCs]
+    const uint32_t C = p.move_chunk;
+    const uint4 *const sm_rec = reinterpret_cast<const uint4 *>(slot);
+    const uint32_t *const sm_off = reinterpret_cast<const uint32_t *>(slot + 16u * C);
+    const uint8_t *const sm_adc = slot + 16u * C + 4u * (C + 8u);
+    uint32_t off_sh = 0, adc_sh = 0;  // where the first wanted element sits in the (16-byte aligned) windows copied
+    auto fetch = [&](const uint32_t k0, const uint32_t a0, const bool want_adc) {
+        // clusters [k0, k0 + n) and/or ADC bytes [a0, a0 + m); windows rounded out to 16 bytes
+        const uint32_t n = k0 < fed_cl ? min(C, fed_cl - k0) : 0u;
+        const uint32_t m = want_adc && a0 < fed_adc ? min(kMoveAdc, fed_adc - a0) : 0u;
+        const size_t o_lo = (sb + k0) & ~static_cast<size_t>(3), o_hi = (sb + k0 + n + 3u) & ~static_cast<size_t>(3);
+        const size_t a_lo = (ab + a0) & ~static_cast<size_t>(15), a_hi = (ab + a0 + m + 15u) & ~static_cast<size_t>(15);
+        if (n) off_sh = static_cast<uint32_t>(sb + k0 - o_lo);
+        if (m) adc_sh = static_cast<uint32_t>(ab + a0 - a_lo);
+        __syncwarp();  // every lane is done with what the slot held
+        if (lane == 0) {
+            // (generic-proxy accesses to the slot, and the acquire above, before the async-proxy copies)
+            asm volatile("fence.proxy.async;" ::: "memory");
+            const uint32_t bytes = n * 16u + (n ? static_cast<uint32_t>(o_hi - o_lo) * 4u : 0u) + (m ? static_cast<uint32_t>(a_hi - a_lo) : 0u);
+            mbar_expect_tx(mbar, bytes);
+            if (n) {
+                bulk_g2s(slot, p.s_rec + sb + k0, n * 16u, mbar, pol_first);
+                bulk_g2s(slot + 16u * C, p.s_off + o_lo, static_cast<uint32_t>(o_hi - o_lo) * 4u, mbar, pol_first);
+            }
+            if (m) bulk_g2s(slot + 16u * C + 4u * (C + 8u), p.s_adc + a_lo, static_cast<uint32_t>(a_hi - a_lo), mbar, pol_first);
+        }
+        mbar_wait(mbar, mbar_phase);
+        mbar_phase ^= 1u;
+    };
+    uint32_t lim = 0;  // ADC bytes of this FED that belong to clusters that fit
+    if (fed_cl) {
+        fetch(0, 0, true);
+#pragma unroll 1
+        for (uint32_t k0 = 0;;) {
+            const uint32_t n = min(C, fed_cl - k0);
+#pragma unroll 2
+            for (uint32_t i = lane; i < n; i += 32) {
+                const uint4 r = sm_rec[i];
+                const uint32_t off = sm_off[off_sh + i];
+                const uint32_t wd = r.y >> 16;
+                const uint32_t k_cl = b_cl + k0 + i, k_adc = b_adc + off;
+                if (all_fit || (k_cl < o.cap_clusters && k_adc + wd <= o.cap_adc)) {
+                    st_stream(o.cl_module + k_cl, r.x, pol_first);
+                    st_stream(o.cl_first + k_cl, r.y & 0xffffu, pol_first);
+                    st_stream(o.cl_width + k_cl, wd, pol_first);
+                    st_stream(o.cl_charge + k_cl, static_cast<int32_t>(r.z), pol_first);
+                    st_stream(o.cl_bary + k_cl, __uint_as_float(r.w), pol_first);
+                    st_stream(o.cl_adc_off + k_cl, k_adc, pol_first);
+                    if (o.cl_snr) o.cl_snr[k_cl] = __ldcg(p.s_snr + sb + k0 + i);
+                    lim = max(lim, off + wd);
+                } else {
+                    // the first cluster that does not fit reports how many were written
+                    const bool prev_fits = k_cl == 0 || (k_cl - 1 < o.cap_clusters && k_adc <= o.cap_adc);
+                    if (prev_fits) *o.n_clusters = k_cl;
+                }
+            }
+            k0 += n;
+            if (k0 >= fed_cl) break;
+            fetch(k0, 0, false);
+        }
+        lim = all_fit ? fed_adc : __reduce_max_sync(kFull, lim);
+        // cluster ADCs: aligned 32-bit words of the output from two aligned words of the slot
+#pragma unroll 1
+        for (uint32_t a0 = 0; a0 < lim;) {
+            const uint32_t m = min(kMoveAdc, lim - a0);
+            uint8_t *const D = o.cl_adc + b_adc + a0;
+            const uint32_t head = min(m, (4u - (static_cast<uint32_t>(reinterpret_cast<uintptr_t>(D)) & 3u)) & 3u);
+            const uint32_t nw = (m - head) >> 2, tail = (m - head) & 3u;
+            if (static_cast<uint32_t>(lane) < head) st_stream(D + lane, sm_adc[adc_sh + lane], pol_first);
+            if (static_cast<uint32_t>(lane) < tail) st_stream(D + head + 4u * nw + lane, sm_adc[adc_sh + head + 4u * nw + lane], pol_first);
+#pragma unroll 2
+            for (uint32_t w = lane; w < nw; w += 32) {
+                const uint32_t s = adc_sh + head + 4u * w;
+                const uint32_t *q = reinterpret_cast<const uint32_t *>(sm_adc + (s & ~3u));
+                st_stream(reinterpret_cast<uint32_t *>(D + head) + w, __funnelshift_r(q[0], q[1], 8u * (s & 3u)), pol_first);
+            }
+            a0 += m;
+            if (a0 < lim) fetch(fed_cl, a0, true);
+        }
+    }
+    if (o.seed_idx) {
+#pragma unroll 1
+        for (uint32_t i = lane; i < fed_seed; i += 32)
+            if (b_seed + i < o.cap_seeds) o.seed_idx[b_seed + i] = f * kFedStrips + __ldcg(p.s_seed + ab + i);
+    }
+    if (f == p.n_feds - 1 && lane == 0) {  // event totals = prefix of the last FED + its own
+        const uint32_t t_cl = b_cl + fed_cl, t_adc = b_adc + fed_adc, n_mal = b_malf + fed_malf, n_over = b_over + fed_over;
+        uint32_t flags = 0;
+        if (t_cl > o.cap_clusters) flags |= SST_FLAG_CLUSTER_CAP;
+        if (t_adc > o.cap_adc) flags |= SST_FLAG_ADC_CAP;
+        if (n_mal) flags |= SST_FLAG_MALFORMED;
+        if (n_over) flags |= SST_FLAG_OVERRUN;
+        if (!(flags & (SST_FLAG_CLUSTER_CAP | SST_FLAG_ADC_CAP))) *o.n_clusters = t_cl;
+        o.dev_status[SST_ST_FLAGS] = flags;
+        o.dev_status[SST_ST_N_MALFORMED] = n_mal;
+        o.dev_status[SST_ST_N_CLUSTERS] = t_cl;
+        o.dev_status[SST_ST_N_ADC] = t_adc;
+        o.dev_status[SST_ST_N_OVERRUN] = n_over;
+        o.dev_status[SST_ST_N_SEEDS] = b_seed + fed_seed;
+        o.dev_status[SST_ST_N_PRESENT] = 0;
+        o.dev_status[7] = 0;
+    }
+}
+
+// Tickets total .. 2 * total - 1 are the (event, FED) pairs again, in the same FED-major order.  A
+// warp that finds the FED tickets used up moves staged FEDs while the last FEDs are still being
+// worked on by others; a pair is moved once it and all its predecessors of the event carry this
+// launch's epoch.  Every warp of the grid is resident (the grid never exceeds the resident
+// capacity) and every FED ticket has been drawn by a running warp before the first move ticket is,
+// so a wait always ends.
+__device__ __forceinline__ void move_phase(const KParams &p, unsigned long long *mbar, uint8_t *slot, uint32_t &mbar_phase,
+                                           uint32_t ticket, const uint32_t total, const int lane) {
+    while (ticket < 2u * total) {
+        const uint32_t t = ticket - total;
+        uint32_t next_ticket = 0;
+        if (lane == 0) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
+        const uint32_t f = t / p.n_events;
+        move_fed(p, mbar, slot, mbar_phase, t - f * p.n_events, f, lane);
+        ticket = __shfl_sync(kFull, next_ticket, 0);
+    }
+}
+
 // ------------------------------------------------------------------------------ the kernel
 // Every warp works alone: it draws (event, FED) tickets until the launch's work is used up and
 // never meets a block-wide barrier.  A CTA is just 1..kWarpsPerCta such warps sharing the SM's
@@ -1090,6 +1293,13 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
             process_fed(p, mbar, slot, ticket, lane, true, mbar_phase, next_ticket);
         ticket = __shfl_sync(kFull, next_ticket, 0);
     }
+    // The ordered move, in the same launch (plain outputs only): tickets total .. 2 * total - 1 are
+    // the (event, FED) pairs again, in the same FED-major order.  A warp that finds the FED tickets
+    // used up moves staged FEDs while the last FEDs are still being worked on by others; a pair is
+    // moved once it and all its predecessors of the event carry this launch's epoch.  Every warp of
+    // the grid is resident (the grid never exceeds the resident capacity) and every FED ticket has
+    // been drawn by a running warp before the first move ticket is, so the wait always ends.
+    if (p.fused_move) move_phase(p, mbar, slot, mbar_phase, ticket, total, lane);
 }
 
 // ------------------------------------------------------------------------------ a7, second half
@@ -1308,7 +1518,7 @@ struct sst_ctx {
     // per-stream scratch (ticket counter, FED states, slow-path lists), taken from the pool on a
     // stream's first launch and kept: stream order makes reuse safe, the epoch and the running
     // ticket base make clearing unnecessary
-    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t cap_events; unsigned long long ticket_base; };
+    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t cap_events; unsigned long long ticket_base; uint32_t epoch; };
     // cross-stream dependencies of the batched entry point: one event per stream, made on first use
     struct StreamEvent { cudaStream_t stream; cudaEvent_t ev; };
     std::vector<StreamEvent> stream_events;
@@ -1399,7 +1609,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     for (auto &s : ctx->slots)
         if (s.stream == st) sl = &s;
     if (!sl) {
-        ctx->slots.push_back({st, nullptr, 0u, 0ull});
+        ctx->slots.push_back({st, nullptr, 0u, 0ull, 0u});
         sl = &ctx->slots.back();
     }
     if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 16, 32 or kMaxEv events
@@ -1417,6 +1627,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         sl->mem = mem;
         sl->cap_events = want;
         sl->ticket_base = 0;
+        sl->epoch = 0;
     }
     uint8_t *const blk = sl->mem;
     const ScratchLayout L = scratch_layout(ctx, sl->cap_events);
@@ -1459,13 +1670,26 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         kp.ev[e].packed = packed ? packed[e] : nullptr;
         kp.ev[e].raw_limit = raw_limit ? std::min(raw_limit[e], ctx->cfg.max_raw_bytes) : ctx->cfg.max_raw_bytes;
     }
+    bool extras = false;
+    for (uint32_t e = 0; e < n; ++e) extras = extras || outs[e]->hit_x || outs[e]->compact_strip;
+    // plain outputs: sst_event_kernel moves the staged clusters itself (one launch); the packed
+    // host block, hit coordinates and the compact SoA take sst_emit_kernel behind it
+    const bool fused = !packed && !extras && ctx->cfg.move_mode == 0;
+    kp.fused_move = fused ? 1u : 0u;
+    kp.move_chunk = std::min(1024u, ((ctx->slot_bytes - (kMoveAdc + 32u) - 32u) / 20u) & ~31u);  // (slot_bytes >= 4096)
+    // the epoch tags this launch's FED aggregates; before a tag is used again the words are cleared
+    if (sl->epoch == kEpochs) {
+        SST_CU(cudaMemsetAsync(blk + L.o_state, 0, L.state_bytes, st));
+        sl->epoch = 0;
+    }
+    kp.epoch = ++sl->epoch;
     sst_event_kernel<<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
     cudaError_t err = cudaGetLastError();
     if (err == cudaSuccess) {
         // every warp draws one ticket too many before it stops
-        sl->ticket_base += static_cast<unsigned long long>(total) + grid * wpc;
-        bool extras = false;
-        for (uint32_t e = 0; e < n; ++e) extras = extras || outs[e]->hit_x || outs[e]->compact_strip;
+        sl->ticket_base += static_cast<unsigned long long>(total) * (fused ? 2u : 1u) + grid * wpc;
+    }
+    if (err == cudaSuccess && !fused) {
         // the move is launched as a programmatic dependent of the event kernel: its CTAs are set up
         // while that kernel's last warps finish (the kernel itself waits for its completion)
         cudaLaunchConfig_t lc{};
@@ -1480,7 +1704,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         lc.numAttrs = 1;
         if (packed) err = cudaLaunchKernelEx(&lc, sst_emit_kernel<true, false>, kp);
         else if (extras) err = cudaLaunchKernelEx(&lc, sst_emit_kernel<false, true>, kp);
-        else err = cudaLaunchKernelEx(&lc, sst_emit_kernel<false, false>, kp);
+        else err = cudaLaunchKernelEx(&lc, sst_emit_kernel<false, false>, kp);  // (move_mode 1)
         if (err == cudaSuccess) err = cudaGetLastError();
     }
     if (err != cudaSuccess) {
@@ -1489,6 +1713,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         cu_ok(ctx, err);
         cudaMemsetAsync(blk, 0, L.o_rec, st);
         sl->ticket_base = 0;
+        sl->epoch = 0;
         return SST_ERR_CUDA;
     }
     return SST_OK;
@@ -1500,7 +1725,8 @@ extern "C" {
 
 sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (out_ctx) *out_ctx = nullptr;
-    if (!cfg || !out_ctx || cfg->n_feds == 0 || cfg->n_feds > kMaxFeds || cfg->max_raw_bytes == 0)
+    if (!cfg || !out_ctx || cfg->n_feds == 0 || cfg->n_feds > kMaxFeds || cfg->max_raw_bytes == 0 ||
+        cfg->move_mode > 1)
         return SST_ERR_INVALID_ARG;
     sst_ctx *ctx = new (std::nothrow) sst_ctx();
     if (!ctx) return SST_ERR_INVALID_ARG;
@@ -2161,7 +2387,7 @@ sst_status sst_get_info(const sst_ctx *ctx, sst_info *info) {
     info->threads = 32 * static_cast<uint32_t>(ctx->wpc);
     info->ctas_per_sm = static_cast<uint32_t>(ctx->ctas_per_sm);
     info->sm_count = static_cast<uint32_t>(ctx->sm_count);
-    info->kernels_per_event = 2;
+    info->kernels_per_event = ctx->cfg.move_mode == 0 ? 1 : 2;  // (launches with plain outputs)
     info->slot_bytes = ctx->slot_bytes;
     info->events_per_launch = kMaxEv;
     return SST_OK;

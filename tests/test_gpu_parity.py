@@ -15,10 +15,25 @@ pytestmark = pytest.mark.gpu
 REL = 1e-6   # north_star: "Barycenters and float S/N must agree within 1e-6 relative"
 
 
-@pytest.fixture(scope="module")
-def H():
-    from paper_2101_11489_b200 import harness
-    return harness
+class _Harness:
+    """The harness module with sst_config.move_mode preset: every test runs with the ordered move
+    inside sst_event_kernel (0, the default) and with sst_emit_kernel behind it (1)."""
+
+    def __init__(self, move_mode):
+        from paper_2101_11489_b200 import harness
+        self._h, self.move_mode = harness, move_mode
+
+    def Detector(self, *a, **kw):
+        kw.setdefault("move_mode", self.move_mode)
+        return self._h.Detector(*a, **kw)
+
+    def __getattr__(self, name):
+        return getattr(self._h, name)
+
+
+@pytest.fixture(scope="module", params=[0, 1], ids=["move-in-kernel", "move-kernel"])
+def H(request):
+    return _Harness(request.param)
 
 
 def gpu_run(H, n_feds, raw, fed_offsets, gain, noise, bad, chan_module, thresholds, cap_clusters=None,
