@@ -50,6 +50,7 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <thread>
 #include <vector>
 
 #include "sst.h"
@@ -89,7 +90,7 @@ struct EventDesc {
 };
 
 struct KParams {
-    const float2 *calib;     // {noise (+inf at bad strips), gain} per strip
+    const float2 *calib;     // {noise (+inf at bad strips), gain factor (see gain_apply)} per strip
     const uint2 *chan_info;  // {module id, first channel | end channel << 8 of the module}
     const float2 *calib_orig;  // {noise, gain} as uploaded (the compact SoA reports these)
     const uint8_t *bad;        // bad flags as uploaded
@@ -213,6 +214,14 @@ __device__ __forceinline__ uint32_t gain_correct(float adc, float gain) {
     const float u = __fadd_rn(__fdiv_rn(adc, gain), 0.5f);
     const float fl = floorf(u);
     return fl >= 254.0f ? 254u : static_cast<uint32_t>(fl);
+}
+
+// The same through the strip's factor c from sst_upload_calib: c > 0 means
+// min(254, floor(fma(adc, c, 0.5))) was checked there to equal gain_correct(adc, gain) for every
+// adc 1..255 (c is 1/gain or a neighbour of it); c < 0 is -gain of a strip that has no such factor.
+__device__ __forceinline__ uint32_t gain_apply(float adc, float c) {
+    if (c > 0.0f) return min(254u, __float2uint_rz(__fmaf_rn(adc, c, 0.5f)));
+    return gain_correct(adc, -c);
 }
 
 __device__ __forceinline__ unsigned long long warp_sum64(unsigned long long v) {
@@ -655,7 +664,28 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             // software pipeline of depth one: the next entry's list reads and calibration gather
             // are issued before the current entry is worked on
             const uint32_t elast = min(max(e1, e0 + 1u), P) - 1u;
-            uint32_t sv_n = strip_l[min(e0, P - 1u)], av_n = adc_l[min(e0, P - 1u)];
+            // The lists of the fast path are addressed as 32-bit shared addresses the compiler cannot
+            // re-derive (else it recomputes the warp's slot address, eleven instructions, at every
+            // access inside the loop to save a register).
+            uint32_t sl_sa = 0, al_sa = 0;
+            if (kFast) {
+                sl_sa = smem_addr(strip_l);
+                al_sa = smem_addr(adc_l);
+                asm volatile("" : "+r"(sl_sa), "+r"(al_sa));
+            }
+            auto ld_strip = [&](const uint32_t i) -> uint32_t {
+                if (!kFast) return strip_l[i];
+                uint32_t v;
+                asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(sl_sa + 2u * i));
+                return v;
+            };
+            auto ld_adc = [&](const uint32_t i) -> uint32_t {
+                if (!kFast) return adc_l[i];
+                uint32_t v;
+                asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(al_sa + i));
+                return v;
+            };
+            uint32_t sv_n = ld_strip(min(e0, P - 1u)), av_n = ld_adc(min(e0, P - 1u));
             float2 cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
 #pragma unroll 1
             for (uint32_t i0 = 0; i0 < Lc; i0 += 32u) {  // (uniform: every lane takes Lc steps, the last lanes idle in some)
@@ -669,8 +699,8 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                     const float2 cv = cv_n;
                     {
                         const uint32_t en = min(e + 1u, elast);
-                        sv_n = strip_l[en];
-                        av_n = adc_l[en];
+                        sv_n = ld_strip(en);
+                        av_n = ld_adc(en);
                         cv_n = ld_calib(cal + (sv_n & 0x7fffu), pol_last);
                     }
                     const uint32_t s15 = sv & 0x7fffu;
@@ -693,8 +723,10 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                         if (!is_link) {
                             hd = e; Q = 0; N = 0.0; seed = false;
                         }
-                        const uint32_t q = gain_correct(af, cv.y);
-                        adc_l[e] = static_cast<uint8_t>(q);  // kept for the emit
+                        const uint32_t q = gain_apply(af, cv.y);
+                        // kept for the staging
+                        if (kFast) asm volatile("st.shared.u8 [%0], %1;" ::"r"(al_sa + e), "r"(q) : "memory");
+                        else adc_l[e] = static_cast<uint8_t>(q);
                         Q += q;
                         const double d = static_cast<double>(cv.x);
                         N = __fma_rn(d, d, N);  // exact square, one rounding: the oracle's sum
@@ -919,7 +951,10 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         }
     }
     // publish: the FED's counts, tagged with the launch's epoch, behind everything staged above
-    // (release: the in-kernel move of another warp may read the staging as soon as it sees the word)
+    // (release: the in-kernel move of another warp may read the staging as soon as it sees the word,
+    // and it reads it with TMA bulk copies: the writers order their generic-proxy stores before
+    // async-proxy accesses)
+    if (p.fused_move) asm volatile("fence.proxy.async.global;" ::: "memory");
     __syncwarp();
     if (lane == 0) {
         const unsigned long long v = (static_cast<unsigned long long>(p.epoch) << kShEpoch) |
@@ -1161,8 +1196,7 @@ __device__ __forceinline__ void move_fed(const KParams &p, unsigned long long *m
         if (m) adc_sh = static_cast<uint32_t>(ab + a0 - a_lo);
         __syncwarp();  // every lane is done with what the slot held
         if (lane == 0) {
-            // (generic-proxy accesses to the slot, and the acquire above, before the async-proxy copies)
-            asm volatile("fence.proxy.async;" ::: "memory");
+            fence_proxy_async();  // earlier generic-proxy accesses to the slot before the async writes
             const uint32_t bytes = n * 16u + (n ? static_cast<uint32_t>(o_hi - o_lo) * 4u : 0u) + (m ? static_cast<uint32_t>(a_hi - a_lo) : 0u);
             mbar_expect_tx(mbar, bytes);
             if (n) {
@@ -1539,6 +1573,34 @@ inline bool cu_ok(sst_ctx *ctx, cudaError_t e) {
 // the HOST entry points produce the cluster arrays, the dense SoA, the channel map and the seeds
 bool no_device_only_outputs(const sst_output *o) { return !o->compact_strip && !o->hit_x && o->cap_compact == 0; }
 
+// Gain correction without a division in the kernel (gain_apply): a factor c with
+// min(254, floor(fma(adc, c, 0.5))) == min(254, floor(fl(fl(adc / gain) + 0.5))) -- the defining
+// float32 form, reading s13 -- for EVERY adc in 1..255, searched among 1/gain and its
+// float32 neighbours; -gain when none of them does (the kernel then divides for that strip).
+// (double)adc * c is exact and so is the sum with 0.5 unless it is far below 1, where the floor is
+// 0 either way: rounding it to float32 once is the fused multiply-add.
+float gain_factor(const float g) {
+    const float c0 = 1.0f / g;
+    float cand[5] = {c0, std::nextafterf(c0, INFINITY), std::nextafterf(c0, 0.0f), 0.0f, 0.0f};
+    cand[3] = std::nextafterf(cand[1], INFINITY);
+    cand[4] = std::nextafterf(cand[2], 0.0f);
+    for (const float c : cand) {
+        if (!(c > 0.0f) || !std::isfinite(c)) continue;
+        uint32_t diff = 0;
+        for (int a = 1; a <= 255; ++a) {  // (no early exit: the loop vectorises)
+            const float af = static_cast<float>(a);
+            float u = af / g;
+            u = u + 0.5f;
+            const uint32_t ref = u >= 254.0f ? 254u : static_cast<uint32_t>(static_cast<int32_t>(u));
+            const float v = static_cast<float>(static_cast<double>(af) * static_cast<double>(c) + 0.5);
+            const uint32_t got = v >= 254.0f ? 254u : static_cast<uint32_t>(static_cast<int32_t>(v));
+            diff |= ref ^ got;
+        }
+        if (diff == 0) return c;
+    }
+    return -g;
+}
+
 bool thresholds_ok(const sst_thresholds *t) {
     const float v[3] = {t->channel, t->seed, t->cluster};
     for (float x : v)
@@ -1844,15 +1906,38 @@ sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise,
     } catch (...) {
         return SST_ERR_INVALID_ARG;
     }
-    for (size_t g = 0; g < n; ++g) {
-        if (bad[g]) {
-            // a bad strip is never active: noise = +inf fails every >= test; gain is never used
-            packed[g] = make_float2(INFINITY, 1.0f);
-        } else {
-            if (!std::isfinite(gain[g]) || !(gain[g] > 0.0f) || !std::isfinite(noise[g]) || !(noise[g] > 0.0f))
-                return SST_ERR_BAD_CALIB;
-            packed[g] = make_float2(noise[g], gain[g]);
+    // {noise, gain factor} per strip, by all host cores: the factor search checks 255 ADC values
+    // per candidate
+    {
+        std::atomic<bool> bad_calib{false};
+        const unsigned nt = std::max(1u, std::min(32u, std::thread::hardware_concurrency()));
+        auto work = [&](size_t g0, size_t g1) {
+            for (size_t g = g0; g < g1; ++g) {
+                if (bad[g]) {
+                    // a bad strip is never active: noise = +inf fails every >= test; gain is never used
+                    packed[g] = make_float2(INFINITY, 1.0f);
+                } else {
+                    if (!std::isfinite(gain[g]) || !(gain[g] > 0.0f) || !std::isfinite(noise[g]) || !(noise[g] > 0.0f)) {
+                        bad_calib.store(true);
+                        return;
+                    }
+                    packed[g] = make_float2(noise[g], gain_factor(gain[g]));
+                }
+            }
+        };
+        std::vector<std::thread> pool;
+        const size_t per = (n + nt - 1) / nt;
+        try {
+            for (unsigned t = 1; t < nt; ++t)
+                if (t * per < n) pool.emplace_back(work, t * per, std::min(n, (t + 1) * per));
+        } catch (...) {  // no more threads: the rest is done here
         }
+        const size_t started = pool.size();
+        work(0, std::min(n, per));
+        for (size_t t = started + 1; t < nt; ++t)
+            if (t * per < n) work(t * per, std::min(n, (t + 1) * per));
+        for (auto &th : pool) th.join();
+        if (bad_calib.load()) return SST_ERR_BAD_CALIB;
     }
     SST_CU(cudaSetDevice(ctx->cfg.device));
     SST_CU(cudaMemcpy(ctx->calib, packed.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
