@@ -150,6 +150,69 @@ def test_gain_correction_exhaustive_on_gpu(H, oracle):
     assert g["n_clusters"] > 96 * 250
 
 
+_FACTOR_GAINS = {}
+
+
+def _gains_that_stress_the_factor_search():
+    """The kernel corrects ADCs with a per-strip factor c (1/gain or a float32 neighbour) found at
+    upload, and divides only for strips that have none.  This picks, by an independent float32
+    search in numpy over a million random gains, gains for which 1/gain itself fails for some ADC
+    (a neighbour has to be taken) and gains for which all five candidates fail (the division path),
+    plus extreme and special values.  Expected values come from the oracle as everywhere else."""
+    if _FACTOR_GAINS:
+        return _FACTOR_GAINS["g"]
+    rng = np.random.Generator(np.random.PCG64(11))
+    a = np.arange(1, 256, dtype=np.float32)[None, :]
+    need_nb, need_div = [], []
+    for _ in range(10):
+        g = rng.uniform(0.5, 2.0, 100_000).astype(np.float32)
+        u = (a / g[:, None]).astype(np.float32) + np.float32(0.5)
+        ref = np.minimum(np.floor(u), 254)
+        c0 = (np.float32(1.0) / g).astype(np.float32)
+        ok_any = np.zeros(g.size, bool)
+        ok0 = None
+        for step in (0, 1, -1, 2, -2):
+            c = c0.copy()
+            for _ in range(abs(step)):
+                c = np.nextafter(c, np.float32(np.inf if step > 0 else 0), dtype=np.float32)
+            v = (a.astype(np.float64) * c[:, None].astype(np.float64) + 0.5).astype(np.float32)
+            ok = (np.minimum(np.floor(v), 254) == ref).all(axis=1)
+            if step == 0:
+                ok0 = ok
+            ok_any |= ok
+        need_nb += list(g[~ok0 & ok_any][:12])
+        need_div += list(g[~ok_any])
+    special = np.float32([1.0, 0.5, 2.0, 1.0 / 3, 3.0, 7.0, 255.0, 254.0, 1e-30, 1e30, 1.5e-45, 3e38, 0.8, 1.2, 1.25, 0.999999, 1.000001])
+    gains = np.concatenate([special, np.float32(need_div)[:75], np.float32(need_nb)[:100]])
+    assert len(need_div) >= 20 and len(need_nb) >= 60, (len(need_div), len(need_nb))
+    _FACTOR_GAINS["g"] = gains[:192]
+    return _FACTOR_GAINS["g"]
+
+
+def test_gain_factor_search_edge_gains_on_gpu(H, oracle):
+    """All 255 non-zero ADC values x up to 192 gains chosen to defeat the factor search (see above):
+    the corrected ADCs must equal the oracle's division for every one of them."""
+    gains = _gains_that_stress_the_factor_search()
+    n_feds = 4
+    n = n_feds * synth.FED_STRIPS
+    z = np.zeros(n, np.uint8)
+    gain = np.ones(n, np.float32)
+    for i, gv in enumerate(gains):
+        for half in range(2):
+            ch = 2 * i + half
+            z[ch * 256 + 2 * np.arange(128)] = np.arange(128) + 128 * half
+            gain[ch * 256:(ch + 1) * 256] = gv
+    raw, fo = synth.encode_dense(z, n_feds)
+    noise = np.full(n, 0.125, np.float32)
+    bad = np.zeros(n, np.uint8)
+    cm = cases.module_map_from_sizes(n_feds, (2,))
+    thr = (1.0, 1.0, 1e-3)
+    g = gpu_run(H, n_feds, raw, fo, gain, noise, bad, cm, thr)
+    r = oracle.run(raw, fo, n_feds, gain, noise, bad, cm, thr)
+    compare(g, r)
+    assert g["n_clusters"] > len(gains) * 200
+
+
 # ------------------------------------------------------------------ hand-built raw + malformed
 def test_hand_built_and_malformed_raw(H, oracle):
     E = synth.EMPTY_CHANNEL
