@@ -291,6 +291,12 @@ struct FedCtx {
     uint32_t off[3], len[3];       // of channels lane, lane+32, lane+64
     uint32_t ebase[3];             // first list entry of those channels
     uint32_t opens;                // bit k: channel lane+32k opens a module
+    // A FED whose lists do not fit the slot in one go is worked on in PIECES, channel ranges that
+    // start at module boundaries, one after the other by the same warp (fed_size, P, off, len and
+    // ebase then describe the piece; channels outside it have length 0):
+    uint32_t ch_lo, ch_hi;         // the piece's channels [ch_lo, ch_hi); 0, 96 for a whole FED
+    uint32_t last;                 // the piece ends the FED: the FED's word is published
+    uint32_t cl_base, adc_base, seed_base, ent_base, nz_base;  // counts of the FED's earlier pieces
 };
 
 // a2 pass 1: a lane validates the run lists of its three channels (reading s2b) and
@@ -388,10 +394,15 @@ __device__ __forceinline__ uint32_t fast_strip_base(uint32_t A, uint32_t P16, bo
 // scratch and rp is whatever holds the payload.  Returns false (fast path only) when the cluster
 // records outgrow the slot: the FED is then redone on the slow path (nothing has been published
 // and every output written so far is rewritten identically).
-template <bool kFast>
-__device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, const FedCtx &c,
+template <bool kFast, bool kPiece>
+__device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, FedCtx &c,
                                           const int lane, uint32_t &next_ticket) {
     const uint32_t f = c.f, P = c.P;
+    // kPiece: c describes one piece of a FED (see FedCtx); else the whole FED, and all of this folds away
+    const uint32_t ch_lo = kPiece ? c.ch_lo : 0u, ch_hi = kPiece ? c.ch_hi : static_cast<uint32_t>(kChan);
+    const bool last = kPiece ? c.last != 0 : true;
+    const uint32_t cl_base = kPiece ? c.cl_base : 0u, adc_base = kPiece ? c.adc_base : 0u, seed_base = kPiece ? c.seed_base : 0u,
+                   ent_base = kPiece ? c.ent_base : 0u, nz_base = kPiece ? c.nz_base : 0u;
     const EventDesc &E = p.ev[c.ev];
     const sst_output &o = E.out;
     const uint32_t nw = (P + 31) >> 5;  // mask words in use; every mask has one more (zero) word
@@ -487,7 +498,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     {
         // In a FED without malformed channels or an overrun the per-channel constant is 2 * channel + 2
         // (two length bytes per channel up to and including the entry's own); else it is looked up.
-        const bool regular = c.overrun == 0 && c.n_malformed == 0;
+        const bool regular = !kPiece && c.overrun == 0 && c.n_malformed == 0;
         const bool entry_prefetch = p.n_events < kSlabMinEvents;
         uint32_t run_before = 0, start_before = 0, v_before = 0;  // runs / last run start / its entry below this word
         const uint32_t last = P - 1u;                             // (P > 0 inside the loop)
@@ -535,7 +546,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // The FED's lists are exactly that; they are staged as they are (strip id, raw ADC) and
     // sst_emit_kernel moves them to their place in the event's arrays, adding the calibration.
     if (o.compact_strip) {
-        const size_t cb = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
+        const size_t cb = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start + ent_base;
         uint32_t nz = 0;
 #pragma unroll 1
         for (uint32_t i = lane; i < ((P + 31u) & ~31u); i += 32u) {
@@ -547,7 +558,11 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
             }
             nz += __popc(__ballot_sync(kFull, a != 0));
         }
-        if (lane == 0) p.fed_present[static_cast<size_t>(c.ev) * p.n_feds + f] = (P << 16) | nz;
+        if (kPiece) {
+            c.ent_base = ent_base + P;
+            c.nz_base = nz_base + nz;
+        }
+        if (lane == 0 && last) p.fed_present[static_cast<size_t>(c.ev) * p.n_feds + f] = ((ent_base + P) << 16) | (nz_base + nz);
     }
 
     // ---------------------------------------------------------------- a2: dense SoA
@@ -556,6 +571,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // lists) and leaves as one TMA bulk store per window: no zero-fill pass over HBM, no byte
     // scatter, and the way out costs the LSU pipe nothing.
     if (dense) {
+        const uint32_t s_lo = ch_lo * kStrip, s_hi = ch_hi * kStrip;  // the piece's strips
         if ((reinterpret_cast<uintptr_t>(dense) & 15u) == 0 && window) {
             constexpr uint32_t kWin = 2048;
             uint4 *const win = reinterpret_cast<uint4 *>(window);
@@ -563,9 +579,9 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 #pragma unroll
             for (uint32_t k = 0; k < kWin / 512u; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
 #pragma unroll 1
-            for (uint32_t base = 0; base < static_cast<uint32_t>(kFedStrips); base += kWin) {
+            for (uint32_t base = s_lo; base < s_hi;) {
                 __syncwarp();
-                const uint32_t limit = base + kWin;
+                const uint32_t limit = kPiece ? min((base & ~(kWin - 1u)) + kWin, s_hi) : base + kWin;
                 for (;;) {  // two consecutive entries per lane; the list is sorted by strip
                     const uint32_t i = i0 + 2u * lane;
                     const uint32_t ia = i < P ? i : 0u, ib = i + 1u < P ? i + 1u : 0u;  // loads stay in the lists
@@ -584,7 +600,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 __syncwarp();
                 if (lane == 0) {
                     asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dense + base),
-                                 "r"(smem_addr(window)), "r"(kWin), "l"(pol_first)
+                                 "r"(smem_addr(window)), "r"(limit - base), "l"(pol_first)
                                  : "memory");
                     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -592,10 +608,11 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 __syncwarp();
 #pragma unroll
                 for (uint32_t k = 0; k < kWin / 512u; ++k) win[lane + 32u * k] = make_uint4(0, 0, 0, 0);
+                base = limit;
             }
         } else {  // unaligned output or no room for a window: bytes
 #pragma unroll 1
-            for (uint32_t b = lane; b < static_cast<uint32_t>(kFedStrips); b += 32u) dense[b] = 0;
+            for (uint32_t b = s_lo + lane; b < s_hi; b += 32u) dense[b] = 0;
             __syncwarp();
 #pragma unroll 1
             for (uint32_t i = lane; i < P; i += 32u) dense[strip_l[i] & 0x7fffu] = adc_l[i];
@@ -872,10 +889,10 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     // FED-local order in global scratch.  sst_emit_kernel, launched behind this kernel on the same
     // stream, turns the counts into offsets and moves everything to its (module, first strip)
     // ordered place -- no warp ever waits for another one.
-    const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f;
+    const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f + cl_base;
     const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
     // next FED of this warp: the ticket arrives while the staging runs
-    if (lane == 0) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
+    if (lane == 0 && last) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
     {
         // cluster records: lane per cluster, consecutive lanes write consecutive records
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
@@ -890,7 +907,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                 const uint32_t wi = hd >> 5, b = hd & 31u;
                 const uint32_t ma = mA[wi], mh = mH[wi];
                 // its ADCs start behind those of the members before it
-                off = (mP[wi] & 0xffffu) + __popc(ma & ((1u << b) - 1u));
+                off = adc_base + (mP[wi] & 0xffffu) + __popc(ma & ((1u << b) - 1u));
                 // width: the members behind the head that are not heads themselves, 32 at a time
                 const uint32_t v = __funnelshift_rc(ma & ~mh, mA[wi + 1] & ~mH[wi + 1], b + 1u);
                 uint32_t n1 = __ffs(~v) - 1u;  // trailing ones
@@ -946,10 +963,16 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 #pragma unroll 1
         for (uint32_t w = 0; w < nw; ++w) {
             const uint32_t sw = mS[w];
-            if ((sw >> lane) & 1u) p.s_seed[ab + k0 + __popc(sw & lt)] = strip_l[w * 32u + lane] & 0x7fffu;
+            if ((sw >> lane) & 1u) p.s_seed[ab + seed_base + k0 + __popc(sw & lt)] = strip_l[w * 32u + lane] & 0x7fffu;
             k0 += __popc(sw);
         }
     }
+    if (kPiece) {
+        c.cl_base = cl_base + fed_cl;
+        c.adc_base = adc_base + fed_adc;
+        c.seed_base = seed_base + fed_seed;
+    }
+    if (!last) return true;  // (uniform) more pieces of this FED follow
     // publish: the FED's counts, tagged with the launch's epoch, behind everything staged above
     // (release: the in-kernel move of another warp may read the staging as soon as it sees the word,
     // and it reads it with TMA bulk copies: the writers order their generic-proxy stores before
@@ -960,8 +983,8 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         const unsigned long long v = (static_cast<unsigned long long>(p.epoch) << kShEpoch) |
                                      (static_cast<unsigned long long>(c.overrun) << kShOver) |
                                      (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
-                                     (static_cast<unsigned long long>(fed_seed) << kShSeed) |
-                                     (static_cast<unsigned long long>(fed_adc) << kShAdc) | fed_cl;
+                                     (static_cast<unsigned long long>(seed_base + fed_seed) << kShSeed) |
+                                     (static_cast<unsigned long long>(adc_base + fed_adc) << kShAdc) | (cl_base + fed_cl);
         asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p.fed_state + static_cast<size_t>(c.ev) * p.n_feds + f), "l"(v) : "memory");
     }
     return true;
@@ -969,6 +992,9 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 
 // ------------------------------------------------------------------------------ one FED, one warp
 // Returns false when the FED has to be redone with force_slow (see fed_lists).
+// kPieces: a FED whose lists do not fit the slot is worked on in pieces (contexts whose slot was
+// sized for that); else it goes through the global scratch.
+template <bool kPieces>
 __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot,
                                             const uint32_t ticket, const int lane, const bool force_slow,
                                             uint32_t &mbar_phase, uint32_t &next_ticket) {
@@ -1085,13 +1111,14 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     if (staged) scan_runs3(slot, c, cnt, runs);
     else scan_runs3(rp, c, cnt, runs);
     // exclusive scans of the 96 strip and run counts (one scan: runs in the upper half word)
-    uint32_t tot = 0;
+    uint32_t tot = 0, exs[3];
     uint32_t *const ktab = chan_off;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         const uint32_t v = cnt[k] | (runs[k] << 16);
         const uint32_t inc = warp_incl_scan(v, lane);
         const uint32_t ex = tot + inc - v;
+        exs[k] = ex;
         c.ebase[k] = ex & 0xffffu;
         // payload address of entry e of this channel: off + (e - ebase) + 2 * (run(e) - rbase + 1),
         // i.e. e + 2 * (runs up to and including its own) + this constant
@@ -1099,14 +1126,98 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         tot += __shfl_sync(kFull, inc, 31);
     }
     c.P = tot & 0xffffu;  // present strips of the FED (<= 24576; the runs, <= 12288, sit in the upper half)
+    c.ch_lo = 0;
+    c.ch_hi = kChan;
+    c.last = 1;
+    c.cl_base = c.adc_base = c.seed_base = c.ent_base = c.nz_base = 0;
     __syncwarp();
 
     // fast path: window / cluster list, strip ids and masks fit behind the ADC list
-    const uint32_t A = (c.fed_size + 15u) & ~15u, P16 = (c.P + 15u) & ~15u;
-    const uint32_t S0 = fast_strip_base(A, P16, o.strip_adc != nullptr);
-    if (!force_slow && staged && ((S0 + 2u * c.P + 15u) & ~15u) + 16u * (((c.P + 31u) >> 5) + 2u) + kTabBytes <= p.slot_bytes)
-        return fed_lists<true>(p, slot, slot, c, lane, next_ticket);
-    return fed_lists<false>(p, slot, rp, c, lane, next_ticket);
+    const bool want_dense = o.strip_adc != nullptr;
+    auto fits = [&](const uint32_t bytes, const uint32_t strips) {
+        const uint32_t A = (bytes + 15u) & ~15u, P16 = (strips + 15u) & ~15u;
+        const uint32_t S0 = fast_strip_base(A, P16, want_dense);
+        return ((S0 + 2u * strips + 15u) & ~15u) + 16u * (((strips + 31u) >> 5) + 2u) + kTabBytes <= p.slot_bytes;
+    };
+    // ---------------------------------------------------------------- a FED in pieces
+    // When the lists of the whole FED do not fit the slot the warp works through it in up to seven
+    // pieces, channel ranges that start where a module starts (nothing links across), each as
+    // large as fits.  A piece's part of the payload is fetched again from global memory (it is
+    // in L2) to the start of the slot; everything per channel is in registers already.
+    // value of a per-channel quantity at boundary b (a channel index, or 96)
+    auto at = [&](const uint32_t (&v)[3], const uint32_t b, const uint32_t at_end) {
+        const uint32_t x0 = __shfl_sync(kFull, v[0], b & 31u), x1 = __shfl_sync(kFull, v[1], b & 31u),
+                       x2 = __shfl_sync(kFull, v[2], b & 31u);
+        return b >= static_cast<uint32_t>(kChan) ? at_end : b < 32u ? x0 : b < 64u ? x1 : x2;
+    };
+    bool slow = force_slow || !staged;
+    unsigned long long plan = 0;  // boundaries, 8 bits each
+    uint32_t n_pieces = 0;        // 0: the whole FED at once
+    if (!kPieces) {
+        slow = slow || !fits(c.fed_size, c.P);
+    } else if (!slow && !fits(c.fed_size, c.P)) {  // (uniform)
+        for (uint32_t lo = 0; lo < static_cast<uint32_t>(kChan);) {
+            // (16-byte granules of the payload; an overrun FED is fetched to its end)
+            const uint32_t g_lo = (at(c.off, lo, c.fed_size + 2u) - 2u) & ~15u, e_lo = at(exs, lo, tot) & 0xffffu;
+            uint32_t best = 0;
+            if (fits(c.fed_size - g_lo, c.P - e_lo)) {
+                best = kChan;
+            } else {
+#pragma unroll
+                for (int k = 2; k >= 0; --k) {
+                    const uint32_t ch = lane + 32 * k;
+                    const uint32_t hi = c.overrun ? c.fed_size : (c.off[k] - 2u + 15u) & ~15u;
+                    const bool ok = ch > lo && ((c.opens >> k) & 1u) && hi >= g_lo && fits(hi - g_lo, (exs[k] & 0xffffu) - e_lo);
+                    const uint32_t m = __ballot_sync(kFull, ok);
+                    if (!best && m) best = 32u * k + 31u - __clz(m);
+                }
+            }
+            if (!best || n_pieces == 7) {  // a module that does not fit, or too many pieces
+                slow = true;
+                break;
+            }
+            plan |= static_cast<unsigned long long>(best) << (8u * n_pieces);
+            ++n_pieces;
+            lo = best;
+        }
+    }
+    if (slow) return fed_lists<false, false>(p, slot, rp, c, lane, next_ticket);
+    if (!kPieces || n_pieces == 0) return fed_lists<true, false>(p, slot, slot, c, lane, next_ticket);
+    FedCtx pc = c;  // the piece's view of the FED (c stays as it is: the whole FED's, in registers)
+    for (uint32_t i = 0, b0 = 0; i < n_pieces; ++i) {
+        const uint32_t b1 = static_cast<uint32_t>(plan >> (8u * i)) & 0xffu;
+        const uint32_t g_lo = (at(c.off, b0, c.fed_size + 2u) - 2u) & ~15u;
+        const uint32_t g_hi = c.overrun || b1 >= static_cast<uint32_t>(kChan) ? c.fed_size : (at(c.off, b1, c.fed_size + 2u) - 2u + 15u) & ~15u;
+        const uint32_t ex0 = at(exs, b0, tot), ex1 = at(exs, b1, tot);
+        __syncwarp();  // every lane is done with the previous piece
+        if (i > 0 && g_hi > g_lo) {
+            if (lane == 0) {
+                fence_proxy_async();
+                mbar_expect_tx(mbar, g_hi - g_lo);
+                bulk_g2s(slot, E.raw + c.fed_start + g_lo, g_hi - g_lo, mbar, policy_evict_first());
+            }
+            mbar_wait(mbar, mbar_phase);
+            mbar_phase ^= 1u;
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const uint32_t ch = lane + 32 * k;
+            const bool in = ch >= b0 && ch < b1;
+            pc.off[k] = in ? c.off[k] - g_lo : 0u;
+            pc.len[k] = in ? c.len[k] : 0u;
+            pc.ebase[k] = in ? (exs[k] & 0xffffu) - (ex0 & 0xffffu) : 0u;
+            if (in) ktab[ch] = pc.off[k] - pc.ebase[k] - 2u * ((exs[k] >> 16) - (ex0 >> 16));
+        }
+        pc.fed_size = g_hi - g_lo;
+        pc.P = (ex1 & 0xffffu) - (ex0 & 0xffffu);
+        pc.ch_lo = b0;
+        pc.ch_hi = b1;
+        pc.last = i + 1u == n_pieces;
+        __syncwarp();
+        if (!fed_lists<true, true>(p, slot, slot, pc, lane, next_ticket)) return false;
+        b0 = b1;
+    }
+    return true;
 }
 
 // ------------------------------------------------------------------------------ a7, second half, in the same launch
@@ -1305,6 +1416,7 @@ __device__ __forceinline__ void move_phase(const KParams &p, unsigned long long 
 // Every warp works alone: it draws (event, FED) tickets until the launch's work is used up and
 // never meets a block-wide barrier.  A CTA is just 1..kWarpsPerCta such warps sharing the SM's
 // shared memory (one driver reserve per CTA instead of one per warp).
+template <bool kPieces>
 __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(const __grid_constant__ KParams p) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -1323,8 +1435,8 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
     ticket = __shfl_sync(kFull, ticket, 0);
     while (ticket < total) {
         uint32_t next_ticket = 0;
-        if (!process_fed(p, mbar, slot, ticket, lane, false, mbar_phase, next_ticket))
-            process_fed(p, mbar, slot, ticket, lane, true, mbar_phase, next_ticket);
+        for (bool slow = false; !process_fed<kPieces>(p, mbar, slot, ticket, lane, slow, mbar_phase, next_ticket); slow = true) {
+        }  // (a FED whose cluster list outgrows the slot is redone through the global scratch)
         ticket = __shfl_sync(kFull, next_ticket, 0);
     }
     // The ordered move, in the same launch (plain outputs only): tickets total .. 2 * total - 1 are
@@ -1544,6 +1656,7 @@ struct sst_ctx {
     std::atomic<int32_t> last_err{0};
     std::atomic<float> packed_ratio{0.0f};  // packed result bytes per raw byte seen by the last packed host call
     int sm_count = 0;
+    int pieces = 1;            // > 1: the slot was sized for FEDs worked on in pieces (sst_event_kernel<true>)
     int wpc = kWarpsPerCta;    // warps per CTA of a full launch
     int ctas_per_sm = 0;       // resident CTAs of wpc warps
     uint32_t slot_bytes = 0;   // shared-memory slot of one warp (one FED)
@@ -1745,7 +1858,8 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         sl->epoch = 0;
     }
     kp.epoch = ++sl->epoch;
-    sst_event_kernel<<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
+    if (ctx->pieces > 1) sst_event_kernel<true><<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
+    else sst_event_kernel<false><<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
     cudaError_t err = cudaGetLastError();
     if (err == cudaSuccess) {
         // every warp draws one ticket too many before it stops
@@ -1831,31 +1945,46 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         const uint32_t p_hint = cfg->fed_strips_hint ? std::min(cfg->fed_strips_hint, static_cast<uint32_t>(kFedStrips))
                                                      : static_cast<uint32_t>(0.5 * m) + 32u;
         const uint32_t r_hint = (static_cast<uint32_t>(std::min(1.15 * m + 64.0, 65536.0)) + 15u) & ~15u;
-        const uint32_t p16 = (p_hint + 15u) & ~15u;
-        const uint32_t gap = r_hint >= p16 + 2048u ? 0u : p16 + 2048u - r_hint;
-        uint32_t need = r_hint + gap + 2u * p_hint + 16u * (p_hint / 32u + 3u) + kTabBytes + 32u;
         int smem_optin = 0;
         cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device);
-        need = std::min(std::max((need + 15u) & ~15u, 4096u), (static_cast<uint32_t>(smem_optin) - kWarpHdr - kTailPad) & ~15u);
         // The dynamic shared-memory limit is per-FUNCTION state shared by every context of the
         // process: it is set to the device maximum, never to this context's size, so contexts with
         // different slot sizes can be used side by side.
-        if (cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
+        if (cudaFuncSetAttribute(sst_event_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess ||
+            cudaFuncSetAttribute(sst_event_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
             return fail(SST_ERR_CUDA);
-        cudaFuncSetAttribute(sst_event_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        const uint32_t stride = kWarpHdr + need + kTailPad;
+        cudaFuncSetAttribute(sst_event_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(sst_event_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        // A large FED may be worked on in K pieces (process_fed): the slot then holds the whole
+        // payload while the channel table is built, and one piece's lists afterwards.  K = 1..4 is
+        // tried, up to the first that keeps 20 warps resident per SM.
         int best_warps = 0;
-        for (int wpc = kWarpsPerCta; wpc >= 1; wpc >>= 1) {
-            int ctas = 0;
-            if (static_cast<size_t>(wpc) * stride > static_cast<size_t>(smem_optin)) continue;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel, 32 * wpc, static_cast<size_t>(wpc) * stride) !=
-                cudaSuccess)
-                continue;
-            if (ctas * wpc > best_warps) {
-                best_warps = ctas * wpc;
-                ctx->wpc = wpc;
-                ctx->ctas_per_sm = ctas;
+        uint32_t need = 0;
+        for (uint32_t K = 1; K <= 4; ++K) {
+            const uint32_t pk = (p_hint + K - 1) / K + (K > 1 ? 64u : 0u);                      // strips of a piece
+            const uint32_t rk = K > 1 ? ((r_hint / K + 256u + 15u) & ~15u) : r_hint;             // its payload bytes
+            const uint32_t p16 = (pk + 15u) & ~15u;
+            const uint32_t gap = rk >= p16 + 2048u ? 0u : p16 + 2048u - rk;
+            uint32_t need_k = std::max(rk + gap + 2u * pk + 16u * (pk / 32u + 3u), K > 1 ? r_hint : 0u) + kTabBytes + 32u;
+            need_k = std::min(std::max((need_k + 15u) & ~15u, 4096u), (static_cast<uint32_t>(smem_optin) - kWarpHdr - kTailPad) & ~15u);
+            const uint32_t stride = kWarpHdr + need_k + kTailPad;
+            for (int wpc = kWarpsPerCta; wpc >= 1; wpc >>= 1) {
+                int ctas = 0;
+                if (static_cast<size_t>(wpc) * stride > static_cast<size_t>(smem_optin)) continue;
+                if ((K > 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<true>, 32 * wpc, static_cast<size_t>(wpc) * stride)
+                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<false>, 32 * wpc, static_cast<size_t>(wpc) * stride)) !=
+                    cudaSuccess)
+                    continue;
+                if (ctas * wpc > best_warps) {
+                    best_warps = ctas * wpc;
+                    ctx->wpc = wpc;
+                    ctx->ctas_per_sm = ctas;
+                    ctx->pieces = static_cast<int>(K);
+                    need = need_k;
+                }
             }
+            // pieces repeat the per-FED fixed work: they pay only while the SM is short of warps
+            if (best_warps >= 20) break;
         }
         cudaGetLastError();
         if (best_warps < 1) return fail(SST_ERR_CUDA);
@@ -1870,7 +1999,8 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, cfg->device);
         cudaDeviceGetAttribute(&smem_reserved, cudaDevAttrReservedSharedMemoryPerBlock, cfg->device);
         size_t api_avail = 0;
-        cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel, ctx->ctas_per_sm, 32 * ctx->wpc);
+        if (ctx->pieces > 1) cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel<true>, ctx->ctas_per_sm, 32 * ctx->wpc);
+        else cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel<false>, ctx->ctas_per_sm, 32 * ctx->wpc);
         const size_t tries[2] = {smem_sm > 0 ? static_cast<size_t>(smem_sm) / ctx->ctas_per_sm - smem_reserved : 0, api_avail};
         for (size_t avail : tries) {
             avail = std::min<size_t>(avail, static_cast<size_t>(smem_optin));
@@ -1880,7 +2010,8 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
             const uint32_t keep = ctx->slot_bytes;
             set_slot(slot);
             int check = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel, 32 * ctx->wpc, ctx->smem_bytes) == cudaSuccess &&
+            if ((ctx->pieces > 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel<true>, 32 * ctx->wpc, ctx->smem_bytes)
+                                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel<false>, 32 * ctx->wpc, ctx->smem_bytes)) == cudaSuccess &&
                 check >= ctx->ctas_per_sm)
                 break;
             set_slot(keep);  // the grown slot lost a CTA
