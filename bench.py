@@ -9,8 +9,9 @@ once, per-event output buffers taken from the library's stream-ordered pool.
   value      whole-job events/s with the raw data already resident in HBM (CUDA-event timed)
   e2e        the same metric through sst_unpack_cluster_host_packed: pinned HOST buffers, H2D of the raw
              data and D2H of the clusters inside the timed region
-  roofline   algorithmic HBM bytes of a launch / launch duration for sst_event_kernel (the dominant
-             kernel; sst_emit_kernel behind it moves the staged clusters into order) against
+  roofline   algorithmic HBM bytes of a launch / launch duration for sst_event_kernel (the one kernel
+             of a launch with plain outputs: its warps also move the staged clusters into order once
+             the FED work is used up; --move-mode 1 leaves that to sst_emit_kernel behind it) against
              MEASURED_PEAKS.json
   cpu_baseline  the CPU oracle as it stands, timed on this box's host cores (reported, not a target)
 
@@ -269,8 +270,8 @@ def run_reference(args):
 
 # --------------------------------------------------------------------------- GPU arm
 def ncu_traffic(cfg_id: int):
-    """Measured DRAM bytes per step (read + write of both kernels) from the committed ncu launch
-    list summary profiles/traffic.csv (rows: workload, kernel, read bytes, write bytes), or None."""
+    """Measured DRAM bytes per step (read + write of every kernel of a step) from the committed ncu
+    launch list summary profiles/traffic.csv (rows: workload, kernel, read bytes, write bytes), or None."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(p):
         return None
@@ -725,7 +726,7 @@ def main():
         if traffic is not None:
             dram_gbs = traffic / (ms_step * 1e-3) / 1e9
             dram = {"bytes_per_step": traffic, "achieved": dram_gbs, "frac": dram_gbs / peak,
-                    "source": "profiles/traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum of both kernels, "
+                    "source": "profiles/traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum of the kernels of a step, "
                               "one step) over this run's step time"}
         line = {
             "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
@@ -742,14 +743,15 @@ def main():
                          "events_per_launch": n_events / launches_step,
                          "launch_us": dur_us,
                          "dram": dram,
-                         "limiter": "not HBM: sst_event_kernel is bound by instruction issue and the L1/LSU path "
-                                    "(profiles/r02_*.md); the calibration term of the algorithmic bytes is served by L2",
+                         "limiter": "not HBM: a warp works through its FED as one long chain of dependent steps, eight "
+                                    "warps per scheduler hide ~70 % of it (issue slots 70 % busy, DRAM ~30 %; "
+                                    "profiles/r02_final.md); the calibration term of the algorithmic bytes is served by L2",
                          "how": "achieved = algorithmic bytes per launch / launch duration, B_alg = raw + N dense + 32 B x "
                                 "noise sectors of present strips + 32 B x gain sectors of accepted-cluster strips + 20 B x "
-                                "clusters + cluster ADC bytes; sst_emit_kernel (the ordered move of the staged clusters) "
-                                "runs behind every sst_event_kernel, so launch duration = CUDA-event span of the timed "
-                                "region / sst_event_kernel launches (the emit kernel's time is charged to it); `dram` is "
-                                "the same span against the DRAM bytes ncu measured",
+                                "clusters + cluster ADC bytes; launch duration = CUDA-event span of the timed region / "
+                                "sst_event_kernel launches (move_mode 0: the ordered move of the staged clusters is part of "
+                                "that kernel; move_mode 1: sst_emit_kernel runs behind it and its time is charged to it); "
+                                "`dram` is the same span against the DRAM bytes ncu measured",
                          "serial": serial},
             "pipelined": pipelined,
             "default_hint": default_hint,
