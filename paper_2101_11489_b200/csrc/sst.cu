@@ -1657,6 +1657,8 @@ struct sst_ctx {
     std::atomic<float> packed_ratio{0.0f};  // packed result bytes per raw byte seen by the last packed host call
     int sm_count = 0;
     int pieces = 1;            // > 1: the slot was sized for FEDs worked on in pieces (sst_event_kernel<true>)
+    uint32_t whole_slot = 0;   // pieces > 1: slot that holds a whole large FED, for launches too small to fill
+    int whole_warps_sm = 0;    //             the GPU (their latency is one FED's: pieces only add to it)
     int wpc = kWarpsPerCta;    // warps per CTA of a full launch
     int ctas_per_sm = 0;       // resident CTAs of wpc warps
     uint32_t slot_bytes = 0;   // shared-memory slot of one warp (one FED)
@@ -1776,8 +1778,18 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     // warps per CTA: full CTAs once the work fills the GPU, smaller ones to spread a small launch
     const uint32_t sms = static_cast<uint32_t>(ctx->sm_count);
     const uint32_t wfull = static_cast<uint32_t>(ctx->wpc);
-    const uint32_t wpc = std::min(wfull, total >= 16u * sms ? 8u : total >= 8u * sms ? 4u : total >= 4u * sms ? 2u : 1u);
-    const uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (wfull / wpc);
+    uint32_t wpc = std::min(wfull, total >= 16u * sms ? 8u : total >= 8u * sms ? 4u : total >= 4u * sms ? 2u : 1u);
+    uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (wfull / wpc);
+    uint32_t slot_bytes = ctx->slot_bytes;
+    bool pieces = ctx->pieces > 1;
+    // a launch that whole-FED slots can hold in one wave takes those: one warp per CTA, no pieces
+    if (pieces && ctx->whole_slot && total <= sms * static_cast<uint32_t>(ctx->whole_warps_sm)) {
+        pieces = false;
+        slot_bytes = ctx->whole_slot;
+        wpc = 1;
+        capacity = sms * static_cast<uint32_t>(ctx->whole_warps_sm);
+    }
+    const uint32_t warp_stride = kWarpHdr + slot_bytes + kTailPad;
     const uint32_t grid = std::min((total + wpc - 1) / wpc, capacity);
     std::lock_guard<std::mutex> lock(ctx->slot_mu);
     sst_ctx::Slot *sl = nullptr;
@@ -1837,7 +1849,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.max_raw_bytes = ctx->cfg.max_raw_bytes;
     kp.n_feds = nf;
     kp.n_events = n;
-    kp.slot_bytes = ctx->slot_bytes;
+    kp.slot_bytes = slot_bytes;
     for (uint32_t e = 0; e < n; ++e) {
         kp.ev[e].raw = raw[e];
         kp.ev[e].fed_offsets = fed_offsets[e];
@@ -1851,15 +1863,15 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     // host block, hit coordinates and the compact SoA take sst_emit_kernel behind it
     const bool fused = !packed && !extras && ctx->cfg.move_mode == 0;
     kp.fused_move = fused ? 1u : 0u;
-    kp.move_chunk = std::min(1024u, ((ctx->slot_bytes - (kMoveAdc + 32u) - 32u) / 20u) & ~31u);  // (slot_bytes >= 4096)
+    kp.move_chunk = std::min(1024u, ((slot_bytes - (kMoveAdc + 32u) - 32u) / 20u) & ~31u);  // (slot_bytes >= 4096)
     // the epoch tags this launch's FED aggregates; before a tag is used again the words are cleared
     if (sl->epoch == kEpochs) {
         SST_CU(cudaMemsetAsync(blk + L.o_state, 0, L.state_bytes, st));
         sl->epoch = 0;
     }
     kp.epoch = ++sl->epoch;
-    if (ctx->pieces > 1) sst_event_kernel<true><<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
-    else sst_event_kernel<false><<<grid, 32 * wpc, wpc * ctx->warp_stride, st>>>(kp);
+    if (pieces) sst_event_kernel<true><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
+    else sst_event_kernel<false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
     cudaError_t err = cudaGetLastError();
     if (err == cudaSuccess) {
         // every warp draws one ticket too many before it stops
@@ -1959,7 +1971,7 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         // payload while the channel table is built, and one piece's lists afterwards.  K = 1..4 is
         // tried, up to the first that keeps 20 warps resident per SM.
         int best_warps = 0;
-        uint32_t need = 0;
+        uint32_t need = 0, need_whole = 0;
         for (uint32_t K = 1; K <= 4; ++K) {
             const uint32_t pk = (p_hint + K - 1) / K + (K > 1 ? 64u : 0u);                      // strips of a piece
             const uint32_t rk = K > 1 ? ((r_hint / K + 256u + 15u) & ~15u) : r_hint;             // its payload bytes
@@ -1968,6 +1980,7 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
             uint32_t need_k = std::max(rk + gap + 2u * pk + 16u * (pk / 32u + 3u), K > 1 ? r_hint : 0u) + kTabBytes + 32u;
             need_k = std::min(std::max((need_k + 15u) & ~15u, 4096u), (static_cast<uint32_t>(smem_optin) - kWarpHdr - kTailPad) & ~15u);
             const uint32_t stride = kWarpHdr + need_k + kTailPad;
+            if (K == 1) need_whole = need_k;
             for (int wpc = kWarpsPerCta; wpc >= 1; wpc >>= 1) {
                 int ctas = 0;
                 if (static_cast<size_t>(wpc) * stride > static_cast<size_t>(smem_optin)) continue;
@@ -2015,6 +2028,14 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
                 check >= ctx->ctas_per_sm)
                 break;
             set_slot(keep);  // the grown slot lost a CTA
+        }
+        if (ctx->pieces > 1) {
+            int ctas = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<false>, 32, kWarpHdr + need_whole + kTailPad) == cudaSuccess &&
+                ctas > 0) {
+                ctx->whole_slot = need_whole;
+                ctx->whole_warps_sm = ctas;
+            }
         }
         cudaGetLastError();
     }
