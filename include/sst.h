@@ -55,9 +55,11 @@ typedef struct {
     uint32_t max_events_in_flight; /* hint for the pool (0 = default 8)                         */
     uint32_t fed_strips_hint;      /* present (zero-suppressed) strips of a LARGE FED, e.g. the 99th
                                       percentile: sizes the per-FED shared-memory working set and
-                                      with it the number of FEDs in flight per SM.  0 = derive it from
+                                      with it the number of FEDs in flight per SM (when whole FEDs of
+                                      that size would leave an SM fewer than 20 of them, the context is
+                                      sized for FEDs worked on in pieces).  0 = derive it from
                                       max_raw_bytes / n_feds.  A FED above the hint is still processed
-                                      correctly, through a slower global-memory path               */
+                                      correctly, in pieces or through a slower global-memory path   */
     uint32_t move_mode;            /* how the staged clusters reach their ordered place (same results):
                                       0 = inside sst_event_kernel, by the warps that find the FED work
                                       used up (one launch; launches that want the packed host block, hit
@@ -149,7 +151,12 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx);
  * (non-zero = bad strip, never active), chan_module[n_feds*96] = module id of every channel,
  * non-decreasing, equal ids = same module, a module never crosses a FED.  The arrays are
  * validated, copied to the device in an internal layout and may be freed on return (the call
- * synchronises).  Must not run concurrently with sst_unpack_cluster on the same context. */
+ * synchronises).  The internal layout holds, per strip, the noise (+inf at bad strips) and a gain
+ * FACTOR with which one fused multiply-add reproduces min(254, floor(adc / gain + 0.5)) of the
+ * float32 division for every adc in 1..255: the call searches and verifies it per strip on all
+ * host cores (~5 core-seconds for 10.8 M strips); strips without such a factor keep their gain
+ * and are divided on the device.  Must not run concurrently with sst_unpack_cluster on the same
+ * context. */
 sst_status sst_upload_calib(sst_ctx *ctx, const float *gain, const float *noise, const uint8_t *bad,
                             const uint32_t *chan_module);
 
@@ -257,8 +264,9 @@ const char *sst_status_string(sst_status s);
 /* Static facts about the compiled kernel and this context, for benchmarks: bytes of dynamic
  * shared memory per CTA of sst_event_kernel (a CTA is threads/32 independent warps, one FED at a
  * time each), threads per CTA, resident CTAs per SM as reported by the occupancy API, SM count,
- * kernels per launch (sst_event_kernel + sst_emit_kernel), the part of a warp's shared memory
- * that holds a FED's payload and lists, events one launch can take. */
+ * kernels per launch with plain outputs (1; 2 with move_mode 1: sst_event_kernel + sst_emit_kernel),
+ * the part of a warp's shared memory that holds a FED's payload and lists, events one launch can
+ * take. */
 typedef struct {
     uint32_t smem_bytes, threads, ctas_per_sm, sm_count, kernels_per_event, slot_bytes, events_per_launch;
 } sst_info;

@@ -1,7 +1,7 @@
 // sst.cu -- libsst: unpack + three-threshold clustering of strip-tracker FED data on B200.
 //
-// Two kernels per launch, ONE WARP PER FED (a FED is 96 channels x 256 strips;
-// modules never cross a FED, reading s10).
+// ONE WARP PER FED (a FED is 96 channels x 256 strips; modules never cross a FED,
+// DESIGN.md reading s10), one kernel launch per batch of up to 64 events.
 //
 // sst_event_kernel: a CTA is up to eight independent warps, each with a ~7 KB shared-memory slot,
 // so 32 FEDs are in flight per SM and the serial parts of the method (the channel-length chain,
@@ -21,24 +21,31 @@
 //                             the ADC list is the payload squeezed in place.  The dense SoA is put
 //                             together in a 2 KB shared-memory window that leaves by TMA bulk store
 //   a3-a6 sweep             : lane per CHUNK of consecutive entries, walked serially: one 8-byte
-//                             gather of {noise, gain}, exact >= tests, link to the previous entry,
-//                             q = min(254, floor(adc/gain + .5)) in float32, and the open
-//                             candidate's (charge, sum noise^2 in double left to right, seed) in
-//                             registers; a candidate is tested where it ends (leftmost-seed
+//                             gather of {noise, gain factor}, exact >= tests, link to the previous
+//                             entry, q = min(254, floor(adc/gain + .5)) (one FMA with a factor
+//                             verified per strip at upload to reproduce the float32 division), and
+//                             the open candidate's (charge, sum noise^2 in double left to right,
+//                             seed) in registers; a candidate is tested where it ends (leftmost-seed
 //                             ownership is implicit: one test per maximal run).  Results are bits
 //                             (links, seeds, ends of accepted clusters) kept in registers and
 //                             flushed by all lanes together; a bit smear turns ends into members
 //   a4 seed-index array     : seed mask + ordered compaction; materialised on request
 //   a7 ordered output, 1/2  : counts by popcount scan, cluster records built lane per cluster and
 //                             staged FED-locally in global scratch, FED totals in one 64-bit word
+//                             tagged with the launch's epoch (release)
 //   compact SoA (request)   : the FED's lists staged as they are
 //
-// sst_emit_kernel (a7, 2/2), behind it on the same stream: exclusive prefix of the FED totals,
-// staged clusters moved to their (module, first strip)-ordered place; on request the clusters'
-// global hit coordinates and the compact SoA with the calibration gathered per entry
-// (PAPER.md:25, :31).  No warp waits for another.
+// A FED whose lists do not fit the slot is worked on in PIECES (channel ranges that start at module
+// boundaries, sst_event_kernel<true>: contexts whose FEDs are large keep their warps per SM that
+// way), or, when even that fails, through a pooled global scratch.
 //
-// FEDs whose payload or lists exceed the slot run the same code on a pooled global scratch.
+// a7, 2/2, the ordered move: a warp that finds the FED tickets used up goes on to MOVE staged FEDs
+// -- exclusive prefix of the state words of the FED's predecessors (acquire), the staged FED into
+// its free slot by TMA bulk copies, the cluster arrays streamed out in (module, first strip) order
+// -- while the last FEDs are still being worked on by others.  Launches that want the packed host
+// block, the clusters' global hit coordinates or the compact SoA with the calibration
+// gathered per entry, and contexts with move_mode 1, take sst_emit_kernel behind
+// sst_event_kernel on the same stream instead: one warp per (event, FED), no waiting.
 // No tensor cores: nothing here is a contraction.
 #include <cuda_runtime.h>
 
