@@ -269,6 +269,7 @@ const char *sst_status_string(sst_status s);
  * take. */
 typedef struct {
     uint32_t smem_bytes, threads, ctas_per_sm, sm_count, kernels_per_event, slot_bytes, events_per_launch;
+    uint32_t pieces; /* 1: the slot was sized for whole FEDs; > 1: for FEDs worked on in that many pieces */
 } sst_info;
 sst_status sst_get_info(const sst_ctx *ctx, sst_info *info);
 

@@ -49,7 +49,7 @@ class sst_output(C.Structure):
 class sst_info(C.Structure):
     _fields_ = [("smem_bytes", C.c_uint32), ("threads", C.c_uint32), ("ctas_per_sm", C.c_uint32),
                 ("sm_count", C.c_uint32), ("kernels_per_event", C.c_uint32), ("slot_bytes", C.c_uint32),
-                ("events_per_launch", C.c_uint32)]
+                ("events_per_launch", C.c_uint32), ("pieces", C.c_uint32)]
 
 
 class SSTError(RuntimeError):

@@ -2634,6 +2634,7 @@ sst_status sst_get_info(const sst_ctx *ctx, sst_info *info) {
     info->kernels_per_event = ctx->cfg.move_mode == 0 ? 1 : 2;  // (launches with plain outputs)
     info->slot_bytes = ctx->slot_bytes;
     info->events_per_launch = kMaxEv;
+    info->pieces = static_cast<uint32_t>(ctx->pieces);
     return SST_OK;
 }
 

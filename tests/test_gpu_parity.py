@@ -936,6 +936,56 @@ def _random_event(rng, n_feds):
     return raw, fo, gain, noise, bad, cm
 
 
+def test_feds_in_pieces_with_irregular_structure(H, oracle):
+    """A context sized for FEDs in pieces (sst_info.pieces > 1) whose slot is far smaller than its
+    FEDs: 10 events x 5 FEDs of random structure at 15-95 % occupancy (malformed channels, recorded
+    zeros, split runs, full channels, modules of 1-5 channels, so piece boundaries fall anywhere a
+    module starts), one FED with a chain overrun and one with unaligned offsets among them, every
+    optional output on, in one batch call issued three times.  FEDs that need more than seven pieces
+    (95 % occupancy) take the global-scratch path in the same launch."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    n_ev, nf = 10, 5
+    evs = []
+    rng = np.random.Generator(np.random.PCG64(77))
+    # one calibration / module map for all events: take those of the first draw
+    raw0, fo0, gain, noise, bad, cm = _random_event(rng, nf)
+    for i in range(n_ev):
+        r, f, *_ = _random_event(np.random.Generator(np.random.PCG64(500 + i)), nf)
+        evs.append([r, f])
+    # event 3: the length chain of FED 2 overruns (a length word made huge)
+    r3 = evs[3][0].copy()
+    r3[int(evs[3][1][2]) + 1] = 0xff
+    evs[3][0] = r3
+    # event 6: FED 1 moved by 1 byte of its padding (unaligned start of FED 2)
+    off, ln, _, _ = oracle.unpack(evs[6][0], evs[6][1], nf)
+    used = int(off[1 * 96 + 95]) + int(ln[1 * 96 + 95]) - int(evs[6][1][1])
+    if (int(evs[6][1][2]) - int(evs[6][1][1])) - used >= 1:
+        evs[6][0], evs[6][1] = cases.move_fed_padding(evs[6][0], evs[6][1], 1, used, 1)
+    thr = (2.0, 3.0, 5.0)
+    mrb = (max(int(e[0].size) for e in evs) + 4095) // 4096 * 4096
+    want = [oracle.run(e[0], e[1], nf, gain, noise, bad, cm, thr, cap_clusters=mrb, cap_adc=mrb + 1) for e in evs]
+    strips = [int(np.count_nonzero(w.adc.reshape(nf, -1), axis=1).max()) for w in want]
+    det = H.Detector(nf, gain, noise, bad, cm, max_raw_bytes=mrb, fed_strips_hint=3000)
+    try:
+        info = det.info()
+        assert info["pieces"] > 1, info
+        assert max(strips) * 3 > info["slot_bytes"], "the FEDs must not fit the slot whole"
+        streams = [torch.cuda.Stream() for _ in range(4)]
+        d_in = [det.upload_raw(e[0], e[1]) for e in evs]
+        outs = [det.alloc_outputs(mrb, mrb + 1, chan_map=True, seeds=True, snr=True, cap_seeds=mrb) for _ in range(n_ev)]
+        batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], thr, [o.out for o in outs], [s.cuda_stream for s in streams])
+        torch.cuda.synchronize()
+        for _ in range(3):
+            B.sst_unpack_cluster_batch(det.ctx, batch)
+        torch.cuda.synchronize()
+        for o, w in zip(outs, want):
+            compare(H.unsigned_view(o.numpy()), w)
+        assert sum(int(w.status[4]) for w in want) >= 1 and sum(int(w.status[1]) for w in want) >= 1
+    finally:
+        det.close()
+
+
 @pytest.mark.parametrize("seed", range(24))
 def test_random_structure(H, oracle, seed):
     rng = np.random.Generator(np.random.PCG64(1000 + seed))
