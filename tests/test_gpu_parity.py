@@ -936,6 +936,37 @@ def _random_event(rng, n_feds):
     return raw, fo, gain, noise, bad, cm
 
 
+def test_epoch_wraps_after_4095_launches_on_a_stream(H, oracle):
+    """The FED state words carry a 12-bit launch epoch (what the in-kernel move waits for); it wraps
+    after 4095 launches of a stream, before which the words are cleared.  4096 launches of small
+    events on one stream, the first and the last a two-event batch (with the events swapped), so
+    that the last launch meets words of its own epoch left by the first unless they were cleared."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf = 3
+    cfg, cal, evs = synth.make_config(0, n_feds=nf, event_seeds=[1, 2])
+    mrb = (max(int(e.raw.size) for e in evs) + 4095) // 4096 * 4096
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        st = torch.cuda.Stream()
+        d_in = [det.upload_raw(e.raw, e.fed_offsets) for e in evs]
+        outs = [det.alloc_outputs(mrb // 2 + 1, mrb, seeds=True, chan_map=True, snr=True, cap_seeds=mrb) for _ in evs]
+        both_ev = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs], [st.cuda_stream])
+        swapped = B.Batch([d[0] for d in d_in[::-1]], [d[1] for d in d_in[::-1]], (2, 3, 5), [o.out for o in outs[::-1]], [st.cuda_stream])
+        # launch 1 (epoch 1) leaves the other event's words at index 1; launches 2..4095 touch index 0
+        # only; launch 4096 is the first of the next round of epochs, again with epoch 1
+        B.sst_unpack_cluster_batch(det.ctx, swapped)
+        for i in range(4094):
+            det.run(d_in[i & 1][0], d_in[i & 1][1], (2, 3, 5), outs[i & 1], stream=st)
+        B.sst_unpack_cluster_batch(det.ctx, both_ev)
+        torch.cuda.synchronize()
+        for e, o in zip(evs, outs):
+            r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            compare(H.unsigned_view(o.numpy()), r)
+    finally:
+        det.close()
+
+
 def test_feds_in_pieces_with_irregular_structure(H, oracle):
     """A context sized for FEDs in pieces (sst_info.pieces > 1) whose slot is far smaller than its
     FEDs: 10 events x 5 FEDs of random structure at 15-95 % occupancy (malformed channels, recorded
