@@ -280,9 +280,10 @@ def test_unaligned_fed_offsets_use_the_slow_path(H, oracle):
 
 
 # ------------------------------------------------------------------ generated events
-@pytest.mark.parametrize("cid,nf", [(0, 24), (1, 37), (2, 29), (4, 41)])
+@pytest.mark.parametrize("cid,nf", [(0, 24), (1, 37), (2, 29), (4, 41), (0, 1000)])
 def test_generated_configs_small(H, oracle, cid, nf):
-    """Sizes the oracle finishes in well under a second: several CTAs and a ragged FED count."""
+    """Sizes the oracle finishes in well under a second: several CTAs and a ragged FED count; 1000
+    FEDs: more than one pass of the prefix over the FED state words (448 per pass)."""
     cfg, cal, evs = synth.make_config(cid, n_feds=nf)
     ev = evs[0]
     det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size))
