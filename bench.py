@@ -19,7 +19,8 @@ After the timed loop the output blocks of the TIMED launches are read back and e
 every event is compared with the oracle (bit-exact; barycenter 1e-6 relative); a difference fails
 the run.  `--config 1|2|4` times 64 events of that BASELINE.json config instead of config 3.
 `--sweep` prints the single-event latencies, events/s against events per call and against the
-number of streams, and the OpenMP oracle's N x M table.  `--impl reference` times the oracle alone
+number of streams, and the OpenMP oracle's N x M table.  `--trace` prints where a warp's time goes,
+phase by phase, and the timeline of a launch (sst_config.trace).  `--impl reference` times the oracle alone
 on the same config (see the task's contract).
 """
 from __future__ import annotations
@@ -372,6 +373,52 @@ def run_sweep(args):
     print(json.dumps({"sweep": out}))
 
 
+TRACE_PHASES = ("ticket + prologue", "payload staging (TMA wait)", "length chain", "pass 1 + scan", "pass 2", "expansion",
+                "dense SoA", "sweep", "members and heads", "counts + cluster list", "staging of the clusters", "publish")
+
+
+def run_trace(args):
+    """Where a warp's time goes, FED phase by FED phase, and the timeline of one launch: a context
+    created with sst_config.trace = 1 (the traced instantiations of sst_event_kernel), one launch of
+    n events of the chosen config for n = 1, 8, 64; sst_trace_read after each."""
+    import torch
+    from paper_2101_11489_b200 import binding as B, harness
+    torch.cuda.set_device(0)
+    n_feds = args.n_feds
+    calib = synth.make_calibration(n_feds, synth.CONFIGS[args.config].bad_frac)
+    events = generate_events(args.config, n_feds, range(1, N_EVENTS + 1), calib)
+    mhz = float(subprocess.check_output(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", "0"],
+                                        text=True).split()[0])
+    max_raw = (max(int(e[0].size) for e in events) + 4095) // 4096 * 4096
+    hint = int(1.02 * np.percentile([int(e[2]["p99_fed_strips"]) for e in events], 90)) + 16
+    det = harness.Detector(n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module, max_raw_bytes=max_raw,
+                           max_events_in_flight=N_STREAMS, fed_strips_hint=hint, move_mode=MOVE_MODE, trace=1)
+    st = torch.cuda.Stream()
+    d_in = [det.upload_raw(e[0], e[1]) for e in events]
+    outs = [harness.PooledOutputs(det, max_raw // 3 + 1, max_raw, st.cuda_stream, dense=True) for _ in events]
+    out = {"config": args.config, "n_feds": n_feds, "move_mode": MOVE_MODE, "sm_max_mhz": mhz, "info": det.info(), "launches": []}
+    for n in (1, 8, 64):
+        batch = B.Batch([d[0] for d in d_in[:n]], [d[1] for d in d_in[:n]], THRESHOLDS, [o.out for o in outs[:n]], [st.cuda_stream])
+        for _ in range(3):
+            B.sst_unpack_cluster_batch(det.ctx, batch)
+        B.sst_trace_read(det.ctx, st.cuda_stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        B.sst_unpack_cluster_batch(det.ctx, batch)
+        e1.record(st)
+        t = B.sst_trace_read(det.ctx, st.cuda_stream)
+        feds = max(t[0], 1)
+        phases = {name: t[1 + i] / feds / mhz for i, name in enumerate(TRACE_PHASES)}
+        out["launches"].append({
+            "events": n, "feds": t[0], "launch_us_cuda_events": 1e3 * e0.elapsed_time(e1),
+            "us_per_fed_by_phase": phases, "us_per_fed": sum(phases.values()),
+            "feds_moved_in_kernel": t[13], "us_per_moved_fed": t[14] / max(t[13], 1) / mhz,
+            "timeline_us": {"first_warp_out_of_fed_tickets": (t[21] - t[20]) / 1e3, "last_warp_out_of_fed_tickets": (t[22] - t[20]) / 1e3,
+                            "kernel_end": (t[23] - t[20]) / 1e3}})
+    det.close()
+    print(json.dumps({"trace": out}))
+
+
 def respawn_under_torchrun(args):
     """`python bench.py --gpus N` with N > 1 and no launcher: start N ranks (one per GPU)."""
     import socket
@@ -397,6 +444,9 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle timing (rank 0, N=1)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (and with it the verification)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--trace", action="store_true",
+                    help="instead of the bench line: per-phase time of a FED and the timeline of a launch of 1, 8 and 64 "
+                         "events, from a context with sst_config.trace = 1")
     ap.add_argument("--move-mode", type=int, default=0, choices=[0, 1],
                     help="sst_config.move_mode: 0 = the ordered move inside sst_event_kernel, 1 = sst_emit_kernel behind it")
     ap.add_argument("--sweep", action="store_true",
@@ -409,6 +459,8 @@ def main():
         args.warmup = 3
     if args.sweep:
         return run_sweep(args)
+    if args.trace:
+        return run_trace(args)
     world_env = os.environ.get("WORLD_SIZE")
     if world_env is None and args.gpus > 1:
         return respawn_under_torchrun(args)

@@ -65,6 +65,10 @@ typedef struct {
                                       used up (one launch; launches that want the packed host block, hit
                                       coordinates or the compact SoA always take the second kernel);
                                       1 = always by sst_emit_kernel, launched behind it              */
+    uint32_t trace;                /* 1 = launch the traced instantiations of sst_event_kernel: lane 0 of
+                                      every warp adds the cycles of each phase of each FED and the
+                                      launch's timeline to 32 words per stream (sst_trace_read); same
+                                      results, ~1 % slower.  0 = no tracing code in the kernel at all  */
 } sst_config;
 
 /* S/N thresholds of the "three thresholds" algorithm: a strip is active at
@@ -272,6 +276,21 @@ typedef struct {
     uint32_t pieces; /* 1: the slot was sized for whole FEDs; > 1: for FEDs worked on in that many pieces */
 } sst_info;
 sst_status sst_get_info(const sst_ctx *ctx, sst_info *info);
+
+/* Tracing (contexts created with trace = 1).  Waits for `stream`, copies the stream's 32 trace words
+ * to HOST `out` and clears them; SST_ERR_INVALID_ARG without tracing or before the stream's first
+ * launch.  Words (sums over all FEDs of all launches of the stream since the last read):
+ *   [0]  FEDs worked on
+ *   [1..12] clock64 cycles of lane 0 per phase: 1 ticket + prologue, 2 payload staging (TMA wait),
+ *        3 length chain, 4 pass 1 + scan (+ piece planning), 5 pass 2, 6 expansion (+ compact staging),
+ *        7 dense SoA, 8 sweep, 9 members and heads, 10 counts + cluster list, 11 staging of the clusters,
+ *        12 publish
+ *   [13] FEDs moved inside sst_event_kernel, [14] cycles of those moves
+ *   [20..23] %globaltimer nanoseconds of the LAST launch read: first warp started, first warp out of
+ *        FED tickets, last warp out of FED tickets, last warp done (kernel end)
+ * The rest is 0. */
+#define SST_TRACE_WORDS 32
+sst_status sst_trace_read(sst_ctx *ctx, void *stream, uint64_t *out);
 
 #ifdef __cplusplus
 }

@@ -22,12 +22,13 @@ SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB =
 EXPORTS = ["sst_create", "sst_upload_calib", "sst_upload_geometry", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
            "sst_unpack_cluster_host_batch", "sst_unpack_cluster_host_packed",
            "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_event_download", "sst_destroy", "sst_last_cuda_error",
-           "sst_status_string", "sst_get_info"]
+           "sst_status_string", "sst_get_info", "sst_trace_read"]
 
 
 class sst_config(C.Structure):
     _fields_ = [("n_feds", C.c_uint32), ("device", C.c_int32), ("max_raw_bytes", C.c_uint32),
-                ("max_events_in_flight", C.c_uint32), ("fed_strips_hint", C.c_uint32), ("move_mode", C.c_uint32)]
+                ("max_events_in_flight", C.c_uint32), ("fed_strips_hint", C.c_uint32), ("move_mode", C.c_uint32),
+                ("trace", C.c_uint32)]
 
 
 class sst_thresholds(C.Structure):
@@ -89,6 +90,7 @@ def load():
     L.sst_status_string.argtypes = [C.c_int]
     L.sst_status_string.restype = C.c_char_p
     L.sst_get_info.argtypes = [vp, C.POINTER(sst_info)]
+    L.sst_trace_read.argtypes = [vp, vp, C.POINTER(C.c_uint64)]
     for name in EXPORTS:
         if name not in ("sst_last_cuda_error", "sst_status_string"):
             getattr(L, name).restype = C.c_int
@@ -116,9 +118,9 @@ def _ptr(t) -> Optional[int]:
 
 
 def sst_create(n_feds: int, device: int = 0, max_raw_bytes: int = 1 << 22, max_events_in_flight: int = 8,
-               fed_strips_hint: int = 0, move_mode: int = 0):
+               fed_strips_hint: int = 0, move_mode: int = 0, trace: int = 0):
     L = load()
-    cfg = sst_config(n_feds, device, max_raw_bytes, max_events_in_flight, fed_strips_hint, move_mode)
+    cfg = sst_config(n_feds, device, max_raw_bytes, max_events_in_flight, fed_strips_hint, move_mode, trace)
     ctx = C.c_void_p()
     _check(None, L.sst_create(C.byref(cfg), C.byref(ctx)), "sst_create")
     return ctx
@@ -302,3 +304,13 @@ def sst_get_info(ctx) -> dict:
     info = sst_info()
     _check(ctx, load().sst_get_info(ctx, C.byref(info)), "sst_get_info")
     return {k: getattr(info, k) for k, _ in sst_info._fields_}
+
+
+TRACE_WORDS = 32
+
+
+def sst_trace_read(ctx, stream: int):
+    """The stream's 32 trace words (include/sst.h) as a list; waits for the stream."""
+    out = (C.c_uint64 * TRACE_WORDS)()
+    _check(ctx, load().sst_trace_read(ctx, stream, out), "sst_trace_read")
+    return list(out)

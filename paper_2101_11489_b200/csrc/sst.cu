@@ -108,6 +108,7 @@ struct KParams {
     uint8_t *s_cadc;
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
     unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, + tickets + warps)
+    unsigned long long *trace;      // 32 words of the stream's scratch (sst_trace_read), used by the traced kernels
     unsigned long long ticket_base;
     uint32_t epoch;       // tag of this launch's FED aggregates
     uint32_t move_chunk;  // clusters per bulk copy of the in-kernel move (from the slot size)
@@ -289,6 +290,10 @@ __device__ __forceinline__ void walk_chain_speculative(uint32_t stage_addr, uint
     }
 }
 
+// Tracing (sst_config.trace, kernel instantiations of their own): lane 0 of a warp adds the clock64
+// cycles since its previous stamp to the slot of the phase that just ended, per FED.
+enum { kTrFeds = 0, kTrMoved = 13, kTrMoveCycles = 14, kTrStart = 20, kTrFirstOut = 21, kTrLastOut = 22, kTrEnd = 23 };
+
 struct FedCtx {
     uint32_t ev, f;
     uint32_t fo0;                  // the FED's start offset as given (reported in chan_off)
@@ -304,7 +309,19 @@ struct FedCtx {
     uint32_t ch_lo, ch_hi;         // the piece's channels [ch_lo, ch_hi); 0, 96 for a whole FED
     uint32_t last;                 // the piece ends the FED: the FED's word is published
     uint32_t cl_base, adc_base, seed_base, ent_base, nz_base;  // counts of the FED's earlier pieces
+    long long t_prev;              // tracing: clock64 at the previous stamp
 };
+
+// slot k - 1 is the phase that ends where stamp k stands: 1 ticket + prologue, 2 payload staging,
+// 3 chain, 4 pass 1 + scan, 5 pass 2, 6 expansion (+ compact staging), 7 dense SoA, 8 sweep,
+// 9 members and heads, 10 counts + cluster list, 11 staging of the clusters, 12 publish (stamp 13)
+__device__ __forceinline__ void trace_stamp(const KParams &p, FedCtx &c, const int lane, const int k) {
+    if (lane == 0) {
+        const long long t = clock64();
+        atomicAdd(p.trace + (k - 1), static_cast<unsigned long long>(t - c.t_prev));
+        c.t_prev = t;
+    }
+}
 
 // a2 pass 1: a lane validates the run lists of its three channels (reading s2b) and
 // counts their strips and runs, one channel after the other.  The loop body has no exit: a
@@ -401,7 +418,7 @@ __device__ __forceinline__ uint32_t fast_strip_base(uint32_t A, uint32_t P16, bo
 // scratch and rp is whatever holds the payload.  Returns false (fast path only) when the cluster
 // records outgrow the slot: the FED is then redone on the slow path (nothing has been published
 // and every output written so far is rewritten identically).
-template <bool kFast, bool kPiece>
+template <bool kFast, bool kPiece, bool kTrace>
 __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const uint8_t *rp, FedCtx &c,
                                           const int lane, uint32_t &next_ticket) {
     const uint32_t f = c.f, P = c.P;
@@ -460,6 +477,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     uint8_t *const dense = o.strip_adc ? o.strip_adc + static_cast<size_t>(f) * kFedStrips : nullptr;
     const float2 *cal = p.calib + static_cast<size_t>(f) * kFedStrips;
 
+    if (kTrace) trace_stamp(p, c, lane, 5);
     // ---------------------------------------------------------------- a2 pass 2: the run starts
     // Lane per channel again, headers only: the list entry of the first strip of every run gets
     // 1 + its strip id (bit 15 marks strip 0 of a channel that opens a module: nothing links across
@@ -496,6 +514,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     }
     __syncwarp();
 
+    if (kTrace) trace_stamp(p, c, lane, 6);
     // ---------------------------------------------------------------- a2: expansion, lane per entry
     // Entry e belongs to the last run that starts at or before it (the non-zero entries, by ballot):
     // its strip id is that run's first strip + the distance, and its ADC byte sits at e + 2 * (runs
@@ -572,6 +591,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         if (lane == 0 && last) p.fed_present[static_cast<size_t>(c.ev) * p.n_feds + f] = ((ent_base + P) << 16) | (nz_base + nz);
     }
 
+    if (kTrace) trace_stamp(p, c, lane, 7);
     // ---------------------------------------------------------------- a2: dense SoA
     // The FED's 24576-byte block of the dense strip array is put together 2048 strips at a time
     // in a shared-memory window (zeros, then the present strips of the window from the sorted
@@ -627,6 +647,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         __syncwarp();
     }
 
+    if (kTrace) trace_stamp(p, c, lane, 8);
     // ---------------------------------------------------------------- a3..a6: one sweep over the lists
     // Lane per CHUNK of consecutive entries, walked serially: active/seed tests, link to the previous
     // entry, and the running (charge, noise^2, seed) of the open candidate are thread-local, so a
@@ -829,6 +850,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     }
     __syncwarp();
 
+    if (kTrace) trace_stamp(p, c, lane, 9);
     // ---------------------------------------------------------------- a5: members and heads
     // Lane per mask word: the end bits of the accepted clusters are smeared down along the links
     // (across word boundaries until nothing changes: a second round only happens for clusters
@@ -859,6 +881,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     }
     __syncwarp();
 
+    if (kTrace) trace_stamp(p, c, lane, 10);
     // ---------------------------------------------------------------- counts and cluster records
     // lane per mask word: exclusive prefix of (accepted heads, accepted members) per word, then
     // every head's list entry goes into the FED's cluster list, in order
@@ -891,6 +914,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     }
     __syncwarp();
 
+    if (kTrace) trace_stamp(p, c, lane, 11);
     // ---------------------------------------------------------------- a7, first half: publish + stage
     // The FED's counts go into its state word; its clusters, cluster ADCs and seeds are staged in
     // FED-local order in global scratch.  sst_emit_kernel, launched behind this kernel on the same
@@ -980,6 +1004,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         c.seed_base = seed_base + fed_seed;
     }
     if (!last) return true;  // (uniform) more pieces of this FED follow
+    if (kTrace) trace_stamp(p, c, lane, 12);
     // publish: the FED's counts, tagged with the launch's epoch, behind everything staged above
     // (release: the in-kernel move of another warp may read the staging as soon as it sees the word,
     // and it reads it with TMA bulk copies: the writers order their generic-proxy stores before
@@ -994,6 +1019,10 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
                                      (static_cast<unsigned long long>(adc_base + fed_adc) << kShAdc) | (cl_base + fed_cl);
         asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p.fed_state + static_cast<size_t>(c.ev) * p.n_feds + f), "l"(v) : "memory");
     }
+    if (kTrace) {
+        trace_stamp(p, c, lane, 13);
+        if (lane == 0) atomicAdd(p.trace + kTrFeds, 1ull);
+    }
     return true;
 }
 
@@ -1001,11 +1030,12 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
 // Returns false when the FED has to be redone with force_slow (see fed_lists).
 // kPieces: a FED whose lists do not fit the slot is worked on in pieces (contexts whose slot was
 // sized for that); else it goes through the global scratch.
-template <bool kPieces>
+template <bool kPieces, bool kTrace>
 __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long *mbar, uint8_t *slot,
                                             const uint32_t ticket, const int lane, const bool force_slow,
                                             uint32_t &mbar_phase, uint32_t &next_ticket) {
     FedCtx c;
+    if (kTrace) c.t_prev = clock64();
     // FED-major order: the same FED of all the launch's events back to back, so the FED's slab of
     // the calibration (196 KB) is reused from L2 while it is hot
     c.f = ticket / p.n_events;
@@ -1024,6 +1054,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     uint32_t *const chan_off = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes);
     uint16_t *const chan_len = reinterpret_cast<uint16_t *>(chan_off + kChan + 1);
 
+    if (kTrace) trace_stamp(p, c, lane, 2);
     // ---------------------------------------------------------------- a1: stage the FED payload
     // lanes 0/1 fetch the two offsets; lane 0 starts the bulk copy
     const uint32_t fo = lane < 2 ? E.fed_offsets[f + lane] : 0u;
@@ -1070,6 +1101,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         mbar_phase ^= 1u;
     }
 
+    if (kTrace) trace_stamp(p, c, lane, 3);
     // ---------------------------------------------------------------- a1: walk the length chain
     if (staged) {
         const uint32_t sa = smem_addr(slot);
@@ -1107,6 +1139,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     }
     __syncwarp();  // the channel table is in registers: its place in the slot is free
 
+    if (kTrace) trace_stamp(p, c, lane, 4);
     // ---------------------------------------------------------------- a2 pass 1: run headers
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -1188,8 +1221,8 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
             lo = best;
         }
     }
-    if (slow) return fed_lists<false, false>(p, slot, rp, c, lane, next_ticket);
-    if (!kPieces || n_pieces == 0) return fed_lists<true, false>(p, slot, slot, c, lane, next_ticket);
+    if (slow) return fed_lists<false, false, kTrace>(p, slot, rp, c, lane, next_ticket);
+    if (!kPieces || n_pieces == 0) return fed_lists<true, false, kTrace>(p, slot, slot, c, lane, next_ticket);
     FedCtx pc = c;  // the piece's view of the FED (c stays as it is: the whole FED's, in registers)
     for (uint32_t i = 0, b0 = 0; i < n_pieces; ++i) {
         const uint32_t b1 = static_cast<uint32_t>(plan >> (8u * i)) & 0xffu;
@@ -1221,7 +1254,7 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
         pc.ch_hi = b1;
         pc.last = i + 1u == n_pieces;
         __syncwarp();
-        if (!fed_lists<true, true>(p, slot, slot, pc, lane, next_ticket)) return false;
+        if (!fed_lists<true, true, kTrace>(p, slot, slot, pc, lane, next_ticket)) return false;
         b0 = b1;
     }
     return true;
@@ -1407,6 +1440,7 @@ __device__ __forceinline__ void move_fed(const KParams &p, unsigned long long *m
 // launch's epoch.  Every warp of the grid is resident (the grid never exceeds the resident
 // capacity) and every FED ticket has been drawn by a running warp before the first move ticket is,
 // so a wait always ends.
+template <bool kTrace>
 __device__ __forceinline__ void move_phase(const KParams &p, unsigned long long *mbar, uint8_t *slot, uint32_t &mbar_phase,
                                            uint32_t ticket, const uint32_t total, const int lane) {
     while (ticket < 2u * total) {
@@ -1414,7 +1448,12 @@ __device__ __forceinline__ void move_phase(const KParams &p, unsigned long long 
         uint32_t next_ticket = 0;
         if (lane == 0) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
         const uint32_t f = t / p.n_events;
+        const long long t0 = kTrace ? clock64() : 0;
         move_fed(p, mbar, slot, mbar_phase, t - f * p.n_events, f, lane);
+        if (kTrace && lane == 0) {
+            atomicAdd(p.trace + kTrMoveCycles, static_cast<unsigned long long>(clock64() - t0));
+            atomicAdd(p.trace + kTrMoved, 1ull);
+        }
         ticket = __shfl_sync(kFull, next_ticket, 0);
     }
 }
@@ -1423,7 +1462,7 @@ __device__ __forceinline__ void move_phase(const KParams &p, unsigned long long 
 // Every warp works alone: it draws (event, FED) tickets until the launch's work is used up and
 // never meets a block-wide barrier.  A CTA is just 1..kWarpsPerCta such warps sharing the SM's
 // shared memory (one driver reserve per CTA instead of one per warp).
-template <bool kPieces>
+template <bool kPieces, bool kTrace>
 __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(const __grid_constant__ KParams p) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -1436,13 +1475,19 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
     }
     __syncwarp();
     const uint32_t total = p.n_events * p.n_feds;
+    auto wall_ns = [] {  // tracing: the launch's timeline on the GPU's nanosecond clock
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        return t;
+    };
+    if (kTrace && lane == 0) atomicMin(p.trace + kTrStart, wall_ns());
     uint32_t mbar_phase = 0;
     uint32_t ticket = 0;
     if (lane == 0) ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
     ticket = __shfl_sync(kFull, ticket, 0);
     while (ticket < total) {
         uint32_t next_ticket = 0;
-        for (bool slow = false; !process_fed<kPieces>(p, mbar, slot, ticket, lane, slow, mbar_phase, next_ticket); slow = true) {
+        for (bool slow = false; !process_fed<kPieces, kTrace>(p, mbar, slot, ticket, lane, slow, mbar_phase, next_ticket); slow = true) {
         }  // (a FED whose cluster list outgrows the slot is redone through the global scratch)
         ticket = __shfl_sync(kFull, next_ticket, 0);
     }
@@ -1452,7 +1497,13 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
     // moved once it and all its predecessors of the event carry this launch's epoch.  Every warp of
     // the grid is resident (the grid never exceeds the resident capacity) and every FED ticket has
     // been drawn by a running warp before the first move ticket is, so the wait always ends.
-    if (p.fused_move) move_phase(p, mbar, slot, mbar_phase, ticket, total, lane);
+    if (kTrace && lane == 0) {
+        const unsigned long long t = wall_ns();
+        atomicMin(p.trace + kTrFirstOut, t);
+        atomicMax(p.trace + kTrLastOut, t);
+    }
+    if (p.fused_move) move_phase<kTrace>(p, mbar, slot, mbar_phase, ticket, total, lane);
+    if (kTrace && lane == 0) atomicMax(p.trace + kTrEnd, wall_ns());
 }
 
 // ------------------------------------------------------------------------------ a7, second half
@@ -1753,8 +1804,8 @@ ScratchLayout scratch_layout(const sst_ctx *ctx, size_t cap_events) {
     // a cluster costs >= 2 raw bytes: one ADC byte and a separator (an inactive strip, or a run header)
     L.cl_slots = static_cast<size_t>(ctx->cfg.max_raw_bytes) / 2 + nf + 8;
     L.state_bytes = sizeof(unsigned long long) * nf * cap_events;
-    L.o_ticket = 0;
-    L.o_state = 256;
+    L.o_ticket = 0;  // (+ 256: the 32 trace words)
+    L.o_state = 512;
     // slow-path lists
     L.o_rec = L.o_state + up(L.state_bytes);
     L.o_mask = L.o_rec + up(4 * L.ents * cap_events);
@@ -1818,6 +1869,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
             cudaFreeAsync(mem, st);
             return SST_ERR_CUDA;
         }
+        cudaMemsetAsync(mem + Ln.o_ticket + 256 + 8 * kTrStart, 0xff, 16, st);  // trace: the two minima
         sl->mem = mem;
         sl->cap_events = want;
         sl->ticket_base = 0;
@@ -1837,6 +1889,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.s_cadc = blk + L.o_cadc;
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
     kp.ticket_base = sl->ticket_base;
+    kp.trace = reinterpret_cast<unsigned long long *>(blk + L.o_ticket + 256);
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
     kp.g_rec = reinterpret_cast<uint32_t *>(blk + L.o_rec);
     kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
@@ -1877,8 +1930,11 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         sl->epoch = 0;
     }
     kp.epoch = ++sl->epoch;
-    if (pieces) sst_event_kernel<true><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
-    else sst_event_kernel<false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
+    const bool trace = ctx->cfg.trace != 0;
+    if (pieces && trace) sst_event_kernel<true, true><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
+    else if (pieces) sst_event_kernel<true, false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
+    else if (trace) sst_event_kernel<false, true><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
+    else sst_event_kernel<false, false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
     cudaError_t err = cudaGetLastError();
     if (err == cudaSuccess) {
         // every warp draws one ticket too many before it stops
@@ -1921,7 +1977,7 @@ extern "C" {
 sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
     if (out_ctx) *out_ctx = nullptr;
     if (!cfg || !out_ctx || cfg->n_feds == 0 || cfg->n_feds > kMaxFeds || cfg->max_raw_bytes == 0 ||
-        cfg->move_mode > 1)
+        cfg->move_mode > 1 || cfg->trace > 1)
         return SST_ERR_INVALID_ARG;
     sst_ctx *ctx = new (std::nothrow) sst_ctx();
     if (!ctx) return SST_ERR_INVALID_ARG;
@@ -1969,11 +2025,15 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         // The dynamic shared-memory limit is per-FUNCTION state shared by every context of the
         // process: it is set to the device maximum, never to this context's size, so contexts with
         // different slot sizes can be used side by side.
-        if (cudaFuncSetAttribute(sst_event_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess ||
-            cudaFuncSetAttribute(sst_event_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
+        if (cudaFuncSetAttribute(sst_event_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess ||
+            cudaFuncSetAttribute(sst_event_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess ||
+            cudaFuncSetAttribute(sst_event_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess ||
+            cudaFuncSetAttribute(sst_event_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin) != cudaSuccess)
             return fail(SST_ERR_CUDA);
-        cudaFuncSetAttribute(sst_event_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        cudaFuncSetAttribute(sst_event_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(sst_event_kernel<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(sst_event_kernel<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(sst_event_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(sst_event_kernel<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         // A large FED may be worked on in K pieces (process_fed): the slot then holds the whole
         // payload while the channel table is built, and one piece's lists afterwards.  K = 1..4 is
         // tried, up to the first that keeps 20 warps resident per SM.
@@ -1991,8 +2051,8 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
             for (int wpc = kWarpsPerCta; wpc >= 1; wpc >>= 1) {
                 int ctas = 0;
                 if (static_cast<size_t>(wpc) * stride > static_cast<size_t>(smem_optin)) continue;
-                if ((K > 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<true>, 32 * wpc, static_cast<size_t>(wpc) * stride)
-                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<false>, 32 * wpc, static_cast<size_t>(wpc) * stride)) !=
+                if ((K > 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<true, false>, 32 * wpc, static_cast<size_t>(wpc) * stride)
+                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<false, false>, 32 * wpc, static_cast<size_t>(wpc) * stride)) !=
                     cudaSuccess)
                     continue;
                 if (ctas * wpc > best_warps) {
@@ -2019,8 +2079,8 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
         cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, cfg->device);
         cudaDeviceGetAttribute(&smem_reserved, cudaDevAttrReservedSharedMemoryPerBlock, cfg->device);
         size_t api_avail = 0;
-        if (ctx->pieces > 1) cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel<true>, ctx->ctas_per_sm, 32 * ctx->wpc);
-        else cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel<false>, ctx->ctas_per_sm, 32 * ctx->wpc);
+        if (ctx->pieces > 1) cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel<true, false>, ctx->ctas_per_sm, 32 * ctx->wpc);
+        else cudaOccupancyAvailableDynamicSMemPerBlock(&api_avail, sst_event_kernel<false, false>, ctx->ctas_per_sm, 32 * ctx->wpc);
         const size_t tries[2] = {smem_sm > 0 ? static_cast<size_t>(smem_sm) / ctx->ctas_per_sm - smem_reserved : 0, api_avail};
         for (size_t avail : tries) {
             avail = std::min<size_t>(avail, static_cast<size_t>(smem_optin));
@@ -2030,15 +2090,15 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
             const uint32_t keep = ctx->slot_bytes;
             set_slot(slot);
             int check = 0;
-            if ((ctx->pieces > 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel<true>, 32 * ctx->wpc, ctx->smem_bytes)
-                                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel<false>, 32 * ctx->wpc, ctx->smem_bytes)) == cudaSuccess &&
+            if ((ctx->pieces > 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel<true, false>, 32 * ctx->wpc, ctx->smem_bytes)
+                                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&check, sst_event_kernel<false, false>, 32 * ctx->wpc, ctx->smem_bytes)) == cudaSuccess &&
                 check >= ctx->ctas_per_sm)
                 break;
             set_slot(keep);  // the grown slot lost a CTA
         }
         if (ctx->pieces > 1) {
             int ctas = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<false>, 32, kWarpHdr + need_whole + kTailPad) == cudaSuccess &&
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, sst_event_kernel<false, false>, 32, kWarpHdr + need_whole + kTailPad) == cudaSuccess &&
                 ctas > 0) {
                 ctx->whole_slot = need_whole;
                 ctx->whole_warps_sm = ctas;
@@ -2610,6 +2670,23 @@ sst_status sst_destroy(sst_ctx *ctx) {
     if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
     delete ctx;
     return SST_OK;
+}
+
+sst_status sst_trace_read(sst_ctx *ctx, void *stream, uint64_t *out) {
+    if (!ctx || !out || !ctx->cfg.trace) return SST_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    std::lock_guard<std::mutex> lock(ctx->slot_mu);
+    for (auto &s : ctx->slots) {
+        if (s.stream != st || !s.mem) continue;
+        uint8_t *tr = s.mem + 256;
+        SST_CU(cudaMemcpyAsync(out, tr, SST_TRACE_WORDS * 8, cudaMemcpyDeviceToHost, st));
+        SST_CU(cudaMemsetAsync(tr, 0, SST_TRACE_WORDS * 8, st));
+        SST_CU(cudaMemsetAsync(tr + 8 * kTrStart, 0xff, 16, st));
+        SST_CU(cudaStreamSynchronize(st));
+        return SST_OK;
+    }
+    return SST_ERR_INVALID_ARG;  // nothing was launched on this stream
 }
 
 int32_t sst_last_cuda_error(const sst_ctx *ctx) { return ctx ? ctx->last_err.load() : 0; }

@@ -54,7 +54,7 @@ class Detector:
 
     def __init__(self, n_feds: int, gain, noise, bad, chan_module, device: int = 0,
                  max_raw_bytes: int = 1 << 22, max_events_in_flight: int = 8, fed_strips_hint: int = 0,
-                 move_mode: int = 0):
+                 move_mode: int = 0, trace: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise B.SSTError("no CUDA device: libsst has no CPU fallback")
@@ -63,7 +63,7 @@ class Detector:
         self.n_feds = n_feds
         self.n_strips = n_feds * B.FED_STRIPS
         self.max_raw_bytes = int(max_raw_bytes)
-        self.ctx = B.sst_create(n_feds, device, self.max_raw_bytes, max_events_in_flight, fed_strips_hint, move_mode)
+        self.ctx = B.sst_create(n_feds, device, self.max_raw_bytes, max_events_in_flight, fed_strips_hint, move_mode, trace)
         B.sst_upload_calib(self.ctx, gain, noise, bad, chan_module)
 
     def upload_geometry(self, geom):

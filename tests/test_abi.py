@@ -29,7 +29,7 @@ def test_library_builds_loads_and_exports_everything():
 def test_binding_struct_layout_matches_header():
     # sst_output: 4 pointers, 3 uint32 (+pad), 10 pointers, 5 pointers, uint32 (+pad), 3 pointers
     assert ctypes.sizeof(binding.sst_output) == 4 * 8 + 16 + 10 * 8 + 5 * 8 + 8 + 3 * 8
-    assert ctypes.sizeof(binding.sst_config) == 24
+    assert ctypes.sizeof(binding.sst_config) == 28
     assert ctypes.sizeof(binding.sst_info) == 32
     assert ctypes.sizeof(binding.sst_thresholds) == 12
 

@@ -937,6 +937,33 @@ def _random_event(rng, n_feds):
     return raw, fo, gain, noise, bad, cm
 
 
+def test_traced_context_gives_the_same_results_and_a_trace(H, oracle):
+    """sst_config.trace = 1 launches the traced instantiations of sst_event_kernel: same outputs, and
+    sst_trace_read returns the FED count, per-phase cycles and (move in the kernel) the moved FEDs."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf = 24
+    cfg, cal, evs = synth.make_config(0, n_feds=nf)
+    ev = evs[0]
+    for hint in (0, 40):  # whole FEDs; a slot too small for them (pieces or the global scratch)
+        det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=int(ev.raw.size), trace=1, fed_strips_hint=hint)
+        try:
+            st = torch.cuda.Stream()
+            d_raw, d_fo = det.upload_raw(ev.raw, ev.fed_offsets)
+            outs = det.alloc_outputs(int(ev.raw.size), int(ev.raw.size), chan_map=True, seeds=True, snr=True)
+            for _ in range(2):
+                det.run(d_raw, d_fo, (2, 3, 5), outs, stream=st)
+            t = B.sst_trace_read(det.ctx, st.cuda_stream)
+            r = oracle.run(ev.raw, ev.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            compare(H.unsigned_view(outs.numpy()), r)
+            assert t[0] == 2 * nf and all(x > 0 for x in t[1:13]), t
+            assert t[13] == (2 * nf if H.move_mode == 0 else 0)
+            assert t[20] <= t[21] <= t[22] <= t[23]
+            assert B.sst_trace_read(det.ctx, st.cuda_stream)[0] == 0  # cleared by the read
+        finally:
+            det.close()
+
+
 def test_epoch_wraps_after_4095_launches_on_a_stream(H, oracle):
     """The FED state words carry a 12-bit launch epoch (what the in-kernel move waits for); it wraps
     after 4095 launches of a stream, before which the words are cleared.  4096 launches of small
