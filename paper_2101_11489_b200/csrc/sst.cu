@@ -528,41 +528,59 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         const bool entry_prefetch = p.n_events < kSlabMinEvents;
         uint32_t run_before = 0, start_before = 0, v_before = 0;  // runs / last run start / its entry below this word
         const uint32_t last = P - 1u;                             // (P > 0 inside the loop)
-        uint32_t v_next = strip_l[min(static_cast<uint32_t>(lane), last)];
-#pragma unroll 1
-        for (uint32_t w = 0; w < nw; ++w) {
-            const uint32_t e = w * 32u + lane;
-            const bool in = e < P;
-            const uint32_t v = in ? v_next : 0u;
-            v_next = strip_l[min(e + 32u, last)];  // the next word's entries, ahead of their use
-            const uint32_t m = __ballot_sync(kFull, v != 0);
+        // two words of 32 entries per iteration, interleaved: the second word's carries follow from
+        // the first word's ballot, everything else is independent (a warp is bound by the latency of
+        // its own dependent steps, so two chains at once run nearly as fast as one)
+        uint32_t vn_a = strip_l[min(static_cast<uint32_t>(lane), last)], vn_b = strip_l[min(static_cast<uint32_t>(lane) + 32u, last)];
+        auto entry = [&](const uint32_t e, const uint32_t v, const uint32_t m, const uint32_t runs0, const uint32_t start0,
+                         const uint32_t v0, uint32_t &sid, uint32_t &mark, uint32_t &a) {
             const uint32_t below = m & le;
             const uint32_t top = 31u - __clz(below);  // (-1 when below == 0: the shuffle result is then unused)
             const uint32_t vs = __shfl_sync(kFull, v, top);
-            const uint32_t d = below ? lane - top : e - start_before;  // distance to the run's first strip
-            const uint32_t s0 = below ? vs : v_before;
-            const uint32_t sid = (s0 & 0x7fffu) - 1u + d;
-            const uint32_t r1 = run_before + __popc(below);  // 1 + index of the entry's run
+            const uint32_t d = below ? lane - top : e - start0;  // distance to the run's first strip
+            const uint32_t s0 = below ? vs : v0;
+            sid = (s0 & 0x7fffu) - 1u + d;
+            mark = d == 0 ? s0 & 0x8000u : 0u;
+            const uint32_t r1 = runs0 + __popc(below);  // 1 + index of the entry's run
             const uint32_t ch = min(sid >> 8, static_cast<uint32_t>(kChan - 1));
             uint32_t kc = 2u * ch + 2u;
             if (!regular) kc = ktab[ch];
-            const uint32_t a = rp[min(min(e, last) + 2u * r1 + kc, c.fed_size - 1u)];  // (clamped: lanes past the end)
+            a = rp[min(min(e, last) + 2u * r1 + kc, c.fed_size - 1u)];  // (clamped: lanes past the end)
+        };
+#pragma unroll 1
+        for (uint32_t w = 0; w < nw; w += 2u) {
+            const uint32_t e_a = w * 32u + lane, e_b = e_a + 32u;
+            const bool in_a = e_a < P, in_b = e_b < P;
+            const uint32_t v_a = in_a ? vn_a : 0u, v_b = in_b ? vn_b : 0u;
+            vn_a = strip_l[min(e_a + 64u, last)];  // the next iteration's entries, ahead of their use
+            vn_b = strip_l[min(e_b + 64u, last)];
+            const uint32_t m_a = __ballot_sync(kFull, v_a != 0), m_b = __ballot_sync(kFull, v_b != 0);
+            // carries into the second word
+            const uint32_t mt_a = 31u - __clz(m_a), mt_b = 31u - __clz(m_b);
+            const uint32_t va_top = __shfl_sync(kFull, v_a, mt_a), vb_top = __shfl_sync(kFull, v_b, mt_b);
+            const uint32_t runs_b = run_before + __popc(m_a);
+            const uint32_t start_b = m_a ? w * 32u + mt_a : start_before, v0_b = m_a ? va_top : v_before;
+            uint32_t sid_a, sid_b, mark_a, mark_b, a_a, a_b;
+            entry(e_a, v_a, m_a, run_before, start_before, v_before, sid_a, mark_a, a_a);
+            entry(e_b, v_b, m_b, runs_b, start_b, v0_b, sid_b, mark_b, a_b);
             // a launch of few events cannot amortise a slab prefetch: the entry's calibration line is
             // requested now and arrives while the dense SoA is assembled
             if (entry_prefetch) {  // (uniform)
-                if (in) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(cal + sid));
+                if (in_a) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(cal + sid_a));
+                if (in_b) asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(cal + sid_b));
             }
-            __syncwarp();
-            if (in) {
-                adc_l[e] = static_cast<uint8_t>(a);
-                strip_l[e] = static_cast<uint16_t>(d == 0 ? sid | (s0 & 0x8000u) : sid);
+            __syncwarp();  // all reads of both words before their writes
+            if (in_a) {
+                adc_l[e_a] = static_cast<uint8_t>(a_a);
+                strip_l[e_a] = static_cast<uint16_t>(sid_a | mark_a);
             }
-            if (m) {
-                const uint32_t mt = 31u - __clz(m);
-                v_before = __shfl_sync(kFull, v, mt);
-                start_before = w * 32u + mt;
+            if (in_b) {
+                adc_l[e_b] = static_cast<uint8_t>(a_b);
+                strip_l[e_b] = static_cast<uint16_t>(sid_b | mark_b);
             }
-            run_before += __popc(m);
+            run_before = runs_b + __popc(m_b);
+            start_before = m_b ? (w + 1u) * 32u + mt_b : start_b;
+            v_before = m_b ? vb_top : v0_b;
         }
     }
     __syncwarp();  // lists complete; the payload is dead from here on
