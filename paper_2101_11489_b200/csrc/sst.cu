@@ -75,6 +75,7 @@ constexpr uint32_t kHostChunk = 4;       // events per launch of the HOST entry 
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxFeds = 4096;
 constexpr uint32_t kTabBytes = ((kChan + 1) * 4 + kChan * 2 + 15) & ~15;  // channel table of the FED, at the slot's end
+constexpr uint32_t kFrameBytes = (3 * kChan + 16) * 4;  // what a FED in pieces keeps in its slot from piece to piece
 constexpr uint32_t kWarpHdr = 16;        // mbarrier in front of a warp's slot
 constexpr uint32_t kTailPad = 16;        // readable bytes behind the slot
 constexpr uint32_t kSlabAhead = 2;       // FEDs between a calibration slab prefetch and its use
@@ -1021,8 +1022,8 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
         c.adc_base = adc_base + fed_adc;
         c.seed_base = seed_base + fed_seed;
     }
-    if (!last) return true;  // (uniform) more pieces of this FED follow
     if (kTrace) trace_stamp(p, c, lane, 12);
+    if (!last) return true;  // (uniform) more pieces of this FED follow
     // publish: the FED's counts, tagged with the launch's epoch, behind everything staged above
     // (release: the in-kernel move of another warp may read the staging as soon as it sees the word,
     // and it reads it with TMA bulk copies: the writers order their generic-proxy stores before
@@ -1192,11 +1193,14 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
 
     // fast path: window / cluster list, strip ids and masks fit behind the ADC list
     const bool want_dense = o.strip_adc != nullptr;
-    auto fits = [&](const uint32_t bytes, const uint32_t strips) {
+    auto fits_in = [&](const uint32_t bytes, const uint32_t strips, const uint32_t room) {
         const uint32_t A = (bytes + 15u) & ~15u, P16 = (strips + 15u) & ~15u;
         const uint32_t S0 = fast_strip_base(A, P16, want_dense);
-        return ((S0 + 2u * strips + 15u) & ~15u) + 16u * (((strips + 31u) >> 5) + 2u) + kTabBytes <= p.slot_bytes;
+        return ((S0 + 2u * strips + 15u) & ~15u) + 16u * (((strips + 31u) >> 5) + 2u) + kTabBytes <= room;
     };
+    auto fits = [&](const uint32_t bytes, const uint32_t strips) { return fits_in(bytes, strips, p.slot_bytes); };
+    // (a piece leaves room for the frame that carries the FED from piece to piece)
+    auto fits_piece = [&](const uint32_t bytes, const uint32_t strips) { return fits_in(bytes, strips, p.slot_bytes - kFrameBytes); };
     // ---------------------------------------------------------------- a FED in pieces
     // When the lists of the whole FED do not fit the slot the warp works through it in up to seven
     // pieces, channel ranges that start where a module starts (nothing links across), each as
@@ -1218,14 +1222,14 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
             // (16-byte granules of the payload; an overrun FED is fetched to its end)
             const uint32_t g_lo = (at(c.off, lo, c.fed_size + 2u) - 2u) & ~15u, e_lo = at(exs, lo, tot) & 0xffffu;
             uint32_t best = 0;
-            if (fits(c.fed_size - g_lo, c.P - e_lo)) {
+            if (fits_piece(c.fed_size - g_lo, c.P - e_lo)) {
                 best = kChan;
             } else {
 #pragma unroll
                 for (int k = 2; k >= 0; --k) {
                     const uint32_t ch = lane + 32 * k;
                     const uint32_t hi = c.overrun ? c.fed_size : (c.off[k] - 2u + 15u) & ~15u;
-                    const bool ok = ch > lo && ((c.opens >> k) & 1u) && hi >= g_lo && fits(hi - g_lo, (exs[k] & 0xffffu) - e_lo);
+                    const bool ok = ch > lo && ((c.opens >> k) & 1u) && hi >= g_lo && fits_piece(hi - g_lo, (exs[k] & 0xffffu) - e_lo);
                     const uint32_t m = __ballot_sync(kFull, ok);
                     if (!best && m) best = 32u * k + 31u - __clz(m);
                 }
@@ -1241,39 +1245,99 @@ __device__ __forceinline__ bool process_fed(const KParams &p, unsigned long long
     }
     if (slow) return fed_lists<false, false, kTrace>(p, slot, rp, c, lane, next_ticket);
     if (!kPieces || n_pieces == 0) return fed_lists<true, false, kTrace>(p, slot, slot, c, lane, next_ticket);
-    FedCtx pc = c;  // the piece's view of the FED (c stays as it is: the whole FED's, in registers)
-    for (uint32_t i = 0, b0 = 0; i < n_pieces; ++i) {
-        const uint32_t b1 = static_cast<uint32_t>(plan >> (8u * i)) & 0xffu;
-        const uint32_t g_lo = (at(c.off, b0, c.fed_size + 2u) - 2u) & ~15u;
-        const uint32_t g_hi = c.overrun || b1 >= static_cast<uint32_t>(kChan) ? c.fed_size : (at(c.off, b1, c.fed_size + 2u) - 2u + 15u) & ~15u;
-        const uint32_t ex0 = at(exs, b0, tot), ex1 = at(exs, b1, tot);
-        __syncwarp();  // every lane is done with the previous piece
-        if (i > 0 && g_hi > g_lo) {
-            if (lane == 0) {
-                fence_proxy_async();
-                mbar_expect_tx(mbar, g_hi - g_lo);
-                bulk_g2s(slot, E.raw + c.fed_start + g_lo, g_hi - g_lo, mbar, policy_evict_first());
-            }
-            mbar_wait(mbar, mbar_phase);
-            mbar_phase ^= 1u;
-        }
+    // What the pieces need of the FED goes into a frame at the top of the slot (below the channel
+    // table; piece 0 stays clear of it, the rest of the payload up there is fetched again anyway)
+    // and comes back at the start of every piece: nothing of it stays in registers across a piece
+    // (with ~150 bytes of spills per thread and no L1 to speak of beside 229 KB of shared memory,
+    // every spilled value would come back from L2).
+    uint32_t *const fr = reinterpret_cast<uint32_t *>(slot + p.slot_bytes - kTabBytes - kFrameBytes);
+    uint32_t *const fs = fr + 3 * kChan;  // scalars
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const uint32_t ch = lane + 32 * k;
+        fr[ch] = c.off[k];
+        fr[kChan + ch] = c.len[k];
+        fr[2 * kChan + ch] = exs[k] | (((c.opens >> k) & 1u) << 31);  // (strips 16 bits, runs 14 bits)
+    }
+    if (lane == 0) {
+        fs[0] = tot;
+        fs[1] = c.fed_size;
+        fs[2] = static_cast<uint32_t>(plan);
+        fs[3] = static_cast<uint32_t>(plan >> 32);
+        fs[4] = n_pieces;
+        fs[5] = c.overrun;
+        fs[6] = c.n_malformed;
+        fs[7] = c.fed_start;
+        fs[8] = fs[9] = fs[10] = fs[11] = fs[12] = 0;  // clusters, ADC bytes, seeds, entries, non-zero entries so far
+        fs[13] = c.fo0;
+        fs[14] = static_cast<uint32_t>(c.t_prev);  // (tracing)
+        fs[15] = static_cast<uint32_t>(static_cast<unsigned long long>(c.t_prev) >> 32);
+    }
+    for (uint32_t i = 0;; ++i) {
+        __syncwarp();  // every lane is done with the previous piece; the frame is written
+        if (i >= fs[4]) break;
+        const unsigned long long pl = fs[2] | (static_cast<unsigned long long>(fs[3]) << 32);
+        const uint32_t b0 = i ? static_cast<uint32_t>(pl >> (8u * (i - 1u))) & 0xffu : 0u;
+        const uint32_t b1 = static_cast<uint32_t>(pl >> (8u * i)) & 0xffu;
+        const uint32_t fed_size = fs[1], over = fs[5];
+        const uint32_t off_b0 = b0 < static_cast<uint32_t>(kChan) ? fr[b0] : fed_size + 2u;
+        const uint32_t off_b1 = b1 < static_cast<uint32_t>(kChan) ? fr[b1] : fed_size + 2u;
+        const uint32_t ex0 = (b0 < static_cast<uint32_t>(kChan) ? fr[2 * kChan + b0] : fs[0]) & 0x7fffffffu;
+        const uint32_t ex1 = (b1 < static_cast<uint32_t>(kChan) ? fr[2 * kChan + b1] : fs[0]) & 0x7fffffffu;
+        const uint32_t g_lo = (off_b0 - 2u) & ~15u;
+        const uint32_t g_hi = over || b1 >= static_cast<uint32_t>(kChan) ? fed_size : (off_b1 - 2u + 15u) & ~15u;
+        FedCtx pc;
+        pc.ev = ticket - f * p.n_events;
+        pc.f = f;
+        pc.fo0 = fs[13];
+        pc.fed_start = fs[7];
+        pc.overrun = over;
+        pc.n_malformed = fs[6];
+        pc.opens = 0;
+        pc.t_prev = kTrace ? static_cast<long long>(fs[14] | (static_cast<unsigned long long>(fs[15]) << 32)) : 0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             const uint32_t ch = lane + 32 * k;
             const bool in = ch >= b0 && ch < b1;
-            pc.off[k] = in ? c.off[k] - g_lo : 0u;
-            pc.len[k] = in ? c.len[k] : 0u;
-            pc.ebase[k] = in ? (exs[k] & 0xffffu) - (ex0 & 0xffffu) : 0u;
-            if (in) ktab[ch] = pc.off[k] - pc.ebase[k] - 2u * ((exs[k] >> 16) - (ex0 >> 16));
+            const uint32_t xk = fr[2 * kChan + ch];
+            pc.off[k] = in ? fr[ch] - g_lo : 0u;
+            pc.len[k] = in ? fr[kChan + ch] : 0u;
+            pc.ebase[k] = in ? (xk & 0xffffu) - (ex0 & 0xffffu) : 0u;
+            pc.opens |= (xk >> 31) << k;
+            if (in) ktab[ch] = pc.off[k] - pc.ebase[k] - 2u * (((xk >> 16) & 0x3fffu) - (ex0 >> 16));
         }
         pc.fed_size = g_hi - g_lo;
         pc.P = (ex1 & 0xffffu) - (ex0 & 0xffffu);
         pc.ch_lo = b0;
         pc.ch_hi = b1;
-        pc.last = i + 1u == n_pieces;
+        pc.last = i + 1u == fs[4];
+        pc.cl_base = fs[8];
+        pc.adc_base = fs[9];
+        pc.seed_base = fs[10];
+        pc.ent_base = fs[11];
+        pc.nz_base = fs[12];
+        if (i > 0 && g_hi > g_lo) {
+            __syncwarp();
+            if (lane == 0) {
+                fence_proxy_async();
+                mbar_expect_tx(mbar, g_hi - g_lo);
+                bulk_g2s(slot, p.ev[pc.ev].raw + pc.fed_start + g_lo, g_hi - g_lo, mbar, policy_evict_first());
+            }
+            mbar_wait(mbar, mbar_phase);
+            mbar_phase ^= 1u;
+        }
         __syncwarp();
         if (!fed_lists<true, true, kTrace>(p, slot, slot, pc, lane, next_ticket)) return false;
-        b0 = b1;
+        if (lane == 0) {
+            fs[8] = pc.cl_base;
+            fs[9] = pc.adc_base;
+            fs[10] = pc.seed_base;
+            fs[11] = pc.ent_base;
+            fs[12] = pc.nz_base;
+            fs[14] = static_cast<uint32_t>(pc.t_prev);
+            fs[15] = static_cast<uint32_t>(static_cast<unsigned long long>(pc.t_prev) >> 32);
+        }
     }
     return true;
 }
@@ -2062,7 +2126,7 @@ sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
             const uint32_t rk = K > 1 ? ((r_hint / K + 256u + 15u) & ~15u) : r_hint;             // its payload bytes
             const uint32_t p16 = (pk + 15u) & ~15u;
             const uint32_t gap = rk >= p16 + 2048u ? 0u : p16 + 2048u - rk;
-            uint32_t need_k = std::max(rk + gap + 2u * pk + 16u * (pk / 32u + 3u), K > 1 ? r_hint : 0u) + kTabBytes + 32u;
+            uint32_t need_k = std::max(rk + gap + 2u * pk + 16u * (pk / 32u + 3u) + (K > 1 ? kFrameBytes : 0u), K > 1 ? r_hint : 0u) + kTabBytes + 32u;
             need_k = std::min(std::max((need_k + 15u) & ~15u, 4096u), (static_cast<uint32_t>(smem_optin) - kWarpHdr - kTailPad) & ~15u);
             const uint32_t stride = kWarpHdr + need_k + kTailPad;
             if (K == 1) need_whole = need_k;
