@@ -333,8 +333,23 @@ def run_sweep(args):
                     b.record(st)
                 torch.cuda.synchronize()
             us = float(np.median([a.elapsed_time(b) for a, b in evs_t])) * 1e3
+            # the same call captured in a CUDA graph and replayed
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=st):
+                det.run(d_raw, d_fo, thr, outs, stream=st)
+            for rep in range(2):
+                with torch.cuda.stream(st):
+                    torch.cuda._sleep(2_000_000)
+                    for a, b in evs_t:
+                        a.record(st)
+                        graph.replay()
+                        b.record(st)
+                torch.cuda.synchronize()
+            us_graph = float(np.median([a.elapsed_time(b) for a, b in evs_t])) * 1e3
+            del graph
             g = outs.numpy()
             out["single_event"].append({"config": cid, "n_feds": nf, "thresholds": list(thr), "latency_us": us,
+                                        "latency_us_graph_replay": us_graph,
                                         "present_strips": int(ev.meta["present"]), "clusters": int(g["n_clusters"]),
                                         "raw_bytes": int(ev.raw.size), "info": det.info()})
         del outs

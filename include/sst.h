@@ -21,6 +21,10 @@
  *     sst_output.dev_status once the stream has completed.
  *   - After sst_upload_calib returns the context is read-only: sst_unpack_cluster may be called
  *     concurrently from several host threads on different streams.
+ *   - CUDA graphs: once a stream has seen one plain call (which takes the stream's scratch from the
+ *     pool), sst_unpack_cluster / sst_unpack_cluster_batch on that stream can be captured
+ *     (cudaStreamBeginCapture) and the graph replayed: a launch is nothing but its parameters, the
+ *     kernel keeps its work counter and the epoch of its FED words in device memory itself.
  */
 #ifndef SST_H
 #define SST_H

@@ -108,10 +108,10 @@ struct KParams {
     uint16_t *s_csid;          // staged list of a FED: strip ids and raw ADCs, for the compact SoA
     uint8_t *s_cadc;
     unsigned long long *fed_state;  // [kMaxEv][n_feds]
-    unsigned long long *ticket;     // monotone counter; this launch owns [ticket_base, + tickets + warps)
+    unsigned long long *ticket;     // the stream's launch header: [0] ticket counter (0 when a launch starts: the last warp of
+                                    // a launch to finish resets it), [1] warps finished, [2] launches so far modulo 4095
     unsigned long long *trace;      // 32 words of the stream's scratch (sst_trace_read), used by the traced kernels
-    unsigned long long ticket_base;
-    uint32_t epoch;       // tag of this launch's FED aggregates
+    uint32_t state_words;  // words of fed_state (all events the scratch holds): cleared when the epoch starts over
     uint32_t move_chunk;  // clusters per bulk copy of the in-kernel move (from the slot size)
     uint32_t fused_move;  // 1: sst_event_kernel moves the staged clusters itself once its FED tickets are used up
     // global scratch of the slow path, one slice set per event
@@ -132,6 +132,15 @@ struct KParams {
     uint32_t max_raw_bytes, n_feds, n_events, slot_bytes;
     EventDesc ev[kMaxEv];
 };
+
+// The tag of this launch's FED aggregates, 1..4095: the stream's launch count (header word 2, kept
+// by the kernel itself -- see the end of sst_event_kernel -- so that a launch is nothing but its
+// parameters and can be captured in a CUDA graph and replayed) + 1.  Constant while a launch runs.
+__device__ __forceinline__ uint32_t launch_epoch(const KParams &p) {
+    return static_cast<uint32_t>(__ldg(p.ticket + 2)) + 1u;
+}
+// (every warp keeps it in the eight free bytes between its mbarrier and its slot)
+__device__ __forceinline__ uint32_t warp_epoch(const uint8_t *slot) { return *reinterpret_cast<const uint32_t *>(slot - 8); }
 
 // ------------------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_addr(const void *p) {
@@ -942,7 +951,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     const size_t sb = static_cast<size_t>(c.ev) * p.s_cl_stride + c.fed_start / 2u + f + cl_base;
     const size_t ab = static_cast<size_t>(c.ev) * p.g_ents + c.fed_start;
     // next FED of this warp: the ticket arrives while the staging runs
-    if (lane == 0 && last) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
+    if (lane == 0 && last) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull));
     {
         // cluster records: lane per cluster, consecutive lanes write consecutive records
         const uint2 *cinfo = p.chan_info + static_cast<size_t>(f) * kChan;
@@ -1031,7 +1040,7 @@ __device__ __forceinline__ bool fed_lists(const KParams &p, uint8_t *slot, const
     if (p.fused_move) asm volatile("fence.proxy.async.global;" ::: "memory");
     __syncwarp();
     if (lane == 0) {
-        const unsigned long long v = (static_cast<unsigned long long>(p.epoch) << kShEpoch) |
+        const unsigned long long v = (static_cast<unsigned long long>(warp_epoch(slot)) << kShEpoch) |
                                      (static_cast<unsigned long long>(c.overrun) << kShOver) |
                                      (static_cast<unsigned long long>(c.n_malformed) << kShMalf) |
                                      (static_cast<unsigned long long>(seed_base + fed_seed) << kShSeed) |
@@ -1368,16 +1377,17 @@ __device__ __forceinline__ void move_fed(const KParams &p, unsigned long long *m
     const sst_output &o = E.out;
     const unsigned long long *const st = p.fed_state + static_cast<size_t>(ev) * p.n_feds;
     const uint32_t fed_start = __ldg(E.fed_offsets + f);
+    const uint32_t epoch = warp_epoch(slot);
     // ---- round trip 1: state words.  clusters | ADC bytes << 32 ; seeds | malformed << 32 | overrun << 52
     unsigned long long own, accA, accB;
     for (uint32_t tries = 0;; ++tries) {
         own = ld_state_acquire(st + f);
         // (after a miss: wait for the FED's own word alone -- in FED-major order it is the last to appear)
-        while (tries && static_cast<uint32_t>(own >> kShEpoch) != p.epoch) {
+        while (tries && static_cast<uint32_t>(own >> kShEpoch) != epoch) {
             __nanosleep(400);
             own = ld_state_acquire(st + f);
         }
-        bool ok = static_cast<uint32_t>(own >> kShEpoch) == p.epoch;
+        bool ok = static_cast<uint32_t>(own >> kShEpoch) == epoch;
         accA = accB = 0;
         constexpr int kW = 14;  // words per lane in flight (448 FEDs per pass)
 #pragma unroll 1
@@ -1386,12 +1396,12 @@ __device__ __forceinline__ void move_fed(const KParams &p, unsigned long long *m
 #pragma unroll
             for (int k = 0; k < kW; ++k) {
                 const uint32_t j = j0 + 32 * k;
-                v[k] = static_cast<unsigned long long>(p.epoch) << kShEpoch;
+                v[k] = static_cast<unsigned long long>(epoch) << kShEpoch;
                 if (j < f) v[k] = ld_state(st + j);
             }
 #pragma unroll
             for (int k = 0; k < kW; ++k) {
-                ok = ok && static_cast<uint32_t>(v[k] >> kShEpoch) == p.epoch;
+                ok = ok && static_cast<uint32_t>(v[k] >> kShEpoch) == epoch;
                 accA += (v[k] & 0x3fffull) | (((v[k] >> kShAdc) & 0x7fffull) << 32);
                 accB += ((v[k] >> kShSeed) & 0x7fffull) | (((v[k] >> kShMalf) & 0x7full) << 32) | (((v[k] >> kShOver) & 1ull) << 52);
             }
@@ -1528,7 +1538,7 @@ __device__ __forceinline__ void move_phase(const KParams &p, unsigned long long 
     while (ticket < 2u * total) {
         const uint32_t t = ticket - total;
         uint32_t next_ticket = 0;
-        if (lane == 0) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
+        if (lane == 0) next_ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull));
         const uint32_t f = t / p.n_events;
         const long long t0 = kTrace ? clock64() : 0;
         move_fed(p, mbar, slot, mbar_phase, t - f * p.n_events, f, lane);
@@ -1554,6 +1564,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
     if (lane == 0) {
         mbar_init(mbar, 1);
         fence_proxy_async();
+        *reinterpret_cast<uint32_t *>(mine + 8) = launch_epoch(p);
     }
     __syncwarp();
     const uint32_t total = p.n_events * p.n_feds;
@@ -1565,7 +1576,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
     if (kTrace && lane == 0) atomicMin(p.trace + kTrStart, wall_ns());
     uint32_t mbar_phase = 0;
     uint32_t ticket = 0;
-    if (lane == 0) ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull) - p.ticket_base);
+    if (lane == 0) ticket = static_cast<uint32_t>(atomicAdd(p.ticket, 1ull));
     ticket = __shfl_sync(kFull, ticket, 0);
     while (ticket < total) {
         uint32_t next_ticket = 0;
@@ -1586,6 +1597,25 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
     }
     if (p.fused_move) move_phase<kTrace>(p, mbar, slot, mbar_phase, ticket, total, lane);
     if (kTrace && lane == 0) atomicMax(p.trace + kTrEnd, wall_ns());
+    // The last warp of the launch to get here leaves the stream's header ready for the next launch:
+    // ticket counter and warp count at zero, one launch more -- and when the epoch starts over with
+    // that, every FED state word cleared, so that a word of this round of epochs is never taken for
+    // one of the next.  (The launch's parameters hold nothing that changes from launch to launch.)
+    uint32_t left = 0;
+    if (lane == 0) left = static_cast<uint32_t>(atomicAdd(p.ticket + 1, 1ull)) + 1u == gridDim.x * (blockDim.x >> 5);
+    if (__shfl_sync(kFull, left, 0)) {
+        const unsigned long long n = p.ticket[2] + 1ull == kEpochs ? 0ull : p.ticket[2] + 1ull;
+        if (n == 0) {
+#pragma unroll 1
+            for (uint32_t i = lane; i < p.state_words; i += 32) p.fed_state[i] = 0ull;
+        }
+        __syncwarp();
+        if (lane == 0) {
+            p.ticket[0] = 0ull;
+            p.ticket[1] = 0ull;
+            p.ticket[2] = n;
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------ a7, second half
@@ -1804,10 +1834,10 @@ struct sst_ctx {
     uint32_t slot_bytes = 0;   // shared-memory slot of one warp (one FED)
     uint32_t warp_stride = 0;  // mbarrier + slot + tail pad
     uint32_t smem_bytes = 0;   // kWarpsPerCta * warp_stride
-    // per-stream scratch (ticket counter, FED states, slow-path lists), taken from the pool on a
-    // stream's first launch and kept: stream order makes reuse safe, the epoch and the running
-    // ticket base make clearing unnecessary
-    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t cap_events; unsigned long long ticket_base; uint32_t epoch; };
+    // per-stream scratch (launch header, FED states, slow-path lists), taken from the pool on a
+    // stream's first launch and kept: stream order makes reuse safe, and every launch leaves the
+    // header ready for the next
+    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t cap_events; };
     // cross-stream dependencies of the batched entry point: one event per stream, made on first use
     struct StreamEvent { cudaStream_t stream; cudaEvent_t ev; };
     std::vector<StreamEvent> stream_events;
@@ -1936,7 +1966,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     for (auto &s : ctx->slots)
         if (s.stream == st) sl = &s;
     if (!sl) {
-        ctx->slots.push_back({st, nullptr, 0u, 0ull, 0u});
+        ctx->slots.push_back({st, nullptr, 0u});
         sl = &ctx->slots.back();
     }
     if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 16, 32 or kMaxEv events
@@ -1954,8 +1984,6 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         cudaMemsetAsync(mem + Ln.o_ticket + 256 + 8 * kTrStart, 0xff, 16, st);  // trace: the two minima
         sl->mem = mem;
         sl->cap_events = want;
-        sl->ticket_base = 0;
-        sl->epoch = 0;
     }
     uint8_t *const blk = sl->mem;
     const ScratchLayout L = scratch_layout(ctx, sl->cap_events);
@@ -1970,7 +1998,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     kp.s_csid = reinterpret_cast<uint16_t *>(blk + L.o_csid);
     kp.s_cadc = blk + L.o_cadc;
     kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
-    kp.ticket_base = sl->ticket_base;
+    kp.state_words = static_cast<uint32_t>(sl->cap_events) * nf;
     kp.trace = reinterpret_cast<unsigned long long *>(blk + L.o_ticket + 256);
     kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
     kp.g_rec = reinterpret_cast<uint32_t *>(blk + L.o_rec);
@@ -2006,22 +2034,12 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     const bool fused = !packed && !extras && ctx->cfg.move_mode == 0;
     kp.fused_move = fused ? 1u : 0u;
     kp.move_chunk = std::min(1024u, ((slot_bytes - (kMoveAdc + 32u) - 32u) / 20u) & ~31u);  // (slot_bytes >= 4096)
-    // the epoch tags this launch's FED aggregates; before a tag is used again the words are cleared
-    if (sl->epoch == kEpochs) {
-        SST_CU(cudaMemsetAsync(blk + L.o_state, 0, L.state_bytes, st));
-        sl->epoch = 0;
-    }
-    kp.epoch = ++sl->epoch;
     const bool trace = ctx->cfg.trace != 0;
     if (pieces && trace) sst_event_kernel<true, true><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
     else if (pieces) sst_event_kernel<true, false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
     else if (trace) sst_event_kernel<false, true><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
     else sst_event_kernel<false, false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
     cudaError_t err = cudaGetLastError();
-    if (err == cudaSuccess) {
-        // every warp draws one ticket too many before it stops
-        sl->ticket_base += static_cast<unsigned long long>(total) * (fused ? 2u : 1u) + grid * wpc;
-    }
     if (err == cudaSuccess && !fused) {
         // the move is launched as a programmatic dependent of the event kernel: its CTAs are set up
         // while that kernel's last warps finish (the kernel itself waits for its completion)
@@ -2041,12 +2059,10 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         if (err == cudaSuccess) err = cudaGetLastError();
     }
     if (err != cudaSuccess) {
-        // a launch that did not happen must not leave the stream's ticket counter and the host's
-        // copy of it apart: start the stream's scratch over (stream-ordered, like everything else)
+        // (the header of a launch that did not happen is as the launch before left it; clearing the
+        // ticket counter and the warp count again costs nothing)
         cu_ok(ctx, err);
-        cudaMemsetAsync(blk, 0, L.o_rec, st);
-        sl->ticket_base = 0;
-        sl->epoch = 0;
+        cudaMemsetAsync(blk, 0, 16, st);  // (ticket counter and warp count)
         return SST_ERR_CUDA;
     }
     return SST_OK;

@@ -964,6 +964,48 @@ def test_traced_context_gives_the_same_results_and_a_trace(H, oracle):
             det.close()
 
 
+def test_launch_captured_in_a_cuda_graph_and_replayed(H, oracle):
+    """A launch is nothing but its parameters (the kernel keeps the ticket counter and the epoch
+    itself): sst_unpack_cluster_batch of three events is captured in a CUDA graph after one plain
+    call on the stream (which takes the stream's scratch from the pool) and replayed five times, with
+    other inputs copied into the same device buffers before the last replay."""
+    import torch
+    from paper_2101_11489_b200 import binding as B
+    nf = 9
+    cfg, cal, evs = synth.make_config(0, n_feds=nf, event_seeds=[1, 2, 3, 4, 5, 6])
+    mrb = (max(int(e.raw.size) for e in evs) + 4095) // 4096 * 4096
+    det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
+    try:
+        st = torch.cuda.Stream()
+        d_in = [det.upload_raw(e.raw, e.fed_offsets) for e in evs[:3]]
+        outs = [det.alloc_outputs(mrb // 2 + 1, mrb, seeds=True, chan_map=True, snr=True, cap_seeds=mrb) for _ in range(3)]
+        batch = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs], [st.cuda_stream])
+        with torch.cuda.stream(st):
+            B.sst_unpack_cluster_batch(det.ctx, batch)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            B.sst_unpack_cluster_batch(det.ctx, batch)
+        for _ in range(4):
+            g.replay()
+        torch.cuda.synchronize()
+        for e, o in zip(evs[:3], outs):
+            r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            compare(H.unsigned_view(o.numpy()), r)
+        for d, e in zip(d_in, evs[3:]):  # other events through the same graph
+            fresh = det.upload_raw(e.raw, e.fed_offsets)
+            d[0].copy_(fresh[0])
+            d[1].copy_(fresh[1])
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        for e, o in zip(evs[3:], outs):
+            r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            compare(H.unsigned_view(o.numpy()), r)
+    finally:
+        det.close()
+
+
 def test_epoch_wraps_after_4095_launches_on_a_stream(H, oracle):
     """The FED state words carry a 12-bit launch epoch (what the in-kernel move waits for); it wraps
     after 4095 launches of a stream, before which the words are cleared.  4096 launches of small
