@@ -46,8 +46,10 @@ typedef enum {
     SST_ERR_INVALID_ARG = 1, /* NULL pointer, n_feds == 0, threshold not finite or <= 0, ... */
     SST_ERR_CUDA = 2,        /* a CUDA call failed; sst_last_cuda_error() returns its code   */
     SST_ERR_NO_CALIB = 3,    /* sst_unpack_cluster before sst_upload_calib                   */
-    SST_ERR_BAD_CALIB = 4    /* gain/noise not finite or <= 0 at a non-bad strip; module map
+    SST_ERR_BAD_CALIB = 4,   /* gain/noise not finite or <= 0 at a non-bad strip; module map
                                 decreasing, or a module crossing a FED boundary             */
+    SST_ERR_TOO_LARGE = 5    /* sst_unpack_cluster_noalloc: the context's one-event scratch is larger
+                                than SST_NOALLOC_SCRATCH_BYTES; nothing was enqueued        */
 } sst_status;
 
 typedef struct {
@@ -200,6 +202,41 @@ sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *
 sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
                                     const uint32_t *const *fed_offsets, const sst_thresholds *thr,
                                     const sst_output *outs, void *const *streams, uint32_t n_streams);
+
+/* One event WITHOUT any allocation at call time: same arguments, same kernels and bit-for-bit the
+ * same results as sst_unpack_cluster, but the scratch the kernels need between their
+ * phases (work counter, per-FED totals, staged clusters, slow-path lists) is a fixed array compiled
+ * into the library instead of a block taken from the context's pool on the stream's first event.
+ *
+ * Who needs it: code that must not reach the CUDA allocator once it is running.  Trigger and
+ * data-acquisition loops fix their device-memory budget at start-up and cannot afford an allocation
+ * that may stall the device, fail half-way through a run or grow the process's footprint; so do hosts
+ * that have handed all device memory to an allocator of their own and plug-ins that run where the
+ * embedding framework forbids allocation calls.  sst_unpack_cluster's first event on a new stream
+ * (and any larger batch later) calls cudaMallocFromPoolAsync; this entry point never calls cudaMalloc,
+ * cudaFree, their Async/pool forms or any library routine that allocates -- only cudaSetDevice, one
+ * cudaMemsetAsync and the kernel launches.  raw, fed_offsets and every array of `out` are still the
+ * caller's DEVICE buffers; the context (sst_create, sst_upload_calib: both allocate) is set up before.
+ *
+ * The price and the limit:
+ *   - The array is SST_NOALLOC_SCRATCH_BYTES (32 MiB) of device memory that every GPU on which the
+ *     library's kernels are loaded holds until the process exits, whether or not this call is used.
+ *   - A context fits when the scratch of ONE event does: about 26 bytes per byte of
+ *     cfg.max_raw_bytes plus 200 bytes per FED, i.e. a 440-FED detector with max_raw_bytes up to
+ *     ~1.3 MB (one full-detector event of BASELINE.json config 1).  A larger context is refused with
+ *     SST_ERR_TOO_LARGE before anything is enqueued.  One event per call; no batch form.
+ *   - There is ONE array per GPU, shared by every context, stream and host thread of the process, and
+ *     it keeps whatever the last call left in it.  Each call therefore first clears, on `stream`, the
+ *     part that has to start at zero (work counter and per-FED words).  Two calls whose GPU work can
+ *     overlap -- different streams, different contexts, different host threads -- RACE on it and give
+ *     wrong results: keep all calls of a GPU on one stream, or order them with events.  The other
+ *     entry points use pool scratch and may run beside it.
+ *   - The FIRST call on each GPU looks up the array's device address (cudaGetSymbolAddress, with that
+ *     GPU current) and keeps it; make that first call during set-up, before any stream capture begins.
+ *   - A context created with trace = 1 is accepted but this call is never traced. */
+#define SST_NOALLOC_SCRATCH_BYTES (32u << 20)
+sst_status sst_unpack_cluster_noalloc(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
+                                      const sst_thresholds *thr, const sst_output *out, void *stream);
 
 /* The same event with HOST buffers: raw[raw_bytes] and fed_offsets[n_feds+1] are copied to
  * pooled device buffers on `stream`, the event is processed, and dev_status, n_clusters and the

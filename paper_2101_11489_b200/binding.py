@@ -17,9 +17,11 @@ N_CHAN, N_STRIP, FED_STRIPS = 96, 256, 96 * 256
 ST_WORDS = 8
 ST_FLAGS, ST_N_MALFORMED, ST_N_CLUSTERS, ST_N_ADC, ST_N_OVERRUN, ST_N_SEEDS, ST_N_PRESENT = range(7)
 FLAG_CLUSTER_CAP, FLAG_ADC_CAP, FLAG_MALFORMED, FLAG_OVERRUN, FLAG_COMPACT_CAP = 1, 2, 4, 8, 16
-SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB = range(5)
+SST_OK, SST_ERR_INVALID_ARG, SST_ERR_CUDA, SST_ERR_NO_CALIB, SST_ERR_BAD_CALIB, SST_ERR_TOO_LARGE = range(6)
+NOALLOC_SCRATCH_BYTES = 32 << 20
 
-EXPORTS = ["sst_create", "sst_upload_calib", "sst_upload_geometry", "sst_unpack_cluster", "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
+EXPORTS = ["sst_create", "sst_upload_calib", "sst_upload_geometry", "sst_unpack_cluster", "sst_unpack_cluster_noalloc",
+           "sst_unpack_cluster_batch", "sst_unpack_cluster_host",
            "sst_unpack_cluster_host_batch", "sst_unpack_cluster_host_packed",
            "sst_event_alloc", "sst_event_free", "sst_event_upload", "sst_event_download", "sst_destroy", "sst_last_cuda_error",
            "sst_status_string", "sst_get_info", "sst_trace_read"]
@@ -74,6 +76,7 @@ def load():
     L.sst_upload_calib.argtypes = [vp, vp, vp, vp, vp]
     L.sst_upload_geometry.argtypes = [vp, vp, C.c_uint32]
     L.sst_unpack_cluster.argtypes = [vp, vp, vp, C.POINTER(sst_thresholds), C.POINTER(sst_output), vp]
+    L.sst_unpack_cluster_noalloc.argtypes = [vp, vp, vp, C.POINTER(sst_thresholds), C.POINTER(sst_output), vp]
     L.sst_unpack_cluster_batch.argtypes = [vp, C.c_uint32, vp, vp, C.POINTER(sst_thresholds), vp, vp, C.c_uint32]
     L.sst_unpack_cluster_host.argtypes = [vp, vp, C.c_uint32, vp, C.POINTER(sst_thresholds),
                                           C.POINTER(sst_output), vp]
@@ -162,6 +165,19 @@ def sst_unpack_cluster(ctx, raw, fed_offsets, thresholds, out: sst_output, strea
     rc = load().sst_unpack_cluster(ctx, _ptr(raw), _ptr(fed_offsets), C.byref(thr), C.byref(out),
                                    C.c_void_p(stream))
     _check(ctx, rc, "sst_unpack_cluster")
+
+
+def sst_unpack_cluster_noalloc(ctx, raw, fed_offsets, thresholds, out: sst_output, stream: int = 0):
+    """sst_unpack_cluster for callers that must not allocate device memory while they run (real-time
+    loops with a fixed memory budget, hosts whose own allocator owns the GPU): the kernels' scratch is
+    the library's built-in 32 MiB array, one per GPU and shared by all calls, so calls that could
+    overlap on the GPU must be ordered by the caller.  Raises SSTError (SST_ERR_TOO_LARGE) for a
+    context whose one-event scratch does not fit.  Same arguments and results as sst_unpack_cluster;
+    does not synchronise."""
+    thr = thresholds if isinstance(thresholds, sst_thresholds) else sst_thresholds(*map(float, thresholds))
+    rc = load().sst_unpack_cluster_noalloc(ctx, _ptr(raw), _ptr(fed_offsets), C.byref(thr), C.byref(out),
+                                           C.c_void_p(stream))
+    _check(ctx, rc, "sst_unpack_cluster_noalloc")
 
 
 class Batch:

@@ -2070,6 +2070,124 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
 
 }  // namespace
 
+// ------------------------------------------------------ scratch of sst_unpack_cluster_noalloc
+// The one block of scratch that is not taken from a pool: part of the library's device image, so
+// every GPU that loads the kernels holds these 32 MiB until the process ends.  For callers that may
+// not allocate once they run (include/sst.h).  HOST code must not use this name as a pointer: on the
+// host it only stands for the symbol; noalloc_scratch() below asks the runtime for the device
+// address, once per GPU.
+static __device__ __align__(256) uint8_t sst_noalloc_scratch[SST_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+uint8_t *g_noalloc_ptr[kNoallocMaxDevices] = {};  // device address of sst_noalloc_scratch per GPU ordinal
+
+// Device address of the static scratch on the context's GPU, which the caller has made current.
+// The look-up (cudaGetSymbolAddress) runs on the first call per GPU and is remembered.
+sst_status noalloc_scratch(sst_ctx *ctx, uint8_t **out) {
+    const int dev = ctx->cfg.device;
+    if (dev < 0 || dev >= kNoallocMaxDevices) return SST_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void *ptr = nullptr;
+        SST_CU(cudaGetSymbolAddress(&ptr, sst_noalloc_scratch));
+        if (!ptr) return SST_ERR_CUDA;
+        g_noalloc_ptr[dev] = static_cast<uint8_t *>(ptr);
+    }
+    *out = g_noalloc_ptr[dev];
+    return SST_OK;
+}
+
+// One event on `st` with the static scratch at `blk` laid out as the pool scratch of one event is
+// (scratch_layout(ctx, 1)); the launch itself is what launch_events does for n = 1.  Nothing here
+// allocates.  The array holds what the last call -- of any context -- left: the launch header and
+// the FED words are cleared first, so every call runs as a stream's very first launch (epoch 1).
+sst_status launch_event_noalloc(sst_ctx *ctx, uint8_t *blk, const uint8_t *raw, const uint32_t *fed_offsets,
+                                const sst_thresholds *thr, const sst_output *out, cudaStream_t st) {
+    const ScratchLayout L = scratch_layout(ctx, 1);
+    const uint32_t nf = ctx->cfg.n_feds;
+    const uint32_t sms = static_cast<uint32_t>(ctx->sm_count);
+    const uint32_t wfull = static_cast<uint32_t>(ctx->wpc);
+    uint32_t wpc = std::min(wfull, nf >= 16u * sms ? 8u : nf >= 8u * sms ? 4u : nf >= 4u * sms ? 2u : 1u);
+    uint32_t capacity = static_cast<uint32_t>(ctx->sm_count * ctx->ctas_per_sm) * (wfull / wpc);
+    uint32_t slot_bytes = ctx->slot_bytes;
+    bool pieces = ctx->pieces > 1;
+    if (pieces && ctx->whole_slot && nf <= sms * static_cast<uint32_t>(ctx->whole_warps_sm)) {
+        pieces = false;
+        slot_bytes = ctx->whole_slot;
+        wpc = 1;
+        capacity = sms * static_cast<uint32_t>(ctx->whole_warps_sm);
+    }
+    const uint32_t warp_stride = kWarpHdr + slot_bytes + kTailPad;
+    const uint32_t grid = std::min((nf + wpc - 1) / wpc, capacity);
+    SST_CU(cudaMemsetAsync(blk, 0, L.o_rec, st));  // work counter, warp count, launch count; every FED word
+    KParams kp{};
+    kp.calib = ctx->calib;
+    kp.chan_info = ctx->chan_info;
+    kp.calib_orig = ctx->calib_orig;
+    kp.bad = ctx->bad;
+    kp.geom = ctx->geom;
+    kp.n_geom = ctx->n_geom;
+    kp.fed_present = reinterpret_cast<uint32_t *>(blk + L.o_present);
+    kp.s_csid = reinterpret_cast<uint16_t *>(blk + L.o_csid);
+    kp.s_cadc = blk + L.o_cadc;
+    kp.ticket = reinterpret_cast<unsigned long long *>(blk + L.o_ticket);
+    kp.state_words = nf;
+    kp.trace = reinterpret_cast<unsigned long long *>(blk + L.o_ticket + 256);
+    kp.fed_state = reinterpret_cast<unsigned long long *>(blk + L.o_state);
+    kp.g_rec = reinterpret_cast<uint32_t *>(blk + L.o_rec);
+    kp.g_mask = reinterpret_cast<uint32_t *>(blk + L.o_mask);
+    kp.g_strip = reinterpret_cast<uint16_t *>(blk + L.o_strip);
+    kp.g_adc = blk + L.o_adc;
+    kp.s_rec = reinterpret_cast<uint4 *>(blk + L.o_srec);
+    kp.s_off = reinterpret_cast<uint32_t *>(blk + L.o_soff);
+    kp.s_snr = reinterpret_cast<float *>(blk + L.o_ssnr);
+    kp.s_adc = blk + L.o_sadc;
+    kp.s_seed = reinterpret_cast<uint16_t *>(blk + L.o_sseed);
+    kp.s_cl_stride = static_cast<uint32_t>(L.cl_slots);
+    kp.g_ents = static_cast<uint32_t>(L.ents);
+    kp.g_mwords = static_cast<uint32_t>(L.mwords);
+    kp.tcl2 = static_cast<double>(thr->cluster) * static_cast<double>(thr->cluster);
+    kp.t_ch = thr->channel;
+    kp.t_seed = thr->seed;
+    kp.max_raw_bytes = ctx->cfg.max_raw_bytes;
+    kp.n_feds = nf;
+    kp.n_events = 1;
+    kp.slot_bytes = slot_bytes;
+    kp.ev[0].raw = raw;
+    kp.ev[0].fed_offsets = fed_offsets;
+    kp.ev[0].out = *out;
+    kp.ev[0].packed = nullptr;
+    kp.ev[0].raw_limit = ctx->cfg.max_raw_bytes;
+    const bool extras = out->hit_x || out->compact_strip;
+    const bool fused = !extras && ctx->cfg.move_mode == 0;
+    kp.fused_move = fused ? 1u : 0u;
+    kp.move_chunk = std::min(1024u, ((slot_bytes - (kMoveAdc + 32u) - 32u) / 20u) & ~31u);
+    if (pieces) sst_event_kernel<true, false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
+    else sst_event_kernel<false, false><<<grid, 32 * wpc, wpc * warp_stride, st>>>(kp);
+    cudaError_t err = cudaGetLastError();
+    if (err == cudaSuccess && !fused) {
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3((nf + 3) / 4);
+        lc.blockDim = dim3(128);
+        lc.dynamicSmemBytes = 0;
+        lc.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        lc.attrs = at;
+        lc.numAttrs = 1;
+        if (extras) err = cudaLaunchKernelEx(&lc, sst_emit_kernel<false, true>, kp);
+        else err = cudaLaunchKernelEx(&lc, sst_emit_kernel<false, false>, kp);
+        if (err == cudaSuccess) err = cudaGetLastError();
+    }
+    return cu_ok(ctx, err) ? SST_OK : SST_ERR_CUDA;
+}
+
+}  // namespace
+
 extern "C" {
 
 sst_status sst_create(const sst_config *cfg, sst_ctx **out_ctx) {
@@ -2299,6 +2417,21 @@ sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *
     if (!ctx->has_calib) return SST_ERR_NO_CALIB;
     SST_CU(cudaSetDevice(ctx->cfg.device));
     return launch_events(ctx, 1, &raw, &fed_offsets, thr, &out, static_cast<cudaStream_t>(stream));
+}
+
+// sst_unpack_cluster for callers that may not allocate (include/sst.h): the scratch is the static
+// array above instead of a pool block.  The first call on a GPU also fetches the array's address.
+sst_status sst_unpack_cluster_noalloc(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,
+                                      const sst_thresholds *thr, const sst_output *out, void *stream) {
+    if (!ctx || !raw || !fed_offsets || !thr || !output_ok(out) || !thresholds_ok(thr))
+        return SST_ERR_INVALID_ARG;
+    if (!ctx->has_calib) return SST_ERR_NO_CALIB;
+    if (scratch_layout(ctx, 1).total > static_cast<size_t>(SST_NOALLOC_SCRATCH_BYTES)) return SST_ERR_TOO_LARGE;
+    SST_CU(cudaSetDevice(ctx->cfg.device));
+    uint8_t *blk = nullptr;
+    const sst_status s = noalloc_scratch(ctx, &blk);
+    if (s != SST_OK) return s;
+    return launch_event_noalloc(ctx, blk, raw, fed_offsets, thr, out, static_cast<cudaStream_t>(stream));
 }
 
 sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
@@ -2796,6 +2929,7 @@ const char *sst_status_string(sst_status s) {
         case SST_ERR_CUDA: return "SST_ERR_CUDA";
         case SST_ERR_NO_CALIB: return "SST_ERR_NO_CALIB";
         case SST_ERR_BAD_CALIB: return "SST_ERR_BAD_CALIB";
+        case SST_ERR_TOO_LARGE: return "SST_ERR_TOO_LARGE";
     }
     return "SST_ERR_UNKNOWN";
 }

@@ -135,6 +135,11 @@ class Detector:
         st = self.torch.cuda.current_stream(self.device) if stream is None else stream
         B.sst_unpack_cluster(self.ctx, d_raw, d_fo, thresholds, outputs.out, st.cuda_stream)
 
+    def run_noalloc(self, d_raw, d_fo, thresholds: Sequence[float], outputs: EventOutputs, stream=None):
+        """The same event through sst_unpack_cluster_noalloc (scratch in the library's static array)."""
+        st = self.torch.cuda.current_stream(self.device) if stream is None else stream
+        B.sst_unpack_cluster_noalloc(self.ctx, d_raw, d_fo, thresholds, outputs.out, st.cuda_stream)
+
 
 _FIELDS = (("strip_adc", np.uint8, "N"), ("chan_off", np.uint32, "C"), ("chan_len", np.uint16, "C"),
            ("seed_idx", np.uint32, "S"), ("cl_module", np.uint32, "K"), ("cl_first", np.uint16, "K"),
