@@ -25,6 +25,13 @@
  *     pool), sst_unpack_cluster / sst_unpack_cluster_batch on that stream can be captured
  *     (cudaStreamBeginCapture) and the graph replayed: a launch is nothing but its parameters, the
  *     kernel keeps its work counter and the epoch of its FED words in device memory itself.
+ *     The limits, because the graph holds the address of that stream's scratch: the plain call before
+ *     the capture must have had at least as many events as the captured one (a capture that would
+ *     have to allocate returns SST_ERR_INVALID_ARG and records nothing); after a capture the stream's
+ *     scratch is never reallocated, so a later call on that stream with more events than it holds is
+ *     refused with SST_ERR_INVALID_ARG; replay the graph on the captured stream only (or ordered
+ *     with that stream's other work), one replay in flight at a time -- the replays share one work
+ *     counter -- and never after sst_destroy.
  */
 #ifndef SST_H
 #define SST_H
@@ -74,8 +81,9 @@ typedef struct {
     uint32_t trace;                /* 1 = launch the traced instantiations of sst_event_kernel: lane 0 of
                                       every warp adds the cycles of each phase of each FED and the
                                       launch's timeline to 32 words per stream (sst_trace_read); same
-                                      results, ~1 % slower.  0 = no tracing code in the kernel at all  */
-} sst_config;
+                                      results, ~7 % slower.  0 = no tracing code in the kernel at all  */
+} sst_config; /* zero-initialise it: move_mode and trace must be 0 or 1, else sst_create returns
+                 SST_ERR_INVALID_ARG */
 
 /* S/N thresholds of the "three thresholds" algorithm: a strip is active at
  * adc/noise >= channel, a seed at adc/noise >= seed (both decided in exact arithmetic), a
@@ -182,8 +190,10 @@ sst_status sst_upload_geometry(sst_ctx *ctx, const float *geom, uint32_t n_modul
  * fed_offsets: DEVICE [n_feds+1] byte offsets of the FEDs in raw (16-byte multiples for the
  * fast path; the offsets must not step back: a FED with start > end, end > cfg.max_raw_bytes or a
  * start below any earlier entry of fed_offsets is flagged and empty).  thr and
- * out are HOST structs read before the call returns.  The work is enqueued on `stream` as two
- * kernel launches (unpack + cluster per FED, then the ordered move of the clusters); the call
+ * out are HOST structs read before the call returns.  The work is enqueued on `stream` as ONE
+ * kernel launch (sst_event_kernel: unpack + cluster per FED, then the ordered move of the clusters
+ * by the warps that run out of FEDs) when cfg.move_mode is 0 and `out` asks for neither the compact
+ * SoA nor hit coordinates, else as two (sst_emit_kernel does the move behind it); the call
  * does not synchronise.  Scratch comes from the context's
  * stream-ordered pool: one block per stream, allocated on the stream's first event and reused
  * (so a stream must not be driven by two host threads at once). */
@@ -196,8 +206,9 @@ sst_status sst_unpack_cluster(sst_ctx *ctx, const uint8_t *raw, const uint32_t *
  * they share the calibration in L2): a launch runs on the first stream of its group after that
  * stream has waited (by CUDA event) for whatever the group's other streams had enqueued, and
  * those streams wait for the launch in turn -- so every event's inputs are honoured and its
- * result is complete in stream order on its own stream.  Every event's result is exactly what
- * sst_unpack_cluster gives.  raw, fed_offsets, outs and streams are HOST arrays read before the
+ * result is complete in stream order on its own stream.  The streams thus only ORDER the events'
+ * inputs and results; they add no concurrency: all events of a group run in one launch on one
+ * stream.  Every event's result is exactly what sst_unpack_cluster gives.  raw, fed_offsets, outs and streams are HOST arrays read before the
  * call returns.  Does not synchronise. */
 sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8_t *const *raw,
                                     const uint32_t *const *fed_offsets, const sst_thresholds *thr,

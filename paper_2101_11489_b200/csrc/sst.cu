@@ -1439,7 +1439,10 @@ __device__ __forceinline__ void move_fed(const KParams &p, unsigned long long *m
         if (m) adc_sh = static_cast<uint32_t>(ab + a0 - a_lo);
         __syncwarp();  // every lane is done with what the slot held
         if (lane == 0) {
-            fence_proxy_async();  // earlier generic-proxy accesses to the slot before the async writes
+            // earlier generic-proxy accesses to the slot before the async writes; and, on the reader's
+            // side too, the staging in global memory (seen through the acquire of the state words)
+            // before the async reads
+            asm volatile("fence.proxy.async;" ::: "memory");
             const uint32_t bytes = n * 16u + (n ? static_cast<uint32_t>(o_hi - o_lo) * 4u : 0u) + (m ? static_cast<uint32_t>(a_hi - a_lo) : 0u);
             mbar_expect_tx(mbar, bytes);
             if (n) {
@@ -1599,15 +1602,23 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta, kMinCtas) sst_event_kernel(
     if (kTrace && lane == 0) atomicMax(p.trace + kTrEnd, wall_ns());
     // The last warp of the launch to get here leaves the stream's header ready for the next launch:
     // ticket counter and warp count at zero, one launch more -- and when the epoch starts over with
-    // that, every FED state word cleared, so that a word of this round of epochs is never taken for
-    // one of the next.  (The launch's parameters hold nothing that changes from launch to launch.)
+    // that, the TAG of every FED state word cleared (tag 0 is no launch's epoch), so that a word of
+    // this round of epochs is never taken for one of the next.  The counts stay: sst_emit_kernel,
+    // when it runs behind this launch, still reads them (it ignores the tags).  (The launch's
+    // parameters hold nothing that changes from launch to launch.)
+    // The fences order this warp's earlier writes before its count, and the header writes below
+    // after the counts of all the others.
     uint32_t left = 0;
-    if (lane == 0) left = static_cast<uint32_t>(atomicAdd(p.ticket + 1, 1ull)) + 1u == gridDim.x * (blockDim.x >> 5);
+    if (lane == 0) {
+        __threadfence();
+        left = static_cast<uint32_t>(atomicAdd(p.ticket + 1, 1ull)) + 1u == gridDim.x * (blockDim.x >> 5);
+        __threadfence();
+    }
     if (__shfl_sync(kFull, left, 0)) {
         const unsigned long long n = p.ticket[2] + 1ull == kEpochs ? 0ull : p.ticket[2] + 1ull;
         if (n == 0) {
 #pragma unroll 1
-            for (uint32_t i = lane; i < p.state_words; i += 32) p.fed_state[i] = 0ull;
+            for (uint32_t i = lane; i < p.state_words; i += 32) p.fed_state[i] &= (1ull << kShEpoch) - 1ull;
         }
         __syncwarp();
         if (lane == 0) {
@@ -1837,7 +1848,9 @@ struct sst_ctx {
     // per-stream scratch (launch header, FED states, slow-path lists), taken from the pool on a
     // stream's first launch and kept: stream order makes reuse safe, and every launch leaves the
     // header ready for the next
-    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t cap_events; };
+    // `captured`: a stream capture has recorded launches that point into `mem`; the block is then
+    // never reallocated (a replay of that graph would use freed memory)
+    struct Slot { cudaStream_t stream; uint8_t *mem; uint32_t cap_events; bool captured; };
     // cross-stream dependencies of the batched entry point: one event per stream, made on first use
     struct StreamEvent { cudaStream_t stream; cudaEvent_t ev; };
     std::vector<StreamEvent> stream_events;
@@ -1966,10 +1979,16 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
     for (auto &s : ctx->slots)
         if (s.stream == st) sl = &s;
     if (!sl) {
-        ctx->slots.push_back({st, nullptr, 0u});
+        ctx->slots.push_back({st, nullptr, 0u, false});
         sl = &ctx->slots.back();
     }
+    cudaStreamCaptureStatus capture = cudaStreamCaptureStatusNone;
+    SST_CU(cudaStreamIsCapturing(st, &capture));
+    const bool capturing = capture != cudaStreamCaptureStatusNone;
     if (sl->cap_events < n) {  // (re)allocate the stream's scratch for 1, 8, 16, 32 or kMaxEv events
+        // not inside a capture (the allocation would become part of the graph) and not once a graph
+        // holds the block's address: the stream must have seen a plain call at least this large before
+        if (capturing || sl->captured) return SST_ERR_INVALID_ARG;
         if (sl->mem) SST_CU(cudaFreeAsync(sl->mem, st));
         sl->mem = nullptr;
         sl->cap_events = 0;
@@ -1985,6 +2004,7 @@ sst_status launch_events(sst_ctx *ctx, uint32_t n, const uint8_t *const *raw, co
         sl->mem = mem;
         sl->cap_events = want;
     }
+    if (capturing) sl->captured = true;
     uint8_t *const blk = sl->mem;
     const ScratchLayout L = scratch_layout(ctx, sl->cap_events);
     KParams kp{};

@@ -1002,37 +1002,85 @@ def test_launch_captured_in_a_cuda_graph_and_replayed(H, oracle):
         for e, o in zip(evs[3:], outs):
             r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
             compare(H.unsigned_view(o.numpy()), r)
+        # The graph holds the address of the stream's scratch (sized for up to 8 events by the plain
+        # call): a later call on that stream that would need a larger block is refused instead of
+        # freeing what the graph points into, and the graph still replays
+        big = B.Batch([d_in[i % 3][0] for i in range(9)], [d_in[i % 3][1] for i in range(9)], (2, 3, 5),
+                      [outs[i % 3].out for i in range(9)], [st.cuda_stream])
+        with pytest.raises(B.SSTError, match="SST_ERR_INVALID_ARG"):
+            B.sst_unpack_cluster_batch(det.ctx, big)
+        g.replay()
+        torch.cuda.synchronize()
+        for e, o in zip(evs[3:], outs):
+            r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+            compare(H.unsigned_view(o.numpy()), r)
+        # a capture on a stream that has not seen a plain call would have to allocate: refused too
+        st2 = torch.cuda.Stream()
+        unprimed = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs], [st2.cuda_stream])
+        torch.cuda.synchronize()
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2, stream=st2):
+            with pytest.raises(B.SSTError, match="SST_ERR_INVALID_ARG"):
+                B.sst_unpack_cluster_batch(det.ctx, unprimed)
+            outs[0].tensors["n_clusters"].add_(0)   # (something to record: an empty capture only earns a warning)
+        torch.cuda.synchronize()
     finally:
         det.close()
 
 
-def test_epoch_wraps_after_4095_launches_on_a_stream(H, oracle):
+@pytest.mark.parametrize("wrap_extras", [False, True], ids=["plain-at-wrap", "emit-kernel-at-wrap"])
+def test_epoch_wraps_after_4095_launches_on_a_stream(H, oracle, wrap_extras):
     """The FED state words carry a 12-bit launch epoch (what the in-kernel move waits for); it wraps
-    after 4095 launches of a stream, before which the words are cleared.  4096 launches of small
-    events on one stream, the first and the last a two-event batch (with the events swapped), so
-    that the last launch meets words of its own epoch left by the first unless they were cleared."""
+    after 4095 launches of a stream, and the launch that wraps it clears the words' tags.  4096
+    launches of small events on one stream, the first and the last a two-event batch (with the events
+    swapped), so that the last launch meets words of its own epoch left by the first unless the tags
+    were cleared.  The result of launch 4095 -- the one that clears -- is checked on its own: when
+    sst_emit_kernel runs behind it (move_mode 1, or the compact SoA and hits wanted), that kernel
+    still needs the counts in those words."""
     import torch
     from paper_2101_11489_b200 import binding as B
     nf = 3
     cfg, cal, evs = synth.make_config(0, n_feds=nf, event_seeds=[1, 2])
     mrb = (max(int(e.raw.size) for e in evs) + 4095) // 4096 * 4096
+    geom = synth.make_geometry(cal.chan_module)
     det = H.Detector(nf, cal.gain, cal.noise, cal.bad, cal.chan_module, max_raw_bytes=mrb)
     try:
+        det.upload_geometry(geom)
         st = torch.cuda.Stream()
         d_in = [det.upload_raw(e.raw, e.fed_offsets) for e in evs]
-        outs = [det.alloc_outputs(mrb // 2 + 1, mrb, seeds=True, chan_map=True, snr=True, cap_seeds=mrb) for _ in evs]
+        kw = dict(seeds=True, chan_map=True, snr=True, cap_seeds=mrb)
+        outs = [det.alloc_outputs(mrb // 2 + 1, mrb, **kw) for _ in evs]
+        at_wrap = det.alloc_outputs(mrb // 2 + 1, mrb, compact=wrap_extras, hits=wrap_extras, **kw)
+        want = [oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5)) for e in evs]
         both_ev = B.Batch([d[0] for d in d_in], [d[1] for d in d_in], (2, 3, 5), [o.out for o in outs], [st.cuda_stream])
         swapped = B.Batch([d[0] for d in d_in[::-1]], [d[1] for d in d_in[::-1]], (2, 3, 5), [o.out for o in outs[::-1]], [st.cuda_stream])
         # launch 1 (epoch 1) leaves the other event's words at index 1; launches 2..4095 touch index 0
-        # only; launch 4096 is the first of the next round of epochs, again with epoch 1
+        # only; launch 4095 has the last epoch of the round and clears the tags; launch 4096 is the
+        # first of the next round, again with epoch 1
         B.sst_unpack_cluster_batch(det.ctx, swapped)
-        for i in range(4094):
+        for i in range(4093):
             det.run(d_in[i & 1][0], d_in[i & 1][1], (2, 3, 5), outs[i & 1], stream=st)
-        B.sst_unpack_cluster_batch(det.ctx, both_ev)
+        det.run(d_in[1][0], d_in[1][1], (2, 3, 5), at_wrap, stream=st)      # launch 4095
         torch.cuda.synchronize()
-        for e, o in zip(evs, outs):
-            r = oracle.run(e.raw, e.fed_offsets, nf, cal.gain, cal.noise, cal.bad, cal.chan_module, (2, 3, 5))
+        g = H.unsigned_view(at_wrap.numpy())
+        compare(g, want[1])
+        assert g["n_clusters"] > 0
+        if wrap_extras:
+            compare_next(g, want[1], oracle, cal, geom)
+        for o in outs:
+            o.tensors["n_clusters"].zero_()
+        B.sst_unpack_cluster_batch(det.ctx, both_ev)                        # launch 4096
+        torch.cuda.synchronize()
+        for r, o in zip(want, outs):
             compare(H.unsigned_view(o.numpy()), r)
+        # and the launches after the wrap go on as before (epoch 2, 3)
+        for i in range(2):
+            det.run(d_in[i][0], d_in[i][1], (2, 3, 5), at_wrap, stream=st)
+            torch.cuda.synchronize()
+            g = H.unsigned_view(at_wrap.numpy())
+            compare(g, want[i])
+            if wrap_extras:
+                compare_next(g, want[i], oracle, cal, geom)
     finally:
         det.close()
 
