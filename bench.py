@@ -47,6 +47,7 @@ N_STREAMS = 8
 THRESHOLDS = (2.0, 3.0, 5.0)
 METRIC = "events/s unpack+cluster (full-detector events, 440 FEDs x 96 x 256 strips)"
 FALLBACK_HBM_GBS = 6650.0   # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+SPEC_HBM_GBS = 8000.0       # the 8 TB/s BASELINE.md section 2 reads the north_star's 50 % target against (frac_spec)
 
 
 # --------------------------------------------------------------------------- workload
@@ -193,29 +194,56 @@ def compare_with_oracle(g, r, what, dense=True):
     same("dev_status", np.asarray(g["status"]).view(np.uint32)[:5], r.status[:5])
 
 
-def time_oracle_omp(events, calib, thresholds, budget_s: float):
-    """OpenMP build of the oracle in the paper's N x M shapes (Table 1): N events in
-    flight x M threads per event, over the divisors of the core count.  Returns (table, cores)."""
+OMP_ENV = {"OMP_PROC_BIND": "spread,close", "OMP_PLACES": "cores"}
+
+
+def omp_leg(args):
+    """--omp-leg (a child of time_oracle_omp): the OpenMP build of the oracle in the paper's N x M
+    shapes (Table 1) -- N events in flight x M threads per event, over the divisors of
+    the core count -- on the first `--events` events of the workload.  Prints {"table", "cores"}."""
     from oracle import sst_oracle as O
     O.build()
+    cfg = synth.CONFIGS[args.config]
+    thr = cfg.thresholds[0]
+    calib = synth.make_calibration(args.n_feds, cfg.bad_frac)
+    events = generate_events(args.config, args.n_feds, list(range(1, args.events + 1)), calib)
     cores = os.cpu_count() or 1
     shapes = sorted({(cores // m, m) for m in (1, 2, 4, 8, 16, 32) if m <= cores and cores % m == 0})
     raws = [e[0] for e in events]
     fos = [e[1] for e in events]
     table = []
-    per = max(budget_s / len(shapes), 1.0)
+    per = max(args.cpu_budget / len(shapes), 1.0)
     for n_outer, n_inner in shapes:
+        run = lambda: O.events_omp(raws, fos, calib.n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module,
+                                   thr, n_outer, n_inner)
+        run()   # untimed: the threads of this shape exist and hold their work arrays
         t0 = time.perf_counter()
         done = 0
         while True:
-            O.events_omp(raws, fos, calib.n_feds, calib.gain, calib.noise, calib.bad, calib.chan_module,
-                         thresholds, n_outer, n_inner)
+            run()
             done += len(raws)
             dt = time.perf_counter() - t0
             if dt >= per:
                 break
         table.append({"N": n_outer, "M": n_inner, "events_per_s": done / dt})
-    return table, cores
+    print(json.dumps({"table": table, "cores": cores}))
+
+
+def time_oracle_omp(cfg_id: int, n_feds: int, n_events: int, budget_s: float):
+    """The OpenMP leg of the CPU baseline, in a process of its own so that the thread binding
+    BASELINE.md section 3.2 asks for (OMP_PROC_BIND / OMP_PLACES; `spread,close` is its nested form: the N
+    event threads spread over the cores, the M threads of an event close to theirs) is in the
+    environment before the OpenMP runtime starts and binds nothing of this process.  The child
+    regenerates the same seeded events (seeds 1..n_events).  Returns (table, cores, env)."""
+    env = dict(os.environ)
+    env.update(OMP_ENV)
+    cmd = [sys.executable, os.path.abspath(__file__), "--omp-leg", "--config", str(cfg_id), "--n-feds", str(n_feds),
+           "--events", str(n_events), "--cpu-budget", str(budget_s)]
+    out = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=600)
+    if out.returncode != 0:
+        raise RuntimeError("OpenMP oracle leg failed: " + out.stderr[-2000:])
+    doc = json.loads(out.stdout.strip().splitlines()[-1])
+    return doc["table"], doc["cores"], dict(OMP_ENV)
 
 
 CONFIG_NOTES = {1: "generator of config 1 (2% occupancy, seeds 1..N)", 2: "generator of config 2 (6% occupancy, "
@@ -238,7 +266,7 @@ def run_reference(args):
     if rank != 0:
         return
     n_feds = args.n_feds
-    per_step = args.ref_events
+    per_step = min(args.ref_events, args.events)
     cfg = synth.CONFIGS[args.config]
     thr = cfg.thresholds[0]
     calib = synth.make_calibration(n_feds, cfg.bad_frac)
@@ -257,12 +285,13 @@ def run_reference(args):
         step()
     dt = time.perf_counter() - t0
     value = per_step * args.steps / dt
-    sample = f"{per_step} events of the workload per step (seeds 1..{per_step}), sequential oracle, 1 thread"
+    sample = (f"each step = the first {per_step} of the workload's {args.events} events (seeds 1..{per_step}), "
+              "sequential oracle, 1 thread")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8/f32/f64", "data": "synthetic",
-        "config": workload_config(args.config, n_feds, per_step, thr),
+        "config": workload_config(args.config, n_feds, args.events, thr),
         "cpu_baseline": {"value": value, "unit": "events/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -270,14 +299,25 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------- GPU arm
+def git_blob_sha1(path: str) -> str:
+    """What `git hash-object` prints for the file."""
+    import hashlib
+    data = open(path, "rb").read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
 def ncu_traffic(cfg_id: int):
     """Measured DRAM bytes per step (read + write of every kernel of a step) from the committed ncu
-    launch list summary profiles/traffic.csv (rows: workload, kernel, read bytes, write bytes), or None."""
+    launch list summary profiles/traffic.csv (rows: workload, kernel, read bytes, write bytes), or None;
+    and whether the capture is STALE: the file names the git blob of the sst.cu it was taken from
+    (a `# sst.cu blob: <sha1>` line), which is compared with the source this run was built from."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(p):
-        return None
-    tot, found = 0.0, False
+        return None, None
+    tot, found, blob = 0.0, False, None
     for line in open(p):
+        if line.startswith("# sst.cu blob:"):
+            blob = line.split(":", 1)[1].strip()
         f = [x.strip() for x in line.split(",")]
         if len(f) >= 4 and f[0] == f"config{cfg_id}":
             try:
@@ -285,7 +325,8 @@ def ncu_traffic(cfg_id: int):
                 found = True
             except ValueError:
                 pass
-    return tot if found else None
+    stale = blob != git_blob_sha1(os.path.join(ROOT, "paper_2101_11489_b200", "csrc", "sst.cu"))
+    return (tot if found else None), stale
 
 
 MOVE_MODE = 0  # sst_config.move_mode of the detectors the bench makes (--move-mode)
@@ -383,8 +424,8 @@ def run_sweep(args):
         r = rate(N_EVENTS, ns)
         out["streams"].append({"events": N_EVENTS, "streams": ns, "events_per_s": r})
     det.close()
-    table, cores = time_oracle_omp(events[:16], calib, thr, 24.0)
-    out["omp_oracle"] = {"cores": cores, "events_per_pass": 16, "table": table}
+    table, cores, omp_env = time_oracle_omp(3, n_feds, 16, 24.0)
+    out["omp_oracle"] = {"cores": cores, "events_per_pass": 16, "table": table, "env": omp_env}
     print(json.dumps({"sweep": out}))
 
 
@@ -459,6 +500,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle timing (rank 0, N=1)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (and with it the verification)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--omp-leg", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--trace", action="store_true",
                     help="instead of the bench line: per-phase time of a FED and the timeline of a launch of 1, 8 and 64 "
                          "events, from a context with sst_config.trace = 1")
@@ -476,6 +518,8 @@ def main():
         return run_sweep(args)
     if args.trace:
         return run_trace(args)
+    if args.omp_leg:
+        return omp_leg(args)
     world_env = os.environ.get("WORLD_SIZE")
     if world_env is None and args.gpus > 1:
         return respawn_under_torchrun(args)
@@ -602,7 +646,7 @@ def main():
     kernels_per_launch = int(info.get("kernels_per_event", 1))
     dur_us = 1e3 * ms_total / launches
     achieved = (b_alg_step / launches_step) / (dur_us * 1e-6) / 1e9
-    traffic = ncu_traffic(args.config)
+    traffic, traffic_stale = ncu_traffic(args.config)
 
     # ---- two batches in flight: consecutive steps alternate between two halves of the stream set (and
     # two sets of output blocks), so the ordered move of one step overlaps the event kernel of the next
@@ -782,17 +826,19 @@ def main():
         cpu = {"value": rate, "unit": "events/s", "cores": 1, "kind": "oracle",
                "sample": f"{n_done} events of the workload (seeds 1..{min(n_done, n_events)}), {dt:.1f} s of oracle time, "
                          "oracle/sst_oracle.c -O2 sequential"}
-        table, cores = time_oracle_omp(events[:16], calib, thr, max(args.cpu_budget / 2, 4.0))
+        table, cores, omp_env = time_oracle_omp(args.config, n_feds, min(16, n_events), max(args.cpu_budget / 2, 4.0))
         best = max(table, key=lambda t: t["events_per_s"])
         cpu_omp = {"value": best["events_per_s"], "unit": "events/s", "cores": cores, "kind": "oracle (OpenMP build)",
-                   "shape_NxM": f"{best['N']}x{best['M']}", "table": table,
-                   "sample": "16 events of the workload per pass, N events in flight x M threads per event"}
+                   "shape_NxM": f"{best['N']}x{best['M']}", "table": table, "env": omp_env,
+                   "sample": f"{min(16, n_events)} events of the workload per pass (seeds 1..{min(16, n_events)}), N events in "
+                             "flight x M threads per event, in a child process with that environment; one untimed pass per shape"}
 
     if rank == 0:
         dram = None
         if traffic is not None:
             dram_gbs = traffic / (ms_step * 1e-3) / 1e9
-            dram = {"bytes_per_step": traffic, "achieved": dram_gbs, "frac": dram_gbs / peak,
+            dram = {"bytes_per_step": traffic, "achieved": dram_gbs, "frac": dram_gbs / peak, "frac_spec": dram_gbs / SPEC_HBM_GBS,
+                    "traffic_stale": traffic_stale,
                     "source": "profiles/traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum of the kernels of a step, "
                               "one step) over this run's step time"}
         line = {
@@ -805,7 +851,8 @@ def main():
             "clusters_per_s": value * clusters_step / n_events,
             "host_wall_ms_per_step": 1e3 * t_host / args.steps,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "peak_source": peak_src,
+                         "frac_spec": achieved / SPEC_HBM_GBS, "spec_peak": SPEC_HBM_GBS,
+                         "traffic": traffic, "traffic_stale": traffic_stale, "peak_source": peak_src,
                          "kernel": "sst_event_kernel", "algorithmic_bytes_per_launch": b_alg_step / launches_step,
                          "events_per_launch": n_events / launches_step,
                          "launch_us": dur_us,

@@ -30,6 +30,23 @@ void sst_oracle_cluster(const uint8_t *adc, const float *gain, const float *nois
 
 #define FED_STRIPS (96u * 256u)
 
+/* Work arrays of one FED range (chan_off, chan_len, adc, active, seed): kept per THREAD from call to
+ * call and only ever grown, so the timed loop does not pay malloc/free and page faults of ~3 bytes
+ * per strip slot per range per event.  Still allocated and first touched by the thread that uses
+ * them, inside the parallel region. */
+static __thread uint8_t *tl_buf = NULL;
+static __thread uint64_t tl_cap = 0;
+static uint8_t *thread_work(uint64_t bytes)
+{
+    if (bytes > tl_cap) {
+        free(tl_buf);
+        tl_buf = (uint8_t *)malloc(bytes);
+        tl_cap = tl_buf ? bytes : 0;
+        if (tl_buf) memset(tl_buf, 0, bytes);
+    }
+    return tl_buf;
+}
+
 typedef struct {
     uint32_t n_cl, n_adc, n_seeds;
     uint32_t *cl_module;
@@ -71,10 +88,16 @@ int sst_oracle_events_omp(uint32_t n_events, const uint8_t *const *raws, const u
             const uint32_t nf = f1 - f0;
             const uint64_t n = (uint64_t)nf * FED_STRIPS, g0 = (uint64_t)f0 * FED_STRIPS;
             uint32_t status[8] = {0};
-            uint32_t *chan_off = (uint32_t *)malloc(nf * 96 * sizeof(uint32_t));
-            uint16_t *chan_len = (uint16_t *)malloc(nf * 96 * sizeof(uint16_t));
-            uint8_t *adc = (uint8_t *)malloc(n), *active = (uint8_t *)malloc(n),
-                    *seed = (uint8_t *)malloc(n);
+            const uint64_t n_al = (n + 63) & ~(uint64_t)63;
+            uint8_t *work = thread_work(3 * n_al + (uint64_t)nf * 96 * 6 + 64);
+            if (!work) {
+#pragma omp atomic write
+                failed = 1;
+                continue;
+            }
+            uint8_t *adc = work, *active = work + n_al, *seed = work + 2 * n_al;
+            uint32_t *chan_off = (uint32_t *)(work + 3 * n_al);
+            uint16_t *chan_len = (uint16_t *)(work + 3 * n_al + (uint64_t)nf * 96 * 4);
             sst_oracle_unpack(raws[e], raw_bytes[e], fed_offsets[e] + f0, nf, chan_off, chan_len,
                               adc, status);
             part_t *p = &parts[m];
@@ -94,7 +117,6 @@ int sst_oracle_events_omp(uint32_t n_events, const uint8_t *const *raws, const u
                                t_cl, cap, cap, &p->n_cl, p->cl_module, p->cl_first, p->cl_width,
                                p->cl_charge, p->cl_bary, p->cl_adc_off, p->cl_adc, NULL, status);
             p->n_adc = status[3];
-            free(chan_off); free(chan_len); free(adc); free(active); free(seed);
         }
         /* concatenate in FED order */
         uint64_t h = 14695981039346656037ull;
