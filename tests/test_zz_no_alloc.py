@@ -128,6 +128,31 @@ def test_noalloc_with_the_second_kernel_and_a_full_detector_event():
         full.close()
 
 
+def test_noalloc_on_its_own_stream_beside_pooled_calls_on_another():
+    """sst.h: the other entry points use pool scratch and may run beside the no-allocation call.  A
+    batch of the pooled path on one stream and no-allocation calls on a second stream, enqueued
+    alternately without synchronising, several rounds."""
+    from paper_2101_11489_b200 import binding as B, harness
+    import torch
+    a = _Case(harness, 1, 37, [21, 22, 23], 0)
+    try:
+        s_pool, s_static = torch.cuda.Stream(), torch.cuda.Stream()
+        pooled = [a.outputs() for _ in range(3)]
+        static = [a.outputs() for _ in range(3)]
+        batch = B.Batch([d[0] for d in a.inputs], [d[1] for d in a.inputs], a.thr, [o.out for o in pooled], [s_pool.cuda_stream])
+        torch.cuda.synchronize()
+        for _ in range(5):
+            B.sst_unpack_cluster_batch(a.det.ctx, batch)
+            for i in range(3):
+                a.det.run_noalloc(*a.inputs[i], a.thr, static[i], stream=s_static)
+        torch.cuda.synchronize()
+        for i in range(3):
+            same(harness.unsigned_view(pooled[i].numpy()), a.want[i])
+            same(harness.unsigned_view(static[i].numpy()), a.want[i])
+    finally:
+        a.close()
+
+
 def test_noalloc_refuses_a_context_beyond_the_limit():
     from paper_2101_11489_b200 import binding as B, harness
     import torch
