@@ -243,7 +243,8 @@ sst_status sst_unpack_cluster_batch(sst_ctx *ctx, uint32_t n_events, const uint8
  *     wrong results: keep all calls of a GPU on one stream, or order them with events.  The other
  *     entry points use pool scratch and may run beside it.
  *   - The FIRST call on each GPU looks up the array's device address (cudaGetSymbolAddress, with that
- *     GPU current) and keeps it; make that first call during set-up, before any stream capture begins.
+ *     GPU current), keeps it, and has the runtime load the kernels the entry point can launch; make
+ *     that first call during set-up, before any stream capture begins.
  *   - A context created with trace = 1 is accepted but this call is never traced. */
 #define SST_NOALLOC_SCRATCH_BYTES (32u << 20)
 sst_status sst_unpack_cluster_noalloc(sst_ctx *ctx, const uint8_t *raw, const uint32_t *fed_offsets,

@@ -2114,6 +2114,14 @@ sst_status noalloc_scratch(sst_ctx *ctx, uint8_t **out) {
         void *ptr = nullptr;
         SST_CU(cudaGetSymbolAddress(&ptr, sst_noalloc_scratch));
         if (!ptr) return SST_ERR_CUDA;
+        // also part of the set-up: have the runtime load the four kernels this entry point can launch
+        // now, so that no later call is the first use of one (loading a kernel is the runtime's
+        // business, but it is work a caller on a fixed budget wants behind it)
+        cudaFuncAttributes fa;
+        SST_CU(cudaFuncGetAttributes(&fa, sst_event_kernel<false, false>));
+        SST_CU(cudaFuncGetAttributes(&fa, sst_event_kernel<true, false>));
+        SST_CU(cudaFuncGetAttributes(&fa, sst_emit_kernel<false, false>));
+        SST_CU(cudaFuncGetAttributes(&fa, sst_emit_kernel<false, true>));
         g_noalloc_ptr[dev] = static_cast<uint8_t *>(ptr);
     }
     *out = g_noalloc_ptr[dev];
