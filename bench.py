@@ -858,8 +858,8 @@ def main():
                          "launch_us": dur_us,
                          "dram": dram,
                          "limiter": "not HBM: a warp works through its FED as one long chain of dependent steps, eight "
-                                    "warps per scheduler hide ~70 % of it (issue slots 70 % busy, DRAM ~30 %; "
-                                    "profiles/r02_final.md); the calibration term of the algorithmic bytes is served by L2",
+                                    "warps per scheduler hide ~67 % of it (issue slots 67 % busy, DRAM 31 %, 11.9 cycles per issued "
+                                    "instruction; profiles/r03_final.md); the calibration term of the algorithmic bytes is served by L2",
                          "how": "achieved = algorithmic bytes per launch / launch duration, B_alg = raw + N dense + 32 B x "
                                 "noise sectors of present strips + 32 B x gain sectors of accepted-cluster strips + 20 B x "
                                 "clusters + cluster ADC bytes; launch duration = CUDA-event span of the timed region / "
